@@ -1,0 +1,203 @@
+/* ami.h -- C ABI of the B200-native batched AMI evaluation path.
+ *
+ * What this library computes is defined by arXiv 2311.17189 (TorchAmi); citations are line
+ * numbers of /root/reference/PAPER.md, "P<n>" are the readings listed in DESIGN.md.
+ *
+ *   ami_construct   host, one-time: labelled diagram R0 -> symbolic result of
+ *                   the n nested Matsubara sums, Eqs. 1-5, stored as a flat term
+ *                   table (unfactorised form of PAPER.md:100, Eq. 6) plus evaluation plans, with a
+ *                   device-resident copy.
+ *   ami_dispersion  kernel: internal momenta -> line energies, Eqs. 8-18, 2D
+ *                   tight-binding dispersion.
+ *   ami_evaluate    kernel: the table evaluated for a batch of energies x external frequencies x
+ *                   inverse temperatures, complex128.
+ *   ami_run         streamed driver: (generate or copy momenta) -> dispersion -> evaluate, chunked
+ *                   and double-buffered over CUDA streams ("repeatedly call this
+ *                   function for different energy batches", :291).
+ *
+ * Conventions
+ *   - Every function returns int: 0 = AMI_OK, negative = error (see enum).  Nothing throws or
+ *     aborts across this boundary.  ami_strerror() names a code, ami_last_cuda_error() gives the
+ *     CUDA runtime's message for the last AMI_ECUDA on this thread.
+ *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. a torch tensor's
+ *     data_ptr()); h_* and unprefixed array arguments are HOST pointers, read during the call
+ *     only.  The library owns only ami_table objects.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Kernel
+ *     entry points are asynchronous on it; host arrays they take are copied before returning.
+ *   - complex128 = two doubles (re, im), interleaved.
+ *   - The supplied energies are the NEGATIVE of the dispersion, e_i = -eps(k_i) (PAPER.md:84,
+ *     :219); external frequencies come LAST in every alpha row.
+ *   - There is no CPU fallback: a table built with device = -1 can be inspected and exported but
+ *     every kernel entry point returns AMI_ECUDA for it.
+ */
+#ifndef AMI_B200_H
+#define AMI_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  AMI_OK = 0,
+  AMI_EINVAL = -1,             /* bad argument (null pointer, negative size, bad enum, ...) */
+  AMI_EUNSUPPORTED_ALPHA = -2, /* |alpha_p| != 1 met at a summation (Eq. 4 is for +-1; P8) */
+  AMI_ENOPOLE = -3,            /* a term with no line depending on nu_p (P9) */
+  AMI_ECUDA = -4,              /* CUDA runtime error, or table has no device copy */
+  AMI_ENOMEM = -5,             /* host or device allocation failed */
+  AMI_EUNSUPPORTED = -6        /* valid request outside the built limits (see ami_limits) */
+};
+
+/* Built limits (compile-time constants of the kernels). */
+enum {
+  AMI_MAX_INT = 12,   /* internal sums m */
+  AMI_MAX_EXT = 4,    /* external frequencies */
+  AMI_MAX_EPS = 32,   /* energy symbols */
+  AMI_MAX_DERIV = 6   /* highest Fermi/Bose derivative order */
+};
+
+typedef struct ami_table ami_table;
+
+/* Which representation ami_evaluate executes. */
+enum {
+  AMI_PLAN_AUTO = 0,  /* the library's fastest plan for this table */
+  AMI_PLAN_FLAT = 1,  /* the flat term table, term by term (SURVEY 8(a) S3 as written) */
+  AMI_PLAN_TREE = 2   /* terms grouped by denominator product, Fermi products prefix-shared */
+};
+
+typedef struct ami_info {
+  int32_t n_int, n_ext, n_g, n_eps;
+  int32_t n_fermi_leaves;   /* U_F: distinct (energy combination, sigma, derivative order) */
+  int32_t n_den_leaves;     /* U_D: distinct denominators (sign-canonical), excluding the unit leaf */
+  int32_t max_deriv;        /* highest derivative order in the table */
+  int32_t max_den_per_term; /* denominators per term (powers count as repeats) */
+  int64_t n_terms;          /* T_flat after merging identical terms */
+  int64_t n_terms_raw;      /* terms produced by the recursion before merging */
+  int64_t n_multipoles;     /* pole groups with multiplicity > 1 met during construction */
+  int64_t n_groups;         /* distinct denominator products (tree plan) */
+  int64_t n_tree_nodes;     /* Fermi-trie nodes of the tree plan */
+  int64_t n_den_nodes;      /* denominator-trie nodes of the tree plan */
+  int64_t table_bytes;      /* bytes of the device-resident copy (all plans) */
+  int64_t fp64_ops_flat;    /* FP64 instructions per (sample,frequency,beta) of the flat term loop */
+  int64_t fp64_ops_tree;    /* same for the tree plan */
+  int32_t has_device_copy;
+  int32_t reserved;
+} ami_info;
+
+/* ami_construct -- Eqs. 1-5, API of PAPER.md:246.
+ *   n_int   number of Matsubara sums m (N_INT);  n_ext number of external frequencies (>= 0)
+ *   n_g     number of Green's functions N in R0;  n_eps number of distinct energy symbols
+ *   alpha   [n_g][n_int + n_ext] frequency coefficients, external LAST
+ *   eps     [n_g][n_eps] energy coefficients; rows of R0 are unit vectors, lines with equal
+ *           alpha must share a symbol so that a double pole is recognised
+ *   slot_is_fermionic [n_int + n_ext]: statistics of each frequency slot (P5); internal slots
+ *           must be fermionic (Eq. 3), else AMI_EINVAL
+ *   sum_order [n_int] order of the sums, or NULL for 0..n_int-1
+ *   prefactor the constant A of Eq. 6, usually 1
+ *   device  CUDA device ordinal for the resident copy, or -1 for a host-only table
+ *   out     receives the table; destroy with ami_table_destroy
+ * Errors: AMI_EINVAL, AMI_EUNSUPPORTED_ALPHA, AMI_ENOPOLE, AMI_EUNSUPPORTED (limits), AMI_ENOMEM,
+ * AMI_ECUDA. */
+int ami_construct(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha, const int32_t* eps,
+                  const uint8_t* slot_is_fermionic, const int32_t* sum_order, double prefactor, int device,
+                  ami_table** out);
+
+int ami_table_info(const ami_table* tab, ami_info* info);
+
+/* Serialises the flat table for inspection and tests.  Call with host_buf = NULL to get the size
+ * in *bytes; then with a buffer of at least that size.  Layout (little endian, all int32 unless
+ * noted): magic 'AMI1', n_int, n_ext, n_eps, U_F, U_D, T, m_f (Fermi factors per term = n_int),
+ * n_d (denominator slots per term); then
+ *   leafF_c   int32 [U_F][n_eps]   energy combination of each Fermi/Bose leaf
+ *   leafF_sig int32 [U_F]          sigma = +1 / -1   (f_sigma(E) = 1/(sigma e^{beta E} + 1))
+ *   leafF_k   int32 [U_F]          derivative order
+ *   leafD_c   int32 [U_D][n_eps]   energy combination of each denominator
+ *   leafD_a   int32 [U_D][n_ext]   external-frequency coefficients of each denominator
+ *   fidx      int32 [T][m_f]       Fermi leaf of each factor
+ *   didx      int32 [T][n_d]       denominator leaf of each factor, -1 = empty slot (factor 1)
+ *   coef      float64 [T]          sign and rational prefactor of the term (without A)
+ * The term value is A * coef * prod_a f^{(k)}_{sigma}(leafF_c . e) * prod_b 1/(leafD_a . z + leafD_c . e). */
+int ami_table_export(const ami_table* tab, void* host_buf, size_t* bytes);
+
+void ami_table_destroy(ami_table* tab);
+
+/* ami_dispersion -- Eqs. 8-18 for the 2D square lattice:
+ *   K_i = sum_l alpha^i_l k_l + sum_x alpha^i_ext,x q_x,   e_i = 2 t (cos K_i,x + cos K_i,y) + mu
+ * i.e. e_i = -eps(K_i) with eps(k) = -2t(cos kx + cos ky) - mu.
+ *   d_k     momenta; component c (0 = x, 1 = y) of internal momentum l of sample s is at
+ *           d_k[s * k_stride_sample + (2*l + c) * k_stride_comp].  The paper's layout (Eq. 8,
+ *           row-major [N][2m]) is (2m, 1); SoA [2m][N] is (1, N).
+ *   q       host [n_ext][2] external momenta;  t, mu: hopping and chemical potential
+ *   d_e     out, float64 [n_eps][n] (SoA: sample index fastest) */
+int ami_dispersion(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
+                   const double* q, double t, double mu, int64_t n, double* d_e, void* stream);
+
+/* ami_evaluate -- PAPER.md:106-113, :282-289.
+ *   d_e     energies, [n_eps][n_e] float64, or complex128 if e_is_complex
+ *   z_ext   host complex128 [n_f][n_ext]: external frequency values (i nu_ext on the Matsubara axis,
+ *           omega + i Gamma after analytic continuation).  The paper's frequency_t rows
+ *           also carry m internal placeholders; only the external columns are used (P13).
+ *   beta    host [n_b] inverse temperatures (the paper's ami_vars holds one)
+ *   e_reg   regulator eta, applied as in P10: added to the argument of every sigma = -1
+ *           leaf and to every denominator whose frequency part is identically zero for that
+ *           frequency; decided by table and frequency metadata only, never by sample values.
+ *   plan    AMI_PLAN_*
+ *   d_out   complex128 [n_b][n_f][n_e] (rows = frequencies, energy index fastest) */
+int ami_evaluate(const ami_table* tab, const void* d_e, int e_is_complex, int64_t n_e, const double* z_ext,
+                 int n_f, const double* beta, int n_b, double e_reg, int plan, void* d_out, void* stream);
+
+/* Streamed driver.  Source of the momenta: if h_k / d_k are both NULL they are generated on the
+ * device from `seed` with the counter-based generator of P22 (sample index = first_sample + s);
+ * else read from the given buffer, layout [n][2*n_int] (Eq. 8).  Results: per-sample values to
+ * h_out / d_out (complex128 [n_b][n_f][n]) when given, and/or the running sum over samples to
+ * h_sum (complex128 [n_b][n_f], Monte-Carlo tally of PAPER.md:291) when want_sum. */
+typedef struct ami_run_cfg {
+  int64_t n;             /* samples */
+  int64_t chunk;         /* samples per chunk (0 = library default) */
+  uint64_t seed;
+  int64_t first_sample;
+  const double* h_k;     /* host momenta or NULL */
+  const double* d_k;     /* device momenta or NULL */
+  const double* q;       /* host [n_ext][2] */
+  double t, mu;
+  const double* z_ext;   /* host complex128 [n_f][n_ext] */
+  int32_t n_f;
+  const double* beta;    /* host [n_b] */
+  int32_t n_b;
+  double e_reg;
+  int32_t plan;
+  int32_t want_sum;
+  void* h_out;           /* host complex128 [n_b][n_f][n] or NULL */
+  void* d_out;           /* device complex128 [n_b][n_f][n] or NULL */
+  void* h_sum;           /* host complex128 [n_b][n_f] or NULL */
+  void* stream;          /* caller's stream; internal copy/compute streams are ordered after it */
+} ami_run_cfg;
+
+typedef struct ami_run_stats {
+  int64_t n_chunks;
+  int64_t kernel_launches;  /* kernels of this library launched by the call */
+  int64_t h2d_bytes, d2h_bytes;
+  double gpu_ms;            /* CUDA-event time from first to last operation of the call */
+} ami_run_stats;
+
+int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_stats* stats);
+
+/* Fills d_k [n][2*n_int] with the momenta of samples first_sample .. first_sample+n-1 (P22). */
+int ami_generate_momenta(const ami_table* tab, uint64_t seed, int64_t first_sample, int64_t n, double* d_k,
+                         void* stream);
+
+/* Register-only DFMA chain used by bench.py to measure the FP64 pipe peak of the device the
+ * bench runs on (MEASURED_PEAKS.json has no FP64 figure).  Returns in *dfma_per_s the measured
+ * rate of double-precision FMA lane-operations per second. */
+int ami_fp64_peak_probe(int device, double* dfma_per_s, double* elapsed_ms);
+
+const char* ami_strerror(int code);
+const char* ami_last_cuda_error(void);
+int ami_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AMI_B200_H */

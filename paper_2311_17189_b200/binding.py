@@ -1,0 +1,230 @@
+"""Thin ctypes binding of include/ami.h: argument marshalling only.  Every step of the path
+runs in the CUDA kernels of libami_b200.so; PyTorch supplies device memory and streams.
+There is no CPU fallback: without the built library, or without a device copy of the table,
+every call raises."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libami_b200.so")
+
+PLAN_AUTO, PLAN_FLAT, PLAN_TREE = 0, 1, 2
+
+EXPORTS = [
+    "ami_construct", "ami_table_info", "ami_table_export", "ami_table_destroy", "ami_dispersion",
+    "ami_evaluate", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
+    "ami_last_cuda_error", "ami_version",
+]
+
+
+class AmiError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"ami error {code}: {msg}")
+        self.code = code
+
+
+class ami_info(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("n_int", "n_ext", "n_g", "n_eps", "n_fermi_leaves", "n_den_leaves",
+                                         "max_deriv", "max_den_per_term")] + \
+               [(n, C.c_int64) for n in ("n_terms", "n_terms_raw", "n_multipoles", "n_groups", "n_tree_nodes",
+                                         "n_den_nodes", "table_bytes", "fp64_ops_flat", "fp64_ops_tree")] + \
+               [("has_device_copy", C.c_int32), ("reserved", C.c_int32)]
+
+
+class ami_run_cfg(C.Structure):
+    _fields_ = [("n", C.c_int64), ("chunk", C.c_int64), ("seed", C.c_uint64), ("first_sample", C.c_int64),
+                ("h_k", C.c_void_p), ("d_k", C.c_void_p), ("q", C.c_void_p), ("t", C.c_double),
+                ("mu", C.c_double), ("z_ext", C.c_void_p), ("n_f", C.c_int32), ("beta", C.c_void_p),
+                ("n_b", C.c_int32), ("e_reg", C.c_double), ("plan", C.c_int32), ("want_sum", C.c_int32),
+                ("h_out", C.c_void_p), ("d_out", C.c_void_p), ("h_sum", C.c_void_p), ("stream", C.c_void_p)]
+
+
+class ami_run_stats(C.Structure):
+    _fields_ = [("n_chunks", C.c_int64), ("kernel_launches", C.c_int64), ("h2d_bytes", C.c_int64),
+                ("d2h_bytes", C.c_int64), ("gpu_ms", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run __graft_entry__.build() "
+                               "(python -m paper_2311_17189_b200.build); there is no fallback path")
+        L = C.CDLL(LIB_PATH)
+        L.ami_construct.argtypes = [C.c_int] * 4 + [C.c_void_p] * 4 + [C.c_double, C.c_int, C.POINTER(C.c_void_p)]
+        L.ami_table_info.argtypes = [C.c_void_p, C.POINTER(ami_info)]
+        L.ami_table_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
+        L.ami_table_destroy.argtypes = [C.c_void_p]
+        L.ami_table_destroy.restype = None
+        L.ami_dispersion.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
+                                     C.c_double, C.c_int64, C.c_void_p, C.c_void_p]
+        L.ami_evaluate.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_int, C.c_void_p,
+                                   C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
+        L.ami_run.argtypes = [C.c_void_p, C.POINTER(ami_run_cfg), C.POINTER(ami_run_stats)]
+        L.ami_generate_momenta.argtypes = [C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
+        L.ami_fp64_peak_probe.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.ami_strerror.restype = C.c_char_p
+        L.ami_strerror.argtypes = [C.c_int]
+        L.ami_last_cuda_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        msg = lib().ami_strerror(rc).decode()
+        if rc in (-4, -5):
+            msg += " [" + lib().ami_last_cuda_error().decode() + "]"
+        raise AmiError(rc, msg)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(int(stream))
+
+
+def _host(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _z_host(z_ext, n_ext):
+    return np.ascontiguousarray(np.asarray(z_ext, dtype=np.complex128).reshape(-1, max(n_ext, 1)))
+
+
+class AmiTable:
+    """ami_construct: the symbolic result of one labelled diagram, resident on
+    ``device`` (a CUDA ordinal) or host-only when ``device`` is None."""
+
+    def __init__(self, n_int, n_ext, alpha, eps, slot_is_fermionic, sum_order=None, prefactor=1.0, device=0):
+        alpha = _host(alpha, np.int32)
+        eps = _host(eps, np.int32)
+        stat = _host(slot_is_fermionic, np.uint8)
+        so = None if sum_order is None else _host(sum_order, np.int32)
+        if alpha.ndim != 2 or eps.ndim != 2 or alpha.shape[0] != eps.shape[0] or alpha.shape[1] != n_int + n_ext \
+                or stat.shape != (n_int + n_ext,):
+            raise AmiError(-1, "shape mismatch")
+        h = C.c_void_p()
+        _check(lib().ami_construct(n_int, n_ext, alpha.shape[0], eps.shape[1], alpha.ctypes.data, eps.ctypes.data,
+                                   stat.ctypes.data, None if so is None else so.ctypes.data, float(prefactor),
+                                   -1 if device is None else int(device), C.byref(h)))
+        self._h = h
+        self.device = device
+        self.info = self._info()
+        self.n_int, self.n_ext, self.n_eps = n_int, n_ext, eps.shape[1]
+
+    @classmethod
+    def from_diagram(cls, d, **kw):
+        return cls(d.n_int, d.n_ext, d.alpha, d.eps, d.slot_is_fermionic, **kw)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().ami_table_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _info(self) -> dict:
+        s = ami_info()
+        _check(lib().ami_table_info(self._h, C.byref(s)))
+        return {n: getattr(s, n) for n, _ in ami_info._fields_ if n != "reserved"}
+
+    def export(self) -> dict:
+        """ami_table_export parsed into numpy arrays (layout documented in include/ami.h)."""
+        n = C.c_size_t(0)
+        _check(lib().ami_table_export(self._h, None, C.byref(n)))
+        buf = np.zeros(n.value, dtype=np.uint8)
+        _check(lib().ami_table_export(self._h, buf.ctypes.data, C.byref(n)))
+        w = buf[: (n.value // 4) * 4].view(np.int32)
+        assert w[0] == 0x31494D41
+        n_int, n_ext, n_eps, UF, UD, T, mf, nd = (int(x) for x in w[1:9])
+        pos = 9
+
+        def take(*shape):
+            nonlocal pos
+            cnt = int(np.prod(shape)) if shape else 1
+            a = w[pos:pos + cnt].reshape(shape).copy()
+            pos += cnt
+            return a
+
+        out = {"n_int": n_int, "n_ext": n_ext, "n_eps": n_eps,
+               "leafF_c": take(UF, n_eps), "leafF_sig": take(UF), "leafF_k": take(UF),
+               "leafD_c": take(UD, n_eps), "leafD_a": take(UD, n_ext),
+               "fidx": take(T, mf), "didx": take(T, nd)}
+        off = (pos * 4 + 7) // 8 * 8
+        out["coef"] = buf[off:off + 8 * T].view(np.float64).copy()
+        return out
+
+    # ---- kernels -------------------------------------------------------------------------
+    def dispersion(self, k, q, t, mu, out=None, stream=None):
+        """ami_dispersion.  k: CUDA float64 tensor [n][n_int][2] (Eq. 8 layout) -> e [n_eps][n]."""
+        import torch
+        assert k.is_cuda and k.dtype == torch.float64 and k.is_contiguous()
+        n = k.shape[0]
+        if out is None:
+            out = torch.empty((self.n_eps, n), dtype=torch.float64, device=k.device)
+        qh = _host(np.asarray(q, dtype=np.float64).reshape(max(self.n_ext, 1), 2), np.float64)
+        _check(lib().ami_dispersion(self._h, C.c_void_p(k.data_ptr()), 2 * self.n_int, 1, qh.ctypes.data, float(t),
+                                    float(mu), n, C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        return out
+
+    def evaluate(self, e, z_ext, beta, e_reg=0.0, plan=PLAN_AUTO, out=None, stream=None):
+        """ami_evaluate.  e: CUDA tensor [n_eps][n_e], float64 or complex128 -> complex128
+        [n_b][n_f][n_e]."""
+        import torch
+        assert e.is_cuda and e.is_contiguous() and e.shape[0] == self.n_eps
+        is_c = e.dtype == torch.complex128
+        assert is_c or e.dtype == torch.float64
+        z = _z_host(z_ext, self.n_ext)
+        b = _host(np.atleast_1d(beta), np.float64)
+        n_e, n_f, n_b = e.shape[1], z.shape[0], b.shape[0]
+        if out is None:
+            out = torch.empty((n_b, n_f, n_e), dtype=torch.complex128, device=e.device)
+        assert out.is_contiguous() and out.dtype == torch.complex128 and out.numel() == n_b * n_f * n_e
+        _check(lib().ami_evaluate(self._h, C.c_void_p(e.data_ptr()), int(is_c), n_e, z.ctypes.data, n_f,
+                                  b.ctypes.data, n_b, float(e_reg), int(plan), C.c_void_p(out.data_ptr()),
+                                  _stream_ptr(stream)))
+        return out
+
+    def generate_momenta(self, seed, first_sample, n, stream=None):
+        import torch
+        k = torch.empty((n, self.n_int, 2), dtype=torch.float64, device=f"cuda:{self.device}")
+        _check(lib().ami_generate_momenta(self._h, int(seed), int(first_sample), n, C.c_void_p(k.data_ptr()),
+                                          _stream_ptr(stream)))
+        return k
+
+    def run(self, n, q, t, mu, z_ext, beta, e_reg=0.0, plan=PLAN_AUTO, seed=0, first_sample=0, chunk=0,
+            h_k=None, d_k=None, h_out=None, d_out=None, want_sum=False, stream=None):
+        """ami_run, the streamed driver.  h_k / h_out are (preferably pinned) CPU tensors or numpy
+        arrays; d_k / d_out CUDA tensors.  Returns (stats dict, sums or None)."""
+        z = _z_host(z_ext, self.n_ext)
+        b = _host(np.atleast_1d(beta), np.float64)
+        qh = _host(np.asarray(q, dtype=np.float64).reshape(max(self.n_ext, 1), 2), np.float64)
+        cfg = ami_run_cfg()
+        cfg.n, cfg.chunk, cfg.seed, cfg.first_sample = int(n), int(chunk), int(seed), int(first_sample)
+        ptr = lambda x: None if x is None else (x.ctypes.data if isinstance(x, np.ndarray) else x.data_ptr())
+        cfg.h_k, cfg.d_k, cfg.h_out, cfg.d_out = ptr(h_k), ptr(d_k), ptr(h_out), ptr(d_out)
+        cfg.q, cfg.t, cfg.mu = qh.ctypes.data, float(t), float(mu)
+        cfg.z_ext, cfg.n_f, cfg.beta, cfg.n_b = z.ctypes.data, z.shape[0], b.ctypes.data, b.shape[0]
+        cfg.e_reg, cfg.plan, cfg.want_sum = float(e_reg), int(plan), int(bool(want_sum))
+        sums = np.zeros((b.shape[0], z.shape[0]), dtype=np.complex128) if want_sum else None
+        cfg.h_sum = None if sums is None else sums.ctypes.data
+        cfg.stream = _stream_ptr(stream)
+        st = ami_run_stats()
+        _check(lib().ami_run(self._h, C.byref(cfg), C.byref(st)))
+        return {n_: getattr(st, n_) for n_, _ in ami_run_stats._fields_}, sums
+
+
+def fp64_peak_probe(device=0):
+    """Measured DFMA lane-operations per second of ``device`` (register-only chains)."""
+    r, ms = C.c_double(0), C.c_double(0)
+    _check(lib().ami_fp64_peak_probe(int(device), C.byref(r), C.byref(ms)))
+    return r.value, ms.value

@@ -1,0 +1,463 @@
+// The C ABI of include/ami.h: argument checking, device residency, launches, streamed driver.
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "ami_kernels.cuh"
+
+namespace ami {
+long long flat_fp64_ops(const FlatTable& ft);
+}
+
+namespace {
+
+thread_local std::string g_cuda_err;
+
+int cuda_fail(cudaError_t rc) {
+  g_cuda_err = std::string(cudaGetErrorName(rc)) + ": " + cudaGetErrorString(rc);
+  return rc == cudaErrorMemoryAllocation ? AMI_ENOMEM : AMI_ECUDA;
+}
+#define CU(x)                                   \
+  do {                                          \
+    cudaError_t rc_ = (x);                      \
+    if (rc_ != cudaSuccess) return cuda_fail(rc_); \
+  } while (0)
+
+template <class T>
+int upload(const std::vector<T>& h, T** d, int64_t& bytes) {
+  *d = nullptr;
+  const size_t n = std::max<size_t>(h.size(), 1) * sizeof(T);
+  CU(cudaMalloc((void**)d, n));
+  if (!h.empty()) CU(cudaMemcpy(*d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+  bytes += (int64_t)n;
+  return AMI_OK;
+}
+
+// Q_k polynomials of f^{(k)} = beta^k f g Q_k(f):  Q_1 = -1, Q_{k+1} = (2f-1) Q_k - (f - f^2) Q_k'
+std::vector<double> deriv_polys() {
+  const int S = 8;
+  std::vector<double> Q((AMI_MAX_DERIV + 1) * S, 0.0);
+  Q[1 * S + 0] = -1.0;
+  for (int k = 1; k < AMI_MAX_DERIV; ++k) {
+    const double* q = &Q[k * S];
+    double* r = &Q[(k + 1) * S];
+    for (int i = 0; i < S - 2; ++i) {
+      r[i + 1] += 2.0 * q[i];
+      r[i] -= q[i];
+      if (i >= 1) {
+        r[i] -= i * q[i];         // -f * (i q_i f^{i-1})
+        r[i + 1] += i * q[i];     // +f^2 * (i q_i f^{i-1})
+      }
+    }
+  }
+  return Q;
+}
+
+int make_device_copy(ami_table* tab, int device) {
+  using namespace ami;
+  const FlatTable& ft = tab->flat;
+  ami_device_copy& dc = tab->dev;
+  CU(cudaSetDevice(device));
+  dc.device = device;
+  const int UF = (int)ft.leafF.size(), UD = (int)ft.leafD.size();
+  std::vector<int32_t> ptr;
+  std::vector<int8_t> sym, coef, sig, kk, da, sa;
+  ptr.push_back(0);
+  for (const LeafF& l : ft.leafF) {
+    for (int i = 0; i < ft.n_eps; ++i)
+      if (l.c[i]) { sym.push_back((int8_t)i); coef.push_back((int8_t)l.c[i]); }
+    ptr.push_back((int32_t)sym.size());
+    sig.push_back((int8_t)l.sigma);
+    kk.push_back((int8_t)l.k);
+  }
+  for (const LeafD& l : ft.leafD) {
+    for (int i = 0; i < ft.n_eps; ++i)
+      if (l.c[i]) { sym.push_back((int8_t)i); coef.push_back((int8_t)l.c[i]); }
+    ptr.push_back((int32_t)sym.size());
+    for (int x = 0; x < ft.n_ext; ++x) da.push_back((int8_t)l.a[x]);
+  }
+  const int nd = ft.max_den;
+  std::vector<uint16_t> tix;
+  std::vector<double> tco;
+  for (const FlatTerm& t : ft.terms) {
+    for (int f : t.f) tix.push_back((uint16_t)f);
+    for (int j = 0; j < nd; ++j) tix.push_back((uint16_t)(j < (int)t.d.size() ? t.d[j] : UD));
+    tco.push_back((double)t.num / (double)t.den);
+  }
+  for (int v : ft.sym_alpha) sa.push_back((int8_t)v);
+  (void)UF;
+  int rc;
+  if ((rc = upload(ptr, &dc.leaf_ptr, dc.bytes))) return rc;
+  if ((rc = upload(sym, &dc.leaf_sym, dc.bytes))) return rc;
+  if ((rc = upload(coef, &dc.leaf_coef, dc.bytes))) return rc;
+  if ((rc = upload(sig, &dc.leafF_sig, dc.bytes))) return rc;
+  if ((rc = upload(kk, &dc.leafF_k, dc.bytes))) return rc;
+  if ((rc = upload(da, &dc.leafD_a, dc.bytes))) return rc;
+  if ((rc = upload(tix, &dc.term_idx, dc.bytes))) return rc;
+  if ((rc = upload(tco, &dc.term_coef, dc.bytes))) return rc;
+  if ((rc = upload(tab->tree.code, &dc.tree_code, dc.bytes))) return rc;
+  if ((rc = upload(tab->tree.consts, &dc.tree_consts, dc.bytes))) return rc;
+  if ((rc = upload(sa, &dc.sym_alpha, dc.bytes))) return rc;
+  if ((rc = upload(deriv_polys(), &dc.derivQ, dc.bytes))) return rc;
+  return AMI_OK;
+}
+
+void free_device_copy(ami_device_copy& dc) {
+  if (dc.device < 0) return;
+  cudaSetDevice(dc.device);
+  cudaFree(dc.leaf_ptr); cudaFree(dc.leaf_sym); cudaFree(dc.leaf_coef); cudaFree(dc.leafF_sig);
+  cudaFree(dc.leafF_k); cudaFree(dc.leafD_a); cudaFree(dc.term_idx); cudaFree(dc.term_coef);
+  cudaFree(dc.tree_code); cudaFree(dc.tree_consts); cudaFree(dc.sym_alpha); cudaFree(dc.derivQ);
+  dc = ami_device_copy();
+}
+
+}  // namespace
+
+extern "C" {
+
+int ami_version(void) { return 1; }
+
+const char* ami_strerror(int code) {
+  switch (code) {
+    case AMI_OK: return "ok";
+    case AMI_EINVAL: return "invalid argument";
+    case AMI_EUNSUPPORTED_ALPHA: return "|alpha_p| != 1 met at a summation (unsupported)";
+    case AMI_ENOPOLE: return "a term has no pole in the summed frequency";
+    case AMI_ECUDA: return "CUDA error, or the table has no device copy";
+    case AMI_ENOMEM: return "out of memory";
+    case AMI_EUNSUPPORTED: return "outside the built limits";
+    default: return "unknown error";
+  }
+}
+
+const char* ami_last_cuda_error(void) { return g_cuda_err.c_str(); }
+
+int ami_construct(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha, const int32_t* eps,
+                  const uint8_t* slot_is_fermionic, const int32_t* sum_order, double prefactor, int device,
+                  ami_table** out) {
+  if (!out) return AMI_EINVAL;
+  *out = nullptr;
+  ami_table* tab = new (std::nothrow) ami_table;
+  if (!tab) return AMI_ENOMEM;
+  int rc;
+  try {
+    rc = ami::construct_flat(n_int, n_ext, n_g, n_eps, alpha, eps, slot_is_fermionic, sum_order, prefactor,
+                             tab->flat);
+    if (rc == AMI_OK) {
+      ami::build_tree_plan(tab->flat, tab->tree);
+      tab->fp64_ops_flat = ami::flat_fp64_ops(tab->flat);
+    }
+  } catch (const std::bad_alloc&) {
+    rc = AMI_ENOMEM;
+  } catch (...) {
+    rc = AMI_EINVAL;
+  }
+  if (rc == AMI_OK && device >= 0) {
+    rc = make_device_copy(tab, device);
+    if (rc != AMI_OK) free_device_copy(tab->dev);
+  }
+  if (rc != AMI_OK) { delete tab; return rc; }
+  *out = tab;
+  return AMI_OK;
+}
+
+void ami_table_destroy(ami_table* tab) {
+  if (!tab) return;
+  free_device_copy(tab->dev);
+  delete tab;
+}
+
+int ami_table_info(const ami_table* tab, ami_info* info) {
+  if (!tab || !info) return AMI_EINVAL;
+  const ami::FlatTable& ft = tab->flat;
+  memset(info, 0, sizeof *info);
+  info->n_int = ft.n_int; info->n_ext = ft.n_ext; info->n_g = ft.n_g; info->n_eps = ft.n_eps;
+  info->n_fermi_leaves = (int32_t)ft.leafF.size();
+  info->n_den_leaves = (int32_t)ft.leafD.size();
+  info->max_deriv = ft.max_deriv;
+  info->max_den_per_term = ft.max_den;
+  info->n_terms = (int64_t)ft.terms.size();
+  info->n_terms_raw = ft.n_terms_raw;
+  info->n_multipoles = ft.n_multipoles;
+  info->n_groups = tab->tree.n_groups;
+  info->n_tree_nodes = tab->tree.n_fnodes;
+  info->n_den_nodes = tab->tree.n_dnodes;
+  info->table_bytes = tab->dev.bytes;
+  info->fp64_ops_flat = tab->fp64_ops_flat;
+  info->fp64_ops_tree = tab->tree.fp64_ops;
+  info->has_device_copy = tab->dev.device >= 0;
+  return AMI_OK;
+}
+
+int ami_table_export(const ami_table* tab, void* host_buf, size_t* bytes) {
+  if (!tab || !bytes) return AMI_EINVAL;
+  const ami::FlatTable& ft = tab->flat;
+  const size_t UF = ft.leafF.size(), UD = ft.leafD.size(), T = ft.terms.size();
+  const size_t mf = ft.n_int, nd = ft.max_den;
+  const size_t n_i32 = 9 + UF * ft.n_eps + 2 * UF + UD * ft.n_eps + UD * ft.n_ext + T * mf + T * nd;
+  size_t need = n_i32 * 4;
+  need = (need + 7) / 8 * 8 + T * 8;
+  if (!host_buf) { *bytes = need; return AMI_OK; }
+  if (*bytes < need) return AMI_EINVAL;
+  int32_t* w = (int32_t*)host_buf;
+  *w++ = 0x31494D41;  // 'AMI1'
+  *w++ = ft.n_int; *w++ = ft.n_ext; *w++ = ft.n_eps; *w++ = (int32_t)UF; *w++ = (int32_t)UD;
+  *w++ = (int32_t)T; *w++ = (int32_t)mf; *w++ = (int32_t)nd;
+  for (const auto& l : ft.leafF) for (int v : l.c) *w++ = v;
+  for (const auto& l : ft.leafF) *w++ = l.sigma;
+  for (const auto& l : ft.leafF) *w++ = l.k;
+  for (const auto& l : ft.leafD) for (int v : l.c) *w++ = v;
+  for (const auto& l : ft.leafD) for (int v : l.a) *w++ = v;
+  for (const auto& t : ft.terms) for (int v : t.f) *w++ = v;
+  for (const auto& t : ft.terms)
+    for (size_t j = 0; j < nd; ++j) *w++ = j < t.d.size() ? t.d[j] : -1;
+  char* p = (char*)host_buf + (n_i32 * 4 + 7) / 8 * 8;
+  for (const auto& t : ft.terms) {
+    double c = (double)t.num / (double)t.den;
+    memcpy(p, &c, 8);
+    p += 8;
+  }
+  *bytes = need;
+  return AMI_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// kernel entry points
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+void fill_table_params(const ami_table* tab, ami::EvalParams& p) {
+  const ami::FlatTable& ft = tab->flat;
+  const ami_device_copy& dc = tab->dev;
+  p.leaf_ptr = dc.leaf_ptr; p.leaf_sym = dc.leaf_sym; p.leaf_coef = dc.leaf_coef;
+  p.leafF_sig = dc.leafF_sig; p.leafF_k = dc.leafF_k; p.leafD_a = dc.leafD_a;
+  p.term_idx = dc.term_idx; p.term_coef = dc.term_coef;
+  p.tree_code = dc.tree_code; p.tree_consts = dc.tree_consts; p.derivQ = dc.derivQ;
+  p.n_eps = ft.n_eps; p.n_ext = ft.n_ext;
+  p.U_F = (int)ft.leafF.size(); p.U_D = (int)ft.leafD.size();
+  p.m_f = ft.n_int; p.n_d = ft.max_den;
+  p.T = (long long)ft.terms.size();
+  p.prefactor = ft.prefactor;
+}
+
+// Launches the evaluation for all (beta, frequency) pairs, split so that one launch carries at
+// most kMaxBeta temperatures and kMaxFreqWords frequency words.  `out` points at sample 0 of
+// row (b=0,f=0); rows are out_row_stride samples apart.
+int evaluate_impl(const ami_table* tab, const void* d_e, int e_is_complex, int64_t n_e, int64_t e_stride,
+                  const double* z_ext, int n_f, const double* beta, int n_b, double e_reg, int plan,
+                  void* d_out, int64_t out_row_stride, cudaStream_t st, int* launches) {
+  using namespace ami;
+  EvalParams p;
+  memset(&p, 0, sizeof p);
+  fill_table_params(tab, p);
+  p.e = (const double*)d_e; p.out = (double*)d_out;
+  p.n_e = n_e; p.e_stride = e_stride; p.out_row_stride = out_row_stride;
+  p.n_f_total = n_f; p.e_reg = e_reg;
+  const int n_ext = tab->flat.n_ext;
+  const int f_chunk = n_ext ? std::max(1, kMaxFreqWords / n_ext) : kMaxFreqWords;
+  const bool use_tree = (plan == AMI_PLAN_TREE || plan == AMI_PLAN_AUTO) && !tab->tree.code.empty();
+  for (int b0 = 0; b0 < n_b; b0 += kMaxBeta) {
+    p.b0 = b0; p.n_b = std::min(kMaxBeta, n_b - b0);
+    for (int i = 0; i < p.n_b; ++i) p.beta[i] = beta[b0 + i];
+    for (int f0 = 0; f0 < n_f; f0 += f_chunk) {
+      p.f0 = f0; p.n_f = std::min(f_chunk, n_f - f0);
+      for (int i = 0; i < p.n_f * n_ext * 2; ++i) p.z[i] = z_ext[(size_t)f0 * n_ext * 2 + i];
+      cudaError_t rc = use_tree ? launch_eval_tree(p, e_is_complex != 0, st, launches)
+                                : launch_eval_flat(p, e_is_complex != 0, st, launches);
+      if (rc != cudaSuccess) return cuda_fail(rc);
+    }
+  }
+  return AMI_OK;
+}
+
+int check_device(const ami_table* tab) {
+  if (!tab) return AMI_EINVAL;
+  if (tab->dev.device < 0) { g_cuda_err = "table has no device copy"; return AMI_ECUDA; }
+  CU(cudaSetDevice(tab->dev.device));
+  return AMI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ami_dispersion(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
+                   const double* q, double t, double mu, int64_t n, double* d_e, void* stream) {
+  int rc = check_device(tab);
+  if (rc) return rc;
+  if (n < 0 || (n > 0 && (!d_k || !d_e)) || (tab->flat.n_ext > 0 && !q)) return AMI_EINVAL;
+  ami::DispParams p;
+  memset(&p, 0, sizeof p);
+  p.sym_alpha = tab->dev.sym_alpha;
+  p.n_int = tab->flat.n_int; p.n_ext = tab->flat.n_ext; p.n_eps = tab->flat.n_eps;
+  p.k = d_k; p.k_stride_sample = k_stride_sample; p.k_stride_comp = k_stride_comp; p.n = n;
+  for (int i = 0; i < 2 * p.n_ext; ++i) p.q[i] = q[i];
+  p.t = t; p.mu = mu; p.e = d_e; p.e_stride = n;
+  CU(ami::launch_dispersion(p, (cudaStream_t)stream));
+  return AMI_OK;
+}
+
+int ami_evaluate(const ami_table* tab, const void* d_e, int e_is_complex, int64_t n_e, const double* z_ext,
+                 int n_f, const double* beta, int n_b, double e_reg, int plan, void* d_out, void* stream) {
+  int rc = check_device(tab);
+  if (rc) return rc;
+  if (n_e < 0 || n_f < 0 || n_b < 0 || (n_f > 0 && tab->flat.n_ext > 0 && !z_ext) || (n_b > 0 && !beta) ||
+      plan < AMI_PLAN_AUTO || plan > AMI_PLAN_TREE)
+    return AMI_EINVAL;
+  if (n_e == 0 || n_f == 0 || n_b == 0) return AMI_OK;
+  if (!d_e || !d_out) return AMI_EINVAL;
+  return evaluate_impl(tab, d_e, e_is_complex, n_e, n_e, z_ext, n_f, beta, n_b, e_reg, plan, d_out, n_e,
+                       (cudaStream_t)stream, nullptr);
+}
+
+int ami_generate_momenta(const ami_table* tab, uint64_t seed, int64_t first_sample, int64_t n, double* d_k,
+                         void* stream) {
+  int rc = check_device(tab);
+  if (rc) return rc;
+  if (n < 0 || first_sample < 0 || (n > 0 && !d_k)) return AMI_EINVAL;
+  CU(ami::launch_generate_momenta(seed, first_sample, n, 2 * tab->flat.n_int, d_k, (cudaStream_t)stream));
+  return AMI_OK;
+}
+
+int ami_fp64_peak_probe(int device, double* dfma_per_s, double* elapsed_ms) {
+  if (!dfma_per_s || !elapsed_ms || device < 0) return AMI_EINVAL;
+  CU(cudaSetDevice(device));
+  CU(ami::run_fp64_probe(dfma_per_s, elapsed_ms));
+  return AMI_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// S4: streamed driver.  Chunks alternate between two internal streams, each with its own
+// momentum / energy / output buffers, so that the copy (or generation) of chunk c+1 overlaps
+// the evaluation of chunk c (PAPER.md:113: repeated calls over energy batches; :291 tally).
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+struct RunBuffers {
+  cudaStream_t st[2] = {nullptr, nullptr};
+  cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_done[2] = {nullptr, nullptr};
+  double* k[2] = {nullptr, nullptr};
+  double* e[2] = {nullptr, nullptr};
+  double* out[2] = {nullptr, nullptr};
+  double* partial = nullptr;
+  double* sum = nullptr;
+  ~RunBuffers() {
+    for (int i = 0; i < 2; ++i) {
+      if (st[i]) cudaStreamDestroy(st[i]);
+      if (ev_done[i]) cudaEventDestroy(ev_done[i]);
+      cudaFree(k[i]); cudaFree(e[i]); cudaFree(out[i]);
+    }
+    if (ev_start) cudaEventDestroy(ev_start);
+    if (ev_stop) cudaEventDestroy(ev_stop);
+    cudaFree(partial); cudaFree(sum);
+  }
+};
+
+}  // namespace
+
+extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_stats* stats) {
+  int rc = check_device(tab);
+  if (rc) return rc;
+  if (!cfg || cfg->n < 0 || cfg->n_f < 0 || cfg->n_b < 0 || cfg->chunk < 0 || cfg->first_sample < 0 ||
+      (cfg->n_b > 0 && !cfg->beta) || (cfg->n_f > 0 && tab->flat.n_ext > 0 && !cfg->z_ext) ||
+      (tab->flat.n_ext > 0 && !cfg->q) || (cfg->h_k && cfg->d_k) || (cfg->want_sum && !cfg->h_sum))
+    return AMI_EINVAL;
+  ami_run_stats local;
+  memset(&local, 0, sizeof local);
+  const int64_t rows = (int64_t)cfg->n_b * cfg->n_f;
+  const int n_comp = 2 * tab->flat.n_int, n_eps = tab->flat.n_eps;
+  if (cfg->n == 0 || rows == 0) {
+    if (cfg->want_sum) memset(cfg->h_sum, 0, (size_t)rows * 16);
+    if (stats) *stats = local;
+    return AMI_OK;
+  }
+  int64_t chunk = cfg->chunk ? cfg->chunk : (int64_t)1 << 20;
+  // keep a chunk's output below ~256 MiB
+  while (chunk > 1024 && chunk * rows * 16 > ((int64_t)256 << 20)) chunk /= 2;
+  if (chunk > cfg->n) chunk = cfg->n;
+  const bool direct_out = cfg->d_out != nullptr;   // kernels write straight into the caller's buffer
+  RunBuffers rb;
+  cudaStream_t user = (cudaStream_t)cfg->stream;
+  CU(cudaEventCreate(&rb.ev_start));
+  CU(cudaEventCreate(&rb.ev_stop));
+  for (int i = 0; i < 2; ++i) {
+    CU(cudaStreamCreateWithFlags(&rb.st[i], cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&rb.ev_done[i], cudaEventDisableTiming));
+    if (!cfg->d_k) CU(cudaMalloc((void**)&rb.k[i], (size_t)chunk * n_comp * 8));
+    CU(cudaMalloc((void**)&rb.e[i], (size_t)chunk * n_eps * 8));
+    if (!direct_out) CU(cudaMalloc((void**)&rb.out[i], (size_t)chunk * rows * 16));
+  }
+  if (cfg->want_sum) {
+    CU(cudaMalloc((void**)&rb.partial, (size_t)rows * 64 * 16));
+    CU(cudaMalloc((void**)&rb.sum, (size_t)rows * 16));
+    CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 16, user));
+  }
+  CU(cudaEventRecord(rb.ev_start, user));
+  CU(cudaStreamWaitEvent(rb.st[0], rb.ev_start, 0));
+  CU(cudaStreamWaitEvent(rb.st[1], rb.ev_start, 0));
+  int launches = 0;
+  for (int64_t c0 = 0, ci = 0; c0 < cfg->n; c0 += chunk, ++ci) {
+    const int s = (int)(ci & 1);
+    const int64_t nc = std::min(chunk, cfg->n - c0);
+    cudaStream_t st = rb.st[s];
+    const double* kbuf;
+    if (cfg->d_k) {
+      kbuf = cfg->d_k + c0 * n_comp;
+    } else if (cfg->h_k) {
+      CU(cudaMemcpyAsync(rb.k[s], cfg->h_k + c0 * n_comp, (size_t)nc * n_comp * 8, cudaMemcpyHostToDevice, st));
+      local.h2d_bytes += nc * n_comp * 8;
+      kbuf = rb.k[s];
+    } else {
+      CU(ami::launch_generate_momenta(cfg->seed, cfg->first_sample + c0, nc, n_comp, rb.k[s], st));
+      ++launches;
+      kbuf = rb.k[s];
+    }
+    ami::DispParams dp;
+    memset(&dp, 0, sizeof dp);
+    dp.sym_alpha = tab->dev.sym_alpha;
+    dp.n_int = tab->flat.n_int; dp.n_ext = tab->flat.n_ext; dp.n_eps = n_eps;
+    dp.k = kbuf; dp.k_stride_sample = n_comp; dp.k_stride_comp = 1; dp.n = nc;
+    for (int i = 0; i < 2 * dp.n_ext; ++i) dp.q[i] = cfg->q[i];
+    dp.t = cfg->t; dp.mu = cfg->mu; dp.e = rb.e[s]; dp.e_stride = nc;
+    CU(ami::launch_dispersion(dp, st));
+    ++launches;
+    double* obuf = direct_out ? (double*)cfg->d_out + 2 * c0 : rb.out[s];
+    const int64_t ostride = direct_out ? cfg->n : nc;
+    rc = evaluate_impl(tab, rb.e[s], 0, nc, nc, cfg->z_ext, cfg->n_f, cfg->beta, cfg->n_b, cfg->e_reg, cfg->plan,
+                       obuf, ostride, st, &launches);
+    if (rc) return rc;
+    if (cfg->h_out) {
+      CU(cudaMemcpy2DAsync((char*)cfg->h_out + (size_t)c0 * 16, (size_t)cfg->n * 16, obuf, (size_t)ostride * 16,
+                           (size_t)nc * 16, (size_t)rows, cudaMemcpyDeviceToHost, st));
+      local.d2h_bytes += nc * rows * 16;
+    }
+    if (cfg->want_sum) {
+      // tallies are chained in chunk order so that the running sum is deterministic
+      if (ci > 0) CU(cudaStreamWaitEvent(st, rb.ev_done[s ^ 1], 0));
+      CU(ami::launch_block_sums(obuf, rows, nc, ostride, rb.partial, rb.sum, st, &launches));
+    }
+    CU(cudaEventRecord(rb.ev_done[s], st));
+    ++local.n_chunks;
+  }
+  for (int i = 0; i < 2; ++i) {
+    CU(cudaEventRecord(rb.ev_done[i], rb.st[i]));
+    CU(cudaStreamWaitEvent(user, rb.ev_done[i], 0));
+  }
+  if (cfg->want_sum) {
+    CU(cudaMemcpyAsync(cfg->h_sum, rb.sum, (size_t)rows * 16, cudaMemcpyDeviceToHost, user));
+    local.d2h_bytes += rows * 16;
+  }
+  CU(cudaEventRecord(rb.ev_stop, user));
+  CU(cudaEventSynchronize(rb.ev_stop));   // results in host buffers are complete on return
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, rb.ev_start, rb.ev_stop));
+  local.gpu_ms = ms;
+  local.kernel_launches = launches;
+  if (stats) *stats = local;
+  return AMI_OK;
+}

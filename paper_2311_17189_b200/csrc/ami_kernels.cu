@@ -1,0 +1,339 @@
+// CUDA kernels of the AMI hot path for sm_100a: dispersion (S1), leaf + term phases of the
+// evaluation (S2 + S3, flat plan), momentum generation and tallies for the streamed driver (S4).
+// One thread owns one sample; every table read is warp-uniform; per-sample leaf values live in
+// shared memory as [slot][thread] so that every access is conflict-free.
+#include <cstdio>
+
+#include "ami_device.cuh"
+#include "ami_kernels.cuh"
+
+namespace ami {
+using namespace amidev;
+
+// ------------------------------------------------------------------------------------------
+// S1: ami_dispersion.  K_i = sum_l alpha^i_l k_l + alpha^i_ext q ; e_i = 2t(cos Kx + cos Ky) + mu
+// (Eqs. 9-18).  The +-1/0 combinations are formed in registers: no matmul.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dispersion_kernel(DispParams p) {
+  __shared__ int8_t s_alpha[AMI_MAX_EPS * (AMI_MAX_INT + AMI_MAX_EXT)];
+  const int L = p.n_int + p.n_ext;
+  for (int i = threadIdx.x; i < p.n_eps * L; i += blockDim.x) s_alpha[i] = p.sym_alpha[i];
+  __syncthreads();
+  const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (s >= p.n) return;
+  double kx[AMI_MAX_INT], ky[AMI_MAX_INT];
+  const double* ks = p.k + s * p.k_stride_sample;
+#pragma unroll
+  for (int l = 0; l < AMI_MAX_INT; ++l) {
+    if (l < p.n_int) {
+      kx[l] = ks[(2 * l) * p.k_stride_comp];
+      ky[l] = ks[(2 * l + 1) * p.k_stride_comp];
+    }
+  }
+  for (int i = 0; i < p.n_eps; ++i) {
+    double Kx = 0.0, Ky = 0.0;
+#pragma unroll
+    for (int l = 0; l < AMI_MAX_INT; ++l) {
+      if (l < p.n_int) {
+        const double a = (double)s_alpha[i * L + l];
+        Kx = fma(a, kx[l], Kx);
+        Ky = fma(a, ky[l], Ky);
+      }
+    }
+    for (int x = 0; x < p.n_ext; ++x) {
+      const double a = (double)s_alpha[i * L + p.n_int + x];
+      Kx = fma(a, p.q[2 * x], Kx);
+      Ky = fma(a, p.q[2 * x + 1], Ky);
+    }
+    p.e[i * p.e_stride + s] = fma(2.0 * p.t, cos(Kx) + cos(Ky), p.mu);
+  }
+}
+
+cudaError_t launch_dispersion(const DispParams& p, cudaStream_t st) {
+  if (p.n == 0) return cudaSuccess;
+  const int nt = 256;
+  dispersion_kernel<<<(unsigned)((p.n + nt - 1) / nt), nt, 0, st>>>(p);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// S2 + S3, flat plan: leaves once per sample, then the term table term by term.
+// ------------------------------------------------------------------------------------------
+template <bool CE>
+__global__ void eval_flat_kernel(EvalParams p) {
+  extern __shared__ double sm[];
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const long long s_raw = blockIdx.x * (long long)nt + tid;
+  const long long s = s_raw < p.n_e ? s_raw : p.n_e - 1;
+  constexpr int W = CE ? 2 : 1;
+  double* sE = sm;                                   // [n_eps * W][nt]
+  double* sF = sE + (size_t)p.n_eps * W * nt;        // [U_F * W][nt]
+  double* sD = sF + (size_t)p.U_F * W * nt;          // [(U_D + 1) * 2][nt]
+  for (int i = 0; i < p.n_eps; ++i) {
+    if (CE) {
+      sE[(2 * i) * nt + tid] = p.e[2 * (i * p.e_stride + s)];
+      sE[(2 * i + 1) * nt + tid] = p.e[2 * (i * p.e_stride + s) + 1];
+    } else {
+      sE[i * nt + tid] = p.e[i * p.e_stride + s];
+    }
+  }
+  const int stride_t = p.m_f + p.n_d;
+  for (int b = 0; b < p.n_b; ++b) {
+    const double beta = p.beta[b];
+    // ---- Fermi/Bose leaves (independent of the external frequency) ----
+    for (int u = 0; u < p.U_F; ++u) {
+      const int j0 = p.leaf_ptr[u], j1 = p.leaf_ptr[u + 1];
+      const int sig = p.leafF_sig[u], k = p.leafF_k[u];
+      double Er = 0.0, Ei = 0.0;
+      for (int j = j0; j < j1; ++j) {
+        const int sy = p.leaf_sym[j];
+        const double c = (double)p.leaf_coef[j];
+        if (CE) {
+          Er = fma(c, sE[(2 * sy) * nt + tid], Er);
+          Ei = fma(c, sE[(2 * sy + 1) * nt + tid], Ei);
+        } else {
+          Er = fma(c, sE[sy * nt + tid], Er);
+        }
+      }
+      if (sig < 0) Er += p.e_reg;                    // P10(a)
+      if (CE) {
+        const cplx v = fermi_cplx(cplx{Er, Ei}, beta, sig, k, p.derivQ);
+        sF[(2 * u) * nt + tid] = v.re;
+        sF[(2 * u + 1) * nt + tid] = v.im;
+      } else {
+        sF[u * nt + tid] = fermi_real(Er, beta, sig, k, p.derivQ);
+      }
+    }
+    for (int f = 0; f < p.n_f; ++f) {
+      // ---- denominators: 1/(a . z + c . e), regulator rule P10(b) ----
+      for (int u = 0; u < p.U_D; ++u) {
+        const int j0 = p.leaf_ptr[p.U_F + u], j1 = p.leaf_ptr[p.U_F + u + 1];
+        double Dr = 0.0, Di = 0.0;
+        bool freq_zero = true;
+        for (int x = 0; x < p.n_ext; ++x) {
+          const int a = p.leafD_a[u * p.n_ext + x];
+          const double zr = p.z[2 * (f * p.n_ext + x)], zi = p.z[2 * (f * p.n_ext + x) + 1];
+          if (a != 0 && !(zr == 0.0 && zi == 0.0)) freq_zero = false;
+          Dr = fma((double)a, zr, Dr);
+          Di = fma((double)a, zi, Di);
+        }
+        for (int j = j0; j < j1; ++j) {
+          const int sy = p.leaf_sym[j];
+          const double c = (double)p.leaf_coef[j];
+          if (CE) {
+            Dr = fma(c, sE[(2 * sy) * nt + tid], Dr);
+            Di = fma(c, sE[(2 * sy + 1) * nt + tid], Di);
+          } else {
+            Dr = fma(c, sE[sy * nt + tid], Dr);
+          }
+        }
+        if (freq_zero) Dr += p.e_reg;
+        const cplx r = crcp(cplx{Dr, Di});
+        sD[(2 * u) * nt + tid] = r.re;
+        sD[(2 * u + 1) * nt + tid] = r.im;
+      }
+      sD[(2 * p.U_D) * nt + tid] = 1.0;              // unit leaf fills empty denominator slots
+      sD[(2 * p.U_D + 1) * nt + tid] = 0.0;
+      // ---- terms ----
+      double accr = 0.0, acci = 0.0;
+      for (long long t = 0; t < p.T; ++t) {
+        const uint16_t* ix = p.term_idx + t * stride_t;
+        cplx pr;
+        if (CE) {
+          pr = cplx{p.term_coef[t], 0.0};
+          for (int a = 0; a < p.m_f; ++a) {
+            const int u = ix[a];
+            pr = cmul(pr, cplx{sF[(2 * u) * nt + tid], sF[(2 * u + 1) * nt + tid]});
+          }
+        } else {
+          double pf = p.term_coef[t];
+          for (int a = 0; a < p.m_f; ++a) pf *= sF[ix[a] * nt + tid];
+          pr = cplx{pf, 0.0};
+        }
+        for (int d = 0; d < p.n_d; ++d) {
+          const int u = ix[p.m_f + d];
+          pr = cmul(pr, cplx{sD[(2 * u) * nt + tid], sD[(2 * u + 1) * nt + tid]});
+        }
+        accr += pr.re;
+        acci += pr.im;
+      }
+      if (s_raw < p.n_e) {
+        double2* o = reinterpret_cast<double2*>(p.out) +
+                     ((long long)(p.b0 + b) * p.n_f_total + (p.f0 + f)) * p.out_row_stride + s;
+        *o = make_double2(p.prefactor * accr, p.prefactor * acci);
+      }
+    }
+  }
+}
+
+static int pick_block(size_t bytes_per_thread, size_t fixed_bytes, size_t* smem_out) {
+  // largest block whose scratch fits in half of the SM's shared memory (two resident CTAs),
+  // falling back to one CTA per SM for large tables
+  const size_t half = 110 * 1024, full = 220 * 1024;
+  for (int nt : {256, 128, 64}) {
+    size_t need = bytes_per_thread * nt + fixed_bytes;
+    if (need <= half) { *smem_out = need; return nt; }
+  }
+  for (int nt : {128, 64, 32}) {
+    size_t need = bytes_per_thread * nt + fixed_bytes;
+    if (need <= full) { *smem_out = need; return nt; }
+  }
+  return 0;
+}
+
+cudaError_t launch_eval_flat(const EvalParams& p, bool ce, cudaStream_t st, int* launches) {
+  if (p.n_e == 0) return cudaSuccess;
+  const int W = ce ? 2 : 1;
+  const size_t per_thread = sizeof(double) * ((size_t)p.n_eps * W + (size_t)p.U_F * W + 2 * ((size_t)p.U_D + 1));
+  size_t smem = 0;
+  const int nt = pick_block(per_thread, 0, &smem);
+  if (!nt) return cudaErrorInvalidConfiguration;
+  auto kern = ce ? eval_flat_kernel<true> : eval_flat_kernel<false>;
+  cudaError_t rc = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (rc != cudaSuccess) return rc;
+  kern<<<(unsigned)((p.n_e + nt - 1) / nt), nt, smem, st>>>(p);
+  if (launches) ++*launches;
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// S4 helpers: counter-based momenta (reading P22) and deterministic tallies.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double uniform01(uint64_t seed, uint64_t ctr) {
+  uint64_t z = seed + 0x9E3779B97F4A7C15ull * (ctr + 1ull);
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  z = z ^ (z >> 31);
+  return (double)(z >> 11) * 0x1.0p-53;
+}
+
+__global__ void __launch_bounds__(256) momenta_kernel(uint64_t seed, long long first, long long n, int n_comp,
+                                                      double* __restrict__ k) {
+  const long long total = n * n_comp;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total;
+       i += (long long)gridDim.x * blockDim.x) {
+    const double u = uniform01(seed, (uint64_t)(first * n_comp + i));
+    k[i] = __dmul_rn(u - 0.5, 6.283185307179586);
+  }
+}
+
+cudaError_t launch_generate_momenta(uint64_t seed, long long first, long long n, int n_comp, double* d_k,
+                                    cudaStream_t st) {
+  if (n == 0) return cudaSuccess;
+  const long long total = n * n_comp;
+  long long blocks = (total + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  momenta_kernel<<<(unsigned)blocks, 256, 0, st>>>(seed, first, n, n_comp, d_k);
+  return cudaGetLastError();
+}
+
+// Per-row sums of complex values: fixed grid, fixed order -> deterministic.
+constexpr int kSumBlocks = 64;
+__global__ void __launch_bounds__(256) row_partial_kernel(const double2* __restrict__ v, long long n,
+                                                          long long row_stride, double2* __restrict__ partial) {
+  __shared__ double2 sh[256];
+  const long long row = blockIdx.y;
+  const double2* r = v + row * row_stride;
+  const long long per = (n + gridDim.x - 1) / gridDim.x;
+  const long long a = blockIdx.x * per, b = a + per < n ? a + per : n;
+  double2 acc = make_double2(0.0, 0.0);
+  for (long long i = a + threadIdx.x; i < b; i += blockDim.x) {
+    acc.x += r[i].x;
+    acc.y += r[i].y;
+  }
+  sh[threadIdx.x] = acc;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (threadIdx.x < w) {
+      sh[threadIdx.x].x += sh[threadIdx.x + w].x;
+      sh[threadIdx.x].y += sh[threadIdx.x + w].y;
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) partial[row * gridDim.x + blockIdx.x] = sh[0];
+}
+__global__ void row_final_kernel(const double2* __restrict__ partial, int n_partial, double2* __restrict__ sum) {
+  const long long row = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  (void)row;
+  const long long r = blockIdx.x;
+  if (threadIdx.x == 0) {
+    double2 acc = sum[r];
+    for (int i = 0; i < n_partial; ++i) {
+      acc.x += partial[r * n_partial + i].x;
+      acc.y += partial[r * n_partial + i].y;
+    }
+    sum[r] = acc;
+  }
+}
+
+cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long n, long long row_stride,
+                              double* d_partial, double* d_sum, cudaStream_t st, int* launches) {
+  if (n_rows == 0) return cudaSuccess;
+  dim3 grid(kSumBlocks, (unsigned)n_rows);
+  row_partial_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(d_vals), n, row_stride,
+                                           reinterpret_cast<double2*>(d_partial));
+  row_final_kernel<<<(unsigned)n_rows, 32, 0, st>>>(reinterpret_cast<const double2*>(d_partial), kSumBlocks,
+                                                    reinterpret_cast<double2*>(d_sum));
+  if (launches) *launches += 2;
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// FP64 pipe probe: independent DFMA chains held in registers.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters, double a, double b) {
+  double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6,
+         x7 = x0 + 7;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+  }
+  out[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
+cudaError_t run_fp64_probe(double* dfma_per_s, double* ms_out) {
+  cudaDeviceProp prop;
+  int dev = 0;
+  cudaError_t rc = cudaGetDevice(&dev);
+  if (rc != cudaSuccess) return rc;
+  rc = cudaGetDeviceProperties(&prop, dev);
+  if (rc != cudaSuccess) return rc;
+  const int blocks = prop.multiProcessorCount * 8, nt = 256, iters = 4096;
+  double* d = nullptr;
+  rc = cudaMalloc(&d, sizeof(double) * blocks * nt);
+  if (rc != cudaSuccess) return rc;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 6; ++rep) {
+    cudaEventRecord(e0);
+    dfma_probe_kernel<<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
+    cudaEventRecord(e1);
+    rc = cudaEventSynchronize(e1);
+    if (rc != cudaSuccess) break;
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep >= 2 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d);
+  if (rc != cudaSuccess) return rc;
+  const double ops = (double)blocks * nt * (double)iters * 64.0;
+  *dfma_per_s = ops / (best * 1e-3);
+  *ms_out = best;
+  return cudaSuccess;
+}
+
+}  // namespace ami
+
+namespace ami {
+// tree plan: see ami_eval_tree.cu (until the plan exists for a table the flat kernel runs)
+cudaError_t launch_eval_tree(const EvalParams& p, bool ce, cudaStream_t st, int* launches) {
+  return launch_eval_flat(p, ce, st, launches);
+}
+}  // namespace ami

@@ -1,0 +1,59 @@
+// Kernel parameter blocks and launcher declarations (internal).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "ami_table.hpp"
+
+namespace ami {
+
+constexpr int kMaxFreqWords = 64;   // n_f * n_ext complex values per launch
+constexpr int kMaxBeta = 8;         // inverse temperatures per launch
+
+struct EvalParams {
+  // table (device pointers)
+  const int32_t* leaf_ptr;
+  const int8_t* leaf_sym;
+  const int8_t* leaf_coef;
+  const int8_t* leafF_sig;
+  const int8_t* leafF_k;
+  const int8_t* leafD_a;
+  const uint16_t* term_idx;
+  const double* term_coef;
+  const uint32_t* tree_code;
+  const double* tree_consts;
+  const double* derivQ;
+  int n_eps, n_ext, U_F, U_D, m_f, n_d;
+  long long T;
+  // batch
+  const double* e;          // [n_eps][n_e] (complex: interleaved)
+  double* out;              // complex128, row r = b * n_f_total + f at out + 2 * r * out_row_stride
+  long long n_e, e_stride, out_row_stride;
+  int n_f, n_b, n_f_total, f0, b0;
+  double e_reg, prefactor;
+  double beta[kMaxBeta];
+  double z[2 * kMaxFreqWords];  // [n_f][n_ext] complex
+};
+
+struct DispParams {
+  const int8_t* sym_alpha;   // [n_eps][L]
+  int n_int, n_ext, n_eps;
+  const double* k;
+  long long k_stride_sample, k_stride_comp, n;
+  double q[2 * AMI_MAX_EXT];
+  double t, mu;
+  double* e;                 // [n_eps][n]
+  long long e_stride;
+};
+
+cudaError_t launch_dispersion(const DispParams& p, cudaStream_t st);
+cudaError_t launch_eval_flat(const EvalParams& p, bool e_is_complex, cudaStream_t st, int* launches);
+cudaError_t launch_eval_tree(const EvalParams& p, bool e_is_complex, cudaStream_t st, int* launches);
+cudaError_t launch_generate_momenta(uint64_t seed, long long first, long long n, int n_comp, double* d_k,
+                                    cudaStream_t st);
+cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long n, long long row_stride,
+                              double* d_partial, double* d_sum, cudaStream_t st, int* launches);
+cudaError_t run_fp64_probe(double* dfma_per_s, double* ms);
+
+}  // namespace ami

@@ -1,0 +1,230 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the CPU oracle on the same seeded
+inputs, element by element (norm: tests/parity.py, reading P20)."""
+import math
+
+import numpy as np
+import pytest
+
+import ami_inputs as A
+from parity import check_parity
+
+pytestmark = pytest.mark.gpu
+
+PLANS = {"flat": 1, "auto": 0}
+
+
+@pytest.fixture(scope="module")
+def ami():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2311_17189_b200 import build
+    build.build()
+    import paper_2311_17189_b200 as pkg
+    pkg.lib()  # raises if the extension is missing: no fallback
+    return pkg
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+    return torch
+
+
+def gpu_energies(torch, tab, cfg, k_host):
+    k = torch.from_numpy(np.ascontiguousarray(k_host)).cuda()
+    return tab.dispersion(k, [cfg.q], cfg.t, cfg.mu)
+
+
+def truth_for(oracle_mod, cfg, e_rows, z, beta, e_reg, quad=True):
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    return ot.evaluate(e_rows, z, beta, e_reg=e_reg, quad=quad, threads=oracle_mod.hardware_threads(), want_S=True)
+
+
+# ------------------------------------------------------------------ S1 dispersion
+@pytest.mark.parametrize("name,n", [("cfg1", 10_000), ("cfg3", 4133), ("cfg4", 1000), ("cfg5", 777)])
+def test_dispersion_parity(ami, torch_mod, oracle_mod, name, n):
+    cfg = A.get_config(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    k = cfg.momenta(n)
+    e = gpu_energies(torch_mod, tab, cfg, k).cpu().numpy()
+    want = oracle_mod.OracleTable.from_diagram(cfg.diagram).dispersion(k, [cfg.q], cfg.t, cfg.mu, quad=True)
+    assert e.shape == (cfg.diagram.n_eps, n)
+    # |e| <= 4t + |mu|; K is a sum of up to m+1 doubles of size pi, so a few ulp of 4*pi in the angle
+    np.testing.assert_allclose(e.T, want, rtol=0, atol=2e-14)
+
+
+def test_dispersion_soa_layout(ami, torch_mod):
+    """SoA momenta [2m][N] through the stride arguments of the ABI."""
+    import ctypes as C
+    cfg = A.get_config("cfg3")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    k = torch_mod.from_numpy(cfg.momenta(1000)).cuda()
+    ref = tab.dispersion(k, [cfg.q], cfg.t, cfg.mu)
+    ksoa = k.reshape(1000, -1).t().contiguous()
+    out = torch_mod.empty_like(ref)
+    q = np.array(cfg.q)
+    rc = ami.lib().ami_dispersion(tab._h, C.c_void_p(ksoa.data_ptr()), 1, 1000, q.ctypes.data, cfg.t, cfg.mu, 1000,
+                                  C.c_void_p(out.data_ptr()), C.c_void_p(torch_mod.cuda.current_stream().cuda_stream))
+    assert rc == 0
+    torch_mod.cuda.synchronize()
+    assert torch_mod.equal(out, ref)
+
+
+# ------------------------------------------------------------------ S2 + S3 evaluate
+def run_eval_case(ami, torch, oracle_mod, cfg, n, plan, betas=None, z=None, n_truth=None, start=0):
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    k = cfg.momenta(n, start=start)
+    e_dev = gpu_energies(torch, tab, cfg, k)
+    betas = cfg.betas if betas is None else betas
+    z = cfg.z_ext if z is None else z
+    out = tab.evaluate(e_dev, z, betas, e_reg=cfg.e_reg, plan=plan).cpu().numpy()
+    assert out.shape == (len(betas), len(z), n)
+    e_rows = e_dev.cpu().numpy().T.copy()
+    sel = np.arange(n) if n_truth is None or n_truth >= n else np.linspace(0, n - 1, n_truth).astype(np.int64)
+    stats = []
+    for b, beta in enumerate(betas):
+        truth, S = truth_for(oracle_mod, cfg, e_rows[sel], z, beta, cfg.e_reg)
+        stats.append(check_parity(out[b][:, sel], truth, S, label=f"{cfg.name} beta={beta}"))
+    return stats
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+def test_cfg1_order2(ami, torch_mod, oracle_mod, plan):
+    run_eval_case(ami, torch_mod, oracle_mod, A.get_config("cfg1"), 10_000, PLANS[plan])
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+@pytest.mark.parametrize("mu,beta", [(0.0, 2.0), (-0.5, 5.0), (0.0, 10.0)])
+@pytest.mark.parametrize("name", ["cfg2_se", "cfg2_bubble", "cfg2_bubble_doubled"])
+def test_cfg2_sweep_points(ami, torch_mod, oracle_mod, name, mu, beta, plan):
+    """8 frequencies; the bosonic n = 0 case goes through the regulator rule P10(b)."""
+    cfg = A.get_config(name, mu=mu, beta=beta)
+    run_eval_case(ami, torch_mod, oracle_mod, cfg, 5000 + 37, PLANS[plan])
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+def test_cfg3_order4(ami, torch_mod, oracle_mod, plan):
+    st = run_eval_case(ami, torch_mod, oracle_mod, A.get_config("cfg3"), 20_000 + 11, PLANS[plan])
+    assert st[0]["n_nonfinite"] == 0
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+def test_cfg4_order6(ami, torch_mod, oracle_mod, plan):
+    run_eval_case(ami, torch_mod, oracle_mod, A.get_config("cfg4"), 4096 + 5, PLANS[plan], n_truth=1500)
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+def test_cfg5_grid(ami, torch_mod, oracle_mod, plan):
+    """64 continued frequencies x 4 temperatures (launch splitting over frequencies)."""
+    run_eval_case(ami, torch_mod, oracle_mod, A.get_config("cfg5"), 600 + 3, PLANS[plan], n_truth=150)
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+def test_complex_energies_variant_5b(ami, torch_mod, oracle_mod, plan):
+    """P19: complex energies e_j - i gamma_j make the Fermi/Bose arguments complex."""
+    cfg = A.get_config("cfg5")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    n = 500
+    e_real = gpu_energies(torch_mod, tab, cfg, cfg.momenta(n)).cpu().numpy()
+    gam = A.uniform01(99, np.arange(e_real.size, dtype=np.uint64)).reshape(e_real.shape) * 0.05
+    e_c = e_real - 1j * gam
+    z = cfg.z_ext[::8]
+    out = tab.evaluate(torch_mod.from_numpy(e_c).cuda(), z, [5.0], plan=PLANS[plan]).cpu().numpy()
+    truth, S = truth_for(oracle_mod, cfg, e_c.T.copy(), z, 5.0, 0.0)
+    check_parity(out[0], truth, S, label="5b")
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+def test_stress8_large_table(ami, torch_mod, oracle_mod, plan):
+    """Order 8, 4e4 terms: the table is far larger than any on-chip staging tile."""
+    cfg = A.get_config("stress8")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    n = 96 + 7
+    e_dev = gpu_energies(torch_mod, tab, cfg, cfg.momenta(n))
+    out = tab.evaluate(e_dev, cfg.z_ext, cfg.betas, plan=PLANS[plan]).cpu().numpy()
+    truth, S = truth_for(oracle_mod, cfg, e_dev.cpu().numpy().T.copy(), cfg.z_ext, cfg.betas[0], 0.0, quad=False)
+    # double oracle as truth here (quad is too slow for 4e4 terms): 1e-10 * S still holds
+    check_parity(out[0], truth, S, label="stress8")
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 32, 33, 257])
+def test_edge_sizes(ami, torch_mod, oracle_mod, n):
+    cfg = A.get_config("cfg3")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    e = torch_mod.zeros((cfg.diagram.n_eps, n), dtype=torch_mod.float64, device="cuda")
+    if n:
+        e = gpu_energies(torch_mod, tab, cfg, cfg.momenta(n))
+    out = tab.evaluate(e, cfg.z_ext, cfg.betas)
+    assert out.shape == (1, 1, n)
+    if n:
+        truth, S = truth_for(oracle_mod, cfg, e.cpu().numpy().T.copy(), cfg.z_ext, cfg.betas[0], 0.0)
+        check_parity(out.cpu().numpy()[0], truth, S)
+
+
+def test_degenerate_samples_nonfinite_agree(ami, torch_mod, oracle_mod):
+    """Exactly degenerate bubble at Omega = 0 without regulator: 0/0 on both sides; with the
+    regulator both are finite and agree."""
+    cfg = A.get_config("cfg2_bubble")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    e_rows = np.array([[0.3, -0.7], [0.5, 0.5], [1.25, 1.25], [-0.2, 0.9]])
+    e_dev = torch_mod.from_numpy(e_rows.T.copy()).cuda()
+    z = np.array([[0j], [2j * math.pi / 5.0]])
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    for eta in (0.0, 1e-8):
+        out = tab.evaluate(e_dev, z, [5.0], e_reg=eta).cpu().numpy()
+        truth, S = ot.evaluate(e_rows, z, 5.0, e_reg=eta, quad=True, want_S=True)
+        check_parity(out[0], truth, S, label=f"eta={eta}")
+        assert np.isfinite(out[0][1]).all()
+        assert np.isfinite(out[0][0]).all() == (eta > 0)
+
+
+# ------------------------------------------------------------------ S4 streamed driver
+def test_generated_momenta_bitwise(ami, torch_mod):
+    """P22: device generator == host generator, bit for bit."""
+    cfg = A.get_config("cfg4")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    k = tab.generate_momenta(cfg.seed, 12345, 5000).cpu().numpy()
+    np.testing.assert_array_equal(k, cfg.momenta(5000, start=12345))
+
+
+@pytest.mark.parametrize("mode", ["generated", "host", "device"])
+def test_run_streamed_matches_stagewise(ami, torch_mod, oracle_mod, mode):
+    cfg = A.get_config("cfg3")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    n, chunk = 10_000 + 77, 3000   # 4 chunks, ragged tail
+    k_host = cfg.momenta(n)
+    ref = tab.evaluate(gpu_energies(torch_mod, tab, cfg, k_host), cfg.z_ext, cfg.betas)
+    h_out = torch_mod.empty((1, 1, n), dtype=torch_mod.complex128).pin_memory()
+    kw = {}
+    if mode == "host":
+        kw["h_k"] = torch_mod.from_numpy(k_host).pin_memory()
+    elif mode == "device":
+        kw["d_k"] = torch_mod.from_numpy(k_host).cuda()
+    stats, sums = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, chunk=chunk,
+                          h_out=h_out, want_sum=True, **kw)
+    assert stats["n_chunks"] == 4 and stats["kernel_launches"] >= 8
+    assert stats["d2h_bytes"] == n * 16 + 16
+    assert stats["h2d_bytes"] == (n * 8 * 8 if mode == "host" else 0)
+    np.testing.assert_array_equal(h_out.numpy(), ref.cpu().numpy())   # same kernels, same inputs
+    total = ref.cpu().numpy().sum()
+    assert abs(sums[0, 0] - total) <= 1e-12 * np.abs(ref.cpu().numpy()).sum()
+    # and against the oracle end to end on a subset
+    sel = np.arange(0, n, 97)
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    e_rows = ot.dispersion(k_host[sel], [cfg.q], cfg.t, cfg.mu)
+    truth, S = ot.evaluate(e_rows, cfg.z_ext, cfg.betas[0], quad=True, want_S=True)
+    check_parity(h_out.numpy()[0][:, sel], truth, S, label="run")
+
+
+def test_run_device_output_and_determinism(ami, torch_mod):
+    cfg = A.get_config("cfg1")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    n = 10_000
+    d_out = torch_mod.empty((1, 1, n), dtype=torch_mod.complex128, device="cuda")
+    s1, sum1 = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, chunk=1024, d_out=d_out,
+                       want_sum=True)
+    first = d_out.clone()
+    s2, sum2 = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, chunk=1024, d_out=d_out,
+                       want_sum=True)
+    assert torch_mod.equal(first, d_out) and sum1[0, 0] == sum2[0, 0]   # deterministic tallies
+    assert s1["n_chunks"] == 10

@@ -1,0 +1,141 @@
+"""CPU-only tests of the product's host logic: the C-ABI library loads and exports every symbol
+include/ami.h declares, ami_construct builds tables whose VALUES (not shape: tables are not
+unique, reading P14) agree with the oracle, error codes, and no compute without a device."""
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+import ami_inputs as A
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def ami():
+    from paper_2311_17189_b200 import build
+    build.build()
+    import paper_2311_17189_b200 as pkg
+    return pkg
+
+
+def test_library_exports_every_declared_symbol(ami):
+    header = open(os.path.join(ROOT, "include", "ami.h")).read()
+    declared = set(re.findall(r"^\s*(?:int|void|const char\*)\s+(ami_\w+)\s*\(", header, flags=re.M))
+    assert declared == set(ami.EXPORTS), declared ^ set(ami.EXPORTS)
+    L = ami.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    assert L.ami_version() >= 1
+
+
+def numpy_eval_export(tab, e, z, beta, prefactor=1.0):
+    """Evaluates an exported flat table with numpy (test-side restatement of the layout documented
+    in include/ami.h; real energies, derivative order <= 1)."""
+    def f_sig(E, sig):
+        return 1.0 / (sig * np.exp(beta * E) + 1.0)
+
+    F = []
+    for c, sig, k in zip(tab["leafF_c"], tab["leafF_sig"], tab["leafF_k"]):
+        E = e @ c
+        f = f_sig(E, sig)
+        F.append(f if k == 0 else -beta * f * (1 - f))
+        assert k <= 1
+    D = [1.0 / (e @ c + a @ z) for c, a in zip(tab["leafD_c"], tab["leafD_a"])]
+    total = np.zeros(e.shape[0], dtype=complex)
+    for fi, di, co in zip(tab["fidx"], tab["didx"], tab["coef"]):
+        term = np.full(e.shape[0], co, dtype=complex)
+        for u in fi:
+            term = term * F[u]
+        for u in di:
+            if u >= 0:
+                term = term * D[u]
+        total += term
+    return prefactor * total
+
+
+DIAGRAMS = {
+    "order1": A.order1_line, "bubble": A.bubble, "bubble_doubled": A.doubled_line_bubble,
+    "se2": A.self_energy_order2, "se2_doubled1": lambda: A.self_energy_order2_doubled(1),
+    "se3": lambda: A.random_self_energy(3, 1), "cfg3": lambda: A.get_config("cfg3").diagram,
+    "se4_b": lambda: A.random_self_energy(4, 0), "cfg5": lambda: A.get_config("cfg5").diagram,
+    "cfg4": lambda: A.get_config("cfg4").diagram,
+}
+
+
+@pytest.mark.parametrize("name", list(DIAGRAMS))
+def test_construct_values_match_oracle(ami, oracle_mod, name):
+    d = DIAGRAMS[name]()
+    tab = ami.AmiTable.from_diagram(d, device=None, prefactor=-2.0)
+    ex = tab.export()
+    assert ex["fidx"].shape[1] == d.n_int
+    rng = np.random.default_rng(3)
+    e = rng.uniform(-1.5, 1.5, size=(24, d.n_eps))
+    beta = 2.0
+    z = np.array([1j * math.pi / beta if d.slot_is_fermionic[-1] else 2j * math.pi / beta])
+    got = numpy_eval_export(ex, e, z, beta, prefactor=-2.0)
+    want, S = oracle_mod.OracleTable.from_diagram(d, prefactor=-2.0).evaluate(e, [z], beta, quad=True, want_S=True)
+    assert np.max(np.abs(got - want[0]) / S[0]) < 1e-12
+    info = tab.info
+    assert info["n_terms"] == len(ex["coef"]) and info["has_device_copy"] == 0
+    assert info["n_terms"] <= info["n_terms_raw"]
+
+
+def test_construct_sum_order_and_errors(ami, oracle_mod):
+    d = A.random_self_energy(4, 1)
+    rng = np.random.default_rng(5)
+    e = rng.uniform(-1.5, 1.5, size=(16, d.n_eps))
+    beta, z = 2.0, np.array([1j * math.pi / 2.0])
+    ref = numpy_eval_export(ami.AmiTable.from_diagram(d, device=None).export(), e, z, beta)
+    n_ok = 0
+    for so in ([3, 2, 1, 0], [1, 3, 0, 2], [2, 0, 3, 1]):
+        try:
+            t = ami.AmiTable.from_diagram(d, device=None, sum_order=so)
+        except ami.AmiError as ex:
+            assert ex.code == -2
+            with pytest.raises(oracle_mod.OracleError):  # the oracle rejects the same order
+                oracle_mod.OracleTable.from_diagram(d, sum_order=so)
+            continue
+        np.testing.assert_allclose(numpy_eval_export(t.export(), e, z, beta), ref, rtol=1e-9)
+        n_ok += 1
+    assert n_ok >= 1
+    o1 = A.order1_line()
+    with pytest.raises(ami.AmiError) as ei:
+        ami.AmiTable(1, 1, [[2, 0]], o1.eps, o1.slot_is_fermionic, device=None)
+    assert ei.value.code == -2
+    with pytest.raises(ami.AmiError) as ei:
+        ami.AmiTable(2, 1, [[1, 0, 0]], o1.eps, [1, 1, 1], device=None)
+    assert ei.value.code == -3
+    with pytest.raises(ami.AmiError) as ei:
+        ami.AmiTable(1, 1, [[1, 0]], o1.eps, [0, 1], device=None)  # bosonic internal sum
+    assert ei.value.code == -1
+    with pytest.raises(ami.AmiError) as ei:
+        ami.AmiTable(2, 1, [[1, 0, 0], [0, 1, 0]], np.eye(2, dtype=np.int32), [1, 1, 1], sum_order=[0, 0], device=None)
+    assert ei.value.code == -1
+
+
+def test_no_cpu_fallback(ami):
+    """A host-only table cannot be evaluated: every kernel entry point refuses (AMI_ECUDA)."""
+    import ctypes as C
+    tab = ami.AmiTable.from_diagram(A.self_energy_order2(), device=None)
+    L = ami.lib()
+    buf = np.zeros(64)
+    z = np.zeros(2)
+    b = np.ones(1)
+    rc = L.ami_evaluate(tab._h, buf.ctypes.data, 0, 1, z.ctypes.data, 1, b.ctypes.data, 1, 0.0, 0,
+                        buf.ctypes.data, None)
+    assert rc == -4
+    rc = L.ami_dispersion(tab._h, buf.ctypes.data, 4, 1, z.ctypes.data, 1.0, 0.0, 1, buf.ctypes.data, None)
+    assert rc == -4
+    assert b"no device copy" in L.ami_last_cuda_error()
+    assert L.ami_strerror(-2).startswith(b"|alpha_p|")
+
+
+def test_merging_and_sign_canonical_denominators(ami):
+    ex = ami.AmiTable.from_diagram(A.self_energy_order2(), device=None).export()
+    # the four flat terms of the order-2 self-energy share ONE denominator up to sign
+    assert ex["leafD_c"].shape[0] == 1 and len(ex["coef"]) == 4
+    first = [next(v for v in np.concatenate([a, c]) if v != 0) for a, c in zip(ex["leafD_a"], ex["leafD_c"])]
+    assert all(v > 0 for v in first)
