@@ -70,7 +70,7 @@ enum {
 typedef struct ami_info {
   int32_t n_int, n_ext, n_g, n_eps;
   int32_t n_fermi_leaves;   /* U_F: distinct (energy combination, sigma, derivative order) */
-  int32_t n_den_leaves;     /* U_D: distinct denominators (sign-canonical), excluding the unit leaf */
+  int32_t n_den_leaves;     /* U_D: distinct denominators (oriented as produced, P10), excluding the unit leaf */
   int32_t max_deriv;        /* highest derivative order in the table */
   int32_t max_den_per_term; /* denominators per term (powers count as repeats) */
   int64_t n_terms;          /* T_flat after merging identical terms */

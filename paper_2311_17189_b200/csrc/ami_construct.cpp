@@ -9,7 +9,9 @@
 // (Q: the lines sharing the pole, s_Q = prod alpha_p over Q; Z: other lines that depend on nu_p;
 // C: lines that do not), using d^r/dz^r G = (-alpha)^r r! G^{r+1}.  The result is the
 // unfactorised term list of PAPER.md:100 (Eq. 6 with FT a plain product), merged and stored with
-// dictionaries of distinct Fermi/Bose leaves and distinct sign-canonical denominators.
+// dictionaries of distinct Fermi/Bose leaves and distinct denominators.  Denominators keep the
+// orientation in which the recursion produced them (D and -D are different leaves): the regulator
+// of reading P10 is added to D as it arises, and 1/(D+eta) != -1/(-D+eta).
 #include <algorithm>
 #include <map>
 #include <numeric>
@@ -192,14 +194,6 @@ int construct_flat(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alph
       for (int l = 0; l < n_int; ++l)
         if (g.a[l]) return AMI_EINVAL;        // cannot happen: every internal slot was summed
       LeafD key{std::vector<int>(g.a.begin() + n_int, g.a.end()), g.e};
-      int sign = 0;
-      for (int v : key.a) if (!sign && v) sign = v > 0 ? 1 : -1;
-      for (int v : key.c) if (!sign && v) sign = v > 0 ? 1 : -1;
-      if (sign < 0) {
-        for (int& v : key.a) v = -v;
-        for (int& v : key.c) v = -v;
-        num = -num;                            // 1/(-D) = -1/D
-      }
       auto it = dmap.find(key);
       if (it == dmap.end()) {
         it = dmap.emplace(key, (int)ft.leafD.size()).first;

@@ -20,7 +20,7 @@ struct LeafF {
     return c < o.c;
   }
 };
-// A distinct denominator  a . z_ext + c . e, sign-canonical (first non-zero entry positive)
+// A distinct denominator  a . z_ext + c . e, in the orientation the recursion produced (P10)
 struct LeafD {
   std::vector<int> a;   // [n_ext]
   std::vector<int> c;   // [n_eps]

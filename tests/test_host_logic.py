@@ -133,9 +133,10 @@ def test_no_cpu_fallback(ami):
     assert L.ami_strerror(-2).startswith(b"|alpha_p|")
 
 
-def test_merging_and_sign_canonical_denominators(ami):
+def test_denominators_keep_their_orientation(ami):
+    """The order-2 self-energy has one denominator up to sign; both orientations are kept as
+    separate leaves because the regulator is added to D as it arises (reading P10)."""
     ex = ami.AmiTable.from_diagram(A.self_energy_order2(), device=None).export()
-    # the four flat terms of the order-2 self-energy share ONE denominator up to sign
-    assert ex["leafD_c"].shape[0] == 1 and len(ex["coef"]) == 4
-    first = [next(v for v in np.concatenate([a, c]) if v != 0) for a, c in zip(ex["leafD_a"], ex["leafD_c"])]
-    assert all(v > 0 for v in first)
+    assert ex["leafD_c"].shape[0] == 2 and len(ex["coef"]) == 4
+    np.testing.assert_array_equal(ex["leafD_c"][0], -ex["leafD_c"][1])
+    np.testing.assert_array_equal(ex["leafD_a"][0], -ex["leafD_a"][1])
