@@ -1,0 +1,424 @@
+#!/usr/bin/env python
+"""bench.py -- the hot path of SURVEY.md section 8(a) timed on B200 (contract: see DESIGN.md "Measurement").
+
+One step = one pass of the whole hot path over one batch of synthetic input with the momenta already
+resident in HBM: S1 ami_dispersion (momenta -> line energies) then S2+S3 ami_evaluate (leaf phase + term
+phase), all through the C ABI of include/ami.h.  Prints ONE JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample of the
+same workload.  Nothing here reads /root/reference.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "ami_term_evaluations_per_s"
+UNIT = "term-evals/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg3", help="cfg1 | cfg2_se | cfg2_bubble | cfg3 | cfg4 | cfg5 | stress8")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=0, help="override samples per step per GPU")
+    ap.add_argument("--plan", default="auto", choices=["auto", "flat", "tree"])
+    ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads and the CPU baseline")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks: sampled DURING the timed region
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    BAD = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown")
+
+    def __init__(self, index=0, period=0.05):
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.sm_max = None
+        self._stop = threading.Event()
+        self._th = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:  # noqa: BLE001
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:  # noqa: BLE001
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in names.items():
+                    if mask & bit:
+                        self.reasons.add(k)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._th = threading.Thread(target=self._loop, daemon=True)
+            self._th.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._th:
+            self._th.join()
+        med = int(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.sm_max, "reasons": sorted(self.reasons),
+                "n_samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------
+# algorithmic FP64 work:
+#   W = 2 N_eps c_cos [S1] + N_b U_F (c_exp + c_rcp + 4) [Fermi/Bose] + N_f U_D (c_rcp + 8) [reciprocals]
+#       + N_f N_b * (term-loop FP64 instructions of the representation executed)
+# c_* = FP64-pipe instructions of one double cos / exp / reciprocal as compiled for sm_100a (counted
+# in the SASS of this library, DESIGN.md table "leaf costs").
+# ------------------------------------------------------------------------------------------------
+C_COS, C_EXP, C_RCP = 38, 23, 6
+
+
+def fp64_work_per_sample(info, n_f, n_b, plan_ops):
+    disp = 2 * info["n_eps"] * C_COS
+    fermi = n_b * info["n_fermi_leaves"] * (C_EXP + C_RCP + 4)
+    dens = n_f * info["n_den_leaves"] * (C_RCP + 8)
+    terms = n_f * n_b * plan_ops
+    return {"dispersion": disp, "evaluate": fermi + dens + terms, "fermi": fermi, "denominators": dens,
+            "terms": terms}
+
+
+def load_measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def dist_setup(args):
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        backend = "gloo" if args.impl == "reference" else "nccl"
+        if args.impl != "reference":
+            import torch
+            torch.cuda.set_device(local)
+        dist_mod.init_process_group(backend=backend, rank=rank, world_size=world)
+        dist = dist_mod
+    return dist, rank, local, world
+
+
+def samples_per_step(cfg, args):
+    return args.n if args.n > 0 else cfg.n_samples
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on the host cores
+# ------------------------------------------------------------------------------------------------
+def oracle_rate(cfg, n_sample, threads):
+    """term-evaluations/s of the double-precision oracle over n_sample samples of the workload
+    (dispersion + evaluate for every beta and frequency), and the seconds it took."""
+    import oracle
+    ot = oracle.OracleTable.from_diagram(cfg.diagram)
+    T = ot.info()["T"]
+    k = cfg.momenta(n_sample)
+    t0 = time.perf_counter()
+    e = ot.dispersion(k, [cfg.q], cfg.t, cfg.mu, threads=threads)
+    for beta in cfg.betas:
+        ot.evaluate(e, cfg.z_ext, beta, e_reg=cfg.e_reg, quad=False, threads=threads)
+    dt = time.perf_counter() - t0
+    units = n_sample * len(cfg.betas) * len(cfg.z_ext)
+    return T, units, dt
+
+
+def oracle_sample_size(cfg, threads, seconds):
+    """Calibrates on a small sample so that one timed pass takes about `seconds`."""
+    n0 = 4096
+    _, units, dt = oracle_rate(cfg, n0, threads)
+    per_sample = max(dt / n0, 1e-9)
+    return int(max(n0, min(cfg.n_samples, seconds / per_sample)))
+
+
+def run_reference(args, dist, rank, world):
+    import ami_inputs as A
+    import oracle
+    if rank != 0:
+        return
+    cfg = A.get_config(args.workload)
+    threads = oracle.hardware_threads()
+    n_s = oracle_sample_size(cfg, threads, min(args.cpu_seconds, 180.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_rate(cfg, max(4096, n_s // 8), threads)
+    tot_units, tot_dt, T = 0, 0.0, 0
+    for _ in range(args.steps):
+        T, units, dt = oracle_rate(cfg, n_s, threads)
+        tot_units += units
+        tot_dt += dt
+    value = T * tot_units / tot_dt
+    sample = f"{n_s} of {cfg.n_samples} samples x {len(cfg.z_ext)} freq x {len(cfg.betas)} beta per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "samples_per_s": tot_units / tot_dt,
+        "config": {"workload": cfg.name, "T_flat": T, "sample": sample, "precision": "double"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm: the CUDA path through the C ABI
+# ------------------------------------------------------------------------------------------------
+def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, sample_clocks):
+    """Times `steps` passes of S1 + S2/S3 over rotating resident momentum batches (the set of inputs is
+    larger than L2, so no batch is served from cache).  Returns a dict of device-timed results."""
+    from paper_2311_17189_b200 import sharding
+    tab = pkg.AmiTable.from_diagram(cfg.diagram, device=torch.cuda.current_device())
+    info = tab.info
+    m, n_eps = cfg.diagram.n_int, cfg.diagram.n_eps
+    n_f, n_b = len(cfg.z_ext), len(cfg.betas)
+    bytes_in = n * 2 * m * 8
+    n_rot = int(max(2, min(8, -(-300_000_000 // max(bytes_in + n * n_eps * 8, 1)))))
+    ks = [tab.generate_momenta(cfg.seed, first_sample + r * n, n) for r in range(n_rot)]
+    es = [torch.empty((n_eps, n), dtype=torch.float64, device="cuda") for _ in range(n_rot)]
+    out = torch.empty((n_b, n_f, n), dtype=torch.complex128, device="cuda")
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def step(i, events=None):
+        r = i % n_rot
+        if events:
+            events[0].record()
+        tab.dispersion(ks[r], [cfg.q], cfg.t, cfg.mu, out=es[r])
+        if events:
+            events[1].record()
+        tab.evaluate(es[r], cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan, out=out)
+        if events:
+            events[2].record()
+
+    for i in range(warmup):
+        step(i)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(torch.cuda.current_device()) if sample_clocks else None
+    if sampler:
+        sampler.start()
+    l0 = pkg.kernel_launches()
+    t_beg.record()
+    for i in range(steps):
+        step(warmup + i, ev[i])
+    t_end.record()
+    torch.cuda.synchronize()
+    launches = pkg.kernel_launches() - l0
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+    total_ms = sharding.max_over_ranks(t_beg.elapsed_time(t_end), dist)
+    disp_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    eval_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
+    checksum = complex(out[0, 0, : min(n, 1024)].sum().item())
+    return {"tab": tab, "info": info, "total_ms": total_ms, "disp_ms": disp_ms, "eval_ms": eval_ms,
+            "launches": launches, "clocks": clocks, "n_rot": n_rot, "checksum": checksum,
+            "bytes_in": bytes_in, "bytes_e": n * n_eps * 8, "bytes_out": n * n_f * n_b * 16}
+
+
+def time_e2e(pkg, torch, tab, cfg, n, steps, warmup, plan, first_sample, dist):
+    """Same metric through ami_run with HOST buffers: pinned momenta in, pinned complex128 results
+    out, every step; host<->device copies are inside the timed region."""
+    from paper_2311_17189_b200 import sharding
+    m = cfg.diagram.n_int
+    n_f, n_b = len(cfg.z_ext), len(cfg.betas)
+    h_k = torch.from_numpy(cfg.momenta(n, start=first_sample).reshape(n, 2 * m)).pin_memory()
+    h_out = torch.empty((n_b, n_f, n), dtype=torch.complex128).pin_memory()
+    stats = None
+    for _ in range(max(1, warmup)):
+        stats, _ = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan, h_k=h_k,
+                           h_out=h_out)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        stats, _ = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan, h_k=h_k,
+                           h_out=h_out)
+    torch.cuda.synchronize()
+    dt = sharding.max_over_ranks(time.perf_counter() - t0, dist)
+    return {"seconds": dt, "h2d": int(stats["h2d_bytes"]), "d2h": int(stats["d2h_bytes"]),
+            "chunks": int(stats["n_chunks"]), "launches_per_step": int(stats["kernel_launches"]),
+            "finite": bool(torch.isfinite(torch.view_as_real(h_out[0, 0, :1024])).all().item())}
+
+
+def roofline_objects(res, n, n_f, n_b, plan_ops, peaks, dfma_per_s):
+    """Roofline of the dominant kernel (ami_evaluate): FP64-pipe bound.  Work counted in FP64-pipe
+    instruction slots per sample, expressed as DFMA-equivalent TFLOP/s (slot = 2 flop)
+    against the DFMA-chain rate measured in this run; the HBM leg is reported beside it."""
+    w = fp64_work_per_sample(res["info"], n_f, n_b, plan_ops)
+    t_eval = res["eval_ms"] * 1e-3
+    t_disp = res["disp_ms"] * 1e-3
+    peak_tf = 2.0 * dfma_per_s / 1e12
+    ach = 2.0 * w["evaluate"] * n / t_eval / 1e12
+    eval_bytes = res["bytes_e"] + res["bytes_out"]
+    disp_bytes = res["bytes_in"] + res["bytes_e"]
+    roof = {"bound": "alu", "kernel": "ami_evaluate", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
+            "frac": ach / peak_tf, "traffic": None,
+            "peak_source": "DFMA-chain probe run by this bench (FP64 pipe; MEASURED_PEAKS.json has no FP64 figure)",
+            "flop_convention": "FP64-pipe instruction slots x 2",
+            "fp64_slots_per_sample": w,
+            "hbm_leg": {"algorithmic_bytes": eval_bytes, "achieved_gbs": eval_bytes / t_eval / 1e9,
+                        "peak_gbs": peaks["hbm_gbs"], "frac": eval_bytes / t_eval / 1e9 / peaks["hbm_gbs"],
+                        "peak_source": peaks["source"]}}
+    disp = {"kernel": "ami_dispersion", "ms": res["disp_ms"],
+            "alu_frac": 2.0 * w["dispersion"] * n / t_disp / 1e12 / peak_tf,
+            "hbm_frac": disp_bytes / t_disp / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": disp_bytes}
+    return roof, disp
+
+
+PLAN_IDS = {"auto": 0, "flat": 1, "tree": 2}
+
+
+def plan_ops_for(info, plan):
+    """Term-loop FP64 slots per (sample, frequency, beta) of the representation ami_evaluate executes."""
+    if plan != "flat" and info.get("fp64_ops_tree", 0) > 0:
+        return int(info["fp64_ops_tree"]), "tree"
+    return int(info["fp64_ops_flat"]), "flat"
+
+
+def run_ours(args, dist, rank, local, world):
+    import torch
+    import ami_inputs as A
+    import paper_2311_17189_b200 as pkg
+    from paper_2311_17189_b200 import sharding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    pkg.lib()   # raises if libami_b200.so has not been built
+    cfg = A.get_config(args.workload)
+    n = samples_per_step(cfg, args)
+    first, _ = sharding.weak_range(n, rank, world)
+    n_f, n_b = len(cfg.z_ext), len(cfg.betas)
+    plan = PLAN_IDS[args.plan]
+    dfma_per_s, _ = pkg.fp64_peak_probe(local)
+    peaks = load_measured_peaks()
+
+    res = time_workload(pkg, torch, cfg, n, args.steps, args.warmup, plan, first, dist, sample_clocks=True)
+    info = res["info"]
+    T = int(info["n_terms"])
+    plan_ops, plan_name = plan_ops_for(info, args.plan)
+    units_per_step = n * n_f * n_b * world
+    ms_per_step = res["total_ms"] / args.steps
+    value = T * units_per_step / (ms_per_step * 1e-3)
+    roof, disp = roofline_objects(res, n, n_f, n_b, plan_ops, peaks, dfma_per_s)
+    e2e = time_e2e(pkg, torch, res["tab"], cfg, n, max(2, args.steps // 4), 1, plan, first, dist)
+    e2e_steps = max(2, args.steps // 4)
+    e2e_value = T * units_per_step * e2e_steps / e2e["seconds"]
+    launches = int(sharding.sum_over_ranks([res["launches"]], dist)[0])
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "samples_per_s": units_per_step / (ms_per_step * 1e-3),
+        "config": {"workload": cfg.name, "order": cfg.diagram.n_int, "n_green": cfg.diagram.n_g,
+                   "samples_per_gpu": n, "n_freq": n_f, "n_beta": n_b, "T_flat": T,
+                   "U_F": int(info["n_fermi_leaves"]), "U_D": int(info["n_den_leaves"]), "plan": plan_name,
+                   "l2": f"inputs rotated over {res['n_rot']} resident batches (> L2)",
+                   "parallelism": "replicas" if world == 1 else f"sample-sharded x{world}, no collective"},
+        "kernels": {"ami_evaluate_ms": res["eval_ms"], "ami_dispersion_ms": res["disp_ms"], "dispersion": disp},
+        "roofline": roof,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
+                "steps": e2e_steps, "chunks_per_step": e2e["chunks"], "api": "ami_run(h_k -> h_out)"},
+        "gpu_launches": launches,
+        "clocks": res["clocks"],
+        "fp64_probe_dfma_per_s": dfma_per_s,
+    }
+    if world == 1 and rank == 0 and not args.no_extra:
+        # secondary workloads (north_star names order 4 AND order 6), short runs, same code path
+        others = {}
+        for name in ("cfg4", "cfg5", "cfg2_se", "cfg1"):
+            if name == cfg.name:
+                continue
+            c2 = A.get_config(name)
+            r2 = time_workload(pkg, torch, c2, c2.n_samples, 6, 3, plan, 0, None, sample_clocks=False)
+            i2 = r2["info"]
+            ops2, pn2 = plan_ops_for(i2, args.plan)
+            f2, b2 = len(c2.z_ext), len(c2.betas)
+            roof2, disp2 = roofline_objects(r2, c2.n_samples, f2, b2, ops2, peaks, dfma_per_s)
+            ms2 = r2["total_ms"] / 6
+            others[name] = {"T_flat": int(i2["n_terms"]), "samples": c2.n_samples, "n_freq": f2, "n_beta": b2,
+                            "plan": pn2, "ms_per_step": ms2, "eval_ms": r2["eval_ms"], "disp_ms": r2["disp_ms"],
+                            "term_evals_per_s": int(i2["n_terms"]) * c2.n_samples * f2 * b2 / (ms2 * 1e-3),
+                            "samples_per_s": c2.n_samples * f2 * b2 / (ms2 * 1e-3),
+                            "alu_frac": roof2["frac"], "hbm_frac": roof2["hbm_leg"]["frac"]}
+            del r2
+            torch.cuda.empty_cache()
+        line["other_workloads"] = others
+        import oracle
+        threads = oracle.hardware_threads()
+        n_s = oracle_sample_size(cfg, threads, args.cpu_seconds)
+        Tq, units, dt = oracle_rate(cfg, n_s, threads)
+        line["cpu_baseline"] = {"value": Tq * units / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": f"first {n_s} of {cfg.n_samples} samples x {n_f} freq x {n_b} beta, "
+                                          f"double precision, {dt:.1f} s"}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    dist, rank, local, world = dist_setup(args)
+    try:
+        if args.impl == "reference":
+            run_reference(args, dist, rank, world)
+        else:
+            run_ours(args, dist, rank, local, world)
+    finally:
+        if dist is not None:
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

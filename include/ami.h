@@ -193,6 +193,10 @@ int ami_generate_momenta(const ami_table* tab, uint64_t seed, int64_t first_samp
  * rate of double-precision FMA lane-operations per second. */
 int ami_fp64_peak_probe(int device, double* dfma_per_s, double* elapsed_ms);
 
+/* Total number of kernels this library has launched in the calling process so far (all tables, all
+ * streams); bench.py reports the difference over its timed region as "gpu_launches". */
+int64_t ami_kernel_launches(void);
+
 const char* ami_strerror(int code);
 const char* ami_last_cuda_error(void);
 int ami_version(void);

@@ -17,7 +17,7 @@ PLAN_AUTO, PLAN_FLAT, PLAN_TREE = 0, 1, 2
 EXPORTS = [
     "ami_construct", "ami_table_info", "ami_table_export", "ami_table_destroy", "ami_dispersion",
     "ami_evaluate", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
-    "ami_last_cuda_error", "ami_version",
+    "ami_last_cuda_error", "ami_version", "ami_kernel_launches",
 ]
 
 
@@ -73,6 +73,7 @@ def lib():
         L.ami_strerror.restype = C.c_char_p
         L.ami_strerror.argtypes = [C.c_int]
         L.ami_last_cuda_error.restype = C.c_char_p
+        L.ami_kernel_launches.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -221,6 +222,11 @@ class AmiTable:
         st = ami_run_stats()
         _check(lib().ami_run(self._h, C.byref(cfg), C.byref(st)))
         return {n_: getattr(st, n_) for n_, _ in ami_run_stats._fields_}, sums
+
+
+def kernel_launches() -> int:
+    """Kernels launched by the library in this process so far."""
+    return int(lib().ami_kernel_launches())
 
 
 def fp64_peak_probe(device=0):

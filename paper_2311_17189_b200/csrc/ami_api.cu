@@ -118,6 +118,8 @@ extern "C" {
 
 int ami_version(void) { return 1; }
 
+int64_t ami_kernel_launches(void) { return (int64_t)ami::total_launches(); }
+
 const char* ami_strerror(int code) {
   switch (code) {
     case AMI_OK: return "ok";

@@ -2,6 +2,7 @@
 // evaluation (S2 + S3, flat plan), momentum generation and tallies for the streamed driver (S4).
 // One thread owns one sample; every table read is warp-uniform; per-sample leaf values live in
 // shared memory as [slot][thread] so that every access is conflict-free.
+#include <atomic>
 #include <cstdio>
 
 #include "ami_device.cuh"
@@ -9,6 +10,13 @@
 
 namespace ami {
 using namespace amidev;
+
+static std::atomic<long long> g_launches{0};
+long long total_launches() { return g_launches.load(); }
+static inline void count_launch(int* launches, int n = 1) {
+  g_launches += n;
+  if (launches) *launches += n;
+}
 
 // ------------------------------------------------------------------------------------------
 // S1: ami_dispersion.  K_i = sum_l alpha^i_l k_l + alpha^i_ext q ; e_i = 2t(cos Kx + cos Ky) + mu
@@ -53,6 +61,7 @@ cudaError_t launch_dispersion(const DispParams& p, cudaStream_t st) {
   if (p.n == 0) return cudaSuccess;
   const int nt = 256;
   dispersion_kernel<<<(unsigned)((p.n + nt - 1) / nt), nt, 0, st>>>(p);
+  count_launch(nullptr);
   return cudaGetLastError();
 }
 
@@ -192,7 +201,7 @@ cudaError_t launch_eval_flat(const EvalParams& p, bool ce, cudaStream_t st, int*
   cudaError_t rc = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (rc != cudaSuccess) return rc;
   kern<<<(unsigned)((p.n_e + nt - 1) / nt), nt, smem, st>>>(p);
-  if (launches) ++*launches;
+  count_launch(launches);
   return cudaGetLastError();
 }
 
@@ -224,6 +233,7 @@ cudaError_t launch_generate_momenta(uint64_t seed, long long first, long long n,
   long long blocks = (total + 255) / 256;
   if (blocks > 148 * 16) blocks = 148 * 16;
   momenta_kernel<<<(unsigned)blocks, 256, 0, st>>>(seed, first, n, n_comp, d_k);
+  count_launch(nullptr);
   return cudaGetLastError();
 }
 
@@ -274,7 +284,7 @@ cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long 
                                            reinterpret_cast<double2*>(d_partial));
   row_final_kernel<<<(unsigned)n_rows, 32, 0, st>>>(reinterpret_cast<const double2*>(d_partial), kSumBlocks,
                                                     reinterpret_cast<double2*>(d_sum));
-  if (launches) *launches += 2;
+  count_launch(launches, 2);
   return cudaGetLastError();
 }
 

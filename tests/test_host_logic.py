@@ -23,7 +23,7 @@ def ami():
 
 def test_library_exports_every_declared_symbol(ami):
     header = open(os.path.join(ROOT, "include", "ami.h")).read()
-    declared = set(re.findall(r"^\s*(?:int|void|const char\*)\s+(ami_\w+)\s*\(", header, flags=re.M))
+    declared = set(re.findall(r"^\s*(?:int|int64_t|void|const char\*)\s+(ami_\w+)\s*\(", header, flags=re.M))
     assert declared == set(ami.EXPORTS), declared ^ set(ami.EXPORTS)
     L = ami.lib()
     for name in declared:
