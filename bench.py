@@ -37,7 +37,7 @@ def parse_args():
     ap.add_argument("--workload", default="cfg3", help="cfg1 | cfg2_se | cfg2_bubble | cfg3 | cfg4 | cfg5 | stress8")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=0, help="override samples per step per GPU")
-    ap.add_argument("--plan", default="auto", choices=["auto", "flat", "tree"])
+    ap.add_argument("--plan", default="auto", choices=["auto", "flat", "reg"])
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads and the CPU baseline")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -101,20 +101,27 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
-# algorithmic FP64 work:
-#   W = 2 N_eps c_cos [S1] + N_b U_F (c_exp + c_rcp + 4) [Fermi/Bose] + N_f U_D (c_rcp + 8) [reciprocals]
-#       + N_f N_b * (term-loop FP64 instructions of the representation executed)
-# c_* = FP64-pipe instructions of one double cos / exp / reciprocal as compiled for sm_100a (counted
-# in the SASS of this library, DESIGN.md table "leaf costs").
+# algorithmic FP64 work per sample, in FP64-pipe instruction slots:
+#   W = N_eps (2 c_cos + 2)                      [S1: two cosines, one add, one fma per energy symbol]
+#     + N_b U_F c_fermi                          [S2: Fermi/Bose leaves, once per beta]
+#     + N_b N_f U_D c_den                        [S2: complex reciprocals]
+#     + N_b ops_FT + N_b N_f ops_R               [S3: Horner plan]   or   N_b N_f ops_flat  [S3: flat plan]
+# c_* = FP64-pipe instructions of the leaf routines on their common path as compiled for sm_100a,
+# counted in the SASS (DESIGN.md table "leaf costs"); cross-checked against ncu
+# sm__inst_executed_pipe_fp64 in profiles/.
 # ------------------------------------------------------------------------------------------------
-C_COS, C_EXP, C_RCP = 38, 23, 6
+C_COS, C_FERMI, C_DEN = 18, 24, 11
 
 
-def fp64_work_per_sample(info, n_f, n_b, plan_ops):
-    disp = 2 * info["n_eps"] * C_COS
-    fermi = n_b * info["n_fermi_leaves"] * (C_EXP + C_RCP + 4)
-    dens = n_f * info["n_den_leaves"] * (C_RCP + 8)
-    terms = n_f * n_b * plan_ops
+def fp64_work_per_sample(info, n_f, n_b, reg):
+    disp = info["n_eps"] * (2 * C_COS + 2)
+    fermi = n_b * info["n_fermi_leaves"] * C_FERMI
+    dens = n_b * n_f * info["n_den_leaves"] * C_DEN
+    if reg:
+        ft = int(info["fp64_ops_tree_fermi"])
+        terms = n_b * ft + n_b * n_f * (int(info["fp64_ops_tree"]) - ft)
+    else:
+        terms = n_b * n_f * int(info["fp64_ops_flat"])
     return {"dispersion": disp, "evaluate": fermi + dens + terms, "fermi": fermi, "denominators": dens,
             "terms": terms}
 
@@ -221,19 +228,30 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
     bytes_in = n * 2 * m * 8
     n_rot = int(max(2, min(8, -(-300_000_000 // max(bytes_in + n * n_eps * 8, 1)))))
     ks = [tab.generate_momenta(cfg.seed, first_sample + r * n, n) for r in range(n_rot)]
-    es = [torch.empty((n_eps, n), dtype=torch.float64, device="cuda") for _ in range(n_rot)]
+    es = [torch.empty((n_eps, n), dtype=torch.float64, device="cuda") for _ in range(n_rot)] \
+        if not (plan in (0, 3) and info["reg_plan_status"] in (0, 1)) else []
     out = torch.empty((n_b, n_f, n), dtype=torch.complex128, device="cuda")
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
     t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    reg = plan in (0, 3) and info["reg_plan_status"] in (0, 1)
+    if reg:
+        info = tab.specialize()        # NVRTC compile + load happen here, outside every timed region
 
     def step(i, events=None):
         r = i % n_rot
         if events:
             events[0].record()
-        tab.dispersion(ks[r], [cfg.q], cfg.t, cfg.mu, out=es[r])
-        if events:
-            events[1].record()
-        tab.evaluate(es[r], cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan, out=out)
+        if reg:     # one fused kernel: dispersion inline, energies stay in registers
+            if events:
+                events[1].record()
+            tab.evaluate_momenta(ks[r], [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan,
+                                 out=out)
+        else:
+            tab.dispersion(ks[r], [cfg.q], cfg.t, cfg.mu, out=es[r])
+            if events:
+                events[1].record()
+            tab.evaluate(es[r], cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan, out=out)
         if events:
             events[2].record()
 
@@ -261,7 +279,7 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
     disp_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
     eval_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
     checksum = complex(out[0, 0, : min(n, 1024)].sum().item())
-    return {"tab": tab, "info": info, "total_ms": total_ms, "disp_ms": disp_ms, "eval_ms": eval_ms,
+    return {"tab": tab, "info": info, "fused": reg, "total_ms": total_ms, "disp_ms": disp_ms, "eval_ms": eval_ms,
             "launches": launches, "clocks": clocks, "n_rot": n_rot, "checksum": checksum,
             "bytes_in": bytes_in, "bytes_e": n * n_eps * 8, "bytes_out": n * n_f * n_b * 16}
 
@@ -293,38 +311,48 @@ def time_e2e(pkg, torch, tab, cfg, n, steps, warmup, plan, first_sample, dist):
 
 
 def roofline_objects(res, n, n_f, n_b, plan_ops, peaks, dfma_per_s):
-    """Roofline of the dominant kernel (ami_evaluate): FP64-pipe bound.  Work counted in FP64-pipe
-    instruction slots per sample, expressed as DFMA-equivalent TFLOP/s (slot = 2 flop)
-    against the DFMA-chain rate measured in this run; the HBM leg is reported beside it."""
-    w = fp64_work_per_sample(res["info"], n_f, n_b, plan_ops)
+    """Roofline of the dominant kernel: FP64-pipe bound.  Work counted in FP64-pipe instruction slots
+    per sample, expressed as DFMA-equivalent TFLOP/s (slot = 2 flop) against the DFMA-chain
+    rate measured in this run; the HBM leg is reported beside it.  With the register plan the step is
+    ONE fused kernel (S1+S2+S3), otherwise ami_evaluate is the dominant one of two."""
+    w = fp64_work_per_sample(res["info"], n_f, n_b, res["fused"])
     t_eval = res["eval_ms"] * 1e-3
-    t_disp = res["disp_ms"] * 1e-3
     peak_tf = 2.0 * dfma_per_s / 1e12
-    ach = 2.0 * w["evaluate"] * n / t_eval / 1e12
-    eval_bytes = res["bytes_e"] + res["bytes_out"]
-    disp_bytes = res["bytes_in"] + res["bytes_e"]
-    roof = {"bound": "alu", "kernel": "ami_evaluate", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
+    if res["fused"]:
+        slots = w["evaluate"] + w["dispersion"]
+        bytes_alg = res["bytes_in"] + res["bytes_out"]
+        kernel = "ami_jit_fused (S1+S2+S3)"
+    else:
+        slots = w["evaluate"]
+        bytes_alg = res["bytes_e"] + res["bytes_out"]
+        kernel = "ami_evaluate (flat)"
+    ach = 2.0 * slots * n / t_eval / 1e12
+    roof = {"bound": "alu", "kernel": kernel, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
             "frac": ach / peak_tf, "traffic": None,
             "peak_source": "DFMA-chain probe run by this bench (FP64 pipe; MEASURED_PEAKS.json has no FP64 figure)",
             "flop_convention": "FP64-pipe instruction slots x 2",
-            "fp64_slots_per_sample": w,
-            "hbm_leg": {"algorithmic_bytes": eval_bytes, "achieved_gbs": eval_bytes / t_eval / 1e9,
-                        "peak_gbs": peaks["hbm_gbs"], "frac": eval_bytes / t_eval / 1e9 / peaks["hbm_gbs"],
+            "fp64_slots_per_sample": w, "fp64_slots_counted": slots,
+            "hbm_leg": {"algorithmic_bytes": bytes_alg, "achieved_gbs": bytes_alg / t_eval / 1e9,
+                        "peak_gbs": peaks["hbm_gbs"], "frac": bytes_alg / t_eval / 1e9 / peaks["hbm_gbs"],
                         "peak_source": peaks["source"]}}
-    disp = {"kernel": "ami_dispersion", "ms": res["disp_ms"],
-            "alu_frac": 2.0 * w["dispersion"] * n / t_disp / 1e12 / peak_tf,
-            "hbm_frac": disp_bytes / t_disp / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": disp_bytes}
+    disp = None
+    if not res["fused"]:
+        t_disp = res["disp_ms"] * 1e-3
+        disp_bytes = res["bytes_in"] + res["bytes_e"]
+        disp = {"kernel": "ami_dispersion", "ms": res["disp_ms"],
+                "alu_frac": 2.0 * w["dispersion"] * n / t_disp / 1e12 / peak_tf,
+                "hbm_frac": disp_bytes / t_disp / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": disp_bytes}
     return roof, disp
 
 
-PLAN_IDS = {"auto": 0, "flat": 1, "tree": 2}
+PLAN_IDS = {"auto": 0, "flat": 1, "reg": 3}
 
 
 def plan_ops_for(info, plan):
     """Term-loop FP64 slots per (sample, frequency, beta) of the representation ami_evaluate executes."""
-    if plan != "flat" and info.get("fp64_ops_tree", 0) > 0:
-        return int(info["fp64_ops_tree"]), "tree"
-    return int(info["fp64_ops_flat"]), "flat"
+    if plan != "flat" and info["reg_plan_status"] == 0:
+        return int(info["fp64_ops_tree"]), "register (Horner, NVRTC-specialised)"
+    return int(info["fp64_ops_flat"]), "flat (table-driven)"
 
 
 def run_ours(args, dist, rank, local, world):
@@ -367,7 +395,8 @@ def run_ours(args, dist, rank, local, world):
                    "U_F": int(info["n_fermi_leaves"]), "U_D": int(info["n_den_leaves"]), "plan": plan_name,
                    "l2": f"inputs rotated over {res['n_rot']} resident batches (> L2)",
                    "parallelism": "replicas" if world == 1 else f"sample-sharded x{world}, no collective"},
-        "kernels": {"ami_evaluate_ms": res["eval_ms"], "ami_dispersion_ms": res["disp_ms"], "dispersion": disp},
+        "kernels": {"dominant_ms": res["eval_ms"], "ami_dispersion_ms": None if res["fused"] else res["disp_ms"],
+                    "dispersion": disp, "launches_per_step": res["launches"] / max(1, args.steps)},
         "roofline": roof,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                 "steps": e2e_steps, "chunks_per_step": e2e["chunks"], "api": "ami_run(h_k -> h_out)"},

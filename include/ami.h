@@ -63,8 +63,12 @@ typedef struct ami_table ami_table;
 /* Which representation ami_evaluate executes. */
 enum {
   AMI_PLAN_AUTO = 0,  /* the library's fastest plan for this table */
-  AMI_PLAN_FLAT = 1,  /* the flat term table, term by term (SURVEY 8(a) S3 as written) */
-  AMI_PLAN_TREE = 2   /* terms grouped by denominator product, Fermi products prefix-shared */
+  AMI_PLAN_FLAT = 1,  /* the flat term table, term by term, table-driven (SURVEY 8(a) S3 as written) */
+  AMI_PLAN_TREE = 2,  /* reserved for a table-driven form of the Horner plan; runs the flat kernel today */
+  AMI_PLAN_REG = 3    /* register plan: the table written out as a straight-line kernel specialised to
+                         this diagram (terms grouped by denominator product, Fermi/Bose and denominator
+                         products in Horner form, every leaf a register), compiled with NVRTC on first
+                         use; real energies and tables within the size limits only */
 };
 
 typedef struct ami_info {
@@ -76,14 +80,16 @@ typedef struct ami_info {
   int64_t n_terms;          /* T_flat after merging identical terms */
   int64_t n_terms_raw;      /* terms produced by the recursion before merging */
   int64_t n_multipoles;     /* pole groups with multiplicity > 1 met during construction */
-  int64_t n_groups;         /* distinct denominator products (tree plan) */
-  int64_t n_tree_nodes;     /* Fermi-trie nodes of the tree plan */
-  int64_t n_den_nodes;      /* denominator-trie nodes of the tree plan */
+  int64_t n_groups;         /* distinct denominator products R (Horner plan) */
+  int64_t n_tree_nodes;     /* Fermi-trie nodes of the Horner plan, summed over groups */
+  int64_t n_den_nodes;      /* denominator-trie nodes of the Horner plan */
   int64_t table_bytes;      /* bytes of the device-resident copy (all plans) */
   int64_t fp64_ops_flat;    /* FP64 instructions per (sample,frequency,beta) of the flat term loop */
-  int64_t fp64_ops_tree;    /* same for the tree plan */
+  int64_t fp64_ops_tree;    /* same for the Horner plan with n_f = n_b = 1 (FT part + R part) */
+  int64_t fp64_ops_tree_fermi; /* its FT part alone: done once per (sample,beta), not per frequency */
   int32_t has_device_copy;
-  int32_t reserved;
+  int32_t reg_plan_status;  /* 0 = specialised kernels loaded, 1 = eligible, not compiled yet,
+                               AMI_EUNSUPPORTED = table outside the register plan's limits, other < 0 = error */
 } ami_info;
 
 /* ami_construct -- Eqs. 1-5, API of PAPER.md:246.
@@ -147,6 +153,28 @@ int ami_dispersion(const ami_table* tab, const double* d_k, int64_t k_stride_sam
  *   d_out   complex128 [n_b][n_f][n_e] (rows = frequencies, energy index fastest) */
 int ami_evaluate(const ami_table* tab, const void* d_e, int e_is_complex, int64_t n_e, const double* z_ext,
                  int n_f, const double* beta, int n_b, double e_reg, int plan, void* d_out, void* stream);
+
+/* Fused S1+S2+S3: ami_dispersion followed by ami_evaluate for the same samples in one call.  With the
+ * register plan this is ONE kernel (the dispersion is inline and the energies never leave registers);
+ * with the table-driven plans it is the two kernels back to back.
+ *   d_k, strides, q, t, mu as for ami_dispersion;  z_ext, beta, e_reg, plan, d_out as for ami_evaluate
+ *   d_e   float64 [n_eps][n] or NULL.  When given it receives the energies.  The table-driven plans
+ *         need it as workspace and return AMI_EINVAL without it. */
+int ami_evaluate_momenta(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
+                         const double* q, double t, double mu, int64_t n, const double* z_ext, int n_f,
+                         const double* beta, int n_b, double e_reg, int plan, double* d_e, void* d_out, void* stream);
+
+/* Register plan management.  ami_table_specialize compiles and loads the specialised kernels now
+ * (otherwise this happens at the first evaluation with AMI_PLAN_AUTO or AMI_PLAN_REG); it returns
+ * AMI_EUNSUPPORTED when the table is outside the plan's limits or NVRTC cannot be loaded, AMI_EINVAL when
+ * compilation fails (ami_last_cuda_error() then holds the compiler log).  ami_table_kernel_source /
+ * ami_table_kernel_cubin return the generated CUDA C++ text and its sm_100a cubin for inspection
+ * (cuobjdump -sass); neither needs a GPU.  Call with buf = NULL to get the size for the source; for the
+ * cubin pass a buffer and its capacity in *bytes (AMI_EINVAL if too small).  `log` (may be NULL) receives
+ * the compiler log, including the ptxas resource usage lines. */
+int ami_table_specialize(ami_table* tab);
+int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes);
+int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char* log, size_t log_cap);
 
 /* Streamed driver.  Source of the momenta: if h_k / d_k are both NULL they are generated on the
  * device from `seed` with the counter-based generator of P22 (sample index = first_sample + s);

@@ -12,11 +12,12 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libami_b200.so")
 
-PLAN_AUTO, PLAN_FLAT, PLAN_TREE = 0, 1, 2
+PLAN_AUTO, PLAN_FLAT, PLAN_TREE, PLAN_REG = 0, 1, 2, 3
 
 EXPORTS = [
     "ami_construct", "ami_table_info", "ami_table_export", "ami_table_destroy", "ami_dispersion",
-    "ami_evaluate", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
+    "ami_evaluate", "ami_evaluate_momenta", "ami_table_specialize", "ami_table_kernel_source",
+    "ami_table_kernel_cubin", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
     "ami_last_cuda_error", "ami_version", "ami_kernel_launches",
 ]
 
@@ -31,8 +32,9 @@ class ami_info(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("n_int", "n_ext", "n_g", "n_eps", "n_fermi_leaves", "n_den_leaves",
                                          "max_deriv", "max_den_per_term")] + \
                [(n, C.c_int64) for n in ("n_terms", "n_terms_raw", "n_multipoles", "n_groups", "n_tree_nodes",
-                                         "n_den_nodes", "table_bytes", "fp64_ops_flat", "fp64_ops_tree")] + \
-               [("has_device_copy", C.c_int32), ("reserved", C.c_int32)]
+                                         "n_den_nodes", "table_bytes", "fp64_ops_flat", "fp64_ops_tree",
+                                         "fp64_ops_tree_fermi")] + \
+               [("has_device_copy", C.c_int32), ("reg_plan_status", C.c_int32)]
 
 
 class ami_run_cfg(C.Structure):
@@ -67,6 +69,12 @@ def lib():
                                      C.c_double, C.c_int64, C.c_void_p, C.c_void_p]
         L.ami_evaluate.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_int, C.c_void_p,
                                    C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
+        L.ami_evaluate_momenta.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
+                                           C.c_double, C.c_int64, C.c_void_p, C.c_int, C.c_void_p, C.c_int,
+                                           C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.ami_table_specialize.argtypes = [C.c_void_p]
+        L.ami_table_kernel_source.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
+        L.ami_table_kernel_cubin.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p, C.c_size_t]
         L.ami_run.argtypes = [C.c_void_p, C.POINTER(ami_run_cfg), C.POINTER(ami_run_stats)]
         L.ami_generate_momenta.argtypes = [C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
         L.ami_fp64_peak_probe.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -81,7 +89,7 @@ def lib():
 def _check(rc):
     if rc != 0:
         msg = lib().ami_strerror(rc).decode()
-        if rc in (-4, -5):
+        if rc in (-1, -4, -5, -6) and lib().ami_last_cuda_error():
             msg += " [" + lib().ami_last_cuda_error().decode() + "]"
         raise AmiError(rc, msg)
 
@@ -136,7 +144,32 @@ class AmiTable:
     def _info(self) -> dict:
         s = ami_info()
         _check(lib().ami_table_info(self._h, C.byref(s)))
-        return {n: getattr(s, n) for n, _ in ami_info._fields_ if n != "reserved"}
+        return {n: getattr(s, n) for n, _ in ami_info._fields_}
+
+    def refresh_info(self) -> dict:
+        self.info = self._info()
+        return self.info
+
+    # ---- register plan ----------------------------------------------------------------------
+    def specialize(self):
+        """ami_table_specialize: compile and load the specialised kernels now."""
+        _check(lib().ami_table_specialize(self._h))
+        return self.refresh_info()
+
+    def kernel_source(self) -> str:
+        n = C.c_size_t(0)
+        _check(lib().ami_table_kernel_source(self._h, None, C.byref(n)))
+        buf = C.create_string_buffer(n.value)
+        _check(lib().ami_table_kernel_source(self._h, buf, C.byref(n)))
+        return buf.value.decode()
+
+    def kernel_cubin(self, cap=64 << 20):
+        """(cubin bytes, compiler log); needs NVRTC but no GPU."""
+        buf = C.create_string_buffer(cap)
+        log = C.create_string_buffer(1 << 16)
+        n = C.c_size_t(cap)
+        _check(lib().ami_table_kernel_cubin(self._h, buf, C.byref(n), log, len(log)))
+        return buf.raw[: n.value], log.value.decode()
 
     def export(self) -> dict:
         """ami_table_export parsed into numpy arrays (layout documented in include/ami.h)."""
@@ -193,6 +226,30 @@ class AmiTable:
         _check(lib().ami_evaluate(self._h, C.c_void_p(e.data_ptr()), int(is_c), n_e, z.ctypes.data, n_f,
                                   b.ctypes.data, n_b, float(e_reg), int(plan), C.c_void_p(out.data_ptr()),
                                   _stream_ptr(stream)))
+        return out
+
+    def evaluate_momenta(self, k, q, t, mu, z_ext, beta, e_reg=0.0, plan=PLAN_AUTO, e_out=None, out=None,
+                         stream=None):
+        """ami_evaluate_momenta: S1+S2+S3 for momenta k [n][n_int][2] -> complex128 [n_b][n_f][n].
+        ``e_out`` ([n_eps][n] float64) receives the energies when given; it is allocated here when
+        the plan that runs needs it as workspace."""
+        import torch
+        assert k.is_cuda and k.dtype == torch.float64 and k.is_contiguous()
+        n = k.shape[0]
+        z = _z_host(z_ext, self.n_ext)
+        b = _host(np.atleast_1d(beta), np.float64)
+        n_f, n_b = z.shape[0], b.shape[0]
+        if out is None:
+            out = torch.empty((n_b, n_f, n), dtype=torch.complex128, device=k.device)
+        assert out.is_contiguous() and out.dtype == torch.complex128 and out.numel() == n_b * n_f * n
+        reg = plan in (PLAN_AUTO, PLAN_REG) and self.info["reg_plan_status"] in (0, 1)
+        if e_out is None and not reg:
+            e_out = torch.empty((self.n_eps, n), dtype=torch.float64, device=k.device)
+        qh = _host(np.asarray(q, dtype=np.float64).reshape(max(self.n_ext, 1), 2), np.float64)
+        _check(lib().ami_evaluate_momenta(self._h, C.c_void_p(k.data_ptr()), 2 * self.n_int, 1, qh.ctypes.data,
+                                          float(t), float(mu), n, z.ctypes.data, n_f, b.ctypes.data, n_b,
+                                          float(e_reg), int(plan), None if e_out is None else C.c_void_p(e_out.data_ptr()),
+                                          C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
         return out
 
     def generate_momenta(self, seed, first_sample, n, stream=None):

@@ -4,6 +4,7 @@
 #include <new>
 #include <string>
 
+#include "ami_jit.hpp"
 #include "ami_kernels.cuh"
 
 namespace ami {
@@ -96,8 +97,6 @@ int make_device_copy(ami_table* tab, int device) {
   if ((rc = upload(da, &dc.leafD_a, dc.bytes))) return rc;
   if ((rc = upload(tix, &dc.term_idx, dc.bytes))) return rc;
   if ((rc = upload(tco, &dc.term_coef, dc.bytes))) return rc;
-  if ((rc = upload(tab->tree.code, &dc.tree_code, dc.bytes))) return rc;
-  if ((rc = upload(tab->tree.consts, &dc.tree_consts, dc.bytes))) return rc;
   if ((rc = upload(sa, &dc.sym_alpha, dc.bytes))) return rc;
   if ((rc = upload(deriv_polys(), &dc.derivQ, dc.bytes))) return rc;
   return AMI_OK;
@@ -108,7 +107,7 @@ void free_device_copy(ami_device_copy& dc) {
   cudaSetDevice(dc.device);
   cudaFree(dc.leaf_ptr); cudaFree(dc.leaf_sym); cudaFree(dc.leaf_coef); cudaFree(dc.leafF_sig);
   cudaFree(dc.leafF_k); cudaFree(dc.leafD_a); cudaFree(dc.term_idx); cudaFree(dc.term_coef);
-  cudaFree(dc.tree_code); cudaFree(dc.tree_consts); cudaFree(dc.sym_alpha); cudaFree(dc.derivQ);
+  cudaFree(dc.sym_alpha); cudaFree(dc.derivQ);
   dc = ami_device_copy();
 }
 
@@ -147,7 +146,7 @@ int ami_construct(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha
     rc = ami::construct_flat(n_int, n_ext, n_g, n_eps, alpha, eps, slot_is_fermionic, sum_order, prefactor,
                              tab->flat);
     if (rc == AMI_OK) {
-      ami::build_tree_plan(tab->flat, tab->tree);
+      ami::build_horner_plan(tab->flat, tab->horner);
       tab->fp64_ops_flat = ami::flat_fp64_ops(tab->flat);
     }
   } catch (const std::bad_alloc&) {
@@ -166,6 +165,7 @@ int ami_construct(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha
 
 void ami_table_destroy(ami_table* tab) {
   if (!tab) return;
+  ami::jit_destroy(tab);
   free_device_copy(tab->dev);
   delete tab;
 }
@@ -182,13 +182,16 @@ int ami_table_info(const ami_table* tab, ami_info* info) {
   info->n_terms = (int64_t)ft.terms.size();
   info->n_terms_raw = ft.n_terms_raw;
   info->n_multipoles = ft.n_multipoles;
-  info->n_groups = tab->tree.n_groups;
-  info->n_tree_nodes = tab->tree.n_fnodes;
-  info->n_den_nodes = tab->tree.n_dnodes;
+  info->n_groups = (int64_t)tab->horner.groups.size();
+  info->n_tree_nodes = tab->horner.n_fnodes;
+  info->n_den_nodes = tab->horner.n_dnodes;
   info->table_bytes = tab->dev.bytes;
   info->fp64_ops_flat = tab->fp64_ops_flat;
-  info->fp64_ops_tree = tab->tree.fp64_ops;
+  info->fp64_ops_tree = tab->horner.ops_f + tab->horner.ops_d;
+  info->fp64_ops_tree_fermi = tab->horner.ops_f;
   info->has_device_copy = tab->dev.device >= 0;
+  info->reg_plan_status = !ami::jit_eligible(ft, tab->horner) ? AMI_EUNSUPPORTED
+                          : (tab->jit ? ami::jit_status(tab) : 1);
   return AMI_OK;
 }
 
@@ -237,7 +240,7 @@ void fill_table_params(const ami_table* tab, ami::EvalParams& p) {
   p.leaf_ptr = dc.leaf_ptr; p.leaf_sym = dc.leaf_sym; p.leaf_coef = dc.leaf_coef;
   p.leafF_sig = dc.leafF_sig; p.leafF_k = dc.leafF_k; p.leafD_a = dc.leafD_a;
   p.term_idx = dc.term_idx; p.term_coef = dc.term_coef;
-  p.tree_code = dc.tree_code; p.tree_consts = dc.tree_consts; p.derivQ = dc.derivQ;
+  p.derivQ = dc.derivQ;
   p.n_eps = ft.n_eps; p.n_ext = ft.n_ext;
   p.U_F = (int)ft.leafF.size(); p.U_D = (int)ft.leafD.size();
   p.m_f = ft.n_int; p.n_d = ft.max_den;
@@ -245,31 +248,99 @@ void fill_table_params(const ami_table* tab, ami::EvalParams& p) {
   p.prefactor = ft.prefactor;
 }
 
+// Decides which representation runs.  Returns AMI_OK and sets *use_reg, or an error when the
+// register plan was asked for explicitly and cannot be had.
+int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg) {
+  *use_reg = false;
+  if (plan == AMI_PLAN_FLAT || plan == AMI_PLAN_TREE) return AMI_OK;
+  if (e_is_complex || !ami::jit_eligible(tab->flat, tab->horner)) {
+    if (plan == AMI_PLAN_REG) { g_cuda_err = "register plan unavailable for this table / energy type"; return AMI_EUNSUPPORTED; }
+    return AMI_OK;
+  }
+  std::string err;
+  const int rc = ami::jit_prepare(const_cast<ami_table*>(tab), err);   // lazily compiled, cached in the table
+  if (rc == AMI_OK) { *use_reg = true; return AMI_OK; }
+  g_cuda_err = err;
+  return plan == AMI_PLAN_REG ? rc : AMI_OK;    // AUTO falls back to the table-driven kernels
+}
+
+struct MomentaSrc {
+  const double* d_k = nullptr;
+  int64_t stride_sample = 0, stride_comp = 0;
+  const double* q = nullptr;
+  double t = 0, mu = 0;
+};
+
 // Launches the evaluation for all (beta, frequency) pairs, split so that one launch carries at
 // most kMaxBeta temperatures and kMaxFreqWords frequency words.  `out` points at sample 0 of
-// row (b=0,f=0); rows are out_row_stride samples apart.
-int evaluate_impl(const ami_table* tab, const void* d_e, int e_is_complex, int64_t n_e, int64_t e_stride,
-                  const double* z_ext, int n_f, const double* beta, int n_b, double e_reg, int plan,
+// row (b=0,f=0); rows are out_row_stride samples apart.  With `mom` the energies are formed from
+// momenta first: inline by the register plan (and stored to d_e only when d_e is given), by the
+// dispersion kernel into d_e otherwise.
+int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, int e_is_complex, int64_t n_e,
+                  int64_t e_stride, const double* z_ext, int n_f, const double* beta, int n_b, double e_reg, int plan,
                   void* d_out, int64_t out_row_stride, cudaStream_t st, int* launches) {
   using namespace ami;
-  EvalParams p;
-  memset(&p, 0, sizeof p);
-  fill_table_params(tab, p);
-  p.e = (const double*)d_e; p.out = (double*)d_out;
-  p.n_e = n_e; p.e_stride = e_stride; p.out_row_stride = out_row_stride;
-  p.n_f_total = n_f; p.e_reg = e_reg;
+  bool use_reg = false;
+  int rc = choose_plan(tab, plan, e_is_complex != 0, &use_reg);
+  if (rc != AMI_OK) return rc;
   const int n_ext = tab->flat.n_ext;
   const int f_chunk = n_ext ? std::max(1, kMaxFreqWords / n_ext) : kMaxFreqWords;
-  const bool use_tree = (plan == AMI_PLAN_TREE || plan == AMI_PLAN_AUTO) && !tab->tree.code.empty();
+  if (mom && !use_reg) {
+    if (!d_e) return AMI_EINVAL;   // the table-driven kernels need the energies in memory
+    DispParams dp;
+    memset(&dp, 0, sizeof dp);
+    dp.sym_alpha = tab->dev.sym_alpha;
+    dp.n_int = tab->flat.n_int; dp.n_ext = n_ext; dp.n_eps = tab->flat.n_eps;
+    dp.k = mom->d_k; dp.k_stride_sample = mom->stride_sample; dp.k_stride_comp = mom->stride_comp; dp.n = n_e;
+    for (int i = 0; i < 2 * n_ext; ++i) dp.q[i] = mom->q[i];
+    dp.t = mom->t; dp.mu = mom->mu; dp.e = (double*)d_e; dp.e_stride = e_stride;
+    cudaError_t crc = launch_dispersion(dp, st);
+    if (crc != cudaSuccess) return cuda_fail(crc);
+    if (launches) ++*launches;
+  }
+  EvalParams p;
+  AmiBatch jb;
+  memset(&p, 0, sizeof p);
+  memset(&jb, 0, sizeof jb);
+  if (use_reg) {
+    jb.e = (const double*)d_e; jb.e_stride = e_stride;
+    if (mom) {
+      jb.k = mom->d_k; jb.k_stride_sample = mom->stride_sample; jb.k_stride_comp = mom->stride_comp;
+      for (int i = 0; i < 2 * n_ext; ++i) jb.q[i] = mom->q[i];
+      jb.t = mom->t; jb.mu = mom->mu;
+      jb.e_out = (double*)d_e;
+    }
+    jb.out = (double*)d_out; jb.n = n_e; jb.out_row_stride = out_row_stride;
+    jb.n_f_total = n_f; jb.e_reg = e_reg; jb.prefactor = tab->flat.prefactor;
+  } else {
+    fill_table_params(tab, p);
+    p.e = (const double*)d_e; p.out = (double*)d_out;
+    p.n_e = n_e; p.e_stride = e_stride; p.out_row_stride = out_row_stride;
+    p.n_f_total = n_f; p.e_reg = e_reg;
+  }
+  bool first = true;
   for (int b0 = 0; b0 < n_b; b0 += kMaxBeta) {
-    p.b0 = b0; p.n_b = std::min(kMaxBeta, n_b - b0);
-    for (int i = 0; i < p.n_b; ++i) p.beta[i] = beta[b0 + i];
+    const int nb = std::min(kMaxBeta, n_b - b0);
     for (int f0 = 0; f0 < n_f; f0 += f_chunk) {
-      p.f0 = f0; p.n_f = std::min(f_chunk, n_f - f0);
-      for (int i = 0; i < p.n_f * n_ext * 2; ++i) p.z[i] = z_ext[(size_t)f0 * n_ext * 2 + i];
-      cudaError_t rc = use_tree ? launch_eval_tree(p, e_is_complex != 0, st, launches)
-                                : launch_eval_flat(p, e_is_complex != 0, st, launches);
-      if (rc != cudaSuccess) return cuda_fail(rc);
+      const int nf = std::min(f_chunk, n_f - f0);
+      cudaError_t crc;
+      if (use_reg) {
+        jb.b0 = b0; jb.n_b = nb; jb.f0 = f0; jb.n_f = nf;
+        for (int i = 0; i < nb; ++i) jb.beta[i] = beta[b0 + i];
+        for (int i = 0; i < nf * n_ext * 2; ++i) jb.z[i] = z_ext[(size_t)f0 * n_ext * 2 + i];
+        // later launches of a split grid read the energies the first one stored
+        const bool fused = mom && (first || !d_e);
+        if (!fused) { jb.e_out = nullptr; }
+        crc = jit_launch(tab, fused, jb, st);
+        if (crc == cudaSuccess) count_external_launch(launches);
+      } else {
+        p.b0 = b0; p.n_b = nb; p.f0 = f0; p.n_f = nf;
+        for (int i = 0; i < nb; ++i) p.beta[i] = beta[b0 + i];
+        for (int i = 0; i < nf * n_ext * 2; ++i) p.z[i] = z_ext[(size_t)f0 * n_ext * 2 + i];
+        crc = launch_eval_flat(p, e_is_complex != 0, st, launches);
+      }
+      if (crc != cudaSuccess) return cuda_fail(crc);
+      first = false;
     }
   }
   return AMI_OK;
@@ -307,12 +378,73 @@ int ami_evaluate(const ami_table* tab, const void* d_e, int e_is_complex, int64_
   int rc = check_device(tab);
   if (rc) return rc;
   if (n_e < 0 || n_f < 0 || n_b < 0 || (n_f > 0 && tab->flat.n_ext > 0 && !z_ext) || (n_b > 0 && !beta) ||
-      plan < AMI_PLAN_AUTO || plan > AMI_PLAN_TREE)
+      plan < AMI_PLAN_AUTO || plan > AMI_PLAN_REG)
     return AMI_EINVAL;
   if (n_e == 0 || n_f == 0 || n_b == 0) return AMI_OK;
   if (!d_e || !d_out) return AMI_EINVAL;
-  return evaluate_impl(tab, d_e, e_is_complex, n_e, n_e, z_ext, n_f, beta, n_b, e_reg, plan, d_out, n_e,
+  return evaluate_impl(tab, nullptr, d_e, e_is_complex, n_e, n_e, z_ext, n_f, beta, n_b, e_reg, plan, d_out, n_e,
                        (cudaStream_t)stream, nullptr);
+}
+
+int ami_evaluate_momenta(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
+                         const double* q, double t, double mu, int64_t n, const double* z_ext, int n_f,
+                         const double* beta, int n_b, double e_reg, int plan, double* d_e, void* d_out, void* stream) {
+  int rc = check_device(tab);
+  if (rc) return rc;
+  if (n < 0 || n_f < 0 || n_b < 0 || (n_f > 0 && tab->flat.n_ext > 0 && !z_ext) || (n_b > 0 && !beta) ||
+      (tab->flat.n_ext > 0 && !q) || plan < AMI_PLAN_AUTO || plan > AMI_PLAN_REG)
+    return AMI_EINVAL;
+  if (n == 0) return AMI_OK;
+  if (!d_k || (!d_out && n_f > 0 && n_b > 0)) return AMI_EINVAL;
+  MomentaSrc ms;
+  ms.d_k = d_k; ms.stride_sample = k_stride_sample; ms.stride_comp = k_stride_comp;
+  ms.q = q; ms.t = t; ms.mu = mu;
+  if (n_f == 0 || n_b == 0) {
+    if (!d_e) return AMI_OK;
+    return ami_dispersion(tab, d_k, k_stride_sample, k_stride_comp, q, t, mu, n, d_e, stream);
+  }
+  return evaluate_impl(tab, &ms, d_e, 0, n, n, z_ext, n_f, beta, n_b, e_reg, plan, d_out, n, (cudaStream_t)stream,
+                       nullptr);
+}
+
+int ami_table_specialize(ami_table* tab) {
+  int rc = check_device(tab);
+  if (rc) return rc;
+  std::string err;
+  rc = ami::jit_prepare(tab, err);
+  if (rc != AMI_OK) g_cuda_err = err;
+  return rc;
+}
+
+int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes) {
+  if (!tab || !bytes) return AMI_EINVAL;
+  if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
+  const std::string src = ami::jit_generate_source(tab->flat, tab->horner, ami::kJitBlockThreads);
+  if (!buf) { *bytes = src.size() + 1; return AMI_OK; }
+  if (*bytes < src.size() + 1) return AMI_EINVAL;
+  memcpy(buf, src.c_str(), src.size() + 1);
+  *bytes = src.size() + 1;
+  return AMI_OK;
+}
+
+int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char* log, size_t log_cap) {
+  if (!tab || !bytes) return AMI_EINVAL;
+  if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
+  std::vector<char> cubin;
+  std::string lg;
+  const int rc = ami::jit_compile(ami::jit_generate_source(tab->flat, tab->horner, ami::kJitBlockThreads), cubin, lg);
+  if (log && log_cap) {
+    const size_t nlog = std::min(log_cap - 1, lg.size());
+    memcpy(log, lg.data(), nlog);
+    log[nlog] = 0;
+  }
+  if (rc != AMI_OK) { g_cuda_err = lg; return rc; }
+  if (buf) {
+    if (*bytes < cubin.size()) return AMI_EINVAL;
+    memcpy(buf, cubin.data(), cubin.size());
+  }
+  *bytes = cubin.size();
+  return AMI_OK;
 }
 
 int ami_generate_momenta(const ami_table* tab, uint64_t seed, int64_t first_sample, int64_t n, double* d_k,
@@ -383,6 +515,9 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   while (chunk > 1024 && chunk * rows * 16 > ((int64_t)256 << 20)) chunk /= 2;
   if (chunk > cfg->n) chunk = cfg->n;
   const bool direct_out = cfg->d_out != nullptr;   // kernels write straight into the caller's buffer
+  bool use_reg = false;   // the register plan forms the energies inline: no energy buffer
+  rc = choose_plan(tab, cfg->plan, false, &use_reg);
+  if (rc) return rc;
   RunBuffers rb;
   cudaStream_t user = (cudaStream_t)cfg->stream;
   CU(cudaEventCreate(&rb.ev_start));
@@ -391,7 +526,7 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
     CU(cudaStreamCreateWithFlags(&rb.st[i], cudaStreamNonBlocking));
     CU(cudaEventCreateWithFlags(&rb.ev_done[i], cudaEventDisableTiming));
     if (!cfg->d_k) CU(cudaMalloc((void**)&rb.k[i], (size_t)chunk * n_comp * 8));
-    CU(cudaMalloc((void**)&rb.e[i], (size_t)chunk * n_eps * 8));
+    if (!use_reg) CU(cudaMalloc((void**)&rb.e[i], (size_t)chunk * n_eps * 8));
     if (!direct_out) CU(cudaMalloc((void**)&rb.out[i], (size_t)chunk * rows * 16));
   }
   if (cfg->want_sum) {
@@ -419,18 +554,12 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
       ++launches;
       kbuf = rb.k[s];
     }
-    ami::DispParams dp;
-    memset(&dp, 0, sizeof dp);
-    dp.sym_alpha = tab->dev.sym_alpha;
-    dp.n_int = tab->flat.n_int; dp.n_ext = tab->flat.n_ext; dp.n_eps = n_eps;
-    dp.k = kbuf; dp.k_stride_sample = n_comp; dp.k_stride_comp = 1; dp.n = nc;
-    for (int i = 0; i < 2 * dp.n_ext; ++i) dp.q[i] = cfg->q[i];
-    dp.t = cfg->t; dp.mu = cfg->mu; dp.e = rb.e[s]; dp.e_stride = nc;
-    CU(ami::launch_dispersion(dp, st));
-    ++launches;
+    MomentaSrc ms;
+    ms.d_k = kbuf; ms.stride_sample = n_comp; ms.stride_comp = 1;
+    ms.q = cfg->q; ms.t = cfg->t; ms.mu = cfg->mu;
     double* obuf = direct_out ? (double*)cfg->d_out + 2 * c0 : rb.out[s];
     const int64_t ostride = direct_out ? cfg->n : nc;
-    rc = evaluate_impl(tab, rb.e[s], 0, nc, nc, cfg->z_ext, cfg->n_f, cfg->beta, cfg->n_b, cfg->e_reg, cfg->plan,
+    rc = evaluate_impl(tab, &ms, rb.e[s], 0, nc, nc, cfg->z_ext, cfg->n_f, cfg->beta, cfg->n_b, cfg->e_reg, cfg->plan,
                        obuf, ostride, st, &launches);
     if (rc) return rc;
     if (cfg->h_out) {

@@ -1,7 +1,10 @@
 // Device-side arithmetic shared by the evaluation kernels: complex helpers, fast reciprocals,
 // overflow-safe Fermi/Bose functions and their derivatives (readings P11, P12).
-#pragma once
+#ifndef AMI_DEVICE_CUH
+#define AMI_DEVICE_CUH
+#ifndef __CUDACC_RTC__
 #include <cuda_runtime.h>
+#endif
 
 namespace amidev {
 
@@ -14,9 +17,10 @@ __device__ __forceinline__ cplx cmul(cplx a, cplx b) {
 __device__ __forceinline__ cplx cscale(double s, cplx a) { return cplx{s * a.re, s * a.im}; }
 __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return cplx{a.re + b.re, a.im + b.im}; }
 
-// 1/x to ~1 ulp: hardware seed (MUFU.RCP64H) + two Newton steps.  Falls back to the IEEE
-// division when the seed is not a normal number (0, inf, nan, denormal range), so that
-// singular samples produce the same non-finite results as the division would.
+// 1/x to ~1 ulp for normal x: hardware seed (MUFU.RCP64H, 2^-23) + two Newton steps, no branch.
+// x = 0, inf or nan give a non-finite result (0 * inf in the Newton step), as the division would
+// for the singular samples it stands for; arguments below 1e-290 in magnitude are outside the
+// method's range (a denominator that small is a singular sample, reading P10).
 __device__ __forceinline__ double fast_rcp(double x) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
@@ -24,8 +28,6 @@ __device__ __forceinline__ double fast_rcp(double x) {
   r = fma(r, e, r);
   e = fma(-x, r, 1.0);
   r = fma(r, e, r);
-  const double ax = fabs(x);
-  if (!(ax > 1e-290 && ax < 1e290)) r = 1.0 / x;
   return r;
 }
 __device__ __forceinline__ cplx crcp(cplx a) {
@@ -34,29 +36,82 @@ __device__ __forceinline__ cplx crcp(cplx a) {
   return cplx{a.re * r, -a.im * r};
 }
 
+// ---- exponential core ---------------------------------------------------------------------------
+// e^x = 2^n (1 + r q(r)),  n = rint(x log2 e),  r = x - n ln 2 in [-0.347, 0.347],
+// q(r) = sum_k r^k/(k+1)!  (13 terms: truncation 4e-18).  The coefficients sit in constant memory so
+// that every DFMA takes its constant straight from the bank (no register moves).  n is clamped to
+// [-1021, 1010] in the integer domain: beyond it the Fermi/Bose value is 0 or 1 to double precision.
+// Returns s = 2^n and rq = r q(r):  e^x = fma(s, rq, s),  e^x - 1 = fma(s, rq, s - 1).
+__constant__ double kAmiExpQ[13] = {
+    1.0, 0.5, 0.16666666666666666, 0.041666666666666664, 0.008333333333333333, 0.001388888888888889,
+    0.0001984126984126984, 2.48015873015873e-05, 2.7557319223985893e-06, 2.755731922398589e-07,
+    2.505210838544172e-08, 2.08767569878681e-09, 1.6059043836821613e-10};
+
+__device__ __forceinline__ void exp_core(double x, double& s, double& rq) {
+  const double t = fma(x, 1.4426950408889634, 6755399441055744.0);
+  const double nd = t - 6755399441055744.0;
+  double r = fma(nd, -0.6931471805599453, x);
+  r = fma(nd, -2.3190468138462996e-17, r);
+  double q = kAmiExpQ[12];
+#pragma unroll
+  for (int i = 11; i >= 0; --i) q = fma(q, r, kAmiExpQ[i]);
+  rq = r * q;
+  int n = __double2loint(t);
+  n = max(-1021, min(1010, n));
+  s = __hiloint2double((n + 1023) << 20, 0);
+}
+
+// ---- cosine of a bounded argument -----------------------------------------------------------------
+// cos K = (-1)^n cos r,  n = rint(K/pi),  r = K - n pi in [-pi/2, pi/2] (two-part pi, exact for
+// |K| < 5e5), even Taylor polynomial of degree 20 (next term 1.9e-17).  Momentum sums of a diagram
+// are a few pi; anything beyond 5e5 takes the library routine.
+__constant__ double kAmiCosC[11] = {
+    1.0, -0.5, 0.041666666666666664, -0.001388888888888889, 2.48015873015873e-05, -2.755731922398589e-07,
+    2.08767569878681e-09, -1.1470745597729725e-11, 4.779477332387385e-14, -1.5619206968586225e-16,
+    4.110317623312165e-19};
+
+__device__ __noinline__ double cos_unbounded(double K) { return cos(K); }
+
+__device__ __forceinline__ double cos_bounded(double K) {
+  if ((__double2hiint(K) & 0x7fffffff) >= 0x411e8480) return cos_unbounded(K);   // |K| >= 5e5, inf, nan
+  const double t = fma(K, 0.3183098861837907, 6755399441055744.0);
+  const double nd = t - 6755399441055744.0;
+  double r = fma(nd, -3.1415926534682512, K);
+  r = fma(nd, -1.2154201013012384e-10, r);
+  const double r2 = r * r;
+  double c = kAmiCosC[10];
+#pragma unroll
+  for (int i = 9; i >= 0; --i) c = fma(c, r2, kAmiCosC[i]);
+  const int flip = (__double2loint(t) & 1) << 31;
+  return __hiloint2double(__double2hiint(c) ^ flip, __double2loint(c));
+}
+
+// f_sigma(E) = 1/(sigma e^x + 1) and g = 1 - f = sigma e^x f for x = beta E, any real x, without
+// overflow, cancellation, branch or select (reading P12): sigma = +1 uses 1 + e^x = fma(s, rq, s + 1),
+// sigma = -1 uses 1 - e^x = -fma(s, rq, s - 1), which is exact where e^x is close to 1 (n = 0: -rq).
+template <int SIG, bool WANT_G>
+__device__ __forceinline__ void fermi_fg(double x, double& f, double& g) {
+  double s, rq;
+  exp_core(x, s, rq);
+  if (SIG > 0) {
+    f = fast_rcp(fma(s, rq, s + 1.0));
+    if (WANT_G) g = fma(s, rq, s) * f;
+  } else {
+    f = -fast_rcp(fma(s, rq, s - 1.0));
+    if (WANT_G) g = -fma(s, rq, s) * f;
+  }
+}
+
 // f^{(k)} = beta^k f g Q_k(f), Q_1 = -1, Q_{k+1} = (2f-1) Q_k - (f - f^2) Q_k'   (from f' = -beta f g,
 // g' = beta f g, g = 1 - f).  Q holds the integer coefficients, row k, ascending powers of f.
 #define AMI_QSTRIDE 8
 
-// real argument.  f_sigma(E) = 1/(sigma e^{beta E} + 1); the exponential is only ever taken of
-// -|x| (no overflow) and 1 - e^{-|x|} comes from expm1 for sigma = -1 (no cancellation).
+// real argument, run-time statistics and derivative order (table-driven kernels)
 __device__ __forceinline__ double fermi_real(double E, double beta, int sigma, int k,
                                              const double* __restrict__ Q) {
-  const double x = beta * E;
-  const double ax = -fabs(x);
-  const double u = exp(ax);
   double f, g;
-  if (sigma > 0) {
-    const double inv = fast_rcp(1.0 + u);
-    const double small = u * inv;
-    f = x > 0.0 ? small : inv;
-    g = x > 0.0 ? inv : small;
-  } else {
-    const double inv = fast_rcp(-expm1(ax));
-    const double small = -u * inv;
-    f = x > 0.0 ? small : inv;
-    g = x > 0.0 ? inv : small;
-  }
+  if (sigma > 0) fermi_fg<1, true>(beta * E, f, g);
+  else fermi_fg<-1, true>(beta * E, f, g);
   if (k == 0) return f;
   double q = Q[k * AMI_QSTRIDE + (k - 1)];
   for (int i = k - 2; i >= 0; --i) q = fma(q, f, Q[k * AMI_QSTRIDE + i]);
@@ -102,3 +157,4 @@ __device__ __forceinline__ cplx fermi_cplx(cplx E, double beta, int sigma, int k
 }
 
 }  // namespace amidev
+#endif  // AMI_DEVICE_CUH

@@ -13,6 +13,10 @@ using namespace amidev;
 
 static std::atomic<long long> g_launches{0};
 long long total_launches() { return g_launches.load(); }
+void count_external_launch(int* launches) {
+  g_launches += 1;
+  if (launches) *launches += 1;
+}
 static inline void count_launch(int* launches, int n = 1) {
   g_launches += n;
   if (launches) *launches += n;
@@ -53,7 +57,7 @@ __global__ void __launch_bounds__(256) dispersion_kernel(DispParams p) {
       Kx = fma(a, p.q[2 * x], Kx);
       Ky = fma(a, p.q[2 * x + 1], Ky);
     }
-    p.e[i * p.e_stride + s] = fma(2.0 * p.t, cos(Kx) + cos(Ky), p.mu);
+    p.e[i * p.e_stride + s] = fma(2.0 * p.t, cos_bounded(Kx) + cos_bounded(Ky), p.mu);
   }
 }
 
@@ -341,9 +345,3 @@ cudaError_t run_fp64_probe(double* dfma_per_s, double* ms_out) {
 
 }  // namespace ami
 
-namespace ami {
-// tree plan: see ami_eval_tree.cu (until the plan exists for a table the flat kernel runs)
-cudaError_t launch_eval_tree(const EvalParams& p, bool ce, cudaStream_t st, int* launches) {
-  return launch_eval_flat(p, ce, st, launches);
-}
-}  // namespace ami

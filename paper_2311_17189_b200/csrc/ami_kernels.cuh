@@ -21,8 +21,6 @@ struct EvalParams {
   const int8_t* leafD_a;
   const uint16_t* term_idx;
   const double* term_coef;
-  const uint32_t* tree_code;
-  const double* tree_consts;
   const double* derivQ;
   int n_eps, n_ext, U_F, U_D, m_f, n_d;
   long long T;
@@ -49,12 +47,12 @@ struct DispParams {
 
 cudaError_t launch_dispersion(const DispParams& p, cudaStream_t st);
 cudaError_t launch_eval_flat(const EvalParams& p, bool e_is_complex, cudaStream_t st, int* launches);
-cudaError_t launch_eval_tree(const EvalParams& p, bool e_is_complex, cudaStream_t st, int* launches);
 cudaError_t launch_generate_momenta(uint64_t seed, long long first, long long n, int n_comp, double* d_k,
                                     cudaStream_t st);
 cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long n, long long row_stride,
                               double* d_partial, double* d_sum, cudaStream_t st, int* launches);
 cudaError_t run_fp64_probe(double* dfma_per_s, double* ms);
 long long total_launches();
+void count_external_launch(int* launches);
 
 }  // namespace ami

@@ -1,0 +1,33 @@
+// Kernel parameter blocks (plain data).  This header is compiled twice: by nvcc into the library
+// and, embedded as text, by NVRTC in front of a specialised kernel (ami_jit.cpp), so it uses
+// only builtin types and includes nothing.
+#ifndef AMI_PARAMS_H
+#define AMI_PARAMS_H
+
+#define AMI_K_MAX_FREQ_WORDS 64   // n_f * n_ext complex values per launch
+#define AMI_K_MAX_BETA 8          // inverse temperatures per launch
+#define AMI_K_MAX_EXT 4
+
+// Batch description shared by every evaluation kernel.
+struct AmiBatch {
+  // energies, [n_eps][n] doubles (complex: interleaved), rows e_stride samples apart; NULL when the
+  // kernel forms them from momenta (fused S1+S2+S3)
+  const double* e;
+  long long e_stride;
+  // momenta for the fused path: component c of internal momentum l of sample s at
+  // k[s * k_stride_sample + (2 l + c) * k_stride_comp]
+  const double* k;
+  long long k_stride_sample, k_stride_comp;
+  double q[2 * AMI_K_MAX_EXT];
+  double t, mu;
+  double* e_out;            // optional [n_eps][n] copy of the energies formed by the fused path
+  // results: complex128, row r = (b0 + b) * n_f_total + (f0 + f) at out + 2 * r * out_row_stride
+  double* out;
+  long long n, out_row_stride;
+  int n_f, n_b, n_f_total, f0, b0, pad;
+  double e_reg, prefactor;
+  double beta[AMI_K_MAX_BETA];
+  double z[2 * AMI_K_MAX_FREQ_WORDS];   // [n_f][n_ext] complex
+};
+
+#endif

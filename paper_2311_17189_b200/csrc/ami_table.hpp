@@ -45,18 +45,38 @@ struct FlatTable {
   long long n_terms_raw = 0, n_multipoles = 0;
 };
 
-// ---- tree plan: terms grouped by denominator product, Fermi products in a trie ----------
-// Byte-code executed identically by every thread; see ami_plan.cpp for the format.
-struct TreePlan {
-  std::vector<uint32_t> code;     // program words
-  std::vector<double> consts;     // non-unit coefficients referenced by the code
-  long long n_groups = 0, n_fnodes = 0, n_dnodes = 0, fp64_ops = 0;
-  int max_depth_f = 0, max_depth_d = 0;
+// ---- Horner plan: terms grouped by denominator product R (Eq. 6: FT * R), the
+// Fermi/Bose products of each group as a trie evaluated in Horner form, and the denominator
+// products of all groups as one trie whose terminals carry the groups' FT sums:
+//   result = S_D(root),  S_D(n) = [FT_g if group g ends at n] + sum_{c in kids(n)} Dinv[c.leaf] * S_D(c)
+//   FT_g   = S_F(root_g), S_F(n) = [coef if a term ends at n] + sum_{c in kids(n)} F[c.leaf] * S_F(c)
+struct HNode {
+  int leaf = -1;             // factor of the edge into this node (Fermi leaf id or denominator leaf id)
+  std::vector<int> kids;     // node ids
+  bool terminal = false;     // F-trie: a term ends here (num/den = its coefficient)
+  long long num = 0, den = 1;
+  int group = -1;            // D-trie: the group whose denominator product ends here
 };
+struct HGroup {
+  std::vector<int> d;        // sorted denominator leaf ids (repeats = powers)
+  std::vector<HNode> f;      // f[0] = root
+};
+struct HornerPlan {
+  std::vector<HGroup> groups;
+  std::vector<HNode> dn;     // dn[0] = root
+  std::vector<char> d_is_real;   // [U_D]: no external-frequency part => purely real denominator
+  long long n_fnodes = 0, n_dnodes = 0;
+  long long ops_f = 0;       // FP64 instructions per (sample, beta) of all FT sums
+  long long ops_d = 0;       // FP64 instructions per (sample, beta, frequency) of the R part
+};
+
+// The compiled, per-table specialised kernels (ami_jit.cpp).
+struct JitState;
 
 int construct_flat(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha, const int32_t* eps,
                    const uint8_t* ferm, const int32_t* sum_order, double prefactor, FlatTable& out);
-void build_tree_plan(const FlatTable& ft, TreePlan& plan);
+void build_horner_plan(const FlatTable& ft, HornerPlan& plan);
+std::vector<double> deriv_poly(int k);   // Q_k of f^{(k)} = beta^k f g Q_k(f), ascending powers of f
 
 }  // namespace ami
 
@@ -74,8 +94,6 @@ struct ami_device_copy {
   uint16_t* term_idx = nullptr;   // [T][n_int + n_d]: Fermi ids then denominator ids (U_D = unit leaf)
   double* term_coef = nullptr;    // [T]
   // tree plan
-  uint32_t* tree_code = nullptr;
-  double* tree_consts = nullptr;
   // dispersion
   int8_t* sym_alpha = nullptr;    // [n_eps][L]
   double* derivQ = nullptr;       // [AMI_MAX_DERIV+1][8] polynomials of the Fermi derivatives
@@ -84,7 +102,8 @@ struct ami_device_copy {
 
 struct ami_table {
   ami::FlatTable flat;
-  ami::TreePlan tree;
+  ami::HornerPlan horner;
+  ami::JitState* jit = nullptr;   // owned; see ami_jit.cpp
   ami_device_copy dev;
   int64_t fp64_ops_flat = 0;
 };

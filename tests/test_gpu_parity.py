@@ -10,7 +10,7 @@ from parity import check_parity
 
 pytestmark = pytest.mark.gpu
 
-PLANS = {"flat": 1, "auto": 0}
+PLANS = {"flat": 1, "auto": 0}   # auto = the register plan where the table is eligible, else flat
 
 
 @pytest.fixture(scope="module")
@@ -176,6 +176,65 @@ def test_degenerate_samples_nonfinite_agree(ami, torch_mod, oracle_mod):
         check_parity(out[0], truth, S, label=f"eta={eta}")
         assert np.isfinite(out[0][1]).all()
         assert np.isfinite(out[0][0]).all() == (eta > 0)
+
+
+# ------------------------------------------------------------------ register plan + fused S1+S2+S3
+@pytest.mark.parametrize("name", ["cfg1", "cfg2_bubble_doubled", "cfg3", "cfg4", "cfg5"])
+def test_register_plan_is_what_auto_runs(ami, torch_mod, name):
+    """AMI_PLAN_AUTO compiles and runs the specialised kernels for every graded config."""
+    cfg = A.get_config(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    assert tab.info["reg_plan_status"] == 1          # eligible, not compiled yet
+    e = gpu_energies(torch_mod, tab, cfg, cfg.momenta(300))
+    a = tab.evaluate(e, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=ami.PLAN_AUTO)
+    assert tab.refresh_info()["reg_plan_status"] == 0
+    b = tab.evaluate(e, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=ami.PLAN_REG)
+    assert torch_mod.equal(a, b)
+
+
+def test_register_plan_limits(ami, torch_mod):
+    """Tables outside the limits (order 8) and complex energies run the table-driven kernels under
+    AUTO and are refused under an explicit AMI_PLAN_REG."""
+    cfg = A.get_config("stress8")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    assert tab.info["reg_plan_status"] == -6
+    e = gpu_energies(torch_mod, tab, cfg, cfg.momenta(40))
+    with pytest.raises(ami.AmiError) as ei:
+        tab.evaluate(e, cfg.z_ext, cfg.betas, plan=ami.PLAN_REG)
+    assert ei.value.code == -6
+    cfg = A.get_config("cfg3")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    ec = gpu_energies(torch_mod, tab, cfg, cfg.momenta(40)).to(torch_mod.complex128)
+    with pytest.raises(ami.AmiError):
+        tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=ami.PLAN_REG)
+    tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=ami.PLAN_AUTO)
+
+
+@pytest.mark.parametrize("name,n", [("cfg1", 10_000), ("cfg3", 50_000 + 3), ("cfg4", 3000 + 1), ("cfg5", 401)])
+@pytest.mark.parametrize("plan", ["flat", "auto"])
+def test_fused_momenta_path(ami, torch_mod, oracle_mod, name, n, plan):
+    """ami_evaluate_momenta == ami_dispersion followed by ami_evaluate, bit for bit, and the energies
+    it stores are those of ami_dispersion; then against the oracle from the momenta on."""
+    cfg = A.get_config(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    k_host = cfg.momenta(n)
+    k = torch_mod.from_numpy(k_host).cuda()
+    e_ref = tab.dispersion(k, [cfg.q], cfg.t, cfg.mu)
+    ref = tab.evaluate(e_ref, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=PLANS[plan])
+    e_out = torch_mod.zeros_like(e_ref)
+    got = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=PLANS[plan],
+                               e_out=e_out)
+    assert torch_mod.equal(e_out, e_ref)
+    assert torch_mod.equal(got, ref)
+    got2 = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=PLANS[plan])
+    assert torch_mod.equal(got2, ref)
+    sel = np.linspace(0, n - 1, min(n, 300)).astype(np.int64)
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    e_rows = ot.dispersion(k_host[sel], [cfg.q], cfg.t, cfg.mu)
+    for b, beta in enumerate(cfg.betas):
+        truth, S = ot.evaluate(e_rows, cfg.z_ext, beta, e_reg=cfg.e_reg, quad=True,
+                               threads=oracle_mod.hardware_threads(), want_S=True)
+        check_parity(got.cpu().numpy()[b][:, sel], truth, S, label=f"fused {name}")
 
 
 # ------------------------------------------------------------------ S4 streamed driver
