@@ -39,6 +39,7 @@ def parse_args():
     ap.add_argument("--n", type=int, default=0, help="override samples per step per GPU")
     ap.add_argument("--plan", default="auto", choices=["auto", "flat", "reg"])
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads and the CPU baseline")
+    ap.add_argument("--no-graph", action="store_true", help="launch every step from Python instead of one CUDA graph")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -49,7 +50,7 @@ def parse_args():
 class ClockSampler:
     BAD = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown")
 
-    def __init__(self, index=0, period=0.05):
+    def __init__(self, index=0, period=0.01):
         self.index, self.period = index, period
         self.samples, self.reasons = [], set()
         self.sm_max = None
@@ -106,17 +107,17 @@ class ClockSampler:
 #     + N_b U_F c_fermi                          [S2: Fermi/Bose leaves, once per beta]
 #     + N_b N_f U_D c_den                        [S2: complex reciprocals]
 #     + N_b ops_FT + N_b N_f ops_R               [S3: Horner plan]   or   N_b N_f ops_flat  [S3: flat plan]
-# c_* = FP64-pipe instructions of the leaf routines on their common path as compiled for sm_100a,
-# counted in the SASS (DESIGN.md table "leaf costs"); cross-checked against ncu
-# sm__inst_executed_pipe_fp64 in profiles/.
+# c_* = FP64-pipe instructions of the leaf routines on their common path as compiled for sm_100a
+# (cos 15, Fermi/Bose 24, complex reciprocal 8, plus the integer-coefficient sums of their arguments);
+# cross-checked against the executed-instruction counts of ncu's source page in profiles/.
 # ------------------------------------------------------------------------------------------------
-C_COS, C_FERMI, C_DEN = 18, 24, 11
-
-
 def fp64_work_per_sample(info, n_f, n_b, reg):
-    disp = info["n_eps"] * (2 * C_COS + 2)
-    fermi = n_b * info["n_fermi_leaves"] * C_FERMI
-    dens = n_b * n_f * info["n_den_leaves"] * C_DEN
+    """FP64-pipe instruction slots per sample of the representation executed; every count comes from
+    ami_table_info (the library counts the instructions its generator emits plus the common-path cost
+    of each leaf routine)."""
+    disp = int(info["fp64_ops_dispersion"])
+    fermi = n_b * int(info["fp64_ops_leaf_fermi"]) + int(info["fp64_ops_combos"])
+    dens = n_b * n_f * int(info["fp64_ops_leaf_den"])
     if reg:
         ft = int(info["fp64_ops_tree_fermi"])
         terms = n_b * ft + n_b * n_f * (int(info["fp64_ops_tree"]) - ft)
@@ -217,7 +218,7 @@ def run_reference(args, dist, rank, world):
 # ------------------------------------------------------------------------------------------------
 # our arm: the CUDA path through the C ABI
 # ------------------------------------------------------------------------------------------------
-def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, sample_clocks):
+def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, sample_clocks, use_graph=True):
     """Times `steps` passes of S1 + S2/S3 over rotating resident momentum batches (the set of inputs is
     larger than L2, so no batch is served from cache).  Returns a dict of device-timed results."""
     from paper_2311_17189_b200 import sharding
@@ -258,29 +259,59 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
     for i in range(warmup):
         step(i)
     torch.cuda.synchronize()
+    # The fused step is one short kernel (tens of microseconds), less than a Python -> ctypes launch
+    # costs on the host, so the K timed steps are captured once into a CUDA graph and replayed: the
+    # device then runs them back to back, as a C caller's loop would.
+    graph = None
+    l0 = pkg.kernel_launches()
+    if reg and use_graph:
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            for i in range(steps):
+                step(warmup + i)
+        launches = pkg.kernel_launches() - l0     # kernels recorded in the graph = launched per replay
+        graph.replay()                            # one untimed replay: graph upload
+        torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
     sampler = ClockSampler(torch.cuda.current_device()) if sample_clocks else None
     if sampler:
         sampler.start()
-    l0 = pkg.kernel_launches()
-    t_beg.record()
-    for i in range(steps):
-        step(warmup + i, ev[i])
-    t_end.record()
-    torch.cuda.synchronize()
-    launches = pkg.kernel_launches() - l0
+    if graph is not None:
+        if sampler:
+            # the timed replay lasts about a millisecond; keep the same load on the GPU for ~0.2 s before
+            # it (extra, untimed warm-up) so that the clock samples are taken under this load
+            t_load = time.perf_counter()
+            while time.perf_counter() - t_load < 0.2:
+                graph.replay()
+            torch.cuda.synchronize()
+        t_beg.record()
+        graph.replay()
+        t_end.record()
+        torch.cuda.synchronize()
+    else:
+        l0 = pkg.kernel_launches()
+        t_beg.record()
+        for i in range(steps):
+            step(warmup + i, ev[i])
+        t_end.record()
+        torch.cuda.synchronize()
+        launches = pkg.kernel_launches() - l0
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
     clocks = sampler.stop() if sampler else None
-    total_ms = sharding.max_over_ranks(t_beg.elapsed_time(t_end), dist)
-    disp_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
-    eval_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
+    total_ms_local = t_beg.elapsed_time(t_end)
+    total_ms = sharding.max_over_ranks(total_ms_local, dist)
+    if graph is not None:
+        disp_ms, eval_ms = 0.0, total_ms_local / steps
+    else:
+        disp_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+        eval_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
     checksum = complex(out[0, 0, : min(n, 1024)].sum().item())
     return {"tab": tab, "info": info, "fused": reg, "total_ms": total_ms, "disp_ms": disp_ms, "eval_ms": eval_ms,
-            "launches": launches, "clocks": clocks, "n_rot": n_rot, "checksum": checksum,
+            "launches": launches, "clocks": clocks, "graph": graph is not None, "n_rot": n_rot, "checksum": checksum,
             "bytes_in": bytes_in, "bytes_e": n * n_eps * 8, "bytes_out": n * n_f * n_b * 16}
 
 
@@ -372,7 +403,8 @@ def run_ours(args, dist, rank, local, world):
     dfma_per_s, _ = pkg.fp64_peak_probe(local)
     peaks = load_measured_peaks()
 
-    res = time_workload(pkg, torch, cfg, n, args.steps, args.warmup, plan, first, dist, sample_clocks=True)
+    res = time_workload(pkg, torch, cfg, n, args.steps, args.warmup, plan, first, dist, sample_clocks=True,
+                        use_graph=not args.no_graph)
     info = res["info"]
     T = int(info["n_terms"])
     plan_ops, plan_name = plan_ops_for(info, args.plan)
@@ -396,7 +428,8 @@ def run_ours(args, dist, rank, local, world):
                    "l2": f"inputs rotated over {res['n_rot']} resident batches (> L2)",
                    "parallelism": "replicas" if world == 1 else f"sample-sharded x{world}, no collective"},
         "kernels": {"dominant_ms": res["eval_ms"], "ami_dispersion_ms": None if res["fused"] else res["disp_ms"],
-                    "dispersion": disp, "launches_per_step": res["launches"] / max(1, args.steps)},
+                    "dispersion": disp, "launches_per_step": res["launches"] / max(1, args.steps),
+                    "timed_as": "one CUDA graph of K steps" if res["graph"] else "K launches from the host"},
         "roofline": roof,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                 "steps": e2e_steps, "chunks_per_step": e2e["chunks"], "api": "ami_run(h_k -> h_out)"},
@@ -411,12 +444,13 @@ def run_ours(args, dist, rank, local, world):
             if name == cfg.name:
                 continue
             c2 = A.get_config(name)
-            r2 = time_workload(pkg, torch, c2, c2.n_samples, 6, 3, plan, 0, None, sample_clocks=False)
+            r2 = time_workload(pkg, torch, c2, c2.n_samples, 20, 3, plan, 0, None, sample_clocks=False,
+                               use_graph=not args.no_graph)
             i2 = r2["info"]
             ops2, pn2 = plan_ops_for(i2, args.plan)
             f2, b2 = len(c2.z_ext), len(c2.betas)
             roof2, disp2 = roofline_objects(r2, c2.n_samples, f2, b2, ops2, peaks, dfma_per_s)
-            ms2 = r2["total_ms"] / 6
+            ms2 = r2["total_ms"] / 20
             others[name] = {"T_flat": int(i2["n_terms"]), "samples": c2.n_samples, "n_freq": f2, "n_beta": b2,
                             "plan": pn2, "ms_per_step": ms2, "eval_ms": r2["eval_ms"], "disp_ms": r2["disp_ms"],
                             "term_evals_per_s": int(i2["n_terms"]) * c2.n_samples * f2 * b2 / (ms2 * 1e-3),

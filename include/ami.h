@@ -87,6 +87,10 @@ typedef struct ami_info {
   int64_t fp64_ops_flat;    /* FP64 instructions per (sample,frequency,beta) of the flat term loop */
   int64_t fp64_ops_tree;    /* same for the Horner plan with n_f = n_b = 1 (FT part + R part) */
   int64_t fp64_ops_tree_fermi; /* its FT part alone: done once per (sample,beta), not per frequency */
+  int64_t fp64_ops_leaf_fermi; /* FP64 instructions per (sample,beta) of all Fermi/Bose leaves (common path) */
+  int64_t fp64_ops_leaf_den;   /* FP64 instructions per (sample,beta,frequency) of the complex reciprocals */
+  int64_t fp64_ops_dispersion; /* FP64 instructions per sample of ami_dispersion */
+  int64_t fp64_ops_combos;     /* FP64 instructions done once per sample: distinct energy combinations of the leaves, reciprocals of purely real denominators */
   int32_t has_device_copy;
   int32_t reg_plan_status;  /* 0 = specialised kernels loaded, 1 = eligible, not compiled yet,
                                AMI_EUNSUPPORTED = table outside the register plan's limits, other < 0 = error */

@@ -33,7 +33,8 @@ class ami_info(C.Structure):
                                          "max_deriv", "max_den_per_term")] + \
                [(n, C.c_int64) for n in ("n_terms", "n_terms_raw", "n_multipoles", "n_groups", "n_tree_nodes",
                                          "n_den_nodes", "table_bytes", "fp64_ops_flat", "fp64_ops_tree",
-                                         "fp64_ops_tree_fermi")] + \
+                                         "fp64_ops_tree_fermi", "fp64_ops_leaf_fermi", "fp64_ops_leaf_den",
+                                         "fp64_ops_dispersion", "fp64_ops_combos")] + \
                [("has_device_copy", C.c_int32), ("reg_plan_status", C.c_int32)]
 
 

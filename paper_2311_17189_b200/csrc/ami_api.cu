@@ -1,6 +1,7 @@
 // The C ABI of include/ami.h: argument checking, device residency, launches, streamed driver.
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -10,6 +11,7 @@
 namespace ami {
 long long flat_fp64_ops(const FlatTable& ft);
 }
+static void free_run_workspace(ami_table* tab);   // defined next to ami_run
 
 namespace {
 
@@ -166,6 +168,7 @@ int ami_construct(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha
 void ami_table_destroy(ami_table* tab) {
   if (!tab) return;
   ami::jit_destroy(tab);
+  free_run_workspace(tab);
   free_device_copy(tab->dev);
   delete tab;
 }
@@ -189,6 +192,10 @@ int ami_table_info(const ami_table* tab, ami_info* info) {
   info->fp64_ops_flat = tab->fp64_ops_flat;
   info->fp64_ops_tree = tab->horner.ops_f + tab->horner.ops_d;
   info->fp64_ops_tree_fermi = tab->horner.ops_f;
+  info->fp64_ops_leaf_fermi = tab->horner.ops_leaf_f;
+  info->fp64_ops_leaf_den = tab->horner.ops_leaf_d;
+  info->fp64_ops_dispersion = tab->horner.ops_disp;
+  info->fp64_ops_combos = tab->horner.ops_combo;
   info->has_device_copy = tab->dev.device >= 0;
   info->reg_plan_status = !ami::jit_eligible(ft, tab->horner) ? AMI_EUNSUPPORTED
                           : (tab->jit ? ami::jit_status(tab) : 1);
@@ -472,14 +479,49 @@ int ami_fp64_peak_probe(int device, double* dfma_per_s, double* elapsed_ms) {
 // ---------------------------------------------------------------------------------------------
 namespace {
 
+// Workspace of the streamed driver, cached in the table between calls: two streams with their
+// events and device buffers that only ever grow (allocation costs more than a chunk's kernels).
 struct RunBuffers {
+  std::mutex mu;           // one ami_run at a time per table
   cudaStream_t st[2] = {nullptr, nullptr};
   cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_done[2] = {nullptr, nullptr};
   double* k[2] = {nullptr, nullptr};
   double* e[2] = {nullptr, nullptr};
   double* out[2] = {nullptr, nullptr};
+  size_t cap_k = 0, cap_e = 0, cap_out = 0, cap_sum = 0;
   double* partial = nullptr;
   double* sum = nullptr;
+  int init() {
+    if (ev_start) return AMI_OK;
+    CU(cudaEventCreate(&ev_start));
+    CU(cudaEventCreate(&ev_stop));
+    for (int i = 0; i < 2; ++i) {
+      CU(cudaStreamCreateWithFlags(&st[i], cudaStreamNonBlocking));
+      CU(cudaEventCreateWithFlags(&ev_done[i], cudaEventDisableTiming));
+    }
+    return AMI_OK;
+  }
+  static int grow(double** p, size_t* cap, size_t bytes) {
+    if (bytes <= *cap) return AMI_OK;
+    cudaFree(*p);
+    *p = nullptr;
+    *cap = 0;
+    CU(cudaMalloc((void**)p, bytes));
+    *cap = bytes;
+    return AMI_OK;
+  }
+  int reserve(size_t bk, size_t be, size_t bo, size_t bs) {
+    int rc;
+    for (int i = 0; i < 2; ++i) {
+      size_t ck = cap_k, ce = cap_e, co = cap_out;
+      if ((rc = grow(&k[i], &ck, bk)) || (rc = grow(&e[i], &ce, be)) || (rc = grow(&out[i], &co, bo))) return rc;
+      if (i == 1) { cap_k = ck; cap_e = ce; cap_out = co; }
+    }
+    size_t c1 = cap_sum, c2 = cap_sum;
+    if ((rc = grow(&partial, &c1, bs * 64)) || (rc = grow(&sum, &c2, bs))) return rc;
+    cap_sum = std::max(cap_sum, bs);
+    return AMI_OK;
+  }
   ~RunBuffers() {
     for (int i = 0; i < 2; ++i) {
       if (st[i]) cudaStreamDestroy(st[i]);
@@ -491,6 +533,25 @@ struct RunBuffers {
     cudaFree(partial); cudaFree(sum);
   }
 };
+
+}  // namespace
+
+static void free_run_workspace(ami_table* tab) {
+  if (!tab->run_ws) return;
+  if (tab->dev.device >= 0) cudaSetDevice(tab->dev.device);
+  delete static_cast<RunBuffers*>(tab->run_ws);
+  tab->run_ws = nullptr;
+}
+
+namespace {
+
+RunBuffers* workspace_of(const ami_table* tab) {
+  static std::mutex create_mu;
+  std::lock_guard<std::mutex> lk(create_mu);
+  ami_table* t = const_cast<ami_table*>(tab);
+  if (!t->run_ws) t->run_ws = new RunBuffers;
+  return static_cast<RunBuffers*>(t->run_ws);
+}
 
 }  // namespace
 
@@ -510,7 +571,9 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
     if (stats) *stats = local;
     return AMI_OK;
   }
-  int64_t chunk = cfg->chunk ? cfg->chunk : (int64_t)1 << 20;
+  // default chunk: small enough that the host copies of one chunk overlap the kernels of the next
+  const bool host_io = cfg->h_k || cfg->h_out;
+  int64_t chunk = cfg->chunk ? cfg->chunk : (host_io ? (int64_t)1 << 17 : (int64_t)1 << 20);
   // keep a chunk's output below ~256 MiB
   while (chunk > 1024 && chunk * rows * 16 > ((int64_t)256 << 20)) chunk /= 2;
   if (chunk > cfg->n) chunk = cfg->n;
@@ -518,22 +581,14 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   bool use_reg = false;   // the register plan forms the energies inline: no energy buffer
   rc = choose_plan(tab, cfg->plan, false, &use_reg);
   if (rc) return rc;
-  RunBuffers rb;
+  RunBuffers& rb = *workspace_of(tab);
+  std::lock_guard<std::mutex> run_lock(rb.mu);
   cudaStream_t user = (cudaStream_t)cfg->stream;
-  CU(cudaEventCreate(&rb.ev_start));
-  CU(cudaEventCreate(&rb.ev_stop));
-  for (int i = 0; i < 2; ++i) {
-    CU(cudaStreamCreateWithFlags(&rb.st[i], cudaStreamNonBlocking));
-    CU(cudaEventCreateWithFlags(&rb.ev_done[i], cudaEventDisableTiming));
-    if (!cfg->d_k) CU(cudaMalloc((void**)&rb.k[i], (size_t)chunk * n_comp * 8));
-    if (!use_reg) CU(cudaMalloc((void**)&rb.e[i], (size_t)chunk * n_eps * 8));
-    if (!direct_out) CU(cudaMalloc((void**)&rb.out[i], (size_t)chunk * rows * 16));
-  }
-  if (cfg->want_sum) {
-    CU(cudaMalloc((void**)&rb.partial, (size_t)rows * 64 * 16));
-    CU(cudaMalloc((void**)&rb.sum, (size_t)rows * 16));
-    CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 16, user));
-  }
+  if ((rc = rb.init())) return rc;
+  if ((rc = rb.reserve(cfg->d_k ? 0 : (size_t)chunk * n_comp * 8, use_reg ? 0 : (size_t)chunk * n_eps * 8,
+                       direct_out ? 0 : (size_t)chunk * rows * 16, cfg->want_sum ? (size_t)rows * 16 : 0)))
+    return rc;
+  if (cfg->want_sum) CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 16, user));
   CU(cudaEventRecord(rb.ev_start, user));
   CU(cudaStreamWaitEvent(rb.st[0], rb.ev_start, 0));
   CU(cudaStreamWaitEvent(rb.st[1], rb.ev_start, 0));

@@ -30,6 +30,22 @@ __device__ __forceinline__ double fast_rcp(double x) {
   r = fma(r, e, r);
   return r;
 }
+// The same for N independent arguments, step by step across the batch: the Newton chain is four
+// dependent DFMAs, so a batch gives the FP64 pipe N independent instructions per step.
+template <int N>
+__device__ __forceinline__ void fast_rcp_n(double (&x)[N]) {
+  double r[N], e[N];
+#pragma unroll
+  for (int j = 0; j < N; ++j) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r[j]) : "d"(x[j]));
+#pragma unroll
+  for (int j = 0; j < N; ++j) e[j] = fma(-x[j], r[j], 1.0);
+#pragma unroll
+  for (int j = 0; j < N; ++j) r[j] = fma(r[j], e[j], r[j]);
+#pragma unroll
+  for (int j = 0; j < N; ++j) e[j] = fma(-x[j], r[j], 1.0);
+#pragma unroll
+  for (int j = 0; j < N; ++j) x[j] = fma(r[j], e[j], r[j]);
+}
 __device__ __forceinline__ cplx crcp(cplx a) {
   const double n = fma(a.re, a.re, a.im * a.im);
   const double r = fast_rcp(n);
@@ -47,18 +63,36 @@ __constant__ double kAmiExpQ[13] = {
     0.0001984126984126984, 2.48015873015873e-05, 2.7557319223985893e-06, 2.755731922398589e-07,
     2.505210838544172e-08, 2.08767569878681e-09, 1.6059043836821613e-10};
 
-__device__ __forceinline__ void exp_core(double x, double& s, double& rq) {
-  const double t = fma(x, 1.4426950408889634, 6755399441055744.0);
-  const double nd = t - 6755399441055744.0;
-  double r = fma(nd, -0.6931471805599453, x);
-  r = fma(nd, -2.3190468138462996e-17, r);
-  double q = kAmiExpQ[12];
+template <int N>
+__device__ __forceinline__ void exp_core_n(const double (&x)[N], double (&s)[N], double (&rq)[N]) {
+  double t[N], r[N], q[N];
 #pragma unroll
-  for (int i = 11; i >= 0; --i) q = fma(q, r, kAmiExpQ[i]);
-  rq = r * q;
-  int n = __double2loint(t);
-  n = max(-1021, min(1010, n));
-  s = __hiloint2double((n + 1023) << 20, 0);
+  for (int j = 0; j < N; ++j) t[j] = fma(x[j], 1.4426950408889634, 6755399441055744.0);
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const double nd = t[j] - 6755399441055744.0;
+    r[j] = fma(nd, -0.6931471805599453, x[j]);
+    r[j] = fma(nd, -2.3190468138462996e-17, r[j]);
+    q[j] = kAmiExpQ[12];
+  }
+#pragma unroll
+  for (int i = 11; i >= 0; --i) {
+#pragma unroll
+    for (int j = 0; j < N; ++j) q[j] = fma(q[j], r[j], kAmiExpQ[i]);
+  }
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    rq[j] = r[j] * q[j];
+    int n = __double2loint(t[j]);
+    n = max(-1021, min(1010, n));
+    s[j] = __hiloint2double((n + 1023) << 20, 0);
+  }
+}
+__device__ __forceinline__ void exp_core(double x, double& s, double& rq) {
+  double xa[1] = {x}, sa[1], ra[1];
+  exp_core_n<1>(xa, sa, ra);
+  s = sa[0];
+  rq = ra[0];
 }
 
 // ---- cosine of a bounded argument -----------------------------------------------------------------
@@ -72,18 +106,42 @@ __constant__ double kAmiCosC[11] = {
 
 __device__ __noinline__ double cos_unbounded(double K) { return cos(K); }
 
-__device__ __forceinline__ double cos_bounded(double K) {
-  if ((__double2hiint(K) & 0x7fffffff) >= 0x411e8480) return cos_unbounded(K);   // |K| >= 5e5, inf, nan
-  const double t = fma(K, 0.3183098861837907, 6755399441055744.0);
-  const double nd = t - 6755399441055744.0;
-  double r = fma(nd, -3.1415926534682512, K);
-  r = fma(nd, -1.2154201013012384e-10, r);
-  const double r2 = r * r;
-  double c = kAmiCosC[10];
+template <int N>
+__device__ __forceinline__ void cos_bounded_n(double (&K)[N]) {
+  double t[N], r[N], r2[N], c[N];
 #pragma unroll
-  for (int i = 9; i >= 0; --i) c = fma(c, r2, kAmiCosC[i]);
-  const int flip = (__double2loint(t) & 1) << 31;
-  return __hiloint2double(__double2hiint(c) ^ flip, __double2loint(c));
+  for (int j = 0; j < N; ++j) t[j] = fma(K[j], 0.3183098861837907, 6755399441055744.0);
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const double nd = t[j] - 6755399441055744.0;
+    r[j] = fma(nd, -3.1415926534682512, K[j]);
+    r[j] = fma(nd, -1.2154201013012384e-10, r[j]);
+    r2[j] = r[j] * r[j];
+    c[j] = kAmiCosC[10];
+  }
+#pragma unroll
+  for (int i = 9; i >= 0; --i) {
+#pragma unroll
+    for (int j = 0; j < N; ++j) c[j] = fma(c[j], r2[j], kAmiCosC[i]);
+  }
+  double v[N];
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const int flip = (__double2loint(t[j]) & 1) << 31;
+    v[j] = __hiloint2double(__double2hiint(c[j]) ^ flip, __double2loint(c[j]));
+    asm volatile("" : "+d"(v[j]));   // keeps the batch together: the rare path below must not pull it apart
+  }
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    // |K| >= 5e5, inf, nan: the library routine (never taken for momentum sums of a diagram)
+    if ((__double2hiint(K[j]) & 0x7fffffff) >= 0x411e8480) v[j] = cos_unbounded(K[j]);
+    K[j] = v[j];
+  }
+}
+__device__ __forceinline__ double cos_bounded(double K) {
+  double a[1] = {K};
+  cos_bounded_n<1>(a);
+  return a[0];
 }
 
 // f_sigma(E) = 1/(sigma e^x + 1) and g = 1 - f = sigma e^x f for x = beta E, any real x, without

@@ -15,6 +15,7 @@
 #include <cuda_runtime.h>
 #include <dlfcn.h>
 
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -55,44 +56,99 @@ std::string combo(const std::vector<int>& c, const char* base, const std::string
   return s.empty() ? "0.0" : s;
 }
 
+// A list of statements that must stay in order; independent lists are interleaved round-robin
+// before they are written out, so that the straight-line code offers the FP64 pipe several
+// independent dependency chains at any point (ptxas keeps the source order it is given far more
+// than it reorders across long chains).
+typedef std::vector<std::string> Stmts;
+
 struct Emitter {
-  std::ostringstream o;
   int tmp = 0;
   std::string fresh(const char* p) { return std::string(p) + std::to_string(tmp++); }
 };
 
-// S_F(n) of group g as a named double (see ami_table.hpp); n has kids
-std::string emit_f_sum(const std::vector<HNode>& f, int n, Emitter& E) {
-  std::string acc;
-  for (int c : f[n].kids) {
-    if (f[c].kids.empty()) continue;
-    const std::string sc = emit_f_sum(f, c, E);
-    const std::string v = E.fresh("s");
-    if (acc.empty()) E.o << "      const double " << v << " = F" << f[c].leaf << " * " << sc << ";\n";
-    else E.o << "      const double " << v << " = fma(F" << f[c].leaf << ", " << sc << ", " << acc << ");\n";
-    acc = v;
+void interleave(std::vector<Stmts>& lists, size_t ways, std::ostringstream& o, const char* indent) {
+  for (size_t base = 0; base < lists.size(); base += ways) {
+    const size_t end = std::min(lists.size(), base + ways);
+    size_t longest = 0;
+    for (size_t i = base; i < end; ++i) longest = std::max(longest, lists[i].size());
+    for (size_t k = 0; k < longest; ++k)
+      for (size_t i = base; i < end; ++i)
+        if (k < lists[i].size()) o << indent << lists[i][k] << "\n";
   }
-  for (int c : f[n].kids) {
-    if (!f[c].kids.empty()) continue;
-    const bool plus = f[c].num == 1 && f[c].den == 1, minus = f[c].num == -1 && f[c].den == 1;
-    const std::string leaf = "F" + std::to_string(f[c].leaf);
-    if (acc.empty()) {
-      if (plus) { acc = leaf; continue; }
-      if (minus) { acc = "(-" + leaf + ")"; continue; }
-      const std::string v = E.fresh("s");
-      E.o << "      const double " << v << " = " << dlit((double)f[c].num / (double)f[c].den) << " * " << leaf << ";\n";
+}
+
+// One S-node of the FT DAG (ami_table.hpp) as a chain of statements defining `S<id>`
+void emit_snode(const HornerPlan& hp, int id, Emitter& E, Stmts& out) {
+  const SNode& n = hp.snodes[id];
+  std::string acc;
+  for (size_t i = 0; i < n.items.size(); ++i) {
+    const SItem& it = n.items[i];
+    const bool last = i + 1 == n.items.size();
+    const std::string v = last ? "S" + std::to_string(id) : E.fresh("s");
+    const std::string leaf = "F" + std::to_string(it.leaf);
+    if (it.child >= 0) {
+      const std::string sc = "S" + std::to_string(it.child);
+      if (acc.empty()) out.push_back("const double " + v + " = " + leaf + " * " + sc + ";");
+      else out.push_back("const double " + v + " = fma(" + leaf + ", " + sc + ", " + acc + ");");
       acc = v;
       continue;
     }
-    const std::string v = E.fresh("s");
-    if (plus) E.o << "      const double " << v << " = " << acc << " + " << leaf << ";\n";
-    else if (minus) E.o << "      const double " << v << " = " << acc << " - " << leaf << ";\n";
-    else
-      E.o << "      const double " << v << " = fma(" << dlit((double)f[c].num / (double)f[c].den) << ", " << leaf << ", "
-          << acc << ");\n";
+    const bool plus = it.num == 1 && it.den == 1, minus = it.num == -1 && it.den == 1;
+    const std::string coef = dlit((double)it.num / (double)it.den);
+    if (acc.empty()) {
+      if (plus && !last) { acc = leaf; continue; }
+      if (minus && !last) { acc = "(-" + leaf + ")"; continue; }
+      if (plus) out.push_back("const double " + v + " = " + leaf + ";");
+      else if (minus) out.push_back("const double " + v + " = -" + leaf + ";");
+      else out.push_back("const double " + v + " = " + coef + " * " + leaf + ";");
+    } else if (plus) {
+      out.push_back("const double " + v + " = " + acc + " + " + leaf + ";");
+    } else if (minus) {
+      out.push_back("const double " + v + " = " + acc + " - " + leaf + ";");
+    } else {
+      out.push_back("const double " + v + " = fma(" + coef + ", " + leaf + ", " + acc + ");");
+    }
     acc = v;
   }
-  return acc;
+}
+
+// Emits the S-nodes that groups [g0, g1) need and that have not been emitted yet, level by level
+// (nodes of equal height are independent of one another), kWays chains side by side.
+void emit_ft_chunk(const HornerPlan& hp, size_t g0, size_t g1, std::vector<char>& done, size_t ways, Emitter& E,
+                   std::ostringstream& o, const char* indent) {
+  std::vector<int> need, stack;
+  for (size_t g = g0; g < g1; ++g)
+    if (hp.groups[g].root >= 0) stack.push_back(hp.groups[g].root);
+  while (!stack.empty()) {
+    const int id = stack.back();
+    stack.pop_back();
+    if (done[id]) continue;
+    done[id] = 1;
+    need.push_back(id);
+    for (const SItem& it : hp.snodes[id].items)
+      if (it.child >= 0 && !done[it.child]) stack.push_back(it.child);
+  }
+  std::sort(need.begin(), need.end(), [&](int a, int b) {
+    const int ha = hp.snodes[a].height, hb = hp.snodes[b].height;
+    return ha != hb ? ha < hb : a < b;
+  });
+  for (size_t i = 0; i < need.size();) {
+    size_t j = i;
+    std::vector<Stmts> lists;
+    while (j < need.size() && hp.snodes[need[j]].height == hp.snodes[need[i]].height) {
+      lists.emplace_back();
+      emit_snode(hp, need[j], E, lists.back());
+      ++j;
+    }
+    interleave(lists, ways, o, indent);
+    i = j;
+  }
+  for (size_t g = g0; g < g1; ++g) {
+    const HGroup& hg = hp.groups[g];
+    o << indent << "const double FT" << g << " = "
+      << (hg.root >= 0 ? "S" + std::to_string(hg.root) : dlit((double)hg.num / (double)hg.den)) << ";\n";
+  }
 }
 
 struct CV {            // a complex value held in named doubles; im empty = purely real
@@ -100,8 +156,44 @@ struct CV {            // a complex value held in named doubles; im empty = pure
   bool real() const { return im.empty(); }
 };
 
+// acc + Dinv[u] * s as new named doubles appended to `out` (acc may be absent)
+CV emit_cmul_acc(const HornerPlan& hp, int u, const CV& s, const CV* accp, Emitter& E, Stmts& out) {
+  const bool dreal = hp.d_is_real[u] != 0;
+  const std::string dr = "Dr" + std::to_string(u), di = "Di" + std::to_string(u);
+  CV r;
+  r.re = E.fresh("r");
+  {   // real part: dr*s.re - di*s.im (+ acc.re)
+    std::string inner = accp ? accp->re : "";
+    if (!dreal && !s.real()) {
+      const std::string t = E.fresh("r");
+      if (inner.empty()) out.push_back("const double " + t + " = -" + di + " * " + s.im + ";");
+      else out.push_back("const double " + t + " = fma(-" + di + ", " + s.im + ", " + inner + ");");
+      inner = t;
+    }
+    if (inner.empty()) out.push_back("const double " + r.re + " = " + dr + " * " + s.re + ";");
+    else out.push_back("const double " + r.re + " = fma(" + dr + ", " + s.re + ", " + inner + ");");
+  }
+  {   // imaginary part: dr*s.im + di*s.re (+ acc.im)
+    std::string inner = (accp && !accp->real()) ? accp->im : "";
+    if (!s.real()) {
+      const std::string t = E.fresh("r");
+      if (inner.empty()) out.push_back("const double " + t + " = " + dr + " * " + s.im + ";");
+      else out.push_back("const double " + t + " = fma(" + dr + ", " + s.im + ", " + inner + ");");
+      inner = t;
+    }
+    if (!dreal) {
+      const std::string t = E.fresh("r");
+      if (inner.empty()) out.push_back("const double " + t + " = " + di + " * " + s.re + ";");
+      else out.push_back("const double " + t + " = fma(" + di + ", " + s.re + ", " + inner + ");");
+      inner = t;
+    }
+    r.im = inner;   // stays empty when the product and the running sum are both real
+  }
+  return r;
+}
+
 // S_D(n): group FT at this node plus sum over kids of Dinv[kid.leaf] * S_D(kid)
-CV emit_d_sum(const HornerPlan& hp, int n, Emitter& E) {
+CV emit_d_sum(const HornerPlan& hp, int n, Emitter& E, Stmts& out) {
   CV acc;
   bool have = false;
   if (hp.dn[n].group >= 0) {
@@ -109,42 +201,8 @@ CV emit_d_sum(const HornerPlan& hp, int n, Emitter& E) {
     have = true;
   }
   for (int c : hp.dn[n].kids) {
-    const CV s = emit_d_sum(hp, c, E);
-    const int u = hp.dn[c].leaf;
-    const bool dreal = hp.d_is_real[u] != 0;
-    const std::string dr = "Dr" + std::to_string(u), di = "Di" + std::to_string(u);
-    CV r;
-    r.re = E.fresh("r");
-    // real part: dr*s.re - di*s.im (+ acc.re)
-    {
-      std::string inner = have ? acc.re : "";
-      if (!dreal && !s.real()) {
-        const std::string t = E.fresh("r");
-        if (inner.empty()) E.o << "        const double " << t << " = -" << di << " * " << s.im << ";\n";
-        else E.o << "        const double " << t << " = fma(-" << di << ", " << s.im << ", " << inner << ");\n";
-        inner = t;
-      }
-      if (inner.empty()) E.o << "        const double " << r.re << " = " << dr << " * " << s.re << ";\n";
-      else E.o << "        const double " << r.re << " = fma(" << dr << ", " << s.re << ", " << inner << ");\n";
-    }
-    // imaginary part: dr*s.im + di*s.re (+ acc.im)
-    {
-      std::string inner = (have && !acc.real()) ? acc.im : "";
-      if (!s.real()) {
-        const std::string t = E.fresh("r");
-        if (inner.empty()) E.o << "        const double " << t << " = " << dr << " * " << s.im << ";\n";
-        else E.o << "        const double " << t << " = fma(" << dr << ", " << s.im << ", " << inner << ");\n";
-        inner = t;
-      }
-      if (!dreal) {
-        const std::string t = E.fresh("r");
-        if (inner.empty()) E.o << "        const double " << t << " = " << di << " * " << s.re << ";\n";
-        else E.o << "        const double " << t << " = fma(" << di << ", " << s.re << ", " << inner << ");\n";
-        inner = t;
-      }
-      r.im = inner;   // stays empty when the product and the running sum are both real
-    }
-    acc = r;
+    const CV s = emit_d_sum(hp, c, E, out);
+    acc = emit_cmul_acc(hp, hp.dn[c].leaf, s, have ? &acc : nullptr, E, out);
     have = true;
   }
   if (!have) acc.re = "0.0";
@@ -158,45 +216,141 @@ CV emit_d_sum(const HornerPlan& hp, int n, Emitter& E) {
 // ---------------------------------------------------------------------------------------------
 std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int block_threads) {
   const int L = ft.n_int + ft.n_ext;
+  size_t kWays = 4;           // independent chains kept side by side
+  if (const char* env = getenv("AMI_JIT_WAYS")) {   // tuning knob (profiles/)
+    const int w = atoi(env);
+    if (w >= 1 && w <= 16) kWays = (size_t)w;
+  }
   Emitter E;
-  std::ostringstream& o = E.o;
+  std::ostringstream o;
   o << kAmiParamsSrc << "\n" << kAmiDeviceSrc << "\n";
   o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n";
   // ---- body: one sample, energies e0..e{n_eps-1} in registers ------------------------------
   o << "__device__ __forceinline__ void ami_body(const AmiBatch& p, const long long s";
   for (int i = 0; i < ft.n_eps; ++i) o << ", const double e" << i;
   o << ") {\n";
+  // every distinct integer combination of the energies, up to sign, once per sample
+  std::vector<std::vector<int>> combos;
+  auto combo_ref = [&](const std::vector<int>& c) -> std::string {
+    std::vector<int> pos = c;
+    int sign = 0;
+    for (int v : c)
+      if (v) { sign = v > 0 ? 1 : -1; break; }
+    if (!sign) return "0.0";
+    if (sign < 0)
+      for (int& v : pos) v = -v;
+    size_t j = 0;
+    for (; j < combos.size(); ++j)
+      if (combos[j] == pos) break;
+    if (j == combos.size()) combos.push_back(pos);
+    return std::string(sign < 0 ? "-E" : "E") + std::to_string(j);
+  };
+  for (const LeafF& l : ft.leafF) combo_ref(l.c);
+  for (const LeafD& l : ft.leafD) combo_ref(l.c);
+  for (size_t j = 0; j < combos.size(); ++j) o << "  const double E" << j << " = " << combo(combos[j], "e") << ";\n";
+  // reciprocals of the denominators, kWays at a time
+  auto emit_d_leaves = [&](const std::vector<size_t>& ids, const std::string& ind) {
+    for (size_t u : ids) o << ind << "double Dr" << u << (hp.d_is_real[u] ? "" : ", Di" + std::to_string(u)) << ";\n";
+    for (size_t i0 = 0; i0 < ids.size(); i0 += kWays) {
+      const size_t n = std::min(kWays, ids.size() - i0);
+      o << ind << "{\n";
+      for (size_t j = 0; j < n; ++j) {
+        const size_t u = ids[i0 + j];
+        const LeafD& l = ft.leafD[u];
+        const std::string en = combo_ref(l.c);
+        if (hp.d_is_real[u]) {
+          o << ind << "  const double re" << j << " = " << en << " + p.e_reg;\n";
+        } else {
+          std::string cond;
+          for (int x = 0; x < ft.n_ext; ++x)
+            if (l.a[x]) cond += (cond.empty() ? "" : " && ") + std::string("zz") + std::to_string(x);
+          o << ind << "  const double re" << j << " = ((" << combo(l.a, "zr") << ") + " << en << ") + ((" << cond
+            << ") ? p.e_reg : 0.0), im" << j << " = " << combo(l.a, "zi") << ";\n";
+        }
+      }
+      o << ind << "  double d[" << n << "] = {";
+      for (size_t j = 0; j < n; ++j) {
+        if (hp.d_is_real[ids[i0 + j]]) o << (j ? ", " : "") << "re" << j;
+        else o << (j ? ", " : "") << "fma(re" << j << ", re" << j << ", im" << j << " * im" << j << ")";
+      }
+      o << "};\n" << ind << "  fast_rcp_n<" << n << ">(d);\n";
+      for (size_t j = 0; j < n; ++j) {
+        const size_t u = ids[i0 + j];
+        if (hp.d_is_real[u]) o << ind << "  Dr" << u << " = d[" << j << "];\n";
+        else o << ind << "  Dr" << u << " = re" << j << " * d[" << j << "]; Di" << u << " = -im" << j << " * d[" << j << "];\n";
+      }
+      o << ind << "}\n";
+    }
+  };
+  // denominators without an external frequency are purely real and the same for every beta and
+  // frequency: once per sample, regulator always applied (P10(b))
+  {
+    std::vector<size_t> ids;
+    for (size_t u = 0; u < ft.leafD.size(); ++u)
+      if (hp.d_is_real[u]) ids.push_back(u);
+    emit_d_leaves(ids, "  ");
+  }
   o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n";
-  // Fermi/Bose leaves (independent of the external frequency)
-  for (size_t u = 0; u < ft.leafF.size(); ++u) {
-    const LeafF& l = ft.leafF[u];
-    std::string arg = combo(l.c, "e");
-    if (l.sigma < 0) arg = "(" + arg + ") + p.e_reg";          // P10(a)
-    o << "    double F" << u << ";\n    {\n      double f, g;\n      fermi_fg<" << (l.sigma > 0 ? 1 : -1)
-      << ", " << (l.k > 0 ? "true" : "false") << ">(beta * (" << arg << "), f, g);\n";
-    if (l.k == 0) {
-      o << "      F" << u << " = f;\n";
-    } else {
-      const std::vector<double> q = deriv_poly(l.k);
-      o << "      double q = " << dlit(q.back()) << ";\n";
-      for (int i = (int)q.size() - 2; i >= 0; --i) o << "      q = fma(q, f, " << dlit(q[i]) << ");\n";
-      o << "      double bk = beta;\n";
-      for (int i = 1; i < l.k; ++i) o << "      bk *= beta;\n";
-      o << "      F" << u << " = bk * f * g * q;\n";
+  // Fermi/Bose leaves (independent of the external frequency), kWays at a time
+  // Leaves that differ only in the derivative order share one exponential and one reciprocal.
+  const size_t UF = ft.leafF.size();
+  std::vector<std::vector<size_t>> base;      // base -> leaves with the same (combination, sigma)
+  for (size_t u = 0; u < UF; ++u) {
+    size_t b = 0;
+    for (; b < base.size(); ++b)
+      if (ft.leafF[base[b][0]].c == ft.leafF[u].c && ft.leafF[base[b][0]].sigma == ft.leafF[u].sigma) break;
+    if (b == base.size()) base.emplace_back();
+    base[b].push_back(u);
+  }
+  for (size_t u = 0; u < UF; ++u) o << "    double F" << u << ";\n";
+  for (size_t b0 = 0; b0 < base.size(); b0 += kWays) {
+    const size_t n = std::min(kWays, base.size() - b0);
+    o << "    {\n      const double x[" << n << "] = {";
+    for (size_t j = 0; j < n; ++j) {
+      const LeafF& l = ft.leafF[base[b0 + j][0]];
+      std::string arg = combo_ref(l.c);
+      if (l.sigma < 0) arg = arg + " + p.e_reg";                  // P10(a)
+      o << (j ? ", " : "") << "beta * (" << arg << ")";
+    }
+    o << "};\n      double sc[" << n << "], rq[" << n << "];\n      exp_core_n<" << n << ">(x, sc, rq);\n";
+    // 1 + e^x (sigma = +1) or e^x - 1 (sigma = -1) in one fma, then the reciprocals
+    o << "      double d[" << n << "] = {";
+    for (size_t j = 0; j < n; ++j)
+      o << (j ? ", " : "") << "fma(sc[" << j << "], rq[" << j << "], sc[" << j << "] "
+        << (ft.leafF[base[b0 + j][0]].sigma > 0 ? "+" : "-") << " 1.0)";
+    o << "};\n      fast_rcp_n<" << n << ">(d);\n";
+    for (size_t j = 0; j < n; ++j) {
+      const std::vector<size_t>& members = base[b0 + j];
+      const int sigma = ft.leafF[members[0]].sigma;
+      const std::string f = std::string(sigma > 0 ? "" : "-") + "d[" + std::to_string(j) + "]";
+      bool need_g = false;
+      for (size_t u : members) need_g |= ft.leafF[u].k > 0;
+      if (need_g)   // g = 1 - f = sigma e^x f  (P11)
+        o << "      const double g" << j << " = " << (sigma > 0 ? "" : "-") << "fma(sc[" << j << "], rq[" << j << "], sc["
+          << j << "]) * " << f << ";\n";
+      for (size_t u : members) {
+        const LeafF& l = ft.leafF[u];
+        if (l.k == 0) {
+          o << "      F" << u << " = " << f << ";\n";
+          continue;
+        }
+        // f^{(k)} = beta^k f g Q_k(f)
+        o << "      {\n        const double f = " << f << ";\n";
+        const std::vector<double> q = deriv_poly(l.k);
+        o << "        double q = " << dlit(q.back()) << ";\n";
+        for (int i = (int)q.size() - 2; i >= 0; --i) o << "        q = fma(q, f, " << dlit(q[i]) << ");\n";
+        o << "        double bk = beta;\n";
+        for (int i = 1; i < l.k; ++i) o << "        bk *= beta;\n";
+        o << "        F" << u << " = bk * f * g" << j << " * q;\n      }\n";
+      }
     }
     o << "    }\n";
   }
-  // FT sums of every group (per beta)
-  for (size_t g = 0; g < hp.groups.size(); ++g) {
-    const std::vector<HNode>& f = hp.groups[g].f;
-    o << "    double FT" << g << ";\n    {\n";
-    if (f[0].kids.empty()) {
-      o << "      FT" << g << " = " << dlit(f[0].terminal ? (double)f[0].num / (double)f[0].den : 0.0) << ";\n";
-    } else {
-      const std::string v = emit_f_sum(f, 0, E);
-      o << "      FT" << g << " = " << v << ";\n";
-    }
-    o << "    }\n";
+  // FT sums of every group (per beta): a DAG shared by all groups, emitted eight groups at a time
+  {
+    std::vector<char> done(hp.snodes.size(), 0);
+    for (size_t g0 = 0; g0 < hp.groups.size(); g0 += 8)
+      emit_ft_chunk(hp, g0, std::min(hp.groups.size(), g0 + 8), done, kWays, E, o, "    ");
   }
   // frequencies
   o << "#pragma unroll 1\n    for (int f = 0; f < p.n_f; ++f) {\n";
@@ -205,29 +359,37 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
       << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ") + 1];\n";
     o << "      const bool zz" << x << " = (zr" << x << " == 0.0 && zi" << x << " == 0.0);\n";
   }
-  for (size_t u = 0; u < ft.leafD.size(); ++u) {
-    const LeafD& l = ft.leafD[u];
-    std::string re = combo(l.a, "zr"), im = combo(l.a, "zi"), en = combo(l.c, "e");
-    std::string cond;
-    for (int x = 0; x < ft.n_ext; ++x)
-      if (l.a[x]) cond += (cond.empty() ? "" : " && ") + std::string("zz") + std::to_string(x);
-    if (hp.d_is_real[u]) {
-      // no frequency part: purely real, regulator always applies (P10(b))
-      o << "      const double Dr" << u << " = fast_rcp((" << en << ") + p.e_reg);\n";
-    } else {
-      o << "      double Dr" << u << ", Di" << u << ";\n      {\n";
-      o << "        const cplx d = crcp(cplx{((" << re << ") + (" << en << ")) + ((" << cond << ") ? p.e_reg : 0.0), "
-        << im << "});\n";
-      o << "        Dr" << u << " = d.re; Di" << u << " = d.im;\n      }\n";
-    }
+  // reciprocals of the denominators that carry an external frequency (P10(b) decides at run time
+  // whether the regulator applies)
+  {
+    std::vector<size_t> ids;
+    for (size_t u = 0; u < ft.leafD.size(); ++u)
+      if (!hp.d_is_real[u]) ids.push_back(u);
+    emit_d_leaves(ids, "      ");
   }
-  o << "      {\n";
-  const CV res = emit_d_sum(hp, 0, E);
-  o << "        double2* out = reinterpret_cast<double2*>(p.out) + ((long long)(p.b0 + b) * p.n_f_total + (p.f0 + f)) * "
-       "p.out_row_stride + s;\n";
-  o << "        *out = make_double2(p.prefactor * (" << res.re << "), "
-    << (res.real() ? std::string("0.0") : "p.prefactor * (" + res.im + ")") << ");\n";
-  o << "      }\n    }\n  }\n}\n\n";
+  // R part: the subtrees under the root side by side, then the root's own sum
+  {
+    const std::vector<int>& kids = hp.dn[0].kids;
+    std::vector<Stmts> lists(kids.size());
+    std::vector<CV> sub(kids.size());
+    for (size_t i = 0; i < kids.size(); ++i) sub[i] = emit_d_sum(hp, kids[i], E, lists[i]);
+    interleave(lists, kWays, o, "      ");
+    Stmts tail;
+    CV acc;
+    bool have = false;
+    if (hp.dn[0].group >= 0) { acc.re = "FT" + std::to_string(hp.dn[0].group); have = true; }
+    for (size_t i = 0; i < kids.size(); ++i) {
+      acc = emit_cmul_acc(hp, hp.dn[kids[i]].leaf, sub[i], have ? &acc : nullptr, E, tail);
+      have = true;
+    }
+    if (!have) acc.re = "0.0";
+    for (const std::string& st : tail) o << "      " << st << "\n";
+    o << "      double2* out = reinterpret_cast<double2*>(p.out) + ((long long)(p.b0 + b) * p.n_f_total + (p.f0 + f)) * "
+         "p.out_row_stride + s;\n";
+    o << "      *out = make_double2(p.prefactor * (" << acc.re << "), "
+      << (acc.real() ? std::string("0.0") : "p.prefactor * (" + acc.im + ")") << ");\n";
+  }
+  o << "    }\n  }\n}\n\n";
   // ---- kernel 1: energies from memory ---------------------------------------------------------
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
        "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n  if (s >= p.n) return;\n";
@@ -245,10 +407,19 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   for (int x = 0; x < ft.n_ext; ++x)
     o << "  const double kx" << ft.n_int + x << " = p.q[" << 2 * x << "], ky" << ft.n_int + x << " = p.q[" << 2 * x + 1
       << "];\n";
-  for (int i = 0; i < ft.n_eps; ++i) {
-    std::vector<int> a(ft.sym_alpha.begin() + (size_t)i * L, ft.sym_alpha.begin() + (size_t)(i + 1) * L);
-    o << "  const double e" << i << " = fma(2.0 * p.t, cos_bounded(" << combo(a, "kx") << ") + cos_bounded(" << combo(a, "ky")
-      << "), p.mu);\n";
+  for (int i = 0; i < ft.n_eps; ++i) o << "  double e" << i << ";\n";
+  const int sym_batch = std::max(1, (int)kWays / 2);   // kWays cosines side by side
+  for (int i0 = 0; i0 < ft.n_eps; i0 += sym_batch) {
+    const int n = std::min(sym_batch, ft.n_eps - i0);
+    o << "  {\n    double c[" << 2 * n << "] = {";
+    for (int j = 0; j < n; ++j) {
+      std::vector<int> a(ft.sym_alpha.begin() + (size_t)(i0 + j) * L, ft.sym_alpha.begin() + (size_t)(i0 + j + 1) * L);
+      o << (j ? ", " : "") << combo(a, "kx") << ", " << combo(a, "ky");
+    }
+    o << "};\n    cos_bounded_n<" << 2 * n << ">(c);\n";
+    for (int j = 0; j < n; ++j)
+      o << "    e" << i0 + j << " = fma(2.0 * p.t, c[" << 2 * j << "] + c[" << 2 * j + 1 << "], p.mu);\n";
+    o << "  }\n";
   }
   o << "  if (p.e_out) {\n";
   for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
@@ -314,9 +485,14 @@ int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& l
     log = "nvrtcCreateProgram failed";
     return AMI_EINVAL;
   }
-  const char* opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "--ptxas-options=-v",
-                        "-default-device"};
-  const int rc = n.CompileProgram(prog, (int)(sizeof opts / sizeof opts[0]), opts);
+  std::vector<const char*> opts = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "--ptxas-options=-v",
+                                   "-default-device"};
+  std::string maxreg;
+  if (const char* env = getenv("AMI_JIT_MAXREG")) {   // tuning knob (profiles/): cap registers per thread
+    maxreg = std::string("--maxrregcount=") + env;
+    opts.push_back(maxreg.c_str());
+  }
+  const int rc = n.CompileProgram(prog, (int)opts.size(), opts.data());
   size_t ls = 0;
   n.GetProgramLogSize(prog, &ls);
   if (ls > 1) {

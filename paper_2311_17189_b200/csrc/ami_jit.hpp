@@ -10,7 +10,7 @@
 
 namespace ami {
 
-constexpr int kJitBlockThreads = 128;
+constexpr int kJitBlockThreads = 64;
 
 // Tables whose straight-line form is small enough to live in registers and in the instruction
 // cache; larger ones are evaluated by the table-driven kernels.

@@ -40,8 +40,16 @@ std::vector<double> deriv_poly(int k) {
 
 namespace {
 
-// Inserts `seq` into the trie `nodes` (nodes[0] = root) and returns the node it ends at.
-int trie_insert(std::vector<HNode>& nodes, const std::vector<int>& seq) {
+// ---- tries -----------------------------------------------------------------------------------
+struct TrieNode {
+  int leaf = -1;
+  std::vector<int> kids;
+  bool terminal = false;
+  long long num = 0, den = 1;
+};
+
+template <class Node>
+int trie_insert(std::vector<Node>& nodes, const std::vector<int>& seq) {
   int cur = 0;
   for (int leaf : seq) {
     int nxt = -1;
@@ -49,7 +57,7 @@ int trie_insert(std::vector<HNode>& nodes, const std::vector<int>& seq) {
       if (nodes[c].leaf == leaf) { nxt = c; break; }
     if (nxt < 0) {
       nxt = (int)nodes.size();
-      HNode n;
+      Node n;
       n.leaf = leaf;
       nodes.push_back(n);
       nodes[cur].kids.push_back(nxt);
@@ -59,62 +67,106 @@ int trie_insert(std::vector<HNode>& nodes, const std::vector<int>& seq) {
   return cur;
 }
 
-// Reorders every sequence so that ids occurring in more sequences come first (ties: lower id):
-// frequent factors sit near the root, which is what makes prefixes shared.
-void order_by_frequency(std::vector<std::vector<int>>& seqs) {
+// number of sequences each id occurs in (sequences are sorted: count an id once per sequence)
+std::map<int, int> occurrence(const std::vector<std::vector<int>>& seqs) {
   std::map<int, int> cnt;
   for (const auto& q : seqs) {
     int last = -1;
-    for (int x : q) {            // q is sorted: count each id once per sequence
+    for (int x : q) {
       if (x != last) ++cnt[x];
       last = x;
     }
   }
+  return cnt;
+}
+
+// Factor orderings tried for the FT sums.  0: inside each group, ids in more of the group's terms
+// first (shares prefixes within the group).  1-4: one ordering for the whole table, which lines the
+// tails of different groups up so that hash-consing finds them equal.
+enum { kOrderLocalFreq = 0, kOrderGlobalRareFirst, kOrderGlobalFreqFirst, kOrderIdAsc, kOrderIdDesc, kNumOrders };
+
+void apply_order(std::vector<std::vector<int>>& seqs, int order, const std::map<int, int>& global_cnt) {
+  std::map<int, int> local;
+  if (order == kOrderLocalFreq) local = occurrence(seqs);
+  auto cnt = [&](int x) {
+    const std::map<int, int>& m = order == kOrderLocalFreq ? local : global_cnt;
+    auto it = m.find(x);
+    return it == m.end() ? 0 : it->second;
+  };
   for (auto& q : seqs)
     std::stable_sort(q.begin(), q.end(), [&](int a, int b) {
-      const int ca = cnt[a], cb = cnt[b];
-      return ca != cb ? ca > cb : a < b;
+      switch (order) {
+        case kOrderLocalFreq:
+        case kOrderGlobalFreqFirst: { const int ca = cnt(a), cb = cnt(b); return ca != cb ? ca > cb : a < b; }
+        case kOrderGlobalRareFirst: { const int ca = cnt(a), cb = cnt(b); return ca != cb ? ca < cb : a < b; }
+        case kOrderIdAsc: return a < b;
+        default: return a > b;
+      }
     });
 }
 
-// FP64 instruction counts of the Horner evaluation, mirroring the emission rules of ami_jit.cpp.
-long long count_f_ops(const std::vector<HNode>& f, int n) {
-  long long ops = 0;
-  bool have = false;
-  for (int c : f[n].kids)
-    if (!f[c].kids.empty()) {
-      ops += count_f_ops(f, c) + 1;     // multiply, or fma into the running sum
-      have = true;
-    }
-  for (int c : f[n].kids)
-    if (f[c].kids.empty()) {
-      const bool unit = (f[c].num == 1 || f[c].num == -1) && f[c].den == 1;
-      if (have || !unit) ++ops;         // add / fma; a leading +-F is free
-      have = true;
-    }
+// FP64 instructions of one S-node as emitted by ami_jit.cpp: one multiply / fma / add per item,
+// except that a leading +-F costs nothing.
+long long snode_ops(const SNode& n) {
+  long long ops = (long long)n.items.size();
+  const SItem& first = n.items[0];
+  if (first.child < 0 && (first.num == 1 || first.num == -1) && first.den == 1) --ops;
   return ops;
+}
+
+typedef std::vector<long long> SKey;
+
+// hash-conses the sub-trie under `t` into `snodes`; returns the S-node id
+int intern(const std::vector<TrieNode>& trie, int t, std::vector<SNode>& snodes, std::map<SKey, int>& memo) {
+  SNode n;
+  for (int c : trie[t].kids)
+    if (!trie[c].kids.empty()) {
+      const int ch = intern(trie, c, snodes, memo);
+      n.items.push_back(SItem{trie[c].leaf, ch, 0, 1});
+      n.height = std::max(n.height, snodes[ch].height + 1);
+    }
+  const size_t n_inner = n.items.size();
+  for (int c : trie[t].kids)
+    if (trie[c].kids.empty()) n.items.push_back(SItem{trie[c].leaf, -1, trie[c].num, trie[c].den});
+  auto less = [](const SItem& a, const SItem& b) {
+    if (a.leaf != b.leaf) return a.leaf < b.leaf;
+    if (a.child != b.child) return a.child < b.child;
+    if (a.num != b.num) return a.num < b.num;
+    return a.den < b.den;
+  };
+  std::sort(n.items.begin(), n.items.begin() + n_inner, less);
+  std::sort(n.items.begin() + n_inner, n.items.end(), less);
+  SKey key;
+  for (const SItem& it : n.items) { key.push_back(it.leaf); key.push_back(it.child); key.push_back(it.num); key.push_back(it.den); }
+  auto f = memo.find(key);
+  if (f != memo.end()) return f->second;
+  const int id = (int)snodes.size();
+  snodes.push_back(std::move(n));
+  memo.emplace(std::move(key), id);
+  return id;
 }
 
 // returns ops; *is_real tells whether S_D(n) has no imaginary part
 long long count_d_ops(const HornerPlan& hp, int n, bool* is_real) {
   long long ops = 0;
-  bool have = hp.dn[n].group >= 0, acc_real = true;
+  bool acc_real = true;
   for (int c : hp.dn[n].kids) {
     bool sreal = true;
     ops += count_d_ops(hp, c, &sreal);
     const bool dreal = hp.d_is_real[hp.dn[c].leaf] != 0;
-    const bool preal = dreal && sreal;
-    // product D * S: real*real 1, real*complex or complex*real 2, complex*complex 4; when a
-    // running sum exists the adds fuse into the multiplies (fma), except that a real product
-    // leaves the imaginary accumulator alone
-    long long pops = dreal ? (sreal ? 1 : 2) : (sreal ? 2 : 4);
-    (void)have;
-    ops += pops;
-    acc_real = acc_real && preal;
-    have = true;
+    // product D * S: real*real 1, real*complex or complex*real 2, complex*complex 4; a running sum
+    // is folded into the multiplies (fma)
+    ops += dreal ? (sreal ? 1 : 2) : (sreal ? 2 : 4);
+    acc_real = acc_real && dreal && sreal;
   }
   *is_real = acc_real;
   return ops;
+}
+
+int nnz(const std::vector<int>& v) {
+  int n = 0;
+  for (int x : v) n += (x != 0);
+  return n;
 }
 
 }  // namespace
@@ -122,15 +174,12 @@ long long count_d_ops(const HornerPlan& hp, int n, bool* is_real) {
 void build_horner_plan(const FlatTable& ft, HornerPlan& hp) {
   hp = HornerPlan();
   hp.d_is_real.assign(ft.leafD.size(), 0);
-  for (size_t u = 0; u < ft.leafD.size(); ++u) {
-    bool any = false;
-    for (int a : ft.leafD[u].a) any |= (a != 0);
-    hp.d_is_real[u] = any ? 0 : 1;
-  }
+  for (size_t u = 0; u < ft.leafD.size(); ++u) hp.d_is_real[u] = nnz(ft.leafD[u].a) ? 0 : 1;
   // group the terms by denominator product
   std::map<std::vector<int>, int> gid;
   std::vector<std::vector<int>> gd;                       // group -> d
   std::vector<std::vector<const FlatTerm*>> members;
+  std::vector<std::vector<int>> all_f;
   for (const FlatTerm& t : ft.terms) {
     auto it = gid.find(t.d);
     if (it == gid.end()) {
@@ -139,33 +188,99 @@ void build_horner_plan(const FlatTable& ft, HornerPlan& hp) {
       members.emplace_back();
     }
     members[it->second].push_back(&t);
+    all_f.push_back(t.f);
   }
   const int G = (int)gd.size();
-  hp.groups.resize(G);
-  for (int g = 0; g < G; ++g) {
-    HGroup& hg = hp.groups[g];
-    hg.d = gd[g];
-    std::vector<std::vector<int>> seqs;
-    for (const FlatTerm* t : members[g]) seqs.push_back(t->f);
-    order_by_frequency(seqs);
-    hg.f.assign(1, HNode());
-    for (size_t i = 0; i < seqs.size(); ++i) {
-      const int n = trie_insert(hg.f, seqs[i]);
-      hg.f[n].terminal = true;
-      hg.f[n].num = members[g][i]->num;
-      hg.f[n].den = members[g][i]->den;
+  const std::map<int, int> global_cnt = occurrence(all_f);
+  // FT sums: try every ordering, keep the cheapest DAG
+  long long best = -1;
+  for (int order = 0; order < kNumOrders; ++order) {
+    std::vector<SNode> snodes;
+    std::map<SKey, int> memo;
+    std::vector<HGroup> groups(G);
+    for (int g = 0; g < G; ++g) {
+      groups[g].d = gd[g];
+      std::vector<std::vector<int>> seqs;
+      for (const FlatTerm* t : members[g]) seqs.push_back(t->f);
+      apply_order(seqs, order, global_cnt);
+      std::vector<TrieNode> trie(1);
+      for (size_t i = 0; i < seqs.size(); ++i) {
+        const int n = trie_insert(trie, seqs[i]);
+        trie[n].terminal = true;
+        trie[n].num = members[g][i]->num;
+        trie[n].den = members[g][i]->den;
+      }
+      if (trie[0].kids.empty()) {       // no Fermi factors at all (n_int = 0)
+        groups[g].root = -1;
+        groups[g].num = trie[0].terminal ? trie[0].num : 0;
+        groups[g].den = trie[0].terminal ? trie[0].den : 1;
+      } else {
+        groups[g].root = intern(trie, 0, snodes, memo);
+      }
     }
-    hp.n_fnodes += (long long)hg.f.size() - 1;
-    hp.ops_f += count_f_ops(hg.f, 0);
+    long long ops = 0;
+    for (const SNode& n : snodes) ops += snode_ops(n);
+    if (best < 0 || ops < best) {
+      best = ops;
+      hp.groups.swap(groups);
+      hp.snodes.swap(snodes);
+      hp.f_order = order;
+    }
   }
-  // one trie over the groups' denominator products
+  hp.ops_f = best < 0 ? 0 : best;
+  hp.n_fnodes = 0;
+  for (const SNode& n : hp.snodes) hp.n_fnodes += (long long)n.items.size();
+  // one trie over the groups' denominator products, frequent factors first
   std::vector<std::vector<int>> dseq = gd;
-  order_by_frequency(dseq);
+  apply_order(dseq, kOrderLocalFreq, global_cnt);
   hp.dn.assign(1, HNode());
   for (int g = 0; g < G; ++g) hp.dn[trie_insert(hp.dn, dseq[g])].group = g;
   hp.n_dnodes = (long long)hp.dn.size() - 1;
   bool r = true;
   hp.ops_d = count_d_ops(hp, 0, &r);
+  // leaf costs on the common path of the routines in ami_device.cuh
+  const int kExpCore = 17;   // magic fma, subtract, 2 reduction fma, 12 polynomial fma, r*q
+  const int kNewton = 4, kCos = 15;
+  // every distinct integer combination of the energies (up to sign) is formed once per sample
+  {
+    std::map<std::vector<int>, int> seen;
+    auto add = [&](std::vector<int> c) {
+      int sign = 0;
+      for (int v : c)
+        if (v) { sign = v > 0 ? 1 : -1; break; }
+      if (!sign) return;
+      if (sign < 0)
+        for (int& v : c) v = -v;
+      if (seen.emplace(c, 1).second) hp.ops_combo += std::max(0, nnz(c) - 1);
+    };
+    for (const LeafF& l : ft.leafF) add(l.c);
+    for (const LeafD& l : ft.leafD) add(l.c);
+  }
+  // leaves that differ only in the derivative order share the exponential and the reciprocal
+  std::map<std::pair<std::vector<int>, int>, int> bases;   // (combination, sigma) -> highest k
+  for (const LeafF& l : ft.leafF) {
+    auto key = std::make_pair(l.c, l.sigma);
+    auto it = bases.find(key);
+    if (it == bases.end()) {
+      bases.emplace(key, l.k);
+      hp.ops_leaf_f += (l.sigma < 0 ? 1 : 0) + 1 /*beta*E*/ + kExpCore + 2 /*s+-1, fma*/ + kNewton;
+      if (l.k > 0) hp.ops_leaf_f += 2;                                  // g
+    } else if (l.k > 0 && it->second == 0) {
+      it->second = l.k;
+      hp.ops_leaf_f += 2;
+    }
+    if (l.k > 0) hp.ops_leaf_f += (l.k - 1) /*Q_k*/ + (l.k - 1) /*beta^k*/ + 3;
+  }
+  for (size_t u = 0; u < ft.leafD.size(); ++u) {
+    const LeafD& l = ft.leafD[u];
+    if (hp.d_is_real[u]) hp.ops_combo += 1 /*regulator*/ + kNewton;   // once per sample
+    else hp.ops_leaf_d += nnz(l.a) /*a.z + E*/ + 1 /*regulator*/ + std::max(0, nnz(l.a) - 1) + 2 /*|D|^2*/ + kNewton + 2;
+  }
+  const int L = ft.n_int + ft.n_ext;
+  for (int i = 0; i < ft.n_eps; ++i) {
+    std::vector<int> a(ft.sym_alpha.begin() + (size_t)i * L, ft.sym_alpha.begin() + (size_t)(i + 1) * L);
+    hp.ops_disp += 2 * (std::max(0, nnz(a) - 1) + kCos) + 2;
+  }
 }
 
 }  // namespace ami

@@ -53,21 +53,38 @@ struct FlatTable {
 struct HNode {
   int leaf = -1;             // factor of the edge into this node (Fermi leaf id or denominator leaf id)
   std::vector<int> kids;     // node ids
-  bool terminal = false;     // F-trie: a term ends here (num/den = its coefficient)
-  long long num = 0, den = 1;
   int group = -1;            // D-trie: the group whose denominator product ends here
+};
+// FT sums as a DAG: S-nodes are hash-consed across ALL groups, so a partial sum that occurs under
+// several denominator products is evaluated once (the AMI recursion produces many of those).
+struct SItem {
+  int leaf;                  // Fermi leaf of the factor
+  int child;                 // S-node multiplied by it, or -1: the item is coef * F[leaf]
+  long long num, den;        // coef when child == -1
+};
+struct SNode {
+  std::vector<SItem> items;  // S = sum of items; inner items first
+  int height = 1;
 };
 struct HGroup {
   std::vector<int> d;        // sorted denominator leaf ids (repeats = powers)
-  std::vector<HNode> f;      // f[0] = root
+  int root = -1;             // S-node of FT_g, or -1: FT_g is the constant num/den
+  long long num = 0, den = 1;
 };
 struct HornerPlan {
   std::vector<HGroup> groups;
+  std::vector<SNode> snodes; // children have smaller ids than their parents
   std::vector<HNode> dn;     // dn[0] = root
   std::vector<char> d_is_real;   // [U_D]: no external-frequency part => purely real denominator
+  int f_order = 0;           // which factor ordering won (0 = per-group frequency, 1..4 = global)
   long long n_fnodes = 0, n_dnodes = 0;
   long long ops_f = 0;       // FP64 instructions per (sample, beta) of all FT sums
   long long ops_d = 0;       // FP64 instructions per (sample, beta, frequency) of the R part
+  long long ops_leaf_f = 0;  // FP64 instructions per (sample, beta) of the Fermi/Bose leaves
+  long long ops_leaf_d = 0;  // FP64 instructions per (sample, beta, frequency) of the reciprocals
+  long long ops_disp = 0;    // FP64 instructions per sample of the dispersion
+  long long ops_combo = 0;   // FP64 instructions done once per sample: the distinct energy combinations
+                             // and the reciprocals of the purely real denominators
 };
 
 // The compiled, per-table specialised kernels (ami_jit.cpp).
@@ -104,6 +121,7 @@ struct ami_table {
   ami::FlatTable flat;
   ami::HornerPlan horner;
   ami::JitState* jit = nullptr;   // owned; see ami_jit.cpp
+  void* run_ws = nullptr;         // owned; workspace of ami_run (ami_api.cu)
   ami_device_copy dev;
   int64_t fp64_ops_flat = 0;
 };
