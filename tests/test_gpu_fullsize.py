@@ -1,0 +1,106 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times
+(ami_evaluate_momenta, the fused S1+S2+S3 call, and ami_run for the sweep), on sampled outputs the
+oracle can compute one by one, plus properties that hold at any size."""
+import numpy as np
+import pytest
+
+import ami_inputs as A
+from parity import check_parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ami():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2311_17189_b200 import build
+    build.build()
+    import paper_2311_17189_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def oracle_subset(oracle_mod, cfg, sel, betas=None):
+    """Truth for the samples `sel` of the config's counter-based sample stream, from the momenta on."""
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    k = np.concatenate([cfg.momenta(1, start=int(i)) for i in sel], axis=0)
+    e_rows = ot.dispersion(k, [cfg.q], cfg.t, cfg.mu)
+    out = []
+    for beta in (cfg.betas if betas is None else betas):
+        out.append(ot.evaluate(e_rows, cfg.z_ext, beta, e_reg=cfg.e_reg, quad=True,
+                               threads=oracle_mod.hardware_threads(), want_S=True))
+    return out
+
+
+@pytest.mark.parametrize("name,n_truth", [("cfg1", 10_000), ("cfg3", 3000), ("cfg4", 600), ("cfg5", 24)])
+def test_full_size_fused_call(ami, oracle_mod, name, n_truth):
+    import torch
+    cfg = A.get_config(name)
+    n = cfg.n_samples
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    k = tab.generate_momenta(cfg.seed, 0, n)
+    out = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg)
+    assert tab.refresh_info()["reg_plan_status"] == 0          # the specialised kernel is what ran
+    assert out.shape == (len(cfg.betas), len(cfg.z_ext), n)
+    assert bool(torch.isfinite(torch.view_as_real(out)).all())
+    sel = np.unique(np.concatenate([np.linspace(0, n - 1, n_truth).astype(np.int64), [0, 63, 64, n - 65, n - 1]]))
+    got = out[:, :, torch.from_numpy(sel).cuda()].cpu().numpy()
+    for b, (truth, S) in enumerate(oracle_subset(oracle_mod, cfg, sel)):
+        check_parity(got[b], truth, S, label=f"{name} full size beta#{b}")
+    # property at any size: the same samples evaluated as a small separate batch give the same bits
+    k_sel = k[torch.from_numpy(sel).cuda()].contiguous()
+    again = tab.evaluate_momenta(k_sel, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg)
+    assert np.array_equal(again.cpu().numpy(), got)
+
+
+@pytest.mark.parametrize("name", ["cfg2_se", "cfg2_bubble", "cfg2_bubble_doubled"])
+def test_cfg2_sweep_large_batch_streamed(ami, oracle_mod, name):
+    """N = 1e7 samples x 8 frequencies through the streamed driver with device-generated momenta
+    (1.28 GB of results, chunked), tally included; sampled parity and tally consistency."""
+    import torch
+    cfg = A.get_config(name, mu=-0.5, beta=10.0)
+    n = 10_000_000
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    d_out = torch.empty((1, 8, n), dtype=torch.complex128, device="cuda")
+    stats, sums = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, seed=cfg.seed,
+                          d_out=d_out, want_sum=True)
+    assert stats["n_chunks"] >= 5 and stats["h2d_bytes"] == 0
+    sel = np.linspace(0, n - 1, 4000).astype(np.int64)
+    got = d_out[:, :, torch.from_numpy(sel).cuda()].cpu().numpy()
+    (truth, S), = oracle_subset(oracle_mod, cfg, sel)
+    check_parity(got[0], truth, S, label=f"{name} 1e7")
+    ref = d_out[0].sum(dim=1).cpu().numpy()
+    scale = d_out[0].abs().sum(dim=1).cpu().numpy()
+    assert np.all(np.abs(sums[0] - ref) <= 1e-11 * scale)
+
+
+@pytest.mark.parametrize("n", [0, 1, 63, 64, 65, 129])
+def test_fused_edge_sizes(ami, oracle_mod, n):
+    import torch
+    cfg = A.get_config("cfg4")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    k = torch.from_numpy(cfg.momenta(n)).cuda() if n else torch.empty((0, 6, 2), dtype=torch.float64, device="cuda")
+    out = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg)
+    assert out.shape == (1, 1, n)
+    if n:
+        (truth, S), = oracle_subset(oracle_mod, cfg, np.arange(n))
+        check_parity(out.cpu().numpy()[0], truth, S, label=f"fused n={n}")
+
+
+def test_large_momenta_take_the_library_cosine(ami, oracle_mod):
+    """Momenta far outside the Brillouin zone (|K| >= 5e5) leave the bounded-range cosine."""
+    import torch
+    cfg = A.get_config("cfg3")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    k_host = cfg.momenta(256)
+    k_host[::3] += 2.0 * np.pi * 200_000        # same physics, huge argument
+    k_host[1::7] *= 1.0e5
+    k = torch.from_numpy(k_host).cuda()
+    e = tab.dispersion(k, [cfg.q], cfg.t, cfg.mu).cpu().numpy()
+    want = oracle_mod.OracleTable.from_diagram(cfg.diagram).dispersion(k_host, [cfg.q], cfg.t, cfg.mu, quad=True)
+    # the argument itself is only known to ~ulp(1e6) = 1e-10 once the momenta are that large
+    np.testing.assert_allclose(e.T, want, rtol=0, atol=5e-9)
+    e2 = torch.zeros((cfg.diagram.n_eps, 256), dtype=torch.float64, device="cuda")
+    tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_out=e2)
+    assert np.array_equal(e2.cpu().numpy(), e)
