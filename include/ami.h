@@ -86,7 +86,7 @@ typedef struct ami_info {
   int64_t table_bytes;      /* bytes of the device-resident copy (all plans) */
   int64_t fp64_ops_flat;    /* FP64 instructions per (sample,frequency,beta) of the flat term loop */
   int64_t fp64_ops_tree;    /* same for the Horner plan with n_f = n_b = 1 (FT part + R part) */
-  int64_t fp64_ops_tree_fermi; /* its FT part alone: done once per (sample,beta), not per frequency */
+  int64_t fp64_ops_tree_fermi; /* its frequency-independent part (FT sums and products under purely real denominators): once per (sample,beta) */
   int64_t fp64_ops_leaf_fermi; /* FP64 instructions per (sample,beta) of all Fermi/Bose leaves (common path) */
   int64_t fp64_ops_leaf_den;   /* FP64 instructions per (sample,beta,frequency) of the complex reciprocals */
   int64_t fp64_ops_dispersion; /* FP64 instructions per sample of ami_dispersion */

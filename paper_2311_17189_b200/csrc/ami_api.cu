@@ -190,8 +190,8 @@ int ami_table_info(const ami_table* tab, ami_info* info) {
   info->n_den_nodes = tab->horner.n_dnodes;
   info->table_bytes = tab->dev.bytes;
   info->fp64_ops_flat = tab->fp64_ops_flat;
-  info->fp64_ops_tree = tab->horner.ops_f + tab->horner.ops_d;
-  info->fp64_ops_tree_fermi = tab->horner.ops_f;
+  info->fp64_ops_tree = tab->horner.ops_f + tab->horner.ops_d_beta + tab->horner.ops_d;
+  info->fp64_ops_tree_fermi = tab->horner.ops_f + tab->horner.ops_d_beta;
   info->fp64_ops_leaf_fermi = tab->horner.ops_leaf_f;
   info->fp64_ops_leaf_den = tab->horner.ops_leaf_d;
   info->fp64_ops_dispersion = tab->horner.ops_disp;

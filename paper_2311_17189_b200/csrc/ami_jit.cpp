@@ -192,16 +192,31 @@ CV emit_cmul_acc(const HornerPlan& hp, int u, const CV& s, const CV* accp, Emitt
   return r;
 }
 
-// S_D(n): group FT at this node plus sum over kids of Dinv[kid.leaf] * S_D(kid)
-CV emit_d_sum(const HornerPlan& hp, int n, Emitter& E, Stmts& out) {
+// Frequency-independent part of S_D(n): Q(n) = [FT_g if group g ends at n] + sum over kids c with a
+// purely real denominator of Dr_c * Q(c).  Denominators are ordered complex first (ami_plan.cpp), so
+// everything below a real denominator is real.  Returns the name of the value, "" if there is none.
+std::string emit_q(const HornerPlan& hp, int n, Emitter& E, Stmts& out) {
+  std::string acc;
+  if (hp.dn[n].group >= 0) acc = "FT" + std::to_string(hp.dn[n].group);
+  for (int c : hp.dn[n].kids) {
+    if (!hp.d_is_real[hp.dn[c].leaf]) continue;
+    const std::string qc = emit_q(hp, c, E, out);   // never empty: a trie leaf carries a group
+    const std::string v = E.fresh("q"), dr = "Dr" + std::to_string(hp.dn[c].leaf);
+    if (acc.empty()) out.push_back("const double " + v + " = " + dr + " * " + qc + ";");
+    else out.push_back("const double " + v + " = fma(" + dr + ", " + qc + ", " + acc + ");");
+    acc = v;
+  }
+  return acc;
+}
+
+// S_D(n) = Q(n) + sum over kids c with a complex denominator of Dinv_c * S_D(c)
+CV emit_d_sum(const HornerPlan& hp, const std::vector<std::string>& qname, int n, Emitter& E, Stmts& out) {
   CV acc;
   bool have = false;
-  if (hp.dn[n].group >= 0) {
-    acc.re = "FT" + std::to_string(hp.dn[n].group);
-    have = true;
-  }
+  if (!qname[n].empty()) { acc.re = qname[n]; have = true; }
   for (int c : hp.dn[n].kids) {
-    const CV s = emit_d_sum(hp, c, E, out);
+    if (hp.d_is_real[hp.dn[c].leaf]) continue;
+    const CV s = emit_d_sum(hp, qname, c, E, out);
     acc = emit_cmul_acc(hp, hp.dn[c].leaf, s, have ? &acc : nullptr, E, out);
     have = true;
   }
@@ -352,6 +367,17 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     for (size_t g0 = 0; g0 < hp.groups.size(); g0 += 8)
       emit_ft_chunk(hp, g0, std::min(hp.groups.size(), g0 + 8), done, kWays, E, o, "    ");
   }
+  // frequency-independent parts of the R sums (products under purely real denominators), per beta
+  std::vector<std::string> qname(hp.dn.size());
+  {
+    std::vector<Stmts> lists;
+    for (size_t n = 0; n < hp.dn.size(); ++n) {
+      if (n != 0 && hp.d_is_real[hp.dn[n].leaf]) continue;
+      lists.emplace_back();
+      qname[n] = emit_q(hp, (int)n, E, lists.back());
+    }
+    interleave(lists, kWays, o, "    ");
+  }
   // frequencies
   o << "#pragma unroll 1\n    for (int f = 0; f < p.n_f; ++f) {\n";
   for (int x = 0; x < ft.n_ext; ++x) {
@@ -369,15 +395,17 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   }
   // R part: the subtrees under the root side by side, then the root's own sum
   {
-    const std::vector<int>& kids = hp.dn[0].kids;
+    std::vector<int> kids;
+    for (int c : hp.dn[0].kids)
+      if (!hp.d_is_real[hp.dn[c].leaf]) kids.push_back(c);
     std::vector<Stmts> lists(kids.size());
     std::vector<CV> sub(kids.size());
-    for (size_t i = 0; i < kids.size(); ++i) sub[i] = emit_d_sum(hp, kids[i], E, lists[i]);
+    for (size_t i = 0; i < kids.size(); ++i) sub[i] = emit_d_sum(hp, qname, kids[i], E, lists[i]);
     interleave(lists, kWays, o, "      ");
     Stmts tail;
     CV acc;
     bool have = false;
-    if (hp.dn[0].group >= 0) { acc.re = "FT" + std::to_string(hp.dn[0].group); have = true; }
+    if (!qname[0].empty()) { acc.re = qname[0]; have = true; }
     for (size_t i = 0; i < kids.size(); ++i) {
       acc = emit_cmul_acc(hp, hp.dn[kids[i]].leaf, sub[i], have ? &acc : nullptr, E, tail);
       have = true;

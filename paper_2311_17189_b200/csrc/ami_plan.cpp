@@ -146,21 +146,21 @@ int intern(const std::vector<TrieNode>& trie, int t, std::vector<SNode>& snodes,
   return id;
 }
 
-// returns ops; *is_real tells whether S_D(n) has no imaginary part
-long long count_d_ops(const HornerPlan& hp, int n, bool* is_real) {
-  long long ops = 0;
-  bool acc_real = true;
+// FP64 instructions of the R part as emitted by ami_jit.cpp.  Denominators are ordered complex
+// first, so the subtree under a real denominator is real and independent of the frequency: its
+// products (one instruction each) are done once per (sample, beta) [*per_beta]; an edge with a complex
+// denominator costs 2 when the sum below it is real (no complex kids), else 4 [*per_freq].
+void count_d_ops(const HornerPlan& hp, int n, long long* per_beta, long long* per_freq) {
   for (int c : hp.dn[n].kids) {
-    bool sreal = true;
-    ops += count_d_ops(hp, c, &sreal);
-    const bool dreal = hp.d_is_real[hp.dn[c].leaf] != 0;
-    // product D * S: real*real 1, real*complex or complex*real 2, complex*complex 4; a running sum
-    // is folded into the multiplies (fma)
-    ops += dreal ? (sreal ? 1 : 2) : (sreal ? 2 : 4);
-    acc_real = acc_real && dreal && sreal;
+    count_d_ops(hp, c, per_beta, per_freq);
+    if (hp.d_is_real[hp.dn[c].leaf]) {
+      *per_beta += 1;
+    } else {
+      bool sub_complex = false;
+      for (int cc : hp.dn[c].kids) sub_complex |= !hp.d_is_real[hp.dn[cc].leaf];
+      *per_freq += sub_complex ? 4 : 2;
+    }
   }
-  *is_real = acc_real;
-  return ops;
 }
 
 int nnz(const std::vector<int>& v) {
@@ -231,13 +231,22 @@ void build_horner_plan(const FlatTable& ft, HornerPlan& hp) {
   hp.n_fnodes = 0;
   for (const SNode& n : hp.snodes) hp.n_fnodes += (long long)n.items.size();
   // one trie over the groups' denominator products, frequent factors first
+  // complex denominators (those with an external frequency) first, then frequent ones first
   std::vector<std::vector<int>> dseq = gd;
-  apply_order(dseq, kOrderLocalFreq, global_cnt);
+  {
+    const std::map<int, int> cnt = occurrence(dseq);
+    for (auto& q : dseq)
+      std::stable_sort(q.begin(), q.end(), [&](int a, int b) {
+        const int ra = hp.d_is_real[a], rb = hp.d_is_real[b];
+        if (ra != rb) return ra < rb;
+        const int ca = cnt.at(a), cb = cnt.at(b);
+        return ca != cb ? ca > cb : a < b;
+      });
+  }
   hp.dn.assign(1, HNode());
   for (int g = 0; g < G; ++g) hp.dn[trie_insert(hp.dn, dseq[g])].group = g;
   hp.n_dnodes = (long long)hp.dn.size() - 1;
-  bool r = true;
-  hp.ops_d = count_d_ops(hp, 0, &r);
+  count_d_ops(hp, 0, &hp.ops_d_beta, &hp.ops_d);
   // leaf costs on the common path of the routines in ami_device.cuh
   const int kExpCore = 17;   // magic fma, subtract, 2 reduction fma, 12 polynomial fma, r*q
   const int kNewton = 4, kCos = 15;

@@ -80,6 +80,7 @@ struct HornerPlan {
   long long n_fnodes = 0, n_dnodes = 0;
   long long ops_f = 0;       // FP64 instructions per (sample, beta) of all FT sums
   long long ops_d = 0;       // FP64 instructions per (sample, beta, frequency) of the R part
+  long long ops_d_beta = 0;  // R-part products under purely real denominators: per (sample, beta) only
   long long ops_leaf_f = 0;  // FP64 instructions per (sample, beta) of the Fermi/Bose leaves
   long long ops_leaf_d = 0;  // FP64 instructions per (sample, beta, frequency) of the reciprocals
   long long ops_disp = 0;    // FP64 instructions per sample of the dispersion
