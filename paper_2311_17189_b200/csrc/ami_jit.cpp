@@ -462,7 +462,10 @@ bool jit_eligible(const FlatTable& ft, const HornerPlan& hp) {
     if (off[0] == '1') return false;
   long long leaf_doubles = (long long)ft.leafF.size();
   for (size_t u = 0; u < ft.leafD.size(); ++u) leaf_doubles += hp.d_is_real[u] ? 1 : 2;
-  return leaf_doubles <= 160 && hp.n_fnodes + 4 * hp.n_dnodes <= 24000;
+  long long max_leaf = 160, max_edges = 24000;
+  if (const char* env = getenv("AMI_JIT_MAX_LEAF_DOUBLES")) max_leaf = atoll(env);   // tuning knobs
+  if (const char* env = getenv("AMI_JIT_MAX_EDGES")) max_edges = atoll(env);
+  return leaf_doubles <= max_leaf && hp.n_fnodes + 4 * hp.n_dnodes <= max_edges;
 }
 
 // ---------------------------------------------------------------------------------------------
