@@ -127,6 +127,16 @@ def fp64_work_per_sample(info, n_f, n_b, reg):
             "terms": terms}
 
 
+def ncu_traffic(workload, fused):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+    p = os.path.join(ROOT, "profiles", "r01_dram_traffic.json")
+    if not fused or not os.path.exists(p):
+        return None
+    with open(p) as f:
+        d = json.load(f).get(workload)
+    return None if d is None else int(d["dram_bytes_read"]) + int(d["dram_bytes_write"])
+
+
 def load_measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -446,6 +456,8 @@ def run_ours(args, dist, rank, local, world):
     ms_per_step = res["total_ms"] / args.steps
     value = T * units_per_step / (ms_per_step * 1e-3)
     roof, disp = roofline_objects(res, n, n_f, n_b, plan_ops, peaks, dfma_per_s)
+    if n == cfg.n_samples:
+        roof["traffic"] = ncu_traffic(cfg.name, res["fused"])     # per launch, from profiles/ (ncu --set full)
     e2e = time_e2e(pkg, torch, res["tab"], cfg, n, max(2, args.steps // 4), 1, plan, first, dist)
     e2e_steps = max(2, args.steps // 4)
     e2e_value = T * units_per_step * e2e_steps / e2e["seconds"]

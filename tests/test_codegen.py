@@ -1,0 +1,64 @@
+"""CPU tests of the register plan's generator: the specialised kernels of every graded config are
+generated and compiled to an sm_100a cubin with NVRTC (no GPU needed), the plan's instruction counts
+are consistent, and tables outside the limits are refused."""
+import pytest
+
+import ami_inputs as A
+
+
+@pytest.fixture(scope="module")
+def ami():
+    from paper_2311_17189_b200 import build
+    build.build()
+    import paper_2311_17189_b200 as pkg
+    return pkg
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2_bubble", "cfg2_bubble_doubled", "cfg3", "cfg4", "cfg5"])
+def test_specialised_kernels_compile_for_sm100a(ami, name):
+    cfg = A.get_config(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram, device=None)
+    info = tab.info
+    assert info["reg_plan_status"] == 1
+    src = tab.kernel_source()
+    assert 'extern "C" __global__' in src and "ami_jit_eval" in src and "ami_jit_fused" in src
+    assert "oracle" not in src                       # the product shares nothing with the oracle
+    for u in range(info["n_fermi_leaves"]):
+        assert f"F{u} = " in src
+    try:
+        cubin, log = tab.kernel_cubin()
+    except ami.AmiError as e:
+        if e.code == -6:
+            pytest.skip("NVRTC library not available on this machine")
+        raise
+    assert cubin[:4] == b"\x7fELF" and len(cubin) > 10_000
+    assert "ami_jit_fused" in log and "registers" in log
+    # counts reported for the roofline: Horner plan far below the flat loop, parts add up
+    assert 0 < info["fp64_ops_tree"] < info["fp64_ops_flat"]
+    assert 0 <= info["fp64_ops_tree_fermi"] <= info["fp64_ops_tree"]
+    assert info["fp64_ops_leaf_fermi"] >= 24 * 1 and info["fp64_ops_dispersion"] >= 32 * info["n_eps"]
+
+
+def test_generated_source_is_deterministic(ami):
+    cfg = A.get_config("cfg3")
+    a = ami.AmiTable.from_diagram(cfg.diagram, device=None).kernel_source()
+    b = ami.AmiTable.from_diagram(cfg.diagram, device=None).kernel_source()
+    assert a == b
+
+
+def test_hash_consing_shares_sums_across_groups(ami):
+    """Order 6: the FT sums as one DAG need several times fewer instructions than the flat Fermi
+    products (688 terms x 6 factors)."""
+    info = ami.AmiTable.from_diagram(A.get_config("cfg4").diagram, device=None).info
+    assert info["n_terms"] == 688 and info["n_groups"] == 48
+    assert info["fp64_ops_tree"] * 20 < info["fp64_ops_flat"]
+
+
+def test_order8_is_outside_the_register_plan(ami):
+    tab = ami.AmiTable.from_diagram(A.get_config("stress8").diagram, device=None)
+    assert tab.info["reg_plan_status"] == -6
+    with pytest.raises(ami.AmiError) as ei:
+        tab.kernel_source()
+    assert ei.value.code == -6
+    with pytest.raises(ami.AmiError):      # and no kernel entry point works without a device copy
+        tab.specialize()
