@@ -88,6 +88,12 @@ int make_device_copy(ami_table* tab, int device) {
     for (int j = 0; j < nd; ++j) tix.push_back((uint16_t)(j < (int)t.d.size() ? t.d[j] : UD));
     tco.push_back((double)t.num / (double)t.den);
   }
+  // pad to whole tiles: the flat kernel stages the table through shared memory with bulk copies
+  // whose size must be a multiple of 16 bytes (padded terms are copied, never evaluated)
+  while (tco.size() % ami::kTermTile) {
+    for (int j = 0; j < ft.n_int + nd; ++j) tix.push_back(0);
+    tco.push_back(0.0);
+  }
   for (int v : ft.sym_alpha) sa.push_back((int8_t)v);
   (void)UF;
   int rc;

@@ -72,9 +72,41 @@ cudaError_t launch_dispersion(const DispParams& p, cudaStream_t st) {
 // ------------------------------------------------------------------------------------------
 // S2 + S3, flat plan: leaves once per sample, then the term table term by term.
 // ------------------------------------------------------------------------------------------
+// ---- TMA bulk copies into shared memory, completion on an mbarrier (sm_90+ PTX) ----------------
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_addr(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_addr(dst)),
+               "l"(src), "r"(bytes), "r"(smem_addr(bar))
+               : "memory");
+}
+
+// The term table is staged through shared memory in tiles of kTermTile terms, double buffered:
+// thread 0 issues the bulk copies (index rows + coefficients) of tile i+1 while the block works
+// on tile i; completion is signalled on an mbarrier per buffer.
 template <bool CE>
 __global__ void eval_flat_kernel(EvalParams p) {
   extern __shared__ double sm[];
+  __shared__ unsigned long long bar[2];
   const int tid = threadIdx.x, nt = blockDim.x;
   const long long s_raw = blockIdx.x * (long long)nt + tid;
   const long long s = s_raw < p.n_e ? s_raw : p.n_e - 1;
@@ -91,6 +123,27 @@ __global__ void eval_flat_kernel(EvalParams p) {
     }
   }
   const int stride_t = p.m_f + p.n_d;
+  // tile buffers behind the per-thread scratch: [2][kTermTile] coefficients, then [2][kTermTile][stride_t] ids
+  double* tileC = sD + (size_t)(p.U_D + 1) * 2 * nt;
+  uint16_t* tileI = reinterpret_cast<uint16_t*>(tileC + 2 * kTermTile);
+  const unsigned idx_bytes = (unsigned)(kTermTile * stride_t * sizeof(uint16_t)), coef_bytes = kTermTile * 8u;
+  const long long n_tiles = (p.T + kTermTile - 1) / kTermTile;
+  if (tid == 0) {
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  unsigned issued = 0, waited = 0;     // tiles requested / consumed so far (uniform across the block)
+  auto request = [&](long long tile) {
+    if (tid == 0) {
+      const int buf = (int)(issued & 1);
+      mbar_expect_tx(&bar[buf], idx_bytes + coef_bytes);
+      bulk_g2s(tileI + (size_t)buf * kTermTile * stride_t, p.term_idx + tile * kTermTile * stride_t, idx_bytes, &bar[buf]);
+      bulk_g2s(tileC + (size_t)buf * kTermTile, p.term_coef + tile * kTermTile, coef_bytes, &bar[buf]);
+    }
+    ++issued;
+  };
   for (int b = 0; b < p.n_b; ++b) {
     const double beta = p.beta[b];
     // ---- Fermi/Bose leaves (independent of the external frequency) ----
@@ -147,28 +200,40 @@ __global__ void eval_flat_kernel(EvalParams p) {
       }
       sD[(2 * p.U_D) * nt + tid] = 1.0;              // unit leaf fills empty denominator slots
       sD[(2 * p.U_D + 1) * nt + tid] = 0.0;
-      // ---- terms ----
+      // ---- terms, tile by tile ----
       double accr = 0.0, acci = 0.0;
-      for (long long t = 0; t < p.T; ++t) {
-        const uint16_t* ix = p.term_idx + t * stride_t;
-        cplx pr;
-        if (CE) {
-          pr = cplx{p.term_coef[t], 0.0};
-          for (int a = 0; a < p.m_f; ++a) {
-            const int u = ix[a];
-            pr = cmul(pr, cplx{sF[(2 * u) * nt + tid], sF[(2 * u + 1) * nt + tid]});
+      __syncthreads();                       // leaves of every thread written; previous pass done with the buffers
+      if (n_tiles > 0) request(0);
+      for (long long tile = 0; tile < n_tiles; ++tile) {
+        if (tile + 1 < n_tiles) request(tile + 1);      // its buffer was released by the barrier below
+        const int buf = (int)(waited & 1);
+        mbar_wait(&bar[buf], (waited >> 1) & 1);
+        ++waited;
+        const uint16_t* ti = tileI + (size_t)buf * kTermTile * stride_t;
+        const double* tc = tileC + (size_t)buf * kTermTile;
+        const int n_here = (int)((p.T - tile * kTermTile) < kTermTile ? (p.T - tile * kTermTile) : kTermTile);
+        for (int t = 0; t < n_here; ++t) {
+          const uint16_t* ix = ti + t * stride_t;
+          cplx pr;
+          if (CE) {
+            pr = cplx{tc[t], 0.0};
+            for (int a = 0; a < p.m_f; ++a) {
+              const int u = ix[a];
+              pr = cmul(pr, cplx{sF[(2 * u) * nt + tid], sF[(2 * u + 1) * nt + tid]});
+            }
+          } else {
+            double pf = tc[t];
+            for (int a = 0; a < p.m_f; ++a) pf *= sF[ix[a] * nt + tid];
+            pr = cplx{pf, 0.0};
           }
-        } else {
-          double pf = p.term_coef[t];
-          for (int a = 0; a < p.m_f; ++a) pf *= sF[ix[a] * nt + tid];
-          pr = cplx{pf, 0.0};
+          for (int d = 0; d < p.n_d; ++d) {
+            const int u = ix[p.m_f + d];
+            pr = cmul(pr, cplx{sD[(2 * u) * nt + tid], sD[(2 * u + 1) * nt + tid]});
+          }
+          accr += pr.re;
+          acci += pr.im;
         }
-        for (int d = 0; d < p.n_d; ++d) {
-          const int u = ix[p.m_f + d];
-          pr = cmul(pr, cplx{sD[(2 * u) * nt + tid], sD[(2 * u + 1) * nt + tid]});
-        }
-        accr += pr.re;
-        acci += pr.im;
+        __syncthreads();                     // everyone is done with this buffer before it is refilled
       }
       if (s_raw < p.n_e) {
         double2* o = reinterpret_cast<double2*>(p.out) +
@@ -198,8 +263,9 @@ cudaError_t launch_eval_flat(const EvalParams& p, bool ce, cudaStream_t st, int*
   if (p.n_e == 0) return cudaSuccess;
   const int W = ce ? 2 : 1;
   const size_t per_thread = sizeof(double) * ((size_t)p.n_eps * W + (size_t)p.U_F * W + 2 * ((size_t)p.U_D + 1));
+  const size_t tiles = 2 * (size_t)kTermTile * (8 + (size_t)(p.m_f + p.n_d) * sizeof(uint16_t));
   size_t smem = 0;
-  const int nt = pick_block(per_thread, 0, &smem);
+  const int nt = pick_block(per_thread, tiles, &smem);
   if (!nt) return cudaErrorInvalidConfiguration;
   auto kern = ce ? eval_flat_kernel<true> : eval_flat_kernel<false>;
   cudaError_t rc = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
