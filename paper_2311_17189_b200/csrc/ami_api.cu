@@ -1,4 +1,5 @@
 // The C ABI of include/ami.h: argument checking, device residency, launches, streamed driver.
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
@@ -339,7 +340,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
       cudaError_t crc;
       if (use_reg) {
         jb.b0 = b0; jb.n_b = nb; jb.f0 = f0; jb.n_f = nf;
-        for (int i = 0; i < nb; ++i) jb.beta[i] = beta[b0 + i];
+        for (int i = 0; i < nb; ++i) { jb.beta[i] = beta[b0 + i]; jb.ceta[i] = std::exp(beta[b0 + i] * e_reg); }
         for (int i = 0; i < nf * n_ext * 2; ++i) jb.z[i] = z_ext[(size_t)f0 * n_ext * 2 + i];
         // later launches of a split grid read the energies the first one stored
         const bool fused = mom && (first || !d_e);

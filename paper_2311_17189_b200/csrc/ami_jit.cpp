@@ -260,7 +260,6 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     if (j == combos.size()) combos.push_back(pos);
     return std::string(sign < 0 ? "-E" : "E") + std::to_string(j);
   };
-  for (const LeafF& l : ft.leafF) combo_ref(l.c);
   for (const LeafD& l : ft.leafD) combo_ref(l.c);
   for (size_t j = 0; j < combos.size(); ++j) o << "  const double E" << j << " = " << combo(combos[j], "e") << ";\n";
   // reciprocals of the denominators, kWays at a time
@@ -318,31 +317,66 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     base[b].push_back(u);
   }
   for (size_t u = 0; u < UF; ++u) o << "    double F" << u << ";\n";
+  // One exponential per ENERGY SYMBOL, e^{beta e_i} = 2^{n_i} m_i; the exponential of a leaf's
+  // combination is assembled from them: integer exponents add, mantissas multiply, so nothing can
+  // overflow and 17 FP64 instructions per leaf become one or two multiplies.
+  std::vector<char> sym_used(ft.n_eps, 0);
+  for (const auto& members : base)
+    for (int i = 0; i < ft.n_eps; ++i)
+      if (ft.leafF[members[0]].c[i]) sym_used[i] = 1;
+  std::vector<int> syms;
+  for (int i = 0; i < ft.n_eps; ++i)
+    if (sym_used[i]) syms.push_back(i);
+  for (int i : syms) o << "    int n" << i << "; double m" << i << ";\n";
+  for (size_t i0 = 0; i0 < syms.size(); i0 += kWays) {
+    const size_t n = std::min(kWays, syms.size() - i0);
+    o << "    {\n      const double x[" << n << "] = {";
+    for (size_t j = 0; j < n; ++j) o << (j ? ", " : "") << "beta * e" << syms[i0 + j];
+    o << "};\n      int nn[" << n << "]; double mm[" << n << "];\n      exp_split_n<" << n << ">(x, nn, mm);\n";
+    for (size_t j = 0; j < n; ++j)
+      o << "      n" << syms[i0 + j] << " = nn[" << j << "]; m" << syms[i0 + j] << " = mm[" << j << "];\n";
+    o << "    }\n";
+  }
+  // a leaf with x = beta (E [+ eta]) = ln(A/B): f_sigma = 1/(sigma A/B + 1) = B/(sigma A + B), with
+  // A (B) the product over the symbols with positive (negative) coefficient; A carries e^{beta eta}
+  // for sigma = -1 (P10(a)).  Exponents: A/B = 2^(Na - Nb) Ma/Mb, so d = fma(2^(Na-Nb), sigma Ma, Mb).
+  auto product = [&](const std::vector<int>& c, int sign, std::string* mant, std::string* expo) {
+    for (int i = 0; i < ft.n_eps; ++i) {
+      const int a = c[i] * sign;
+      for (int r = 0; r < a; ++r) {
+        *mant += (mant->empty() ? "" : " * ") + std::string("m") + std::to_string(i);
+        *expo += std::string(sign > 0 ? " + n" : " - n") + std::to_string(i);
+      }
+    }
+  };
   for (size_t b0 = 0; b0 < base.size(); b0 += kWays) {
     const size_t n = std::min(kWays, base.size() - b0);
-    o << "    {\n      const double x[" << n << "] = {";
+    o << "    {\n";
     for (size_t j = 0; j < n; ++j) {
       const LeafF& l = ft.leafF[base[b0 + j][0]];
-      std::string arg = combo_ref(l.c);
-      if (l.sigma < 0) arg = arg + " + p.e_reg";                  // P10(a)
-      o << (j ? ", " : "") << "beta * (" << arg << ")";
+      std::string ma, mb, ex;
+      product(l.c, +1, &ma, &ex);
+      product(l.c, -1, &mb, &ex);
+      if (l.sigma < 0) ma += (ma.empty() ? "" : " * ") + std::string("p.ceta[b]");
+      if (ma.empty()) ma = "1.0";
+      o << "      const double s" << j << " = pow2_clamped(0" << ex << "), a" << j << " = " << ma << ", b" << j << " = "
+        << (mb.empty() ? "1.0" : mb) << ";\n";
     }
-    o << "};\n      double sc[" << n << "], rq[" << n << "];\n      exp_core_n<" << n << ">(x, sc, rq);\n";
-    // 1 + e^x (sigma = +1) or e^x - 1 (sigma = -1) in one fma, then the reciprocals
     o << "      double d[" << n << "] = {";
     for (size_t j = 0; j < n; ++j)
-      o << (j ? ", " : "") << "fma(sc[" << j << "], rq[" << j << "], sc[" << j << "] "
-        << (ft.leafF[base[b0 + j][0]].sigma > 0 ? "+" : "-") << " 1.0)";
+      o << (j ? ", " : "") << "fma(s" << j << ", " << (ft.leafF[base[b0 + j][0]].sigma > 0 ? "" : "-") << "a" << j << ", b"
+        << j << ")";
     o << "};\n      fast_rcp_n<" << n << ">(d);\n";
     for (size_t j = 0; j < n; ++j) {
       const std::vector<size_t>& members = base[b0 + j];
-      const int sigma = ft.leafF[members[0]].sigma;
-      const std::string f = std::string(sigma > 0 ? "" : "-") + "d[" + std::to_string(j) + "]";
-      bool need_g = false;
+      const LeafF& l0 = ft.leafF[members[0]];
+      bool has_b = false, need_g = false;
+      for (int v : l0.c) has_b |= v < 0;
       for (size_t u : members) need_g |= ft.leafF[u].k > 0;
-      if (need_g)   // g = 1 - f = sigma e^x f  (P11)
-        o << "      const double g" << j << " = " << (sigma > 0 ? "" : "-") << "fma(sc[" << j << "], rq[" << j << "], sc["
-          << j << "]) * " << f << ";\n";
+      const std::string f = has_b ? "(b" + std::to_string(j) + " * d[" + std::to_string(j) + "])" : "d[" + std::to_string(j) + "]";
+      if (need_g)   // g = 1 - f = sigma A / (sigma A + B)  (P11)
+        o << "      const double g" << j << " = " << (l0.sigma > 0 ? "" : "-") << "(s" << j << " * a" << j << ") * d[" << j
+          << "];\n";
       for (size_t u : members) {
         const LeafF& l = ft.leafF[u];
         if (l.k == 0) {

@@ -27,6 +27,7 @@ struct AmiBatch {
   int n_f, n_b, n_f_total, f0, b0, pad;
   double e_reg, prefactor;
   double beta[AMI_K_MAX_BETA];
+  double ceta[AMI_K_MAX_BETA];          // exp(beta * e_reg), formed on the host (exactly 1 without regulator)
   double z[2 * AMI_K_MAX_FREQ_WORDS];   // [n_f][n_ext] complex
 };
 

@@ -249,36 +249,51 @@ void build_horner_plan(const FlatTable& ft, HornerPlan& hp) {
   count_d_ops(hp, 0, &hp.ops_d_beta, &hp.ops_d);
   // leaf costs on the common path of the routines in ami_device.cuh
   const int kExpCore = 17;   // magic fma, subtract, 2 reduction fma, 12 polynomial fma, r*q
-  const int kNewton = 4, kCos = 15;
-  // every distinct integer combination of the energies (up to sign) is formed once per sample
+  const int kNewton = 3, kCos = 15;   // one third-order reciprocal step = 3 fma
+  // every distinct integer combination of the energies (up to sign) that a denominator needs is
+  // formed once per sample
   {
     std::map<std::vector<int>, int> seen;
-    auto add = [&](std::vector<int> c) {
+    for (const LeafD& l : ft.leafD) {
+      std::vector<int> c = l.c;
       int sign = 0;
       for (int v : c)
         if (v) { sign = v > 0 ? 1 : -1; break; }
-      if (!sign) return;
+      if (!sign) continue;
       if (sign < 0)
         for (int& v : c) v = -v;
       if (seen.emplace(c, 1).second) hp.ops_combo += std::max(0, nnz(c) - 1);
-    };
-    for (const LeafF& l : ft.leafF) add(l.c);
-    for (const LeafD& l : ft.leafD) add(l.c);
-  }
-  // leaves that differ only in the derivative order share the exponential and the reciprocal
-  std::map<std::pair<std::vector<int>, int>, int> bases;   // (combination, sigma) -> highest k
-  for (const LeafF& l : ft.leafF) {
-    auto key = std::make_pair(l.c, l.sigma);
-    auto it = bases.find(key);
-    if (it == bases.end()) {
-      bases.emplace(key, l.k);
-      hp.ops_leaf_f += (l.sigma < 0 ? 1 : 0) + 1 /*beta*E*/ + kExpCore + 2 /*s+-1, fma*/ + kNewton;
-      if (l.k > 0) hp.ops_leaf_f += 2;                                  // g
-    } else if (l.k > 0 && it->second == 0) {
-      it->second = l.k;
-      hp.ops_leaf_f += 2;
     }
-    if (l.k > 0) hp.ops_leaf_f += (l.k - 1) /*Q_k*/ + (l.k - 1) /*beta^k*/ + 3;
+  }
+  // Fermi/Bose leaves (ami_jit.cpp): one exponential per energy symbol in use, beta*e + exp_split
+  // (17); per distinct (combination, sigma): the mantissa products, one fma, the reciprocal, and one
+  // multiply when the combination has negative coefficients; leaves that differ only in the
+  // derivative order share all of that
+  {
+    std::vector<char> used(ft.n_eps, 0);
+    std::map<std::pair<std::vector<int>, int>, int> bases;   // (combination, sigma) -> highest k
+    for (const LeafF& l : ft.leafF) {
+      auto key = std::make_pair(l.c, l.sigma);
+      auto it = bases.find(key);
+      if (it == bases.end()) {
+        bases.emplace(key, l.k);
+        int npos = 0, nneg = 0;
+        for (int i = 0; i < ft.n_eps; ++i) {
+          if (l.c[i]) used[i] = 1;
+          if (l.c[i] > 0) npos += l.c[i];
+          if (l.c[i] < 0) nneg -= l.c[i];
+        }
+        if (l.sigma < 0) npos += 1;                     // e^{beta eta}
+        hp.ops_leaf_f += std::max(0, npos - 1) + std::max(0, nneg - 1) + 1 /*fma*/ + kNewton + (nneg ? 1 : 0);
+        if (l.k > 0) hp.ops_leaf_f += 2;                // g
+      } else if (l.k > 0 && it->second == 0) {
+        it->second = l.k;
+        hp.ops_leaf_f += 2;
+      }
+      if (l.k > 0) hp.ops_leaf_f += (l.k - 1) /*Q_k*/ + (l.k - 1) /*beta^k*/ + 3;
+    }
+    for (int i = 0; i < ft.n_eps; ++i)
+      if (used[i]) hp.ops_leaf_f += 1 + kExpCore;
   }
   for (size_t u = 0; u < ft.leafD.size(); ++u) {
     const LeafD& l = ft.leafD[u];
