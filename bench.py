@@ -238,6 +238,8 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
     n_f, n_b = len(cfg.z_ext), len(cfg.betas)
     bytes_in = n * 2 * m * 8
     n_rot = int(max(2, min(8, -(-300_000_000 // max(bytes_in + n * n_eps * 8, 1)))))
+    if os.environ.get("AMI_BENCH_NROT"):      # experiment knob: 1 = every step re-reads the same (L2-resident) batch
+        n_rot = int(os.environ["AMI_BENCH_NROT"])
     ks = [tab.generate_momenta(cfg.seed, first_sample + r * n, n) for r in range(n_rot)]
     es = [torch.empty((n_eps, n), dtype=torch.float64, device="cuda") for _ in range(n_rot)] \
         if not (plan in (0, 3) and info["reg_plan_status"] in (0, 1)) else []

@@ -433,7 +433,7 @@ int ami_table_specialize(ami_table* tab) {
 int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes) {
   if (!tab || !bytes) return AMI_EINVAL;
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
-  const std::string src = ami::jit_generate_source(tab->flat, tab->horner, ami::kJitBlockThreads);
+  const std::string src = ami::jit_generate_source(tab->flat, tab->horner, ami::jit_block_threads());
   if (!buf) { *bytes = src.size() + 1; return AMI_OK; }
   if (*bytes < src.size() + 1) return AMI_EINVAL;
   memcpy(buf, src.c_str(), src.size() + 1);
@@ -446,7 +446,7 @@ int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char*
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
   std::vector<char> cubin;
   std::string lg;
-  const int rc = ami::jit_compile(ami::jit_generate_source(tab->flat, tab->horner, ami::kJitBlockThreads), cubin, lg);
+  const int rc = ami::jit_compile(ami::jit_generate_source(tab->flat, tab->horner, ami::jit_block_threads()), cubin, lg);
   if (log && log_cap) {
     const size_t nlog = std::min(log_cap - 1, lg.size());
     memcpy(log, lg.data(), nlog);

@@ -160,12 +160,18 @@ __device__ __forceinline__ void cos_bounded_n(double (&K)[N]) {
     v[j] = __hiloint2double(__double2hiint(c[j]) ^ flip, __double2loint(c[j]));
     asm volatile("" : "+d"(v[j]));   // keeps the batch together: the rare path below must not pull it apart
   }
+  // |K| >= 5e5, inf, nan anywhere in the batch: the library routine for those elements (never taken
+  // for momentum sums of a diagram).  One test per batch: the largest high word decides.
+  int big = 0;
 #pragma unroll
-  for (int j = 0; j < N; ++j) {
-    // |K| >= 5e5, inf, nan: the library routine (never taken for momentum sums of a diagram)
-    if ((__double2hiint(K[j]) & 0x7fffffff) >= 0x411e8480) v[j] = cos_unbounded(K[j]);
-    K[j] = v[j];
+  for (int j = 0; j < N; ++j) big = max(big, __double2hiint(K[j]) & 0x7fffffff);
+  if (big >= 0x411e8480) {
+#pragma unroll
+    for (int j = 0; j < N; ++j)
+      if ((__double2hiint(K[j]) & 0x7fffffff) >= 0x411e8480) v[j] = cos_unbounded(K[j]);
   }
+#pragma unroll
+  for (int j = 0; j < N; ++j) K[j] = v[j];
 }
 __device__ __forceinline__ double cos_bounded(double K) {
   double a[1] = {K};

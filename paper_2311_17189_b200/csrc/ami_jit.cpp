@@ -454,14 +454,18 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   o << "    }\n  }\n}\n\n";
   // ---- kernel 1: energies from memory ---------------------------------------------------------
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
-       "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n  if (s >= p.n) return;\n";
+       "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
+       "#pragma unroll 1\n"
+       "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n";
   for (int i = 0; i < ft.n_eps; ++i) o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
   o << "  ami_body(p, s";
   for (int i = 0; i < ft.n_eps; ++i) o << ", e" << i;
-  o << ");\n}\n\n";
+  o << ");\n  }\n}\n\n";
   // ---- kernel 2: momenta from memory, dispersion inline (Eqs. 8-18) ----------
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_fused(const __grid_constant__ AmiBatch p) {\n"
-       "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n  if (s >= p.n) return;\n"
+       "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
+       "#pragma unroll 1\n"
+       "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n"
        "  const double* ks = p.k + s * p.k_stride_sample;\n";
   for (int l = 0; l < ft.n_int; ++l)
     o << "  const double kx" << l << " = ks[" << 2 * l << " * p.k_stride_comp], ky" << l << " = ks[" << 2 * l + 1
@@ -487,8 +491,17 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
   o << "  }\n  ami_body(p, s";
   for (int i = 0; i < ft.n_eps; ++i) o << ", e" << i;
-  o << ");\n}\n";
+  o << ");\n  }\n}\n";
   return o.str();
+}
+
+int jit_block_threads() {
+  static const int nt = [] {
+    const char* e = getenv("AMI_JIT_NT");
+    const int v = e ? atoi(e) : 0;
+    return (v == 32 || v == 64 || v == 128 || v == 256) ? v : kJitBlockThreadsDefault;
+  }();
+  return nt;
 }
 
 bool jit_eligible(const FlatTable& ft, const HornerPlan& hp) {
@@ -640,7 +653,7 @@ int jit_prepare(ami_table* tab, std::string& err) {
     return js.status;
   }
   std::vector<char> cubin;
-  const std::string src = jit_generate_source(tab->flat, tab->horner, kJitBlockThreads);
+  const std::string src = jit_generate_source(tab->flat, tab->horner, jit_block_threads());
   js.status = jit_compile(src, cubin, js.log);
   if (js.status != AMI_OK) { err = js.log; return js.status; }
   Driver& d = driver();
@@ -668,8 +681,13 @@ cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cuda
   if (b.n == 0) return cudaSuccess;
   AmiBatch copy = b;
   void* args[] = {&copy};
-  const unsigned grid = (unsigned)((b.n + kJitBlockThreads - 1) / kJitBlockThreads);
-  const CUresult rc = driver().LaunchKernel(fused ? js->fn_fused : js->fn_eval, grid, 1, 1, kJitBlockThreads, 1, 1, 0,
+  // One CTA of 64 threads per 64 samples: the hardware CTA scheduler balances the SMs better than a
+  // persistent grid with a static stride does (measured: persistent + L2 prefetch of the next sample
+  // was 12 % slower on cfg3 and 5 % slower on cfg4, profiles/r01_register_plan.md).  The kernels keep
+  // their grid-stride loop, so any grid size is correct.
+  const long long blocks = (b.n + jit_block_threads() - 1) / jit_block_threads();
+  const unsigned grid = (unsigned)blocks;
+  const CUresult rc = driver().LaunchKernel(fused ? js->fn_fused : js->fn_eval, grid, 1, 1, jit_block_threads(), 1, 1, 0,
                                             (CUstream)st, args, nullptr);
   return rc == CUDA_SUCCESS ? cudaSuccess : cudaErrorLaunchFailure;
 }

@@ -10,7 +10,8 @@
 
 namespace ami {
 
-constexpr int kJitBlockThreads = 64;
+constexpr int kJitBlockThreadsDefault = 64;
+int jit_block_threads();   // kJitBlockThreadsDefault unless AMI_JIT_NT overrides it (tuning knob)
 
 // Tables whose straight-line form is small enough to live in registers and in the instruction
 // cache; larger ones are evaluated by the table-driven kernels.
