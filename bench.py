@@ -105,7 +105,7 @@ class ClockSampler:
 # algorithmic FP64 work per sample, in FP64-pipe instruction slots:
 #   W = N_eps (2 c_cos + 2)                      [S1: two cosines, one add, one fma per energy symbol]
 #     + N_b U_F c_fermi                          [S2: Fermi/Bose leaves, once per beta]
-#     + N_b N_f U_D c_den                        [S2: complex reciprocals]
+#     + N_f U_D c_den  (register plan; x N_b for the flat plan)   [S2: complex reciprocals]
 #     + N_b ops_FT + N_b N_f ops_R               [S3: Horner plan]   or   N_b N_f ops_flat  [S3: flat plan]
 # c_* = FP64-pipe instructions of the leaf routines on their common path as compiled for sm_100a
 # (cos 15, Fermi/Bose 24, complex reciprocal 8, plus the integer-coefficient sums of their arguments);
@@ -119,6 +119,7 @@ def fp64_work_per_sample(info, n_f, n_b, reg):
     fermi = n_b * int(info["fp64_ops_leaf_fermi"]) + int(info["fp64_ops_combos"])
     dens = n_b * n_f * int(info["fp64_ops_leaf_den"])
     if reg:
+        dens = n_f * int(info["fp64_ops_leaf_den"])     # complex reciprocals once per frequency, shared by all beta
         ft = int(info["fp64_ops_tree_fermi"])
         terms = n_b * ft + n_b * n_f * (int(info["fp64_ops_tree"]) - ft)
     else:

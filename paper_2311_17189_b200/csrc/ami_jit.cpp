@@ -237,13 +237,13 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     if (w >= 1 && w <= 16) kWays = (size_t)w;
   }
   Emitter E;
-  std::ostringstream o;
-  o << kAmiParamsSrc << "\n" << kAmiDeviceSrc << "\n";
-  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n";
-  // ---- body: one sample, energies e0..e{n_eps-1} in registers ------------------------------
-  o << "__device__ __forceinline__ void ami_body(const AmiBatch& p, const long long s";
-  for (int i = 0; i < ft.n_eps; ++i) o << ", const double e" << i;
-  o << ") {\n";
+  // The body of one sample is generated in four sections that are assembled twice below: once
+  // nested beta { ... frequency { ... } } and once with the beta-only work of all temperatures
+  // done first (section 1), so that the frequency-only work (section 2) is not repeated per beta.
+  //   0: once per sample   1: per beta   2: per frequency   3: per (beta, frequency)
+  std::ostringstream sec[4];
+  int cur = 0;
+#define o sec[cur]
   // every distinct integer combination of the energies, up to sign, once per sample
   std::vector<std::vector<int>> combos;
   auto combo_ref = [&](const std::vector<int>& c) -> std::string {
@@ -304,7 +304,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
       if (hp.d_is_real[u]) ids.push_back(u);
     emit_d_leaves(ids, "  ");
   }
-  o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n";
+  cur = 1;
   // Fermi/Bose leaves (independent of the external frequency), kWays at a time
   // Leaves that differ only in the derivative order share one exponential and one reciprocal.
   const size_t UF = ft.leafF.size();
@@ -413,7 +413,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     interleave(lists, kWays, o, "    ");
   }
   // frequencies
-  o << "#pragma unroll 1\n    for (int f = 0; f < p.n_f; ++f) {\n";
+  cur = 2;
   for (int x = 0; x < ft.n_ext; ++x) {
     o << "      const double zr" << x << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ")], zi" << x
       << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ") + 1];\n";
@@ -428,6 +428,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     emit_d_leaves(ids, "      ");
   }
   // R part: the subtrees under the root side by side, then the root's own sum
+  cur = 3;
   {
     std::vector<int> kids;
     for (int c : hp.dn[0].kids)
@@ -451,16 +452,40 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     o << "      *out = make_double2(p.prefactor * (" << acc.re << "), "
       << (acc.real() ? std::string("0.0") : "p.prefactor * (" + acc.im + ")") << ");\n";
   }
-  o << "    }\n  }\n}\n\n";
+#undef o
+  std::ostringstream o;
+  o << kAmiParamsSrc << "\n" << kAmiDeviceSrc << "\n";
+  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n";
+  std::string sig = "(const AmiBatch& p, const long long s";
+  for (int i = 0; i < ft.n_eps; ++i) sig += ", const double e" + std::to_string(i);
+  sig += ") {\n";
+  // ---- body for one temperature per launch: beta { frequency { } } ----------------------------
+  o << "__device__ __forceinline__ void ami_body" << sig << sec[0].str()
+    << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << sec[1].str()
+    << "#pragma unroll 1\n    for (int f = 0; f < p.n_f; ++f) {\n" << sec[2].str() << sec[3].str() << "    }\n  }\n}\n\n";
+  // ---- body for several temperatures: the per-beta values the R part needs are kept in a small
+  // per-thread array, then frequency { reciprocals once; beta { R part } } --------------------------
+  std::vector<std::string> keep;
+  for (const std::string& q : qname)
+    if (!q.empty() && std::find(keep.begin(), keep.end(), q) == keep.end()) keep.push_back(q);
+  o << "__device__ __forceinline__ void ami_body_mb" << sig << sec[0].str();
+  o << "  double kept[AMI_K_MAX_BETA][" << std::max<size_t>(keep.size(), 1) << "];\n";
+  o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << sec[1].str();
+  for (size_t i = 0; i < keep.size(); ++i) o << "    kept[b][" << i << "] = " << keep[i] << ";\n";
+  o << "  }\n#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n" << sec[2].str()
+    << "#pragma unroll 1\n    for (int b = 0; b < p.n_b; ++b) {\n";
+  for (size_t i = 0; i < keep.size(); ++i) o << "      const double " << keep[i] << " = kept[b][" << i << "];\n";
+  o << sec[3].str() << "    }\n  }\n}\n\n";
   // ---- kernel 1: energies from memory ---------------------------------------------------------
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
        "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
        "#pragma unroll 1\n"
        "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n";
   for (int i = 0; i < ft.n_eps; ++i) o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
-  o << "  ami_body(p, s";
-  for (int i = 0; i < ft.n_eps; ++i) o << ", e" << i;
-  o << ");\n  }\n}\n\n";
+  std::string call_args = "(p, s";
+  for (int i = 0; i < ft.n_eps; ++i) call_args += ", e" + std::to_string(i);
+  call_args += ");\n";
+  o << "  if (p.n_b == 1) ami_body" << call_args << "  else ami_body_mb" << call_args << "  }\n}\n\n";
   // ---- kernel 2: momenta from memory, dispersion inline (Eqs. 8-18) ----------
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_fused(const __grid_constant__ AmiBatch p) {\n"
        "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
@@ -489,9 +514,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   }
   o << "  if (p.e_out) {\n";
   for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
-  o << "  }\n  ami_body(p, s";
-  for (int i = 0; i < ft.n_eps; ++i) o << ", e" << i;
-  o << ");\n  }\n}\n";
+  o << "  }\n  if (p.n_b == 1) ami_body" << call_args << "  else ami_body_mb" << call_args << "  }\n}\n";
   return o.str();
 }
 
