@@ -237,6 +237,42 @@ def test_fused_momenta_path(ami, torch_mod, oracle_mod, name, n, plan):
         check_parity(got.cpu().numpy()[b][:, sel], truth, S, label=f"fused {name}")
 
 
+@pytest.mark.parametrize("plan", ["flat", "auto"])
+@pytest.mark.parametrize("fused", [False, True])
+def test_grid_larger_than_one_launch(ami, torch_mod, oracle_mod, plan, fused):
+    """70 frequencies x 9 temperatures do not fit one launch (64 frequency words, 8 temperatures):
+    the call is split into 2 x 2 launches; every (beta, frequency) row must land in its place."""
+    cfg = A.get_config("cfg5")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    n = 333
+    z = (np.linspace(-3.0, 3.0, 70) + 0.1j).reshape(70, 1)
+    z[5, 0] = 1j * math.pi / 5.0                     # one Matsubara point among the continued ones
+    betas = [1.0, 2.0, 3.0, 5.0, 8.0, 10.0, 13.0, 20.0, 4.0]
+    k_host = cfg.momenta(n)
+    k = torch_mod.from_numpy(k_host).cuda()
+    e = tab.dispersion(k, [cfg.q], cfg.t, cfg.mu)
+    if fused:
+        e_out = torch_mod.zeros_like(e) if plan == "auto" else None
+        out = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, z, betas, plan=PLANS[plan], e_out=e_out)
+        if e_out is not None:
+            assert torch_mod.equal(e_out, e)
+    else:
+        out = tab.evaluate(e, z, betas, plan=PLANS[plan])
+    assert out.shape == (9, 70, n)
+    out = out.cpu().numpy()
+    e_rows = e.cpu().numpy().T.copy()
+    sel = np.arange(0, n, 11)
+    for b in (0, 7, 8):        # first launch, last of the first beta chunk, the second beta chunk
+        truth, S = truth_for(oracle_mod, cfg, e_rows[sel], z, betas[b], 0.0)
+        check_parity(out[b][:, sel], truth, S, label=f"split grid beta#{b}")
+    # rows computed alone equal the rows of the split call, bit for bit
+    one = tab.evaluate(e, z[64:], [betas[8]], plan=PLANS[plan]).cpu().numpy()
+    if plan == "flat":
+        assert np.array_equal(one[0], out[8, 64:])
+    else:   # the several-temperature body keeps per-beta values in memory: same arithmetic, same bits
+        assert np.array_equal(one[0], out[8, 64:])
+
+
 # ------------------------------------------------------------------ S4 streamed driver
 def test_generated_momenta_bitwise(ami, torch_mod):
     """P22: device generator == host generator, bit for bit."""
