@@ -243,12 +243,12 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
         n_rot = int(os.environ["AMI_BENCH_NROT"])
     ks = [tab.generate_momenta(cfg.seed, first_sample + r * n, n) for r in range(n_rot)]
     es = [torch.empty((n_eps, n), dtype=torch.float64, device="cuda") for _ in range(n_rot)] \
-        if not (plan in (0, 3) and info["reg_plan_status"] in (0, 1)) else []
+        if not (plan in (0, 2) and info["reg_plan_status"] in (0, 1)) else []
     out = torch.empty((n_b, n_f, n), dtype=torch.complex128, device="cuda")
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
     t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
-    reg = plan in (0, 3) and info["reg_plan_status"] in (0, 1)
+    reg = plan in (0, 2) and info["reg_plan_status"] in (0, 1)
     if reg:
         info = tab.specialize()        # NVRTC compile + load happen here, outside every timed region
 
@@ -388,7 +388,7 @@ def time_e2e(pkg, torch, tab, cfg, n, steps, warmup, plan, first_sample, dist):
             "finite": bool(torch.isfinite(torch.view_as_real(h_out[0, 0, :1024])).all().item())}
 
 
-def roofline_objects(res, n, n_f, n_b, plan_ops, peaks, dfma_per_s):
+def roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s):
     """Roofline of the dominant kernel: FP64-pipe bound.  Work counted in FP64-pipe instruction slots
     per sample, expressed as DFMA-equivalent TFLOP/s (slot = 2 flop) against the DFMA-chain
     rate measured in this run; the HBM leg is reported beside it.  With the register plan the step is
@@ -423,14 +423,14 @@ def roofline_objects(res, n, n_f, n_b, plan_ops, peaks, dfma_per_s):
     return roof, disp
 
 
-PLAN_IDS = {"auto": 0, "flat": 1, "reg": 3}
+PLAN_IDS = {"auto": 0, "flat": 1, "reg": 2}
 
 
-def plan_ops_for(info, plan):
-    """Term-loop FP64 slots per (sample, frequency, beta) of the representation ami_evaluate executes."""
+def plan_name_of(info, plan):
+    """Name of the representation ami_evaluate executes (after specialisation has been tried)."""
     if plan != "flat" and info["reg_plan_status"] == 0:
-        return int(info["fp64_ops_tree"]), "register (Horner, NVRTC-specialised)"
-    return int(info["fp64_ops_flat"]), "flat (table-driven)"
+        return "register (Horner DAG, NVRTC-specialised)"
+    return "flat (table-driven)"
 
 
 def run_ours(args, dist, rank, local, world):
@@ -454,11 +454,11 @@ def run_ours(args, dist, rank, local, world):
                         use_graph=not args.no_graph)
     info = res["info"]
     T = int(info["n_terms"])
-    plan_ops, plan_name = plan_ops_for(info, args.plan)
+    plan_name = plan_name_of(info, args.plan)
     units_per_step = n * n_f * n_b * world
     ms_per_step = res["total_ms"] / args.steps
     value = T * units_per_step / (ms_per_step * 1e-3)
-    roof, disp = roofline_objects(res, n, n_f, n_b, plan_ops, peaks, dfma_per_s)
+    roof, disp = roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s)
     if n == cfg.n_samples:
         roof["traffic"] = ncu_traffic(cfg.name, res["fused"])     # per launch, from profiles/ (ncu --set full)
     e2e = time_e2e(pkg, torch, res["tab"], cfg, n, max(2, args.steps // 4), 1, plan, first, dist)
@@ -497,9 +497,9 @@ def run_ours(args, dist, rank, local, world):
             r2 = time_workload(pkg, torch, c2, c2.n_samples, 20, 3, plan, 0, None, sample_clocks=False,
                                use_graph=not args.no_graph)
             i2 = r2["info"]
-            ops2, pn2 = plan_ops_for(i2, args.plan)
+            pn2 = plan_name_of(i2, args.plan)
             f2, b2 = len(c2.z_ext), len(c2.betas)
-            roof2, disp2 = roofline_objects(r2, c2.n_samples, f2, b2, ops2, peaks, dfma_per_s)
+            roof2, disp2 = roofline_objects(r2, c2.n_samples, f2, b2, peaks, dfma_per_s)
             ms2 = r2["total_ms"] / 20
             others[name] = {"T_flat": int(i2["n_terms"]), "samples": c2.n_samples, "n_freq": f2, "n_beta": b2,
                             "plan": pn2, "ms_per_step": ms2, "eval_ms": r2["eval_ms"], "disp_ms": r2["disp_ms"],

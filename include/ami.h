@@ -64,8 +64,7 @@ typedef struct ami_table ami_table;
 enum {
   AMI_PLAN_AUTO = 0,  /* the library's fastest plan for this table */
   AMI_PLAN_FLAT = 1,  /* the flat term table, term by term, table-driven (SURVEY 8(a) S3 as written) */
-  AMI_PLAN_TREE = 2,  /* reserved for a table-driven form of the Horner plan; runs the flat kernel today */
-  AMI_PLAN_REG = 3    /* register plan: the table written out as a straight-line kernel specialised to
+  AMI_PLAN_REG = 2    /* register plan: the table written out as a straight-line kernel specialised to
                          this diagram (terms grouped by denominator product, Fermi/Bose and denominator
                          products in Horner form, every leaf a register), compiled with NVRTC on first
                          use; real energies and tables within the size limits only */

@@ -12,7 +12,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libami_b200.so")
 
-PLAN_AUTO, PLAN_FLAT, PLAN_TREE, PLAN_REG = 0, 1, 2, 3
+PLAN_AUTO, PLAN_FLAT, PLAN_REG = 0, 1, 2
 
 EXPORTS = [
     "ami_construct", "ami_table_info", "ami_table_export", "ami_table_destroy", "ami_dispersion",

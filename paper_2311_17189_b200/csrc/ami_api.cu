@@ -266,7 +266,7 @@ void fill_table_params(const ami_table* tab, ami::EvalParams& p) {
 // register plan was asked for explicitly and cannot be had.
 int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg) {
   *use_reg = false;
-  if (plan == AMI_PLAN_FLAT || plan == AMI_PLAN_TREE) return AMI_OK;
+  if (plan == AMI_PLAN_FLAT) return AMI_OK;
   if (e_is_complex || !ami::jit_eligible(tab->flat, tab->horner)) {
     if (plan == AMI_PLAN_REG) { g_cuda_err = "register plan unavailable for this table / energy type"; return AMI_EUNSUPPORTED; }
     return AMI_OK;
