@@ -478,6 +478,8 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   o << sec[3].str() << "    }\n  }\n}\n\n";
   // ---- kernel 1: energies from memory ---------------------------------------------------------
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
+       "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
+       "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
        "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
        "#pragma unroll 1\n"
        "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n";
@@ -488,6 +490,8 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   o << "  if (p.n_b == 1) ami_body" << call_args << "  else ami_body_mb" << call_args << "  }\n}\n\n";
   // ---- kernel 2: momenta from memory, dispersion inline (Eqs. 8-18) ----------
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_fused(const __grid_constant__ AmiBatch p) {\n"
+       "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
+       "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
        "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
        "#pragma unroll 1\n"
        "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n"
@@ -635,6 +639,7 @@ struct Driver {
   CUresult (*LaunchKernel)(CUfunction, unsigned, unsigned, unsigned, unsigned, unsigned, unsigned, unsigned, CUstream,
                            void**, void**) = nullptr;
   CUresult (*GetErrorString)(CUresult, const char**) = nullptr;
+  CUresult (*LaunchKernelEx)(const CUlaunchConfig*, CUfunction, void**, void**) = nullptr;   // optional
   bool ok = false;
 };
 
@@ -651,6 +656,7 @@ Driver& driver() {
            get("cuModuleGetFunction", (void**)&d.ModuleGetFunction) &&
            get("cuModuleUnload", (void**)&d.ModuleUnload) && get("cuLaunchKernel", (void**)&d.LaunchKernel) &&
            get("cuGetErrorString", (void**)&d.GetErrorString);
+    get("cuLaunchKernelEx", (void**)&d.LaunchKernelEx);
   });
   return d;
 }
@@ -710,8 +716,26 @@ cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cuda
   // their grid-stride loop, so any grid size is correct.
   const long long blocks = (b.n + jit_block_threads() - 1) / jit_block_threads();
   const unsigned grid = (unsigned)blocks;
-  const CUresult rc = driver().LaunchKernel(fused ? js->fn_fused : js->fn_eval, grid, 1, 1, jit_block_threads(), 1, 1, 0,
-                                            (CUstream)st, args, nullptr);
+  // Programmatic dependent launch: the kernels begin with griddepcontrol.launch_dependents + .wait, so
+  // the NEXT specialised kernel in the stream may be scheduled while this one drains and starts the
+  // moment it has completed (stream order is kept: nothing is read or written before the wait).
+  static const bool pdl = [] { const char* e = getenv("AMI_JIT_PDL"); return !(e && e[0] == '0'); }();
+  CUresult rc;
+  CUfunction fn = fused ? js->fn_fused : js->fn_eval;
+  if (pdl && driver().LaunchKernelEx) {
+    CUlaunchAttribute attr;
+    memset(&attr, 0, sizeof attr);
+    attr.id = CU_LAUNCH_ATTRIBUTE_PROGRAMMATIC_STREAM_SERIALIZATION;
+    attr.value.programmaticStreamSerializationAllowed = 1;
+    CUlaunchConfig cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDimX = grid; cfg.gridDimY = 1; cfg.gridDimZ = 1;
+    cfg.blockDimX = (unsigned)jit_block_threads(); cfg.blockDimY = 1; cfg.blockDimZ = 1;
+    cfg.sharedMemBytes = 0; cfg.hStream = (CUstream)st; cfg.attrs = &attr; cfg.numAttrs = 1;
+    rc = driver().LaunchKernelEx(&cfg, fn, args, nullptr);
+  } else {
+    rc = driver().LaunchKernel(fn, grid, 1, 1, jit_block_threads(), 1, 1, 0, (CUstream)st, args, nullptr);
+  }
   return rc == CUDA_SUCCESS ? cudaSuccess : cudaErrorLaunchFailure;
 }
 
