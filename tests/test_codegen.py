@@ -62,3 +62,19 @@ def test_order8_is_outside_the_register_plan(ami):
     assert ei.value.code == -6
     with pytest.raises(ami.AmiError):      # and no kernel entry point works without a device copy
         tab.specialize()
+
+
+def test_register_plan_can_be_switched_off():
+    """AMI_DISABLE_JIT=1: every table reports the register plan as unavailable, so AMI_PLAN_AUTO runs
+    the table-driven kernels (checked in a fresh process: the switch is read per call)."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = ("import ami_inputs as A, paper_2311_17189_b200 as P;"
+            "t = P.AmiTable.from_diagram(A.get_config('cfg3').diagram, device=None);"
+            "print(t.info['reg_plan_status'])")
+    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, cwd=root,
+                         env=dict(os.environ, AMI_DISABLE_JIT="1"), timeout=120)
+    assert out.returncode == 0, out.stderr
+    assert out.stdout.strip() == "-6"
