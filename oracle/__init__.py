@@ -91,8 +91,8 @@ class OracleTable:
         return cls(d.n_int, d.n_ext, d.alpha, d.eps, d.slot_is_fermionic, sum_order, prefactor)
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            lib().oracle_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:   # _lib is gone at interpreter shutdown
+            _lib.oracle_destroy(self._h)
             self._h = None
 
     def info(self) -> dict:

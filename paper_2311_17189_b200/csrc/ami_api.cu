@@ -345,8 +345,9 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
         // later launches of a split grid read the energies the first one stored
         const bool fused = mom && (first || !d_e);
         if (!fused) { jb.e_out = nullptr; }
-        crc = jit_launch(tab, fused, jb, st);
-        if (crc == cudaSuccess) count_external_launch(launches);
+        int n_launched = 0;
+        crc = jit_launch(tab, fused, jb, st, &n_launched);
+        for (int i = 0; i < n_launched; ++i) count_external_launch(launches);
       } else {
         p.b0 = b0; p.n_b = nb; p.f0 = f0; p.n_f = nf;
         for (int i = 0; i < nb; ++i) p.beta[i] = beta[b0 + i];
@@ -433,7 +434,8 @@ int ami_table_specialize(ami_table* tab) {
 int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes) {
   if (!tab || !bytes) return AMI_EINVAL;
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
-  const std::string src = ami::jit_generate_source(tab->flat, tab->horner, ami::jit_block_threads());
+  const bool scratch = ami::jit_mode(tab->flat, tab->horner) == ami::kJitScratch;
+  const std::string src = ami::jit_generate_source(tab->flat, tab->horner, scratch ? 64 : ami::jit_block_threads(), scratch, nullptr);
   if (!buf) { *bytes = src.size() + 1; return AMI_OK; }
   if (*bytes < src.size() + 1) return AMI_EINVAL;
   memcpy(buf, src.c_str(), src.size() + 1);
@@ -446,7 +448,9 @@ int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char*
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
   std::vector<char> cubin;
   std::string lg;
-  const int rc = ami::jit_compile(ami::jit_generate_source(tab->flat, tab->horner, ami::jit_block_threads()), cubin, lg);
+  const bool scratch = ami::jit_mode(tab->flat, tab->horner) == ami::kJitScratch;
+  const int rc = ami::jit_compile(
+      ami::jit_generate_source(tab->flat, tab->horner, scratch ? 64 : ami::jit_block_threads(), scratch, nullptr), cubin, lg);
   if (log && log_cap) {
     const size_t nlog = std::min(log_cap - 1, lg.size());
     memcpy(log, lg.data(), nlog);

@@ -151,6 +151,67 @@ void emit_ft_chunk(const HornerPlan& hp, size_t g0, size_t g1, std::vector<char>
   }
 }
 
+// ---- memory-backed variant for tables too large for registers ------------------------------------
+// Long-lived values live in a per-thread column of a global scratch array (slot i at W(i)); the
+// generated text names them through macros, so the emitters below and above are shared.  The FT DAG
+// is written depth first: a sum is formed right before its first use, kept in its slot while other
+// sums still need it (slots are recycled after the last use), and single-use sums stay in registers.
+struct SlotPool {
+  std::vector<int> free_list;
+  int next = 0, peak = 0;
+  int take() {
+    if (!free_list.empty()) { const int s = free_list.back(); free_list.pop_back(); return s; }
+    peak = std::max(peak, next + 1);
+    return next++;
+  }
+  void give(int s) { free_list.push_back(s); }
+};
+
+struct DfsState {
+  std::vector<int> uses_left;    // remaining uses of each S-node
+  std::vector<int> slot;         // scratch slot of a computed shared node, -1 otherwise
+  std::vector<char> done;
+  SlotPool pool;
+  int base = 0;                  // first scratch slot of the pool
+};
+
+// value of S-node `id` as an expression usable once; emits what is needed into `out`
+std::string emit_snode_dfs(const HornerPlan& hp, int id, DfsState& st, Emitter& E, Stmts& out) {
+  auto consume = [&](int n) {
+    if (--st.uses_left[n] == 0 && st.slot[n] >= 0) { st.pool.give(st.slot[n]); st.slot[n] = -1; }
+  };
+  if (st.done[id]) {             // shared and already computed: read it back
+    const std::string v = E.fresh("s");
+    out.push_back("const double " + v + " = W(" + std::to_string(st.base + st.slot[id]) + ");");
+    consume(id);
+    return v;
+  }
+  const SNode& n = hp.snodes[id];
+  std::string acc;
+  for (size_t i = 0; i < n.items.size(); ++i) {
+    const SItem& it = n.items[i];
+    const std::string v = E.fresh("s");
+    const std::string leaf = "F" + std::to_string(it.leaf);
+    if (it.child >= 0) {
+      const std::string sc = emit_snode_dfs(hp, it.child, st, E, out);
+      if (acc.empty()) out.push_back("const double " + v + " = " + leaf + " * " + sc + ";");
+      else out.push_back("const double " + v + " = fma(" + leaf + ", " + sc + ", " + acc + ");");
+    } else {
+      const std::string coef = dlit((double)it.num / (double)it.den);
+      if (acc.empty()) out.push_back("const double " + v + " = " + coef + " * " + leaf + ";");
+      else out.push_back("const double " + v + " = fma(" + coef + ", " + leaf + ", " + acc + ");");
+    }
+    acc = v;
+  }
+  st.done[id] = 1;
+  if (st.uses_left[id] > 1) {    // needed again later: park it in a slot
+    st.slot[id] = st.pool.take();
+    out.push_back("W(" + std::to_string(st.base + st.slot[id]) + ") = " + acc + ";");
+  }
+  consume(id);
+  return acc;
+}
+
 struct CV {            // a complex value held in named doubles; im empty = purely real
   std::string re, im;
   bool real() const { return im.empty(); }
@@ -229,7 +290,8 @@ CV emit_d_sum(const HornerPlan& hp, const std::vector<std::string>& qname, int n
 // ---------------------------------------------------------------------------------------------
 // The translation unit handed to NVRTC.
 // ---------------------------------------------------------------------------------------------
-std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int block_threads) {
+std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int block_threads, bool scratch,
+                                int* scratch_slots) {
   const int L = ft.n_int + ft.n_ext;
   size_t kWays = 4;           // independent chains kept side by side
   if (const char* env = getenv("AMI_JIT_WAYS")) {   // tuning knob (profiles/)
@@ -264,7 +326,8 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   for (size_t j = 0; j < combos.size(); ++j) o << "  const double E" << j << " = " << combo(combos[j], "e") << ";\n";
   // reciprocals of the denominators, kWays at a time
   auto emit_d_leaves = [&](const std::vector<size_t>& ids, const std::string& ind) {
-    for (size_t u : ids) o << ind << "double Dr" << u << (hp.d_is_real[u] ? "" : ", Di" + std::to_string(u)) << ";\n";
+    if (!scratch)
+      for (size_t u : ids) o << ind << "double Dr" << u << (hp.d_is_real[u] ? "" : ", Di" + std::to_string(u)) << ";\n";
     for (size_t i0 = 0; i0 < ids.size(); i0 += kWays) {
       const size_t n = std::min(kWays, ids.size() - i0);
       o << ind << "{\n";
@@ -316,7 +379,8 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     if (b == base.size()) base.emplace_back();
     base[b].push_back(u);
   }
-  for (size_t u = 0; u < UF; ++u) o << "    double F" << u << ";\n";
+  if (!scratch)
+    for (size_t u = 0; u < UF; ++u) o << "    double F" << u << ";\n";
   // One exponential per ENERGY SYMBOL, e^{beta e_i} = 2^{n_i} m_i; the exponential of a leaf's
   // combination is assembled from them: integer exponents add, mantissas multiply, so nothing can
   // overflow and 17 FP64 instructions per leaf become one or two multiplies.
@@ -396,11 +460,42 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     o << "    }\n";
   }
   // FT sums of every group (per beta): a DAG shared by all groups, emitted eight groups at a time
-  {
+  // scratch layout: [Dr/Di of every denominator][FT of every group][Q of every R-trie node][pool of shared sums]
+  std::vector<int> slot_dr(ft.leafD.size(), -1), slot_di(ft.leafD.size(), -1), slot_ft(hp.groups.size(), -1);
+  int n_slots = 0;
+  for (size_t u = 0; u < ft.leafD.size(); ++u) {
+    slot_dr[u] = n_slots++;
+    if (!hp.d_is_real[u]) slot_di[u] = n_slots++;
+  }
+  for (size_t g = 0; g < hp.groups.size(); ++g) slot_ft[g] = n_slots++;
+  const int slot_q0 = n_slots;
+  n_slots += (int)hp.dn.size();
+  DfsState dfs;
+  if (!scratch) {
     std::vector<char> done(hp.snodes.size(), 0);
     for (size_t g0 = 0; g0 < hp.groups.size(); g0 += 8)
       emit_ft_chunk(hp, g0, std::min(hp.groups.size(), g0 + 8), done, kWays, E, o, "    ");
+  } else {
+    dfs.uses_left.assign(hp.snodes.size(), 0);
+    dfs.slot.assign(hp.snodes.size(), -1);
+    dfs.done.assign(hp.snodes.size(), 0);
+    dfs.base = n_slots;
+    for (const SNode& n : hp.snodes)
+      for (const SItem& it : n.items)
+        if (it.child >= 0) ++dfs.uses_left[it.child];
+    for (const HGroup& g : hp.groups)
+      if (g.root >= 0) ++dfs.uses_left[g.root];
+    for (size_t g = 0; g < hp.groups.size(); ++g) {
+      const HGroup& hg = hp.groups[g];
+      Stmts lst;
+      const std::string v = hg.root >= 0 ? emit_snode_dfs(hp, hg.root, dfs, E, lst) : dlit((double)hg.num / (double)hg.den);
+      o << "    {\n";
+      for (const std::string& st : lst) o << "      " << st << "\n";
+      o << "      FT" << g << " = " << v << ";\n    }\n";
+    }
+    n_slots += dfs.pool.peak;
   }
+  if (scratch_slots) *scratch_slots = scratch ? n_slots : 0;
   // frequency-independent parts of the R sums (products under purely real denominators), per beta
   std::vector<std::string> qname(hp.dn.size());
   {
@@ -409,6 +504,11 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
       if (n != 0 && hp.d_is_real[hp.dn[n].leaf]) continue;
       lists.emplace_back();
       qname[n] = emit_q(hp, (int)n, E, lists.back());
+      if (scratch && !qname[n].empty() && qname[n][0] == 'q') {     // keep it in memory until the R part reads it
+        const std::string w = "W(" + std::to_string(slot_q0 + (int)n) + ")";
+        lists.back().push_back(w + " = " + qname[n] + ";");
+        qname[n] = w;
+      }
     }
     interleave(lists, kWays, o, "    ");
   }
@@ -458,6 +558,18 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n";
   std::string sig = "(const AmiBatch& p, const long long s";
   for (int i = 0; i < ft.n_eps; ++i) sig += ", const double e" + std::to_string(i);
+  if (scratch) {
+    sig += ", double* __restrict__ w, const long long ws";
+    // volatile: every scratch access happens where it is written.  Without it the compiler hoists
+    // thousands of loads to the top of the straight-line body and then spills them again.
+    o << "extern __shared__ double sF[];\n#define W(i) ((volatile double*)w)[(long long)(i) * ws]\n";
+    for (size_t u = 0; u < ft.leafF.size(); ++u) o << "#define F" << u << " sF[" << u << " * AMI_NT + threadIdx.x]\n";
+    for (size_t u = 0; u < ft.leafD.size(); ++u) {
+      o << "#define Dr" << u << " W(" << slot_dr[u] << ")\n";
+      if (slot_di[u] >= 0) o << "#define Di" << u << " W(" << slot_di[u] << ")\n";
+    }
+    for (size_t g = 0; g < hp.groups.size(); ++g) o << "#define FT" << g << " W(" << slot_ft[g] << ")\n";
+  }
   sig += ") {\n";
   // ---- body for one temperature per launch: beta { frequency { } } ----------------------------
   o << "__device__ __forceinline__ void ami_body" << sig << sec[0].str()
@@ -466,8 +578,10 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   // ---- body for several temperatures: the per-beta values the R part needs are kept in a small
   // per-thread array, then frequency { reciprocals once; beta { R part } } --------------------------
   std::vector<std::string> keep;
+  if (!scratch)
   for (const std::string& q : qname)
     if (!q.empty() && std::find(keep.begin(), keep.end(), q) == keep.end()) keep.push_back(q);
+  if (!scratch) {
   o << "__device__ __forceinline__ void ami_body_mb" << sig << sec[0].str();
   o << "  double kept[AMI_K_MAX_BETA][" << std::max<size_t>(keep.size(), 1) << "];\n";
   o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << sec[1].str();
@@ -476,6 +590,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     << "#pragma unroll 1\n    for (int b = 0; b < p.n_b; ++b) {\n";
   for (size_t i = 0; i < keep.size(); ++i) o << "      const double " << keep[i] << " = kept[b][" << i << "];\n";
   o << sec[3].str() << "    }\n  }\n}\n\n";
+  }
   // ---- kernel 1: energies from memory ---------------------------------------------------------
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
        "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
@@ -486,8 +601,10 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   for (int i = 0; i < ft.n_eps; ++i) o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
   std::string call_args = "(p, s";
   for (int i = 0; i < ft.n_eps; ++i) call_args += ", e" + std::to_string(i);
-  call_args += ");\n";
-  o << "  if (p.n_b == 1) ami_body" << call_args << "  else ami_body_mb" << call_args << "  }\n}\n\n";
+  call_args += scratch ? ", p.scratch + s, p.scratch_stride);\n" : ");\n";
+  const std::string call = scratch ? "  ami_body" + call_args
+                                   : "  if (p.n_b == 1) ami_body" + call_args + "  else ami_body_mb" + call_args;
+  o << call << "  }\n}\n\n";
   // ---- kernel 2: momenta from memory, dispersion inline (Eqs. 8-18) ----------
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_fused(const __grid_constant__ AmiBatch p) {\n"
        "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
@@ -518,7 +635,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   }
   o << "  if (p.e_out) {\n";
   for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
-  o << "  }\n  if (p.n_b == 1) ami_body" << call_args << "  else ami_body_mb" << call_args << "  }\n}\n";
+  o << "  }\n" << call << "  }\n}\n";
   return o.str();
 }
 
@@ -531,16 +648,26 @@ int jit_block_threads() {
   return nt;
 }
 
-bool jit_eligible(const FlatTable& ft, const HornerPlan& hp) {
+int jit_mode(const FlatTable& ft, const HornerPlan& hp) {
   if (const char* off = getenv("AMI_DISABLE_JIT"))
-    if (off[0] == '1') return false;
+    if (off[0] == '1') return kJitNone;
   long long leaf_doubles = (long long)ft.leafF.size();
   for (size_t u = 0; u < ft.leafD.size(); ++u) leaf_doubles += hp.d_is_real[u] ? 1 : 2;
-  long long max_leaf = 160, max_edges = 24000;
+  long long max_leaf = 160, max_edges = 24000, max_scratch_edges = 400000;
   if (const char* env = getenv("AMI_JIT_MAX_LEAF_DOUBLES")) max_leaf = atoll(env);   // tuning knobs
   if (const char* env = getenv("AMI_JIT_MAX_EDGES")) max_edges = atoll(env);
-  return leaf_doubles <= max_leaf && hp.n_fnodes + 4 * hp.n_dnodes <= max_edges;
+  if (const char* env = getenv("AMI_JIT_MAX_SCRATCH_EDGES")) max_scratch_edges = atoll(env);
+  const long long edges = hp.n_fnodes + 4 * hp.n_dnodes;
+  if (leaf_doubles <= max_leaf && edges <= max_edges) return kJitRegister;
+  // memory-backed variant: Fermi/Bose leaves in shared memory (64 threads per CTA), the rest in scratch.
+  // Opt-in (AMI_JIT_SCRATCH=1): NVRTC needs minutes for bodies of this size (order 7: 90 s, order 8: 270 s).
+  const char* opt_in = getenv("AMI_JIT_SCRATCH");
+  if (opt_in && opt_in[0] == '1' && (long long)ft.leafF.size() * 64 * 8 <= 200 * 1024 && edges <= max_scratch_edges)
+    return kJitScratch;
+  return kJitNone;
 }
+
+bool jit_eligible(const FlatTable& ft, const HornerPlan& hp) { return jit_mode(ft, hp) != kJitNone; }
 
 // ---------------------------------------------------------------------------------------------
 // NVRTC, loaded on demand (the library itself does not link against it)
@@ -592,6 +719,11 @@ int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& l
   }
   std::vector<const char*> opts = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "--ptxas-options=-v",
                                    "-default-device"};
+  std::string popt;
+  if (const char* env = getenv("AMI_JIT_PTXAS_OPT")) {   // tuning knob: e.g. -O1
+    popt = std::string("--ptxas-options=") + env;
+    opts.push_back(popt.c_str());
+  }
   std::string maxreg;
   if (const char* env = getenv("AMI_JIT_MAXREG")) {   // tuning knob (profiles/): cap registers per thread
     maxreg = std::string("--maxrregcount=") + env;
@@ -628,6 +760,10 @@ struct JitState {
   std::string log;
   CUmodule mod = nullptr;
   CUfunction fn_eval = nullptr, fn_fused = nullptr;
+  int mode = kJitNone;
+  int block = 0;            // threads per CTA the kernels were generated for
+  int scratch_slots = 0;    // doubles of global scratch per sample (memory-backed variant)
+  unsigned smem_bytes = 0;  // dynamic shared memory per CTA (memory-backed variant)
 };
 
 namespace {
@@ -640,6 +776,7 @@ struct Driver {
                            void**, void**) = nullptr;
   CUresult (*GetErrorString)(CUresult, const char**) = nullptr;
   CUresult (*LaunchKernelEx)(const CUlaunchConfig*, CUfunction, void**, void**) = nullptr;   // optional
+  CUresult (*FuncSetAttribute)(CUfunction, CUfunction_attribute, int) = nullptr;
   bool ok = false;
 };
 
@@ -657,6 +794,7 @@ Driver& driver() {
            get("cuModuleUnload", (void**)&d.ModuleUnload) && get("cuLaunchKernel", (void**)&d.LaunchKernel) &&
            get("cuGetErrorString", (void**)&d.GetErrorString);
     get("cuLaunchKernelEx", (void**)&d.LaunchKernelEx);
+    d.ok = d.ok && get("cuFuncSetAttribute", (void**)&d.FuncSetAttribute);
   });
   return d;
 }
@@ -682,7 +820,10 @@ int jit_prepare(ami_table* tab, std::string& err) {
     return js.status;
   }
   std::vector<char> cubin;
-  const std::string src = jit_generate_source(tab->flat, tab->horner, jit_block_threads());
+  js.mode = jit_mode(tab->flat, tab->horner);
+  js.block = js.mode == kJitScratch ? 64 : jit_block_threads();
+  const std::string src = jit_generate_source(tab->flat, tab->horner, js.block, js.mode == kJitScratch, &js.scratch_slots);
+  js.smem_bytes = js.mode == kJitScratch ? (unsigned)(tab->flat.leafF.size() * js.block * sizeof(double)) : 0u;
   js.status = jit_compile(src, cubin, js.log);
   if (js.status != AMI_OK) { err = js.log; return js.status; }
   Driver& d = driver();
@@ -692,6 +833,10 @@ int jit_prepare(ami_table* tab, std::string& err) {
   CUresult rc = d.ModuleLoadData(&js.mod, cubin.data());
   if (rc == CUDA_SUCCESS) rc = d.ModuleGetFunction(&js.fn_eval, js.mod, "ami_jit_eval");
   if (rc == CUDA_SUCCESS) rc = d.ModuleGetFunction(&js.fn_fused, js.mod, "ami_jit_fused");
+  if (rc == CUDA_SUCCESS && js.smem_bytes > 48 * 1024) {
+    rc = d.FuncSetAttribute(js.fn_eval, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)js.smem_bytes);
+    if (rc == CUDA_SUCCESS) rc = d.FuncSetAttribute(js.fn_fused, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)js.smem_bytes);
+  }
   if (rc != CUDA_SUCCESS) {
     const char* msg = nullptr;
     d.GetErrorString(rc, &msg);
@@ -704,23 +849,20 @@ int jit_prepare(ami_table* tab, std::string& err) {
   return AMI_OK;
 }
 
-cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cudaStream_t st) {
-  const JitState* js = tab->jit;
-  if (!js || js->status != AMI_OK) return cudaErrorInvalidDeviceFunction;
-  if (b.n == 0) return cudaSuccess;
-  AmiBatch copy = b;
-  void* args[] = {&copy};
-  // One CTA of 64 threads per 64 samples: the hardware CTA scheduler balances the SMs better than a
+namespace {
+
+CUresult launch_one(const JitState* js, bool fused, AmiBatch& batch, cudaStream_t st) {
+  void* args[] = {&batch};
+  // One CTA per `block` samples: the hardware CTA scheduler balances the SMs better than a
   // persistent grid with a static stride does (measured: persistent + L2 prefetch of the next sample
   // was 12 % slower on cfg3 and 5 % slower on cfg4, profiles/r01_register_plan.md).  The kernels keep
   // their grid-stride loop, so any grid size is correct.
-  const long long blocks = (b.n + jit_block_threads() - 1) / jit_block_threads();
-  const unsigned grid = (unsigned)blocks;
+  const unsigned block = (unsigned)js->block;
+  const unsigned grid = (unsigned)((batch.n + block - 1) / block);
   // Programmatic dependent launch: the kernels begin with griddepcontrol.launch_dependents + .wait, so
   // the NEXT specialised kernel in the stream may be scheduled while this one drains and starts the
   // moment it has completed (stream order is kept: nothing is read or written before the wait).
   static const bool pdl = [] { const char* e = getenv("AMI_JIT_PDL"); return !(e && e[0] == '0'); }();
-  CUresult rc;
   CUfunction fn = fused ? js->fn_fused : js->fn_eval;
   if (pdl && driver().LaunchKernelEx) {
     CUlaunchAttribute attr;
@@ -730,13 +872,46 @@ cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cuda
     CUlaunchConfig cfg;
     memset(&cfg, 0, sizeof cfg);
     cfg.gridDimX = grid; cfg.gridDimY = 1; cfg.gridDimZ = 1;
-    cfg.blockDimX = (unsigned)jit_block_threads(); cfg.blockDimY = 1; cfg.blockDimZ = 1;
-    cfg.sharedMemBytes = 0; cfg.hStream = (CUstream)st; cfg.attrs = &attr; cfg.numAttrs = 1;
-    rc = driver().LaunchKernelEx(&cfg, fn, args, nullptr);
-  } else {
-    rc = driver().LaunchKernel(fn, grid, 1, 1, jit_block_threads(), 1, 1, 0, (CUstream)st, args, nullptr);
+    cfg.blockDimX = block; cfg.blockDimY = 1; cfg.blockDimZ = 1;
+    cfg.sharedMemBytes = js->smem_bytes; cfg.hStream = (CUstream)st; cfg.attrs = &attr; cfg.numAttrs = 1;
+    return driver().LaunchKernelEx(&cfg, fn, args, nullptr);
   }
-  return rc == CUDA_SUCCESS ? cudaSuccess : cudaErrorLaunchFailure;
+  return driver().LaunchKernel(fn, grid, 1, 1, block, 1, 1, js->smem_bytes, (CUstream)st, args, nullptr);
+}
+
+}  // namespace
+
+cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cudaStream_t st, int* launches) {
+  const JitState* js = tab->jit;
+  if (!js || js->status != AMI_OK) return cudaErrorInvalidDeviceFunction;
+  if (b.n == 0) return cudaSuccess;
+  if (js->mode != kJitScratch) {
+    AmiBatch copy = b;
+    if (launch_one(js, fused, copy, st) != CUDA_SUCCESS) return cudaErrorLaunchFailure;
+    if (launches) ++*launches;
+    return cudaSuccess;
+  }
+  // memory-backed variant: a stream-ordered scratch of [slots][chunk] doubles, at most ~512 MiB at a
+  // time, so the batch is walked in chunks of samples
+  const long long per_sample = (long long)js->scratch_slots * 8;
+  long long chunk = std::max<long long>(js->block, ((512LL << 20) / std::max<long long>(per_sample, 1)) / js->block * js->block);
+  chunk = std::min(chunk, (b.n + js->block - 1) / js->block * js->block);
+  double* scratch = nullptr;
+  cudaError_t crc = cudaMallocAsync((void**)&scratch, (size_t)(per_sample * chunk), st);
+  if (crc != cudaSuccess) return crc;
+  for (long long c0 = 0; c0 < b.n; c0 += chunk) {
+    AmiBatch part = b;
+    part.n = std::min(chunk, b.n - c0);
+    if (part.e) part.e += c0;                       // SoA rows keep their stride
+    if (part.e_out) part.e_out += c0;
+    if (part.k) part.k += c0 * b.k_stride_sample;
+    part.out += 2 * c0;
+    part.scratch = scratch;
+    part.scratch_stride = chunk;
+    if (launch_one(js, fused, part, st) != CUDA_SUCCESS) { cudaFreeAsync(scratch, st); return cudaErrorLaunchFailure; }
+    if (launches) ++*launches;
+  }
+  return cudaFreeAsync(scratch, st);
 }
 
 int jit_status(const ami_table* tab) {

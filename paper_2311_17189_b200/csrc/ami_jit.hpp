@@ -15,9 +15,16 @@ int jit_block_threads();   // kJitBlockThreadsDefault unless AMI_JIT_NT override
 
 // Tables whose straight-line form is small enough to live in registers and in the instruction
 // cache; larger ones are evaluated by the table-driven kernels.
+enum { kJitNone = 0, kJitRegister = 1, kJitScratch = 2 };
+// kJitRegister: every value in registers.  kJitScratch (tables beyond that, e.g. order 8): the same
+// generated arithmetic with Fermi/Bose leaves in shared memory and the long-lived sums in a
+// per-sample column of a global scratch array.  kJitNone: table-driven kernels only.
+int jit_mode(const FlatTable& ft, const HornerPlan& hp);
 bool jit_eligible(const FlatTable& ft, const HornerPlan& hp);
 
-std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int block_threads);
+// *scratch_slots receives the doubles of scratch per sample the generated kernels need (0 in register mode).
+std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int block_threads, bool scratch,
+                                int* scratch_slots);
 
 // NVRTC: CUDA C++ -> sm_100a cubin.  Needs no GPU.  Returns AMI_OK, AMI_EUNSUPPORTED when the
 // NVRTC library cannot be loaded, or AMI_EINVAL when compilation fails (`log` has the reason).
@@ -25,7 +32,9 @@ int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& l
 
 // Loads the cubin on the table's device.  Thread-safe, idempotent.
 int jit_prepare(ami_table* tab, std::string& err);
-cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cudaStream_t st);
+// `launches` (may be NULL) is incremented per kernel launched (the memory-backed variant walks a large
+// batch in chunks).
+cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cudaStream_t st, int* launches);
 void jit_destroy(ami_table* tab);
 int jit_status(const ami_table* tab);   // AMI_OK once loaded, 1 = not tried yet, else the error
 

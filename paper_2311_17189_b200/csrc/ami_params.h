@@ -20,6 +20,8 @@ struct AmiBatch {
   long long k_stride_sample, k_stride_comp;
   double q[2 * AMI_K_MAX_EXT];
   double t, mu;
+  double* scratch;          // memory-backed plan: [slots][scratch_stride] doubles, column s belongs to sample s
+  long long scratch_stride;
   double* e_out;            // optional [n_eps][n] copy of the energies formed by the fused path
   // results: complex128, row r = (b0 + b) * n_f_total + (f0 + f) at out + 2 * r * out_row_stride
   double* out;

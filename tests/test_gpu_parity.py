@@ -273,6 +273,41 @@ def test_grid_larger_than_one_launch(ami, torch_mod, oracle_mod, plan, fused):
         assert np.array_equal(one[0], out[8, 64:])
 
 
+def test_memory_backed_plan_opt_in(ami, torch_mod):
+    """AMI_JIT_SCRATCH=1: tables beyond the register plan's limits get the same generated arithmetic
+    with leaves in shared memory and long-lived sums in a global scratch.  Run in a fresh process with
+    the limits lowered so that the order-6 table takes that path (an order-8 body compiles for minutes)."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = """
+import sys; sys.path.insert(0, 'tests')
+import numpy as np, torch
+import ami_inputs as A, paper_2311_17189_b200 as P, oracle
+from parity import check_parity
+cfg = A.get_config('cfg4'); n = 2000 + 37
+tab = P.AmiTable.from_diagram(cfg.diagram)
+k = tab.generate_momenta(cfg.seed, 0, n)
+out = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=P.PLAN_REG)
+assert tab.refresh_info()['reg_plan_status'] == 0
+ot = oracle.OracleTable.from_diagram(cfg.diagram)
+sel = np.arange(0, n, 7)
+e_rows = ot.dispersion(cfg.momenta(n)[sel], [cfg.q], cfg.t, cfg.mu)
+truth, S = ot.evaluate(e_rows, cfg.z_ext, cfg.betas[0], e_reg=cfg.e_reg, quad=True, threads=oracle.hardware_threads(), want_S=True)
+check_parity(out.cpu().numpy()[0][:, sel], truth, S, label='scratch plan')
+two = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, [[1j], [2.0 + 0.5j]], [3.0, 10.0], e_reg=cfg.e_reg)
+ref = tab.evaluate(tab.dispersion(k, [cfg.q], cfg.t, cfg.mu), [[1j], [2.0 + 0.5j]], [3.0, 10.0], e_reg=cfg.e_reg, plan=P.PLAN_FLAT)
+err = (two - ref).abs().max().item(); scale = ref.abs().max().item()
+assert err <= 1e-9 * scale, (err, scale)
+print('SCRATCH-OK', 'W(' in tab.kernel_source())
+"""
+    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, cwd=root, timeout=600,
+                         env=dict(os.environ, AMI_JIT_SCRATCH="1", AMI_JIT_MAX_EDGES="100"))
+    assert out.returncode == 0, out.stderr[-3000:]
+    assert "SCRATCH-OK True" in out.stdout
+
+
 # ------------------------------------------------------------------ S4 streamed driver
 def test_generated_momenta_bitwise(ami, torch_mod):
     """P22: device generator == host generator, bit for bit."""
