@@ -67,7 +67,10 @@ enum {
   AMI_PLAN_REG = 2    /* register plan: the table written out as a straight-line kernel specialised to
                          this diagram (terms grouped by denominator product, Fermi/Bose and denominator
                          products in Horner form, every leaf a register), compiled with NVRTC on first
-                         use; real energies and tables within the size limits only */
+                         use; real energies and tables within the size limits only.  With the environment
+                         variable AMI_JIT_SCRATCH=1 larger tables get a memory-backed variant of the same
+                         kernels (leaves in shared memory, long-lived sums in a global scratch); compiling
+                         those takes minutes */
 };
 
 typedef struct ami_info {
