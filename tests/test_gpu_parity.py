@@ -273,6 +273,18 @@ def test_grid_larger_than_one_launch(ami, torch_mod, oracle_mod, plan, fused):
         assert np.array_equal(one[0], out[8, 64:])
 
 
+@pytest.mark.parametrize("plan", list(PLANS))
+@pytest.mark.parametrize("name", ["cfg3", "cfg2_bubble_doubled", "cfg4"])
+def test_extreme_temperatures(ami, torch_mod, oracle_mod, name, plan):
+    """Reading P12 on the GPU: beta from 0.01 to 5000 (beta |E| up to ~1e5: every exponential would
+    overflow if formed naively; the register plan clamps the summed binary exponent instead)."""
+    cfg = A.get_config(name)
+    z = np.array([[1j * math.pi / 7.0 if cfg.diagram.slot_is_fermionic[-1] else 2j * math.pi / 7.0]])
+    sts = run_eval_case(ami, torch_mod, oracle_mod, cfg, 1500 + 3, PLANS[plan], betas=(0.01, 300.0, 5000.0), z=z,
+                        n_truth=400)
+    assert all(st["n_nonfinite"] == 0 for st in sts)
+
+
 def test_memory_backed_plan_opt_in(ami, torch_mod):
     """AMI_JIT_SCRATCH=1: tables beyond the register plan's limits get the same generated arithmetic
     with leaves in shared memory and long-lived sums in a global scratch.  Run in a fresh process with
