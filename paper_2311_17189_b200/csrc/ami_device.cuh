@@ -51,14 +51,14 @@ __device__ __forceinline__ cplx crcp(cplx a) {
 
 // ---- exponential core ---------------------------------------------------------------------------
 // e^x = 2^n (1 + r q(r)),  n = rint(x log2 e),  r = x - n ln 2 in [-0.347, 0.347],
-// q(r) = sum_k r^k/(k+1)!  (13 terms: truncation 4e-18).  The coefficients sit in constant memory so
+// q(r) ~ (e^r - 1)/r as a degree-10 Chebyshev-node fit on that interval (max error of e^r 7e-18).  The coefficients sit in constant memory so
 // that every DFMA takes its constant straight from the bank (no register moves).  n is clamped to
 // [-1021, 1010] in the integer domain: beyond it the Fermi/Bose value is 0 or 1 to double precision.
 // Returns s = 2^n and rq = r q(r):  e^x = fma(s, rq, s),  e^x - 1 = fma(s, rq, s - 1).
-__constant__ double kAmiExpQ[13] = {
-    1.0, 0.5, 0.16666666666666666, 0.041666666666666664, 0.008333333333333333, 0.001388888888888889,
-    0.0001984126984126984, 2.48015873015873e-05, 2.7557319223985893e-06, 2.755731922398589e-07,
-    2.505210838544172e-08, 2.08767569878681e-09, 1.6059043836821613e-10};
+__constant__ double kAmiExpQ[11] = {
+    1.0, 0.5000000000000006, 0.1666666666666667, 0.04166666666657314, 0.008333333333326141, 0.0013888888932488599,
+    0.00019841269874800493, 2.4801504346997686e-05, 2.7557255425746435e-06, 2.7626357241447223e-07,
+    2.510520637395701e-08};
 
 template <int N>
 __device__ __forceinline__ void exp_core_n(const double (&x)[N], double (&s)[N], double (&rq)[N]) {
@@ -70,10 +70,10 @@ __device__ __forceinline__ void exp_core_n(const double (&x)[N], double (&s)[N],
     const double nd = t[j] - 6755399441055744.0;
     r[j] = fma(nd, -0.6931471805599453, x[j]);
     r[j] = fma(nd, -2.3190468138462996e-17, r[j]);
-    q[j] = kAmiExpQ[12];
+    q[j] = kAmiExpQ[10];
   }
 #pragma unroll
-  for (int i = 11; i >= 0; --i) {
+  for (int i = 9; i >= 0; --i) {
 #pragma unroll
     for (int j = 0; j < N; ++j) q[j] = fma(q[j], r[j], kAmiExpQ[i]);
   }
@@ -98,10 +98,10 @@ __device__ __forceinline__ void exp_split_n(const double (&x)[N], int (&n)[N], d
     const double nd = t[j] - 6755399441055744.0;
     r[j] = fma(nd, -0.6931471805599453, x[j]);
     r[j] = fma(nd, -2.3190468138462996e-17, r[j]);
-    q[j] = kAmiExpQ[12];
+    q[j] = kAmiExpQ[10];
   }
 #pragma unroll
-  for (int i = 11; i >= 0; --i) {
+  for (int i = 9; i >= 0; --i) {
 #pragma unroll
     for (int j = 0; j < N; ++j) q[j] = fma(q[j], r[j], kAmiExpQ[i]);
   }
@@ -126,12 +126,11 @@ __device__ __forceinline__ void exp_core(double x, double& s, double& rq) {
 
 // ---- cosine of a bounded argument -----------------------------------------------------------------
 // cos K = (-1)^n cos r,  n = rint(K/pi),  r = K - n pi in [-pi/2, pi/2] (two-part pi, exact for
-// |K| < 5e5), even Taylor polynomial of degree 20 (next term 1.9e-17).  Momentum sums of a diagram
+// |K| < 5e5), even polynomial of degree 16, a Chebyshev-node fit in r^2 on [0, (pi/2)^2] (max error 5.4e-17).  Momentum sums of a diagram
 // are a few pi; anything beyond 5e5 takes the library routine.
-__constant__ double kAmiCosC[11] = {
-    1.0, -0.5, 0.041666666666666664, -0.001388888888888889, 2.48015873015873e-05, -2.755731922398589e-07,
-    2.08767569878681e-09, -1.1470745597729725e-11, 4.779477332387385e-14, -1.5619206968586225e-16,
-    4.110317623312165e-19};
+__constant__ double kAmiCosC[9] = {
+    1.0, -0.4999999999999997, 0.04166666666666388, -0.001388888888877299, 2.4801587277414926e-05,
+    -2.755731639102575e-07, 2.0876561839933163e-09, -1.1462901901757276e-11, 4.608977003001797e-14};
 
 __device__ __noinline__ double cos_unbounded(double K) { return cos(K); }
 
@@ -146,10 +145,10 @@ __device__ __forceinline__ void cos_bounded_n(double (&K)[N]) {
     r[j] = fma(nd, -3.1415926534682512, K[j]);
     r[j] = fma(nd, -1.2154201013012384e-10, r[j]);
     r2[j] = r[j] * r[j];
-    c[j] = kAmiCosC[10];
+    c[j] = kAmiCosC[8];
   }
 #pragma unroll
-  for (int i = 9; i >= 0; --i) {
+  for (int i = 7; i >= 0; --i) {
 #pragma unroll
     for (int j = 0; j < N; ++j) c[j] = fma(c[j], r2[j], kAmiCosC[i]);
   }
