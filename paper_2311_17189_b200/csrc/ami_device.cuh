@@ -126,11 +126,15 @@ __device__ __forceinline__ void exp_core(double x, double& s, double& rq) {
 
 // ---- cosine of a bounded argument -----------------------------------------------------------------
 // cos K = (-1)^n cos r,  n = rint(K/pi),  r = K - n pi in [-pi/2, pi/2] (two-part pi, exact for
-// |K| < 5e5), even polynomial of degree 16, a Chebyshev-node fit in r^2 on [0, (pi/2)^2] (max error 5.4e-17).  Momentum sums of a diagram
+// |K| < 5e5), even Taylor polynomial of degree 20 (next term 1.9e-17).  A degree-16 fit (5e-17) is two FMAs
+// cheaper but differs from the correctly rounded cosine in the last bit often enough that results
+// which are ill-conditioned in the ENERGIES (double pole at zero frequency) moved by 4e-11 against a
+// quad-precision check fed with libm energies; this one stays at 5e-13 (tests/parity_report.py).  Momentum sums of a diagram
 // are a few pi; anything beyond 5e5 takes the library routine.
-__constant__ double kAmiCosC[9] = {
-    1.0, -0.4999999999999997, 0.04166666666666388, -0.001388888888877299, 2.4801587277414926e-05,
-    -2.755731639102575e-07, 2.0876561839933163e-09, -1.1462901901757276e-11, 4.608977003001797e-14};
+__constant__ double kAmiCosC[11] = {
+    1.0, -0.5, 0.041666666666666664, -0.001388888888888889, 2.48015873015873e-05, -2.755731922398589e-07,
+    2.08767569878681e-09, -1.1470745597729725e-11, 4.779477332387385e-14, -1.5619206968586225e-16,
+    4.110317623312165e-19};
 
 __device__ __noinline__ double cos_unbounded(double K) { return cos(K); }
 
@@ -145,10 +149,10 @@ __device__ __forceinline__ void cos_bounded_n(double (&K)[N]) {
     r[j] = fma(nd, -3.1415926534682512, K[j]);
     r[j] = fma(nd, -1.2154201013012384e-10, r[j]);
     r2[j] = r[j] * r[j];
-    c[j] = kAmiCosC[8];
+    c[j] = kAmiCosC[10];
   }
 #pragma unroll
-  for (int i = 7; i >= 0; --i) {
+  for (int i = 9; i >= 0; --i) {
 #pragma unroll
     for (int j = 0; j < N; ++j) c[j] = fma(c[j], r2[j], kAmiCosC[i]);
   }

@@ -249,7 +249,7 @@ void build_horner_plan(const FlatTable& ft, HornerPlan& hp) {
   count_d_ops(hp, 0, &hp.ops_d_beta, &hp.ops_d);
   // leaf costs on the common path of the routines in ami_device.cuh
   const int kExpCore = 15;   // magic fma, subtract, 2 reduction fma, 10 polynomial fma, final fma
-  const int kNewton = 3, kCos = 13;   // one third-order reciprocal step = 3 fma
+  const int kNewton = 3, kCos = 15;   // one third-order reciprocal step = 3 fma
   // every distinct integer combination of the energies (up to sign) that a denominator needs is
   // formed once per sample
   {

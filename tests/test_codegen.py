@@ -36,7 +36,7 @@ def test_specialised_kernels_compile_for_sm100a(ami, name):
     # counts reported for the roofline: Horner plan far below the flat loop, parts add up
     assert 0 < info["fp64_ops_tree"] < info["fp64_ops_flat"]
     assert 0 <= info["fp64_ops_tree_fermi"] <= info["fp64_ops_tree"]
-    assert info["fp64_ops_leaf_fermi"] >= 16 and info["fp64_ops_dispersion"] >= 28 * info["n_eps"]   # >= one exponential; two cosines per symbol
+    assert info["fp64_ops_leaf_fermi"] >= 16 and info["fp64_ops_dispersion"] >= 32 * info["n_eps"]   # >= one exponential; two cosines per symbol
 
 
 def test_generated_source_is_deterministic(ami):
