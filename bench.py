@@ -37,7 +37,7 @@ def parse_args():
     ap.add_argument("--workload", default="cfg3", help="cfg1 | cfg2_se | cfg2_bubble | cfg3 | cfg4 | cfg5 | stress8")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=0, help="override samples per step per GPU")
-    ap.add_argument("--plan", default="auto", choices=["auto", "flat", "reg"])
+    ap.add_argument("--plan", default="auto", choices=["auto", "flat", "reg", "tree"])
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads and the CPU baseline")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from Python instead of one CUDA graph")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
@@ -111,7 +111,7 @@ class ClockSampler:
 # (cos 15, Fermi/Bose 24, complex reciprocal 8, plus the integer-coefficient sums of their arguments);
 # cross-checked against the executed-instruction counts of ncu's source page in profiles/.
 # ------------------------------------------------------------------------------------------------
-def fp64_work_per_sample(info, n_f, n_b, reg):
+def fp64_work_per_sample(info, n_f, n_b, reg, tree=False):
     """FP64-pipe instruction slots per sample of the representation executed; every count comes from
     ami_table_info (the library counts the instructions its generator emits plus the common-path cost
     of each leaf routine)."""
@@ -120,6 +120,9 @@ def fp64_work_per_sample(info, n_f, n_b, reg):
     dens = n_b * n_f * int(info["fp64_ops_leaf_den"])
     if reg:
         dens = n_f * int(info["fp64_ops_leaf_den"])     # complex reciprocals once per frequency, shared by all beta
+        ft = int(info["fp64_ops_tree_fermi"])
+        terms = n_b * ft + n_b * n_f * (int(info["fp64_ops_tree"]) - ft)
+    elif tree:   # same Horner sums, interpreted; leaves per leaf and reciprocals per (beta, frequency) as in the flat plan
         ft = int(info["fp64_ops_tree_fermi"])
         terms = n_b * ft + n_b * n_f * (int(info["fp64_ops_tree"]) - ft)
     else:
@@ -329,7 +332,7 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
             two_stream_ms = time_two_streams(torch, tab, cfg, ks, steps, plan)
         except Exception as exc:  # noqa: BLE001  (extra figure only; the headline never depends on it)
             two_stream_ms = f"unavailable: {exc}"
-    return {"tab": tab, "info": info, "fused": reg, "total_ms": total_ms, "disp_ms": disp_ms, "eval_ms": eval_ms,
+    return {"tab": tab, "info": info, "fused": reg, "tree": plan == 3, "total_ms": total_ms, "disp_ms": disp_ms, "eval_ms": eval_ms,
             "launches": launches, "clocks": clocks, "graph": graph is not None, "two_stream_ms": two_stream_ms, "n_rot": n_rot, "checksum": checksum,
             "bytes_in": bytes_in, "bytes_e": n * n_eps * 8, "bytes_out": n * n_f * n_b * 16}
 
@@ -393,7 +396,7 @@ def roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s):
     per sample, expressed as DFMA-equivalent TFLOP/s (slot = 2 flop) against the DFMA-chain
     rate measured in this run; the HBM leg is reported beside it.  With the register plan the step is
     ONE fused kernel (S1+S2+S3), otherwise ami_evaluate is the dominant one of two."""
-    w = fp64_work_per_sample(res["info"], n_f, n_b, res["fused"])
+    w = fp64_work_per_sample(res["info"], n_f, n_b, res["fused"], res.get("tree", False))
     t_eval = res["eval_ms"] * 1e-3
     peak_tf = 2.0 * dfma_per_s / 1e12
     if res["fused"]:
@@ -423,14 +426,14 @@ def roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s):
     return roof, disp
 
 
-PLAN_IDS = {"auto": 0, "flat": 1, "reg": 2}
+PLAN_IDS = {"auto": 0, "flat": 1, "reg": 2, "tree": 3}
 
 
 def plan_name_of(info, plan):
     """Name of the representation ami_evaluate executes (after specialisation has been tried)."""
     if plan != "flat" and info["reg_plan_status"] == 0:
         return "register (Horner DAG, NVRTC-specialised)"
-    return "flat (table-driven)"
+    return "tree (table-driven Horner program)" if plan == "tree" else "flat (table-driven)"
 
 
 def run_ours(args, dist, rank, local, world):

@@ -64,6 +64,10 @@ typedef struct ami_table ami_table;
 enum {
   AMI_PLAN_AUTO = 0,  /* the library's fastest plan for this table */
   AMI_PLAN_FLAT = 1,  /* the flat term table, term by term, table-driven (SURVEY 8(a) S3 as written) */
+  AMI_PLAN_TREE = 3,  /* the Horner plan (terms grouped by denominator product, Fermi/Bose sums hash-consed
+                         into a DAG) as a program interpreted by a table-driven kernel: one 32-bit word per
+                         multiply-add, staged through shared memory in tiles with TMA; real energies.  What
+                         AMI_PLAN_AUTO runs when the register plan is not available for the table */
   AMI_PLAN_REG = 2    /* register plan: the table written out as a straight-line kernel specialised to
                          this diagram (terms grouped by denominator product, Fermi/Bose and denominator
                          products in Horner form, every leaf a register), compiled with NVRTC on first
@@ -93,6 +97,8 @@ typedef struct ami_info {
   int64_t fp64_ops_leaf_den;   /* FP64 instructions per (sample,beta,frequency) of the complex reciprocals */
   int64_t fp64_ops_dispersion; /* FP64 instructions per sample of ami_dispersion */
   int64_t fp64_ops_combos;     /* FP64 instructions done once per sample: distinct energy combinations of the leaves, reciprocals of purely real denominators */
+  int64_t tree_plan_words;  /* program words of the tree plan (both programs), -1 = table outside its encoding */
+  int64_t tree_plan_slots;  /* value slots (doubles) per sample the tree plan keeps */
   int32_t has_device_copy;
   int32_t reg_plan_status;  /* 0 = specialised kernels loaded, 1 = eligible, not compiled yet,
                                AMI_EUNSUPPORTED = table outside the register plan's limits, other < 0 = error */
@@ -132,6 +138,11 @@ int ami_table_info(const ami_table* tab, ami_info* info);
  *   coef      float64 [T]          sign and rational prefactor of the term (without A)
  * The term value is A * coef * prod_a f^{(k)}_{sigma}(leafF_c . e) * prod_b 1/(leafD_a . z + leafD_c . e). */
 int ami_table_export(const ami_table* tab, void* host_buf, size_t* bytes);
+
+/* Serialises the tree plan's programs for inspection and tests (size query as above).  Layout: uint32
+ * magic 'AMT1', n_words_beta, n_words_freq, n_consts, n_slots; code_beta[]; code_freq[]; pad to 8 bytes;
+ * float64 consts[].  Word = op << 28 | a << 16 | b, the operations are listed in DESIGN.md (6.3). */
+int ami_table_export_tree(const ami_table* tab, void* host_buf, size_t* bytes);
 
 void ami_table_destroy(ami_table* tab);
 

@@ -12,10 +12,10 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libami_b200.so")
 
-PLAN_AUTO, PLAN_FLAT, PLAN_REG = 0, 1, 2
+PLAN_AUTO, PLAN_FLAT, PLAN_REG, PLAN_TREE = 0, 1, 2, 3
 
 EXPORTS = [
-    "ami_construct", "ami_table_info", "ami_table_export", "ami_table_destroy", "ami_dispersion",
+    "ami_construct", "ami_table_info", "ami_table_export", "ami_table_export_tree", "ami_table_destroy", "ami_dispersion",
     "ami_evaluate", "ami_evaluate_momenta", "ami_table_specialize", "ami_table_kernel_source",
     "ami_table_kernel_cubin", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
     "ami_last_cuda_error", "ami_version", "ami_kernel_launches",
@@ -34,7 +34,7 @@ class ami_info(C.Structure):
                [(n, C.c_int64) for n in ("n_terms", "n_terms_raw", "n_multipoles", "n_groups", "n_tree_nodes",
                                          "n_den_nodes", "table_bytes", "fp64_ops_flat", "fp64_ops_tree",
                                          "fp64_ops_tree_fermi", "fp64_ops_leaf_fermi", "fp64_ops_leaf_den",
-                                         "fp64_ops_dispersion", "fp64_ops_combos")] + \
+                                         "fp64_ops_dispersion", "fp64_ops_combos", "tree_plan_words", "tree_plan_slots")] + \
                [("has_device_copy", C.c_int32), ("reg_plan_status", C.c_int32)]
 
 
@@ -64,6 +64,7 @@ def lib():
         L.ami_construct.argtypes = [C.c_int] * 4 + [C.c_void_p] * 4 + [C.c_double, C.c_int, C.POINTER(C.c_void_p)]
         L.ami_table_info.argtypes = [C.c_void_p, C.POINTER(ami_info)]
         L.ami_table_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
+        L.ami_table_export_tree.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.ami_table_destroy.argtypes = [C.c_void_p]
         L.ami_table_destroy.restype = None
         L.ami_dispersion.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
@@ -197,6 +198,19 @@ class AmiTable:
         off = (pos * 4 + 7) // 8 * 8
         out["coef"] = buf[off:off + 8 * T].view(np.float64).copy()
         return out
+
+    def export_tree(self) -> dict:
+        """ami_table_export_tree parsed: the two programs (uint32 words), the constants, the slot count."""
+        n = C.c_size_t(0)
+        _check(lib().ami_table_export_tree(self._h, None, C.byref(n)))
+        buf = np.zeros(n.value, dtype=np.uint8)
+        _check(lib().ami_table_export_tree(self._h, buf.ctypes.data, C.byref(n)))
+        w = buf[: (n.value // 4) * 4].view(np.uint32)
+        assert w[0] == 0x31544D41
+        nb, nf, nc, ns = (int(x) for x in w[1:5])
+        off = ((5 + nb + nf) * 4 + 7) // 8 * 8
+        return {"code_beta": w[5:5 + nb].copy(), "code_freq": w[5 + nb:5 + nb + nf].copy(),
+                "consts": buf[off:off + 8 * nc].view(np.float64).copy(), "n_slots": ns}
 
     # ---- kernels -------------------------------------------------------------------------
     def dispersion(self, k, q, t, mu, out=None, stream=None):

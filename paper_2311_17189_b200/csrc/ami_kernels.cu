@@ -276,6 +276,174 @@ cudaError_t launch_eval_flat(const EvalParams& p, bool ce, cudaStream_t st, int*
 }
 
 // ------------------------------------------------------------------------------------------
+// S2 + S3, tree plan: leaves once per sample as in the flat plan, then the Horner plan of
+// ami_plan.cpp as a PROGRAM (one 32-bit word per multiply-add) interpreted by every thread for its
+// own sample.  The program is staged through shared memory in double-buffered tiles with TMA bulk
+// copies; the value slots V[] live in shared memory when they fit, else in a global scratch column.
+// ------------------------------------------------------------------------------------------
+template <bool VSMEM>
+__global__ void eval_tree_kernel(EvalParams p) {
+  extern __shared__ double sm[];
+  __shared__ unsigned long long bar[2];
+  const int tid = threadIdx.x, nt = blockDim.x;
+  const long long s_raw = blockIdx.x * (long long)nt + tid;
+  const long long s = s_raw < p.n_e ? s_raw : p.n_e - 1;
+  double* sE = sm;                                   // [n_eps][nt]
+  double* sF = sE + (size_t)p.n_eps * nt;            // [U_F][nt]
+  double* sD = sF + (size_t)p.U_F * nt;              // [(U_D + 1) * 2][nt]
+  double* sV = sD + (size_t)(p.U_D + 1) * 2 * nt;    // [n_slots][nt] when VSMEM
+  uint32_t* tile = reinterpret_cast<uint32_t*>(sV + (VSMEM ? (size_t)p.n_slots * nt : 0));   // [2][kProgTile]
+  double* gV = VSMEM ? nullptr : p.v_scratch + s_raw;   // column of this thread (s_raw < v_stride always)
+  auto vload = [&](unsigned slot) -> double { return VSMEM ? sV[slot * nt + tid] : gV[(long long)slot * p.v_stride]; };
+  auto vstore = [&](unsigned slot, double v) {
+    if (VSMEM) sV[slot * nt + tid] = v;
+    else gV[(long long)slot * p.v_stride] = v;
+  };
+  for (int i = 0; i < p.n_eps; ++i) sE[i * nt + tid] = p.e[i * p.e_stride + s];
+  if (tid == 0) {
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  unsigned issued = 0, waited = 0;
+  double acc = 0.0, cr = 0.0, ci = 0.0;
+  // runs one program of n_words words (padded to whole tiles in memory)
+  auto run = [&](const uint32_t* code, long long n_words) {
+    const long long n_tiles = (n_words + kProgTile - 1) / kProgTile;
+    auto request = [&](long long t) {
+      if (tid == 0) {
+        const int buf = (int)(issued & 1);
+        mbar_expect_tx(&bar[buf], kProgTile * 4u);
+        bulk_g2s(tile + (size_t)buf * kProgTile, code + t * kProgTile, kProgTile * 4u, &bar[buf]);
+      }
+      ++issued;
+    };
+    __syncthreads();
+    if (n_tiles > 0) request(0);
+    for (long long t = 0; t < n_tiles; ++t) {
+      if (t + 1 < n_tiles) request(t + 1);
+      const int buf = (int)(waited & 1);
+      mbar_wait(&bar[buf], (waited >> 1) & 1);
+      ++waited;
+      const uint32_t* w = tile + (size_t)buf * kProgTile;
+      const int n_here = (int)((n_words - t * kProgTile) < kProgTile ? (n_words - t * kProgTile) : kProgTile);
+      for (int i = 0; i < n_here; ++i) {
+        const uint32_t word = w[i];
+        const unsigned a = (word >> 16) & 0xfffu, b = word & 0xffffu;
+        switch (word >> 28) {
+          case kOpSetF: acc = sF[a * nt + tid]; break;
+          case kOpSetNegF: acc = -sF[a * nt + tid]; break;
+          case kOpMulFV: acc = sF[a * nt + tid] * vload(b); break;
+          case kOpFmaFV: acc = fma(sF[a * nt + tid], vload(b), acc); break;
+          case kOpAddF: acc += sF[a * nt + tid]; break;
+          case kOpSubF: acc -= sF[a * nt + tid]; break;
+          case kOpMulCF: acc = p.tree_consts[b] * sF[a * nt + tid]; break;
+          case kOpFmaCF: acc = fma(p.tree_consts[b], sF[a * nt + tid], acc); break;
+          case kOpStore:
+            if (a == 0) { vstore(b, acc); } else { vstore(b, cr); vstore(b + 1, ci); }
+            break;
+          case kOpSetV: acc = vload(b); break;
+          case kOpSetC: acc = p.tree_consts[b]; break;
+          case kOpMulDV: acc = sD[(2 * a) * nt + tid] * vload(b); break;
+          case kOpFmaDV: acc = fma(sD[(2 * a) * nt + tid], vload(b), acc); break;
+          case kOpCSetV: cr = b == 0xffffu ? 0.0 : vload(b); ci = 0.0; break;
+          case kOpCFmaDV: {
+            const double v = vload(b);
+            cr = fma(sD[(2 * a) * nt + tid], v, cr);
+            ci = fma(sD[(2 * a + 1) * nt + tid], v, ci);
+            break;
+          }
+          default: {   // kOpCFmaDC
+            const double dr = sD[(2 * a) * nt + tid], di = sD[(2 * a + 1) * nt + tid];
+            const double vr = vload(b), vi = vload(b + 1);
+            cr = fma(dr, vr, fma(-di, vi, cr));
+            ci = fma(dr, vi, fma(di, vr, ci));
+            break;
+          }
+        }
+      }
+      __syncthreads();
+    }
+  };
+  // reciprocal of denominator u for frequency f: 1/(a . z + c . e), regulator rule P10(b).  Denominators
+  // without an external frequency do not depend on f (nor on beta): they are formed once, up front,
+  // because the per-beta program already multiplies by them.
+  auto denominator = [&](int u, int f, bool want_real) {
+    bool is_real = true;
+    for (int x = 0; x < p.n_ext; ++x) is_real = is_real && p.leafD_a[u * p.n_ext + x] == 0;
+    if (is_real != want_real) return;
+    const int j0 = p.leaf_ptr[p.U_F + u], j1 = p.leaf_ptr[p.U_F + u + 1];
+    double Dr = 0.0, Di = 0.0;
+    bool freq_zero = true;
+    for (int x = 0; x < p.n_ext; ++x) {
+      const int a = p.leafD_a[u * p.n_ext + x];
+      const double zr = p.z[2 * (f * p.n_ext + x)], zi = p.z[2 * (f * p.n_ext + x) + 1];
+      if (a != 0 && !(zr == 0.0 && zi == 0.0)) freq_zero = false;
+      Dr = fma((double)a, zr, Dr);
+      Di = fma((double)a, zi, Di);
+    }
+    for (int j = j0; j < j1; ++j) Dr = fma((double)p.leaf_coef[j], sE[p.leaf_sym[j] * nt + tid], Dr);
+    if (freq_zero) Dr += p.e_reg;
+    const cplx r = crcp(cplx{Dr, Di});
+    sD[(2 * u) * nt + tid] = r.re;
+    sD[(2 * u + 1) * nt + tid] = r.im;
+  };
+  for (int u = 0; u < p.U_D; ++u) denominator(u, 0, true);
+  for (int b = 0; b < p.n_b; ++b) {
+    const double beta = p.beta[b];
+    for (int u = 0; u < p.U_F; ++u) {
+      const int j0 = p.leaf_ptr[u], j1 = p.leaf_ptr[u + 1];
+      double Er = 0.0;
+      for (int j = j0; j < j1; ++j) Er = fma((double)p.leaf_coef[j], sE[p.leaf_sym[j] * nt + tid], Er);
+      const int sig = p.leafF_sig[u];
+      if (sig < 0) Er += p.e_reg;                    // P10(a)
+      sF[u * nt + tid] = fermi_real(Er, beta, sig, p.leafF_k[u], p.derivQ);
+    }
+    run(p.tree_beta, p.n_words_beta);
+    for (int f = 0; f < p.n_f; ++f) {
+      for (int u = 0; u < p.U_D; ++u) denominator(u, f, false);
+      run(p.tree_freq, p.n_words_freq);
+      if (s_raw < p.n_e) {
+        double2* o = reinterpret_cast<double2*>(p.out) +
+                     ((long long)(p.b0 + b) * p.n_f_total + (p.f0 + f)) * p.out_row_stride + s;
+        *o = make_double2(p.prefactor * cr, p.prefactor * ci);
+      }
+    }
+  }
+}
+
+// Shared memory of one CTA of nt threads; v_in_smem chooses where the value slots live.
+static size_t tree_smem_bytes(const EvalParams& p, int nt, bool v_in_smem) {
+  const size_t per_thread = sizeof(double) * ((size_t)p.n_eps + p.U_F + 2 * ((size_t)p.U_D + 1) + (v_in_smem ? p.n_slots : 0));
+  return per_thread * nt + 2 * (size_t)kProgTile * 4;
+}
+
+// `v_in_smem` out: whether this table's value slots fit in shared memory (else the caller provides
+// p.v_scratch with v_stride >= the padded sample count of the launch).
+bool tree_values_fit_smem(const EvalParams& p) { return tree_smem_bytes(p, 64, true) <= 200 * 1024; }
+
+cudaError_t launch_eval_tree(const EvalParams& p, cudaStream_t st, int* launches) {
+  if (p.n_e == 0) return cudaSuccess;
+  const bool vs = tree_values_fit_smem(p);
+  int nt = 0;
+  size_t smem = 0;
+  for (int cand : {256, 128, 64})                     // largest CTA with two CTAs per SM, else one
+    if (!nt && tree_smem_bytes(p, cand, vs) <= 110 * 1024) { nt = cand; }
+  for (int cand : {128, 64, 32})
+    if (!nt && tree_smem_bytes(p, cand, vs) <= 220 * 1024) { nt = cand; }
+  if (!nt) return cudaErrorInvalidConfiguration;
+  smem = tree_smem_bytes(p, nt, vs);
+  if (!vs && !p.v_scratch) return cudaErrorInvalidValue;
+  auto kern = vs ? eval_tree_kernel<true> : eval_tree_kernel<false>;
+  cudaError_t rc = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (rc != cudaSuccess) return rc;
+  kern<<<(unsigned)((p.n_e + nt - 1) / nt), nt, smem, st>>>(p);
+  count_launch(launches);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
 // S4 helpers: counter-based momenta (reading P22) and deterministic tallies.
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ double uniform01(uint64_t seed, uint64_t ctr) {

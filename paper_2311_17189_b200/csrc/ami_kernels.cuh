@@ -10,6 +10,7 @@ namespace ami {
 
 constexpr int kMaxFreqWords = 64;   // n_f * n_ext complex values per launch
 constexpr int kMaxBeta = 8;         // inverse temperatures per launch
+constexpr int kProgTile = 1024;     // program words per shared-memory tile of the tree plan (multiple of 4)
 constexpr int kTermTile = 256;      // terms per shared-memory tile of the flat plan (multiple of 8)
 
 struct EvalParams {
@@ -23,6 +24,14 @@ struct EvalParams {
   const uint16_t* term_idx;
   const double* term_coef;
   const double* derivQ;
+  // tree plan: programs (padded to whole tiles), constants, value slots
+  const uint32_t* tree_beta;
+  const uint32_t* tree_freq;
+  const double* tree_consts;
+  long long n_words_beta, n_words_freq;
+  int n_slots;
+  double* v_scratch;           // global value slots [n_slots][v_stride] when they do not fit in shared memory
+  long long v_stride;
   int n_eps, n_ext, U_F, U_D, m_f, n_d;
   long long T;
   // batch
@@ -48,6 +57,8 @@ struct DispParams {
 
 cudaError_t launch_dispersion(const DispParams& p, cudaStream_t st);
 cudaError_t launch_eval_flat(const EvalParams& p, bool e_is_complex, cudaStream_t st, int* launches);
+cudaError_t launch_eval_tree(const EvalParams& p, cudaStream_t st, int* launches);   // real energies
+bool tree_values_fit_smem(const EvalParams& p);
 cudaError_t launch_generate_momenta(uint64_t seed, long long first, long long n, int n_comp, double* d_k,
                                     cudaStream_t st);
 cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long n, long long row_stride,

@@ -88,6 +88,39 @@ struct HornerPlan {
                              // and the reciprocals of the purely real denominators
 };
 
+// ---- tree plan: the Horner plan as a program for a table-driven interpreter (ami_kernels.cu) ----
+// One 32-bit word per operation: op (4 bits) | a (12 bits) | b (16 bits).  A thread keeps one real
+// accumulator `acc` and one complex accumulator `c`; F[] are its Fermi/Bose leaves, D[] its
+// reciprocal denominators, V[] its value slots, C[] the table's constants.
+enum TreeOp : uint32_t {
+  kOpSetF = 0,     // acc = F[a]
+  kOpSetNegF,      // acc = -F[a]
+  kOpMulFV,        // acc = F[a] * V[b]
+  kOpFmaFV,        // acc = fma(F[a], V[b], acc)
+  kOpAddF,         // acc += F[a]
+  kOpSubF,         // acc -= F[a]
+  kOpMulCF,        // acc = C[b] * F[a]
+  kOpFmaCF,        // acc = fma(C[b], F[a], acc)
+  kOpStore,        // a == 0: V[b] = acc;  a == 1: (V[b], V[b+1]) = c
+  kOpSetV,         // acc = V[b]
+  kOpSetC,         // acc = C[b]
+  kOpMulDV,        // acc = Re D[a] * V[b]            (purely real denominator)
+  kOpFmaDV,        // acc = fma(Re D[a], V[b], acc)
+  kOpCSetV,        // c = (V[b], 0);  b == 0xffff: c = 0
+  kOpCFmaDV,       // c += D[a] * V[b]                (complex denominator, real value)
+  kOpCFmaDC        // c += D[a] * (V[b], V[b+1])      (complex denominator, complex value)
+};
+inline uint32_t tree_word(uint32_t op, uint32_t a, uint32_t b) { return (op << 28) | ((a & 0xfffu) << 16) | (b & 0xffffu); }
+
+struct TreeProgram {
+  std::vector<uint32_t> code_beta;   // once per (sample, beta): FT sums and frequency-independent sub-sums
+  std::vector<uint32_t> code_freq;   // once per (sample, beta, frequency): the R part; the result is left in c
+  std::vector<double> consts;
+  int n_slots = 0;                   // doubles of V per sample
+  bool ok = false;                   // false: table outside the encoding's limits (4095 leaves, 65534 slots)
+};
+void build_tree_program(const FlatTable& ft, const HornerPlan& hp, TreeProgram& tp);
+
 // The compiled, per-table specialised kernels (ami_jit.cpp).
 struct JitState;
 
@@ -112,6 +145,9 @@ struct ami_device_copy {
   uint16_t* term_idx = nullptr;   // [T][n_int + n_d]: Fermi ids then denominator ids (U_D = unit leaf)
   double* term_coef = nullptr;    // [T]
   // tree plan
+  uint32_t* tree_beta = nullptr;  // code_beta, padded to whole tiles
+  uint32_t* tree_freq = nullptr;  // code_freq, padded to whole tiles
+  double* tree_consts = nullptr;
   // dispersion
   int8_t* sym_alpha = nullptr;    // [n_eps][L]
   double* derivQ = nullptr;       // [AMI_MAX_DERIV+1][8] polynomials of the Fermi derivatives
@@ -121,6 +157,7 @@ struct ami_device_copy {
 struct ami_table {
   ami::FlatTable flat;
   ami::HornerPlan horner;
+  ami::TreeProgram tree;
   ami::JitState* jit = nullptr;   // owned; see ami_jit.cpp
   void* run_ws = nullptr;         // owned; workspace of ami_run (ami_api.cu)
   ami_device_copy dev;

@@ -10,7 +10,7 @@ from parity import check_parity
 
 pytestmark = pytest.mark.gpu
 
-PLANS = {"flat": 1, "auto": 0}   # auto = the register plan where the table is eligible, else flat
+PLANS = {"flat": 1, "tree": 3, "auto": 0}   # auto = the register plan where the table is eligible, else flat
 
 
 @pytest.fixture(scope="module")
@@ -122,6 +122,8 @@ def test_cfg5_grid(ami, torch_mod, oracle_mod, plan):
 @pytest.mark.parametrize("plan", list(PLANS))
 def test_complex_energies_variant_5b(ami, torch_mod, oracle_mod, plan):
     """P19: complex energies e_j - i gamma_j make the Fermi/Bose arguments complex."""
+    if plan == "tree":
+        pytest.skip("the tree plan takes real energies (complex ones run the flat plan)")
     cfg = A.get_config("cfg5")
     tab = ami.AmiTable.from_diagram(cfg.diagram)
     n = 500
@@ -211,7 +213,7 @@ def test_register_plan_limits(ami, torch_mod):
 
 
 @pytest.mark.parametrize("name,n", [("cfg1", 10_000), ("cfg3", 50_000 + 3), ("cfg4", 3000 + 1), ("cfg5", 401)])
-@pytest.mark.parametrize("plan", ["flat", "auto"])
+@pytest.mark.parametrize("plan", ["flat", "tree", "auto"])
 def test_fused_momenta_path(ami, torch_mod, oracle_mod, name, n, plan):
     """ami_evaluate_momenta == ami_dispersion followed by ami_evaluate, bit for bit, and the energies
     it stores are those of ami_dispersion; then against the oracle from the momenta on."""
@@ -237,7 +239,7 @@ def test_fused_momenta_path(ami, torch_mod, oracle_mod, name, n, plan):
         check_parity(got.cpu().numpy()[b][:, sel], truth, S, label=f"fused {name}")
 
 
-@pytest.mark.parametrize("plan", ["flat", "auto"])
+@pytest.mark.parametrize("plan", ["flat", "tree", "auto"])
 @pytest.mark.parametrize("fused", [False, True])
 def test_grid_larger_than_one_launch(ami, torch_mod, oracle_mod, plan, fused):
     """70 frequencies x 9 temperatures do not fit one launch (64 frequency words, 8 temperatures):
@@ -267,10 +269,8 @@ def test_grid_larger_than_one_launch(ami, torch_mod, oracle_mod, plan, fused):
         check_parity(out[b][:, sel], truth, S, label=f"split grid beta#{b}")
     # rows computed alone equal the rows of the split call, bit for bit
     one = tab.evaluate(e, z[64:], [betas[8]], plan=PLANS[plan]).cpu().numpy()
-    if plan == "flat":
-        assert np.array_equal(one[0], out[8, 64:])
-    else:   # the several-temperature body keeps per-beta values in memory: same arithmetic, same bits
-        assert np.array_equal(one[0], out[8, 64:])
+    # (the register plan's several-temperature body keeps per-beta values in memory: same arithmetic, same bits)
+    assert np.array_equal(one[0], out[8, 64:])
 
 
 @pytest.mark.parametrize("plan", list(PLANS))

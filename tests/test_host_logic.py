@@ -140,3 +140,59 @@ def test_denominators_keep_their_orientation(ami):
     assert ex["leafD_c"].shape[0] == 2 and len(ex["coef"]) == 4
     np.testing.assert_array_equal(ex["leafD_c"][0], -ex["leafD_c"][1])
     np.testing.assert_array_equal(ex["leafD_a"][0], -ex["leafD_a"][1])
+
+
+def numpy_run_tree(tab_export, prog, e, z, beta):
+    """Interprets the exported tree-plan programs with numpy, all samples at once (test-side restatement
+    of the word format documented in include/ami.h and DESIGN.md 6.3; derivative order <= 1)."""
+    F = []
+    for c, sig, k in zip(tab_export["leafF_c"], tab_export["leafF_sig"], tab_export["leafF_k"]):
+        f = 1.0 / (sig * np.exp(beta * (e @ c)) + 1.0)
+        F.append(f if k == 0 else -beta * f * (1 - f))
+        assert k <= 1
+    D = [1.0 / (e @ c + a @ z + 0j) for c, a in zip(tab_export["leafD_c"], tab_export["leafD_a"])]
+    n = e.shape[0]
+    V = np.zeros((prog["n_slots"] + 2, n))
+    C = prog["consts"]
+    acc = np.zeros(n)
+    cplx = np.zeros(n, dtype=complex)
+    for code in (prog["code_beta"], prog["code_freq"]):
+        for w in code:
+            op, a, b = int(w) >> 28, (int(w) >> 16) & 0xfff, int(w) & 0xffff
+            if op == 0: acc = F[a].copy()
+            elif op == 1: acc = -F[a]
+            elif op == 2: acc = F[a] * V[b]
+            elif op == 3: acc = F[a] * V[b] + acc
+            elif op == 4: acc = acc + F[a]
+            elif op == 5: acc = acc - F[a]
+            elif op == 6: acc = C[b] * F[a]
+            elif op == 7: acc = C[b] * F[a] + acc
+            elif op == 8:
+                if a == 0: V[b] = acc
+                else: V[b], V[b + 1] = cplx.real.copy(), cplx.imag.copy()
+            elif op == 9: acc = V[b].copy()
+            elif op == 10: acc = np.full(n, C[b])
+            elif op == 11: acc = D[a].real * V[b]
+            elif op == 12: acc = D[a].real * V[b] + acc
+            elif op == 13: cplx = (V[b] if b != 0xffff else np.zeros(n)) + 0j
+            elif op == 14: cplx = cplx + D[a] * V[b]
+            else: cplx = cplx + D[a] * (V[b] + 1j * V[b + 1])
+    return cplx
+
+
+@pytest.mark.parametrize("name", list(DIAGRAMS))
+def test_tree_program_values_match_oracle(ami, oracle_mod, name):
+    """The Horner plan serialised as a program (hash-consed FT sums, frequency-independent sub-sums,
+    complex R part) reproduces the oracle's values when interpreted on the CPU."""
+    d = DIAGRAMS[name]()
+    tab = ami.AmiTable.from_diagram(d, device=None)
+    assert tab.info["tree_plan_words"] > 0
+    ex, prog = tab.export(), tab.export_tree()
+    assert len(prog["code_beta"]) + len(prog["code_freq"]) == tab.info["tree_plan_words"]
+    rng = np.random.default_rng(5)
+    e = rng.uniform(-1.5, 1.5, size=(16, d.n_eps))
+    beta = 2.0
+    z = np.array([1j * math.pi / beta if d.slot_is_fermionic[-1] else 2j * math.pi / beta])
+    got = numpy_run_tree(ex, prog, e, z, beta)
+    want, S = oracle_mod.OracleTable.from_diagram(d).evaluate(e, [z], beta, quad=True, want_S=True)
+    assert np.max(np.abs(got - want[0]) / S[0]) < 1e-12
