@@ -65,8 +65,8 @@ enum {
   AMI_PLAN_AUTO = 0,  /* the library's fastest plan for this table */
   AMI_PLAN_FLAT = 1,  /* the flat term table, term by term, table-driven (SURVEY 8(a) S3 as written) */
   AMI_PLAN_TREE = 3,  /* the Horner plan (terms grouped by denominator product, Fermi/Bose sums hash-consed
-                         into a DAG) as a program interpreted by a table-driven kernel: one 32-bit word per
-                         multiply-add, staged through shared memory in tiles with TMA; real energies.  What
+                         into a DAG) as a program interpreted by a table-driven kernel: node lists of uniform
+                         multiply-add items, staged through shared memory in tiles with TMA; real energies.  What
                          AMI_PLAN_AUTO runs when the register plan is not available for the table */
   AMI_PLAN_REG = 2    /* register plan: the table written out as a straight-line kernel specialised to
                          this diagram (terms grouped by denominator product, Fermi/Bose and denominator
@@ -141,7 +141,8 @@ int ami_table_export(const ami_table* tab, void* host_buf, size_t* bytes);
 
 /* Serialises the tree plan's programs for inspection and tests (size query as above).  Layout: uint32
  * magic 'AMT1', n_words_beta, n_words_freq, n_consts, n_slots; code_beta[]; code_freq[]; pad to 8 bytes;
- * float64 consts[].  Word = op << 28 | a << 16 | b, the operations are listed in DESIGN.md (6.3). */
+ * float64 consts[].  A program is a list of nodes: header word count << 16 | dst, then `count` item words
+ * flag << 28 | a << 16 | b; DESIGN.md (6.3) says what a node computes. */
 int ami_table_export_tree(const ami_table* tab, void* host_buf, size_t* bytes);
 
 void ami_table_destroy(ami_table* tab);

@@ -109,8 +109,8 @@ int make_device_copy(ami_table* tab, int device) {
   if ((rc = upload(sa, &dc.sym_alpha, dc.bytes))) return rc;
   {   // tree programs, padded to whole tiles (bulk copies move whole tiles; padding is never executed)
     std::vector<uint32_t> cb = tab->tree.code_beta, cf = tab->tree.code_freq;
-    while (cb.size() % ami::kProgTile) cb.push_back(0);
-    while (cf.size() % ami::kProgTile) cf.push_back(0);
+    while (cb.size() % ami::kTreeTileWords) cb.push_back(0);
+    while (cf.size() % ami::kTreeTileWords) cf.push_back(0);
     if ((rc = upload(cb, &dc.tree_beta, dc.bytes))) return rc;
     if ((rc = upload(cf, &dc.tree_freq, dc.bytes))) return rc;
     if ((rc = upload(tab->tree.consts, &dc.tree_consts, dc.bytes))) return rc;
@@ -269,7 +269,7 @@ void fill_table_params(const ami_table* tab, ami::EvalParams& p) {
   p.derivQ = dc.derivQ;
   p.tree_beta = dc.tree_beta; p.tree_freq = dc.tree_freq; p.tree_consts = dc.tree_consts;
   p.n_words_beta = (long long)tab->tree.code_beta.size(); p.n_words_freq = (long long)tab->tree.code_freq.size();
-  p.n_slots = tab->tree.n_slots;
+  p.n_slots = tab->tree.n_slots; p.n_consts = (int)tab->tree.consts.size();
   p.n_eps = ft.n_eps; p.n_ext = ft.n_ext;
   p.U_F = (int)ft.leafF.size(); p.U_D = (int)ft.leafD.size();
   p.m_f = ft.n_int; p.n_d = ft.max_den;
@@ -286,7 +286,7 @@ int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg
   const bool tree_ok = tab->tree.ok && !e_is_complex;
   // AUTO prefers the interpreted Horner program to the flat table only where it pays: per word the
   // interpreter costs several times a flat factor, but large tables have 50-70x fewer words than
-  // flat factors (measured: order 4 1.06 vs 0.57 ms, order 6 1.19 vs 1.29 ms, order 8 13.8 vs 49.5 ms)
+  // flat factors (measured: order 4 0.86 vs 0.57 ms, order 6 0.95 vs 1.29 ms, order 8 15.9 vs 49.5 ms)
   const bool tree_auto = tree_ok && tab->flat.terms.size() >= 500;
   if (plan == AMI_PLAN_TREE) {
     if (!tree_ok) { g_cuda_err = "tree plan unavailable for this table / energy type"; return AMI_EUNSUPPORTED; }

@@ -292,9 +292,15 @@ __global__ void eval_tree_kernel(EvalParams p) {
   double* sF = sE + (size_t)p.n_eps * nt;            // [U_F][nt]
   double* sD = sF + (size_t)p.U_F * nt;              // [(U_D + 1) * 2][nt]
   double* sV = sD + (size_t)(p.U_D + 1) * 2 * nt;    // [n_slots][nt] when VSMEM
-  uint32_t* tile = reinterpret_cast<uint32_t*>(sV + (VSMEM ? (size_t)p.n_slots * nt : 0));   // [2][kProgTile]
+  uint32_t* tile = reinterpret_cast<uint32_t*>(sV + (VSMEM ? (size_t)p.n_slots * nt : 0));   // [2][kTreeTileWords]
   double* gV = VSMEM ? nullptr : p.v_scratch + s_raw;   // column of this thread (s_raw < v_stride always)
-  auto vload = [&](unsigned slot) -> double { return VSMEM ? sV[slot * nt + tid] : gV[(long long)slot * p.v_stride]; };
+  // V[0 .. n_consts) are the table's constants: the same for every thread, read from one shared copy
+  double* sC = reinterpret_cast<double*>(tile + 2 * kTreeTileWords);                 // [n_consts]
+  const unsigned nc = (unsigned)p.n_consts;
+  auto vload = [&](unsigned slot) -> double {
+    if (slot < nc) return sC[slot];
+    return VSMEM ? sV[slot * nt + tid] : gV[(long long)slot * p.v_stride];
+  };
   auto vstore = [&](unsigned slot, double v) {
     if (VSMEM) sV[slot * nt + tid] = v;
     else gV[(long long)slot * p.v_stride] = v;
@@ -307,15 +313,16 @@ __global__ void eval_tree_kernel(EvalParams p) {
   }
   __syncthreads();
   unsigned issued = 0, waited = 0;
-  double acc = 0.0, cr = 0.0, ci = 0.0;
-  // runs one program of n_words words (padded to whole tiles in memory)
-  auto run = [&](const uint32_t* code, long long n_words) {
-    const long long n_tiles = (n_words + kProgTile - 1) / kProgTile;
+  double cr = 0.0, ci = 0.0;
+  // runs one program of n_words words (padded to whole tiles in memory): a list of nodes, each a header
+  // (count, dst) and `count` uniform items; COMPLEX selects the node kind (format in ami_table.hpp)
+  auto run = [&](const uint32_t* code, long long n_words, const bool COMPLEX) {
+    const long long n_tiles = (n_words + kTreeTileWords - 1) / kTreeTileWords;
     auto request = [&](long long t) {
       if (tid == 0) {
         const int buf = (int)(issued & 1);
-        mbar_expect_tx(&bar[buf], kProgTile * 4u);
-        bulk_g2s(tile + (size_t)buf * kProgTile, code + t * kProgTile, kProgTile * 4u, &bar[buf]);
+        mbar_expect_tx(&bar[buf], kTreeTileWords * 4u);
+        bulk_g2s(tile + (size_t)buf * kTreeTileWords, code + t * kTreeTileWords, kTreeTileWords * 4u, &bar[buf]);
       }
       ++issued;
     };
@@ -326,46 +333,45 @@ __global__ void eval_tree_kernel(EvalParams p) {
       const int buf = (int)(waited & 1);
       mbar_wait(&bar[buf], (waited >> 1) & 1);
       ++waited;
-      const uint32_t* w = tile + (size_t)buf * kProgTile;
-      const int n_here = (int)((n_words - t * kProgTile) < kProgTile ? (n_words - t * kProgTile) : kProgTile);
-      for (int i = 0; i < n_here; ++i) {
-        const uint32_t word = w[i];
-        const unsigned a = (word >> 16) & 0xfffu, b = word & 0xffffu;
-        switch (word >> 28) {
-          case kOpSetF: acc = sF[a * nt + tid]; break;
-          case kOpSetNegF: acc = -sF[a * nt + tid]; break;
-          case kOpMulFV: acc = sF[a * nt + tid] * vload(b); break;
-          case kOpFmaFV: acc = fma(sF[a * nt + tid], vload(b), acc); break;
-          case kOpAddF: acc += sF[a * nt + tid]; break;
-          case kOpSubF: acc -= sF[a * nt + tid]; break;
-          case kOpMulCF: acc = p.tree_consts[b] * sF[a * nt + tid]; break;
-          case kOpFmaCF: acc = fma(p.tree_consts[b], sF[a * nt + tid], acc); break;
-          case kOpStore:
-            if (a == 0) { vstore(b, acc); } else { vstore(b, cr); vstore(b + 1, ci); }
-            break;
-          case kOpSetV: acc = vload(b); break;
-          case kOpSetC: acc = p.tree_consts[b]; break;
-          case kOpMulDV: acc = sD[(2 * a) * nt + tid] * vload(b); break;
-          case kOpFmaDV: acc = fma(sD[(2 * a) * nt + tid], vload(b), acc); break;
-          case kOpCSetV: cr = b == 0xffffu ? 0.0 : vload(b); ci = 0.0; break;
-          case kOpCFmaDV: {
-            const double v = vload(b);
-            cr = fma(sD[(2 * a) * nt + tid], v, cr);
-            ci = fma(sD[(2 * a + 1) * nt + tid], v, ci);
-            break;
+      const uint32_t* w = tile + (size_t)buf * kTreeTileWords;
+      const int n_here = (int)((n_words - t * kTreeTileWords) < kTreeTileWords ? (n_words - t * kTreeTileWords) : kTreeTileWords);
+      int pos = 0;
+      while (pos < n_here) {
+        const uint32_t hdr = w[pos];
+        const int count = (int)(hdr >> 16);
+        const unsigned dst = hdr & 0xffffu;
+        const uint32_t* it = w + pos + 1;
+        if (!COMPLEX) {
+          double acc = 0.0;
+#pragma unroll 4
+          for (int i = 0; i < count; ++i) {
+            const uint32_t word = it[i];
+            acc = fma(sF[((word >> 16) & 0xfffu) * nt + tid], vload(word & 0xffffu), acc);
           }
-          default: {   // kOpCFmaDC
+          if (dst != kTreeNoDst) vstore(dst, acc);
+        } else {
+          double ar = 0.0, ai = 0.0;
+#pragma unroll 2
+          for (int i = 0; i < count; ++i) {
+            const uint32_t word = it[i];
+            const unsigned a = (word >> 16) & 0xfffu, b = word & 0xffffu;
             const double dr = sD[(2 * a) * nt + tid], di = sD[(2 * a + 1) * nt + tid];
-            const double vr = vload(b), vi = vload(b + 1);
-            cr = fma(dr, vr, fma(-di, vi, cr));
-            ci = fma(dr, vi, fma(di, vr, ci));
-            break;
+            const double vr = vload(b), vi = (word >> 28) ? vload(b + 1) : 0.0;
+            ar = fma(dr, vr, fma(-di, vi, ar));
+            ai = fma(dr, vi, fma(di, vr, ai));
           }
+          if (dst != kTreeNoDst) { vstore(dst, ar); vstore(dst + 1, ai); }
+          else { cr = ar; ci = ai; }
         }
+        pos += 1 + count;
       }
       __syncthreads();
     }
   };
+  // constants of the table into the first value slots; the unit leaf L[U_F + 2 U_D] = 1, D[U_D] = 1
+  for (int i = tid; i < p.n_consts; i += nt) sC[i] = p.tree_consts[i];      // visible after run()'s first barrier
+  sD[(2 * p.U_D) * nt + tid] = 1.0;
+  sD[(2 * p.U_D + 1) * nt + tid] = 0.0;
   // reciprocal of denominator u for frequency f: 1/(a . z + c . e), regulator rule P10(b).  Denominators
   // without an external frequency do not depend on f (nor on beta): they are formed once, up front,
   // because the per-beta program already multiplies by them.
@@ -400,10 +406,10 @@ __global__ void eval_tree_kernel(EvalParams p) {
       if (sig < 0) Er += p.e_reg;                    // P10(a)
       sF[u * nt + tid] = fermi_real(Er, beta, sig, p.leafF_k[u], p.derivQ);
     }
-    run(p.tree_beta, p.n_words_beta);
+    run(p.tree_beta, p.n_words_beta, false);
     for (int f = 0; f < p.n_f; ++f) {
       for (int u = 0; u < p.U_D; ++u) denominator(u, f, false);
-      run(p.tree_freq, p.n_words_freq);
+      run(p.tree_freq, p.n_words_freq, true);
       if (s_raw < p.n_e) {
         double2* o = reinterpret_cast<double2*>(p.out) +
                      ((long long)(p.b0 + b) * p.n_f_total + (p.f0 + f)) * p.out_row_stride + s;
@@ -416,7 +422,7 @@ __global__ void eval_tree_kernel(EvalParams p) {
 // Shared memory of one CTA of nt threads; v_in_smem chooses where the value slots live.
 static size_t tree_smem_bytes(const EvalParams& p, int nt, bool v_in_smem) {
   const size_t per_thread = sizeof(double) * ((size_t)p.n_eps + p.U_F + 2 * ((size_t)p.U_D + 1) + (v_in_smem ? p.n_slots : 0));
-  return per_thread * nt + 2 * (size_t)kProgTile * 4;
+  return per_thread * nt + 2 * (size_t)kTreeTileWords * 4 + (size_t)p.n_consts * sizeof(double);
 }
 
 // `v_in_smem` out: whether this table's value slots fit in shared memory (else the caller provides

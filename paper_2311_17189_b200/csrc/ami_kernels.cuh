@@ -10,7 +10,6 @@ namespace ami {
 
 constexpr int kMaxFreqWords = 64;   // n_f * n_ext complex values per launch
 constexpr int kMaxBeta = 8;         // inverse temperatures per launch
-constexpr int kProgTile = 1024;     // program words per shared-memory tile of the tree plan (multiple of 4)
 constexpr int kTermTile = 256;      // terms per shared-memory tile of the flat plan (multiple of 8)
 
 struct EvalParams {
@@ -29,7 +28,7 @@ struct EvalParams {
   const uint32_t* tree_freq;
   const double* tree_consts;
   long long n_words_beta, n_words_freq;
-  int n_slots;
+  int n_slots, n_consts;
   double* v_scratch;           // global value slots [n_slots][v_stride] when they do not fit in shared memory
   long long v_stride;
   int n_eps, n_ext, U_F, U_D, m_f, n_d;

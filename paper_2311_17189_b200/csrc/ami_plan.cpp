@@ -309,7 +309,8 @@ void build_horner_plan(const FlatTable& ft, HornerPlan& hp) {
 
 
 // ---------------------------------------------------------------------------------------------
-// Tree program: the Horner plan written as words for the table-driven interpreter.
+// Tree program: the Horner plan written as node lists for the table-driven interpreter
+// (format in ami_table.hpp).
 // ---------------------------------------------------------------------------------------------
 namespace {
 
@@ -320,32 +321,46 @@ struct TreeBuilder {
   std::vector<int> uses_left, slot_of;       // S-nodes
   std::vector<char> keep;                     // S-nodes that are some group's FT: never recycled
   std::vector<int> free_slots;
-  std::map<std::pair<long long, long long>, int> const_id;
+  std::map<std::pair<long long, long long>, int> const_slot;
   std::vector<int> q_slot;                    // D-trie node -> slot of Q(n), -1 = none
   std::vector<int> s_slot;                    // D-trie node -> first slot of its complex S pair
   bool overflow = false;
+  const uint32_t UF, UD;
 
-  TreeBuilder(const FlatTable& f, const HornerPlan& h, TreeProgram& t) : ft(f), hp(h), tp(t) {}
+  TreeBuilder(const FlatTable& f, const HornerPlan& h, TreeProgram& t)
+      : ft(f), hp(h), tp(t), UF((uint32_t)f.leafF.size()), UD((uint32_t)f.leafD.size()) {}
+
+  uint32_t leaf_re_d(int u) const { return UF + 2u * (uint32_t)u; }   // index of Re D[u] in L[]
+  uint32_t leaf_one() const { return UF + 2u * UD; }                  // L[...] = 1
 
   int take() {
     if (!free_slots.empty()) { const int s = free_slots.back(); free_slots.pop_back(); return s; }
-    if (tp.n_slots >= 65534) { overflow = true; return 0; }
+    if (tp.n_slots >= 65533) { overflow = true; return 0; }
     return tp.n_slots++;
   }
   int take_pair() {                // two consecutive slots, never recycled
-    if (tp.n_slots >= 65533) { overflow = true; return 0; }
+    if (tp.n_slots >= 65532) { overflow = true; return 0; }
     const int s = tp.n_slots;
     tp.n_slots += 2;
     return s;
   }
-  int constant(long long num, long long den) {
-    auto it = const_id.find({num, den});
-    if (it != const_id.end()) return it->second;
-    const int id = (int)tp.consts.size();
-    if (id >= 65535) { overflow = true; return 0; }
+  int constant(long long num, long long den) {     // constants were collected up front: V[slot] = num/den
+    auto it = const_slot.find({num, den});
+    if (it == const_slot.end()) { overflow = true; return 0; }
+    return it->second;
+  }
+  void add_constant(long long num, long long den) {
+    if (const_slot.count({num, den})) return;
+    const_slot.emplace(std::make_pair(num, den), (int)tp.consts.size());
     tp.consts.push_back((double)num / (double)den);
-    const_id.emplace(std::make_pair(num, den), id);
-    return id;
+  }
+  // appends one node; a node never straddles a tile
+  void emit(std::vector<uint32_t>& code, uint32_t dst, const std::vector<uint32_t>& items) {
+    if (items.size() + 1 > (size_t)kTreeTileWords) { overflow = true; return; }
+    while (code.size() % kTreeTileWords + 1 + items.size() > (size_t)kTreeTileWords)
+      code.push_back(tree_header(0, kTreeNoDst));
+    code.push_back(tree_header((uint32_t)items.size(), dst));
+    code.insert(code.end(), items.begin(), items.end());
   }
   void consume(int n) {
     if (--uses_left[n] == 0 && !keep[n] && slot_of[n] >= 0) { free_slots.push_back(slot_of[n]); slot_of[n] = -1; }
@@ -354,43 +369,36 @@ struct TreeBuilder {
   int snode(int id, std::vector<uint32_t>& code) {
     if (slot_of[id] >= 0) return slot_of[id];
     const SNode& n = hp.snodes[id];
+    std::vector<uint32_t> items;
     std::vector<int> child_slot(n.items.size(), -1);
     for (size_t i = 0; i < n.items.size(); ++i)
       if (n.items[i].child >= 0) child_slot[i] = snode(n.items[i].child, code);
     for (size_t i = 0; i < n.items.size(); ++i) {
       const SItem& it = n.items[i];
-      const bool first = i == 0;
-      if (it.child >= 0) {
-        code.push_back(tree_word(first ? kOpMulFV : kOpFmaFV, it.leaf, child_slot[i]));
-      } else if (it.den == 1 && (it.num == 1 || it.num == -1)) {
-        code.push_back(tree_word(first ? (it.num > 0 ? kOpSetF : kOpSetNegF) : (it.num > 0 ? kOpAddF : kOpSubF), it.leaf, 0));
-      } else {
-        code.push_back(tree_word(first ? kOpMulCF : kOpFmaCF, it.leaf, constant(it.num, it.den)));
-      }
+      items.push_back(tree_item(0, (uint32_t)it.leaf, (uint32_t)(it.child >= 0 ? child_slot[i] : constant(it.num, it.den))));
     }
     for (const SItem& it : n.items)
       if (it.child >= 0) consume(it.child);
     slot_of[id] = take();
-    code.push_back(tree_word(kOpStore, 0, slot_of[id]));
+    emit(code, (uint32_t)slot_of[id], items);
     return slot_of[id];
   }
   // Q(n) = [FT of the group ending at n] + sum over kids with a real denominator of Dr * Q(kid);
   // returns its slot or -1 when there is nothing
   int qnode(int n, const std::vector<int>& ft_slot, std::vector<uint32_t>& code) {
     const HNode& nd = hp.dn[n];
-    std::vector<std::pair<int, int>> real_kids;    // (leaf, slot of Q(kid))
-    for (int c : nd.kids)
-      if (hp.d_is_real[hp.dn[c].leaf]) real_kids.emplace_back(hp.dn[c].leaf, qnode(c, ft_slot, code));
+    std::vector<uint32_t> items;
     const int ftq = nd.group >= 0 ? ft_slot[nd.group] : -1;
-    if (real_kids.empty()) return ftq;              // alias of the FT slot (or nothing)
-    bool have = false;
-    if (ftq >= 0) { code.push_back(tree_word(kOpSetV, 0, ftq)); have = true; }
-    for (const auto& k : real_kids) {
-      code.push_back(tree_word(have ? kOpFmaDV : kOpMulDV, k.first, k.second));
-      have = true;
-    }
+    if (ftq >= 0) items.push_back(tree_item(0, leaf_one(), (uint32_t)ftq));
+    bool any = false;
+    for (int c : nd.kids)
+      if (hp.d_is_real[hp.dn[c].leaf]) {
+        items.push_back(tree_item(0, leaf_re_d(hp.dn[c].leaf), (uint32_t)qnode(c, ft_slot, code)));
+        any = true;
+      }
+    if (!any) return ftq;                           // alias of the FT slot (or nothing)
     const int s = take();
-    code.push_back(tree_word(kOpStore, 0, s));
+    emit(code, (uint32_t)s, items);
     return s;
   }
   bool has_complex_kids(int n) const {
@@ -398,22 +406,21 @@ struct TreeBuilder {
       if (!hp.d_is_real[hp.dn[c].leaf]) return true;
     return false;
   }
-  // S(n) = Q(n) + sum over kids with a complex denominator of D * S(kid), left in c for the root,
+  // S(n) = Q(n) + sum over kids with a complex denominator of D * S(kid): the result for the root,
   // stored as a pair otherwise
   void rnode(int n, std::vector<uint32_t>& code) {
     for (int c : hp.dn[n].kids)
       if (!hp.d_is_real[hp.dn[c].leaf] && has_complex_kids(c)) rnode(c, code);
-    code.push_back(tree_word(kOpCSetV, 0, q_slot[n] >= 0 ? q_slot[n] : 0xffff));
+    std::vector<uint32_t> items;
+    if (q_slot[n] >= 0) items.push_back(tree_item(0, UD, (uint32_t)q_slot[n]));        // D[U_D] = 1
     for (int c : hp.dn[n].kids) {
       const int u = hp.dn[c].leaf;
       if (hp.d_is_real[u]) continue;
-      if (has_complex_kids(c)) code.push_back(tree_word(kOpCFmaDC, u, s_slot[c]));
-      else if (q_slot[c] >= 0) code.push_back(tree_word(kOpCFmaDV, u, q_slot[c]));
+      if (has_complex_kids(c)) items.push_back(tree_item(1, (uint32_t)u, (uint32_t)s_slot[c]));
+      else if (q_slot[c] >= 0) items.push_back(tree_item(0, (uint32_t)u, (uint32_t)q_slot[c]));
     }
-    if (n != 0) {
-      s_slot[n] = take_pair();
-      code.push_back(tree_word(kOpStore, 1, s_slot[n]));
-    }
+    if (n != 0) s_slot[n] = take_pair();
+    emit(code, n != 0 ? (uint32_t)s_slot[n] : kTreeNoDst, items);
   }
 };
 
@@ -421,8 +428,15 @@ struct TreeBuilder {
 
 void build_tree_program(const FlatTable& ft, const HornerPlan& hp, TreeProgram& tp) {
   tp = TreeProgram();
-  if (ft.leafF.size() > 4095 || ft.leafD.size() > 4095) return;
+  if (ft.leafF.size() + 2 * ft.leafD.size() + 1 > 4095) return;
   TreeBuilder b(ft, hp, tp);
+  // constants first: they occupy V[0 .. n_consts)
+  for (const SNode& n : hp.snodes)
+    for (const SItem& it : n.items)
+      if (it.child < 0) b.add_constant(it.num, it.den);
+  for (const HGroup& g : hp.groups)
+    if (g.root < 0) b.add_constant(g.num, g.den);
+  tp.n_slots = (int)tp.consts.size();
   b.uses_left.assign(hp.snodes.size(), 0);
   b.slot_of.assign(hp.snodes.size(), -1);
   b.keep.assign(hp.snodes.size(), 0);
@@ -431,17 +445,11 @@ void build_tree_program(const FlatTable& ft, const HornerPlan& hp, TreeProgram& 
       if (it.child >= 0) ++b.uses_left[it.child];
   for (const HGroup& g : hp.groups)
     if (g.root >= 0) { ++b.uses_left[g.root]; b.keep[g.root] = 1; }
-  // FT of every group
+  // FT of every group (a group without Fermi factors IS its constant)
   std::vector<int> ft_slot(hp.groups.size(), -1);
   for (size_t g = 0; g < hp.groups.size(); ++g) {
     const HGroup& hg = hp.groups[g];
-    if (hg.root >= 0) {
-      ft_slot[g] = b.snode(hg.root, tp.code_beta);
-    } else {
-      tp.code_beta.push_back(tree_word(kOpSetC, 0, b.constant(hg.num, hg.den)));
-      ft_slot[g] = b.take();
-      tp.code_beta.push_back(tree_word(kOpStore, 0, ft_slot[g]));
-    }
+    ft_slot[g] = hg.root >= 0 ? b.snode(hg.root, tp.code_beta) : b.constant(hg.num, hg.den);
   }
   b.free_slots.clear();          // what follows lives until the frequency loop has run: no recycling
   // frequency-independent sub-sums of the nodes the R part visits

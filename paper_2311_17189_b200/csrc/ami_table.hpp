@@ -89,35 +89,27 @@ struct HornerPlan {
 };
 
 // ---- tree plan: the Horner plan as a program for a table-driven interpreter (ami_kernels.cu) ----
-// One 32-bit word per operation: op (4 bits) | a (12 bits) | b (16 bits).  A thread keeps one real
-// accumulator `acc` and one complex accumulator `c`; F[] are its Fermi/Bose leaves, D[] its
-// reciprocal denominators, V[] its value slots, C[] the table's constants.
-enum TreeOp : uint32_t {
-  kOpSetF = 0,     // acc = F[a]
-  kOpSetNegF,      // acc = -F[a]
-  kOpMulFV,        // acc = F[a] * V[b]
-  kOpFmaFV,        // acc = fma(F[a], V[b], acc)
-  kOpAddF,         // acc += F[a]
-  kOpSubF,         // acc -= F[a]
-  kOpMulCF,        // acc = C[b] * F[a]
-  kOpFmaCF,        // acc = fma(C[b], F[a], acc)
-  kOpStore,        // a == 0: V[b] = acc;  a == 1: (V[b], V[b+1]) = c
-  kOpSetV,         // acc = V[b]
-  kOpSetC,         // acc = C[b]
-  kOpMulDV,        // acc = Re D[a] * V[b]            (purely real denominator)
-  kOpFmaDV,        // acc = fma(Re D[a], V[b], acc)
-  kOpCSetV,        // c = (V[b], 0);  b == 0xffff: c = 0
-  kOpCFmaDV,       // c += D[a] * V[b]                (complex denominator, real value)
-  kOpCFmaDC        // c += D[a] * (V[b], V[b+1])      (complex denominator, complex value)
-};
-inline uint32_t tree_word(uint32_t op, uint32_t a, uint32_t b) { return (op << 28) | ((a & 0xfffu) << 16) | (b & 0xffffu); }
+// A program is a list of NODES.  A node is one header word  count << 16 | dst  followed by `count`
+// item words  flag << 28 | a << 16 | b.  Executing a node:
+//   real node (per-beta program):        acc = sum_i L[a_i] * V[b_i];                V[dst] = acc
+//   complex node (per-frequency program): c  = sum_i D[a_i] * (V[b_i], flag_i ? V[b_i+1] : 0);
+//                                          (V[dst], V[dst+1]) = c, or c is the result when dst == 0xffff
+// L[] is the thread's leaf array: L[u] = Fermi/Bose leaf u for u < U_F, L[U_F + 2u] = Re of reciprocal
+// denominator u, L[U_F + 2 U_D] = 1.  D[u] is reciprocal denominator u as a complex number, D[U_D] = 1.
+// V[] are the thread's value slots; V[0 .. n_consts) hold the table's constants (1, -1, coefficients).
+// Items are uniform (no opcode to branch on), so the interpreter's inner loop is a plain FMA loop.
+// A node never straddles a tile of kTreeTileWords words (the builder pads with empty headers).
+constexpr int kTreeTileWords = 1024;
+constexpr uint32_t kTreeNoDst = 0xffffu;
+inline uint32_t tree_header(uint32_t count, uint32_t dst) { return (count << 16) | (dst & 0xffffu); }
+inline uint32_t tree_item(uint32_t flag, uint32_t a, uint32_t b) { return (flag << 28) | ((a & 0xfffu) << 16) | (b & 0xffffu); }
 
 struct TreeProgram {
-  std::vector<uint32_t> code_beta;   // once per (sample, beta): FT sums and frequency-independent sub-sums
-  std::vector<uint32_t> code_freq;   // once per (sample, beta, frequency): the R part; the result is left in c
-  std::vector<double> consts;
-  int n_slots = 0;                   // doubles of V per sample
-  bool ok = false;                   // false: table outside the encoding's limits (4095 leaves, 65534 slots)
+  std::vector<uint32_t> code_beta;   // real nodes, once per (sample, beta): FT sums and frequency-independent sub-sums
+  std::vector<uint32_t> code_freq;   // complex nodes, once per (sample, beta, frequency): the R part
+  std::vector<double> consts;        // preloaded into V[0 .. consts.size())
+  int n_slots = 0;                   // doubles of V per sample, constants included
+  bool ok = false;                   // false: table outside the encoding's limits
 };
 void build_tree_program(const FlatTable& ft, const HornerPlan& hp, TreeProgram& tp);
 

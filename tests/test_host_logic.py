@@ -144,40 +144,44 @@ def test_denominators_keep_their_orientation(ami):
 
 def numpy_run_tree(tab_export, prog, e, z, beta):
     """Interprets the exported tree-plan programs with numpy, all samples at once (test-side restatement
-    of the word format documented in include/ami.h and DESIGN.md 6.3; derivative order <= 1)."""
-    F = []
+    of the node format documented in DESIGN.md 6.3; derivative order <= 1)."""
+    n = e.shape[0]
+    UF, UD = len(tab_export["leafF_c"]), len(tab_export["leafD_c"])
+    D = [1.0 / (e @ c + a @ z + 0j) for c, a in zip(tab_export["leafD_c"], tab_export["leafD_a"])] + [np.ones(n) + 0j]
+    L = []
     for c, sig, k in zip(tab_export["leafF_c"], tab_export["leafF_sig"], tab_export["leafF_k"]):
         f = 1.0 / (sig * np.exp(beta * (e @ c)) + 1.0)
-        F.append(f if k == 0 else -beta * f * (1 - f))
+        L.append(f if k == 0 else -beta * f * (1 - f))
         assert k <= 1
-    D = [1.0 / (e @ c + a @ z + 0j) for c, a in zip(tab_export["leafD_c"], tab_export["leafD_a"])]
-    n = e.shape[0]
+    for d in D:                      # L[U_F + 2u] = Re D[u], L[U_F + 2u + 1] = Im D[u]; the last pair is (1, 0)
+        L += [d.real, d.imag]
     V = np.zeros((prog["n_slots"] + 2, n))
-    C = prog["consts"]
-    acc = np.zeros(n)
-    cplx = np.zeros(n, dtype=complex)
-    for code in (prog["code_beta"], prog["code_freq"]):
-        for w in code:
-            op, a, b = int(w) >> 28, (int(w) >> 16) & 0xfff, int(w) & 0xffff
-            if op == 0: acc = F[a].copy()
-            elif op == 1: acc = -F[a]
-            elif op == 2: acc = F[a] * V[b]
-            elif op == 3: acc = F[a] * V[b] + acc
-            elif op == 4: acc = acc + F[a]
-            elif op == 5: acc = acc - F[a]
-            elif op == 6: acc = C[b] * F[a]
-            elif op == 7: acc = C[b] * F[a] + acc
-            elif op == 8:
-                if a == 0: V[b] = acc
-                else: V[b], V[b + 1] = cplx.real.copy(), cplx.imag.copy()
-            elif op == 9: acc = V[b].copy()
-            elif op == 10: acc = np.full(n, C[b])
-            elif op == 11: acc = D[a].real * V[b]
-            elif op == 12: acc = D[a].real * V[b] + acc
-            elif op == 13: cplx = (V[b] if b != 0xffff else np.zeros(n)) + 0j
-            elif op == 14: cplx = cplx + D[a] * V[b]
-            else: cplx = cplx + D[a] * (V[b] + 1j * V[b + 1])
-    return cplx
+    for i, cst in enumerate(prog["consts"]):
+        V[i] = cst
+    result = None
+    for code, is_complex in ((prog["code_beta"], False), (prog["code_freq"], True)):
+        pos = 0
+        while pos < len(code):
+            count, dst = int(code[pos]) >> 16, int(code[pos]) & 0xffff
+            items = [int(w) for w in code[pos + 1:pos + 1 + count]]
+            assert pos // 1024 == (pos + count) // 1024, "a node straddles a tile"
+            if not is_complex:
+                acc = np.zeros(n)
+                for w in items:
+                    acc = acc + L[(w >> 16) & 0xfff] * V[w & 0xffff]
+                if dst != 0xffff:
+                    V[dst] = acc
+            else:
+                acc = np.zeros(n, dtype=complex)
+                for w in items:
+                    b = w & 0xffff
+                    acc = acc + D[(w >> 16) & 0xfff] * (V[b] + (1j * V[b + 1] if w >> 28 else 0))
+                if dst != 0xffff:
+                    V[dst], V[dst + 1] = acc.real.copy(), acc.imag.copy()
+                else:
+                    result = acc
+            pos += 1 + count
+    return result
 
 
 @pytest.mark.parametrize("name", list(DIAGRAMS))
