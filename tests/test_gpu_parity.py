@@ -370,3 +370,20 @@ def test_run_device_output_and_determinism(ami, torch_mod):
                        want_sum=True)
     assert torch_mod.equal(first, d_out) and sum1[0, 0] == sum2[0, 0]   # deterministic tallies
     assert s1["n_chunks"] == 10
+
+
+def test_run_default_chunking_and_workspace_reuse(ami, torch_mod):
+    """ami_run with host buffers and the library's default chunk (2^17 samples): several chunks on two
+    streams, the cached workspace reused and grown across calls of different sizes and row counts."""
+    cfg = A.get_config("cfg3")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    for n, z, betas in ((300_000 + 17, cfg.z_ext, cfg.betas), (50_000, np.array([[1j], [0.5 + 0.2j]]), (2.0, 8.0, 9.0)),
+                        (400_000, cfg.z_ext, cfg.betas)):
+        k_host = cfg.momenta(n)
+        h_k = torch_mod.from_numpy(k_host.reshape(n, -1)).pin_memory()
+        h_out = torch_mod.empty((len(betas), len(z), n), dtype=torch_mod.complex128).pin_memory()
+        stats, _ = tab.run(n, [cfg.q], cfg.t, cfg.mu, z, betas, h_k=h_k, h_out=h_out)
+        assert stats["n_chunks"] == -(-n // (1 << 17))
+        assert stats["h2d_bytes"] == n * 8 * 8 and stats["d2h_bytes"] == n * 16 * len(betas) * len(z)
+        ref = tab.evaluate_momenta(torch_mod.from_numpy(k_host).cuda(), [cfg.q], cfg.t, cfg.mu, z, betas)
+        assert np.array_equal(h_out.numpy(), ref.cpu().numpy())
