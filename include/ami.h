@@ -198,7 +198,8 @@ int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char*
  * device from `seed` with the counter-based generator of P22 (sample index = first_sample + s);
  * else read from the given buffer, layout [n][2*n_int] (Eq. 8).  Results: per-sample values to
  * h_out / d_out (complex128 [n_b][n_f][n]) when given, and/or the running sum over samples to
- * h_sum (complex128 [n_b][n_f], Monte-Carlo tally of PAPER.md:291) when want_sum. */
+ * h_sum (complex128 [n_b][n_f], Monte-Carlo tally of PAPER.md:291) when want_sum, with the sums of squares
+ * to h_sumsq when that is given too (mean = sum/n, variance of the mean from sumsq/n - mean^2). */
 typedef struct ami_run_cfg {
   int64_t n;             /* samples */
   int64_t chunk;         /* samples per chunk (0 = library default) */
@@ -219,6 +220,8 @@ typedef struct ami_run_cfg {
   void* d_out;           /* device complex128 [n_b][n_f][n] or NULL */
   void* h_sum;           /* host complex128 [n_b][n_f] or NULL */
   void* stream;          /* caller's stream; internal copy/compute streams are ordered after it */
+  void* h_sumsq;         /* host float64 [n_b][n_f][2] or NULL: sums of re^2 and im^2 over the samples (with
+                            want_sum), for the Monte-Carlo error bar of the mean */
 } ami_run_cfg;
 
 typedef struct ami_run_stats {

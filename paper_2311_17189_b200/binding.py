@@ -43,7 +43,8 @@ class ami_run_cfg(C.Structure):
                 ("h_k", C.c_void_p), ("d_k", C.c_void_p), ("q", C.c_void_p), ("t", C.c_double),
                 ("mu", C.c_double), ("z_ext", C.c_void_p), ("n_f", C.c_int32), ("beta", C.c_void_p),
                 ("n_b", C.c_int32), ("e_reg", C.c_double), ("plan", C.c_int32), ("want_sum", C.c_int32),
-                ("h_out", C.c_void_p), ("d_out", C.c_void_p), ("h_sum", C.c_void_p), ("stream", C.c_void_p)]
+                ("h_out", C.c_void_p), ("d_out", C.c_void_p), ("h_sum", C.c_void_p), ("stream", C.c_void_p),
+                ("h_sumsq", C.c_void_p)]
 
 
 class ami_run_stats(C.Structure):
@@ -290,6 +291,8 @@ class AmiTable:
         cfg.e_reg, cfg.plan, cfg.want_sum = float(e_reg), int(plan), int(bool(want_sum))
         sums = np.zeros((b.shape[0], z.shape[0]), dtype=np.complex128) if want_sum else None
         cfg.h_sum = None if sums is None else sums.ctypes.data
+        self.last_sumsq = np.zeros((b.shape[0], z.shape[0], 2)) if want_sum else None   # sums of re^2, im^2
+        cfg.h_sumsq = None if self.last_sumsq is None else self.last_sumsq.ctypes.data
         cfg.stream = _stream_ptr(stream)
         st = ami_run_stats()
         _check(lib().ami_run(self._h, C.byref(cfg), C.byref(st)))

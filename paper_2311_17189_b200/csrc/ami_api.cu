@@ -648,7 +648,10 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   const int64_t rows = (int64_t)cfg->n_b * cfg->n_f;
   const int n_comp = 2 * tab->flat.n_int, n_eps = tab->flat.n_eps;
   if (cfg->n == 0 || rows == 0) {
-    if (cfg->want_sum) memset(cfg->h_sum, 0, (size_t)rows * 16);
+    if (cfg->want_sum) {
+      memset(cfg->h_sum, 0, (size_t)rows * 16);
+      if (cfg->h_sumsq) memset(cfg->h_sumsq, 0, (size_t)rows * 16);
+    }
     if (stats) *stats = local;
     return AMI_OK;
   }
@@ -667,9 +670,9 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   cudaStream_t user = (cudaStream_t)cfg->stream;
   if ((rc = rb.init())) return rc;
   if ((rc = rb.reserve(cfg->d_k ? 0 : (size_t)chunk * n_comp * 8, use_reg ? 0 : (size_t)chunk * n_eps * 8,
-                       direct_out ? 0 : (size_t)chunk * rows * 16, cfg->want_sum ? (size_t)rows * 16 : 0)))
+                       direct_out ? 0 : (size_t)chunk * rows * 16, cfg->want_sum ? (size_t)rows * 32 : 0)))
     return rc;
-  if (cfg->want_sum) CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 16, user));
+  if (cfg->want_sum) CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 32, user));
   CU(cudaEventRecord(rb.ev_start, user));
   CU(cudaStreamWaitEvent(rb.st[0], rb.ev_start, 0));
   CU(cudaStreamWaitEvent(rb.st[1], rb.ev_start, 0));
@@ -715,12 +718,22 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
     CU(cudaEventRecord(rb.ev_done[i], rb.st[i]));
     CU(cudaStreamWaitEvent(user, rb.ev_done[i], 0));
   }
+  std::vector<double> tally;
   if (cfg->want_sum) {
-    CU(cudaMemcpyAsync(cfg->h_sum, rb.sum, (size_t)rows * 16, cudaMemcpyDeviceToHost, user));
-    local.d2h_bytes += rows * 16;
+    tally.resize((size_t)rows * 4);
+    CU(cudaMemcpyAsync(tally.data(), rb.sum, (size_t)rows * 32, cudaMemcpyDeviceToHost, user));
+    local.d2h_bytes += rows * 32;
   }
   CU(cudaEventRecord(rb.ev_stop, user));
   CU(cudaEventSynchronize(rb.ev_stop));   // results in host buffers are complete on return
+  for (int64_t r = 0; cfg->want_sum && r < rows; ++r) {
+    ((double*)cfg->h_sum)[2 * r] = tally[4 * r];
+    ((double*)cfg->h_sum)[2 * r + 1] = tally[4 * r + 1];
+    if (cfg->h_sumsq) {
+      ((double*)cfg->h_sumsq)[2 * r] = tally[4 * r + 2];
+      ((double*)cfg->h_sumsq)[2 * r + 1] = tally[4 * r + 3];
+    }
+  }
   float ms = 0.f;
   CU(cudaEventElapsedTime(&ms, rb.ev_start, rb.ev_stop));
   local.gpu_ms = ms;

@@ -481,19 +481,23 @@ cudaError_t launch_generate_momenta(uint64_t seed, long long first, long long n,
   return cudaGetLastError();
 }
 
-// Per-row sums of complex values: fixed grid, fixed order -> deterministic.
+// Per-row tallies of complex values, (sum re, sum im, sum re^2, sum im^2): fixed grid, fixed order ->
+// deterministic.  The squares give the Monte-Carlo error bar of the mean.
 constexpr int kSumBlocks = 64;
 __global__ void __launch_bounds__(256) row_partial_kernel(const double2* __restrict__ v, long long n,
-                                                          long long row_stride, double2* __restrict__ partial) {
-  __shared__ double2 sh[256];
+                                                          long long row_stride, double4* __restrict__ partial) {
+  __shared__ double4 sh[256];
   const long long row = blockIdx.y;
   const double2* r = v + row * row_stride;
   const long long per = (n + gridDim.x - 1) / gridDim.x;
   const long long a = blockIdx.x * per, b = a + per < n ? a + per : n;
-  double2 acc = make_double2(0.0, 0.0);
+  double4 acc = make_double4(0.0, 0.0, 0.0, 0.0);
   for (long long i = a + threadIdx.x; i < b; i += blockDim.x) {
-    acc.x += r[i].x;
-    acc.y += r[i].y;
+    const double2 x = r[i];
+    acc.x += x.x;
+    acc.y += x.y;
+    acc.z = fma(x.x, x.x, acc.z);
+    acc.w = fma(x.y, x.y, acc.w);
   }
   sh[threadIdx.x] = acc;
   __syncthreads();
@@ -501,33 +505,36 @@ __global__ void __launch_bounds__(256) row_partial_kernel(const double2* __restr
     if (threadIdx.x < w) {
       sh[threadIdx.x].x += sh[threadIdx.x + w].x;
       sh[threadIdx.x].y += sh[threadIdx.x + w].y;
+      sh[threadIdx.x].z += sh[threadIdx.x + w].z;
+      sh[threadIdx.x].w += sh[threadIdx.x + w].w;
     }
     __syncthreads();
   }
   if (threadIdx.x == 0) partial[row * gridDim.x + blockIdx.x] = sh[0];
 }
-__global__ void row_final_kernel(const double2* __restrict__ partial, int n_partial, double2* __restrict__ sum) {
-  const long long row = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  (void)row;
+__global__ void row_final_kernel(const double4* __restrict__ partial, int n_partial, double4* __restrict__ sum) {
   const long long r = blockIdx.x;
   if (threadIdx.x == 0) {
-    double2 acc = sum[r];
+    double4 acc = sum[r];
     for (int i = 0; i < n_partial; ++i) {
       acc.x += partial[r * n_partial + i].x;
       acc.y += partial[r * n_partial + i].y;
+      acc.z += partial[r * n_partial + i].z;
+      acc.w += partial[r * n_partial + i].w;
     }
     sum[r] = acc;
   }
 }
 
+// d_partial: [n_rows][kSumBlocks] double4, d_sum: [n_rows] double4 running tallies
 cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long n, long long row_stride,
                               double* d_partial, double* d_sum, cudaStream_t st, int* launches) {
   if (n_rows == 0) return cudaSuccess;
   dim3 grid(kSumBlocks, (unsigned)n_rows);
   row_partial_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(d_vals), n, row_stride,
-                                           reinterpret_cast<double2*>(d_partial));
-  row_final_kernel<<<(unsigned)n_rows, 32, 0, st>>>(reinterpret_cast<const double2*>(d_partial), kSumBlocks,
-                                                    reinterpret_cast<double2*>(d_sum));
+                                           reinterpret_cast<double4*>(d_partial));
+  row_final_kernel<<<(unsigned)n_rows, 32, 0, st>>>(reinterpret_cast<const double4*>(d_partial), kSumBlocks,
+                                                    reinterpret_cast<double4*>(d_sum));
   count_launch(launches, 2);
   return cudaGetLastError();
 }

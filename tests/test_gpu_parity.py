@@ -345,11 +345,14 @@ def test_run_streamed_matches_stagewise(ami, torch_mod, oracle_mod, mode):
     stats, sums = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, chunk=chunk,
                           h_out=h_out, want_sum=True, **kw)
     assert stats["n_chunks"] == 4 and stats["kernel_launches"] >= 8
-    assert stats["d2h_bytes"] == n * 16 + 16
+    assert stats["d2h_bytes"] == n * 16 + 32       # results + one row of (sum, sum of squares)
     assert stats["h2d_bytes"] == (n * 8 * 8 if mode == "host" else 0)
     np.testing.assert_array_equal(h_out.numpy(), ref.cpu().numpy())   # same kernels, same inputs
     total = ref.cpu().numpy().sum()
     assert abs(sums[0, 0] - total) <= 1e-12 * np.abs(ref.cpu().numpy()).sum()
+    sq = ref.cpu().numpy()[0, 0]
+    want_sq = np.array([np.sum(sq.real ** 2), np.sum(sq.imag ** 2)])
+    assert np.all(np.abs(tab.last_sumsq[0, 0] - want_sq) <= 1e-12 * want_sq)   # Monte-Carlo error bar input
     # and against the oracle end to end on a subset
     sel = np.arange(0, n, 97)
     ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
