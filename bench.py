@@ -412,6 +412,7 @@ def roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s):
             "frac": ach / peak_tf, "traffic": None,
             "peak_source": "DFMA-chain probe run by this bench (FP64 pipe; MEASURED_PEAKS.json has no FP64 figure)",
             "flop_convention": "FP64-pipe instruction slots x 2",
+            "peak_nominal": 2.0 * 148 * 64 * 1.965e9 / 1e12,     # 148 SMs x 64 FP64 lanes x max SM clock (context only)
             "fp64_slots_per_sample": w, "fp64_slots_counted": slots,
             "hbm_leg": {"algorithmic_bytes": bytes_alg, "achieved_gbs": bytes_alg / t_eval / 1e9,
                         "peak_gbs": peaks["hbm_gbs"], "frac": bytes_alg / t_eval / 1e9 / peaks["hbm_gbs"],
