@@ -555,7 +555,8 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
 #undef o
   std::ostringstream o;
   o << kAmiParamsSrc << "\n" << kAmiDeviceSrc << "\n";
-  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n";
+  int tiles = scratch ? 1 : jit_tiles_per_cta();
+  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n#define AMI_U " << tiles << "\n";
   std::string sig = "(const AmiBatch& p, const long long s";
   for (int i = 0; i < ft.n_eps; ++i) sig += ", const double e" + std::to_string(i);
   if (scratch) {
@@ -609,13 +610,19 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_fused(const __grid_constant__ AmiBatch p) {\n"
        "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
        "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
-       "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
-       "#pragma unroll 1\n"
-       "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n"
-       "  const double* ks = p.k + s * p.k_stride_sample;\n";
+       "  // A CTA walks AMI_U consecutive tiles of AMI_NT samples; the momenta of the next tile are loaded into\n"
+       "  // registers before the current one is evaluated, so only the first load of a CTA is exposed.\n"
+       "  const long long base = blockIdx.x * (long long)(AMI_NT * AMI_U) + threadIdx.x;\n";
+  for (int c = 0; c < 2 * ft.n_int; ++c) o << "  double nk" << c << " = 0.0;\n";
+  o << "  if (base < p.n) {\n    const double* kn = p.k + base * p.k_stride_sample;\n";
+  for (int c = 0; c < 2 * ft.n_int; ++c) o << "    nk" << c << " = kn[" << c << " * p.k_stride_comp];\n";
+  o << "  }\n#pragma unroll 1\n  for (int u = 0; u < AMI_U; ++u) {\n"
+       "  const long long s = base + (long long)u * AMI_NT;\n  if (s >= p.n) break;\n";
   for (int l = 0; l < ft.n_int; ++l)
-    o << "  const double kx" << l << " = ks[" << 2 * l << " * p.k_stride_comp], ky" << l << " = ks[" << 2 * l + 1
-      << " * p.k_stride_comp];\n";
+    o << "  const double kx" << l << " = nk" << 2 * l << ", ky" << l << " = nk" << 2 * l + 1 << ";\n";
+  o << "  if (u + 1 < AMI_U && s + AMI_NT < p.n) {\n    const double* kn = p.k + (s + AMI_NT) * p.k_stride_sample;\n";
+  for (int c = 0; c < 2 * ft.n_int; ++c) o << "    nk" << c << " = kn[" << c << " * p.k_stride_comp];\n";
+  o << "  }\n";
   for (int x = 0; x < ft.n_ext; ++x)
     o << "  const double kx" << ft.n_int + x << " = p.q[" << 2 * x << "], ky" << ft.n_int + x << " = p.q[" << 2 * x + 1
       << "];\n";
@@ -637,6 +644,15 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
   o << "  }\n" << call << "  }\n}\n";
   return o.str();
+}
+
+int jit_tiles_per_cta() {
+  static const int u = [] {
+    const char* e = getenv("AMI_JIT_U");
+    const int v = e ? atoi(e) : 0;
+    return (v >= 1 && v <= 16) ? v : kJitTilesPerCtaDefault;
+  }();
+  return u;
 }
 
 int jit_block_threads() {
@@ -762,6 +778,7 @@ struct JitState {
   CUfunction fn_eval = nullptr, fn_fused = nullptr;
   int mode = kJitNone;
   int block = 0;            // threads per CTA the kernels were generated for
+  int tiles = 1;            // tiles of `block` samples one CTA of the fused kernel walks
   int scratch_slots = 0;    // doubles of global scratch per sample (memory-backed variant)
   unsigned smem_bytes = 0;  // dynamic shared memory per CTA (memory-backed variant)
 };
@@ -822,6 +839,7 @@ int jit_prepare(ami_table* tab, std::string& err) {
   std::vector<char> cubin;
   js.mode = jit_mode(tab->flat, tab->horner);
   js.block = js.mode == kJitScratch ? 64 : jit_block_threads();
+  js.tiles = js.mode == kJitScratch ? 1 : jit_tiles_per_cta();
   const std::string src = jit_generate_source(tab->flat, tab->horner, js.block, js.mode == kJitScratch, &js.scratch_slots);
   js.smem_bytes = js.mode == kJitScratch ? (unsigned)(tab->flat.leafF.size() * js.block * sizeof(double)) : 0u;
   js.status = jit_compile(src, cubin, js.log);
@@ -858,7 +876,8 @@ CUresult launch_one(const JitState* js, bool fused, AmiBatch& batch, cudaStream_
   // was 12 % slower on cfg3 and 5 % slower on cfg4, profiles/r01_register_plan.md).  The kernels keep
   // their grid-stride loop, so any grid size is correct.
   const unsigned block = (unsigned)js->block;
-  const unsigned grid = (unsigned)((batch.n + block - 1) / block);
+  const long long per_cta = (long long)block * (fused ? js->tiles : 1);   // the unfused kernel strides over the grid
+  const unsigned grid = (unsigned)((batch.n + per_cta - 1) / per_cta);
   // Programmatic dependent launch: the kernels begin with griddepcontrol.launch_dependents + .wait, so
   // the NEXT specialised kernel in the stream may be scheduled while this one drains and starts the
   // moment it has completed (stream order is kept: nothing is read or written before the wait).

@@ -11,6 +11,8 @@
 namespace ami {
 
 constexpr int kJitBlockThreadsDefault = 64;
+constexpr int kJitTilesPerCtaDefault = 1;
+int jit_tiles_per_cta();    // kJitTilesPerCtaDefault unless AMI_JIT_U overrides it (tuning knob)
 int jit_block_threads();   // kJitBlockThreadsDefault unless AMI_JIT_NT overrides it (tuning knob)
 
 // Tables whose straight-line form is small enough to live in registers and in the instruction
