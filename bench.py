@@ -132,13 +132,17 @@ def fp64_work_per_sample(info, n_f, n_b, reg, tree=False):
 
 
 def ncu_traffic(workload, fused):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
-    p = os.path.join(ROOT, "profiles", "r01_dram_traffic.json")
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture
+    (profiles/r01_dram_traffic.csv; commands in profiles/r01_register_plan.md), or None."""
+    p = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
     if not fused or not os.path.exists(p):
         return None
     with open(p) as f:
-        d = json.load(f).get(workload)
-    return None if d is None else int(d["dram_bytes_read"]) + int(d["dram_bytes_write"])
+        for line in f.read().splitlines()[1:]:
+            w, _kernel, rd, wr = line.split(",")
+            if w == workload:
+                return int(rd) + int(wr)
+    return None
 
 
 def load_measured_peaks():
