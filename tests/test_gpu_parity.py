@@ -390,3 +390,33 @@ def test_run_default_chunking_and_workspace_reuse(ami, torch_mod):
         assert stats["h2d_bytes"] == n * 8 * 8 and stats["d2h_bytes"] == n * 16 * len(betas) * len(z)
         ref = tab.evaluate_momenta(torch_mod.from_numpy(k_host).cuda(), [cfg.q], cfg.t, cfg.mu, z, betas)
         assert np.array_equal(h_out.numpy(), ref.cpu().numpy())
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+def test_two_external_slots_sum_order_and_prefactor(ami, torch_mod, oracle_mod, plan):
+    """The ABI beyond the graded configs: two external frequency slots (the external frequency split
+    into a fermionic and a bosonic part, one of them exactly zero in one row: regulator rule P10(b) needs
+    ALL of a denominator's external values to vanish), a non-default order of the sums, a prefactor."""
+    base = A.get_config("cfg3")
+    d = base.diagram
+    alpha2 = np.concatenate([d.alpha, d.alpha[:, -1:]], axis=1)          # external column twice
+    stat2 = np.concatenate([d.slot_is_fermionic, [0]]).astype(np.uint8)  # fermionic + bosonic
+    order = [2, 0, 3, 1]
+    tab = ami.AmiTable(d.n_int, 2, alpha2, d.eps, stat2, sum_order=order, prefactor=-0.5)
+    ot = oracle_mod.OracleTable(d.n_int, 2, alpha2, d.eps, stat2, sum_order=order, prefactor=-0.5)
+    n = 2000 + 9
+    k_host = base.momenta(n)
+    k = torch_mod.from_numpy(k_host).cuda()
+    q2 = [base.q, (0.0, 0.0)]                     # the second slot carries no momentum
+    beta = 4.0
+    z = np.array([[1j * math.pi / beta, 2j * math.pi / beta], [1j * math.pi / beta, 0j], [0.3 + 0.1j, -0.1 + 0.2j]])
+    out = tab.evaluate_momenta(k, q2, base.t, base.mu, z, [beta], e_reg=1e-8, plan=PLANS[plan]).cpu().numpy()
+    e_rows = ot.dispersion(k_host, q2, base.t, base.mu)
+    truth, S = ot.evaluate(e_rows, z, beta, e_reg=1e-8, quad=True, threads=oracle_mod.hardware_threads(), want_S=True)
+    check_parity(out[0], truth, S, label="two external slots")
+    # same physics as one slot carrying the sum of the two values
+    one = ami.AmiTable.from_diagram(d, sum_order=order, prefactor=-0.5)
+    ref = one.evaluate_momenta(k, [base.q], base.t, base.mu, z.sum(axis=1, keepdims=True)[[0, 2]], [beta], e_reg=1e-8,
+                               plan=PLANS[plan]).cpu().numpy()
+    scale = np.abs(ref[0]).max(axis=1, keepdims=True)
+    assert np.all(np.abs(out[0][[0, 2]] - ref[0]) <= 1e-9 * scale)
