@@ -420,3 +420,28 @@ def test_two_external_slots_sum_order_and_prefactor(ami, torch_mod, oracle_mod, 
                                plan=PLANS[plan]).cpu().numpy()
     scale = np.abs(ref[0]).max(axis=1, keepdims=True)
     assert np.all(np.abs(out[0][[0, 2]] - ref[0]) <= 1e-9 * scale)
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+def test_fused_call_with_soa_momenta(ami, torch_mod, plan):
+    """ami_evaluate_momenta through the raw ABI with SoA momenta [2m][N] (strides 1, N): same bits as
+    the Eq.-8 layout."""
+    import ctypes as C
+    cfg = A.get_config("cfg3")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    n = 3000 + 5
+    k = torch_mod.from_numpy(cfg.momenta(n)).cuda()
+    ref = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, plan=PLANS[plan])
+    ksoa = k.reshape(n, -1).t().contiguous()
+    out = torch_mod.empty_like(ref)
+    e_ws = torch_mod.empty((cfg.diagram.n_eps, n), dtype=torch_mod.float64, device="cuda")
+    q = np.array(cfg.q)
+    z = np.ascontiguousarray(cfg.z_ext, dtype=np.complex128)
+    b = np.array(cfg.betas, dtype=np.float64)
+    rc = ami.lib().ami_evaluate_momenta(tab._h, C.c_void_p(ksoa.data_ptr()), 1, n, q.ctypes.data, cfg.t, cfg.mu, n,
+                                        z.ctypes.data, len(z), b.ctypes.data, len(b), 0.0, PLANS[plan],
+                                        C.c_void_p(e_ws.data_ptr()), C.c_void_p(out.data_ptr()),
+                                        C.c_void_p(torch_mod.cuda.current_stream().cuda_stream))
+    assert rc == 0
+    torch_mod.cuda.synchronize()
+    assert torch_mod.equal(out, ref)
