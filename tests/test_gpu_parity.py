@@ -445,3 +445,32 @@ def test_fused_call_with_soa_momenta(ami, torch_mod, plan):
     assert rc == 0
     torch_mod.cuda.synchronize()
     assert torch_mod.equal(out, ref)
+
+
+def test_argument_errors_and_empty_requests(ami, torch_mod):
+    """Error codes instead of crashes: bad plan, missing buffers; empty grids and batches are no-ops."""
+    import ctypes as C
+    cfg = A.get_config("cfg1")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    L = ami.lib()
+    e = torch_mod.zeros((cfg.diagram.n_eps, 8), dtype=torch_mod.float64, device="cuda")
+    out = torch_mod.zeros((1, 1, 8), dtype=torch_mod.complex128, device="cuda")
+    z = np.ascontiguousarray(cfg.z_ext, dtype=np.complex128)
+    b = np.array(cfg.betas)
+    st = C.c_void_p(torch_mod.cuda.current_stream().cuda_stream)
+
+    def call(plan=0, d_e=e.data_ptr(), d_out=out.data_ptr(), n_e=8, n_f=1, n_b=1, zp=z.ctypes.data, bp=b.ctypes.data):
+        return L.ami_evaluate(tab._h, C.c_void_p(d_e), 0, n_e, zp, n_f, bp, n_b, 0.0, plan, C.c_void_p(d_out), st)
+
+    assert call() == 0
+    assert call(plan=7) == -1 and call(plan=-1) == -1              # AMI_EINVAL
+    assert call(d_out=None) == -1 and call(d_e=None) == -1
+    assert call(n_e=-1) == -1 and call(n_f=-2) == -1
+    assert call(zp=None) == -1 and call(bp=None) == -1
+    assert call(n_e=0) == 0 and call(n_f=0, zp=None) == 0 and call(n_b=0, bp=None) == 0   # nothing to do
+    assert L.ami_evaluate(None, None, 0, 0, None, 0, None, 0, 0.0, 0, None, st) == -1
+    stats, sums = tab.run(0, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, want_sum=True)
+    assert stats["n_chunks"] == 0 and sums[0, 0] == 0
+    with pytest.raises(ami.AmiError):
+        tab.run(10, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, h_k=np.zeros((10, 4)), d_k=torch_mod.zeros((10, 4), dtype=torch_mod.float64, device="cuda"))
+    torch_mod.cuda.synchronize()
