@@ -27,6 +27,7 @@ import numpy as np  # noqa: E402
 
 METRIC = "ami_term_evaluations_per_s"
 UNIT = "term-evals/s"
+SUM_ORDER = "default"
 
 
 def parse_args():
@@ -38,6 +39,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=0, help="override samples per step per GPU")
     ap.add_argument("--plan", default="auto", choices=["auto", "flat", "reg", "tree"])
+    ap.add_argument("--sum-order", default="default", choices=["default", "fewest_terms", "fewest_ops"],
+                    help="order of the Matsubara sums: the configuration's (default) or the one ami_search_sum_order picks")
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads and the CPU baseline")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from Python instead of one CUDA graph")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
@@ -240,7 +243,10 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
     """Times `steps` passes of S1 + S2/S3 over rotating resident momentum batches (the set of inputs is
     larger than L2, so no batch is served from cache).  Returns a dict of device-timed results."""
     from paper_2311_17189_b200 import sharding
-    tab = pkg.AmiTable.from_diagram(cfg.diagram, device=torch.cuda.current_device())
+    sum_order = None
+    if SUM_ORDER != "default":     # experiment knob; term-evals/s then counts the terms of THAT table
+        sum_order = pkg.search_sum_order(cfg.diagram, 0 if SUM_ORDER == "fewest_terms" else 1)[0]
+    tab = pkg.AmiTable.from_diagram(cfg.diagram, device=torch.cuda.current_device(), sum_order=sum_order)
     info = tab.info
     m, n_eps = cfg.diagram.n_int, cfg.diagram.n_eps
     n_f, n_b = len(cfg.z_ext), len(cfg.betas)
@@ -450,6 +456,8 @@ def run_ours(args, dist, rank, local, world):
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local)
     pkg.lib()   # raises if libami_b200.so has not been built
+    global SUM_ORDER
+    SUM_ORDER = args.sum_order
     cfg = A.get_config(args.workload)
     n = samples_per_step(cfg, args)
     first, _ = sharding.weak_range(n, rank, world)
@@ -482,6 +490,7 @@ def run_ours(args, dist, rank, local, world):
         "config": {"workload": cfg.name, "order": cfg.diagram.n_int, "n_green": cfg.diagram.n_g,
                    "samples_per_gpu": n, "n_freq": n_f, "n_beta": n_b, "T_flat": T,
                    "U_F": int(info["n_fermi_leaves"]), "U_D": int(info["n_den_leaves"]), "plan": plan_name,
+                   "sum_order": args.sum_order,
                    "l2": f"inputs rotated over {res['n_rot']} resident batches (> L2)",
                    "parallelism": "replicas" if world == 1 else f"sample-sharded x{world}, no collective"},
         "kernels": {"dominant_ms": res["eval_ms"], "ami_dispersion_ms": None if res["fused"] else res["disp_ms"],

@@ -124,6 +124,22 @@ int ami_construct(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha
 
 int ami_table_info(const ami_table* tab, ami_info* info);
 
+/* ami_search_sum_order -- which order of the Matsubara sums gives the smallest result
+ * ("the order of integration"; the table size depends strongly on it, the value
+ * does not).  Host only, no table is kept.  Orders are enumerated in lexicographic order starting
+ * from 0..n_int-1; at most max_orders of them are constructed (<= 0: all n_int!).  Orders the
+ * recursion rejects (AMI_EUNSUPPORTED_ALPHA, AMI_ENOPOLE, AMI_EUNSUPPORTED) are skipped.
+ *   criterion 0: fewest flat terms T;  1: fewest FP64 operations per sample of the factorised
+ *                (Horner) form, leaves included -- what the register plan executes
+ *   best_order [n_int] out; best_cost, default_cost (cost of 0..n_int-1, -1 if rejected),
+ *   n_tried (orders constructed successfully): optional outs.
+ * Errors: AMI_EINVAL; when no enumerated order is accepted, the code of the last rejection. */
+#define AMI_ORDER_FEWEST_TERMS 0
+#define AMI_ORDER_FEWEST_OPS 1
+int ami_search_sum_order(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha, const int32_t* eps,
+                         const uint8_t* slot_is_fermionic, int criterion, int64_t max_orders,
+                         int32_t* best_order, int64_t* best_cost, int64_t* default_cost, int64_t* n_tried);
+
 /* Serialises the flat table for inspection and tests.  Call with host_buf = NULL to get the size
  * in *bytes; then with a buffer of at least that size.  Layout (little endian, all int32 unless
  * noted): magic 'AMI1', n_int, n_ext, n_eps, U_F, U_D, T, m_f (Fermi factors per term = n_int),

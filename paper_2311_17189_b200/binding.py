@@ -18,7 +18,7 @@ EXPORTS = [
     "ami_construct", "ami_table_info", "ami_table_export", "ami_table_export_tree", "ami_table_destroy", "ami_dispersion",
     "ami_evaluate", "ami_evaluate_momenta", "ami_table_specialize", "ami_table_kernel_source",
     "ami_table_kernel_cubin", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
-    "ami_last_cuda_error", "ami_version", "ami_kernel_launches",
+    "ami_last_cuda_error", "ami_version", "ami_kernel_launches", "ami_search_sum_order",
 ]
 
 
@@ -64,6 +64,8 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.ami_construct.argtypes = [C.c_int] * 4 + [C.c_void_p] * 4 + [C.c_double, C.c_int, C.POINTER(C.c_void_p)]
         L.ami_table_info.argtypes = [C.c_void_p, C.POINTER(ami_info)]
+        L.ami_search_sum_order.argtypes = [C.c_int] * 4 + [C.c_void_p] * 3 + [C.c_int, C.c_int64, C.c_void_p] + \
+            [C.POINTER(C.c_int64)] * 3
         L.ami_table_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.ami_table_export_tree.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.ami_table_destroy.argtypes = [C.c_void_p]
@@ -297,6 +299,23 @@ class AmiTable:
         st = ami_run_stats()
         _check(lib().ami_run(self._h, C.byref(cfg), C.byref(st)))
         return {n_: getattr(st, n_) for n_, _ in ami_run_stats._fields_}, sums
+
+
+ORDER_FEWEST_TERMS, ORDER_FEWEST_OPS = 0, 1
+
+
+def search_sum_order(d, criterion=ORDER_FEWEST_TERMS, max_orders=0):
+    """ami_search_sum_order: the order of the sums of diagram ``d`` with the smallest table
+    (criterion 0) or the fewest FP64 operations per sample of the factorised form (1).
+    Returns (order, cost, cost of the default order or -1, orders accepted)."""
+    alpha, eps = _host(d.alpha, np.int32), _host(d.eps, np.int32)
+    stat = _host(d.slot_is_fermionic, np.uint8)
+    order = np.zeros(d.n_int, dtype=np.int32)
+    best, dflt, tried = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+    _check(lib().ami_search_sum_order(d.n_int, d.n_ext, alpha.shape[0], eps.shape[1], alpha.ctypes.data,
+                                      eps.ctypes.data, stat.ctypes.data, int(criterion), int(max_orders),
+                                      order.ctypes.data, C.byref(best), C.byref(dflt), C.byref(tried)))
+    return order.tolist(), best.value, dflt.value, tried.value
 
 
 def kernel_launches() -> int:

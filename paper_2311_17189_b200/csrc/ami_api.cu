@@ -1,10 +1,12 @@
 // The C ABI of include/ami.h: argument checking, device residency, launches, streamed driver.
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "ami_jit.hpp"
 #include "ami_kernels.cuh"
@@ -180,6 +182,49 @@ int ami_construct(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha
   if (rc != AMI_OK) { delete tab; return rc; }
   *out = tab;
   return AMI_OK;
+}
+
+int ami_search_sum_order(int n_int, int n_ext, int n_g, int n_eps, const int32_t* alpha, const int32_t* eps,
+                         const uint8_t* slot_is_fermionic, int criterion, int64_t max_orders,
+                         int32_t* best_order, int64_t* best_cost, int64_t* default_cost, int64_t* n_tried) {
+  if (!best_order || n_int < 1 || (criterion != AMI_ORDER_FEWEST_TERMS && criterion != AMI_ORDER_FEWEST_OPS))
+    return AMI_EINVAL;
+  std::vector<int32_t> order(n_int);
+  for (int i = 0; i < n_int; ++i) order[i] = i;
+  int64_t best = -1, dflt = -1, tried = 0, seen = 0;
+  int last_rc = AMI_ENOPOLE;
+  try {
+    do {
+      ami::FlatTable ft;
+      const int rc = ami::construct_flat(n_int, n_ext, n_g, n_eps, alpha, eps, slot_is_fermionic, order.data(),
+                                         1.0, ft);
+      if (rc == AMI_EINVAL || rc == AMI_ENOMEM) return rc;
+      if (rc != AMI_OK) last_rc = rc;
+      if (rc == AMI_OK) {
+        int64_t cost = (int64_t)ft.terms.size();
+        if (criterion == AMI_ORDER_FEWEST_OPS) {
+          ami::HornerPlan hp;
+          ami::build_horner_plan(ft, hp);
+          cost = hp.ops_f + hp.ops_d_beta + hp.ops_d + hp.ops_leaf_f + hp.ops_leaf_d + hp.ops_combo;
+        }
+        if (seen == 0) dflt = cost;
+        if (best < 0 || cost < best) {
+          best = cost;
+          for (int i = 0; i < n_int; ++i) best_order[i] = order[i];
+        }
+        ++tried;
+      }
+      ++seen;
+    } while ((max_orders <= 0 || seen < max_orders) && std::next_permutation(order.begin(), order.end()));
+  } catch (const std::bad_alloc&) {
+    return AMI_ENOMEM;
+  } catch (...) {
+    return AMI_EINVAL;
+  }
+  if (best_cost) *best_cost = best;
+  if (default_cost) *default_cost = dflt;
+  if (n_tried) *n_tried = tried;
+  return best < 0 ? last_rc : AMI_OK;
 }
 
 void ami_table_destroy(ami_table* tab) {

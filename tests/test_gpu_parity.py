@@ -35,8 +35,8 @@ def gpu_energies(torch, tab, cfg, k_host):
     return tab.dispersion(k, [cfg.q], cfg.t, cfg.mu)
 
 
-def truth_for(oracle_mod, cfg, e_rows, z, beta, e_reg, quad=True):
-    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+def truth_for(oracle_mod, cfg, e_rows, z, beta, e_reg, quad=True, sum_order=None):
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram, sum_order=sum_order)
     return ot.evaluate(e_rows, z, beta, e_reg=e_reg, quad=quad, threads=oracle_mod.hardware_threads(), want_S=True)
 
 
@@ -71,8 +71,8 @@ def test_dispersion_soa_layout(ami, torch_mod):
 
 
 # ------------------------------------------------------------------ S2 + S3 evaluate
-def run_eval_case(ami, torch, oracle_mod, cfg, n, plan, betas=None, z=None, n_truth=None, start=0):
-    tab = ami.AmiTable.from_diagram(cfg.diagram)
+def run_eval_case(ami, torch, oracle_mod, cfg, n, plan, betas=None, z=None, n_truth=None, start=0, sum_order=None):
+    tab = ami.AmiTable.from_diagram(cfg.diagram, sum_order=sum_order)
     k = cfg.momenta(n, start=start)
     e_dev = gpu_energies(torch, tab, cfg, k)
     betas = cfg.betas if betas is None else betas
@@ -83,7 +83,7 @@ def run_eval_case(ami, torch, oracle_mod, cfg, n, plan, betas=None, z=None, n_tr
     sel = np.arange(n) if n_truth is None or n_truth >= n else np.linspace(0, n - 1, n_truth).astype(np.int64)
     stats = []
     for b, beta in enumerate(betas):
-        truth, S = truth_for(oracle_mod, cfg, e_rows[sel], z, beta, cfg.e_reg)
+        truth, S = truth_for(oracle_mod, cfg, e_rows[sel], z, beta, cfg.e_reg, sum_order=sum_order)
         stats.append(check_parity(out[b][:, sel], truth, S, label=f"{cfg.name} beta={beta}"))
     return stats
 
@@ -474,3 +474,14 @@ def test_argument_errors_and_empty_requests(ami, torch_mod):
     with pytest.raises(ami.AmiError):
         tab.run(10, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, h_k=np.zeros((10, 4)), d_k=torch_mod.zeros((10, 4), dtype=torch_mod.float64, device="cuda"))
     torch_mod.cuda.synchronize()
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+@pytest.mark.parametrize("name,n,crit", [("cfg3", 20_000 + 7, 0), ("cfg5", 300 + 1, 1), ("cfg3", 5000, 1)])
+def test_searched_sum_order(ami, torch_mod, oracle_mod, name, n, crit, plan):
+    """Tables built in the order ami_search_sum_order picks: parity against the oracle
+    summing in that same order, and the same numbers as the default order within both tolerances."""
+    cfg = A.get_config(name)
+    order, best, dflt, _ = ami.search_sum_order(cfg.diagram, crit)
+    assert best <= dflt
+    run_eval_case(ami, torch_mod, oracle_mod, cfg, n, PLANS[plan], sum_order=order, n_truth=150 if name == "cfg5" else None)

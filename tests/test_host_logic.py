@@ -116,6 +116,40 @@ def test_construct_sum_order_and_errors(ami, oracle_mod):
     assert ei.value.code == -1
 
 
+def test_search_sum_order(ami, oracle_mod):
+    """ami_search_sum_order: the order it returns gives a table of the
+    promised size, never larger than the default one, and the same values as the default order."""
+    import itertools
+    d = A.get_config("cfg3").diagram
+    order, best, dflt, tried = ami.search_sum_order(d, ami.ORDER_FEWEST_TERMS)
+    assert sorted(order) == list(range(d.n_int)) and 1 <= tried <= math.factorial(d.n_int)
+    t_def = ami.AmiTable.from_diagram(d, device=None)
+    t_best = ami.AmiTable.from_diagram(d, device=None, sum_order=order)
+    assert t_def.info["n_terms"] == dflt and t_best.info["n_terms"] == best and best <= dflt
+    sizes = []                                   # brute force over all orders through ami_construct
+    for so in itertools.permutations(range(d.n_int)):
+        try:
+            sizes.append(ami.AmiTable.from_diagram(d, device=None, sum_order=list(so)).info["n_terms"])
+        except ami.AmiError:
+            pass
+    assert len(sizes) == tried and min(sizes) == best
+    rng = np.random.default_rng(11)
+    e = rng.uniform(-1.5, 1.5, size=(16, d.n_eps))
+    beta, z = 2.0, np.array([1j * math.pi / 2.0])
+    want, S = oracle_mod.OracleTable.from_diagram(d).evaluate(e, [z], beta, quad=True, want_S=True)
+    got = numpy_eval_export(t_best.export(), e, z, beta)
+    assert np.max(np.abs(got - want[0]) / S[0]) < 1e-12
+    # the operation-count criterion: consistent with ami_table_info of the table it picks
+    order2, best2, dflt2, _ = ami.search_sum_order(d, ami.ORDER_FEWEST_OPS)
+    i2 = ami.AmiTable.from_diagram(d, device=None, sum_order=order2).info
+    assert best2 == i2["fp64_ops_tree"] + i2["fp64_ops_leaf_fermi"] + i2["fp64_ops_leaf_den"] + i2["fp64_ops_combos"]
+    assert best2 <= dflt2
+    # a cap of one order returns the default; bad arguments are refused
+    assert ami.search_sum_order(d, 0, max_orders=1)[:2] == (list(range(d.n_int)), dflt)
+    with pytest.raises(ami.AmiError):
+        ami.search_sum_order(d, 5)
+
+
 def test_no_cpu_fallback(ami):
     """A host-only table cannot be evaluated: every kernel entry point refuses (AMI_ECUDA)."""
     import ctypes as C
