@@ -104,6 +104,45 @@ typedef struct ami_info {
                                AMI_EUNSUPPORTED = table outside the register plan's limits, other < 0 = error */
 } ami_info;
 
+/* ---- Diagram files (Fig. 2; "Feature: Feynman Graph Representation") ----------
+ * A diagram file is plain text, one line of the diagram per row, four integers separated by blanks:
+ *   source target is_fermion spin
+ * source and target are vertex numbers 0..n-1, is_fermion is 1 for a fermionic line and 0 for a
+ * bosonic (interaction) line, spin is a tag that is carried along.  A vertex that is
+ * touched by exactly one row is the far end of an external leg (Fig. 2: vertices 0 and 1).  Text from
+ * '#' to the end of a row is ignored. */
+typedef struct ami_graph_edge {
+  int32_t source, target, is_fermion, spin;
+} ami_graph_edge;
+
+/* read_graph: parses `text` (NUL-terminated).  With edges = NULL only counts the rows.
+ * Errors: AMI_EINVAL for a row that is not four integers, a negative vertex, is_fermion outside
+ * {0,1}, or more rows than `capacity`. */
+int ami_graph_parse(const char* text, ami_graph_edge* edges, int32_t capacity, int32_t* n_edges);
+
+/* label_graph + graph_to_R0: momentum/frequency-conserving labels for every line
+ * and the R0 input of ami_construct.
+ *   Legs: none (n_ext = 0) or one entering and one leaving leg of equal statistics (n_ext = 1; the
+ *   external slot is the LAST column).  The part without the legs must be connected.
+ *   A spanning tree is grown from the bosonic lines first, then the fermionic ones, in file order;
+ *   the lines left over (chords, in file order) carry the independent labels e_0..e_{m-1}, every
+ *   tree line follows from conservation at its vertices,
+ *       sum_in alpha - sum_out alpha = 0   (legs included),
+ *   by leaf stripping.  A bosonic chord would make an internal sum bosonic (Eq. 3 is the fermionic
+ *   sum): AMI_EUNSUPPORTED.  R0 holds the fermionic lines that are not legs, in file order; bosonic
+ *   lines carry no propagator here (contact interaction, reading P23).  Lines of equal alpha share
+ *   one energy symbol whatever their spin tag (P7: the dispersion of this library has one band).
+ * Outputs (any may be NULL; sizes are returned so that a first call can size the buffers):
+ *   n_int, n_ext, n_g, n_eps
+ *   alpha_all [n_edges][n_int + n_ext]  labels of every row of the file, legs and bosons included
+ *   row_of_g  [n_g]                     which row of the file each R0 line is
+ *   alpha     [n_g][n_int + n_ext], eps [n_g][n_eps], slot_is_fermionic [n_int + n_ext]: ami_construct's inputs
+ *   cap_words: capacity, in int32 words, of EACH of alpha_all / alpha / eps (AMI_EINVAL if too small)
+ * Errors: AMI_EINVAL (legs, connectivity, capacity), AMI_EUNSUPPORTED (bosonic chord, limits). */
+int ami_graph_label(const ami_graph_edge* edges, int32_t n_edges, int32_t* n_int, int32_t* n_ext, int32_t* n_g,
+                    int32_t* n_eps, int32_t* alpha_all, int32_t* row_of_g, int32_t* alpha, int32_t* eps,
+                    uint8_t* slot_is_fermionic, int64_t cap_words);
+
 /* ami_construct -- Eqs. 1-5, API of PAPER.md:246.
  *   n_int   number of Matsubara sums m (N_INT);  n_ext number of external frequencies (>= 0)
  *   n_g     number of Green's functions N in R0;  n_eps number of distinct energy symbols

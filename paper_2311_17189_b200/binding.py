@@ -18,7 +18,8 @@ EXPORTS = [
     "ami_construct", "ami_table_info", "ami_table_export", "ami_table_export_tree", "ami_table_destroy", "ami_dispersion",
     "ami_evaluate", "ami_evaluate_momenta", "ami_table_specialize", "ami_table_kernel_source",
     "ami_table_kernel_cubin", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
-    "ami_last_cuda_error", "ami_version", "ami_kernel_launches", "ami_search_sum_order",
+    "ami_last_cuda_error", "ami_version", "ami_kernel_launches", "ami_search_sum_order", "ami_graph_parse",
+    "ami_graph_label",
 ]
 
 
@@ -64,6 +65,8 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.ami_construct.argtypes = [C.c_int] * 4 + [C.c_void_p] * 4 + [C.c_double, C.c_int, C.POINTER(C.c_void_p)]
         L.ami_table_info.argtypes = [C.c_void_p, C.POINTER(ami_info)]
+        L.ami_graph_parse.argtypes = [C.c_char_p, C.c_void_p, C.c_int32, C.POINTER(C.c_int32)]
+        L.ami_graph_label.argtypes = [C.c_void_p, C.c_int32] + [C.POINTER(C.c_int32)] * 4 + [C.c_void_p] * 5 + [C.c_int64]
         L.ami_search_sum_order.argtypes = [C.c_int] * 4 + [C.c_void_p] * 3 + [C.c_int, C.c_int64, C.c_void_p] + \
             [C.POINTER(C.c_int64)] * 3
         L.ami_table_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
@@ -299,6 +302,47 @@ class AmiTable:
         st = ami_run_stats()
         _check(lib().ami_run(self._h, C.byref(cfg), C.byref(st)))
         return {n_: getattr(st, n_) for n_, _ in ami_run_stats._fields_}, sums
+
+
+def read_graph(text_or_path):
+    """ami_graph_parse (read_graph): rows ``source target is_fermion spin`` of a diagram
+    file, or of its text, as an int32 array [n_edges][4]."""
+    text = text_or_path
+    if "\n" not in text and os.path.exists(text):
+        with open(text) as f:
+            text = f.read()
+    raw = text.encode()
+    n = C.c_int32(0)
+    _check(lib().ami_graph_parse(raw, None, 0, C.byref(n)))
+    edges = np.zeros((n.value, 4), dtype=np.int32)
+    _check(lib().ami_graph_parse(raw, edges.ctypes.data, n.value, C.byref(n)))
+    return edges
+
+
+def label_graph(edges):
+    """ami_graph_label (label_graph + graph_to_R0): conserving labels of every line
+    and the inputs of ami_construct.  Returns a namespace that AmiTable.from_diagram accepts
+    (n_int, n_ext, alpha, eps, slot_is_fermionic) plus alpha_all [n_edges][L] and row_of_g [n_g]."""
+    import types
+    edges = _host(edges, np.int32).reshape(-1, 4)
+    sz = [C.c_int32(0) for _ in range(4)]
+    ne = edges.shape[0]
+    _check(lib().ami_graph_label(edges.ctypes.data, ne, *[C.byref(x) for x in sz], None, None, None, None, None, 0))
+    m, n_ext, n_g, n_eps = (x.value for x in sz)
+    L = m + n_ext
+    alpha_all = np.zeros((ne, L), dtype=np.int32)
+    row_of_g = np.zeros(n_g, dtype=np.int32)
+    alpha = np.zeros((n_g, L), dtype=np.int32)
+    eps = np.zeros((n_g, n_eps), dtype=np.int32)
+    stat = np.zeros(L, dtype=np.uint8)
+    cap = max(alpha_all.size, alpha.size, eps.size)
+    alpha_all, alpha, eps = (np.zeros(cap, dtype=np.int32) for _ in range(3))
+    _check(lib().ami_graph_label(edges.ctypes.data, ne, *[C.byref(x) for x in sz], alpha_all.ctypes.data,
+                                 row_of_g.ctypes.data, alpha.ctypes.data, eps.ctypes.data, stat.ctypes.data, cap))
+    return types.SimpleNamespace(n_int=m, n_ext=n_ext, n_g=n_g, n_eps=n_eps,
+                                 alpha=alpha[:n_g * L].reshape(n_g, L).copy(),
+                                 eps=eps[:n_g * n_eps].reshape(n_g, n_eps).copy(), slot_is_fermionic=stat,
+                                 alpha_all=alpha_all[:ne * L].reshape(ne, L).copy(), row_of_g=row_of_g, edges=edges)
 
 
 ORDER_FEWEST_TERMS, ORDER_FEWEST_OPS = 0, 1

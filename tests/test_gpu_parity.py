@@ -485,3 +485,23 @@ def test_searched_sum_order(ami, torch_mod, oracle_mod, name, n, crit, plan):
     order, best, dflt, _ = ami.search_sum_order(cfg.diagram, crit)
     assert best <= dflt
     run_eval_case(ami, torch_mod, oracle_mod, cfg, n, PLANS[plan], sum_order=order, n_truth=150 if name == "cfg5" else None)
+
+
+@pytest.mark.parametrize("plan", list(PLANS))
+def test_diagram_file_to_values(ami, torch_mod, oracle_mod, plan):
+    """Fig. 2's diagram file through read_graph -> label_graph -> ami_construct ->
+    fused evaluation, against the oracle constructed from the same labels."""
+    import os
+    import types
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "fig2_o2_g0_n0.graph")
+    lab = ami.label_graph(ami.read_graph(path))
+    base = A.get_config("cfg1")
+    n = 6000 + 1
+    tab = ami.AmiTable.from_diagram(lab)
+    k = base.momenta(n)
+    out = tab.evaluate_momenta(torch_mod.from_numpy(k).cuda(), [base.q], base.t, base.mu, base.z_ext, base.betas,
+                               plan=PLANS[plan]).cpu().numpy()
+    ot = oracle_mod.OracleTable(lab.n_int, lab.n_ext, lab.alpha, lab.eps, lab.slot_is_fermionic)
+    e = ot.dispersion(k, [base.q], base.t, base.mu, quad=False)
+    truth, S = ot.evaluate(e, base.z_ext, base.betas[0], quad=True, want_S=True)
+    check_parity(out[0], truth, S, label="fig2 diagram file")
