@@ -179,6 +179,14 @@ int ami_search_sum_order(int n_int, int n_ext, int n_g, int n_eps, const int32_t
                          const uint8_t* slot_is_fermionic, int criterion, int64_t max_orders,
                          int32_t* best_order, int64_t* best_cost, int64_t* default_cost, int64_t* n_tried);
 
+/* LaTeX of the flat term table (pretty_print_ft_terms): an `aligned` environment, one
+ * term per row,   sign [coefficient] f_{s}^{(k)}(E) ... \frac{1}{(D)^{p}} ...   with
+ *   f_{+}(E) = 1/(e^{beta E} + 1),  f_{-}(E) = 1/(-e^{beta E} + 1),  ^{(k)} the k-th derivative in E,
+ *   E and D integer combinations of \epsilon_{i} (energy symbol i, the SUPPLIED energies, Eq. 2) and
+ *   z_{j} (external frequency j, i nu or its continuation).  The regulator (P10) is not shown.
+ * Call with buf = NULL to get the size (terminating NUL included) in *bytes. */
+int ami_table_latex(const ami_table* tab, char* buf, size_t* bytes);
+
 /* Serialises the flat table for inspection and tests.  Call with host_buf = NULL to get the size
  * in *bytes; then with a buffer of at least that size.  Layout (little endian, all int32 unless
  * noted): magic 'AMI1', n_int, n_ext, n_eps, U_F, U_D, T, m_f (Fermi factors per term = n_int),

@@ -19,7 +19,7 @@ EXPORTS = [
     "ami_evaluate", "ami_evaluate_momenta", "ami_table_specialize", "ami_table_kernel_source",
     "ami_table_kernel_cubin", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
     "ami_last_cuda_error", "ami_version", "ami_kernel_launches", "ami_search_sum_order", "ami_graph_parse",
-    "ami_graph_label",
+    "ami_graph_label", "ami_table_latex",
 ]
 
 
@@ -72,6 +72,7 @@ def lib():
         L.ami_table_export.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.ami_table_export_tree.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.ami_table_destroy.argtypes = [C.c_void_p]
+        L.ami_table_latex.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.ami_table_destroy.restype = None
         L.ami_dispersion.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
                                      C.c_double, C.c_int64, C.c_void_p, C.c_void_p]
@@ -148,6 +149,14 @@ class AmiTable:
             self._h = None
 
     __del__ = close
+
+    def latex(self) -> str:
+        """ami_table_latex: the flat term table as LaTeX."""
+        n = C.c_size_t(0)
+        _check(lib().ami_table_latex(self._h, None, C.byref(n)))
+        buf = C.create_string_buffer(n.value)
+        _check(lib().ami_table_latex(self._h, buf, C.byref(n)))
+        return buf.value.decode()
 
     def _info(self) -> dict:
         s = ami_info()
