@@ -52,6 +52,8 @@ def lib():
                                       C.c_double, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         L.oracle_dispersion.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
                                         C.c_long, C.c_int, C.c_int, C.c_void_p]
+        L.oracle_dispersion_lattice.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
+                                                C.c_long, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
         L.oracle_fermi.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, C.c_int, C.c_void_p]
         _lib = L
     return _lib
@@ -125,13 +127,15 @@ class OracleTable:
             raise OracleError(rc)
         return (out, S) if want_S else out
 
-    def dispersion(self, k, q, t, mu, quad=False, threads=1):
-        """k: [n_e][n_int][2] (Eq. 8), q: [n_ext][2] -> e [n_e][n_eps], e_i = -eps(K_i)."""
-        k = np.ascontiguousarray(k, dtype=np.float64).reshape(-1, self.n_int, 2)
-        q = np.ascontiguousarray(np.asarray(q, dtype=np.float64).reshape(self.n_ext, 2))
+    def dispersion(self, k, q, t, mu, quad=False, threads=1, dim=2, band=0):
+        """k: [n_e][n_int][dim] (Eq. 8), q: [n_ext][dim] -> e [n_e][n_eps], e_i = -eps(K_i); band 0 =
+        hypercubic tight binding -2t sum cos K_c - mu, band 1 = free particles t |K|^2 - mu."""
+        k = np.ascontiguousarray(k, dtype=np.float64).reshape(-1, self.n_int, dim)
+        q = np.ascontiguousarray(np.asarray(q, dtype=np.float64).reshape(self.n_ext, dim))
         out = np.zeros((k.shape[0], self.n_eps))
-        rc = lib().oracle_dispersion(self._h, k.ctypes.data, q.ctypes.data, float(t), float(mu),
-                                     k.shape[0], 1 if quad else 0, int(threads), out.ctypes.data)
+        rc = lib().oracle_dispersion_lattice(self._h, k.ctypes.data, q.ctypes.data, float(t), float(mu),
+                                             k.shape[0], int(dim), int(band), 1 if quad else 0, int(threads),
+                                             out.ctypes.data)
         if rc:
             raise OracleError(rc)
         return out

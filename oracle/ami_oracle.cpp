@@ -343,20 +343,30 @@ void eval_range(const Table& tb, const double* e, int e_is_complex, long s0, lon
   }
 }
 
-// e_i = -eps(K_i) = 2t(cos Kx + cos Ky) + mu with K_i = sum_l alpha_l k_l + alpha_ext q
-// (Eqs. 9-18; 2D square-lattice tight binding)
+// e_i = -eps(K_i) with K_i = sum_l alpha_l k_l + alpha_ext q, momenta of `dim` components
+// (Eqs. 9-18; Eq. 14 is written for any d).  band 0: tight binding on the hypercubic
+// lattice, eps(K) = -2t sum_c cos K_c - mu (dim = 2: the square lattice of SURVEY.md 8(d));
+// band 1: free particles, eps(K) = t |K|^2 - mu (the paper leaves eps_k to the
+// user).
 template <class T>
-void dispersion_range(const Table& tb, const double* k, const double* q, double t, double mu, long s0,
-                      long s1, double* e_out) {
+void dispersion_range(const Table& tb, const double* k, const double* q, double t, double mu, int dim, int band,
+                      long s0, long s1, double* e_out) {
   const int L = tb.n_int + tb.n_ext;
   for (long s = s0; s < s1; ++s)
     for (int i = 0; i < tb.n_eps; ++i) {
-      T K[2] = {0, 0};
+      T K[3] = {0, 0, 0};
       for (int l = 0; l < tb.n_int; ++l)
-        for (int c = 0; c < 2; ++c) K[c] = K[c] + (T)tb.sym_alpha[i * L + l] * (T)k[(s * tb.n_int + l) * 2 + c];
+        for (int c = 0; c < dim; ++c) K[c] = K[c] + (T)tb.sym_alpha[i * L + l] * (T)k[(s * tb.n_int + l) * dim + c];
       for (int x = 0; x < tb.n_ext; ++x)
-        for (int c = 0; c < 2; ++c) K[c] = K[c] + (T)tb.sym_alpha[i * L + tb.n_int + x] * (T)q[2 * x + c];
-      e_out[s * tb.n_eps + i] = (double)(2 * (T)t * (t_cos(K[0]) + t_cos(K[1])) + (T)mu);
+        for (int c = 0; c < dim; ++c) K[c] = K[c] + (T)tb.sym_alpha[i * L + tb.n_int + x] * (T)q[dim * x + c];
+      T acc = 0;
+      if (band == 0) {
+        for (int c = 0; c < dim; ++c) acc = acc + t_cos(K[c]);
+        e_out[s * tb.n_eps + i] = (double)(2 * (T)t * acc + (T)mu);
+      } else {
+        for (int c = 0; c < dim; ++c) acc = acc + K[c] * K[c];
+        e_out[s * tb.n_eps + i] = (double)((T)mu - (T)t * acc);
+      }
     }
 }
 
@@ -486,16 +496,22 @@ int oracle_evaluate(void* h, const double* e, int e_is_complex, long n_e, const 
   return OR_OK;
 }
 
-// k: [n_e][n_int][2] (Eq. 8), q: [n_ext][2]; e_out: [n_e][n_eps]
-int oracle_dispersion(void* h, const double* k, const double* q, double t, double mu, long n_e,
-                      int precision, int n_threads, double* e_out) {
+// k: [n_e][n_int][dim] (Eq. 8), q: [n_ext][dim]; e_out: [n_e][n_eps]
+int oracle_dispersion_lattice(void* h, const double* k, const double* q, double t, double mu, long n_e, int dim,
+                              int band, int precision, int n_threads, double* e_out) {
   Table* tb = (Table*)h;
-  if (!tb || n_e < 0) return OR_EINVAL;
+  if (!tb || n_e < 0 || dim < 1 || dim > 3 || band < 0 || band > 1) return OR_EINVAL;
   parallel_for(n_e, n_threads, [=](long a, long b) {
-    if (precision == 0) dispersion_range<double>(*tb, k, q, t, mu, a, b, e_out);
-    else dispersion_range<__float128>(*tb, k, q, t, mu, a, b, e_out);
+    if (precision == 0) dispersion_range<double>(*tb, k, q, t, mu, dim, band, a, b, e_out);
+    else dispersion_range<__float128>(*tb, k, q, t, mu, dim, band, a, b, e_out);
   });
   return OR_OK;
+}
+
+// the 2D square-lattice band of the configurations
+int oracle_dispersion(void* h, const double* k, const double* q, double t, double mu, long n_e,
+                      int precision, int n_threads, double* e_out) {
+  return oracle_dispersion_lattice(h, k, q, t, mu, n_e, 2, 0, precision, n_threads, e_out);
 }
 
 // f_sigma^{(k)}(E) for one complex argument; out2 = (re, im).  Used by the pins.

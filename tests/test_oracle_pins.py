@@ -383,6 +383,49 @@ def test_dispersion_random_topology(oracle_mod):
     np.testing.assert_allclose(t.dispersion(kint, [q], 1.0, 0.0, quad=True), want, atol=1e-14)
 
 
+@pytest.mark.parametrize("dim", [1, 2, 3])
+def test_dispersion_lattice_special_points(oracle_mod, dim):
+    """Other dimensions and bands (Eq. 14 is written for any d): values at points where the
+    band is known by inspection.  One line, K = k (order-1 diagram)."""
+    t_ = table(oracle_mod, A.order1_line())
+    tt, mu = 1.3, -0.4
+    pts = {0.0: 2 * tt * dim + mu, math.pi: -2 * tt * dim + mu, math.pi / 3: tt * dim + mu, 2 * math.pi / 3: -tt * dim + mu}
+    for x, want in pts.items():
+        for quad in (False, True):
+            got = t_.dispersion(np.full((1, 1, dim), x), [np.zeros(dim)], tt, mu, quad=quad, dim=dim, band=0)
+            assert abs(got[0, 0] - want) < 4e-15 * dim
+    got = t_.dispersion(np.full((1, 1, dim), math.pi / 2), [np.zeros(dim)], tt, mu, quad=True, dim=dim)
+    assert abs(got[0, 0] - mu) < 1e-15                      # half filling: the band vanishes on the diagonal point
+    k = np.array([1.0, 2.0, 2.0])[:dim].reshape(1, 1, dim)   # free particles: e = mu - t |K|^2
+    want = mu - tt * float((k ** 2).sum())
+    assert t_.dispersion(k, [np.zeros(dim)], tt, mu, dim=dim, band=1)[0, 0] == pytest.approx(want, abs=1e-15)
+    with pytest.raises(oracle_mod.OracleError):
+        t_.dispersion(np.zeros((1, 1, 4)), [np.zeros(4)], tt, mu, dim=4)
+
+
+def test_dispersion_lattice_eq14_and_separability(oracle_mod):
+    """d = 3: K = k . (alpha (x) I_3)^T (Eq. 14) against the oracle's per-symbol loop; the
+    hypercubic band is a sum over components, so the 3D energy is the sum of the 1D energies of the
+    components; d = 2, band 0 is the function the configurations use."""
+    d = A.self_energy_order2()
+    t_ = table(oracle_mod, d)
+    n, m = 40, 2
+    kint = A.momenta(13, n, m, d=3)
+    q = np.array([0.3, -1.1, 2.0])
+    kfull = np.concatenate([kint.reshape(n, 3 * m), np.tile(q, (n, 1))], axis=1)
+    K = kfull @ A.kron_identity(d.symbol_alpha(), 3).T          # [n][n_eps * 3]
+    tt, mu = 0.7, 0.25
+    e3 = t_.dispersion(kint, [q], tt, mu, quad=True, dim=3, band=0)
+    want = 2 * tt * np.cos(K).reshape(n, d.n_eps, 3).sum(axis=2) + mu
+    np.testing.assert_allclose(e3, want, rtol=0, atol=1e-14)
+    parts = sum(t_.dispersion(kint[:, :, c:c + 1], [q[c:c + 1]], tt, 0.0, quad=True, dim=1) for c in range(3))
+    np.testing.assert_allclose(e3 - mu, parts, rtol=0, atol=1e-14)
+    free = t_.dispersion(kint, [q], tt, mu, quad=True, dim=3, band=1)
+    np.testing.assert_allclose(free, mu - tt * (K ** 2).reshape(n, d.n_eps, 3).sum(axis=2), rtol=0, atol=1e-13)
+    k2 = A.momenta(5, 16, m)
+    np.testing.assert_array_equal(t_.dispersion(k2, [q[:2]], tt, mu), t_.dispersion(k2, [q[:2]], tt, mu, dim=2, band=0))
+
+
 # ---------------------------------------------------------------- layout, regulator, threads
 def test_output_layout_and_threads(oracle_mod):
     """[N_F][N_E], energy index fastest; threading changes nothing."""
