@@ -221,6 +221,21 @@ void ami_table_destroy(ami_table* tab);
 int ami_dispersion(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
                    const double* q, double t, double mu, int64_t n, double* d_e, void* stream);
 
+/* ami_dispersion_lattice -- the same map for momenta of dim = 1, 2 or 3 components (Eq. 14 is written for
+ * any dimension d; Eq. 18's index range i*d .. i*d+d-1) and a choice of band (the paper leaves
+ * eps_k to the user):
+ *   AMI_BAND_TIGHT_BINDING  eps(K) = -2t sum_c cos K_c - mu   (hypercubic lattice; dim = 2 is ami_dispersion)
+ *   AMI_BAND_FREE           eps(K) = t |K|^2 - mu             (free particles, t = 1/2m*)
+ * and e_i = -eps(K_i) as above.
+ *   d_k     component c of internal momentum l of sample s at d_k[s * k_stride_sample + (dim*l + c) * k_stride_comp]
+ *   q       host [n_ext][dim];  d_e out, float64 [n_eps][n]
+ * AMI_EINVAL for dim outside 1..3 or an unknown band.  The fused call ami_evaluate_momenta and ami_run keep
+ * the 2D tight-binding band of the configurations: for other bands call this, then ami_evaluate. */
+enum { AMI_BAND_TIGHT_BINDING = 0, AMI_BAND_FREE = 1 };
+int ami_dispersion_lattice(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
+                           const double* q, double t, double mu, int dim, int band, int64_t n, double* d_e,
+                           void* stream);
+
 /* ami_evaluate -- PAPER.md:106-113, :282-289.
  *   d_e     energies, [n_eps][n_e] float64, or complex128 if e_is_complex
  *   z_ext   host complex128 [n_f][n_ext]: external frequency values (i nu_ext on the Matsubara axis,

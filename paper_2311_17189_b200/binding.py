@@ -13,9 +13,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libami_b200.so")
 
 PLAN_AUTO, PLAN_FLAT, PLAN_REG, PLAN_TREE = 0, 1, 2, 3
+BAND_TIGHT_BINDING, BAND_FREE = 0, 1
 
 EXPORTS = [
     "ami_construct", "ami_table_info", "ami_table_export", "ami_table_export_tree", "ami_table_destroy", "ami_dispersion",
+    "ami_dispersion_lattice",
     "ami_evaluate", "ami_evaluate_momenta", "ami_table_specialize", "ami_table_kernel_source",
     "ami_table_kernel_cubin", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
     "ami_last_cuda_error", "ami_version", "ami_kernel_launches", "ami_search_sum_order", "ami_graph_parse",
@@ -76,6 +78,8 @@ def lib():
         L.ami_table_destroy.restype = None
         L.ami_dispersion.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
                                      C.c_double, C.c_int64, C.c_void_p, C.c_void_p]
+        L.ami_dispersion_lattice.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
+                                             C.c_double, C.c_int, C.c_int, C.c_int64, C.c_void_p, C.c_void_p]
         L.ami_evaluate.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_void_p, C.c_int, C.c_void_p,
                                    C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
         L.ami_evaluate_momenta.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
@@ -228,16 +232,22 @@ class AmiTable:
                 "consts": buf[off:off + 8 * nc].view(np.float64).copy(), "n_slots": ns}
 
     # ---- kernels -------------------------------------------------------------------------
-    def dispersion(self, k, q, t, mu, out=None, stream=None):
-        """ami_dispersion.  k: CUDA float64 tensor [n][n_int][2] (Eq. 8 layout) -> e [n_eps][n]."""
+    def dispersion(self, k, q, t, mu, out=None, stream=None, dim=2, band=BAND_TIGHT_BINDING):
+        """ami_dispersion (dim = 2, tight binding) / ami_dispersion_lattice.  k: CUDA float64 tensor
+        [n][n_int][dim] (Eq. 8 layout) -> e [n_eps][n]."""
         import torch
         assert k.is_cuda and k.dtype == torch.float64 and k.is_contiguous()
         n = k.shape[0]
         if out is None:
             out = torch.empty((self.n_eps, n), dtype=torch.float64, device=k.device)
-        qh = _host(np.asarray(q, dtype=np.float64).reshape(max(self.n_ext, 1), 2), np.float64)
-        _check(lib().ami_dispersion(self._h, C.c_void_p(k.data_ptr()), 2 * self.n_int, 1, qh.ctypes.data, float(t),
-                                    float(mu), n, C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        qh = _host(np.asarray(q, dtype=np.float64).reshape(max(self.n_ext, 1), dim), np.float64)
+        if dim == 2 and band == BAND_TIGHT_BINDING:
+            _check(lib().ami_dispersion(self._h, C.c_void_p(k.data_ptr()), 2 * self.n_int, 1, qh.ctypes.data, float(t),
+                                        float(mu), n, C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        else:
+            _check(lib().ami_dispersion_lattice(self._h, C.c_void_p(k.data_ptr()), dim * self.n_int, 1, qh.ctypes.data,
+                                                float(t), float(mu), int(dim), int(band), n,
+                                                C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
         return out
 
     def evaluate(self, e, z_ext, beta, e_reg=0.0, plan=PLAN_AUTO, out=None, stream=None):

@@ -380,6 +380,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
     dp.sym_alpha = tab->dev.sym_alpha;
     dp.n_int = tab->flat.n_int; dp.n_ext = n_ext; dp.n_eps = tab->flat.n_eps;
     dp.k = mom->d_k; dp.k_stride_sample = mom->stride_sample; dp.k_stride_comp = mom->stride_comp; dp.n = n_e;
+    dp.dim = 2; dp.band = AMI_BAND_TIGHT_BINDING;
     for (int i = 0; i < 2 * n_ext; ++i) dp.q[i] = mom->q[i];
     dp.t = mom->t; dp.mu = mom->mu; dp.e = (double*)d_e; dp.e_stride = e_stride;
     cudaError_t crc = launch_dispersion(dp, st);
@@ -467,20 +468,30 @@ int check_device(const ami_table* tab) {
 
 extern "C" {
 
-int ami_dispersion(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
-                   const double* q, double t, double mu, int64_t n, double* d_e, void* stream) {
+int ami_dispersion_lattice(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
+                           const double* q, double t, double mu, int dim, int band, int64_t n, double* d_e,
+                           void* stream) {
   int rc = check_device(tab);
   if (rc) return rc;
-  if (n < 0 || (n > 0 && (!d_k || !d_e)) || (tab->flat.n_ext > 0 && !q)) return AMI_EINVAL;
+  if (n < 0 || (n > 0 && (!d_k || !d_e)) || (tab->flat.n_ext > 0 && !q) || dim < 1 || dim > 3 ||
+      (band != AMI_BAND_TIGHT_BINDING && band != AMI_BAND_FREE))
+    return AMI_EINVAL;
   ami::DispParams p;
   memset(&p, 0, sizeof p);
   p.sym_alpha = tab->dev.sym_alpha;
   p.n_int = tab->flat.n_int; p.n_ext = tab->flat.n_ext; p.n_eps = tab->flat.n_eps;
   p.k = d_k; p.k_stride_sample = k_stride_sample; p.k_stride_comp = k_stride_comp; p.n = n;
-  for (int i = 0; i < 2 * p.n_ext; ++i) p.q[i] = q[i];
+  p.dim = dim; p.band = band;
+  for (int i = 0; i < dim * p.n_ext; ++i) p.q[i] = q[i];
   p.t = t; p.mu = mu; p.e = d_e; p.e_stride = n;
   CU(ami::launch_dispersion(p, (cudaStream_t)stream));
   return AMI_OK;
+}
+
+int ami_dispersion(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
+                   const double* q, double t, double mu, int64_t n, double* d_e, void* stream) {
+  return ami_dispersion_lattice(tab, d_k, k_stride_sample, k_stride_comp, q, t, mu, 2, AMI_BAND_TIGHT_BINDING, n, d_e,
+                                stream);
 }
 
 int ami_evaluate(const ami_table* tab, const void* d_e, int e_is_complex, int64_t n_e, const double* z_ext,

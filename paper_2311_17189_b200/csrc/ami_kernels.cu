@@ -23,9 +23,12 @@ static inline void count_launch(int* launches, int n = 1) {
 }
 
 // ------------------------------------------------------------------------------------------
-// S1: ami_dispersion.  K_i = sum_l alpha^i_l k_l + alpha^i_ext q ; e_i = 2t(cos Kx + cos Ky) + mu
-// (Eqs. 9-18).  The +-1/0 combinations are formed in registers: no matmul.
+// S1: ami_dispersion.  K_i = sum_l alpha^i_l k_l + alpha^i_ext q (Eq. 14, written for any dimension d,
+// PAPER.md:346); e_i = -eps(K_i).  BAND 0: hypercubic tight binding, e = 2t sum_c cos K_c + mu
+// (d = 2: the square lattice of the configurations); BAND 1: free particles, e = mu - t |K|^2 (the paper
+// leaves eps_k to the user).  The +-1/0 combinations are formed in registers: no matmul.
 // ------------------------------------------------------------------------------------------
+template <int DIM, int BAND>
 __global__ void __launch_bounds__(256) dispersion_kernel(DispParams p) {
   __shared__ int8_t s_alpha[AMI_MAX_EPS * (AMI_MAX_INT + AMI_MAX_EXT)];
   const int L = p.n_int + p.n_ext;
@@ -33,38 +36,61 @@ __global__ void __launch_bounds__(256) dispersion_kernel(DispParams p) {
   __syncthreads();
   const long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (s >= p.n) return;
-  double kx[AMI_MAX_INT], ky[AMI_MAX_INT];
+  double k[AMI_MAX_INT][DIM];
   const double* ks = p.k + s * p.k_stride_sample;
 #pragma unroll
   for (int l = 0; l < AMI_MAX_INT; ++l) {
     if (l < p.n_int) {
-      kx[l] = ks[(2 * l) * p.k_stride_comp];
-      ky[l] = ks[(2 * l + 1) * p.k_stride_comp];
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) k[l][c] = ks[(DIM * l + c) * p.k_stride_comp];
     }
   }
   for (int i = 0; i < p.n_eps; ++i) {
-    double Kx = 0.0, Ky = 0.0;
+    double K[DIM];
+#pragma unroll
+    for (int c = 0; c < DIM; ++c) K[c] = 0.0;
 #pragma unroll
     for (int l = 0; l < AMI_MAX_INT; ++l) {
       if (l < p.n_int) {
         const double a = (double)s_alpha[i * L + l];
-        Kx = fma(a, kx[l], Kx);
-        Ky = fma(a, ky[l], Ky);
+#pragma unroll
+        for (int c = 0; c < DIM; ++c) K[c] = fma(a, k[l][c], K[c]);
       }
     }
     for (int x = 0; x < p.n_ext; ++x) {
       const double a = (double)s_alpha[i * L + p.n_int + x];
-      Kx = fma(a, p.q[2 * x], Kx);
-      Ky = fma(a, p.q[2 * x + 1], Ky);
+#pragma unroll
+      for (int c = 0; c < DIM; ++c) K[c] = fma(a, p.q[DIM * x + c], K[c]);
     }
-    p.e[i * p.e_stride + s] = fma(2.0 * p.t, cos_bounded(Kx) + cos_bounded(Ky), p.mu);
+    double acc;
+    if (BAND == 0) {
+      cos_bounded_n<DIM>(K);
+      acc = K[0];
+#pragma unroll
+      for (int c = 1; c < DIM; ++c) acc += K[c];
+      p.e[i * p.e_stride + s] = fma(2.0 * p.t, acc, p.mu);
+    } else {
+      acc = K[0] * K[0];
+#pragma unroll
+      for (int c = 1; c < DIM; ++c) acc = fma(K[c], K[c], acc);
+      p.e[i * p.e_stride + s] = fma(-p.t, acc, p.mu);
+    }
   }
 }
 
 cudaError_t launch_dispersion(const DispParams& p, cudaStream_t st) {
   if (p.n == 0) return cudaSuccess;
   const int nt = 256;
-  dispersion_kernel<<<(unsigned)((p.n + nt - 1) / nt), nt, 0, st>>>(p);
+  const unsigned nb = (unsigned)((p.n + nt - 1) / nt);
+  switch (p.band * 4 + p.dim) {
+    case 1: dispersion_kernel<1, 0><<<nb, nt, 0, st>>>(p); break;
+    case 2: dispersion_kernel<2, 0><<<nb, nt, 0, st>>>(p); break;
+    case 3: dispersion_kernel<3, 0><<<nb, nt, 0, st>>>(p); break;
+    case 5: dispersion_kernel<1, 1><<<nb, nt, 0, st>>>(p); break;
+    case 6: dispersion_kernel<2, 1><<<nb, nt, 0, st>>>(p); break;
+    case 7: dispersion_kernel<3, 1><<<nb, nt, 0, st>>>(p); break;
+    default: return cudaErrorInvalidValue;
+  }
   count_launch(nullptr);
   return cudaGetLastError();
 }

@@ -48,7 +48,8 @@ struct DispParams {
   int n_int, n_ext, n_eps;
   const double* k;
   long long k_stride_sample, k_stride_comp, n;
-  double q[2 * AMI_MAX_EXT];
+  int dim, band;             // momentum components (1..3); 0 = hypercubic tight binding, 1 = free particles
+  double q[3 * AMI_MAX_EXT]; // [n_ext][dim]
   double t, mu;
   double* e;                 // [n_eps][n]
   long long e_stride;

@@ -70,6 +70,48 @@ def test_dispersion_soa_layout(ami, torch_mod):
     assert torch_mod.equal(out, ref)
 
 
+@pytest.mark.parametrize("dim", [1, 2, 3])
+@pytest.mark.parametrize("band", [0, 1])
+def test_dispersion_lattice_parity(ami, torch_mod, oracle_mod, dim, band):
+    """ami_dispersion_lattice (Eq. 14 for d = 1..3, tight-binding and free-particle bands)
+    against the oracle in quad precision, then the values of the order-4 diagram from those energies."""
+    from ami_inputs.rng import momenta
+    cfg = A.get_config("cfg3")
+    n = 2048 + 77
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    k = momenta(cfg.seed + 7 * dim + band, n, cfg.diagram.n_int, d=dim)
+    q = np.array([0.5 * math.pi, -0.25 * math.pi, 1.0][:dim])
+    t, mu = (1.0, -0.2) if band == 0 else (0.5, 1.5)
+    e = tab.dispersion(torch_mod.from_numpy(k).cuda(), [q], t, mu, dim=dim, band=band)
+    want = ot.dispersion(k, [q], t, mu, quad=True, dim=dim, band=band)
+    # tight binding: |e| <= 2 d t + |mu| with a few ulp of (m+1) pi in each angle; free particles:
+    # |K_c| <= 5 pi, so e up to 0.5 * 3 * 250 with a few ulp of that
+    np.testing.assert_allclose(e.cpu().numpy().T, want, rtol=0, atol=2e-14 if band == 0 else 4e-13)
+    if dim == 2 and band == 0:      # the general entry point is the configurations' kernel for d = 2
+        assert torch_mod.equal(e, tab.dispersion(torch_mod.from_numpy(k).cuda(), [q], t, mu))
+    for plan in (ami.PLAN_REG, ami.PLAN_FLAT):
+        got = tab.evaluate(e, cfg.z_ext, cfg.betas, plan=plan).cpu().numpy()
+        truth, S = ot.evaluate(np.ascontiguousarray(e.cpu().numpy().T), cfg.z_ext, cfg.betas[0], quad=True,
+                               threads=oracle_mod.hardware_threads(), want_S=True)
+        ok = np.isfinite(truth[0]) & (S[0] > 1e-290)
+        assert ok.mean() > 0.99
+        assert np.max(np.abs(got[0, 0] - truth[0])[ok] / S[0][ok]) <= 1e-10
+
+
+def test_dispersion_lattice_errors(ami, torch_mod):
+    import ctypes as C
+    cfg = A.get_config("cfg1")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    k = torch_mod.zeros((8, cfg.diagram.n_int, 3), dtype=torch_mod.float64, device="cuda")
+    out = torch_mod.zeros((cfg.diagram.n_eps, 8), dtype=torch_mod.float64, device="cuda")
+    q = np.zeros(4)
+    st = C.c_void_p(torch_mod.cuda.current_stream().cuda_stream)
+    for dim, band in ((0, 0), (4, 0), (2, 2), (2, -1)):
+        assert ami.lib().ami_dispersion_lattice(tab._h, C.c_void_p(k.data_ptr()), 6, 1, q.ctypes.data, 1.0, 0.0, dim,
+                                                band, 8, C.c_void_p(out.data_ptr()), st) == -1
+
+
 # ------------------------------------------------------------------ S2 + S3 evaluate
 def run_eval_case(ami, torch, oracle_mod, cfg, n, plan, betas=None, z=None, n_truth=None, start=0, sum_order=None):
     tab = ami.AmiTable.from_diagram(cfg.diagram, sum_order=sum_order)
