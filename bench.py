@@ -43,6 +43,9 @@ def parse_args():
                     help="order of the Matsubara sums: the configuration's (default) or the one ami_search_sum_order picks")
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads and the CPU baseline")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from Python instead of one CUDA graph")
+    ap.add_argument("--sweep", action="store_true",
+                    help="batch-size sweep (BASELINE config 2: N = 1e3..1e8; the paper's Figs. 4-5 plot time against "
+                         "the batch size): one JSON line with a row per (workload, N); one GPU")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -538,8 +541,50 @@ def run_ours(args, dist, rank, local, world):
         print(json.dumps(line), flush=True)
 
 
+SWEEP = (("cfg2_se", 8), ("cfg2_bubble", 8), ("cfg3", 7), ("cfg4", 7))   # workload, largest power of ten
+
+
+def run_sweep(args, local):
+    """Time per batch against the batch size (Figs. 4-5; BASELINE config 2), device-timed like
+    the headline: K steps of the whole path over rotating resident batches, K reduced for the largest batches."""
+    import torch
+    import ami_inputs as A
+    import paper_2311_17189_b200 as pkg
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    pkg.lib()
+    plan = PLAN_IDS[args.plan]
+    dfma_per_s, _ = pkg.fp64_peak_probe(local)
+    peaks = load_measured_peaks()
+    rows = []
+    for name, top in SWEEP:
+        cfg = A.get_config(name)
+        n_f, n_b = len(cfg.z_ext), len(cfg.betas)
+        for p10 in range(3, top + 1):
+            n = 10 ** p10
+            steps = args.steps if n <= 10 ** 6 else max(3, args.steps // 4)
+            r = time_workload(pkg, torch, cfg, n, steps, args.warmup, plan, 0, None, sample_clocks=False,
+                              use_graph=not args.no_graph)
+            roof, _ = roofline_objects(r, n, n_f, n_b, peaks, dfma_per_s)
+            ms = r["total_ms"] / steps
+            T = int(r["info"]["n_terms"])
+            rows.append({"workload": name, "n": n, "n_freq": n_f, "steps": steps, "ms_per_step": ms,
+                         "ns_per_sample": ms * 1e6 / (n * n_f * n_b), "samples_per_s": n * n_f * n_b / (ms * 1e-3),
+                         "term_evals_per_s": T * n * n_f * n_b / (ms * 1e-3), "alu_frac": roof["frac"],
+                         "hbm_frac": roof["hbm_leg"]["frac"], "launches_per_step": r["launches"] / steps,
+                         "two_stream_ms_per_step": r["two_stream_ms"]})
+            del r
+            torch.cuda.empty_cache()
+    print(json.dumps({"metric": METRIC, "unit": UNIT, "n_gpus": 1, "warmup": args.warmup, "dtype": "f64",
+                      "data": "synthetic", "fp64_probe_dfma_per_s": dfma_per_s, "sweep": rows}), flush=True)
+
+
 def main():
     args = parse_args()
+    if args.sweep:
+        run_sweep(args, 0)
+        return
     dist, rank, local, world = dist_setup(args)
     try:
         if args.impl == "reference":

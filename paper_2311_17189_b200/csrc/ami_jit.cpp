@@ -556,7 +556,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   std::ostringstream o;
   o << kAmiParamsSrc << "\n" << kAmiDeviceSrc << "\n";
   int tiles = scratch ? 1 : jit_tiles_per_cta();
-  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n#define AMI_U " << tiles << "\n";
+  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n#define AMI_U " << tiles << "\n#define AMI_PF " << jit_prefetch_ctas() << "\n";
   std::string sig = "(const AmiBatch& p, const long long s";
   for (int i = 0; i < ft.n_eps; ++i) sig += ", const double e" + std::to_string(i);
   if (scratch) {
@@ -612,7 +612,18 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
        "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
        "  // A CTA walks AMI_U consecutive tiles of AMI_NT samples; the momenta of the next tile are loaded into\n"
        "  // registers before the current one is evaluated, so only the first load of a CTA is exposed.\n"
-       "  const long long base = blockIdx.x * (long long)(AMI_NT * AMI_U) + threadIdx.x;\n";
+       "  const long long base = blockIdx.x * (long long)(AMI_NT * AMI_U) + threadIdx.x;\n"
+       "#if AMI_PF > 0\n"
+       "  // The CTA that will take this one's place on the SM (AMI_PF CTAs further on) finds its momenta in L2:\n"
+       "  // with a few warps per SM the DRAM latency of the first loads is otherwise exposed once per CTA.\n"
+       "  {\n    const long long pb = base + (long long)AMI_PF * (AMI_NT * AMI_U);\n"
+       "    if (pb < p.n) {\n      const double* kp = p.k + pb * p.k_stride_sample;\n"
+       "      if (p.k_stride_comp == 1) {\n";
+  for (int c = 0; c < 2 * ft.n_int; c += 4) o << "        asm volatile(\"prefetch.global.L2 [%0];\" ::\"l\"(kp + " << c << "));\n";
+  o << "      } else {\n";
+  for (int c = 0; c < 2 * ft.n_int; ++c)
+    o << "        asm volatile(\"prefetch.global.L2 [%0];\" ::\"l\"(kp + " << c << " * p.k_stride_comp));\n";
+  o << "      }\n    }\n  }\n#endif\n";
   for (int c = 0; c < 2 * ft.n_int; ++c) o << "  double nk" << c << " = 0.0;\n";
   o << "  if (base < p.n) {\n    const double* kn = p.k + base * p.k_stride_sample;\n";
   for (int c = 0; c < 2 * ft.n_int; ++c) o << "    nk" << c << " = kn[" << c << " * p.k_stride_comp];\n";
@@ -653,6 +664,15 @@ int jit_tiles_per_cta() {
     return (v >= 1 && v <= 16) ? v : kJitTilesPerCtaDefault;
   }();
   return u;
+}
+
+int jit_prefetch_ctas() {
+  static const int pf = [] {
+    const char* e = getenv("AMI_JIT_PF");
+    const int v = e ? atoi(e) : kJitPrefetchCtasDefault;
+    return (v >= 0 && v <= 1 << 20) ? v : kJitPrefetchCtasDefault;
+  }();
+  return pf;
 }
 
 int jit_block_threads() {

@@ -12,6 +12,8 @@ namespace ami {
 
 constexpr int kJitBlockThreadsDefault = 64;
 constexpr int kJitTilesPerCtaDefault = 1;
+constexpr int kJitPrefetchCtasDefault = 0;
+int jit_prefetch_ctas();    // L2 prefetch distance of the fused kernel in CTAs, 0 = off (AMI_JIT_PF, tuning knob)
 int jit_tiles_per_cta();    // kJitTilesPerCtaDefault unless AMI_JIT_U overrides it (tuning knob)
 int jit_block_threads();   // kJitBlockThreadsDefault unless AMI_JIT_NT overrides it (tuning knob)
 
