@@ -549,14 +549,16 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     for (const std::string& st : tail) o << "      " << st << "\n";
     o << "      double2* out = reinterpret_cast<double2*>(p.out) + ((long long)(p.b0 + b) * p.n_f_total + (p.f0 + f)) * "
          "p.out_row_stride + s;\n";
-    o << "      *out = make_double2(p.prefactor * (" << acc.re << "), "
-      << (acc.real() ? std::string("0.0") : "p.prefactor * (" + acc.im + ")") << ");\n";
+    o << "      AMI_STORE(out, make_double2(p.prefactor * (" << acc.re << "), "
+      << (acc.real() ? std::string("0.0") : "p.prefactor * (" + acc.im + ")") << "));\n";
   }
 #undef o
   std::ostringstream o;
   o << kAmiParamsSrc << "\n" << kAmiDeviceSrc << "\n";
   int tiles = scratch ? 1 : jit_tiles_per_cta();
-  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n#define AMI_U " << tiles << "\n#define AMI_PF " << jit_prefetch_ctas() << "\n";
+  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n#define AMI_U " << tiles << "\n#define AMI_PF " << jit_prefetch_ctas() << "\n"
+    << (jit_store_mode() == 1 ? "#define AMI_STORE(p, v) __stcs(p, v)\n"
+        : jit_store_mode() == 2 ? "#define AMI_STORE(p, v) __stwt(p, v)\n" : "#define AMI_STORE(p, v) (*(p) = (v))\n");
   std::string sig = "(const AmiBatch& p, const long long s";
   for (int i = 0; i < ft.n_eps; ++i) sig += ", const double e" + std::to_string(i);
   if (scratch) {
@@ -673,6 +675,15 @@ int jit_prefetch_ctas() {
     return (v >= 0 && v <= 1 << 20) ? v : kJitPrefetchCtasDefault;
   }();
   return pf;
+}
+
+int jit_store_mode() {
+  static const int m = [] {
+    const char* e = getenv("AMI_JIT_STORE");
+    const int v = e ? atoi(e) : kJitStoreModeDefault;
+    return (v >= 0 && v <= 2) ? v : kJitStoreModeDefault;
+  }();
+  return m;
 }
 
 int jit_block_threads() {

@@ -14,6 +14,8 @@ constexpr int kJitBlockThreadsDefault = 64;
 constexpr int kJitTilesPerCtaDefault = 1;
 constexpr int kJitPrefetchCtasDefault = 0;
 int jit_prefetch_ctas();    // L2 prefetch distance of the fused kernel in CTAs, 0 = off (AMI_JIT_PF, tuning knob)
+constexpr int kJitStoreModeDefault = 1;
+int jit_store_mode();       // result stores: 0 plain, 1 streaming (st.global.cs), 2 write-through (AMI_JIT_STORE, tuning knob)
 int jit_tiles_per_cta();    // kJitTilesPerCtaDefault unless AMI_JIT_U overrides it (tuning knob)
 int jit_block_threads();   // kJitBlockThreadsDefault unless AMI_JIT_NT overrides it (tuning knob)
 
