@@ -14,7 +14,7 @@ from dataclasses import dataclass, field
 import numpy as np
 
 from . import diagrams as D
-from .rng import SEED_BASE, momenta
+from .rng import SEED_BASE, energies, momenta
 
 Q_EXT = (math.pi / 2, math.pi / 2)
 
@@ -35,6 +35,11 @@ class Config:
     seed: int = SEED_BASE
     q: tuple = Q_EXT
     meta: dict = field(default_factory=dict)
+
+    def energies(self, n=None, start=0) -> np.ndarray:
+        """[n][n_eps] energies of a workload that supplies them directly (meta["energy_range"])."""
+        return energies(self.seed, self.n_samples if n is None else n, self.diagram.n_eps,
+                        self.meta["energy_range"], start)
 
     def momenta(self, n=None, start=0) -> np.ndarray:
         return momenta(self.seed, self.n_samples if n is None else n, self.diagram.n_int, start)
@@ -79,6 +84,11 @@ def get_config(name: str, **over) -> Config:
         om = np.linspace(-4.0, 4.0, 64)
         c = Config("cfg5", D.random_self_energy(5, TOPOLOGY_SEEDS["cfg5"]), 1.0, 0.0,
                    (2.0, 5.0, 10.0, 20.0), (om + 0.1j).reshape(64, 1), 200_000, seed=SEED_BASE + 5)
+    elif name == "paper_ex1":  # the paper's first example: energies drawn directly
+        beta = 1.0            # in (-8, 8), 100 fermionic frequencies, beta = 1, N_E = 1e6; no dispersion step
+        c = Config("paper_ex1", D.self_energy_order2(), 1.0, 0.0, (beta,),
+                   np.array([[_fermionic(n, beta)] for n in range(100)]), 1_000_000, seed=SEED_BASE + 9,
+                   meta={"energy_range": 8.0})
     elif name == "stress8":  # outside the graded configs: exercises table tiling
         beta = 5.0
         c = Config("stress8", D.random_self_energy(8, TOPOLOGY_SEEDS["stress8"]), 1.0, 0.0, (beta,),

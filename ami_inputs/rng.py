@@ -54,3 +54,13 @@ def momenta(seed: int, n: int, m: int, start: int = 0, d: int = 2) -> np.ndarray
     c = np.arange(n_comp, dtype=np.uint64)[None, :]
     u = uniform01(seed, i * np.uint64(n_comp) + c)
     return ((u - 0.5) * TWO_PI).reshape(n, m, d)
+
+
+def energies(seed: int, n: int, n_eps: int, a: float, start: int = 0) -> np.ndarray:
+    """Energies drawn directly, uniform in [-a, a): the paper's first example fills ``energy_t`` with
+    ``2 a rand - a`` instead of a dispersion.  float64 [n][n_eps], sample
+    ``start + row`` in row ``row``; counter = sample * n_eps + symbol."""
+    i = np.arange(start, start + n, dtype=np.uint64)[:, None]
+    c = np.arange(n_eps, dtype=np.uint64)[None, :]
+    u = uniform01(seed, i * np.uint64(n_eps) + c)
+    return (2.0 * u - 1.0) * a

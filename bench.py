@@ -541,6 +541,36 @@ def run_ours(args, dist, rank, local, world):
         print(json.dumps(line), flush=True)
 
 
+def time_paper_example1(pkg, torch, cfg, steps, warmup, plan, peaks, dfma_per_s):
+    """The paper's first example at its own size: energies supplied directly, [N_F][N_E] results,
+    so a step is ami_evaluate alone (S2+S3).  Energy batches rotate (8 x 24 MB > L2); CUDA events around K calls."""
+    n, n_f, n_b = cfg.n_samples, len(cfg.z_ext), len(cfg.betas)
+    tab = pkg.AmiTable.from_diagram(cfg.diagram, device=torch.cuda.current_device())
+    info = tab.specialize() if plan in (0, 2) else tab.info
+    es = [torch.from_numpy(np.ascontiguousarray(cfg.energies(n, start=r * n).T)).cuda() for r in range(8)]
+    out = torch.empty((n_b, n_f, n), dtype=torch.complex128, device="cuda")
+    for i in range(warmup):
+        tab.evaluate(es[i % 8], cfg.z_ext, cfg.betas, plan=plan, out=out)
+    torch.cuda.synchronize()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = pkg.kernel_launches()
+    t0.record()
+    for i in range(steps):
+        tab.evaluate(es[(warmup + i) % 8], cfg.z_ext, cfg.betas, plan=plan, out=out)
+    t1.record()
+    torch.cuda.synchronize()
+    ms = t0.elapsed_time(t1) / steps
+    reg = plan in (0, 2) and info["reg_plan_status"] == 0
+    w = fp64_work_per_sample(info, n_f, n_b, reg)
+    bytes_alg = n * cfg.diagram.n_eps * 8 + n * n_f * n_b * 16
+    T = int(info["n_terms"])
+    return {"workload": "paper_ex1", "n_e": n, "n_freq": n_f, "beta": cfg.betas[0], "steps": steps, "ms_per_step": ms,
+            "launches_per_step": (pkg.kernel_launches() - l0) / steps, "plan": plan_name_of(info, "auto" if reg else "flat"),
+            "samples_per_s": n * n_f * n_b / (ms * 1e-3), "term_evals_per_s": T * n * n_f * n_b / (ms * 1e-3),
+            "alu_frac": 2.0 * w["evaluate"] * n / (ms * 1e-3) / (2.0 * dfma_per_s),
+            "hbm_frac": bytes_alg / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": bytes_alg}
+
+
 SWEEP = (("cfg2_se", 8), ("cfg2_bubble", 8), ("cfg3", 7), ("cfg4", 7))   # workload, largest power of ten
 
 
@@ -576,8 +606,11 @@ def run_sweep(args, local):
                          "two_stream_ms_per_step": r["two_stream_ms"]})
             del r
             torch.cuda.empty_cache()
+    ex1 = time_paper_example1(pkg, torch, A.get_config("paper_ex1"), max(3, args.steps // 2), args.warmup, plan, peaks,
+                              dfma_per_s)
     print(json.dumps({"metric": METRIC, "unit": UNIT, "n_gpus": 1, "warmup": args.warmup, "dtype": "f64",
-                      "data": "synthetic", "fp64_probe_dfma_per_s": dfma_per_s, "sweep": rows}), flush=True)
+                      "data": "synthetic", "fp64_probe_dfma_per_s": dfma_per_s, "sweep": rows, "paper_ex1": ex1}),
+          flush=True)
 
 
 def main():

@@ -75,6 +75,36 @@ def test_cfg2_sweep_large_batch_streamed(ami, oracle_mod, name):
     assert np.all(np.abs(sums[0] - ref) <= 1e-11 * scale)
 
 
+@pytest.mark.parametrize("plan", ["auto", "flat"])
+def test_paper_example1_full_size(ami, oracle_mod, plan):
+    """The paper's first example at its own size: order-2 self-energy, N_E = 1e6 energy rows
+    drawn in (-8, 8), N_F = 100 fermionic frequencies, beta = 1, through ami_evaluate (no dispersion step);
+    1.6 GB of results [N_F][N_E], sampled parity against the quad oracle."""
+    import torch
+    cfg = A.get_config("paper_ex1")
+    n = cfg.n_samples if plan == "auto" else 200_000
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    e_rows = cfg.energies(n)                                     # [n][n_eps], the paper's orientation
+    e = torch.from_numpy(np.ascontiguousarray(e_rows.T)).cuda()  # the ABI's [n_eps][n]
+    out = tab.evaluate(e, cfg.z_ext, cfg.betas, plan={"auto": ami.PLAN_AUTO, "flat": ami.PLAN_FLAT}[plan])
+    assert out.shape == (1, 100, n)
+    assert bool(torch.isfinite(torch.view_as_real(out)).all())
+    sel = np.unique(np.concatenate([np.linspace(0, n - 1, 3000).astype(np.int64), [0, 63, 64, n - 65, n - 1]]))
+    got = out[0][:, torch.from_numpy(sel).cuda()].cpu().numpy()
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    truth, S = ot.evaluate(np.ascontiguousarray(e_rows[sel]), cfg.z_ext, 1.0, quad=True,
+                           threads=oracle_mod.hardware_threads(), want_S=True)
+    check_parity(got, truth, S, label=f"paper example 1 ({plan})")
+    # the Monte-Carlo reading of the example (PAPER.md:291): row means; against the well-conditioned textbook
+    # form of the order-2 self-energy (SURVEY 8(c)) evaluated with numpy on every sample of the first row
+    if plan == "auto":
+        f = lambda x: 0.5 * (1.0 - np.tanh(0.5 * x))             # noqa: E731  (beta = 1)
+        x1, x2, x3 = -e_rows[:, 0], -e_rows[:, 1], -e_rows[:, 2]
+        ref = -(f(x1) * f(x3) * (1 - f(x2)) + (1 - f(x1)) * (1 - f(x3)) * f(x2)) / (cfg.z_ext[0, 0] + x2 - x1 - x3)
+        mean_gpu = complex(out[0, 0].mean().item())
+        assert abs(mean_gpu - ref.mean()) <= 1e-10 * np.abs(ref).mean()
+
+
 @pytest.mark.parametrize("n", [0, 1, 63, 64, 65, 129])
 def test_fused_edge_sizes(ami, oracle_mod, n):
     import torch

@@ -62,3 +62,16 @@ def test_configs_build():
     c3 = A.get_config("cfg3")
     assert c3.diagram.n_g == 7 and c3.n_samples == 1_000_000 and c3.betas == (8.0,)
     assert A.get_config("cfg4").e_reg == 1e-8 and A.get_config("cfg5").z_ext.shape == (64, 1)
+
+
+def test_energies_range_and_streaming():
+    """Energies of the paper's first example: uniform in [-a, a), stateless."""
+    from ami_inputs.rng import energies
+    e = energies(5, 4000, 3, 8.0)
+    assert e.shape == (4000, 3) and e.min() >= -8.0 and e.max() < 8.0
+    np.testing.assert_array_equal(energies(5, 100, 3, 8.0, start=700), e[700:800])
+    assert abs(e.mean()) < 0.2 and abs(e.std() - 16 / math.sqrt(12)) < 0.1
+    c = A.get_config("paper_ex1")
+    assert c.z_ext.shape == (100, 1) and c.betas == (1.0,) and c.n_samples == 1_000_000
+    assert c.z_ext[3, 0] == 1j * 7 * math.pi
+    np.testing.assert_array_equal(c.energies(10, start=5), energies(c.seed, 10, 3, 8.0, start=5))
