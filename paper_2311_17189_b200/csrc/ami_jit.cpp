@@ -379,7 +379,8 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     if (b == base.size()) base.emplace_back();
     base[b].push_back(u);
   }
-  if (!scratch)
+  const bool smem_f = scratch || jit_fermi_in_smem();
+  if (!smem_f)
     for (size_t u = 0; u < UF; ++u) o << "    double F" << u << ";\n";
   // One exponential per ENERGY SYMBOL, e^{beta e_i} = 2^{n_i} m_i; the exponential of a leaf's
   // combination is assembled from them: integer exponents add, mantissas multiply, so nothing can
@@ -556,11 +557,16 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   std::ostringstream o;
   o << kAmiParamsSrc << "\n" << kAmiDeviceSrc << "\n";
   int tiles = scratch ? 1 : jit_tiles_per_cta();
-  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n#define AMI_U " << tiles << "\n#define AMI_PF " << jit_prefetch_ctas() << "\n"
+  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n#define AMI_U " << tiles << "\n#define AMI_PF " << jit_prefetch_ctas() << "\n#define AMI_MINB " << (scratch ? 1 : jit_min_blocks(block_threads)) << "\n"
     << (jit_store_mode() == 1 ? "#define AMI_STORE(p, v) __stcs(p, v)\n"
         : jit_store_mode() == 2 ? "#define AMI_STORE(p, v) __stwt(p, v)\n" : "#define AMI_STORE(p, v) (*(p) = (v))\n");
   std::string sig = "(const AmiBatch& p, const long long s";
   for (int i = 0; i < ft.n_eps; ++i) sig += ", const double e" + std::to_string(i);
+  if (smem_f && !scratch) {
+    // Fermi/Bose leaves in shared memory as [leaf][thread] (conflict-free), everything else in registers
+    o << "extern __shared__ double sF[];\n";
+    for (size_t u = 0; u < ft.leafF.size(); ++u) o << "#define F" << u << " sF[" << u << " * AMI_NT + threadIdx.x]\n";
+  }
   if (scratch) {
     sig += ", double* __restrict__ w, const long long ws";
     // volatile: every scratch access happens where it is written.  Without it the compiler hoists
@@ -595,7 +601,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   o << sec[3].str() << "    }\n  }\n}\n\n";
   }
   // ---- kernel 1: energies from memory ---------------------------------------------------------
-  o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
+  o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
        "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
        "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
        "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
@@ -609,7 +615,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
                                    : "  if (p.n_b == 1) ami_body" + call_args + "  else ami_body_mb" + call_args;
   o << call << "  }\n}\n\n";
   // ---- kernel 2: momenta from memory, dispersion inline (Eqs. 8-18) ----------
-  o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT) ami_jit_fused(const __grid_constant__ AmiBatch p) {\n"
+  o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_jit_fused(const __grid_constant__ AmiBatch p) {\n"
        "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
        "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
        "  // A CTA walks AMI_U consecutive tiles of AMI_NT samples; the momenta of the next tile are loaded into\n"
@@ -675,6 +681,25 @@ int jit_prefetch_ctas() {
     return (v >= 0 && v <= 1 << 20) ? v : kJitPrefetchCtasDefault;
   }();
   return pf;
+}
+
+int jit_min_blocks(int block_threads) {
+  // __launch_bounds__(AMI_NT, AMI_MINB): the register cap that lets AMI_MINB CTAs share an SM.  (--maxrregcount is
+  // ignored for kernels that carry launch bounds, so this is the knob that changes occupancy.)  Default: 12 warps
+  // per SM = at most 168 registers per thread.  Measured on B200 (profiles/r01_batch_sweep.md): the order-6 kernel
+  // wants 248 registers and runs at 0.77 of the DFMA peak with 8 warps per SM; capped at 168 it spills 80 bytes
+  // and reaches 0.87; at 128 registers the spills cost more than the occupancy gives.
+  static const int env = [] {
+    const char* e = getenv("AMI_JIT_MINB");
+    const int m = e ? atoi(e) : 0;
+    return (m >= 1 && m <= 32) ? m : 0;
+  }();
+  return env ? env : std::max(1, kJitWarpsPerSmTarget * 32 / block_threads);
+}
+
+bool jit_fermi_in_smem() {
+  static const bool v = [] { const char* e = getenv("AMI_JIT_SMEM_F"); return e && e[0] == '1'; }();
+  return v;
 }
 
 int jit_store_mode() {
@@ -872,7 +897,8 @@ int jit_prepare(ami_table* tab, std::string& err) {
   js.block = js.mode == kJitScratch ? 64 : jit_block_threads();
   js.tiles = js.mode == kJitScratch ? 1 : jit_tiles_per_cta();
   const std::string src = jit_generate_source(tab->flat, tab->horner, js.block, js.mode == kJitScratch, &js.scratch_slots);
-  js.smem_bytes = js.mode == kJitScratch ? (unsigned)(tab->flat.leafF.size() * js.block * sizeof(double)) : 0u;
+  js.smem_bytes = (js.mode == kJitScratch || jit_fermi_in_smem())
+                      ? (unsigned)(tab->flat.leafF.size() * js.block * sizeof(double)) : 0u;
   js.status = jit_compile(src, cubin, js.log);
   if (js.status != AMI_OK) { err = js.log; return js.status; }
   Driver& d = driver();

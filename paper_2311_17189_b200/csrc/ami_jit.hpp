@@ -16,6 +16,9 @@ constexpr int kJitPrefetchCtasDefault = 0;
 int jit_prefetch_ctas();    // L2 prefetch distance of the fused kernel in CTAs, 0 = off (AMI_JIT_PF, tuning knob)
 constexpr int kJitStoreModeDefault = 1;
 int jit_store_mode();       // result stores: 0 plain, 1 streaming (st.global.cs), 2 write-through (AMI_JIT_STORE, tuning knob)
+constexpr int kJitWarpsPerSmTarget = 12;   // occupancy the register cap of the specialised kernels is set for
+int jit_min_blocks(int block_threads);   // second argument of __launch_bounds__ (AMI_JIT_MINB overrides; tuning knob)
+bool jit_fermi_in_smem();   // Fermi/Bose leaves in shared memory instead of registers (AMI_JIT_SMEM_F=1, tuning knob)
 int jit_tiles_per_cta();    // kJitTilesPerCtaDefault unless AMI_JIT_U overrides it (tuning knob)
 int jit_block_threads();   // kJitBlockThreadsDefault unless AMI_JIT_NT overrides it (tuning knob)
 
