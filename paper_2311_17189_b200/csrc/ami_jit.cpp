@@ -293,10 +293,10 @@ CV emit_d_sum(const HornerPlan& hp, const std::vector<std::string>& qname, int n
 std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int block_threads, bool scratch,
                                 int* scratch_slots) {
   const int L = ft.n_int + ft.n_ext;
-  size_t kWays = 4;           // independent chains kept side by side
+  size_t kWays = 16;          // independent chains kept side by side (measured: profiles/r01_batch_sweep.md)
   if (const char* env = getenv("AMI_JIT_WAYS")) {   // tuning knob (profiles/)
     const int w = atoi(env);
-    if (w >= 1 && w <= 16) kWays = (size_t)w;
+    if (w >= 1 && w <= 64) kWays = (size_t)w;
   }
   Emitter E;
   // The body of one sample is generated in four sections that are assembled twice below: once
@@ -796,11 +796,7 @@ int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& l
     popt = std::string("--ptxas-options=") + env;
     opts.push_back(popt.c_str());
   }
-  std::string maxreg;
-  if (const char* env = getenv("AMI_JIT_MAXREG")) {   // tuning knob (profiles/): cap registers per thread
-    maxreg = std::string("--maxrregcount=") + env;
-    opts.push_back(maxreg.c_str());
-  }
+  // (no --maxrregcount: it is ignored for kernels with __launch_bounds__; the register cap is AMI_MINB)
   const int rc = n.CompileProgram(prog, (int)opts.size(), opts.data());
   size_t ls = 0;
   n.GetProgramLogSize(prog, &ls);
