@@ -362,6 +362,43 @@ print('SCRATCH-OK', 'W(' in tab.kernel_source())
     assert "SCRATCH-OK True" in out.stdout
 
 
+def test_generator_knobs_do_not_change_the_bits(ami, torch_mod, tmp_path):
+    """The schedule knobs of the specialised kernels (chains side by side, register cap, store policy, tiles per
+    CTA, L2 prefetch, leaves in shared memory) reorder instructions, not arithmetic: every setting returns the
+    bits of the default build, on the single- and the several-temperature body."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = """
+import sys, numpy as np, torch
+import ami_inputs as A, paper_2311_17189_b200 as P
+res = []
+for name in ('cfg3', 'cfg4'):
+    cfg = A.get_config(name); n = 1000 + 29
+    tab = P.AmiTable.from_diagram(cfg.diagram)
+    k = tab.generate_momenta(cfg.seed, 0, n)
+    res.append(tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=P.PLAN_REG).cpu().numpy())
+    res.append(tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, [[1j], [2.0 + 0.5j]], [3.0, 10.0], e_reg=cfg.e_reg, plan=P.PLAN_REG).cpu().numpy())
+    assert tab.refresh_info()['reg_plan_status'] == 0
+np.savez(sys.argv[1], *res)
+"""
+    settings = [{}, {"AMI_JIT_WAYS": "4", "AMI_JIT_MINB": "1", "AMI_JIT_STORE": "0"},
+                {"AMI_JIT_WAYS": "3", "AMI_JIT_MINB": "8", "AMI_JIT_STORE": "2", "AMI_JIT_U": "2", "AMI_JIT_PF": "7"},
+                {"AMI_JIT_SMEM_F": "1", "AMI_JIT_NT": "128", "AMI_JIT_PDL": "0"}]
+    outs = []
+    for i, extra in enumerate(settings):
+        path = str(tmp_path / f"knobs{i}.npz")
+        r = subprocess.run([sys.executable, "-c", code, path], capture_output=True, text=True, cwd=root, timeout=600,
+                           env=dict(os.environ, **extra))
+        assert r.returncode == 0, (extra, r.stderr[-3000:])
+        with np.load(path) as z:
+            outs.append([z[key] for key in z.files])
+    for i in range(1, len(outs)):
+        for a, b in zip(outs[0], outs[i]):
+            assert np.array_equal(a, b, equal_nan=True), settings[i]
+
+
 # ------------------------------------------------------------------ S4 streamed driver
 def test_generated_momenta_bitwise(ami, torch_mod):
     """P22: device generator == host generator, bit for bit."""
