@@ -404,6 +404,27 @@ def time_e2e(pkg, torch, tab, cfg, n, steps, warmup, plan, first_sample, dist):
             "finite": bool(torch.isfinite(torch.view_as_real(h_out[0, 0, :1024])).all().item())}
 
 
+def time_monte_carlo(torch, tab, cfg, n, steps, plan):
+    """S4 in the mode of the paper's Monte-Carlo momentum integration: ami_run generates the
+    momenta on the device from the seed, evaluates them chunk by chunk on two streams and returns only the
+    per-(beta, frequency) sums and sums of squares -- 16 n_f n_b bytes reach the host per step."""
+    tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan, seed=cfg.seed, want_sum=True)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(steps):
+        stats, sums = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan,
+                              seed=cfg.seed, first_sample=(i + 1) * n, want_sum=True)
+    torch.cuda.synchronize()
+    dt = (time.perf_counter() - t0) / steps
+    n_f, n_b = len(cfg.z_ext), len(cfg.betas)
+    mean = sums / n
+    err = np.sqrt(np.maximum(tab.last_sumsq[..., 0] / n - mean.real ** 2, 0.0) / n)
+    return {"samples_per_step": n, "ms_per_step": dt * 1e3, "samples_per_s": n * n_f * n_b / dt,
+            "chunks_per_step": int(stats["n_chunks"]), "launches_per_step": int(stats["kernel_launches"]),
+            "d2h_bytes_per_step": int(stats["d2h_bytes"]), "timed": "host clock around ami_run (synchronous)",
+            "mean_re_first_row": float(mean[0, 0].real), "stderr_re_first_row": float(err[0, 0])}
+
+
 def roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s):
     """Roofline of the dominant kernel: FP64-pipe bound.  Work counted in FP64-pipe instruction slots
     per sample, expressed as DFMA-equivalent TFLOP/s (slot = 2 flop) against the DFMA-chain
@@ -530,6 +551,7 @@ def run_ours(args, dist, rank, local, world):
             del r2
             torch.cuda.empty_cache()
         line["other_workloads"] = others
+        line["monte_carlo"] = time_monte_carlo(torch, res["tab"], cfg, 10 * n, 5, plan)
         import oracle
         threads = oracle.hardware_threads()
         n_s = oracle_sample_size(cfg, threads, args.cpu_seconds)

@@ -357,6 +357,9 @@ struct MomentaSrc {
   int64_t stride_sample = 0, stride_comp = 0;
   const double* q = nullptr;
   double t = 0, mu = 0;
+  bool gen = false;             // register plan only: draw the momenta inside the kernel (d_k unused)
+  uint64_t seed = 0;
+  int64_t first_sample = 0;
 };
 
 // Launches the evaluation for all (beta, frequency) pairs, split so that one launch carries at
@@ -374,7 +377,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
   const int n_ext = tab->flat.n_ext;
   const int f_chunk = n_ext ? std::max(1, kMaxFreqWords / n_ext) : kMaxFreqWords;
   if (mom && !use_reg) {
-    if (!d_e) return AMI_EINVAL;   // the table-driven kernels need the energies in memory
+    if (!d_e || mom->gen) return AMI_EINVAL;   // the table-driven kernels need the energies in memory
     DispParams dp;
     memset(&dp, 0, sizeof dp);
     dp.sym_alpha = tab->dev.sym_alpha;
@@ -395,6 +398,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
     jb.e = (const double*)d_e; jb.e_stride = e_stride;
     if (mom) {
       jb.k = mom->d_k; jb.k_stride_sample = mom->stride_sample; jb.k_stride_comp = mom->stride_comp;
+      jb.gen = mom->gen ? 1 : 0; jb.seed = mom->seed; jb.first_sample = mom->first_sample;
       for (int i = 0; i < 2 * n_ext; ++i) jb.q[i] = mom->q[i];
       jb.t = mom->t; jb.mu = mom->mu;
       jb.e_out = (double*)d_e;
@@ -415,7 +419,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
       for (int64_t c0 = 0; c0 < n_e; c0 += chunk) {
         const int64_t nc = std::min(chunk, n_e - c0);
         MomentaSrc part;
-        if (mom) { part = *mom; part.d_k = mom->d_k + c0 * mom->stride_sample; }
+        if (mom) { part = *mom; part.d_k = mom->d_k + c0 * mom->stride_sample; part.first_sample += c0; }
         rc = evaluate_impl(tab, mom ? &part : nullptr, d_e ? (const double*)d_e + c0 : nullptr, e_is_complex, nc, e_stride,
                            z_ext, n_f, beta, n_b, e_reg, plan, (double*)d_out + 2 * c0, out_row_stride, st, launches);
         if (rc != AMI_OK) return rc;
@@ -655,7 +659,7 @@ struct RunBuffers {
       if (i == 1) { cap_k = ck; cap_e = ce; cap_out = co; }
     }
     size_t c1 = cap_sum, c2 = cap_sum;
-    if ((rc = grow(&partial, &c1, bs * 64)) || (rc = grow(&sum, &c2, bs))) return rc;
+    if ((rc = grow(&partial, &c1, bs * ami::kMaxSumBlocks)) || (rc = grow(&sum, &c2, bs))) return rc;
     cap_sum = std::max(cap_sum, bs);
     return AMI_OK;
   }
@@ -725,7 +729,7 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   std::lock_guard<std::mutex> run_lock(rb.mu);
   cudaStream_t user = (cudaStream_t)cfg->stream;
   if ((rc = rb.init())) return rc;
-  if ((rc = rb.reserve(cfg->d_k ? 0 : (size_t)chunk * n_comp * 8, use_reg ? 0 : (size_t)chunk * n_eps * 8,
+  if ((rc = rb.reserve((cfg->d_k || (use_reg && !cfg->h_k)) ? 0 : (size_t)chunk * n_comp * 8, use_reg ? 0 : (size_t)chunk * n_eps * 8,
                        direct_out ? 0 : (size_t)chunk * rows * 16, cfg->want_sum ? (size_t)rows * 32 : 0)))
     return rc;
   if (cfg->want_sum) CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 32, user));
@@ -744,12 +748,15 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
       CU(cudaMemcpyAsync(rb.k[s], cfg->h_k + c0 * n_comp, (size_t)nc * n_comp * 8, cudaMemcpyHostToDevice, st));
       local.h2d_bytes += nc * n_comp * 8;
       kbuf = rb.k[s];
+    } else if (use_reg) {
+      kbuf = nullptr;     // drawn inside the specialised kernel: no generation launch, no momentum traffic
     } else {
       CU(ami::launch_generate_momenta(cfg->seed, cfg->first_sample + c0, nc, n_comp, rb.k[s], st));
       ++launches;
       kbuf = rb.k[s];
     }
     MomentaSrc ms;
+    ms.gen = !cfg->d_k && !cfg->h_k && use_reg; ms.seed = cfg->seed; ms.first_sample = cfg->first_sample + c0;
     ms.d_k = kbuf; ms.stride_sample = n_comp; ms.stride_comp = 1;
     ms.q = cfg->q; ms.t = cfg->t; ms.mu = cfg->mu;
     double* obuf = direct_out ? (double*)cfg->d_out + 2 * c0 : rb.out[s];

@@ -625,7 +625,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
        "  // The CTA that will take this one's place on the SM (AMI_PF CTAs further on) finds its momenta in L2:\n"
        "  // with a few warps per SM the DRAM latency of the first loads is otherwise exposed once per CTA.\n"
        "  {\n    const long long pb = base + (long long)AMI_PF * (AMI_NT * AMI_U);\n"
-       "    if (pb < p.n) {\n      const double* kp = p.k + pb * p.k_stride_sample;\n"
+       "    if (pb < p.n && !p.gen) {\n      const double* kp = p.k + pb * p.k_stride_sample;\n"
        "      if (p.k_stride_comp == 1) {\n";
   for (int c = 0; c < 2 * ft.n_int; c += 4) o << "        asm volatile(\"prefetch.global.L2 [%0];\" ::\"l\"(kp + " << c << "));\n";
   o << "      } else {\n";
@@ -633,14 +633,24 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     o << "        asm volatile(\"prefetch.global.L2 [%0];\" ::\"l\"(kp + " << c << " * p.k_stride_comp));\n";
   o << "      }\n    }\n  }\n#endif\n";
   for (int c = 0; c < 2 * ft.n_int; ++c) o << "  double nk" << c << " = 0.0;\n";
-  o << "  if (base < p.n) {\n    const double* kn = p.k + base * p.k_stride_sample;\n";
-  for (int c = 0; c < 2 * ft.n_int; ++c) o << "    nk" << c << " = kn[" << c << " * p.k_stride_comp];\n";
+  // momenta of sample `at`: from memory, or drawn in place by the counter-based generator (S4 with a seed:
+  // the momenta never exist in memory)
+  auto emit_momenta = [&](const std::string& at, const std::string& ind) {
+    o << ind << "if (p.gen) {\n" << ind << "  const unsigned long long c0 = (unsigned long long)(p.first_sample + (" << at
+      << ")) * " << 2 * ft.n_int << "ull;\n";
+    for (int c = 0; c < 2 * ft.n_int; ++c) o << ind << "  nk" << c << " = momentum_of(p.seed, c0 + " << c << "ull);\n";
+    o << ind << "} else {\n" << ind << "  const double* kn = p.k + (" << at << ") * p.k_stride_sample;\n";
+    for (int c = 0; c < 2 * ft.n_int; ++c) o << ind << "  nk" << c << " = kn[" << c << " * p.k_stride_comp];\n";
+    o << ind << "}\n";
+  };
+  o << "  if (base < p.n) {\n";
+  emit_momenta("base", "    ");
   o << "  }\n#pragma unroll 1\n  for (int u = 0; u < AMI_U; ++u) {\n"
        "  const long long s = base + (long long)u * AMI_NT;\n  if (s >= p.n) break;\n";
   for (int l = 0; l < ft.n_int; ++l)
     o << "  const double kx" << l << " = nk" << 2 * l << ", ky" << l << " = nk" << 2 * l + 1 << ";\n";
-  o << "  if (u + 1 < AMI_U && s + AMI_NT < p.n) {\n    const double* kn = p.k + (s + AMI_NT) * p.k_stride_sample;\n";
-  for (int c = 0; c < 2 * ft.n_int; ++c) o << "    nk" << c << " = kn[" << c << " * p.k_stride_comp];\n";
+  o << "  if (u + 1 < AMI_U && s + AMI_NT < p.n) {\n";
+  emit_momenta("s + AMI_NT", "    ");
   o << "  }\n";
   for (int x = 0; x < ft.n_ext; ++x)
     o << "  const double kx" << ft.n_int + x << " = p.q[" << 2 * x << "], ky" << ft.n_int + x << " = p.q[" << 2 * x + 1
@@ -977,6 +987,7 @@ cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cuda
     if (part.e) part.e += c0;                       // SoA rows keep their stride
     if (part.e_out) part.e_out += c0;
     if (part.k) part.k += c0 * b.k_stride_sample;
+    part.first_sample += c0;
     part.out += 2 * c0;
     part.scratch = scratch;
     part.scratch_stride = chunk;

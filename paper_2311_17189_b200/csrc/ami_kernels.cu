@@ -2,6 +2,7 @@
 // evaluation (S2 + S3, flat plan), momentum generation and tallies for the streamed driver (S4).
 // One thread owns one sample; every table read is warp-uniform; per-sample leaf values live in
 // shared memory as [slot][thread] so that every access is conflict-free.
+#include <algorithm>
 #include <atomic>
 #include <cstdio>
 
@@ -478,21 +479,12 @@ cudaError_t launch_eval_tree(const EvalParams& p, cudaStream_t st, int* launches
 // ------------------------------------------------------------------------------------------
 // S4 helpers: counter-based momenta (reading P22) and deterministic tallies.
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ double uniform01(uint64_t seed, uint64_t ctr) {
-  uint64_t z = seed + 0x9E3779B97F4A7C15ull * (ctr + 1ull);
-  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
-  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
-  z = z ^ (z >> 31);
-  return (double)(z >> 11) * 0x1.0p-53;
-}
-
 __global__ void __launch_bounds__(256) momenta_kernel(uint64_t seed, long long first, long long n, int n_comp,
                                                       double* __restrict__ k) {
   const long long total = n * n_comp;
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total;
        i += (long long)gridDim.x * blockDim.x) {
-    const double u = uniform01(seed, (uint64_t)(first * n_comp + i));
-    k[i] = __dmul_rn(u - 0.5, 6.283185307179586);
+    k[i] = momentum_of(seed, (unsigned long long)(first * n_comp + i));
   }
 }
 
@@ -509,7 +501,13 @@ cudaError_t launch_generate_momenta(uint64_t seed, long long first, long long n,
 
 // Per-row tallies of complex values, (sum re, sum im, sum re^2, sum im^2): fixed grid, fixed order ->
 // deterministic.  The squares give the Monte-Carlo error bar of the mean.
-constexpr int kSumBlocks = 64;
+// Blocks per row: enough CTAs to fill the machine whatever the number of rows (one row of 1e6 values on 64
+// CTAs ran at a tenth of the HBM bandwidth), a function of (rows, n) only, so the order of the sum is fixed.
+int sum_blocks(long long n_rows, long long n) {
+  long long b = (8 * 148 + n_rows - 1) / n_rows;
+  b = std::min<long long>(b, (n + 1023) / 1024);
+  return (int)std::max<long long>(1, std::min<long long>(b, kMaxSumBlocks));
+}
 __global__ void __launch_bounds__(256) row_partial_kernel(const double2* __restrict__ v, long long n,
                                                           long long row_stride, double4* __restrict__ partial) {
   __shared__ double4 sh[256];
@@ -518,6 +516,7 @@ __global__ void __launch_bounds__(256) row_partial_kernel(const double2* __restr
   const long long per = (n + gridDim.x - 1) / gridDim.x;
   const long long a = blockIdx.x * per, b = a + per < n ? a + per : n;
   double4 acc = make_double4(0.0, 0.0, 0.0, 0.0);
+#pragma unroll 4
   for (long long i = a + threadIdx.x; i < b; i += blockDim.x) {
     const double2 x = r[i];
     acc.x += x.x;
@@ -538,28 +537,38 @@ __global__ void __launch_bounds__(256) row_partial_kernel(const double2* __restr
   }
   if (threadIdx.x == 0) partial[row * gridDim.x + blockIdx.x] = sh[0];
 }
-__global__ void row_final_kernel(const double4* __restrict__ partial, int n_partial, double4* __restrict__ sum) {
+// One warp per row: lane l adds partials l, l+32, ... in that order, lane 0 then adds the 32 lane sums in lane
+// order and folds the result into the running tally.  Fixed order -> deterministic.
+__global__ void __launch_bounds__(32) row_final_kernel(const double4* __restrict__ partial, int n_partial,
+                                                       double4* __restrict__ sum) {
+  __shared__ double4 sh[32];
   const long long r = blockIdx.x;
+  double4 acc = make_double4(0.0, 0.0, 0.0, 0.0);
+#pragma unroll 4
+  for (int i = threadIdx.x; i < n_partial; i += 32) {
+    const double4 x = partial[r * n_partial + i];
+    acc.x += x.x; acc.y += x.y; acc.z += x.z; acc.w += x.w;
+  }
+  sh[threadIdx.x] = acc;
+  __syncwarp();
   if (threadIdx.x == 0) {
-    double4 acc = sum[r];
-    for (int i = 0; i < n_partial; ++i) {
-      acc.x += partial[r * n_partial + i].x;
-      acc.y += partial[r * n_partial + i].y;
-      acc.z += partial[r * n_partial + i].z;
-      acc.w += partial[r * n_partial + i].w;
+    double4 t = sum[r];
+    for (int l = 0; l < 32; ++l) {
+      t.x += sh[l].x; t.y += sh[l].y; t.z += sh[l].z; t.w += sh[l].w;
     }
-    sum[r] = acc;
+    sum[r] = t;
   }
 }
 
-// d_partial: [n_rows][kSumBlocks] double4, d_sum: [n_rows] double4 running tallies
+// d_partial: [n_rows][<= kMaxSumBlocks] double4, d_sum: [n_rows] double4 running tallies
 cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long n, long long row_stride,
                               double* d_partial, double* d_sum, cudaStream_t st, int* launches) {
   if (n_rows == 0) return cudaSuccess;
-  dim3 grid(kSumBlocks, (unsigned)n_rows);
+  const int nblk = sum_blocks(n_rows, n);
+  dim3 grid((unsigned)nblk, (unsigned)n_rows);
   row_partial_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(d_vals), n, row_stride,
                                            reinterpret_cast<double4*>(d_partial));
-  row_final_kernel<<<(unsigned)n_rows, 32, 0, st>>>(reinterpret_cast<const double4*>(d_partial), kSumBlocks,
+  row_final_kernel<<<(unsigned)n_rows, 32, 0, st>>>(reinterpret_cast<const double4*>(d_partial), nblk,
                                                     reinterpret_cast<double4*>(d_sum));
   count_launch(launches, 2);
   return cudaGetLastError();

@@ -10,6 +10,7 @@ namespace ami {
 
 constexpr int kMaxFreqWords = 64;   // n_f * n_ext complex values per launch
 constexpr int kMaxBeta = 8;         // inverse temperatures per launch
+constexpr int kMaxSumBlocks = 8 * 148;   // partial sums per row of the tally kernels
 constexpr int kTermTile = 256;      // terms per shared-memory tile of the flat plan (multiple of 8)
 
 struct EvalParams {

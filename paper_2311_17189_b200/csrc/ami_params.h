@@ -26,7 +26,10 @@ struct AmiBatch {
   // results: complex128, row r = (b0 + b) * n_f_total + (f0 + f) at out + 2 * r * out_row_stride
   double* out;
   long long n, out_row_stride;
-  int n_f, n_b, n_f_total, f0, b0, pad;
+  int n_f, n_b, n_f_total, f0, b0;
+  int gen;                  // fused path: momenta come from the counter-based generator (P22), k is not read
+  unsigned long long seed;  // generator seed and the stream index of sample 0 of this batch
+  long long first_sample;
   double e_reg, prefactor;
   double beta[AMI_K_MAX_BETA];
   double ceta[AMI_K_MAX_BETA];          // exp(beta * e_reg), formed on the host (exactly 1 without regulator)

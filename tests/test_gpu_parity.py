@@ -400,6 +400,35 @@ np.savez(sys.argv[1], *res)
 
 
 # ------------------------------------------------------------------ S4 streamed driver
+@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg5"])
+def test_run_draws_momenta_in_kernel_bitwise(ami, torch_mod, name):
+    """ami_run with a seed and the register plan draws the momenta inside the evaluation kernel (they never exist in
+    memory): same bits as feeding the host generator's momenta (P22) through the same driver, across chunk borders
+    and a non-zero first sample; the table-driven plan, which generates them with momenta_kernel, agrees too."""
+    cfg = A.get_config(name)
+    n, first = (3000 + 41, 777) if name != "cfg5" else (600 + 5, 12345)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    nb, nf = len(cfg.betas), len(cfg.z_ext)
+    outs = []
+    for kw in ({"seed": cfg.seed, "first_sample": first},
+               {"h_k": np.ascontiguousarray(cfg.momenta(n, start=first).reshape(n, -1))}):
+        d_out = torch_mod.zeros((nb, nf, n), dtype=torch_mod.complex128, device="cuda")
+        l0 = ami.kernel_launches()
+        stats, sums = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, chunk=1024, d_out=d_out,
+                              want_sum=True, **kw)
+        outs.append((d_out.cpu().numpy(), sums, ami.kernel_launches() - l0))
+    assert tab.refresh_info()["reg_plan_status"] == 0
+    assert np.array_equal(outs[0][0], outs[1][0], equal_nan=True)
+    assert np.array_equal(outs[0][1], outs[1][1], equal_nan=True)
+    assert outs[0][2] == outs[1][2]                  # no generation launches: evaluate + two tally kernels per chunk
+    flat = torch_mod.zeros((nb, nf, n), dtype=torch_mod.complex128, device="cuda")
+    tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, chunk=1024, d_out=flat, seed=cfg.seed,
+            first_sample=first, plan=ami.PLAN_FLAT)
+    ref = outs[0][0]
+    scale = np.abs(ref).max(axis=-1, keepdims=True)
+    assert np.all(np.abs(flat.cpu().numpy() - ref) <= 1e-9 * scale)
+
+
 def test_generated_momenta_bitwise(ami, torch_mod):
     """P22: device generator == host generator, bit for bit."""
     cfg = A.get_config("cfg4")
