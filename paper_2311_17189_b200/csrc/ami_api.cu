@@ -717,7 +717,7 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   }
   // default chunk: small enough that the host copies of one chunk overlap the kernels of the next
   const bool host_io = cfg->h_k || cfg->h_out;
-  int64_t chunk = cfg->chunk ? cfg->chunk : (host_io ? (int64_t)1 << 17 : (int64_t)1 << 20);
+  int64_t chunk = cfg->chunk ? cfg->chunk : (host_io ? (int64_t)1 << 17 : (int64_t)1 << 22);
   // keep a chunk's output below ~256 MiB
   while (chunk > 1024 && chunk * rows * 16 > ((int64_t)256 << 20)) chunk /= 2;
   if (chunk > cfg->n) chunk = cfg->n;

@@ -537,25 +537,32 @@ __global__ void __launch_bounds__(256) row_partial_kernel(const double2* __restr
   }
   if (threadIdx.x == 0) partial[row * gridDim.x + blockIdx.x] = sh[0];
 }
-// One warp per row: lane l adds partials l, l+32, ... in that order, lane 0 then adds the 32 lane sums in lane
-// order and folds the result into the running tally.  Fixed order -> deterministic.
-__global__ void __launch_bounds__(32) row_final_kernel(const double4* __restrict__ partial, int n_partial,
-                                                       double4* __restrict__ sum) {
-  __shared__ double4 sh[32];
+// One CTA per row: thread t adds partials t, t+256, ... in that order, then a shared-memory tree with a fixed
+// shape, and thread 0 folds the result into the running tally.  Fixed order -> deterministic.
+__global__ void __launch_bounds__(256) row_final_kernel(const double4* __restrict__ partial, int n_partial,
+                                                        double4* __restrict__ sum) {
+  __shared__ double4 sh[256];
   const long long r = blockIdx.x;
   double4 acc = make_double4(0.0, 0.0, 0.0, 0.0);
 #pragma unroll 4
-  for (int i = threadIdx.x; i < n_partial; i += 32) {
+  for (int i = threadIdx.x; i < n_partial; i += 256) {
     const double4 x = partial[r * n_partial + i];
     acc.x += x.x; acc.y += x.y; acc.z += x.z; acc.w += x.w;
   }
   sh[threadIdx.x] = acc;
-  __syncwarp();
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (threadIdx.x < w) {
+      sh[threadIdx.x].x += sh[threadIdx.x + w].x;
+      sh[threadIdx.x].y += sh[threadIdx.x + w].y;
+      sh[threadIdx.x].z += sh[threadIdx.x + w].z;
+      sh[threadIdx.x].w += sh[threadIdx.x + w].w;
+    }
+    __syncthreads();
+  }
   if (threadIdx.x == 0) {
     double4 t = sum[r];
-    for (int l = 0; l < 32; ++l) {
-      t.x += sh[l].x; t.y += sh[l].y; t.z += sh[l].z; t.w += sh[l].w;
-    }
+    t.x += sh[0].x; t.y += sh[0].y; t.z += sh[0].z; t.w += sh[0].w;
     sum[r] = t;
   }
 }
@@ -568,7 +575,7 @@ cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long 
   dim3 grid((unsigned)nblk, (unsigned)n_rows);
   row_partial_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(d_vals), n, row_stride,
                                            reinterpret_cast<double4*>(d_partial));
-  row_final_kernel<<<(unsigned)n_rows, 32, 0, st>>>(reinterpret_cast<const double4*>(d_partial), nblk,
+  row_final_kernel<<<(unsigned)n_rows, 256, 0, st>>>(reinterpret_cast<const double4*>(d_partial), nblk,
                                                     reinterpret_cast<double4*>(d_sum));
   count_launch(launches, 2);
   return cudaGetLastError();
