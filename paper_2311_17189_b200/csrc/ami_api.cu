@@ -352,11 +352,15 @@ int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg
   return AMI_OK;
 }
 
+constexpr int64_t kFusedTallyMaxRows = 16;   // beyond this the warp reductions cost more than re-reading the results
+
 struct MomentaSrc {
   const double* d_k = nullptr;
   int64_t stride_sample = 0, stride_comp = 0;
   const double* q = nullptr;
   double t = 0, mu = 0;
+  double* tally = nullptr;      // register plan only: per-warp partial sums [rows][tally_stride] double4, or NULL
+  int64_t tally_stride = 0;
   bool gen = false;             // register plan only: draw the momenta inside the kernel (d_k unused)
   uint64_t seed = 0;
   int64_t first_sample = 0;
@@ -399,6 +403,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
     if (mom) {
       jb.k = mom->d_k; jb.k_stride_sample = mom->stride_sample; jb.k_stride_comp = mom->stride_comp;
       jb.gen = mom->gen ? 1 : 0; jb.seed = mom->seed; jb.first_sample = mom->first_sample;
+      jb.tally = mom->tally; jb.tally_stride = mom->tally_stride;
       for (int i = 0; i < 2 * n_ext; ++i) jb.q[i] = mom->q[i];
       jb.t = mom->t; jb.mu = mom->mu;
       jb.e_out = (double*)d_e;
@@ -629,7 +634,8 @@ struct RunBuffers {
   double* k[2] = {nullptr, nullptr};
   double* e[2] = {nullptr, nullptr};
   double* out[2] = {nullptr, nullptr};
-  size_t cap_k = 0, cap_e = 0, cap_out = 0, cap_sum = 0;
+  double* wp[2] = {nullptr, nullptr};     // per-warp partial sums of the fused tally
+  size_t cap_k = 0, cap_e = 0, cap_out = 0, cap_sum = 0, cap_wp = 0;
   double* partial = nullptr;
   double* sum = nullptr;
   int init() {
@@ -651,12 +657,14 @@ struct RunBuffers {
     *cap = bytes;
     return AMI_OK;
   }
-  int reserve(size_t bk, size_t be, size_t bo, size_t bs) {
+  int reserve(size_t bk, size_t be, size_t bo, size_t bs, size_t bw) {
     int rc;
     for (int i = 0; i < 2; ++i) {
-      size_t ck = cap_k, ce = cap_e, co = cap_out;
-      if ((rc = grow(&k[i], &ck, bk)) || (rc = grow(&e[i], &ce, be)) || (rc = grow(&out[i], &co, bo))) return rc;
-      if (i == 1) { cap_k = ck; cap_e = ce; cap_out = co; }
+      size_t ck = cap_k, ce = cap_e, co = cap_out, cw = cap_wp;
+      if ((rc = grow(&k[i], &ck, bk)) || (rc = grow(&e[i], &ce, be)) || (rc = grow(&out[i], &co, bo)) ||
+          (rc = grow(&wp[i], &cw, bw)))
+        return rc;
+      if (i == 1) { cap_k = ck; cap_e = ce; cap_out = co; cap_wp = cw; }
     }
     size_t c1 = cap_sum, c2 = cap_sum;
     if ((rc = grow(&partial, &c1, bs * ami::kMaxSumBlocks)) || (rc = grow(&sum, &c2, bs))) return rc;
@@ -667,7 +675,7 @@ struct RunBuffers {
     for (int i = 0; i < 2; ++i) {
       if (st[i]) cudaStreamDestroy(st[i]);
       if (ev_done[i]) cudaEventDestroy(ev_done[i]);
-      cudaFree(k[i]); cudaFree(e[i]); cudaFree(out[i]);
+      cudaFree(k[i]); cudaFree(e[i]); cudaFree(out[i]); cudaFree(wp[i]);
     }
     if (ev_start) cudaEventDestroy(ev_start);
     if (ev_stop) cudaEventDestroy(ev_stop);
@@ -729,8 +737,15 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   std::lock_guard<std::mutex> run_lock(rb.mu);
   cudaStream_t user = (cudaStream_t)cfg->stream;
   if ((rc = rb.init())) return rc;
-  if ((rc = rb.reserve((cfg->d_k || (use_reg && !cfg->h_k)) ? 0 : (size_t)chunk * n_comp * 8, use_reg ? 0 : (size_t)chunk * n_eps * 8,
-                       direct_out ? 0 : (size_t)chunk * rows * 16, cfg->want_sum ? (size_t)rows * 32 : 0)))
+  // Fused tally (register plan, a few rows): the evaluation kernel leaves one partial sum per (row, warp) and the
+  // results are stored only if the caller wants them -- a seeded Monte-Carlo run then moves no sample data at all.
+  const bool fused_tally = use_reg && cfg->want_sum && rows <= kFusedTallyMaxRows;
+  const bool need_out = cfg->h_out || !use_reg || (cfg->want_sum && !fused_tally);
+  const int64_t wp_stride = (chunk + 31) / 32;
+  if ((rc = rb.reserve((cfg->d_k || (use_reg && !cfg->h_k)) ? 0 : (size_t)chunk * n_comp * 8,
+                       use_reg ? 0 : (size_t)chunk * n_eps * 8,
+                       (direct_out || !need_out) ? 0 : (size_t)chunk * rows * 16, cfg->want_sum ? (size_t)rows * 32 : 0,
+                       fused_tally ? (size_t)rows * wp_stride * 32 : 0)))
     return rc;
   if (cfg->want_sum) CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 32, user));
   CU(cudaEventRecord(rb.ev_start, user));
@@ -759,7 +774,8 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
     ms.gen = !cfg->d_k && !cfg->h_k && use_reg; ms.seed = cfg->seed; ms.first_sample = cfg->first_sample + c0;
     ms.d_k = kbuf; ms.stride_sample = n_comp; ms.stride_comp = 1;
     ms.q = cfg->q; ms.t = cfg->t; ms.mu = cfg->mu;
-    double* obuf = direct_out ? (double*)cfg->d_out + 2 * c0 : rb.out[s];
+    double* obuf = direct_out ? (double*)cfg->d_out + 2 * c0 : (need_out ? rb.out[s] : nullptr);
+    if (fused_tally) { ms.tally = rb.wp[s]; ms.tally_stride = wp_stride; }
     const int64_t ostride = direct_out ? cfg->n : nc;
     rc = evaluate_impl(tab, &ms, rb.e[s], 0, nc, nc, cfg->z_ext, cfg->n_f, cfg->beta, cfg->n_b, cfg->e_reg, cfg->plan,
                        obuf, ostride, st, &launches);
@@ -772,7 +788,10 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
     if (cfg->want_sum) {
       // tallies are chained in chunk order so that the running sum is deterministic
       if (ci > 0) CU(cudaStreamWaitEvent(st, rb.ev_done[s ^ 1], 0));
-      CU(ami::launch_block_sums(obuf, rows, nc, ostride, rb.partial, rb.sum, st, &launches));
+      if (fused_tally)
+        CU(ami::launch_warp_partial_sums(rb.wp[s], rows, (nc + 31) / 32, wp_stride, rb.partial, rb.sum, st, &launches));
+      else
+        CU(ami::launch_block_sums(obuf, rows, nc, ostride, rb.partial, rb.sum, st, &launches));
     }
     CU(cudaEventRecord(rb.ev_done[s], st));
     ++local.n_chunks;

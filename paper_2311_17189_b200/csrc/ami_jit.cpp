@@ -548,10 +548,11 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     }
     if (!have) acc.re = "0.0";
     for (const std::string& st : tail) o << "      " << st << "\n";
-    o << "      double2* out = reinterpret_cast<double2*>(p.out) + ((long long)(p.b0 + b) * p.n_f_total + (p.f0 + f)) * "
-         "p.out_row_stride + s;\n";
-    o << "      AMI_STORE(out, make_double2(p.prefactor * (" << acc.re << "), "
-      << (acc.real() ? std::string("0.0") : "p.prefactor * (" + acc.im + ")") << "));\n";
+    o << "      const long long row = (long long)(p.b0 + b) * p.n_f_total + (p.f0 + f);\n";
+    o << "      const double2 val = make_double2(p.prefactor * (" << acc.re << "), "
+      << (acc.real() ? std::string("0.0") : "p.prefactor * (" + acc.im + ")") << ");\n";
+    o << "      if (p.out) AMI_STORE(reinterpret_cast<double2*>(p.out) + row * p.out_row_stride + s, val);\n";
+    o << "      if (p.tally) ami_tally(reinterpret_cast<double4*>(p.tally) + row * p.tally_stride + (s >> 5), val);\n";
   }
 #undef o
   std::ostringstream o;
@@ -560,6 +561,20 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n#define AMI_U " << tiles << "\n#define AMI_PF " << jit_prefetch_ctas() << "\n#define AMI_MINB " << (scratch ? 1 : jit_min_blocks(block_threads)) << "\n"
     << (jit_store_mode() == 1 ? "#define AMI_STORE(p, v) __stcs(p, v)\n"
         : jit_store_mode() == 2 ? "#define AMI_STORE(p, v) __stwt(p, v)\n" : "#define AMI_STORE(p, v) (*(p) = (v))\n");
+  // Fused tally (S4, Monte-Carlo sums of PAPER.md:291): the warp adds its samples' (re, im, re^2, im^2) in a fixed
+  // order and lane 0 stores one partial per (row, warp).  The lanes of a ragged last warp are the low ones.
+  o << "__device__ __forceinline__ void ami_tally(double4* dst, const double2 v) {\n"
+       "  const unsigned mask = __activemask();\n"
+       "  const int lane = threadIdx.x & 31, cnt = __popc(mask);\n"
+       "  double a = v.x, b = v.y, c = v.x * v.x, d = v.y * v.y;\n"
+       "#pragma unroll\n"
+       "  for (int off = 16; off > 0; off >>= 1) {\n"
+       "    const double a2 = __shfl_down_sync(mask, a, off), b2 = __shfl_down_sync(mask, b, off);\n"
+       "    const double c2 = __shfl_down_sync(mask, c, off), d2 = __shfl_down_sync(mask, d, off);\n"
+       "    if (lane + off < cnt) { a += a2; b += b2; c += c2; d += d2; }\n"
+       "  }\n"
+       "  if (lane == 0) *dst = make_double4(a, b, c, d);\n"
+       "}\n";
   std::string sig = "(const AmiBatch& p, const long long s";
   for (int i = 0; i < ft.n_eps; ++i) sig += ", const double e" + std::to_string(i);
   if (smem_f && !scratch) {

@@ -567,6 +567,49 @@ __global__ void __launch_bounds__(256) row_final_kernel(const double4* __restric
   }
 }
 
+// Second stage of the fused tally: the per-warp partials [n_rows][stride] (first n of each row used) written by the
+// specialised kernels are summed like values, without squaring: fixed grid, fixed order.
+__global__ void __launch_bounds__(256) row_partial4_kernel(const double4* __restrict__ v, long long n,
+                                                           long long row_stride, double4* __restrict__ partial) {
+  __shared__ double4 sh[256];
+  const long long row = blockIdx.y;
+  const double4* r = v + row * row_stride;
+  const long long per = (n + gridDim.x - 1) / gridDim.x;
+  const long long a = blockIdx.x * per, b = a + per < n ? a + per : n;
+  double4 acc = make_double4(0.0, 0.0, 0.0, 0.0);
+#pragma unroll 4
+  for (long long i = a + threadIdx.x; i < b; i += blockDim.x) {
+    const double4 x = r[i];
+    acc.x += x.x; acc.y += x.y; acc.z += x.z; acc.w += x.w;
+  }
+  sh[threadIdx.x] = acc;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (threadIdx.x < w) {
+      sh[threadIdx.x].x += sh[threadIdx.x + w].x;
+      sh[threadIdx.x].y += sh[threadIdx.x + w].y;
+      sh[threadIdx.x].z += sh[threadIdx.x + w].z;
+      sh[threadIdx.x].w += sh[threadIdx.x + w].w;
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) partial[row * gridDim.x + blockIdx.x] = sh[0];
+}
+
+cudaError_t launch_warp_partial_sums(const double* d_warp_partials, long long n_rows, long long n_warps,
+                                     long long row_stride, double* d_partial, double* d_sum, cudaStream_t st,
+                                     int* launches) {
+  if (n_rows == 0) return cudaSuccess;
+  const int nblk = sum_blocks(n_rows, n_warps);
+  dim3 grid((unsigned)nblk, (unsigned)n_rows);
+  row_partial4_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double4*>(d_warp_partials), n_warps, row_stride,
+                                            reinterpret_cast<double4*>(d_partial));
+  row_final_kernel<<<(unsigned)n_rows, 256, 0, st>>>(reinterpret_cast<const double4*>(d_partial), nblk,
+                                                     reinterpret_cast<double4*>(d_sum));
+  count_launch(launches, 2);
+  return cudaGetLastError();
+}
+
 // d_partial: [n_rows][<= kMaxSumBlocks] double4, d_sum: [n_rows] double4 running tallies
 cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long n, long long row_stride,
                               double* d_partial, double* d_sum, cudaStream_t st, int* launches) {

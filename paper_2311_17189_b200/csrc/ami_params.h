@@ -23,7 +23,10 @@ struct AmiBatch {
   double* scratch;          // memory-backed plan: [slots][scratch_stride] doubles, column s belongs to sample s
   long long scratch_stride;
   double* e_out;            // optional [n_eps][n] copy of the energies formed by the fused path
-  // results: complex128, row r = (b0 + b) * n_f_total + (f0 + f) at out + 2 * r * out_row_stride
+  // fused tally (or NULL): per-warp partial sums (re, im, re^2, im^2) of row r at tally[(r * tally_stride + (s >> 5)) * 4]
+  double* tally;
+  long long tally_stride;
+  // results (out may be NULL when only the tally is wanted): complex128, row r = (b0 + b) * n_f_total + (f0 + f) at out + 2 * r * out_row_stride
   double* out;
   long long n, out_row_stride;
   int n_f, n_b, n_f_total, f0, b0;

@@ -469,6 +469,32 @@ def test_run_streamed_matches_stagewise(ami, torch_mod, oracle_mod, mode):
     check_parity(h_out.numpy()[0][:, sel], truth, S, label="run")
 
 
+@pytest.mark.parametrize("name,n", [("cfg1", 1), ("cfg1", 33), ("cfg3", 5000 + 19), ("cfg2_se", 4096 + 31)])
+def test_run_fused_tally(ami, torch_mod, name, n):
+    """Register plan with a few rows: the evaluation kernel leaves per-warp partial sums and nothing else has to be
+    stored.  Tally-only call == tally beside stored results == numpy sums of those results (ragged last warp,
+    several chunks, several rows); the squares give the error bar.  Deterministic."""
+    cfg = A.get_config(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    nb, nf = len(cfg.betas), len(cfg.z_ext)
+    kw = dict(e_reg=cfg.e_reg, seed=cfg.seed, first_sample=5, chunk=1000, want_sum=True)
+    _, only = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, **kw)
+    sq_only = tab.last_sumsq.copy()
+    d_out = torch_mod.zeros((nb, nf, n), dtype=torch_mod.complex128, device="cuda")
+    _, both = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, d_out=d_out, **kw)
+    assert tab.refresh_info()["reg_plan_status"] == 0
+    assert np.array_equal(only, both) and np.array_equal(sq_only, tab.last_sumsq)
+    v = d_out.cpu().numpy()
+    assert np.all(np.abs(only - v.sum(axis=-1)) <= 1e-12 * np.abs(v).sum(axis=-1))
+    want_sq = np.stack([np.sum(v.real ** 2, axis=-1), np.sum(v.imag ** 2, axis=-1)], axis=-1)
+    assert np.all(np.abs(sq_only - want_sq) <= 1e-12 * want_sq + 1e-300)
+    _, again = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, **kw)
+    assert np.array_equal(only, again)
+    # the table-driven plan (results re-read by the tally kernels) agrees to rounding
+    _, flat = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, plan=ami.PLAN_FLAT, **kw)
+    assert np.all(np.abs(flat - only) <= 1e-9 * np.abs(v).sum(axis=-1))
+
+
 def test_run_device_output_and_determinism(ami, torch_mod):
     cfg = A.get_config("cfg1")
     tab = ami.AmiTable.from_diagram(cfg.diagram)
