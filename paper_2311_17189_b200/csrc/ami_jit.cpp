@@ -551,8 +551,8 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     o << "      const long long row = (long long)(p.b0 + b) * p.n_f_total + (p.f0 + f);\n";
     o << "      const double2 val = make_double2(p.prefactor * (" << acc.re << "), "
       << (acc.real() ? std::string("0.0") : "p.prefactor * (" + acc.im + ")") << ");\n";
-    o << "      if (p.out) AMI_STORE(reinterpret_cast<double2*>(p.out) + row * p.out_row_stride + s, val);\n";
-    o << "      if (p.tally) ami_tally(reinterpret_cast<double4*>(p.tally) + row * p.tally_stride + (s >> 5), val);\n";
+    o << "      if (!AMI_TALLY || p.out) AMI_STORE(reinterpret_cast<double2*>(p.out) + row * p.out_row_stride + s, val);\n";
+    o << "      if (AMI_TALLY) ami_tally(reinterpret_cast<double4*>(p.tally) + row * p.tally_stride + (s >> 5), val);\n";
   }
 #undef o
   std::ostringstream o;
@@ -596,7 +596,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   }
   sig += ") {\n";
   // ---- body for one temperature per launch: beta { frequency { } } ----------------------------
-  o << "__device__ __forceinline__ void ami_body" << sig << sec[0].str()
+  o << "template <bool AMI_TALLY> __device__ __forceinline__ void ami_body" << sig << sec[0].str()
     << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << sec[1].str()
     << "#pragma unroll 1\n    for (int f = 0; f < p.n_f; ++f) {\n" << sec[2].str() << sec[3].str() << "    }\n  }\n}\n\n";
   // ---- body for several temperatures: the per-beta values the R part needs are kept in a small
@@ -606,7 +606,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   for (const std::string& q : qname)
     if (!q.empty() && std::find(keep.begin(), keep.end(), q) == keep.end()) keep.push_back(q);
   if (!scratch) {
-  o << "__device__ __forceinline__ void ami_body_mb" << sig << sec[0].str();
+  o << "template <bool AMI_TALLY> __device__ __forceinline__ void ami_body_mb" << sig << sec[0].str();
   o << "  double kept[AMI_K_MAX_BETA][" << std::max<size_t>(keep.size(), 1) << "];\n";
   o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << sec[1].str();
   for (size_t i = 0; i < keep.size(); ++i) o << "    kept[b][" << i << "] = " << keep[i] << ";\n";
@@ -626,11 +626,14 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   std::string call_args = "(p, s";
   for (int i = 0; i < ft.n_eps; ++i) call_args += ", e" + std::to_string(i);
   call_args += scratch ? ", p.scratch + s, p.scratch_stride);\n" : ");\n";
-  const std::string call = scratch ? "  ami_body" + call_args
-                                   : "  if (p.n_b == 1) ami_body" + call_args + "  else ami_body_mb" + call_args;
+  // @T@ = <false> / <true>: without / with the fused tally (a compile-time switch: the reductions cost the kernels
+  // that do not tally nothing); @K2@ = name of the fused kernel
+  const std::string call = scratch ? "  ami_body@T@" + call_args
+                                   : "  if (p.n_b == 1) ami_body@T@" + call_args + "  else ami_body_mb@T@" + call_args;
   o << call << "  }\n}\n\n";
+  const size_t k2_begin = o.str().size();
   // ---- kernel 2: momenta from memory, dispersion inline (Eqs. 8-18) ----------
-  o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_jit_fused(const __grid_constant__ AmiBatch p) {\n"
+  o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) @K2@(const __grid_constant__ AmiBatch p) {\n"
        "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
        "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
        "  // A CTA walks AMI_U consecutive tiles of AMI_NT samples; the momenta of the next tile are loaded into\n"
@@ -687,7 +690,16 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   o << "  if (p.e_out) {\n";
   for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
   o << "  }\n" << call << "  }\n}\n";
-  return o.str();
+  auto subst = [](std::string t, const std::string& targ, const std::string& k2) {
+    for (const auto& kv : {std::make_pair(std::string("@T@"), targ), std::make_pair(std::string("@K2@"), k2)})
+      for (size_t at = 0; (at = t.find(kv.first, at)) != std::string::npos; at += kv.second.size())
+        t.replace(at, kv.first.size(), kv.second);
+    return t;
+  };
+  const std::string all = o.str();
+  std::string src = subst(all, "<false>", "ami_jit_fused");
+  src += "\n" + subst(all.substr(k2_begin), "<true>", "ami_jit_fused_tally");
+  return src;
 }
 
 int jit_tiles_per_cta() {
@@ -852,7 +864,7 @@ struct JitState {
   int status = AMI_EUNSUPPORTED;
   std::string log;
   CUmodule mod = nullptr;
-  CUfunction fn_eval = nullptr, fn_fused = nullptr;
+  CUfunction fn_eval = nullptr, fn_fused = nullptr, fn_fused_tally = nullptr;
   int mode = kJitNone;
   int block = 0;            // threads per CTA the kernels were generated for
   int tiles = 1;            // tiles of `block` samples one CTA of the fused kernel walks
@@ -929,6 +941,9 @@ int jit_prepare(ami_table* tab, std::string& err) {
   CUresult rc = d.ModuleLoadData(&js.mod, cubin.data());
   if (rc == CUDA_SUCCESS) rc = d.ModuleGetFunction(&js.fn_eval, js.mod, "ami_jit_eval");
   if (rc == CUDA_SUCCESS) rc = d.ModuleGetFunction(&js.fn_fused, js.mod, "ami_jit_fused");
+  if (rc == CUDA_SUCCESS) rc = d.ModuleGetFunction(&js.fn_fused_tally, js.mod, "ami_jit_fused_tally");
+  if (rc == CUDA_SUCCESS && js.fn_fused_tally && js.smem_bytes > 48 * 1024)
+    rc = d.FuncSetAttribute(js.fn_fused_tally, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)js.smem_bytes);
   if (rc == CUDA_SUCCESS && js.smem_bytes > 48 * 1024) {
     rc = d.FuncSetAttribute(js.fn_eval, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)js.smem_bytes);
     if (rc == CUDA_SUCCESS) rc = d.FuncSetAttribute(js.fn_fused, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)js.smem_bytes);
@@ -960,7 +975,8 @@ CUresult launch_one(const JitState* js, bool fused, AmiBatch& batch, cudaStream_
   // the NEXT specialised kernel in the stream may be scheduled while this one drains and starts the
   // moment it has completed (stream order is kept: nothing is read or written before the wait).
   static const bool pdl = [] { const char* e = getenv("AMI_JIT_PDL"); return !(e && e[0] == '0'); }();
-  CUfunction fn = fused ? js->fn_fused : js->fn_eval;
+  CUfunction fn = fused ? (batch.tally ? js->fn_fused_tally : js->fn_fused) : js->fn_eval;
+  if (!fn) return CUDA_ERROR_INVALID_VALUE;
   if (pdl && driver().LaunchKernelEx) {
     CUlaunchAttribute attr;
     memset(&attr, 0, sizeof attr);
@@ -1003,7 +1019,8 @@ cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cuda
     if (part.e_out) part.e_out += c0;
     if (part.k) part.k += c0 * b.k_stride_sample;
     part.first_sample += c0;
-    part.out += 2 * c0;
+    if (part.out) part.out += 2 * c0;
+    if (part.tally) part.tally += 4 * (c0 >> 5);   // chunks are multiples of the block size
     part.scratch = scratch;
     part.scratch_stride = chunk;
     if (launch_one(js, fused, part, st) != CUDA_SUCCESS) { cudaFreeAsync(scratch, st); return cudaErrorLaunchFailure; }
