@@ -184,15 +184,15 @@ __device__ __forceinline__ double cos_bounded(double K) {
 
 // Counter-based momenta (reading P22; specification in ami_inputs/rng.py): splitmix64 finaliser of
 // seed + GOLDEN (ctr + 1), top 53 bits, k = (u - 1/2) 2 pi with one correctly rounded multiply.
-__device__ __forceinline__ double uniform01(unsigned long long seed, unsigned long long ctr) {
-  unsigned long long z = seed + 0x9E3779B97F4A7C15ull * (ctr + 1ull);
+// momentum_from_state takes z = seed + GOLDEN (ctr + 1) so that consecutive counters cost an addition.
+__device__ __forceinline__ double momentum_from_state(unsigned long long z) {
   z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
   z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
   z = z ^ (z >> 31);
-  return (double)(z >> 11) * 0x1.0p-53;
+  return __dmul_rn((double)(z >> 11) * 0x1.0p-53 - 0.5, 6.283185307179586);
 }
 __device__ __forceinline__ double momentum_of(unsigned long long seed, unsigned long long ctr) {
-  return __dmul_rn(uniform01(seed, ctr) - 0.5, 6.283185307179586);
+  return momentum_from_state(seed + 0x9E3779B97F4A7C15ull * (ctr + 1ull));
 }
 
 // f_sigma(E) = 1/(sigma e^x + 1) and g = 1 - f = sigma e^x f for x = beta E, any real x, without

@@ -654,9 +654,15 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   // momenta of sample `at`: from memory, or drawn in place by the counter-based generator (S4 with a seed:
   // the momenta never exist in memory)
   auto emit_momenta = [&](const std::string& at, const std::string& ind) {
-    o << ind << "if (p.gen) {\n" << ind << "  const unsigned long long c0 = (unsigned long long)(p.first_sample + (" << at
-      << ")) * " << 2 * ft.n_int << "ull;\n";
-    for (int c = 0; c < 2 * ft.n_int; ++c) o << ind << "  nk" << c << " = momentum_of(p.seed, c0 + " << c << "ull);\n";
+    // counter of component c = sample * 2m + c; the generator's state is seed + GOLDEN (counter + 1), so one 64-bit
+    // multiply per sample and an addition per component (arithmetic modulo 2^64: same bits as momentum_of)
+    o << ind << "if (p.gen) {\n" << ind << "  const unsigned long long z0 = p.seed + 0x9E3779B97F4A7C15ull * ((unsigned long long)"
+      << "(p.first_sample + (" << at << ")) * " << 2 * ft.n_int << "ull + 1ull);\n";
+    for (int c = 0; c < 2 * ft.n_int; ++c) {
+      char lit[32];
+      snprintf(lit, sizeof lit, "0x%016llXull", (unsigned long long)(0x9E3779B97F4A7C15ull * (unsigned long long)c));
+      o << ind << "  nk" << c << " = momentum_from_state(z0 + " << lit << ");\n";
+    }
     o << ind << "} else {\n" << ind << "  const double* kn = p.k + (" << at << ") * p.k_stride_sample;\n";
     for (int c = 0; c < 2 * ft.n_int; ++c) o << ind << "  nk" << c << " = kn[" << c << " * p.k_stride_comp];\n";
     o << ind << "}\n";
