@@ -748,14 +748,19 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
                        fused_tally ? (size_t)rows * wp_stride * 32 : 0)))
     return rc;
   if (cfg->want_sum) CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 32, user));
+  // one chunk: everything on the caller's stream (the hops to the internal streams and back cost more than a small
+  // batch's kernels); several chunks: they alternate between the two internal streams
+  const bool single = cfg->n <= chunk;
   CU(cudaEventRecord(rb.ev_start, user));
-  CU(cudaStreamWaitEvent(rb.st[0], rb.ev_start, 0));
-  CU(cudaStreamWaitEvent(rb.st[1], rb.ev_start, 0));
+  if (!single) {
+    CU(cudaStreamWaitEvent(rb.st[0], rb.ev_start, 0));
+    CU(cudaStreamWaitEvent(rb.st[1], rb.ev_start, 0));
+  }
   int launches = 0;
   for (int64_t c0 = 0, ci = 0; c0 < cfg->n; c0 += chunk, ++ci) {
     const int s = (int)(ci & 1);
     const int64_t nc = std::min(chunk, cfg->n - c0);
-    cudaStream_t st = rb.st[s];
+    cudaStream_t st = single ? user : rb.st[s];
     const double* kbuf;
     if (cfg->d_k) {
       kbuf = cfg->d_k + c0 * n_comp;
@@ -793,10 +798,10 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
       else
         CU(ami::launch_block_sums(obuf, rows, nc, ostride, rb.partial, rb.sum, st, &launches));
     }
-    CU(cudaEventRecord(rb.ev_done[s], st));
+    if (!single) CU(cudaEventRecord(rb.ev_done[s], st));
     ++local.n_chunks;
   }
-  for (int i = 0; i < 2; ++i) {
+  for (int i = 0; i < 2 && !single; ++i) {
     CU(cudaEventRecord(rb.ev_done[i], rb.st[i]));
     CU(cudaStreamWaitEvent(user, rb.ev_done[i], 0));
   }
