@@ -50,6 +50,7 @@ def lib():
         L.oracle_describe.argtypes = [C.c_void_p, C.c_char_p, C.c_long]
         L.oracle_evaluate.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_long, C.c_void_p, C.c_int,
                                       C.c_double, C.c_double, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.oracle_evaluate_ex.argtypes = L.oracle_evaluate.argtypes + [C.c_void_p, C.c_void_p]
         L.oracle_dispersion.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
                                         C.c_long, C.c_int, C.c_int, C.c_void_p]
         L.oracle_dispersion_lattice.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
@@ -108,10 +109,11 @@ class OracleTable:
         lib().oracle_describe(self._h, buf, n)
         return buf.value.decode()
 
-    def evaluate(self, e, z_ext, beta, e_reg=0.0, quad=False, threads=1, want_S=False):
+    def evaluate(self, e, z_ext, beta, e_reg=0.0, quad=False, threads=1, want_S=False, want_logs=False):
         """e: [n_e][n_eps] float64 or complex128 (paper's energy_t, PAPER.md:110);
         z_ext: complex [n_f][n_ext].  Returns complex128 [n_f][n_e] and,
-        if want_S, S = sum_t |term_t| with the same shape."""
+        if want_S, S = sum_t |term_t| with the same shape; if want_logs also log2 S and log2 |value|
+        taken before the cast to double (they survive where S itself underflows a double)."""
         e = np.ascontiguousarray(e)
         is_c = np.iscomplexobj(e)
         e = e.astype(np.complex128 if is_c else np.float64)
@@ -120,11 +122,16 @@ class OracleTable:
         n_e, n_f = e.shape[0], z.shape[0]
         out = np.zeros((n_f, n_e), dtype=np.complex128)
         S = np.zeros((n_f, n_e), dtype=np.float64)
-        rc = lib().oracle_evaluate(self._h, e.ctypes.data, int(is_c), n_e, z.ctypes.data, n_f, float(beta),
-                                   float(e_reg), 1 if quad else 0, int(threads), out.ctypes.data,
-                                   S.ctypes.data)
+        l2S = np.zeros((n_f, n_e)) if want_logs else None
+        l2v = np.zeros((n_f, n_e)) if want_logs else None
+        rc = lib().oracle_evaluate_ex(self._h, e.ctypes.data, int(is_c), n_e, z.ctypes.data, n_f, float(beta),
+                                      float(e_reg), 1 if quad else 0, int(threads), out.ctypes.data,
+                                      S.ctypes.data, None if l2S is None else l2S.ctypes.data,
+                                      None if l2v is None else l2v.ctypes.data)
         if rc:
             raise OracleError(rc)
+        if want_logs:
+            return out, S, l2S, l2v
         return (out, S) if want_S else out
 
     def dispersion(self, k, q, t, mu, quad=False, threads=1, dim=2, band=0):

@@ -198,6 +198,8 @@ inline double t_expm1(double x) { return std::expm1(x); }
 inline double t_sin(double x) { return std::sin(x); }
 inline double t_cos(double x) { return std::cos(x); }
 inline double t_sqrt(double x) { return std::sqrt(x); }
+inline double t_log2(double x) { return std::log2(x); }
+inline __float128 t_log2(__float128 x) { return log2q(x); }
 inline __float128 t_exp(__float128 x) { return expq(x); }
 inline __float128 t_expm1(__float128 x) { return expm1q(x); }
 inline __float128 t_sin(__float128 x) { return sinq(x); }
@@ -320,7 +322,8 @@ void eval_one(const Table& tb, const Cx<T>* e, const Cx<T>* zext, const char* ze
 
 template <class T>
 void eval_range(const Table& tb, const double* e, int e_is_complex, long s0, long s1, long n_e,
-                const double* z_ext, int n_f, double beta, double e_reg, double* out, double* S_out) {
+                const double* z_ext, int n_f, double beta, double e_reg, double* out, double* S_out,
+                double* log2S_out, double* log2abs_out) {
   std::vector<Cx<T>> E(tb.n_eps), Z(tb.n_ext);
   std::vector<char> zz(tb.n_ext);
   for (long s = s0; s < s1; ++s) {
@@ -339,6 +342,9 @@ void eval_range(const Table& tb, const double* e, int e_is_complex, long s0, lon
       out[2 * ((long)f * n_e + s)] = (double)v.re;
       out[2 * ((long)f * n_e + s) + 1] = (double)v.im;
       if (S_out) S_out[(long)f * n_e + s] = (double)S;
+      // base-2 logarithms taken in T before the cast: they survive where S and |value| underflow a double
+      if (log2S_out) log2S_out[(long)f * n_e + s] = (double)t_log2(S);
+      if (log2abs_out) log2abs_out[(long)f * n_e + s] = (double)t_log2(cabs_(v));
     }
   }
 }
@@ -483,17 +489,28 @@ long oracle_describe(void* h, char* buf, long cap) {
 // e: [n_e][n_eps] (paper's energy_t; complex interleaved if e_is_complex);
 // z_ext: [n_f][n_ext] complex interleaved; out: [n_f][n_e] complex interleaved;
 // S_out: [n_f][n_e] = sum over terms of |term| (may be NULL).  precision 0 = double, 1 = quad.
-int oracle_evaluate(void* h, const double* e, int e_is_complex, long n_e, const double* z_ext, int n_f,
-                    double beta, double e_reg, int precision, int n_threads, double* out, double* S_out) {
+// log2S_out / log2abs_out (may be NULL): log2 S and log2 |value|, taken in the working precision
+// before the cast to double, so that the scale of a sample whose terms all underflow a double
+// (beta |E| of several hundred) is still known to the parity norm (-inf for an exact zero).
+int oracle_evaluate_ex(void* h, const double* e, int e_is_complex, long n_e, const double* z_ext, int n_f,
+                       double beta, double e_reg, int precision, int n_threads, double* out, double* S_out,
+                       double* log2S_out, double* log2abs_out) {
   Table* tb = (Table*)h;
   if (!tb || n_e < 0 || n_f < 0) return OR_EINVAL;
   parallel_for(n_e, n_threads, [=](long a, long b) {
     if (precision == 0)
-      eval_range<double>(*tb, e, e_is_complex, a, b, n_e, z_ext, n_f, beta, e_reg, out, S_out);
+      eval_range<double>(*tb, e, e_is_complex, a, b, n_e, z_ext, n_f, beta, e_reg, out, S_out, log2S_out, log2abs_out);
     else
-      eval_range<__float128>(*tb, e, e_is_complex, a, b, n_e, z_ext, n_f, beta, e_reg, out, S_out);
+      eval_range<__float128>(*tb, e, e_is_complex, a, b, n_e, z_ext, n_f, beta, e_reg, out, S_out, log2S_out,
+                             log2abs_out);
   });
   return OR_OK;
+}
+
+int oracle_evaluate(void* h, const double* e, int e_is_complex, long n_e, const double* z_ext, int n_f,
+                    double beta, double e_reg, int precision, int n_threads, double* out, double* S_out) {
+  return oracle_evaluate_ex(h, e, e_is_complex, n_e, z_ext, n_f, beta, e_reg, precision, n_threads, out, S_out,
+                            nullptr, nullptr);
 }
 
 // k: [n_e][n_int][dim] (Eq. 8), q: [n_ext][dim]; e_out: [n_e][n_eps]

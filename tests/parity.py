@@ -2,20 +2,35 @@
 
 Literal "1e-10 relative per sample" is not attainable in double for samples whose terms cancel
 (kappa = S/|value| up to 1e18), whichever implementation computes them, so the bar is:
-  (1) every sample:        |gpu - truth| <= 1e-10 * S,  S = sum_t |term_t| from the quad oracle
+  (1) every sample:        |gpu - truth| <= 1e-10 * S + FLOOR,  S = sum_t |term_t| from the quad oracle
                            (for kappa ~ 1 this IS the plain relative error);
-  (2) kappa <= 1e3 subset: |gpu - truth| / |truth| <= 1e-10;
+  (2) kappa <= 1e3 subset: |gpu - truth| <= 1e-10 * |truth| + FLOOR;
   (3) batch mean:          |mean_gpu - mean_truth| <= 1e-10 * mean(S)  and, when the mean itself is
                            well conditioned (mean(S)/|mean| <= 1e3), plain relative <= 1e-10;
-  (4) non-finite truth values must be non-finite on the GPU too;
-  (5) where S < 1e-290 (deep underflow) the GPU value must be < 1e-280 in magnitude.
+  (4) non-finite truth values must be non-finite on the GPU too.
+FLOOR = 1e-300 is an absolute allowance for the output format, applied to EVERY sample alike: the
+result is complex128 (BASELINE.json: "complex128 output per sample"), whose normal range ends at
+2.2e-308, so a value or a bound below that cannot be stated in the result's own format.  It only
+matters where every term underflows (beta |E| of several hundred); there the truth (1e-400, say)
+reads 0 as a double and the GPU value must be below 1e-300 in magnitude -- nothing is exempted.
+kappa is formed from log2 S and log2 |truth| taken in quad precision before the cast to double
+(oracle `want_logs`), so samples whose S underflows a double are still classified.
+`min_wellcond`: floor on the share of kappa <= 1e3 samples.  S is the denominator of rule (1); an
+inflated S would show up as a collapse of that share (S itself is pinned in tests/test_oracle_pins.py).
 """
 import numpy as np
 
 TOL = 1e-10
+FLOOR = 1e-300
+
+# share of samples with kappa <= 1e3 measured with the quad oracle at the configurations' own parameters
+# (cfg1 0.82; cfg2 over its (mu, beta) points 0.73-0.97 / 0.85-0.99 / 0.87-0.99; cfg3 0.45; cfg4 0.28; cfg5 0.41-0.63
+# over its four temperatures), less a margin for small batches
+WELLCOND_FLOOR = {"cfg1": 0.72, "cfg2_se": 0.65, "cfg2_bubble": 0.75, "cfg2_bubble_doubled": 0.78, "cfg3": 0.38,
+                  "cfg4": 0.20, "cfg5": 0.33}
 
 
-def check_parity(gpu, truth, S, tol=TOL, label=""):
+def check_parity(gpu, truth, S, tol=TOL, label="", log2S=None, log2abs=None, min_wellcond=None):
     gpu, truth, S = np.asarray(gpu), np.asarray(truth), np.asarray(S)
     assert gpu.shape == truth.shape == S.shape, (gpu.shape, truth.shape, S.shape)
     fin = np.isfinite(truth.real) & np.isfinite(truth.imag) & np.isfinite(S)
@@ -24,25 +39,34 @@ def check_parity(gpu, truth, S, tol=TOL, label=""):
     assert bad_gpu[~fin].all(), f"{label}: oracle non-finite but GPU finite"
     g, t, s = gpu[fin], truth[fin], S[fin]
     err = np.abs(g - t)
-    # S below 1e-290 (deep underflow at very low temperature: the oracle's quad values do not survive the
-    # cast to double): nothing relative can be said there; the GPU must be just as negligible
-    tiny = s < 1e-290
+    excess = np.maximum(err - FLOOR, 0.0)            # rule (1): err <= tol * S + FLOOR
     with np.errstate(divide="ignore", invalid="ignore"):
-        ratio = np.where(tiny, np.where(err <= 1e-280, 0.0, np.inf), err / np.where(tiny, 1.0, s))
+        ratio = np.where(excess > 0.0, excess / s, 0.0)
     worst_S = float(np.max(ratio)) if err.size else 0.0
     assert worst_S <= tol, f"{label}: worst S-relative error {worst_S:.3e}"
-    kappa = np.where(tiny, 1.0, s / np.maximum(np.abs(t), 1e-300))
-    well = (kappa <= 1e3) & ~tiny
-    worst_rel = float(np.max(err[well] / np.abs(t[well]))) if well.any() else 0.0
+    if log2S is not None and log2abs is not None:
+        with np.errstate(invalid="ignore", over="ignore"):
+            kappa = np.exp2(np.clip(np.asarray(log2S)[fin] - np.asarray(log2abs)[fin], -1000.0, 1000.0))
+        kappa = np.where(np.isnan(kappa), 1.0, kappa)          # exact zeros on both sides
+    else:
+        kappa = s / np.maximum(np.abs(t), 1e-300)
+    well = kappa <= 1e3
+    rel_excess = np.maximum(err[well] - FLOOR, 0.0)             # rule (2): err <= tol * |t| + FLOOR
+    with np.errstate(divide="ignore", invalid="ignore"):
+        rel = np.where(rel_excess > 0.0, rel_excess / np.abs(t[well]), 0.0)
+    worst_rel = float(np.max(rel)) if well.any() else 0.0
     assert worst_rel <= tol, f"{label}: worst relative error on kappa<=1e3: {worst_rel:.3e}"
     stats = {"n": int(err.size), "worst_S_rel": worst_S, "worst_rel_wellcond": worst_rel,
              "frac_wellcond": float(well.mean()) if err.size else 1.0,
              "kappa_median": float(np.median(kappa)) if err.size else 1.0,
              "kappa_max": float(kappa.max()) if err.size else 1.0, "n_nonfinite": int((~fin).sum())}
+    if min_wellcond is not None and err.size:
+        assert stats["frac_wellcond"] >= min_wellcond, \
+            f"{label}: only {stats['frac_wellcond']:.2f} of the samples have kappa <= 1e3 (floor {min_wellcond})"
     if err.size:
         dm = abs(g.mean() - t.mean())
-        assert dm <= tol * s.mean(), f"{label}: batch mean off by {dm / s.mean():.3e} of mean(S)"
+        assert dm <= tol * s.mean() + FLOOR, f"{label}: batch mean off by {dm / s.mean():.3e} of mean(S)"
         if s.mean() <= 1e3 * abs(t.mean()):
-            assert dm <= tol * abs(t.mean()), f"{label}: batch mean relative error {dm / abs(t.mean()):.3e}"
+            assert dm <= tol * abs(t.mean()) + FLOOR, f"{label}: batch mean relative error {dm / abs(t.mean()):.3e}"
         stats["mean_rel"] = float(dm / max(abs(t.mean()), 1e-300))
     return stats

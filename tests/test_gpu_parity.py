@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 import ami_inputs as A
-from parity import check_parity
+from parity import WELLCOND_FLOOR, check_parity
 
 pytestmark = pytest.mark.gpu
 
@@ -35,9 +35,10 @@ def gpu_energies(torch, tab, cfg, k_host):
     return tab.dispersion(k, [cfg.q], cfg.t, cfg.mu)
 
 
-def truth_for(oracle_mod, cfg, e_rows, z, beta, e_reg, quad=True, sum_order=None):
+def truth_for(oracle_mod, cfg, e_rows, z, beta, e_reg, quad=True, sum_order=None, want_logs=False):
     ot = oracle_mod.OracleTable.from_diagram(cfg.diagram, sum_order=sum_order)
-    return ot.evaluate(e_rows, z, beta, e_reg=e_reg, quad=quad, threads=oracle_mod.hardware_threads(), want_S=True)
+    return ot.evaluate(e_rows, z, beta, e_reg=e_reg, quad=quad, threads=oracle_mod.hardware_threads(), want_S=True,
+                       want_logs=want_logs)
 
 
 # ------------------------------------------------------------------ S1 dispersion
@@ -117,6 +118,8 @@ def run_eval_case(ami, torch, oracle_mod, cfg, n, plan, betas=None, z=None, n_tr
     tab = ami.AmiTable.from_diagram(cfg.diagram, sum_order=sum_order)
     k = cfg.momenta(n, start=start)
     e_dev = gpu_energies(torch, tab, cfg, k)
+    # at the configuration's own temperatures and frequencies the share of well-conditioned samples is known
+    floor = WELLCOND_FLOOR.get(cfg.name) if betas is None and z is None else None
     betas = cfg.betas if betas is None else betas
     z = cfg.z_ext if z is None else z
     out = tab.evaluate(e_dev, z, betas, e_reg=cfg.e_reg, plan=plan).cpu().numpy()
@@ -125,8 +128,10 @@ def run_eval_case(ami, torch, oracle_mod, cfg, n, plan, betas=None, z=None, n_tr
     sel = np.arange(n) if n_truth is None or n_truth >= n else np.linspace(0, n - 1, n_truth).astype(np.int64)
     stats = []
     for b, beta in enumerate(betas):
-        truth, S = truth_for(oracle_mod, cfg, e_rows[sel], z, beta, cfg.e_reg, sum_order=sum_order)
-        stats.append(check_parity(out[b][:, sel], truth, S, label=f"{cfg.name} beta={beta}"))
+        truth, S, l2S, l2v = truth_for(oracle_mod, cfg, e_rows[sel], z, beta, cfg.e_reg, sum_order=sum_order,
+                                       want_logs=True)
+        stats.append(check_parity(out[b][:, sel], truth, S, label=f"{cfg.name} beta={beta}", log2S=l2S, log2abs=l2v,
+                                  min_wellcond=floor if len(sel) >= 500 else None))
     return stats
 
 

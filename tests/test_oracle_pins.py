@@ -170,6 +170,116 @@ def test_bose_limits(oracle_mod):
     assert abs(oracle_mod.fermi(-50.0, beta, -1, 0).real - 1.0) < 1e-15
 
 
+# ---------------------------------------------------------------- complex arguments (reading P19)
+def mp_fermi(E, beta, sigma, k=0):
+    """f_sigma^{(k)}(E) = d^k/dE^k 1/(sigma e^{beta E} + 1) at 40 digits (mpmath), for complex E; the
+    derivatives by mpmath's own numerical differentiation of that definition -- independent of the oracle."""
+    import mpmath as mp
+    mp.mp.dps = 40
+    f = lambda x: 1 / (sigma * mp.exp(beta * x) + 1)
+    v = f(mp.mpc(E)) if k == 0 else mp.diff(f, mp.mpc(E), k)
+    return complex(v)
+
+
+@pytest.mark.parametrize("sigma", [1, -1])
+@pytest.mark.parametrize("k", [0, 1, 2])
+def test_fermi_complex_argument(oracle_mod, sigma, k):
+    """The complex-argument branch of the oracle's Fermi/Bose function (energy_t is complex128,
+    PAPER.md:253-255) against the definition 1/(sigma e^{beta E} + 1) evaluated with mpmath: both
+    signs of Re E and Im E, moderate arguments, both tails (Re beta E = -+60, -+700: the branch that
+    exponentiates the argument with Re <= 0) and, for sigma = -1, the neighbourhood of the pole
+    (expm1 branch).  f(conj E) = conj f(E), so a sign slip in the imaginary part of the complex
+    exponential fails the imaginary part here."""
+    beta = 2.5
+    pts = [0.8 - 0.21j, 0.8 + 0.21j, -0.8 - 0.21j, -0.8 + 0.21j, 0.05 + 1.1j, -0.05 - 1.1j, 3.0 + 0.7j, -3.0 - 0.7j,
+           24.0 + 0.3j, -24.0 - 0.3j, 280.0 - 0.4j, -280.0 + 0.4j, 1e-4 + 2e-4j, -1e-4 + 2e-4j, 2e-7 - 1e-7j]
+    for E in pts:
+        want = mp_fermi(E, beta, sigma, k)
+        fg = abs(mp_fermi(E, beta, sigma, 1)) / beta      # |f g|: the scale of the factors of every derivative
+        for quad in (True, False):
+            got = oracle_mod.fermi(E, beta, sigma, k, quad=quad)
+            tol = 1e-13 if quad else 1e-11      # double: beta*E itself is rounded; |f^(k)| ~ 1/|beta E|^(k+1) near the pole
+            # f'' = beta^2 f g (g - f) has a genuine zero at E = 0 (sigma = +1): in double, rounding on the
+            # scale of its own factors, as in test_fermi_double_vs_quad
+            slack = 0.0 if quad else 1e-15 * beta ** k * fg
+            assert abs(got - want) <= tol * abs(want) + slack + 1e-300, (E, sigma, k, quad, got, want)
+        if abs(want.imag) > 1e-290:
+            assert np.sign(got.imag) == np.sign(want.imag), (E, sigma, k)
+
+
+def test_fermi_complex_closed_forms_numpy(oracle_mod):
+    """Same branch against plain numpy complex arithmetic at moderate |beta E| (no mpmath):
+    f = 1/(sigma e^x + 1), f' = -beta sigma e^x/(sigma e^x + 1)^2."""
+    beta = 1.7
+    for sigma in (1, -1):
+        for E in (0.31 + 0.52j, 0.31 - 0.52j, -1.4 + 0.9j, -1.4 - 0.9j, 2.2 + 3.0j):
+            x = np.exp(beta * E)
+            assert abs(oracle_mod.fermi(E, beta, sigma, 0) - 1 / (sigma * x + 1)) < 2e-15
+            assert abs(oracle_mod.fermi(E, beta, sigma, 1) - (-beta * sigma * x / (sigma * x + 1) ** 2)) < 1e-14
+
+
+@pytest.mark.parametrize("beta,n", [(2.0, 1), (5.0, 3)])
+def test_bubble_closed_form_complex_energies(oracle_mod, beta, n):
+    """A whole diagram with complex energies (variant 5b): the bubble closed form
+    (f(a) - f(b))/(i Omega + a - b), a = -e1, b = -e2 complex, f from mpmath."""
+    t = table(oracle_mod, A.bubble())
+    e = RNG.uniform(-3, 3, size=(40, 2)) + 1j * RNG.uniform(-0.4, 0.4, size=(40, 2))
+    Om = 2 * math.pi * n / beta
+    a, b = -e[:, 0], -e[:, 1]
+    fa = np.array([mp_fermi(x, beta, 1) for x in a])
+    fb = np.array([mp_fermi(x, beta, 1) for x in b])
+    den = 1j * Om + a - b
+    want = (fa - fb) / den
+    S_want = (np.abs(fa) + np.abs(fb)) / np.abs(den)
+    for quad, tol in ((True, 1e-14), (False, 1e-13)):
+        got, S = t.evaluate(e, [[1j * Om]], beta, quad=quad, want_S=True)
+        assert np.max(np.abs(got[0] - want) / S_want) <= tol
+        np.testing.assert_allclose(S[0], S_want, rtol=1e-13)
+    # the conjugate energies give the mirrored result: I(conj e, -Omega) = conj I(e, Omega)
+    got_c = t.evaluate(np.conj(e), [[-1j * Om]], beta, quad=True)
+    np.testing.assert_allclose(got_c[0], np.conj(want), rtol=0, atol=1e-13 * S_want.max())
+
+
+# ---------------------------------------------------------------- S = sum_t |term_t|, the scale of the parity norm (P20)
+def test_S_closed_forms(oracle_mod):
+    """S is the denominator of the parity norm (tests/parity.py), so it is pinned like a value:
+    order 1: S = |f(-e1)|;  bubble: S = (|f(a)| + |f(b)|)/|i Om + a - b|;  doubled bubble (3 terms):
+    S = beta f_a (1-f_a)/|den| + (f_a + f_b)/|den|^2.  Prefactor A scales it by |A|."""
+    beta = 3.0
+    e1 = RNG.uniform(-3, 3, size=(30, 1))
+    _, S = table(oracle_mod, A.order1_line()).evaluate(e1, [[1j * math.pi / beta]], beta, quad=True, want_S=True)
+    np.testing.assert_allclose(S[0], fermi(-e1[:, 0], beta), rtol=1e-14)
+    e = RNG.uniform(-3, 3, size=(60, 2))
+    Om = 2 * math.pi * 2 / beta
+    a, b = -e[:, 0], -e[:, 1]
+    fa, fb = fermi(a, beta), fermi(b, beta)
+    den = np.abs(1j * Om + a - b)
+    for quad in (True, False):
+        _, S = table(oracle_mod, A.bubble()).evaluate(e, [[1j * Om]], beta, quad=quad, want_S=True)
+        np.testing.assert_allclose(S[0], (fa + fb) / den, rtol=1e-13)
+        _, S = table(oracle_mod, A.doubled_line_bubble()).evaluate(e, [[1j * Om]], beta, quad=quad, want_S=True)
+        np.testing.assert_allclose(S[0], beta * fa * (1 - fa) / den + (fa + fb) / den ** 2, rtol=1e-12)
+    _, S = table(oracle_mod, A.bubble(), prefactor=-2.5).evaluate(e, [[1j * Om]], beta, quad=True, want_S=True)
+    np.testing.assert_allclose(S[0], 2.5 * (fa + fb) / den, rtol=1e-13)
+    # S >= |value| always, and S = |value| when there is a single term
+    v, S = table(oracle_mod, A.self_energy_order2()).evaluate(RNG.uniform(-3, 3, size=(50, 3)), [[1j * math.pi / beta]],
+                                                               beta, quad=True, want_S=True)
+    assert (S[0] >= np.abs(v[0]) * (1 - 1e-15)).all()
+
+
+def test_log2_scale_survives_underflow(oracle_mod):
+    """log2 S and log2 |value| are taken in quad precision before the cast to double: for one line at
+    beta e1 = -1000 the value e^{-1000}/(1 + e^{-1000}) is 0 as a double but its logarithm is exact;
+    for ordinary samples they agree with log2 of the double outputs."""
+    t = table(oracle_mod, A.order1_line())
+    beta = 10.0
+    v, S, l2S, l2v = t.evaluate(np.array([[-100.0], [0.3], [-2.0]]), [[1j * math.pi / beta]], beta, quad=True, want_logs=True)
+    assert v[0, 0] == 0 and S[0, 0] == 0
+    assert abs(l2S[0, 0] - (-1000.0 / math.log(2))) < 1e-9 and l2S[0, 0] == l2v[0, 0]
+    np.testing.assert_allclose(l2S[0, 1:], np.log2(S[0, 1:]), rtol=0, atol=1e-12)
+    np.testing.assert_allclose(l2v[0, 1:], np.log2(np.abs(v[0, 1:])), rtol=0, atol=1e-12)
+
+
 # ---------------------------------------------------------------- brute-force Eq. 1
 def brute_force(d, e, z_ext, beta, N):
     """beta^-n sum over |n_l| < N (n_l = -N..N-1, symmetric in nu) of prod_j 1/(X^j + E^j),
