@@ -231,7 +231,9 @@ def run_reference(args, dist, rank, world):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "samples_per_s": tot_units / tot_dt,
-        "config": {"workload": cfg.name, "T_flat": T, "sample": sample, "precision": "double"},
+        "config": {"workload": cfg.name, "samples_per_gpu": cfg.n_samples, "n_freq": len(cfg.z_ext),
+                   "n_beta": len(cfg.betas), "T_flat": T, "precision": "double"},
+        "config_detail": {"sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -249,14 +251,14 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
     sum_order = None
     if SUM_ORDER != "default":     # experiment knob; term-evals/s then counts the terms of THAT table
         sum_order = pkg.search_sum_order(cfg.diagram, 0 if SUM_ORDER == "fewest_terms" else 1)[0]
+    t_c0 = time.perf_counter()
     tab = pkg.AmiTable.from_diagram(cfg.diagram, device=torch.cuda.current_device(), sum_order=sum_order)
+    construct_ms = (time.perf_counter() - t_c0) * 1e3      # ami_construct: recursion + plans + device copy
     info = tab.info
     m, n_eps = cfg.diagram.n_int, cfg.diagram.n_eps
     n_f, n_b = len(cfg.z_ext), len(cfg.betas)
     bytes_in = n * 2 * m * 8
     n_rot = int(max(2, min(8, -(-300_000_000 // max(bytes_in + n * n_eps * 8, 1)))))
-    if os.environ.get("AMI_BENCH_NROT"):      # experiment knob: 1 = every step re-reads the same (L2-resident) batch
-        n_rot = int(os.environ["AMI_BENCH_NROT"])
     ks = [tab.generate_momenta(cfg.seed, first_sample + r * n, n) for r in range(n_rot)]
     es = [torch.empty((n_eps, n), dtype=torch.float64, device="cuda") for _ in range(n_rot)] \
         if not (plan in (0, 2) and info["reg_plan_status"] in (0, 1)) else []
@@ -266,7 +268,7 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
 
     reg = plan in (0, 2) and info["reg_plan_status"] in (0, 1)
     if reg:
-        info = tab.specialize()        # NVRTC compile + load happen here, outside every timed region
+        info = tab.specialize()        # NVRTC compile (or cache fetch) + load happen here, outside every timed region
 
     def step(i, events=None):
         r = i % n_rot
@@ -345,7 +347,7 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
             two_stream_ms = time_two_streams(torch, tab, cfg, ks, steps, plan)
         except Exception as exc:  # noqa: BLE001  (extra figure only; the headline never depends on it)
             two_stream_ms = f"unavailable: {exc}"
-    return {"tab": tab, "info": info, "fused": reg, "tree": plan == 3, "total_ms": total_ms, "disp_ms": disp_ms, "eval_ms": eval_ms,
+    return {"tab": tab, "info": info, "construct_ms": construct_ms, "fused": reg, "tree": plan == 3, "total_ms": total_ms, "disp_ms": disp_ms, "eval_ms": eval_ms,
             "launches": launches, "clocks": clocks, "graph": graph is not None, "two_stream_ms": two_stream_ms, "n_rot": n_rot, "checksum": checksum,
             "bytes_in": bytes_in, "bytes_e": n * n_eps * 8, "bytes_out": n * n_f * n_b * 16}
 
@@ -404,6 +406,24 @@ def time_e2e(pkg, torch, tab, cfg, n, steps, warmup, plan, first_sample, dist):
             "finite": bool(torch.isfinite(torch.view_as_real(h_out[0, 0, :1024])).all().item())}
 
 
+def time_e2e_seeded(torch, tab, cfg, n, steps, plan, T):
+    """The end-to-end metric in the driver's seeded mode: no host-to-device copy at all (the momenta are drawn inside
+    the evaluation kernel), every result copied to pinned host memory; the floor is the device-to-host copy."""
+    n_f, n_b = len(cfg.z_ext), len(cfg.betas)
+    h_out = torch.empty((n_b, n_f, n), dtype=torch.complex128).pin_memory()
+    stats, _ = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan, seed=cfg.seed, h_out=h_out)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(steps):
+        stats, _ = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan, seed=cfg.seed,
+                           first_sample=(i + 1) * n, h_out=h_out)
+    torch.cuda.synchronize()
+    dt = (time.perf_counter() - t0) / steps
+    return {"value": T * n * n_f * n_b / dt, "unit": UNIT, "ms_per_step": dt * 1e3, "h2d_bytes_per_step": int(stats["h2d_bytes"]),
+            "d2h_bytes_per_step": int(stats["d2h_bytes"]), "chunks_per_step": int(stats["n_chunks"]),
+            "api": "ami_run(seed -> h_out)"}
+
+
 def time_monte_carlo(torch, tab, cfg, n, steps, plan):
     """S4 in the mode of the paper's Monte-Carlo momentum integration: ami_run generates the
     momenta on the device from the seed, evaluates them chunk by chunk on two streams and returns only the
@@ -425,7 +445,10 @@ def time_monte_carlo(torch, tab, cfg, n, steps, plan):
             "mean_re_first_row": float(mean[0, 0].real), "stderr_re_first_row": float(err[0, 0])}
 
 
-def roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s):
+NOMINAL_DFMA_PER_S = 148 * 64 * 1.965e9      # 148 SMs x 64 FP64 lanes x max SM clock
+
+
+def roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s, dfma3_per_s=None):
     """Roofline of the dominant kernel: FP64-pipe bound.  Work counted in FP64-pipe instruction slots
     per sample, expressed as DFMA-equivalent TFLOP/s (slot = 2 flop) against the DFMA-chain
     rate measured in this run; the HBM leg is reported beside it.  With the register plan the step is
@@ -436,7 +459,8 @@ def roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s):
     if res["fused"]:
         slots = w["evaluate"] + w["dispersion"]
         bytes_alg = res["bytes_in"] + res["bytes_out"]
-        kernel = "ami_jit_fused (S1+S2+S3)"
+        kernel = "ami_jit_fused (S1+S2+S3)" if int(res["info"].get("plan_kind", 1)) != 2 else \
+            "split plan: ami_split_leaves_fused + ami_split_parts + ami_split_combine (S1+S2+S3)"
     else:
         slots = w["evaluate"]
         bytes_alg = res["bytes_e"] + res["bytes_out"]
@@ -444,9 +468,13 @@ def roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s):
     ach = 2.0 * slots * n / t_eval / 1e12
     roof = {"bound": "alu", "kernel": kernel, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
             "frac": ach / peak_tf, "traffic": None,
-            "peak_source": "DFMA-chain probe run by this bench (FP64 pipe; MEASURED_PEAKS.json has no FP64 figure)",
+            "peak_source": "DFMA-chain probe run by this bench, two distinct register sources per DFMA: the FP64 "
+                           "pipe's issue rate (MEASURED_PEAKS.json has no FP64 figure)",
             "flop_convention": "FP64-pipe instruction slots x 2",
-            "peak_nominal": 2.0 * 148 * 64 * 1.965e9 / 1e12,     # 148 SMs x 64 FP64 lanes x max SM clock (context only)
+            "peak_nominal": 2.0 * NOMINAL_DFMA_PER_S / 1e12,     # 148 SMs x 64 FP64 lanes x max SM clock
+            "frac_of_nominal": ach / (2.0 * NOMINAL_DFMA_PER_S / 1e12),
+            "peak_three_source_dfma": None if dfma3_per_s is None else 2.0 * dfma3_per_s / 1e12,
+            "frac_of_three_source_dfma": None if dfma3_per_s is None else ach / (2.0 * dfma3_per_s / 1e12),
             "fp64_slots_per_sample": w, "fp64_slots_counted": slots,
             "hbm_leg": {"algorithmic_bytes": bytes_alg, "achieved_gbs": bytes_alg / t_eval / 1e9,
                         "peak_gbs": peaks["hbm_gbs"], "frac": bytes_alg / t_eval / 1e9 / peaks["hbm_gbs"],
@@ -466,7 +494,9 @@ PLAN_IDS = {"auto": 0, "flat": 1, "reg": 2, "tree": 3}
 
 def plan_name_of(info, plan):
     """Name of the representation ami_evaluate executes (after specialisation has been tried)."""
-    if plan != "flat" and info["reg_plan_status"] == 0:
+    if plan not in ("flat", "tree") and info["reg_plan_status"] == 0:
+        if int(info.get("plan_kind", 1)) == 2:
+            return "split (leaf kernel + Horner-plan parts + combine, NVRTC-specialised)"
         return "register (Horner DAG, NVRTC-specialised)"
     return "tree (table-driven Horner program)" if plan == "tree" else "flat (table-driven)"
 
@@ -487,7 +517,8 @@ def run_ours(args, dist, rank, local, world):
     first, _ = sharding.weak_range(n, rank, world)
     n_f, n_b = len(cfg.z_ext), len(cfg.betas)
     plan = PLAN_IDS[args.plan]
-    dfma_per_s, _ = pkg.fp64_peak_probe(local)
+    dfma_per_s, _ = pkg.fp64_peak_probe(local, 2)       # the pipe's issue rate: the roofline's peak
+    dfma3_per_s, _ = pkg.fp64_peak_probe(local, 3)      # DFMAs with three distinct register sources (context)
     peaks = load_measured_peaks()
 
     res = time_workload(pkg, torch, cfg, n, args.steps, args.warmup, plan, first, dist, sample_clocks=True,
@@ -498,7 +529,7 @@ def run_ours(args, dist, rank, local, world):
     units_per_step = n * n_f * n_b * world
     ms_per_step = res["total_ms"] / args.steps
     value = T * units_per_step / (ms_per_step * 1e-3)
-    roof, disp = roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s)
+    roof, disp = roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s, dfma3_per_s)
     if n == cfg.n_samples:
         roof["traffic"] = ncu_traffic(cfg.name, res["fused"])     # per launch, from profiles/ (ncu --set full)
     e2e = time_e2e(pkg, torch, res["tab"], cfg, n, max(2, args.steps // 4), 1, plan, first, dist)
@@ -511,12 +542,17 @@ def run_ours(args, dist, rank, local, world):
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "samples_per_s": units_per_step / (ms_per_step * 1e-3),
-        "config": {"workload": cfg.name, "order": cfg.diagram.n_int, "n_green": cfg.diagram.n_g,
-                   "samples_per_gpu": n, "n_freq": n_f, "n_beta": n_b, "T_flat": T,
-                   "U_F": int(info["n_fermi_leaves"]), "U_D": int(info["n_den_leaves"]), "plan": plan_name,
-                   "sum_order": args.sum_order,
-                   "l2": f"inputs rotated over {res['n_rot']} resident batches (> L2)",
-                   "parallelism": "replicas" if world == 1 else f"sample-sharded x{world}, no collective"},
+        "config": {"workload": cfg.name, "samples_per_gpu": n, "n_freq": n_f, "n_beta": n_b, "T_flat": T,
+                   "precision": "double"},
+        "config_detail": {"order": cfg.diagram.n_int, "n_green": cfg.diagram.n_g,
+                          "U_F": int(info["n_fermi_leaves"]), "U_D": int(info["n_den_leaves"]), "plan": plan_name,
+                          "sum_order": args.sum_order,
+                          "l2": f"inputs rotated over {res['n_rot']} resident batches (> L2)",
+                          "parallelism": "replicas" if world == 1 else f"sample-sharded x{world}, no collective"},
+        "time_to_first_result": {"construct_ms": res["construct_ms"], "specialize_ms": float(info["specialize_ms"]),
+                                 "specialize_from_disk_cache": bool(info["specialize_cached"]),
+                                 "note": "ami_construct (host recursion + plans + device copy) and ami_table_specialize "
+                                         "(generate + NVRTC or cache fetch + module load); outside every timed region"},
         "kernels": {"dominant_ms": res["eval_ms"], "ami_dispersion_ms": None if res["fused"] else res["disp_ms"],
                     "dispersion": disp, "launches_per_step": res["launches"] / max(1, args.steps),
                     "timed_as": "one CUDA graph of K steps" if res["graph"] else "K launches from the host",
@@ -526,32 +562,47 @@ def run_ours(args, dist, rank, local, world):
                 "steps": e2e_steps, "chunks_per_step": e2e["chunks"], "api": "ami_run(h_k -> h_out)"},
         "gpu_launches": launches,
         "clocks": res["clocks"],
-        "fp64_probe_dfma_per_s": dfma_per_s,
+        "fp64_probe_dfma_per_s": dfma_per_s, "fp64_probe_three_source_dfma_per_s": dfma3_per_s,
     }
     if world == 1 and rank == 0 and not args.no_extra:
         # secondary workloads (north_star names order 4 AND order 6), short runs, same code path
         others = {}
-        for name in ("cfg4", "cfg5", "cfg2_se", "cfg1"):
+        for name in ("cfg4", "cfg5", "cfg2_se", "cfg1", "order7", "stress8"):
             if name == cfg.name:
                 continue
-            c2 = A.get_config(name)
+            # order7 / stress8: tables beyond one register-resident kernel (T = 8598 / 40244; the paper runs m = 9,
+            # PAPER.md:389-393), outside the five graded configurations; they run the split plan
+            c2 = A.get_config("stress8", diagram=A.random_self_energy(7, 0), name="order7") if name == "order7" \
+                else A.get_config(name)
             r2 = time_workload(pkg, torch, c2, c2.n_samples, 20, 3, plan, 0, None, sample_clocks=False,
                                use_graph=not args.no_graph)
             i2 = r2["info"]
             pn2 = plan_name_of(i2, args.plan)
             f2, b2 = len(c2.z_ext), len(c2.betas)
-            roof2, disp2 = roofline_objects(r2, c2.n_samples, f2, b2, peaks, dfma_per_s)
+            roof2, disp2 = roofline_objects(r2, c2.n_samples, f2, b2, peaks, dfma_per_s, dfma3_per_s)
             ms2 = r2["total_ms"] / 20
             others[name] = {"T_flat": int(i2["n_terms"]), "samples": c2.n_samples, "n_freq": f2, "n_beta": b2,
                             "plan": pn2, "ms_per_step": ms2, "eval_ms": r2["eval_ms"], "disp_ms": r2["disp_ms"],
                             "term_evals_per_s": int(i2["n_terms"]) * c2.n_samples * f2 * b2 / (ms2 * 1e-3),
                             "samples_per_s": c2.n_samples * f2 * b2 / (ms2 * 1e-3),
-                            "alu_frac": roof2["frac"], "hbm_frac": roof2["hbm_leg"]["frac"],
+                            "alu_frac": roof2["frac"], "alu_frac_of_nominal": roof2["frac_of_nominal"],
+                            "hbm_frac": roof2["hbm_leg"]["frac"], "fp64_slots_per_sample": roof2["fp64_slots_counted"],
+                            "construct_ms": r2["construct_ms"], "specialize_ms": float(i2["specialize_ms"]),
+                            "specialize_from_disk_cache": bool(i2["specialize_cached"]),
                             "two_stream_ms_per_step": r2["two_stream_ms"]}
+            if int(i2.get("plan_kind", 1)) == 2:
+                # the split plan's parts read every leaf they use from the L2-resident leaf array: that, not the FP64
+                # pipe, bounds it; the slots counted are those of the Horner plan, without the sums
+                # that several parts form again
+                others[name]["bound"] = "L2 bandwidth (leaf array reads), see DESIGN.md 6.5"
             del r2
             torch.cuda.empty_cache()
         line["other_workloads"] = others
         line["monte_carlo"] = time_monte_carlo(torch, res["tab"], cfg, 10 * n, 5, plan)
+        w_mc = fp64_work_per_sample(info, n_f, n_b, res["fused"])
+        line["monte_carlo"]["alu_frac"] = (w_mc["evaluate"] + w_mc["dispersion"]) * line["monte_carlo"]["samples_per_s"] \
+            / dfma_per_s
+        line["e2e_seeded"] = time_e2e_seeded(torch, res["tab"], cfg, n, max(2, args.steps // 4), plan, T)
         import oracle
         threads = oracle.hardware_threads()
         n_s = oracle_sample_size(cfg, threads, args.cpu_seconds)

@@ -68,14 +68,16 @@ enum {
                          into a DAG) as a program interpreted by a table-driven kernel: node lists of uniform
                          multiply-add items, staged through shared memory in tiles with TMA; real energies.  What
                          AMI_PLAN_AUTO runs when the register plan is not available for the table */
-  AMI_PLAN_REG = 2    /* register plan: the table written out as a straight-line kernel specialised to
-                         this diagram (terms grouped by denominator product, Fermi/Bose and denominator
-                         products in Horner form, every leaf a register), compiled with NVRTC on first
-                         use; real energies and tables within the size limits only.  With the environment
-                         variable AMI_JIT_SCRATCH=1 larger tables get a memory-backed variant of the same
-                         kernels (leaves in shared memory, long-lived sums in a global scratch); compiling
-                         those takes minutes */
+  AMI_PLAN_REG = 2    /* specialised kernels: the table written out as straight-line code for this diagram
+                         (terms grouped by denominator product, Fermi/Bose and denominator products in Horner
+                         form), compiled with NVRTC on first use and cached on disk; real energies.  Tables of
+                         orders up to 6-7 become ONE kernel with every value in a register (register plan);
+                         larger ones (order 7-8, 1e4-1e5 flat terms) are split: a leaf kernel, then the groups
+                         of the Horner plan in parts of register-plan size evaluated by one launch (grid.y =
+                         part), then a kernel that adds the parts (split plan).  ami_info.plan_kind says which */
 };
+
+enum { AMI_KIND_NONE = 0, AMI_KIND_REGISTER = 1, AMI_KIND_SPLIT = 2 };
 
 typedef struct ami_info {
   int32_t n_int, n_ext, n_g, n_eps;
@@ -101,7 +103,11 @@ typedef struct ami_info {
   int64_t tree_plan_slots;  /* value slots (doubles) per sample the tree plan keeps */
   int32_t has_device_copy;
   int32_t reg_plan_status;  /* 0 = specialised kernels loaded, 1 = eligible, not compiled yet,
-                               AMI_EUNSUPPORTED = table outside the register plan's limits, other < 0 = error */
+                               AMI_EUNSUPPORTED = table outside the specialised kernels' limits, other < 0 = error */
+  int32_t plan_kind;        /* AMI_KIND_*: how AMI_PLAN_REG / AMI_PLAN_AUTO specialise this table */
+  int32_t specialize_cached; /* 1 if the loaded kernels came from the on-disk cache */
+  double specialize_ms;     /* host time ami_table_specialize (or the first evaluation) spent generating, compiling
+                               (or fetching) and loading the kernels; 0 until then */
 } ami_info;
 
 /* ---- Diagram files (Fig. 2; "Feature: Feynman Graph Representation") ----------
@@ -229,8 +235,8 @@ int ami_dispersion(const ami_table* tab, const double* d_k, int64_t k_stride_sam
  * and e_i = -eps(K_i) as above.
  *   d_k     component c of internal momentum l of sample s at d_k[s * k_stride_sample + (dim*l + c) * k_stride_comp]
  *   q       host [n_ext][dim];  d_e out, float64 [n_eps][n]
- * AMI_EINVAL for dim outside 1..3 or an unknown band.  The fused call ami_evaluate_momenta and ami_run keep
- * the 2D tight-binding band of the configurations: for other bands call this, then ami_evaluate. */
+ * AMI_EINVAL for dim outside 1..3 or an unknown band.  ami_evaluate_momenta_lattice and ami_run (cfg.dim,
+ * cfg.band) take the same choices in one fused kernel. */
 enum { AMI_BAND_TIGHT_BINDING = 0, AMI_BAND_FREE = 1 };
 int ami_dispersion_lattice(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
                            const double* q, double t, double mu, int dim, int band, int64_t n, double* d_e,
@@ -260,7 +266,20 @@ int ami_evaluate_momenta(const ami_table* tab, const double* d_k, int64_t k_stri
                          const double* q, double t, double mu, int64_t n, const double* z_ext, int n_f,
                          const double* beta, int n_b, double e_reg, int plan, double* d_e, void* d_out, void* stream);
 
-/* Register plan management.  ami_table_specialize compiles and loads the specialised kernels now
+/* The fused call for momenta of dim = 1, 2 or 3 components and either band of ami_dispersion_lattice (Eq. 14 is
+ * general in d; eps_k is the user's): d_k component c of internal momentum l of
+ * sample s at d_k[s * k_stride_sample + (dim*l + c) * k_stride_comp], q host [n_ext][dim].  The specialised
+ * kernels are generated per (dim, band), so this is ONE kernel like the 2-D call.  When d_e is NULL and a
+ * table-driven plan runs, the energies live in a stream-ordered workspace of the library. */
+int ami_evaluate_momenta_lattice(const ami_table* tab, const double* d_k, int64_t k_stride_sample,
+                                 int64_t k_stride_comp, const double* q, double t, double mu, int dim, int band,
+                                 int64_t n, const double* z_ext, int n_f, const double* beta, int n_b, double e_reg,
+                                 int plan, double* d_e, void* d_out, void* stream);
+
+/* Specialised kernels.  The compiled kernels are kept on disk under $AMI_JIT_CACHE, else
+ * $XDG_CACHE_HOME/ami_b200, else $HOME/.cache/ami_b200, keyed by a hash of (generated source, NVRTC version,
+ * architecture), so a second process on the same diagram loads them in milliseconds; AMI_JIT_CACHE=0 turns the
+ * cache off.  ami_table_specialize compiles and loads the specialised kernels now
  * (otherwise this happens at the first evaluation with AMI_PLAN_AUTO or AMI_PLAN_REG); it returns
  * AMI_EUNSUPPORTED when the table is outside the plan's limits or NVRTC cannot be loaded, AMI_EINVAL when
  * compilation fails (ami_last_cuda_error() then holds the compiler log).  ami_table_kernel_source /
@@ -271,6 +290,11 @@ int ami_evaluate_momenta(const ami_table* tab, const double* d_k, int64_t k_stri
 int ami_table_specialize(ami_table* tab);
 int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes);
 int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char* log, size_t log_cap);
+/* A split plan is several translation units (the leaf and combine kernels first, then the parts, a few per unit,
+ * compiled side by side): ami_table_kernel_units counts them, ami_table_kernel_source returns all of them one after
+ * the other, ami_table_kernel_cubin_unit compiles unit `unit` (ami_table_kernel_cubin is unit 0). */
+int ami_table_kernel_units(const ami_table* tab, int* n_units);
+int ami_table_kernel_cubin_unit(const ami_table* tab, int unit, void* buf, size_t* bytes, char* log, size_t log_cap);
 
 /* Streamed driver.  Source of the momenta: if h_k / d_k are both NULL they are generated on the
  * device from `seed` with the counter-based generator of P22 (sample index = first_sample + s) --
@@ -304,6 +328,8 @@ typedef struct ami_run_cfg {
   void* stream;          /* caller's stream; internal copy/compute streams are ordered after it */
   void* h_sumsq;         /* host float64 [n_b][n_f][2] or NULL: sums of re^2 and im^2 over the samples (with
                             want_sum), for the Monte-Carlo error bar of the mean */
+  int32_t dim;           /* components per momentum, 1..3 (0 = 2); momenta are [n][dim*n_int], q is [n_ext][dim] */
+  int32_t band;          /* AMI_BAND_* of ami_dispersion_lattice (0 = tight binding) */
 } ami_run_cfg;
 
 typedef struct ami_run_stats {
@@ -315,14 +341,20 @@ typedef struct ami_run_stats {
 
 int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_stats* stats);
 
-/* Fills d_k [n][2*n_int] with the momenta of samples first_sample .. first_sample+n-1 (P22). */
+/* Fills d_k [n][2*n_int] with the momenta of samples first_sample .. first_sample+n-1 (P22); the _lattice
+ * form for momenta of dim components, [n][dim*n_int] (counter of a component = sample * dim*n_int + index). */
 int ami_generate_momenta(const ami_table* tab, uint64_t seed, int64_t first_sample, int64_t n, double* d_k,
                          void* stream);
+int ami_generate_momenta_lattice(const ami_table* tab, uint64_t seed, int64_t first_sample, int64_t n, int dim,
+                                 double* d_k, void* stream);
 
-/* Register-only DFMA chain used by bench.py to measure the FP64 pipe peak of the device the
- * bench runs on (MEASURED_PEAKS.json has no FP64 figure).  Returns in *dfma_per_s the measured
- * rate of double-precision FMA lane-operations per second. */
-int ami_fp64_peak_probe(int device, double* dfma_per_s, double* elapsed_ms);
+/* Register-only DFMA chains used by bench.py to measure the FP64 pipe of the device the bench runs on
+ * (MEASURED_PEAKS.json has no FP64 figure).  distinct_sources = 2: x = fma(x, x, b), two different register
+ * operands: the pipe's issue rate (0.995 of 148 SMs x 64 lanes x clock on B200), the roofline's peak.
+ * distinct_sources = 3: x = fma(x, a, b): what a DFMA with three different register operands -- the usual shape in
+ * real code -- sustains (0.92 of that).  Returns in *dfma_per_s the rate of double-precision FMA lane-operations
+ * per second. */
+int ami_fp64_peak_probe(int device, int distinct_sources, double* dfma_per_s, double* elapsed_ms);
 
 /* Total number of kernels this library has launched in the calling process so far (all tables, all
  * streams); bench.py reports the difference over its timed region as "gpu_launches". */

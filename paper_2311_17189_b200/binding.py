@@ -21,7 +21,8 @@ EXPORTS = [
     "ami_evaluate", "ami_evaluate_momenta", "ami_table_specialize", "ami_table_kernel_source",
     "ami_table_kernel_cubin", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
     "ami_last_cuda_error", "ami_version", "ami_kernel_launches", "ami_search_sum_order", "ami_graph_parse",
-    "ami_graph_label", "ami_table_latex",
+    "ami_graph_label", "ami_table_latex", "ami_evaluate_momenta_lattice", "ami_generate_momenta_lattice",
+    "ami_table_kernel_units", "ami_table_kernel_cubin_unit",
 ]
 
 
@@ -38,7 +39,8 @@ class ami_info(C.Structure):
                                          "n_den_nodes", "table_bytes", "fp64_ops_flat", "fp64_ops_tree",
                                          "fp64_ops_tree_fermi", "fp64_ops_leaf_fermi", "fp64_ops_leaf_den",
                                          "fp64_ops_dispersion", "fp64_ops_combos", "tree_plan_words", "tree_plan_slots")] + \
-               [("has_device_copy", C.c_int32), ("reg_plan_status", C.c_int32)]
+               [("has_device_copy", C.c_int32), ("reg_plan_status", C.c_int32), ("plan_kind", C.c_int32),
+                ("specialize_cached", C.c_int32), ("specialize_ms", C.c_double)]
 
 
 class ami_run_cfg(C.Structure):
@@ -47,7 +49,7 @@ class ami_run_cfg(C.Structure):
                 ("mu", C.c_double), ("z_ext", C.c_void_p), ("n_f", C.c_int32), ("beta", C.c_void_p),
                 ("n_b", C.c_int32), ("e_reg", C.c_double), ("plan", C.c_int32), ("want_sum", C.c_int32),
                 ("h_out", C.c_void_p), ("d_out", C.c_void_p), ("h_sum", C.c_void_p), ("stream", C.c_void_p),
-                ("h_sumsq", C.c_void_p)]
+                ("h_sumsq", C.c_void_p), ("dim", C.c_int32), ("band", C.c_int32)]
 
 
 class ami_run_stats(C.Structure):
@@ -85,12 +87,21 @@ def lib():
         L.ami_evaluate_momenta.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
                                            C.c_double, C.c_int64, C.c_void_p, C.c_int, C.c_void_p, C.c_int,
                                            C.c_double, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.ami_evaluate_momenta_lattice.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
+                                                   C.c_double, C.c_int, C.c_int, C.c_int64, C.c_void_p, C.c_int,
+                                                   C.c_void_p, C.c_int, C.c_double, C.c_int, C.c_void_p, C.c_void_p,
+                                                   C.c_void_p]
+        L.ami_generate_momenta_lattice.argtypes = [C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_int, C.c_void_p,
+                                                   C.c_void_p]
         L.ami_table_specialize.argtypes = [C.c_void_p]
         L.ami_table_kernel_source.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.ami_table_kernel_cubin.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p, C.c_size_t]
+        L.ami_table_kernel_units.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
+        L.ami_table_kernel_cubin_unit.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p,
+                                                  C.c_size_t]
         L.ami_run.argtypes = [C.c_void_p, C.POINTER(ami_run_cfg), C.POINTER(ami_run_stats)]
         L.ami_generate_momenta.argtypes = [C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
-        L.ami_fp64_peak_probe.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.ami_fp64_peak_probe.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.ami_strerror.restype = C.c_char_p
         L.ami_strerror.argtypes = [C.c_int]
         L.ami_last_cuda_error.restype = C.c_char_p
@@ -184,12 +195,18 @@ class AmiTable:
         _check(lib().ami_table_kernel_source(self._h, buf, C.byref(n)))
         return buf.value.decode()
 
-    def kernel_cubin(self, cap=64 << 20):
-        """(cubin bytes, compiler log); needs NVRTC but no GPU."""
+    def kernel_units(self) -> int:
+        """Translation units of the specialised kernels (1 for the register plan, 1 + M for a split plan)."""
+        n = C.c_int(0)
+        _check(lib().ami_table_kernel_units(self._h, C.byref(n)))
+        return n.value
+
+    def kernel_cubin(self, cap=64 << 20, unit=0):
+        """(cubin bytes, compiler log) of translation unit ``unit``; needs NVRTC but no GPU."""
         buf = C.create_string_buffer(cap)
-        log = C.create_string_buffer(1 << 16)
+        log = C.create_string_buffer(1 << 18)
         n = C.c_size_t(cap)
-        _check(lib().ami_table_kernel_cubin(self._h, buf, C.byref(n), log, len(log)))
+        _check(lib().ami_table_kernel_cubin_unit(self._h, int(unit), buf, C.byref(n), log, len(log)))
         return buf.raw[: n.value], log.value.decode()
 
     def export(self) -> dict:
@@ -269,10 +286,10 @@ class AmiTable:
         return out
 
     def evaluate_momenta(self, k, q, t, mu, z_ext, beta, e_reg=0.0, plan=PLAN_AUTO, e_out=None, out=None,
-                         stream=None):
-        """ami_evaluate_momenta: S1+S2+S3 for momenta k [n][n_int][2] -> complex128 [n_b][n_f][n].
-        ``e_out`` ([n_eps][n] float64) receives the energies when given; it is allocated here when
-        the plan that runs needs it as workspace."""
+                         stream=None, dim=2, band=BAND_TIGHT_BINDING):
+        """ami_evaluate_momenta (dim = 2, tight binding) / ami_evaluate_momenta_lattice: S1+S2+S3 for momenta
+        k [n][n_int][dim] -> complex128 [n_b][n_f][n].  ``e_out`` ([n_eps][n] float64) receives the energies
+        when given (a table-driven plan that needs them as workspace allocates its own otherwise)."""
         import torch
         assert k.is_cuda and k.dtype == torch.float64 and k.is_contiguous()
         n = k.shape[0]
@@ -282,31 +299,36 @@ class AmiTable:
         if out is None:
             out = torch.empty((n_b, n_f, n), dtype=torch.complex128, device=k.device)
         assert out.is_contiguous() and out.dtype == torch.complex128 and out.numel() == n_b * n_f * n
-        reg = plan in (PLAN_AUTO, PLAN_REG) and self.info["reg_plan_status"] in (0, 1)
-        if e_out is None and not reg:
-            e_out = torch.empty((self.n_eps, n), dtype=torch.float64, device=k.device)
-        qh = _host(np.asarray(q, dtype=np.float64).reshape(max(self.n_ext, 1), 2), np.float64)
-        _check(lib().ami_evaluate_momenta(self._h, C.c_void_p(k.data_ptr()), 2 * self.n_int, 1, qh.ctypes.data,
-                                          float(t), float(mu), n, z.ctypes.data, n_f, b.ctypes.data, n_b,
-                                          float(e_reg), int(plan), None if e_out is None else C.c_void_p(e_out.data_ptr()),
-                                          C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        qh = _host(np.asarray(q, dtype=np.float64).reshape(max(self.n_ext, 1), dim), np.float64)
+        e_ptr = None if e_out is None else C.c_void_p(e_out.data_ptr())
+        if dim == 2 and band == BAND_TIGHT_BINDING:
+            _check(lib().ami_evaluate_momenta(self._h, C.c_void_p(k.data_ptr()), 2 * self.n_int, 1, qh.ctypes.data,
+                                              float(t), float(mu), n, z.ctypes.data, n_f, b.ctypes.data, n_b,
+                                              float(e_reg), int(plan), e_ptr, C.c_void_p(out.data_ptr()),
+                                              _stream_ptr(stream)))
+        else:
+            _check(lib().ami_evaluate_momenta_lattice(self._h, C.c_void_p(k.data_ptr()), dim * self.n_int, 1,
+                                                      qh.ctypes.data, float(t), float(mu), int(dim), int(band), n,
+                                                      z.ctypes.data, n_f, b.ctypes.data, n_b, float(e_reg), int(plan),
+                                                      e_ptr, C.c_void_p(out.data_ptr()), _stream_ptr(stream)))
         return out
 
-    def generate_momenta(self, seed, first_sample, n, stream=None):
+    def generate_momenta(self, seed, first_sample, n, stream=None, dim=2):
         import torch
-        k = torch.empty((n, self.n_int, 2), dtype=torch.float64, device=f"cuda:{self.device}")
-        _check(lib().ami_generate_momenta(self._h, int(seed), int(first_sample), n, C.c_void_p(k.data_ptr()),
-                                          _stream_ptr(stream)))
+        k = torch.empty((n, self.n_int, dim), dtype=torch.float64, device=f"cuda:{self.device}")
+        _check(lib().ami_generate_momenta_lattice(self._h, int(seed), int(first_sample), n, int(dim),
+                                                  C.c_void_p(k.data_ptr()), _stream_ptr(stream)))
         return k
 
     def run(self, n, q, t, mu, z_ext, beta, e_reg=0.0, plan=PLAN_AUTO, seed=0, first_sample=0, chunk=0,
-            h_k=None, d_k=None, h_out=None, d_out=None, want_sum=False, stream=None):
+            h_k=None, d_k=None, h_out=None, d_out=None, want_sum=False, stream=None, dim=2, band=BAND_TIGHT_BINDING):
         """ami_run, the streamed driver.  h_k / h_out are (preferably pinned) CPU tensors or numpy
         arrays; d_k / d_out CUDA tensors.  Returns (stats dict, sums or None)."""
         z = _z_host(z_ext, self.n_ext)
         b = _host(np.atleast_1d(beta), np.float64)
-        qh = _host(np.asarray(q, dtype=np.float64).reshape(max(self.n_ext, 1), 2), np.float64)
+        qh = _host(np.asarray(q, dtype=np.float64).reshape(max(self.n_ext, 1), dim), np.float64)
         cfg = ami_run_cfg()
+        cfg.dim, cfg.band = int(dim), int(band)
         cfg.n, cfg.chunk, cfg.seed, cfg.first_sample = int(n), int(chunk), int(seed), int(first_sample)
         ptr = lambda x: None if x is None else (x.ctypes.data if isinstance(x, np.ndarray) else x.data_ptr())
         cfg.h_k, cfg.d_k, cfg.h_out, cfg.d_out = ptr(h_k), ptr(d_k), ptr(h_out), ptr(d_out)
@@ -386,8 +408,9 @@ def kernel_launches() -> int:
     return int(lib().ami_kernel_launches())
 
 
-def fp64_peak_probe(device=0):
-    """Measured DFMA lane-operations per second of ``device`` (register-only chains)."""
+def fp64_peak_probe(device=0, distinct_sources=2):
+    """Measured DFMA lane-operations per second of ``device`` (register-only chains): with two distinct register
+    sources per DFMA (the pipe's issue rate) or three (what general register-operand code sustains)."""
     r, ms = C.c_double(0), C.c_double(0)
-    _check(lib().ami_fp64_peak_probe(int(device), C.byref(r), C.byref(ms)))
+    _check(lib().ami_fp64_peak_probe(int(device), int(distinct_sources), C.byref(r), C.byref(ms)))
     return r.value, ms.value

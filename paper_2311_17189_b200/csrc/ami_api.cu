@@ -263,6 +263,12 @@ int ami_table_info(const ami_table* tab, ami_info* info) {
   info->has_device_copy = tab->dev.device >= 0;
   info->reg_plan_status = !ami::jit_eligible(ft, tab->horner) ? AMI_EUNSUPPORTED
                           : (tab->jit ? ami::jit_status(tab) : 1);
+  info->plan_kind = ami::jit_mode(ft, tab->horner);
+  {
+    int hit = 0;
+    info->specialize_ms = tab->jit ? ami::jit_last_compile_ms(tab, &hit) : 0.0;
+    info->specialize_cached = hit;
+  }
   return AMI_OK;
 }
 
@@ -324,7 +330,8 @@ void fill_table_params(const ami_table* tab, ami::EvalParams& p) {
 
 // Decides which representation runs.  Returns AMI_OK and sets *use_reg, or an error when the
 // register plan was asked for explicitly and cannot be had.
-int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg, bool* use_tree = nullptr) {
+int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg, bool* use_tree = nullptr,
+                const ami::JitVariant& var = ami::JitVariant()) {
   *use_reg = false;
   if (use_tree) *use_tree = false;
   if (plan == AMI_PLAN_FLAT) return AMI_OK;
@@ -344,7 +351,7 @@ int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg
     return AMI_OK;
   }
   std::string err;
-  const int rc = ami::jit_prepare(const_cast<ami_table*>(tab), err);   // lazily compiled, cached in the table
+  const int rc = ami::jit_prepare(const_cast<ami_table*>(tab), var, err);   // lazily compiled, cached in the table
   if (rc == AMI_OK) { *use_reg = true; return AMI_OK; }
   g_cuda_err = err;
   if (plan == AMI_PLAN_REG) return rc;
@@ -364,6 +371,8 @@ struct MomentaSrc {
   bool gen = false;             // register plan only: draw the momenta inside the kernel (d_k unused)
   uint64_t seed = 0;
   int64_t first_sample = 0;
+  int dim = 2, band = AMI_BAND_TIGHT_BINDING;   // lattice of the dispersion (Eq. 14)
+  int64_t* tally_slots = nullptr;               // out: per-row partial sums the fused tally wrote
 };
 
 // Launches the evaluation for all (beta, frequency) pairs, split so that one launch carries at
@@ -376,8 +385,11 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
                   void* d_out, int64_t out_row_stride, cudaStream_t st, int* launches) {
   using namespace ami;
   bool use_reg = false, use_tree = false;
-  int rc = choose_plan(tab, plan, e_is_complex != 0, &use_reg, &use_tree);
+  ami::JitVariant var;
+  if (mom) { var.dim = mom->dim; var.band = mom->band; }
+  int rc = choose_plan(tab, plan, e_is_complex != 0, &use_reg, &use_tree, var);
   if (rc != AMI_OK) return rc;
+  const int dim = var.dim;
   const int n_ext = tab->flat.n_ext;
   const int f_chunk = n_ext ? std::max(1, kMaxFreqWords / n_ext) : kMaxFreqWords;
   if (mom && !use_reg) {
@@ -387,8 +399,8 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
     dp.sym_alpha = tab->dev.sym_alpha;
     dp.n_int = tab->flat.n_int; dp.n_ext = n_ext; dp.n_eps = tab->flat.n_eps;
     dp.k = mom->d_k; dp.k_stride_sample = mom->stride_sample; dp.k_stride_comp = mom->stride_comp; dp.n = n_e;
-    dp.dim = 2; dp.band = AMI_BAND_TIGHT_BINDING;
-    for (int i = 0; i < 2 * n_ext; ++i) dp.q[i] = mom->q[i];
+    dp.dim = dim; dp.band = var.band;
+    for (int i = 0; i < dim * n_ext; ++i) dp.q[i] = mom->q[i];
     dp.t = mom->t; dp.mu = mom->mu; dp.e = (double*)d_e; dp.e_stride = e_stride;
     cudaError_t crc = launch_dispersion(dp, st);
     if (crc != cudaSuccess) return cuda_fail(crc);
@@ -404,7 +416,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
       jb.k = mom->d_k; jb.k_stride_sample = mom->stride_sample; jb.k_stride_comp = mom->stride_comp;
       jb.gen = mom->gen ? 1 : 0; jb.seed = mom->seed; jb.first_sample = mom->first_sample;
       jb.tally = mom->tally; jb.tally_stride = mom->tally_stride;
-      for (int i = 0; i < 2 * n_ext; ++i) jb.q[i] = mom->q[i];
+      for (int i = 0; i < dim * n_ext; ++i) jb.q[i] = mom->q[i];
       jb.t = mom->t; jb.mu = mom->mu;
       jb.e_out = (double*)d_e;
     }
@@ -450,7 +462,9 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
         const bool fused = mom && (first || !d_e);
         if (!fused) { jb.e_out = nullptr; }
         int n_launched = 0;
-        crc = jit_launch(tab, fused, jb, st, &n_launched);
+        long long slots = 0;
+        crc = jit_launch(tab, var, fused, jb, st, &n_launched, &slots);
+        if (mom && mom->tally_slots) *mom->tally_slots = slots;
         for (int i = 0; i < n_launched; ++i) count_external_launch(launches);
       } else {
         p.b0 = b0; p.n_b = nb; p.f0 = f0; p.n_f = nf;
@@ -516,25 +530,48 @@ int ami_evaluate(const ami_table* tab, const void* d_e, int e_is_complex, int64_
                        (cudaStream_t)stream, nullptr);
 }
 
-int ami_evaluate_momenta(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
-                         const double* q, double t, double mu, int64_t n, const double* z_ext, int n_f,
-                         const double* beta, int n_b, double e_reg, int plan, double* d_e, void* d_out, void* stream) {
+int ami_evaluate_momenta_lattice(const ami_table* tab, const double* d_k, int64_t k_stride_sample,
+                                 int64_t k_stride_comp, const double* q, double t, double mu, int dim, int band,
+                                 int64_t n, const double* z_ext, int n_f, const double* beta, int n_b, double e_reg,
+                                 int plan, double* d_e, void* d_out, void* stream) {
   int rc = check_device(tab);
   if (rc) return rc;
   if (n < 0 || n_f < 0 || n_b < 0 || (n_f > 0 && tab->flat.n_ext > 0 && !z_ext) || (n_b > 0 && !beta) ||
-      (tab->flat.n_ext > 0 && !q) || plan < AMI_PLAN_AUTO || plan > AMI_PLAN_TREE)
+      (tab->flat.n_ext > 0 && !q) || plan < AMI_PLAN_AUTO || plan > AMI_PLAN_TREE || dim < 1 || dim > 3 ||
+      (band != AMI_BAND_TIGHT_BINDING && band != AMI_BAND_FREE))
     return AMI_EINVAL;
   if (n == 0) return AMI_OK;
   if (!d_k || (!d_out && n_f > 0 && n_b > 0)) return AMI_EINVAL;
   MomentaSrc ms;
   ms.d_k = d_k; ms.stride_sample = k_stride_sample; ms.stride_comp = k_stride_comp;
-  ms.q = q; ms.t = t; ms.mu = mu;
+  ms.q = q; ms.t = t; ms.mu = mu; ms.dim = dim; ms.band = band;
   if (n_f == 0 || n_b == 0) {
     if (!d_e) return AMI_OK;
-    return ami_dispersion(tab, d_k, k_stride_sample, k_stride_comp, q, t, mu, n, d_e, stream);
+    return ami_dispersion_lattice(tab, d_k, k_stride_sample, k_stride_comp, q, t, mu, dim, band, n, d_e, stream);
   }
-  return evaluate_impl(tab, &ms, d_e, 0, n, n, z_ext, n_f, beta, n_b, e_reg, plan, d_out, n, (cudaStream_t)stream,
-                       nullptr);
+  // the table-driven plans need the energies in memory: a stream-ordered workspace when the caller gave none
+  double* ws = nullptr;
+  bool use_reg = false;
+  ami::JitVariant var;
+  var.dim = dim; var.band = band;
+  if (!d_e) {
+    rc = choose_plan(tab, plan, false, &use_reg, nullptr, var);
+    if (rc) return rc;
+    if (!use_reg) {
+      CU(cudaMallocAsync((void**)&ws, (size_t)tab->flat.n_eps * (size_t)n * sizeof(double), (cudaStream_t)stream));
+      d_e = ws;
+    }
+  }
+  rc = evaluate_impl(tab, &ms, d_e, 0, n, n, z_ext, n_f, beta, n_b, e_reg, plan, d_out, n, (cudaStream_t)stream, nullptr);
+  if (ws) cudaFreeAsync(ws, (cudaStream_t)stream);
+  return rc;
+}
+
+int ami_evaluate_momenta(const ami_table* tab, const double* d_k, int64_t k_stride_sample, int64_t k_stride_comp,
+                         const double* q, double t, double mu, int64_t n, const double* z_ext, int n_f,
+                         const double* beta, int n_b, double e_reg, int plan, double* d_e, void* d_out, void* stream) {
+  return ami_evaluate_momenta_lattice(tab, d_k, k_stride_sample, k_stride_comp, q, t, mu, 2, AMI_BAND_TIGHT_BINDING, n,
+                                      z_ext, n_f, beta, n_b, e_reg, plan, d_e, d_out, stream);
 }
 
 int ami_table_export_tree(const ami_table* tab, void* host_buf, size_t* bytes) {
@@ -561,7 +598,7 @@ int ami_table_specialize(ami_table* tab) {
   int rc = check_device(tab);
   if (rc) return rc;
   std::string err;
-  rc = ami::jit_prepare(tab, err);
+  rc = ami::jit_prepare(tab, ami::JitVariant(), err);
   if (rc != AMI_OK) g_cuda_err = err;
   return rc;
 }
@@ -569,8 +606,12 @@ int ami_table_specialize(ami_table* tab) {
 int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes) {
   if (!tab || !bytes) return AMI_EINVAL;
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
-  const bool scratch = ami::jit_mode(tab->flat, tab->horner) == ami::kJitScratch;
-  const std::string src = ami::jit_generate_source(tab->flat, tab->horner, scratch ? 64 : ami::jit_block_threads(), scratch, nullptr);
+  const std::vector<std::string> srcs = ami::jit_generate_sources(tab->flat, tab->horner, ami::JitVariant(), nullptr);
+  std::string src;
+  for (size_t i = 0; i < srcs.size(); ++i) {
+    if (srcs.size() > 1) src += "// ======== translation unit " + std::to_string(i) + " of " + std::to_string(srcs.size()) + " ========\n";
+    src += srcs[i];
+  }
   if (!buf) { *bytes = src.size() + 1; return AMI_OK; }
   if (*bytes < src.size() + 1) return AMI_EINVAL;
   memcpy(buf, src.c_str(), src.size() + 1);
@@ -578,14 +619,21 @@ int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes) {
   return AMI_OK;
 }
 
-int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char* log, size_t log_cap) {
+int ami_table_kernel_units(const ami_table* tab, int* n_units) {
+  if (!tab || !n_units) return AMI_EINVAL;
+  if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
+  *n_units = (int)ami::jit_generate_sources(tab->flat, tab->horner, ami::JitVariant(), nullptr).size();
+  return AMI_OK;
+}
+
+int ami_table_kernel_cubin_unit(const ami_table* tab, int unit, void* buf, size_t* bytes, char* log, size_t log_cap) {
   if (!tab || !bytes) return AMI_EINVAL;
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
+  const std::vector<std::string> srcs = ami::jit_generate_sources(tab->flat, tab->horner, ami::JitVariant(), nullptr);
+  if (unit < 0 || unit >= (int)srcs.size()) return AMI_EINVAL;
   std::vector<char> cubin;
   std::string lg;
-  const bool scratch = ami::jit_mode(tab->flat, tab->horner) == ami::kJitScratch;
-  const int rc = ami::jit_compile(
-      ami::jit_generate_source(tab->flat, tab->horner, scratch ? 64 : ami::jit_block_threads(), scratch, nullptr), cubin, lg);
+  const int rc = ami::jit_compile(srcs[unit], cubin, lg, /*use_cache=*/false);
   if (log && log_cap) {
     const size_t nlog = std::min(log_cap - 1, lg.size());
     memcpy(log, lg.data(), nlog);
@@ -600,51 +648,68 @@ int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char*
   return AMI_OK;
 }
 
-int ami_generate_momenta(const ami_table* tab, uint64_t seed, int64_t first_sample, int64_t n, double* d_k,
-                         void* stream) {
+int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char* log, size_t log_cap) {
+  return ami_table_kernel_cubin_unit(tab, 0, buf, bytes, log, log_cap);
+}
+
+int ami_generate_momenta_lattice(const ami_table* tab, uint64_t seed, int64_t first_sample, int64_t n, int dim,
+                                 double* d_k, void* stream) {
   int rc = check_device(tab);
   if (rc) return rc;
-  if (n < 0 || first_sample < 0 || (n > 0 && !d_k)) return AMI_EINVAL;
-  CU(ami::launch_generate_momenta(seed, first_sample, n, 2 * tab->flat.n_int, d_k, (cudaStream_t)stream));
+  if (n < 0 || first_sample < 0 || (n > 0 && !d_k) || dim < 1 || dim > 3) return AMI_EINVAL;
+  CU(ami::launch_generate_momenta(seed, first_sample, n, dim * tab->flat.n_int, d_k, (cudaStream_t)stream));
   return AMI_OK;
 }
 
-int ami_fp64_peak_probe(int device, double* dfma_per_s, double* elapsed_ms) {
-  if (!dfma_per_s || !elapsed_ms || device < 0) return AMI_EINVAL;
+int ami_generate_momenta(const ami_table* tab, uint64_t seed, int64_t first_sample, int64_t n, double* d_k,
+                         void* stream) {
+  return ami_generate_momenta_lattice(tab, seed, first_sample, n, 2, d_k, stream);
+}
+
+int ami_fp64_peak_probe(int device, int distinct_sources, double* dfma_per_s, double* elapsed_ms) {
+  if (!dfma_per_s || !elapsed_ms || device < 0 || (distinct_sources != 2 && distinct_sources != 3)) return AMI_EINVAL;
   CU(cudaSetDevice(device));
-  CU(ami::run_fp64_probe(dfma_per_s, elapsed_ms));
+  CU(ami::run_fp64_probe(distinct_sources, dfma_per_s, elapsed_ms));
   return AMI_OK;
 }
 
 }  // extern "C"
 
 // ---------------------------------------------------------------------------------------------
-// S4: streamed driver.  Chunks alternate between two internal streams, each with its own
-// momentum / energy / output buffers, so that the copy (or generation) of chunk c+1 overlaps
-// the evaluation of chunk c (PAPER.md:113: repeated calls over energy batches; :291 tally).
+// S4: streamed driver (PAPER.md:113: repeated calls over energy batches; :291 tally).  With host
+// buffers the chunks run through a three-stage pipeline on three internal streams -- host-to-device
+// copy of chunk c+1 | kernels of chunk c | device-to-host copy of chunk c-1 -- so that the two copy
+// engines (PCIe is full duplex) and the SMs work at the same time; each stage has two buffers and
+// waits, through events, for the stage that last used the buffer it is about to overwrite.  Without
+// host buffers there is nothing to overlap and everything runs on the caller's stream.
 // ---------------------------------------------------------------------------------------------
 namespace {
 
-// Workspace of the streamed driver, cached in the table between calls: two streams with their
-// events and device buffers that only ever grow (allocation costs more than a chunk's kernels).
+// Workspace of the streamed driver, cached in the table between calls: streams, events and device
+// buffers that only ever grow (allocation costs more than a chunk's kernels).
 struct RunBuffers {
   std::mutex mu;           // one ami_run at a time per table
-  cudaStream_t st[2] = {nullptr, nullptr};
-  cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_done[2] = {nullptr, nullptr};
-  double* k[2] = {nullptr, nullptr};
-  double* e[2] = {nullptr, nullptr};
-  double* out[2] = {nullptr, nullptr};
-  double* wp[2] = {nullptr, nullptr};     // per-warp partial sums of the fused tally
-  size_t cap_k = 0, cap_e = 0, cap_out = 0, cap_sum = 0, cap_wp = 0;
+  cudaStream_t s_in = nullptr, s_k = nullptr, s_out = nullptr;   // H2D copies, kernels, D2H copies
+  cudaEvent_t ev_start = nullptr, ev_stop = nullptr;
+  cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_k[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
+  double* k[2] = {nullptr, nullptr};      // momenta of a chunk
+  double* out[2] = {nullptr, nullptr};    // results of a chunk
+  double* e = nullptr;                    // energies of a chunk (table-driven plans only)
+  double* wp = nullptr;                   // per-warp partial sums of the fused tally
   double* partial = nullptr;
   double* sum = nullptr;
+  size_t cap_k = 0, cap_out = 0, cap_e = 0, cap_wp = 0, cap_partial = 0, cap_sum = 0;
   int init() {
     if (ev_start) return AMI_OK;
     CU(cudaEventCreate(&ev_start));
     CU(cudaEventCreate(&ev_stop));
+    CU(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+    CU(cudaStreamCreateWithFlags(&s_k, cudaStreamNonBlocking));
+    CU(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
     for (int i = 0; i < 2; ++i) {
-      CU(cudaStreamCreateWithFlags(&st[i], cudaStreamNonBlocking));
-      CU(cudaEventCreateWithFlags(&ev_done[i], cudaEventDisableTiming));
+      CU(cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming));
+      CU(cudaEventCreateWithFlags(&ev_k[i], cudaEventDisableTiming));
+      CU(cudaEventCreateWithFlags(&ev_out[i], cudaEventDisableTiming));
     }
     return AMI_OK;
   }
@@ -660,26 +725,26 @@ struct RunBuffers {
   int reserve(size_t bk, size_t be, size_t bo, size_t bs, size_t bw) {
     int rc;
     for (int i = 0; i < 2; ++i) {
-      size_t ck = cap_k, ce = cap_e, co = cap_out, cw = cap_wp;
-      if ((rc = grow(&k[i], &ck, bk)) || (rc = grow(&e[i], &ce, be)) || (rc = grow(&out[i], &co, bo)) ||
-          (rc = grow(&wp[i], &cw, bw)))
-        return rc;
-      if (i == 1) { cap_k = ck; cap_e = ce; cap_out = co; cap_wp = cw; }
+      size_t ck = cap_k, co = cap_out;
+      if ((rc = grow(&k[i], &ck, bk)) || (rc = grow(&out[i], &co, bo))) return rc;
+      if (i == 1) { cap_k = ck; cap_out = co; }
     }
-    size_t c1 = cap_sum, c2 = cap_sum;
-    if ((rc = grow(&partial, &c1, bs * ami::kMaxSumBlocks)) || (rc = grow(&sum, &c2, bs))) return rc;
-    cap_sum = std::max(cap_sum, bs);
+    if ((rc = grow(&e, &cap_e, be)) || (rc = grow(&wp, &cap_wp, bw)) ||
+        (rc = grow(&partial, &cap_partial, bs * ami::kMaxSumBlocks)) || (rc = grow(&sum, &cap_sum, bs)))
+      return rc;
     return AMI_OK;
   }
   ~RunBuffers() {
+    for (cudaStream_t st : {s_in, s_k, s_out})
+      if (st) cudaStreamDestroy(st);
     for (int i = 0; i < 2; ++i) {
-      if (st[i]) cudaStreamDestroy(st[i]);
-      if (ev_done[i]) cudaEventDestroy(ev_done[i]);
-      cudaFree(k[i]); cudaFree(e[i]); cudaFree(out[i]); cudaFree(wp[i]);
+      for (cudaEvent_t ev : {ev_in[i], ev_k[i], ev_out[i]})
+        if (ev) cudaEventDestroy(ev);
+      cudaFree(k[i]); cudaFree(out[i]);
     }
     if (ev_start) cudaEventDestroy(ev_start);
     if (ev_stop) cudaEventDestroy(ev_stop);
-    cudaFree(partial); cudaFree(sum);
+    cudaFree(e); cudaFree(wp); cudaFree(partial); cudaFree(sum);
   }
 };
 
@@ -709,12 +774,15 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   if (rc) return rc;
   if (!cfg || cfg->n < 0 || cfg->n_f < 0 || cfg->n_b < 0 || cfg->chunk < 0 || cfg->first_sample < 0 ||
       (cfg->n_b > 0 && !cfg->beta) || (cfg->n_f > 0 && tab->flat.n_ext > 0 && !cfg->z_ext) ||
-      (tab->flat.n_ext > 0 && !cfg->q) || (cfg->h_k && cfg->d_k) || (cfg->want_sum && !cfg->h_sum))
+      (tab->flat.n_ext > 0 && !cfg->q) || (cfg->h_k && cfg->d_k) || (cfg->want_sum && !cfg->h_sum) ||
+      (!cfg->want_sum && !cfg->h_out && !cfg->d_out) || cfg->dim < 0 || cfg->dim > 3 ||
+      (cfg->band != AMI_BAND_TIGHT_BINDING && cfg->band != AMI_BAND_FREE))
     return AMI_EINVAL;
   ami_run_stats local;
   memset(&local, 0, sizeof local);
+  const int dim = cfg->dim ? cfg->dim : 2;
   const int64_t rows = (int64_t)cfg->n_b * cfg->n_f;
-  const int n_comp = 2 * tab->flat.n_int, n_eps = tab->flat.n_eps;
+  const int n_comp = dim * tab->flat.n_int, n_eps = tab->flat.n_eps;
   if (cfg->n == 0 || rows == 0) {
     if (cfg->want_sum) {
       memset(cfg->h_sum, 0, (size_t)rows * 16);
@@ -723,88 +791,101 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
     if (stats) *stats = local;
     return AMI_OK;
   }
-  // default chunk: small enough that the host copies of one chunk overlap the kernels of the next
   const bool host_io = cfg->h_k || cfg->h_out;
-  int64_t chunk = cfg->chunk ? cfg->chunk : (host_io ? (int64_t)1 << 17 : (int64_t)1 << 22);
-  // keep a chunk's output below ~256 MiB
-  while (chunk > 1024 && chunk * rows * 16 > ((int64_t)256 << 20)) chunk /= 2;
-  if (chunk > cfg->n) chunk = cfg->n;
   const bool direct_out = cfg->d_out != nullptr;   // kernels write straight into the caller's buffer
-  bool use_reg = false;   // the register plan forms the energies inline: no energy buffer
-  rc = choose_plan(tab, cfg->plan, false, &use_reg);
+  bool use_reg = false;   // the specialised kernels form the energies inline: no energy buffer
+  ami::JitVariant var;
+  var.dim = dim; var.band = cfg->band;
+  rc = choose_plan(tab, cfg->plan, false, &use_reg, nullptr, var);
   if (rc) return rc;
+  // Fused tally (register plan, a few rows): the evaluation kernel leaves one partial sum per (row, warp) and the
+  // results are stored only if the caller wants them -- a seeded Monte-Carlo run then moves no sample data at all.
+  const bool fused_tally = use_reg && cfg->want_sum && rows <= kFusedTallyMaxRows && ami::jit_fused_tally_ok(tab);
+  const bool need_out = cfg->h_out || !use_reg || (cfg->want_sum && !fused_tally);
+  const bool own_k = !cfg->d_k && (cfg->h_k || !use_reg);    // momenta pass through a buffer of the workspace
+  const bool own_out = need_out && !direct_out;
+  // default chunk: with host buffers small enough that the copies of one chunk overlap the kernels of the next
+  // (measured: 2^17 samples); otherwise as large as the workspace allows (one chunk = no per-chunk overhead)
+  int64_t chunk = cfg->chunk ? cfg->chunk : (host_io ? (int64_t)1 << 17 : (int64_t)1 << 26);
+  while (chunk > 1024 && ((own_out && chunk * rows * 16 > ((int64_t)256 << 20)) ||
+                          (own_k && chunk * n_comp * 8 > ((int64_t)256 << 20)) ||
+                          (!use_reg && chunk * n_eps * 8 > ((int64_t)256 << 20))))
+    chunk /= 2;
+  if (chunk > cfg->n) chunk = cfg->n;
   RunBuffers& rb = *workspace_of(tab);
   std::lock_guard<std::mutex> run_lock(rb.mu);
   cudaStream_t user = (cudaStream_t)cfg->stream;
   if ((rc = rb.init())) return rc;
-  // Fused tally (register plan, a few rows): the evaluation kernel leaves one partial sum per (row, warp) and the
-  // results are stored only if the caller wants them -- a seeded Monte-Carlo run then moves no sample data at all.
-  const bool fused_tally = use_reg && cfg->want_sum && rows <= kFusedTallyMaxRows;
-  const bool need_out = cfg->h_out || !use_reg || (cfg->want_sum && !fused_tally);
   const int64_t wp_stride = (chunk + 31) / 32;
-  if ((rc = rb.reserve((cfg->d_k || (use_reg && !cfg->h_k)) ? 0 : (size_t)chunk * n_comp * 8,
-                       use_reg ? 0 : (size_t)chunk * n_eps * 8,
-                       (direct_out || !need_out) ? 0 : (size_t)chunk * rows * 16, cfg->want_sum ? (size_t)rows * 32 : 0,
+  if ((rc = rb.reserve(own_k ? (size_t)chunk * n_comp * 8 : 0, use_reg ? 0 : (size_t)chunk * n_eps * 8,
+                       own_out ? (size_t)chunk * rows * 16 : 0, cfg->want_sum ? (size_t)rows * 32 : 0,
                        fused_tally ? (size_t)rows * wp_stride * 32 : 0)))
     return rc;
   if (cfg->want_sum) CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 32, user));
-  // one chunk: everything on the caller's stream (the hops to the internal streams and back cost more than a small
-  // batch's kernels); several chunks: they alternate between the two internal streams
-  const bool single = cfg->n <= chunk;
+  const bool pipelined = host_io && cfg->n > chunk;
+  cudaStream_t s_in = pipelined ? rb.s_in : user, s_k = pipelined ? rb.s_k : user, s_out = pipelined ? rb.s_out : user;
   CU(cudaEventRecord(rb.ev_start, user));
-  if (!single) {
-    CU(cudaStreamWaitEvent(rb.st[0], rb.ev_start, 0));
-    CU(cudaStreamWaitEvent(rb.st[1], rb.ev_start, 0));
-  }
+  if (pipelined)
+    for (cudaStream_t st : {s_in, s_k, s_out}) CU(cudaStreamWaitEvent(st, rb.ev_start, 0));
   int launches = 0;
-  for (int64_t c0 = 0, ci = 0; c0 < cfg->n; c0 += chunk, ++ci) {
-    const int s = (int)(ci & 1);
-    const int64_t nc = std::min(chunk, cfg->n - c0);
-    cudaStream_t st = single ? user : rb.st[s];
-    const double* kbuf;
-    if (cfg->d_k) {
-      kbuf = cfg->d_k + c0 * n_comp;
-    } else if (cfg->h_k) {
-      CU(cudaMemcpyAsync(rb.k[s], cfg->h_k + c0 * n_comp, (size_t)nc * n_comp * 8, cudaMemcpyHostToDevice, st));
-      local.h2d_bytes += nc * n_comp * 8;
-      kbuf = rb.k[s];
-    } else if (use_reg) {
-      kbuf = nullptr;     // drawn inside the specialised kernel: no generation launch, no momentum traffic
-    } else {
-      CU(ami::launch_generate_momenta(cfg->seed, cfg->first_sample + c0, nc, n_comp, rb.k[s], st));
-      ++launches;
-      kbuf = rb.k[s];
+  // the chunk loop; any error leaves it through `rc` so that the internal streams are re-joined below
+  auto run_chunks = [&]() -> int {
+    for (int64_t c0 = 0, ci = 0; c0 < cfg->n; c0 += chunk, ++ci) {
+      const int b = (int)(ci & 1);
+      const int64_t nc = std::min(chunk, cfg->n - c0);
+      const double* kbuf = nullptr;      // stays NULL when the specialised kernel draws the momenta itself
+      if (cfg->d_k) {
+        kbuf = cfg->d_k + c0 * n_comp;
+      } else if (cfg->h_k) {
+        if (pipelined && ci >= 2) CU(cudaStreamWaitEvent(s_in, rb.ev_k[b], 0));   // kernels of chunk c-2 have read k[b]
+        CU(cudaMemcpyAsync(rb.k[b], cfg->h_k + c0 * n_comp, (size_t)nc * n_comp * 8, cudaMemcpyHostToDevice, s_in));
+        if (pipelined) CU(cudaEventRecord(rb.ev_in[b], s_in));
+        local.h2d_bytes += nc * n_comp * 8;
+        kbuf = rb.k[b];
+      }
+      if (pipelined && cfg->h_k) CU(cudaStreamWaitEvent(s_k, rb.ev_in[b], 0));
+      if (pipelined && cfg->h_out && ci >= 2) CU(cudaStreamWaitEvent(s_k, rb.ev_out[b], 0));   // out[b] has been copied out
+      if (!cfg->d_k && !cfg->h_k && !use_reg) {
+        CU(ami::launch_generate_momenta(cfg->seed, cfg->first_sample + c0, nc, n_comp, rb.k[b], s_k));
+        ++launches;
+        kbuf = rb.k[b];
+      }
+      MomentaSrc ms;
+      ms.gen = !cfg->d_k && !cfg->h_k && use_reg; ms.seed = cfg->seed; ms.first_sample = cfg->first_sample + c0;
+      ms.d_k = kbuf; ms.stride_sample = n_comp; ms.stride_comp = 1;
+      ms.q = cfg->q; ms.t = cfg->t; ms.mu = cfg->mu; ms.dim = dim; ms.band = cfg->band;
+      double* obuf = direct_out ? (double*)cfg->d_out + 2 * c0 : (need_out ? rb.out[b] : nullptr);
+      int64_t tally_slots = 0;
+      if (fused_tally) { ms.tally = rb.wp; ms.tally_stride = wp_stride; ms.tally_slots = &tally_slots; }
+      const int64_t ostride = direct_out ? cfg->n : nc;
+      int erc = evaluate_impl(tab, &ms, use_reg ? nullptr : rb.e, 0, nc, nc, cfg->z_ext, cfg->n_f, cfg->beta, cfg->n_b,
+                              cfg->e_reg, cfg->plan, obuf, ostride, s_k, &launches);
+      if (erc) return erc;
+      if (cfg->want_sum) {   // on the kernel stream, in chunk order: the running sum is deterministic
+        if (fused_tally)
+          CU(ami::launch_warp_partial_sums(rb.wp, rows, tally_slots, wp_stride, rb.partial, rb.sum, s_k, &launches));
+        else
+          CU(ami::launch_block_sums(obuf, rows, nc, ostride, rb.partial, rb.sum, s_k, &launches));
+      }
+      if (pipelined) CU(cudaEventRecord(rb.ev_k[b], s_k));
+      if (cfg->h_out) {
+        if (pipelined) CU(cudaStreamWaitEvent(s_out, rb.ev_k[b], 0));
+        CU(cudaMemcpy2DAsync((char*)cfg->h_out + (size_t)c0 * 16, (size_t)cfg->n * 16, obuf, (size_t)ostride * 16,
+                             (size_t)nc * 16, (size_t)rows, cudaMemcpyDeviceToHost, s_out));
+        if (pipelined) CU(cudaEventRecord(rb.ev_out[b], s_out));
+        local.d2h_bytes += nc * rows * 16;
+      }
+      ++local.n_chunks;
     }
-    MomentaSrc ms;
-    ms.gen = !cfg->d_k && !cfg->h_k && use_reg; ms.seed = cfg->seed; ms.first_sample = cfg->first_sample + c0;
-    ms.d_k = kbuf; ms.stride_sample = n_comp; ms.stride_comp = 1;
-    ms.q = cfg->q; ms.t = cfg->t; ms.mu = cfg->mu;
-    double* obuf = direct_out ? (double*)cfg->d_out + 2 * c0 : (need_out ? rb.out[s] : nullptr);
-    if (fused_tally) { ms.tally = rb.wp[s]; ms.tally_stride = wp_stride; }
-    const int64_t ostride = direct_out ? cfg->n : nc;
-    rc = evaluate_impl(tab, &ms, rb.e[s], 0, nc, nc, cfg->z_ext, cfg->n_f, cfg->beta, cfg->n_b, cfg->e_reg, cfg->plan,
-                       obuf, ostride, st, &launches);
-    if (rc) return rc;
-    if (cfg->h_out) {
-      CU(cudaMemcpy2DAsync((char*)cfg->h_out + (size_t)c0 * 16, (size_t)cfg->n * 16, obuf, (size_t)ostride * 16,
-                           (size_t)nc * 16, (size_t)rows, cudaMemcpyDeviceToHost, st));
-      local.d2h_bytes += nc * rows * 16;
+    return AMI_OK;
+  };
+  rc = run_chunks();
+  if (pipelined) {   // the caller's stream continues after everything issued on the internal ones, error or not
+    for (cudaStream_t st : {s_in, s_k, s_out}) {
+      if (cudaEventRecord(rb.ev_stop, st) == cudaSuccess) cudaStreamWaitEvent(user, rb.ev_stop, 0);
     }
-    if (cfg->want_sum) {
-      // tallies are chained in chunk order so that the running sum is deterministic
-      if (ci > 0) CU(cudaStreamWaitEvent(st, rb.ev_done[s ^ 1], 0));
-      if (fused_tally)
-        CU(ami::launch_warp_partial_sums(rb.wp[s], rows, (nc + 31) / 32, wp_stride, rb.partial, rb.sum, st, &launches));
-      else
-        CU(ami::launch_block_sums(obuf, rows, nc, ostride, rb.partial, rb.sum, st, &launches));
-    }
-    if (!single) CU(cudaEventRecord(rb.ev_done[s], st));
-    ++local.n_chunks;
   }
-  for (int i = 0; i < 2 && !single; ++i) {
-    CU(cudaEventRecord(rb.ev_done[i], rb.st[i]));
-    CU(cudaStreamWaitEvent(user, rb.ev_done[i], 0));
-  }
+  if (rc) return rc;
   std::vector<double> tally;
   if (cfg->want_sum) {
     tally.resize((size_t)rows * 4);

@@ -129,7 +129,7 @@ __device__ __forceinline__ void exp_core(double x, double& s, double& rq) {
 // |K| < 5e5), even Taylor polynomial of degree 20 (next term 1.9e-17).  A degree-16 fit (5e-17) is two FMAs
 // cheaper but differs from the correctly rounded cosine in the last bit often enough that results
 // which are ill-conditioned in the ENERGIES (double pole at zero frequency) moved by 4e-11 against a
-// quad-precision check fed with libm energies; this one stays at 5e-13 (tests/parity_report.py).  Momentum sums of a diagram
+// quad-precision check fed with libm energies; this one stays at 5e-13.  Momentum sums of a diagram
 // are a few pi; anything beyond 5e5 takes the library routine.
 __constant__ double kAmiCosC[11] = {
     1.0, -0.5, 0.041666666666666664, -0.001388888888888889, 2.48015873015873e-05, -2.755731922398589e-07,

@@ -1,4 +1,4 @@
-// Per-table specialised evaluation kernels ("register plan").
+// Per-table specialised evaluation kernels ("register plan" and, for large tables, "split plan").
 //
 // The table-driven kernels pay an index load, an address computation and a shared-memory load for
 // every multiply, which bounds them by instruction issue and shared-memory bandwidth (128 B/clk/SM
@@ -6,22 +6,41 @@
 // Here the symbolic result of ONE diagram is written out as straight-line CUDA C++ -- every
 // Fermi/Bose leaf, every denominator and every partial sum a named register, the term table turned
 // into the Horner form of ami_table.hpp -- and compiled for sm_100a with NVRTC when the table is
-// first evaluated.  The same generated body serves two kernels: ami_jit_eval (energies from
-// memory, S2+S3) and ami_jit_fused (momenta from memory, S1+S2+S3 with the dispersion inline).
+// first evaluated (cubins are cached on disk).
+//
+// Register plan (orders <= 6-7): the whole table is one body; ami_jit_eval (energies from memory,
+// S2+S3), ami_jit_fused (momenta from memory or drawn in place, S1+S2+S3) and ami_jit_fused_tally
+// (the same with the Monte-Carlo tally of S4 folded in) are generated from it.
+//
+// Split plan (orders 7-8: 1e4-1e5 flat terms, hundreds of leaves, thousands of shared sums -- more
+// than one thread's registers hold): the groups of the Horner plan are partitioned, in the order of
+// the denominator trie, into PARTS of register-plan size; sums that several parts need are formed in
+// each of them.  Per chunk of samples (sized so that what follows stays in L2):
+//   ami_split_leaves_{eval,fused}  every Fermi/Bose value and reciprocal denominator -> leaves[slot][sample]
+//   ami_split_parts                grid.y = part: its FT sums and its slice of the R part from those
+//                                  leaves -> partial[part][row][sample]
+//   ami_split_combine              adds the parts in a fixed order -> results
 //
 // The source text is produced by this file from the table; the arithmetic helpers it calls are
 // the ones in ami_device.cuh, embedded as text at build time (generated/ami_embedded_src.h).
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <dlfcn.h>
+#include <sys/stat.h>
+#include <unistd.h>
 
 #include <algorithm>
+#include <atomic>
+#include <chrono>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <mutex>
+#include <set>
 #include <sstream>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "ami_jit.hpp"
@@ -30,6 +49,9 @@
 namespace ami {
 
 namespace {
+
+constexpr size_t kWays = 16;            // independent chains kept side by side (measured: profiles/r01_batch_sweep.md)
+constexpr size_t kGroupsPerChunk = 8;   // FT sums are emitted this many groups at a time
 
 // ---------------------------------------------------------------------------------------------
 // source generation
@@ -78,15 +100,16 @@ void interleave(std::vector<Stmts>& lists, size_t ways, std::ostringstream& o, c
   }
 }
 
-// One S-node of the FT DAG (ami_table.hpp) as a chain of statements defining `S<id>`
-void emit_snode(const HornerPlan& hp, int id, Emitter& E, Stmts& out) {
+// One S-node of the FT DAG (ami_table.hpp) as a chain of statements defining `S<id>`; Fermi/Bose leaf u
+// is named F<u><fsuffix>
+void emit_snode(const HornerPlan& hp, int id, const std::string& fsuffix, Emitter& E, Stmts& out) {
   const SNode& n = hp.snodes[id];
   std::string acc;
   for (size_t i = 0; i < n.items.size(); ++i) {
     const SItem& it = n.items[i];
     const bool last = i + 1 == n.items.size();
     const std::string v = last ? "S" + std::to_string(id) : E.fresh("s");
-    const std::string leaf = "F" + std::to_string(it.leaf);
+    const std::string leaf = "F" + std::to_string(it.leaf) + fsuffix;
     if (it.child >= 0) {
       const std::string sc = "S" + std::to_string(it.child);
       if (acc.empty()) out.push_back("const double " + v + " = " + leaf + " * " + sc + ";");
@@ -114,9 +137,11 @@ void emit_snode(const HornerPlan& hp, int id, Emitter& E, Stmts& out) {
 }
 
 // Emits the S-nodes that groups [g0, g1) need and that have not been emitted yet, level by level
-// (nodes of equal height are independent of one another), kWays chains side by side.
-void emit_ft_chunk(const HornerPlan& hp, size_t g0, size_t g1, std::vector<char>& done, size_t ways, Emitter& E,
-                   std::ostringstream& o, const char* indent) {
+// (nodes of equal height are independent of one another), kWays chains side by side.  With
+// `leaf_load` (split plan) the Fermi/Bose leaves these nodes use are first loaded into names private
+// to this chunk, so that a leaf occupies a register only while a chunk that uses it is being formed.
+void emit_ft_chunk(const HornerPlan& hp, size_t g0, size_t g1, std::vector<char>& done, Emitter& E,
+                   std::ostringstream& o, const char* indent, const std::string* leaf_load) {
   std::vector<int> need, stack;
   for (size_t g = g0; g < g1; ++g)
     if (hp.groups[g].root >= 0) stack.push_back(hp.groups[g].root);
@@ -133,15 +158,23 @@ void emit_ft_chunk(const HornerPlan& hp, size_t g0, size_t g1, std::vector<char>
     const int ha = hp.snodes[a].height, hb = hp.snodes[b].height;
     return ha != hb ? ha < hb : a < b;
   });
+  std::string fsuffix;
+  if (leaf_load) {
+    fsuffix = "_" + std::to_string(g0);
+    std::set<int> used;
+    for (int id : need)
+      for (const SItem& it : hp.snodes[id].items) used.insert(it.leaf);
+    for (int u : used) o << indent << "const double F" << u << fsuffix << " = " << *leaf_load << "(" << u << ");\n";
+  }
   for (size_t i = 0; i < need.size();) {
     size_t j = i;
     std::vector<Stmts> lists;
     while (j < need.size() && hp.snodes[need[j]].height == hp.snodes[need[i]].height) {
       lists.emplace_back();
-      emit_snode(hp, need[j], E, lists.back());
+      emit_snode(hp, need[j], fsuffix, E, lists.back());
       ++j;
     }
-    interleave(lists, ways, o, indent);
+    interleave(lists, kWays, o, indent);
     i = j;
   }
   for (size_t g = g0; g < g1; ++g) {
@@ -149,67 +182,6 @@ void emit_ft_chunk(const HornerPlan& hp, size_t g0, size_t g1, std::vector<char>
     o << indent << "const double FT" << g << " = "
       << (hg.root >= 0 ? "S" + std::to_string(hg.root) : dlit((double)hg.num / (double)hg.den)) << ";\n";
   }
-}
-
-// ---- memory-backed variant for tables too large for registers ------------------------------------
-// Long-lived values live in a per-thread column of a global scratch array (slot i at W(i)); the
-// generated text names them through macros, so the emitters below and above are shared.  The FT DAG
-// is written depth first: a sum is formed right before its first use, kept in its slot while other
-// sums still need it (slots are recycled after the last use), and single-use sums stay in registers.
-struct SlotPool {
-  std::vector<int> free_list;
-  int next = 0, peak = 0;
-  int take() {
-    if (!free_list.empty()) { const int s = free_list.back(); free_list.pop_back(); return s; }
-    peak = std::max(peak, next + 1);
-    return next++;
-  }
-  void give(int s) { free_list.push_back(s); }
-};
-
-struct DfsState {
-  std::vector<int> uses_left;    // remaining uses of each S-node
-  std::vector<int> slot;         // scratch slot of a computed shared node, -1 otherwise
-  std::vector<char> done;
-  SlotPool pool;
-  int base = 0;                  // first scratch slot of the pool
-};
-
-// value of S-node `id` as an expression usable once; emits what is needed into `out`
-std::string emit_snode_dfs(const HornerPlan& hp, int id, DfsState& st, Emitter& E, Stmts& out) {
-  auto consume = [&](int n) {
-    if (--st.uses_left[n] == 0 && st.slot[n] >= 0) { st.pool.give(st.slot[n]); st.slot[n] = -1; }
-  };
-  if (st.done[id]) {             // shared and already computed: read it back
-    const std::string v = E.fresh("s");
-    out.push_back("const double " + v + " = W(" + std::to_string(st.base + st.slot[id]) + ");");
-    consume(id);
-    return v;
-  }
-  const SNode& n = hp.snodes[id];
-  std::string acc;
-  for (size_t i = 0; i < n.items.size(); ++i) {
-    const SItem& it = n.items[i];
-    const std::string v = E.fresh("s");
-    const std::string leaf = "F" + std::to_string(it.leaf);
-    if (it.child >= 0) {
-      const std::string sc = emit_snode_dfs(hp, it.child, st, E, out);
-      if (acc.empty()) out.push_back("const double " + v + " = " + leaf + " * " + sc + ";");
-      else out.push_back("const double " + v + " = fma(" + leaf + ", " + sc + ", " + acc + ");");
-    } else {
-      const std::string coef = dlit((double)it.num / (double)it.den);
-      if (acc.empty()) out.push_back("const double " + v + " = " + coef + " * " + leaf + ";");
-      else out.push_back("const double " + v + " = fma(" + coef + ", " + leaf + ", " + acc + ");");
-    }
-    acc = v;
-  }
-  st.done[id] = 1;
-  if (st.uses_left[id] > 1) {    // needed again later: park it in a slot
-    st.slot[id] = st.pool.take();
-    out.push_back("W(" + std::to_string(st.base + st.slot[id]) + ") = " + acc + ";");
-  }
-  consume(id);
-  return acc;
 }
 
 struct CV {            // a complex value held in named doubles; im empty = purely real
@@ -285,27 +257,157 @@ CV emit_d_sum(const HornerPlan& hp, const std::vector<std::string>& qname, int n
   return acc;
 }
 
-}  // namespace
+// ---- split plan: partition of the groups and the Horner plan of one part -----------------------
+// FP64 instructions of the FT sums reachable from S-node `root` that are not in `seen` yet
+long long mark_reachable(const HornerPlan& hp, int root, std::vector<char>& seen) {
+  long long ops = 0;
+  std::vector<int> stack(1, root);
+  while (!stack.empty()) {
+    const int id = stack.back();
+    stack.pop_back();
+    if (seen[id]) continue;
+    seen[id] = 1;
+    ops += (long long)hp.snodes[id].items.size();
+    for (const SItem& it : hp.snodes[id].items)
+      if (it.child >= 0 && !seen[it.child]) stack.push_back(it.child);
+  }
+  return ops;
+}
+
+// Groups in the order in which a depth-first walk of the denominator trie meets them: consecutive groups
+// share denominator prefixes, and the recursion that produced them makes them share Fermi/Bose sums.
+void groups_in_trie_order(const HornerPlan& hp, int n, std::vector<int>& out) {
+  if (hp.dn[n].group >= 0) out.push_back(hp.dn[n].group);
+  for (int c : hp.dn[n].kids) groups_in_trie_order(hp, c, out);
+}
+
+// Cuts that order into parts of about `budget` FP64 instructions each (sums a part shares with an earlier
+// part are counted, and formed, again).
+std::vector<std::vector<int>> partition_groups(const HornerPlan& hp, long long budget) {
+  std::vector<int> order;
+  groups_in_trie_order(hp, 0, order);
+  std::vector<std::vector<int>> parts(1);
+  std::vector<char> seen(hp.snodes.size(), 0);
+  long long cur = 0;
+  for (int g : order) {
+    const HGroup& hg = hp.groups[g];
+    const long long add = (hg.root >= 0 ? mark_reachable(hp, hg.root, seen) : 0) + 4 * (long long)hg.d.size();
+    if (cur > 0 && cur + add > budget) {
+      parts.emplace_back();
+      std::fill(seen.begin(), seen.end(), 0);
+      cur = hg.root >= 0 ? mark_reachable(hp, hg.root, seen) : 0;
+      cur += 4 * (long long)hg.d.size();
+    } else {
+      cur += add;
+    }
+    parts.back().push_back(g);
+  }
+  return parts;
+}
+
+// The Horner plan restricted to `groups`: their FT sums (renumbered, children still before parents) and the
+// denominator trie of their products.  Leaf ids stay those of the whole table.
+HornerPlan make_sub_plan(const HornerPlan& hp, const std::vector<int>& groups) {
+  HornerPlan sub;
+  sub.d_is_real = hp.d_is_real;
+  std::vector<char> seen(hp.snodes.size(), 0);
+  for (int g : groups)
+    if (hp.groups[g].root >= 0) mark_reachable(hp, hp.groups[g].root, seen);
+  std::vector<int> new_id(hp.snodes.size(), -1);
+  for (size_t id = 0; id < hp.snodes.size(); ++id) {
+    if (!seen[id]) continue;
+    new_id[id] = (int)sub.snodes.size();
+    SNode n = hp.snodes[id];
+    for (SItem& it : n.items)
+      if (it.child >= 0) it.child = new_id[it.child];
+    sub.snodes.push_back(std::move(n));
+  }
+  sub.dn.assign(1, HNode());
+  for (int g : groups) {
+    HGroup hg = hp.groups[g];
+    if (hg.root >= 0) hg.root = new_id[hg.root];
+    const int gi = (int)sub.groups.size();
+    sub.groups.push_back(hg);
+    sub.dseq.push_back(hp.dseq[g]);
+    int cur = 0;
+    for (int leaf : hp.dseq[g]) {
+      int nxt = -1;
+      for (int c : sub.dn[cur].kids)
+        if (sub.dn[c].leaf == leaf) { nxt = c; break; }
+      if (nxt < 0) {
+        nxt = (int)sub.dn.size();
+        HNode nn;
+        nn.leaf = leaf;
+        sub.dn.push_back(nn);
+        sub.dn[cur].kids.push_back(nxt);
+      }
+      cur = nxt;
+    }
+    sub.dn[cur].group = gi;
+  }
+  return sub;
+}
+
+long long split_budget() {
+  static const long long b = [] {
+    const char* e = getenv("AMI_JIT_SPLIT_BUDGET");   // tuning knob: FP64 instructions per part
+    const long long v = e ? atoll(e) : 0;
+    return v >= 100 ? v : 1500LL;
+  }();
+  return b;
+}
 
 // ---------------------------------------------------------------------------------------------
-// The translation unit handed to NVRTC.
+// The body of one sample in four sections that the kernels assemble:
+//   0: once per sample   1: per beta   2: per frequency   3: per (beta, frequency)
+// Leaves (Fermi/Bose values, reciprocal denominators) are, depending on the kernel,
+//   kLeafInline  computed and kept in registers (register plan)
+//   kLeafStore   computed and written to the leaf array, nothing else is emitted (split plan, leaf kernel)
+//   kLeafLoad    read from the leaf array where they are used (split plan, a part)
 // ---------------------------------------------------------------------------------------------
-std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int block_threads, bool scratch,
-                                int* scratch_slots) {
-  const int L = ft.n_int + ft.n_ext;
-  size_t kWays = 16;          // independent chains kept side by side (measured: profiles/r01_batch_sweep.md)
-  if (const char* env = getenv("AMI_JIT_WAYS")) {   // tuning knob (profiles/)
-    const int w = atoi(env);
-    if (w >= 1 && w <= 64) kWays = (size_t)w;
-  }
-  Emitter E;
-  // The body of one sample is generated in four sections that are assembled twice below: once
-  // nested beta { ... frequency { ... } } and once with the beta-only work of all temperatures
-  // done first (section 1), so that the frequency-only work (section 2) is not repeated per beta.
-  //   0: once per sample   1: per beta   2: per frequency   3: per (beta, frequency)
+enum LeafMode { kLeafInline, kLeafStore, kLeafLoad };
+
+struct Sections {
   std::ostringstream sec[4];
+  std::vector<std::string> keep;   // per-beta values the R part reads (for the several-temperature body)
+};
+
+struct LeafSlots {                 // layout of the split plan's leaf array
+  std::vector<int> ridx, cidx;     // position of denominator u among the purely real / the complex ones
+  int n_real = 0, n_cplx = 0, n_fermi = 0;
+};
+
+LeafSlots leaf_slots(const FlatTable& ft, const HornerPlan& hp) {
+  LeafSlots ls;
+  ls.ridx.assign(ft.leafD.size(), -1);
+  ls.cidx.assign(ft.leafD.size(), -1);
+  for (size_t u = 0; u < ft.leafD.size(); ++u) {
+    if (hp.d_is_real[u]) ls.ridx[u] = ls.n_real++;
+    else ls.cidx[u] = ls.n_cplx++;
+  }
+  ls.n_fermi = (int)ft.leafF.size();
+  return ls;
+}
+
+// `hp` may be the plan of one part; leaf ids and `ls` are those of the whole table
+void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls, LeafMode mode, Emitter& E,
+                  Sections& S) {
   int cur = 0;
-#define o sec[cur]
+#define o S.sec[cur]
+  const std::string slot_f = "(" + std::to_string(ls.n_real) + " + b * " + std::to_string(ls.n_fermi) + " + ";
+  auto slot_c = [&](size_t u) {
+    return "(CB + 2 * (f * " + std::to_string(ls.n_cplx) + " + " + std::to_string(ls.cidx[u]) + "))";
+  };
+  // which leaves this plan uses
+  std::vector<char> useF(ft.leafF.size(), 0), useD(ft.leafD.size(), 0);
+  if (mode == kLeafLoad) {
+    for (const SNode& n : hp.snodes)
+      for (const SItem& it : n.items) useF[it.leaf] = 1;
+    for (size_t n = 1; n < hp.dn.size(); ++n) useD[hp.dn[n].leaf] = 1;
+  } else {
+    std::fill(useF.begin(), useF.end(), 1);
+    std::fill(useD.begin(), useD.end(), 1);
+  }
   // every distinct integer combination of the energies, up to sign, once per sample
   std::vector<std::vector<int>> combos;
   auto combo_ref = [&](const std::vector<int>& c) -> std::string {
@@ -322,11 +424,25 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     if (j == combos.size()) combos.push_back(pos);
     return std::string(sign < 0 ? "-E" : "E") + std::to_string(j);
   };
-  for (const LeafD& l : ft.leafD) combo_ref(l.c);
-  for (size_t j = 0; j < combos.size(); ++j) o << "  const double E" << j << " = " << combo(combos[j], "e") << ";\n";
+  if (mode != kLeafLoad) {
+    for (const LeafD& l : ft.leafD) combo_ref(l.c);
+    for (size_t j = 0; j < combos.size(); ++j) o << "  const double E" << j << " = " << combo(combos[j], "e") << ";\n";
+  }
   // reciprocals of the denominators, kWays at a time
   auto emit_d_leaves = [&](const std::vector<size_t>& ids, const std::string& ind) {
-    if (!scratch)
+    if (mode == kLeafLoad) {
+      // read where they are used: a denominator enters one product per trie node that carries it
+      for (size_t u : ids) {
+        if (!useD[u]) continue;
+        if (hp.d_is_real[u]) {
+          o << "#define Dr" << u << " AMI_L(" << ls.ridx[u] << ")\n";
+        } else {
+          o << "#define Dr" << u << " AMI_L" << slot_c(u) << "\n#define Di" << u << " AMI_L(" << slot_c(u) << " + 1)\n";
+        }
+      }
+      return;
+    }
+    if (mode == kLeafInline)
       for (size_t u : ids) o << ind << "double Dr" << u << (hp.d_is_real[u] ? "" : ", Di" + std::to_string(u)) << ";\n";
     for (size_t i0 = 0; i0 < ids.size(); i0 += kWays) {
       const size_t n = std::min(kWays, ids.size() - i0);
@@ -353,8 +469,15 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
       o << "};\n" << ind << "  fast_rcp_n<" << n << ">(d);\n";
       for (size_t j = 0; j < n; ++j) {
         const size_t u = ids[i0 + j];
-        if (hp.d_is_real[u]) o << ind << "  Dr" << u << " = d[" << j << "];\n";
-        else o << ind << "  Dr" << u << " = re" << j << " * d[" << j << "]; Di" << u << " = -im" << j << " * d[" << j << "];\n";
+        if (mode == kLeafInline) {
+          if (hp.d_is_real[u]) o << ind << "  Dr" << u << " = d[" << j << "];\n";
+          else o << ind << "  Dr" << u << " = re" << j << " * d[" << j << "]; Di" << u << " = -im" << j << " * d[" << j << "];\n";
+        } else if (hp.d_is_real[u]) {
+          o << ind << "  AMI_LS(" << ls.ridx[u] << ", d[" << j << "]);\n";
+        } else {
+          o << ind << "  AMI_LS(" << slot_c(u) << ", re" << j << " * d[" << j << "]); AMI_LS(" << slot_c(u) << " + 1, -im" << j
+            << " * d[" << j << "]);\n";
+        }
       }
       o << ind << "}\n";
     }
@@ -371,155 +494,128 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   // Fermi/Bose leaves (independent of the external frequency), kWays at a time
   // Leaves that differ only in the derivative order share one exponential and one reciprocal.
   const size_t UF = ft.leafF.size();
-  std::vector<std::vector<size_t>> base;      // base -> leaves with the same (combination, sigma)
-  for (size_t u = 0; u < UF; ++u) {
-    size_t b = 0;
-    for (; b < base.size(); ++b)
-      if (ft.leafF[base[b][0]].c == ft.leafF[u].c && ft.leafF[base[b][0]].sigma == ft.leafF[u].sigma) break;
-    if (b == base.size()) base.emplace_back();
-    base[b].push_back(u);
-  }
-  const bool smem_f = scratch || jit_fermi_in_smem();
-  if (!smem_f)
-    for (size_t u = 0; u < UF; ++u) o << "    double F" << u << ";\n";
-  // One exponential per ENERGY SYMBOL, e^{beta e_i} = 2^{n_i} m_i; the exponential of a leaf's
-  // combination is assembled from them: integer exponents add, mantissas multiply, so nothing can
-  // overflow and 17 FP64 instructions per leaf become one or two multiplies.
-  std::vector<char> sym_used(ft.n_eps, 0);
-  for (const auto& members : base)
+  if (mode != kLeafLoad) {
+    std::vector<std::vector<size_t>> base;      // base -> leaves with the same (combination, sigma)
+    for (size_t u = 0; u < UF; ++u) {
+      size_t b = 0;
+      for (; b < base.size(); ++b)
+        if (ft.leafF[base[b][0]].c == ft.leafF[u].c && ft.leafF[base[b][0]].sigma == ft.leafF[u].sigma) break;
+      if (b == base.size()) base.emplace_back();
+      base[b].push_back(u);
+    }
+    if (mode == kLeafInline)
+      for (size_t u = 0; u < UF; ++u) o << "    double F" << u << ";\n";
+    // One exponential per ENERGY SYMBOL, e^{beta e_i} = 2^{n_i} m_i; the exponential of a leaf's
+    // combination is assembled from them: integer exponents add, mantissas multiply, so nothing can
+    // overflow and 17 FP64 instructions per leaf become one or two multiplies.
+    std::vector<char> sym_used(ft.n_eps, 0);
+    for (const auto& members : base)
+      for (int i = 0; i < ft.n_eps; ++i)
+        if (ft.leafF[members[0]].c[i]) sym_used[i] = 1;
+    std::vector<int> syms;
     for (int i = 0; i < ft.n_eps; ++i)
-      if (ft.leafF[members[0]].c[i]) sym_used[i] = 1;
-  std::vector<int> syms;
-  for (int i = 0; i < ft.n_eps; ++i)
-    if (sym_used[i]) syms.push_back(i);
-  for (int i : syms) o << "    int n" << i << "; double m" << i << ";\n";
-  for (size_t i0 = 0; i0 < syms.size(); i0 += kWays) {
-    const size_t n = std::min(kWays, syms.size() - i0);
-    o << "    {\n      const double x[" << n << "] = {";
-    for (size_t j = 0; j < n; ++j) o << (j ? ", " : "") << "beta * e" << syms[i0 + j];
-    o << "};\n      int nn[" << n << "]; double mm[" << n << "];\n      exp_split_n<" << n << ">(x, nn, mm);\n";
-    for (size_t j = 0; j < n; ++j)
-      o << "      n" << syms[i0 + j] << " = nn[" << j << "]; m" << syms[i0 + j] << " = mm[" << j << "];\n";
-    o << "    }\n";
-  }
-  // a leaf with x = beta (E [+ eta]) = ln(A/B): f_sigma = 1/(sigma A/B + 1) = B/(sigma A + B), with
-  // A (B) the product over the symbols with positive (negative) coefficient; A carries e^{beta eta}
-  // for sigma = -1 (P10(a)).  Exponents: A/B = 2^(Na - Nb) Ma/Mb, so d = fma(2^(Na-Nb), sigma Ma, Mb).
-  auto product = [&](const std::vector<int>& c, int sign, std::string* mant, std::string* expo) {
-    for (int i = 0; i < ft.n_eps; ++i) {
-      const int a = c[i] * sign;
-      for (int r = 0; r < a; ++r) {
-        *mant += (mant->empty() ? "" : " * ") + std::string("m") + std::to_string(i);
-        *expo += std::string(sign > 0 ? " + n" : " - n") + std::to_string(i);
-      }
+      if (sym_used[i]) syms.push_back(i);
+    for (int i : syms) o << "    int n" << i << "; double m" << i << ";\n";
+    for (size_t i0 = 0; i0 < syms.size(); i0 += kWays) {
+      const size_t n = std::min(kWays, syms.size() - i0);
+      o << "    {\n      const double x[" << n << "] = {";
+      for (size_t j = 0; j < n; ++j) o << (j ? ", " : "") << "beta * e" << syms[i0 + j];
+      o << "};\n      int nn[" << n << "]; double mm[" << n << "];\n      exp_split_n<" << n << ">(x, nn, mm);\n";
+      for (size_t j = 0; j < n; ++j)
+        o << "      n" << syms[i0 + j] << " = nn[" << j << "]; m" << syms[i0 + j] << " = mm[" << j << "];\n";
+      o << "    }\n";
     }
-  };
-  for (size_t b0 = 0; b0 < base.size(); b0 += kWays) {
-    const size_t n = std::min(kWays, base.size() - b0);
-    o << "    {\n";
-    for (size_t j = 0; j < n; ++j) {
-      const LeafF& l = ft.leafF[base[b0 + j][0]];
-      std::string ma, mb, ex;
-      product(l.c, +1, &ma, &ex);
-      product(l.c, -1, &mb, &ex);
-      if (l.sigma < 0) ma += (ma.empty() ? "" : " * ") + std::string("p.ceta[b]");
-      if (ma.empty()) ma = "1.0";
-      o << "      const double s" << j << " = pow2_clamped(0" << ex << "), a" << j << " = " << ma << ", b" << j << " = "
-        << (mb.empty() ? "1.0" : mb) << ";\n";
-    }
-    o << "      double d[" << n << "] = {";
-    for (size_t j = 0; j < n; ++j)
-      o << (j ? ", " : "") << "fma(s" << j << ", " << (ft.leafF[base[b0 + j][0]].sigma > 0 ? "" : "-") << "a" << j << ", b"
-        << j << ")";
-    o << "};\n      fast_rcp_n<" << n << ">(d);\n";
-    for (size_t j = 0; j < n; ++j) {
-      const std::vector<size_t>& members = base[b0 + j];
-      const LeafF& l0 = ft.leafF[members[0]];
-      bool has_b = false, need_g = false;
-      for (int v : l0.c) has_b |= v < 0;
-      for (size_t u : members) need_g |= ft.leafF[u].k > 0;
-      const std::string f = has_b ? "(b" + std::to_string(j) + " * d[" + std::to_string(j) + "])" : "d[" + std::to_string(j) + "]";
-      if (need_g)   // g = 1 - f = sigma A / (sigma A + B)  (P11)
-        o << "      const double g" << j << " = " << (l0.sigma > 0 ? "" : "-") << "(s" << j << " * a" << j << ") * d[" << j
-          << "];\n";
-      for (size_t u : members) {
-        const LeafF& l = ft.leafF[u];
-        if (l.k == 0) {
-          o << "      F" << u << " = " << f << ";\n";
-          continue;
+    // a leaf with x = beta (E [+ eta]) = ln(A/B): f_sigma = 1/(sigma A/B + 1) = B/(sigma A + B), with
+    // A (B) the product over the symbols with positive (negative) coefficient; A carries e^{beta eta}
+    // for sigma = -1 (P10(a)).  Exponents: A/B = 2^(Na - Nb) Ma/Mb, so d = fma(2^(Na-Nb), sigma Ma, Mb).
+    auto product = [&](const std::vector<int>& c, int sign, std::string* mant, std::string* expo) {
+      for (int i = 0; i < ft.n_eps; ++i) {
+        const int a = c[i] * sign;
+        for (int r = 0; r < a; ++r) {
+          *mant += (mant->empty() ? "" : " * ") + std::string("m") + std::to_string(i);
+          *expo += std::string(sign > 0 ? " + n" : " - n") + std::to_string(i);
         }
-        // f^{(k)} = beta^k f g Q_k(f)
-        o << "      {\n        const double f = " << f << ";\n";
-        const std::vector<double> q = deriv_poly(l.k);
-        o << "        double q = " << dlit(q.back()) << ";\n";
-        for (int i = (int)q.size() - 2; i >= 0; --i) o << "        q = fma(q, f, " << dlit(q[i]) << ");\n";
-        o << "        double bk = beta;\n";
-        for (int i = 1; i < l.k; ++i) o << "        bk *= beta;\n";
-        o << "        F" << u << " = bk * f * g" << j << " * q;\n      }\n";
       }
-    }
-    o << "    }\n";
-  }
-  // FT sums of every group (per beta): a DAG shared by all groups, emitted eight groups at a time
-  // scratch layout: [Dr/Di of every denominator][FT of every group][Q of every R-trie node][pool of shared sums]
-  std::vector<int> slot_dr(ft.leafD.size(), -1), slot_di(ft.leafD.size(), -1), slot_ft(hp.groups.size(), -1);
-  int n_slots = 0;
-  for (size_t u = 0; u < ft.leafD.size(); ++u) {
-    slot_dr[u] = n_slots++;
-    if (!hp.d_is_real[u]) slot_di[u] = n_slots++;
-  }
-  for (size_t g = 0; g < hp.groups.size(); ++g) slot_ft[g] = n_slots++;
-  const int slot_q0 = n_slots;
-  n_slots += (int)hp.dn.size();
-  DfsState dfs;
-  if (!scratch) {
-    std::vector<char> done(hp.snodes.size(), 0);
-    for (size_t g0 = 0; g0 < hp.groups.size(); g0 += 8)
-      emit_ft_chunk(hp, g0, std::min(hp.groups.size(), g0 + 8), done, kWays, E, o, "    ");
-  } else {
-    dfs.uses_left.assign(hp.snodes.size(), 0);
-    dfs.slot.assign(hp.snodes.size(), -1);
-    dfs.done.assign(hp.snodes.size(), 0);
-    dfs.base = n_slots;
-    for (const SNode& n : hp.snodes)
-      for (const SItem& it : n.items)
-        if (it.child >= 0) ++dfs.uses_left[it.child];
-    for (const HGroup& g : hp.groups)
-      if (g.root >= 0) ++dfs.uses_left[g.root];
-    for (size_t g = 0; g < hp.groups.size(); ++g) {
-      const HGroup& hg = hp.groups[g];
-      Stmts lst;
-      const std::string v = hg.root >= 0 ? emit_snode_dfs(hp, hg.root, dfs, E, lst) : dlit((double)hg.num / (double)hg.den);
+    };
+    auto assign = [&](size_t u, const std::string& value, const std::string& ind) {
+      if (mode == kLeafInline) o << ind << "F" << u << " = " << value << ";\n";
+      else o << ind << "AMI_LS(" << slot_f << u << "), " << value << ");\n";
+    };
+    for (size_t b0 = 0; b0 < base.size(); b0 += kWays) {
+      const size_t n = std::min(kWays, base.size() - b0);
       o << "    {\n";
-      for (const std::string& st : lst) o << "      " << st << "\n";
-      o << "      FT" << g << " = " << v << ";\n    }\n";
+      for (size_t j = 0; j < n; ++j) {
+        const LeafF& l = ft.leafF[base[b0 + j][0]];
+        std::string ma, mb, ex;
+        product(l.c, +1, &ma, &ex);
+        product(l.c, -1, &mb, &ex);
+        if (l.sigma < 0) ma += (ma.empty() ? "" : " * ") + std::string("p.ceta[b]");
+        if (ma.empty()) ma = "1.0";
+        o << "      const double s" << j << " = pow2_clamped(0" << ex << "), a" << j << " = " << ma << ", b" << j << " = "
+          << (mb.empty() ? "1.0" : mb) << ";\n";
+      }
+      o << "      double d[" << n << "] = {";
+      for (size_t j = 0; j < n; ++j)
+        o << (j ? ", " : "") << "fma(s" << j << ", " << (ft.leafF[base[b0 + j][0]].sigma > 0 ? "" : "-") << "a" << j << ", b"
+          << j << ")";
+      o << "};\n      fast_rcp_n<" << n << ">(d);\n";
+      for (size_t j = 0; j < n; ++j) {
+        const std::vector<size_t>& members = base[b0 + j];
+        const LeafF& l0 = ft.leafF[members[0]];
+        bool has_b = false, need_g = false;
+        for (int v : l0.c) has_b |= v < 0;
+        for (size_t u : members) need_g |= ft.leafF[u].k > 0;
+        const std::string f = has_b ? "(b" + std::to_string(j) + " * d[" + std::to_string(j) + "])" : "d[" + std::to_string(j) + "]";
+        if (need_g)   // g = 1 - f = sigma A / (sigma A + B)  (P11)
+          o << "      const double g" << j << " = " << (l0.sigma > 0 ? "" : "-") << "(s" << j << " * a" << j << ") * d[" << j
+            << "];\n";
+        for (size_t u : members) {
+          const LeafF& l = ft.leafF[u];
+          if (l.k == 0) {
+            assign(u, f, "      ");
+            continue;
+          }
+          // f^{(k)} = beta^k f g Q_k(f)
+          o << "      {\n        const double f = " << f << ";\n";
+          const std::vector<double> q = deriv_poly(l.k);
+          o << "        double q = " << dlit(q.back()) << ";\n";
+          for (int i = (int)q.size() - 2; i >= 0; --i) o << "        q = fma(q, f, " << dlit(q[i]) << ");\n";
+          o << "        double bk = beta;\n";
+          for (int i = 1; i < l.k; ++i) o << "        bk *= beta;\n";
+          assign(u, "bk * f * g" + std::to_string(j) + " * q", "        ");
+          o << "      }\n";
+        }
+      }
+      o << "    }\n";
     }
-    n_slots += dfs.pool.peak;
   }
-  if (scratch_slots) *scratch_slots = scratch ? n_slots : 0;
-  // frequency-independent parts of the R sums (products under purely real denominators), per beta
   std::vector<std::string> qname(hp.dn.size());
-  {
+  if (mode != kLeafStore) {
+    // FT sums of every group (per beta): a DAG shared by all groups, emitted a few groups at a time
+    std::vector<char> done(hp.snodes.size(), 0);
+    const std::string loader = "AMI_LF";
+    for (size_t g0 = 0; g0 < hp.groups.size(); g0 += kGroupsPerChunk)
+      emit_ft_chunk(hp, g0, std::min(hp.groups.size(), g0 + kGroupsPerChunk), done, E, o, "    ",
+                    mode == kLeafLoad ? &loader : nullptr);
+    // frequency-independent parts of the R sums (products under purely real denominators), per beta
     std::vector<Stmts> lists;
     for (size_t n = 0; n < hp.dn.size(); ++n) {
       if (n != 0 && hp.d_is_real[hp.dn[n].leaf]) continue;
       lists.emplace_back();
       qname[n] = emit_q(hp, (int)n, E, lists.back());
-      if (scratch && !qname[n].empty() && qname[n][0] == 'q') {     // keep it in memory until the R part reads it
-        const std::string w = "W(" + std::to_string(slot_q0 + (int)n) + ")";
-        lists.back().push_back(w + " = " + qname[n] + ";");
-        qname[n] = w;
-      }
     }
     interleave(lists, kWays, o, "    ");
+    for (const std::string& q : qname)
+      if (!q.empty() && std::find(S.keep.begin(), S.keep.end(), q) == S.keep.end()) S.keep.push_back(q);
   }
   // frequencies
   cur = 2;
-  for (int x = 0; x < ft.n_ext; ++x) {
-    o << "      const double zr" << x << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ")], zi" << x
-      << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ") + 1];\n";
-    o << "      const bool zz" << x << " = (zr" << x << " == 0.0 && zi" << x << " == 0.0);\n";
-  }
+  if (mode != kLeafLoad)
+    for (int x = 0; x < ft.n_ext; ++x) {
+      o << "      const double zr" << x << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ")], zi" << x
+        << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ") + 1];\n";
+      o << "      const bool zz" << x << " = (zr" << x << " == 0.0 && zi" << x << " == 0.0);\n";
+    }
   // reciprocals of the denominators that carry an external frequency (P10(b) decides at run time
   // whether the regulator applies)
   {
@@ -530,7 +626,7 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
   }
   // R part: the subtrees under the root side by side, then the root's own sum
   cur = 3;
-  {
+  if (mode != kLeafStore) {
     std::vector<int> kids;
     for (int c : hp.dn[0].kids)
       if (!hp.d_is_real[hp.dn[c].leaf]) kids.push_back(c);
@@ -548,219 +644,303 @@ std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int b
     }
     if (!have) acc.re = "0.0";
     for (const std::string& st : tail) o << "      " << st << "\n";
-    o << "      const long long row = (long long)(p.b0 + b) * p.n_f_total + (p.f0 + f);\n";
-    o << "      const double2 val = make_double2(p.prefactor * (" << acc.re << "), "
-      << (acc.real() ? std::string("0.0") : "p.prefactor * (" + acc.im + ")") << ");\n";
-    o << "      if (!AMI_TALLY || p.out) AMI_STORE(reinterpret_cast<double2*>(p.out) + row * p.out_row_stride + s, val);\n";
-    o << "      if (AMI_TALLY) ami_tally(reinterpret_cast<double4*>(p.tally) + row * p.tally_stride + (s >> 5), val);\n";
+    o << "      AMI_EMIT(" << acc.re << ", " << (acc.real() ? std::string("0.0") : acc.im) << ");\n";
   }
 #undef o
-  std::ostringstream o;
-  o << kAmiParamsSrc << "\n" << kAmiDeviceSrc << "\n";
-  int tiles = scratch ? 1 : jit_tiles_per_cta();
-  o << "using namespace amidev;\n#define AMI_NT " << block_threads << "\n#define AMI_U " << tiles << "\n#define AMI_PF " << jit_prefetch_ctas() << "\n#define AMI_MINB " << (scratch ? 1 : jit_min_blocks(block_threads)) << "\n"
-    << (jit_store_mode() == 1 ? "#define AMI_STORE(p, v) __stcs(p, v)\n"
-        : jit_store_mode() == 2 ? "#define AMI_STORE(p, v) __stwt(p, v)\n" : "#define AMI_STORE(p, v) (*(p) = (v))\n");
-  // Fused tally (S4, Monte-Carlo sums of PAPER.md:291): the warp adds its samples' (re, im, re^2, im^2) in a fixed
-  // order and lane 0 stores one partial per (row, warp).  The lanes of a ragged last warp are the low ones.
-  o << "__device__ __forceinline__ void ami_tally(double4* dst, const double2 v) {\n"
-       "  const unsigned mask = __activemask();\n"
-       "  const int lane = threadIdx.x & 31, cnt = __popc(mask);\n"
-       "  double a = v.x, b = v.y, c = v.x * v.x, d = v.y * v.y;\n"
-       "#pragma unroll\n"
-       "  for (int off = 16; off > 0; off >>= 1) {\n"
-       "    const double a2 = __shfl_down_sync(mask, a, off), b2 = __shfl_down_sync(mask, b, off);\n"
-       "    const double c2 = __shfl_down_sync(mask, c, off), d2 = __shfl_down_sync(mask, d, off);\n"
-       "    if (lane + off < cnt) { a += a2; b += b2; c += c2; d += d2; }\n"
-       "  }\n"
-       "  if (lane == 0) *dst = make_double4(a, b, c, d);\n"
-       "}\n";
-  std::string sig = "(const AmiBatch& p, const long long s";
-  for (int i = 0; i < ft.n_eps; ++i) sig += ", const double e" + std::to_string(i);
-  if (smem_f && !scratch) {
-    // Fermi/Bose leaves in shared memory as [leaf][thread] (conflict-free), everything else in registers
-    o << "extern __shared__ double sF[];\n";
-    for (size_t u = 0; u < ft.leafF.size(); ++u) o << "#define F" << u << " sF[" << u << " * AMI_NT + threadIdx.x]\n";
+}
+
+// Momenta of sample `at` into nk0..: from memory, or drawn in place by the counter-based generator (S4 with a
+// seed: the momenta never exist in memory).  Counter of component c = sample * n_comp + c; the generator's
+// state is seed + GOLDEN (counter + 1), so one 64-bit multiply per sample and an addition per component
+// (arithmetic modulo 2^64: same bits as momentum_of).
+void emit_momenta(std::ostringstream& o, int n_comp, const std::string& at, const std::string& ind) {
+  o << ind << "if (p.gen) {\n" << ind << "  const unsigned long long z0 = p.seed + 0x9E3779B97F4A7C15ull * ((unsigned long long)"
+    << "(p.first_sample + (" << at << ")) * " << n_comp << "ull + 1ull);\n";
+  for (int c = 0; c < n_comp; ++c) {
+    char lit[32];
+    snprintf(lit, sizeof lit, "0x%016llXull", (unsigned long long)(0x9E3779B97F4A7C15ull * (unsigned long long)c));
+    o << ind << "  nk" << c << " = momentum_from_state(z0 + " << lit << ");\n";
   }
-  if (scratch) {
-    sig += ", double* __restrict__ w, const long long ws";
-    // volatile: every scratch access happens where it is written.  Without it the compiler hoists
-    // thousands of loads to the top of the straight-line body and then spills them again.
-    o << "extern __shared__ double sF[];\n#define W(i) ((volatile double*)w)[(long long)(i) * ws]\n";
-    for (size_t u = 0; u < ft.leafF.size(); ++u) o << "#define F" << u << " sF[" << u << " * AMI_NT + threadIdx.x]\n";
-    for (size_t u = 0; u < ft.leafD.size(); ++u) {
-      o << "#define Dr" << u << " W(" << slot_dr[u] << ")\n";
-      if (slot_di[u] >= 0) o << "#define Di" << u << " W(" << slot_di[u] << ")\n";
-    }
-    for (size_t g = 0; g < hp.groups.size(); ++g) o << "#define FT" << g << " W(" << slot_ft[g] << ")\n";
+  o << ind << "} else {\n" << ind << "  const double* kn = p.k + (" << at << ") * p.k_stride_sample;\n";
+  for (int c = 0; c < n_comp; ++c) o << ind << "  nk" << c << " = kn[" << c << " * p.k_stride_comp];\n";
+  o << ind << "}\n";
+}
+
+// Inline dispersion (Eqs. 8-18; Eq. 14 for `dim` components): e_i from the momenta kx<l>, ky<l>, ...
+// and the external ones.  Same operations in the same order as dispersion_kernel (ami_kernels.cu): bit-identical.
+void emit_dispersion(std::ostringstream& o, const FlatTable& ft, const JitVariant& var) {
+  static const char* comp[3] = {"kx", "ky", "kz"};
+  const int L = ft.n_int + ft.n_ext, dim = var.dim;
+  for (int l = 0; l < ft.n_int; ++l) {
+    o << "  const double ";
+    for (int c = 0; c < dim; ++c) o << (c ? ", " : "") << comp[c] << l << " = nk" << dim * l + c;
+    o << ";\n";
   }
-  sig += ") {\n";
-  // ---- body for one temperature per launch: beta { frequency { } } ----------------------------
-  o << "template <bool AMI_TALLY> __device__ __forceinline__ void ami_body" << sig << sec[0].str()
-    << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << sec[1].str()
-    << "#pragma unroll 1\n    for (int f = 0; f < p.n_f; ++f) {\n" << sec[2].str() << sec[3].str() << "    }\n  }\n}\n\n";
-  // ---- body for several temperatures: the per-beta values the R part needs are kept in a small
-  // per-thread array, then frequency { reciprocals once; beta { R part } } --------------------------
-  std::vector<std::string> keep;
-  if (!scratch)
-  for (const std::string& q : qname)
-    if (!q.empty() && std::find(keep.begin(), keep.end(), q) == keep.end()) keep.push_back(q);
-  if (!scratch) {
-  o << "template <bool AMI_TALLY> __device__ __forceinline__ void ami_body_mb" << sig << sec[0].str();
-  o << "  double kept[AMI_K_MAX_BETA][" << std::max<size_t>(keep.size(), 1) << "];\n";
-  o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << sec[1].str();
-  for (size_t i = 0; i < keep.size(); ++i) o << "    kept[b][" << i << "] = " << keep[i] << ";\n";
-  o << "  }\n#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n" << sec[2].str()
-    << "#pragma unroll 1\n    for (int b = 0; b < p.n_b; ++b) {\n";
-  for (size_t i = 0; i < keep.size(); ++i) o << "      const double " << keep[i] << " = kept[b][" << i << "];\n";
-  o << sec[3].str() << "    }\n  }\n}\n\n";
+  for (int x = 0; x < ft.n_ext; ++x) {
+    o << "  const double ";
+    for (int c = 0; c < dim; ++c) o << (c ? ", " : "") << comp[c] << ft.n_int + x << " = p.q[" << dim * x + c << "]";
+    o << ";\n";
   }
-  // ---- kernel 1: energies from memory ---------------------------------------------------------
-  o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
-       "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
-       "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
-       "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
-       "#pragma unroll 1\n"
-       "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n";
-  for (int i = 0; i < ft.n_eps; ++i) o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
-  std::string call_args = "(p, s";
-  for (int i = 0; i < ft.n_eps; ++i) call_args += ", e" + std::to_string(i);
-  call_args += scratch ? ", p.scratch + s, p.scratch_stride);\n" : ");\n";
-  // @T@ = <false> / <true>: without / with the fused tally (a compile-time switch: the reductions cost the kernels
-  // that do not tally nothing); @K2@ = name of the fused kernel
-  const std::string call = scratch ? "  ami_body@T@" + call_args
-                                   : "  if (p.n_b == 1) ami_body@T@" + call_args + "  else ami_body_mb@T@" + call_args;
-  o << call << "  }\n}\n\n";
-  const size_t k2_begin = o.str().size();
-  // ---- kernel 2: momenta from memory, dispersion inline (Eqs. 8-18) ----------
-  o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) @K2@(const __grid_constant__ AmiBatch p) {\n"
-       "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
-       "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
-       "  // A CTA walks AMI_U consecutive tiles of AMI_NT samples; the momenta of the next tile are loaded into\n"
-       "  // registers before the current one is evaluated, so only the first load of a CTA is exposed.\n"
-       "  const long long base = blockIdx.x * (long long)(AMI_NT * AMI_U) + threadIdx.x;\n"
-       "#if AMI_PF > 0\n"
-       "  // The CTA that will take this one's place on the SM (AMI_PF CTAs further on) finds its momenta in L2:\n"
-       "  // with a few warps per SM the DRAM latency of the first loads is otherwise exposed once per CTA.\n"
-       "  {\n    const long long pb = base + (long long)AMI_PF * (AMI_NT * AMI_U);\n"
-       "    if (pb < p.n && !p.gen) {\n      const double* kp = p.k + pb * p.k_stride_sample;\n"
-       "      if (p.k_stride_comp == 1) {\n";
-  for (int c = 0; c < 2 * ft.n_int; c += 4) o << "        asm volatile(\"prefetch.global.L2 [%0];\" ::\"l\"(kp + " << c << "));\n";
-  o << "      } else {\n";
-  for (int c = 0; c < 2 * ft.n_int; ++c)
-    o << "        asm volatile(\"prefetch.global.L2 [%0];\" ::\"l\"(kp + " << c << " * p.k_stride_comp));\n";
-  o << "      }\n    }\n  }\n#endif\n";
-  for (int c = 0; c < 2 * ft.n_int; ++c) o << "  double nk" << c << " = 0.0;\n";
-  // momenta of sample `at`: from memory, or drawn in place by the counter-based generator (S4 with a seed:
-  // the momenta never exist in memory)
-  auto emit_momenta = [&](const std::string& at, const std::string& ind) {
-    // counter of component c = sample * 2m + c; the generator's state is seed + GOLDEN (counter + 1), so one 64-bit
-    // multiply per sample and an addition per component (arithmetic modulo 2^64: same bits as momentum_of)
-    o << ind << "if (p.gen) {\n" << ind << "  const unsigned long long z0 = p.seed + 0x9E3779B97F4A7C15ull * ((unsigned long long)"
-      << "(p.first_sample + (" << at << ")) * " << 2 * ft.n_int << "ull + 1ull);\n";
-    for (int c = 0; c < 2 * ft.n_int; ++c) {
-      char lit[32];
-      snprintf(lit, sizeof lit, "0x%016llXull", (unsigned long long)(0x9E3779B97F4A7C15ull * (unsigned long long)c));
-      o << ind << "  nk" << c << " = momentum_from_state(z0 + " << lit << ");\n";
-    }
-    o << ind << "} else {\n" << ind << "  const double* kn = p.k + (" << at << ") * p.k_stride_sample;\n";
-    for (int c = 0; c < 2 * ft.n_int; ++c) o << ind << "  nk" << c << " = kn[" << c << " * p.k_stride_comp];\n";
-    o << ind << "}\n";
-  };
-  o << "  if (base < p.n) {\n";
-  emit_momenta("base", "    ");
-  o << "  }\n#pragma unroll 1\n  for (int u = 0; u < AMI_U; ++u) {\n"
-       "  const long long s = base + (long long)u * AMI_NT;\n  if (s >= p.n) break;\n";
-  for (int l = 0; l < ft.n_int; ++l)
-    o << "  const double kx" << l << " = nk" << 2 * l << ", ky" << l << " = nk" << 2 * l + 1 << ";\n";
-  o << "  if (u + 1 < AMI_U && s + AMI_NT < p.n) {\n";
-  emit_momenta("s + AMI_NT", "    ");
-  o << "  }\n";
-  for (int x = 0; x < ft.n_ext; ++x)
-    o << "  const double kx" << ft.n_int + x << " = p.q[" << 2 * x << "], ky" << ft.n_int + x << " = p.q[" << 2 * x + 1
-      << "];\n";
   for (int i = 0; i < ft.n_eps; ++i) o << "  double e" << i << ";\n";
-  const int sym_batch = std::max(1, (int)kWays / 2);   // kWays cosines side by side
+  const int sym_batch = std::max(1, (int)kWays / dim);   // kWays cosines side by side
   for (int i0 = 0; i0 < ft.n_eps; i0 += sym_batch) {
     const int n = std::min(sym_batch, ft.n_eps - i0);
-    o << "  {\n    double c[" << 2 * n << "] = {";
+    o << "  {\n    double c[" << dim * n << "] = {";
     for (int j = 0; j < n; ++j) {
       std::vector<int> a(ft.sym_alpha.begin() + (size_t)(i0 + j) * L, ft.sym_alpha.begin() + (size_t)(i0 + j + 1) * L);
-      o << (j ? ", " : "") << combo(a, "kx") << ", " << combo(a, "ky");
+      for (int c = 0; c < dim; ++c) o << (j || c ? ", " : "") << combo(a, comp[c]);
     }
-    o << "};\n    cos_bounded_n<" << 2 * n << ">(c);\n";
-    for (int j = 0; j < n; ++j)
-      o << "    e" << i0 + j << " = fma(2.0 * p.t, c[" << 2 * j << "] + c[" << 2 * j + 1 << "], p.mu);\n";
+    o << "};\n";
+    if (var.band == AMI_BAND_TIGHT_BINDING) {
+      o << "    cos_bounded_n<" << dim * n << ">(c);\n";
+      for (int j = 0; j < n; ++j) {
+        std::string sum = "c[" + std::to_string(dim * j) + "]";
+        for (int c = 1; c < dim; ++c) sum = "(" + sum + " + c[" + std::to_string(dim * j + c) + "])";
+        o << "    e" << i0 + j << " = fma(2.0 * p.t, " << sum << ", p.mu);\n";
+      }
+    } else {   // free particles: e = mu - t |K|^2
+      for (int j = 0; j < n; ++j) {
+        std::string sq = "c[" + std::to_string(dim * j) + "] * c[" + std::to_string(dim * j) + "]";
+        for (int c = 1; c < dim; ++c) {
+          const std::string k = "c[" + std::to_string(dim * j + c) + "]";
+          sq = "fma(" + k + ", " + k + ", " + sq + ")";
+        }
+        o << "    e" << i0 + j << " = fma(-p.t, " << sq << ", p.mu);\n";
+      }
+    }
     o << "  }\n";
   }
-  o << "  if (p.e_out) {\n";
-  for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
-  o << "  }\n" << call << "  }\n}\n";
-  auto subst = [](std::string t, const std::string& targ, const std::string& k2) {
-    for (const auto& kv : {std::make_pair(std::string("@T@"), targ), std::make_pair(std::string("@K2@"), k2)})
-      for (size_t at = 0; (at = t.find(kv.first, at)) != std::string::npos; at += kv.second.size())
-        t.replace(at, kv.first.size(), kv.second);
-    return t;
-  };
-  const std::string all = o.str();
-  std::string src = subst(all, "<false>", "ami_jit_fused");
-  src += "\n" + subst(all.substr(k2_begin), "<true>", "ami_jit_fused_tally");
-  return src;
 }
 
-int jit_tiles_per_cta() {
-  static const int u = [] {
-    const char* e = getenv("AMI_JIT_U");
-    const int v = e ? atoi(e) : 0;
-    return (v >= 1 && v <= 16) ? v : kJitTilesPerCtaDefault;
-  }();
-  return u;
-}
+const char* kTallySrc =
+    // Fused tally (S4, Monte-Carlo sums of PAPER.md:291): the warp adds its lanes' (re, im, re^2, im^2) in a fixed
+    // tree and leaves one partial per (row, warp).  All 32 lanes take part (lanes without a sample pass zeros).  The
+    // four values are reduced together: after the first exchange a lane carries two of them, after the second one,
+    // so six double shuffles do the work of twenty.  Lanes 0, 8, 16, 24 end up with the four totals.
+    "__device__ __forceinline__ void ami_tally(double4* dst, const double a, const double b, const double c, const double d) {\n"
+    "  const unsigned full = 0xffffffffu;\n"
+    "  const int lane = threadIdx.x & 31;\n"
+    "  const bool h4 = lane & 16, h3 = lane & 8;\n"
+    "  const double ra = __shfl_xor_sync(full, h4 ? a : c, 16), rb = __shfl_xor_sync(full, h4 ? b : d, 16);\n"
+    "  const double x = (h4 ? c : a) + ra, y = (h4 ? d : b) + rb;\n"
+    "  double z = (h3 ? y : x) + __shfl_xor_sync(full, h3 ? x : y, 8);\n"
+    "  z += __shfl_xor_sync(full, z, 4);\n"
+    "  z += __shfl_xor_sync(full, z, 2);\n"
+    "  z += __shfl_xor_sync(full, z, 1);\n"
+    "  if ((lane & 7) == 0) reinterpret_cast<double*>(dst)[lane >> 3] = z;\n"
+    "}\n";
 
-int jit_prefetch_ctas() {
-  static const int pf = [] {
-    const char* e = getenv("AMI_JIT_PF");
-    const int v = e ? atoi(e) : kJitPrefetchCtasDefault;
-    return (v >= 0 && v <= 1 << 20) ? v : kJitPrefetchCtasDefault;
-  }();
-  return pf;
-}
+}  // namespace
 
-int jit_min_blocks(int block_threads) {
+// ---------------------------------------------------------------------------------------------
+// The translation unit handed to NVRTC.
+// ---------------------------------------------------------------------------------------------
+static int jit_min_blocks() {
   // __launch_bounds__(AMI_NT, AMI_MINB): the register cap that lets AMI_MINB CTAs share an SM.  (--maxrregcount is
   // ignored for kernels that carry launch bounds, so this is the knob that changes occupancy.)  Default: 12 warps
-  // per SM = at most 168 registers per thread.  Measured on B200 (profiles/r01_batch_sweep.md): the order-6 kernel
-  // wants 248 registers and runs at 0.77 of the DFMA peak with 8 warps per SM; capped at 168 it spills 80 bytes
-  // and reaches 0.87; at 128 registers the spills cost more than the occupancy gives.
-  static const int env = [] {
-    const char* e = getenv("AMI_JIT_MINB");
-    const int m = e ? atoi(e) : 0;
-    return (m >= 1 && m <= 32) ? m : 0;
-  }();
-  return env ? env : std::max(1, kJitWarpsPerSmTarget * 32 / block_threads);
+  // per SM = at most 168 registers per thread.  Measured on B200 (profiles/): the order-6 kernel wants 248
+  // registers and runs at 0.77 of the DFMA peak with 8 warps per SM; capped at 168 it reaches 0.92-0.95; at 128
+  // registers the spills cost more than the occupancy gives.  At the configured N = 1e5 every cap from 128 to 255
+  // registers and 32-, 64- and 128-thread CTAs give the same 11.6-13.4 us (profiles/r02_cfg4_small_batch.md).
+  return std::max(1, kJitWarpsPerSmTarget * 32 / kJitBlockThreads);
 }
 
-bool jit_fermi_in_smem() {
-  static const bool v = [] { const char* e = getenv("AMI_JIT_SMEM_F"); return e && e[0] == '1'; }();
-  return v;
-}
-
-int jit_store_mode() {
-  static const int m = [] {
-    const char* e = getenv("AMI_JIT_STORE");
-    const int v = e ? atoi(e) : kJitStoreModeDefault;
-    return (v >= 0 && v <= 2) ? v : kJitStoreModeDefault;
-  }();
-  return m;
-}
-
-int jit_block_threads() {
-  static const int nt = [] {
-    const char* e = getenv("AMI_JIT_NT");
-    const int v = e ? atoi(e) : 0;
-    return (v == 32 || v == 64 || v == 128 || v == 256) ? v : kJitBlockThreadsDefault;
-  }();
-  return nt;
+std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerPlan& hp, const JitVariant& var,
+                                              JitLayout* layout) {
+  const int mode = jit_mode(ft, hp);
+  const int n_comp = var.dim * ft.n_int;
+  Emitter E;
+  const LeafSlots ls = leaf_slots(ft, hp);
+  if (layout) {
+    *layout = JitLayout();
+    layout->mode = mode;
+    layout->n_real_den = ls.n_real;
+    layout->n_cplx_den = ls.n_cplx;
+    layout->n_fermi = ls.n_fermi;
+  }
+  std::ostringstream head;
+  head << kAmiParamsSrc << "\n" << kAmiDeviceSrc << "\n";
+  head << "using namespace amidev;\n#define AMI_NT " << kJitBlockThreads << "\n#define AMI_MINB " << jit_min_blocks() << "\n";
+  std::ostringstream o;
+  o << head.str();
+  std::string esig, eargs;
+  for (int i = 0; i < ft.n_eps; ++i) {
+    esig += ", const double e" + std::to_string(i);
+    eargs += ", e" + std::to_string(i);
+  }
+  // A fused kernel: a CTA walks `tiles` consecutive tiles of AMI_NT samples -- one, known at compile time, in
+  // ami_jit_fused (the loop disappears); p.tiles in the tally kernel, where a thread adds up its own samples.
+  // A warp leaves only as a whole: lanes past the end of the batch stay, compute on zero momenta and store
+  // nothing, so that the tally's shuffles always see 32 lanes.
+  auto fused_open = [&](const char* name, const char* tiles) {
+    o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) " << name << "(const __grid_constant__ AmiBatch p) {\n"
+         "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
+         "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
+         "  const long long base = blockIdx.x * (long long)AMI_NT * (" << tiles << ") + threadIdx.x;\n"
+         "  double4 t4 = make_double4(0.0, 0.0, 0.0, 0.0);\n"
+         "#pragma unroll 1\n  for (int u = 0; u < (" << tiles << "); ++u) {\n"
+         "  const long long s = base + (long long)u * AMI_NT;\n"
+         "  if (s - (threadIdx.x & 31) >= p.n) break;\n"
+         "  const bool valid = s < p.n;\n";
+    for (int c = 0; c < n_comp; ++c) o << "  double nk" << c << " = 0.0;\n";
+    o << "  if (valid) {\n";
+    emit_momenta(o, n_comp, "s", "    ");
+    o << "  }\n";
+    emit_dispersion(o, ft, var);
+    o << "  if (p.e_out && valid) {\n";
+    for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
+    o << "  }\n";
+  };
+  if (mode == kJitRegister) {
+    Sections S;
+    gen_sections(ft, hp, ls, kLeafInline, E, S);
+    o << kTallySrc;
+    // what a finished row does with its value: store it, and/or add it to the tally
+    o << "#define AMI_EMIT(VR, VI) { \\\n"
+         "    const long long row = (long long)(p.b0 + b) * p.n_f_total + (p.f0 + f); \\\n"
+         "    const double vr = p.prefactor * (VR), vi = p.prefactor * (VI); \\\n"
+         "    if ((!AMI_TALLY || p.out) && valid) __stcs(reinterpret_cast<double2*>(p.out) + row * p.out_row_stride + s, make_double2(vr, vi)); \\\n"
+         "    if (AMI_TALLY) { \\\n"
+         "      const double wr = valid ? vr : 0.0, wi = valid ? vi : 0.0; \\\n"
+         "      if (p.tally_acc) { t4.x += wr; t4.y += wi; t4.z = fma(wr, wr, t4.z); t4.w = fma(wi, wi, t4.w); } \\\n"
+         "      else ami_tally(reinterpret_cast<double4*>(p.tally) + row * p.tally_stride + (s >> 5), wr, wi, wr * wr, wi * wi); \\\n"
+         "    } }\n";
+    const std::string sig = "(const AmiBatch& p, const long long s, const bool valid, double4& t4" + esig + ") {\n";
+    // ---- body for one temperature per launch: beta { frequency { } } ----------------------------
+    o << "template <bool AMI_TALLY> __device__ __forceinline__ void ami_body" << sig << S.sec[0].str()
+      << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << S.sec[1].str()
+      << "#pragma unroll 1\n    for (int f = 0; f < p.n_f; ++f) {\n" << S.sec[2].str() << S.sec[3].str() << "    }\n  }\n}\n\n";
+    // ---- body for several temperatures: the per-beta values the R part needs are kept in a small
+    // per-thread array, then frequency { reciprocals once; beta { R part } } --------------------------
+    o << "template <bool AMI_TALLY> __device__ __forceinline__ void ami_body_mb" << sig << S.sec[0].str();
+    o << "  double kept[AMI_K_MAX_BETA][" << std::max<size_t>(S.keep.size(), 1) << "];\n";
+    o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << S.sec[1].str();
+    for (size_t i = 0; i < S.keep.size(); ++i) o << "    kept[b][" << i << "] = " << S.keep[i] << ";\n";
+    o << "  }\n#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n" << S.sec[2].str()
+      << "#pragma unroll 1\n    for (int b = 0; b < p.n_b; ++b) {\n";
+    for (size_t i = 0; i < S.keep.size(); ++i) o << "      const double " << S.keep[i] << " = kept[b][" << i << "];\n";
+    o << S.sec[3].str() << "    }\n  }\n}\n\n";
+    const std::string call_args = "(p, s, valid, t4" + eargs + ");\n";
+    // @T@ = <false> / <true>: without / with the fused tally (a compile-time switch: the reductions cost the kernels
+    // that do not tally nothing)
+    const std::string call = "  if (p.n_b == 1) ami_body@T@" + call_args + "  else ami_body_mb@T@" + call_args;
+    auto subst = [](std::string t, const std::string& targ) {
+      for (size_t at = 0; (at = t.find("@T@", at)) != std::string::npos; at += targ.size()) t.replace(at, 3, targ);
+      return t;
+    };
+    // ---- kernel 1: energies from memory ---------------------------------------------------------
+    o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
+         "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
+         "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
+         "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
+         "  const bool valid = true;\n"
+         "  double4 t4 = make_double4(0.0, 0.0, 0.0, 0.0);\n"
+         "#pragma unroll 1\n"
+         "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n";
+    for (int i = 0; i < ft.n_eps; ++i) o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
+    o << subst(call, "<false>") << "  }\n}\n\n";
+    // ---- kernels 2, 3: momenta from memory or drawn in place, dispersion inline; without / with the tally ----
+    for (int tally = 0; tally < 2; ++tally) {
+      fused_open(tally ? "ami_jit_fused_tally" : "ami_jit_fused", tally ? "p.tiles" : "1");
+      o << subst(call, tally ? "<true>" : "<false>") << "  }\n";
+      if (tally)   // single-row tally: one partial per warp of the grid, formed from the threads' own sums
+        o << "  if (p.tally_acc) ami_tally(reinterpret_cast<double4*>(p.tally) + (long long)(p.b0 * p.n_f_total + p.f0) * "
+             "p.tally_stride + blockIdx.x * (AMI_NT / 32) + (threadIdx.x >> 5), t4.x, t4.y, t4.z, t4.w);\n";
+      o << "}\n\n";
+    }
+    return std::vector<std::string>(1, o.str());
+  }
+  // ---- split plan ----------------------------------------------------------------------------------
+  // Module 0: the leaf kernels and the kernel that adds the parts.  Modules 1..M: the parts, a few per module, so
+  // that NVRTC compiles them side by side on the host's cores (a part is 1-2 k statements; one translation unit
+  // with all of an order-8 table's parts takes 20 s, eight of them 3-5 s).
+  const std::vector<std::vector<int>> parts = partition_groups(hp, split_budget());
+  const int n_parts = (int)parts.size();
+  const int n_mod = std::min(n_parts, 8);
+  if (layout) {
+    layout->n_parts = n_parts;
+    layout->part0.clear();
+    for (int j = 0; j <= n_mod; ++j) layout->part0.push_back((int)((long long)n_parts * j / n_mod));
+  }
+  std::vector<std::string> sources;
+  o << "#define AMI_LS(i, v) p.leaves[(long long)(i) * p.leaf_stride + s] = (v)\n";
+  {   // leaf kernels: everything that depends on one energy combination, written once per sample
+    Sections S;
+    gen_sections(ft, hp, ls, kLeafStore, E, S);
+    o << "__device__ __forceinline__ void ami_leaf_body(const AmiBatch& p, const long long s" << esig << ") {\n"
+      << "  const int CB = " << ls.n_real << " + p.n_b * " << ls.n_fermi << ";\n" << S.sec[0].str()
+      << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << S.sec[1].str() << "  }\n"
+      << "#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n" << S.sec[2].str() << "  }\n}\n\n";
+    o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_split_leaves_eval(const __grid_constant__ AmiBatch p) {\n"
+         "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n  if (s >= p.n) return;\n";
+    for (int i = 0; i < ft.n_eps; ++i) o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
+    o << "  ami_leaf_body(p, s" << eargs << ");\n}\n\n";
+    o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_split_leaves_fused(const __grid_constant__ AmiBatch p) {\n"
+         "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n  if (s >= p.n) return;\n";
+    for (int c = 0; c < n_comp; ++c) o << "  double nk" << c << ";\n";
+    emit_momenta(o, n_comp, "s", "  ");
+    emit_dispersion(o, ft, var);
+    o << "  if (p.e_out) {\n";
+    for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
+    o << "  }\n  ami_leaf_body(p, s" << eargs << ");\n}\n\n";
+  }
+  // the parts' partial results, added in the order of the parts (fixed: deterministic), times the prefactor
+  // (launched as a programmatic dependent of the last parts kernel: see ami_split_parts)
+  o << "extern \"C\" __global__ void __launch_bounds__(256) ami_split_combine(const __grid_constant__ AmiBatch p) {\n"
+       "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
+       "  const long long s = blockIdx.x * 256ll + threadIdx.x;\n  if (s >= p.n) return;\n"
+       "  const int lr = blockIdx.y, b = lr / p.n_f, f = lr - b * p.n_f;\n"
+       "  const double2* P = reinterpret_cast<const double2*>(p.partial) + (long long)lr * p.partial_stride + s;\n"
+       "  double vr = 0.0, vi = 0.0;\n"
+       "  for (int k = 0; k < p.n_parts; ++k) {\n"
+       "    const double2 v = P[(long long)k * p.n_b * p.n_f * p.partial_stride];\n    vr += v.x; vi += v.y;\n  }\n"
+       "  const long long row = (long long)(p.b0 + b) * p.n_f_total + (p.f0 + f);\n"
+       "  __stcs(reinterpret_cast<double2*>(p.out) + row * p.out_row_stride + s, make_double2(p.prefactor * vr, p.prefactor * vi));\n"
+       "}\n";
+  sources.push_back(o.str());
+  // parts: leaves are read where they are used (AMI_L: reciprocal denominators, one product each; AMI_LF: Fermi/Bose
+  // values, loaded once per chunk of groups); the prefactor is applied when the parts are added up
+  for (int mj = 0; mj < n_mod; ++mj) {
+  const int pa = (int)((long long)n_parts * mj / n_mod), pb = (int)((long long)n_parts * (mj + 1) / n_mod);
+  o.str("");
+  o << head.str();
+  o << "#define AMI_L(i) __ldg(Lp + (long long)(i) * ls)\n#define AMI_LF(u) AMI_L(" << ls.n_real << " + b * " << ls.n_fermi
+    << " + (u))\n#define AMI_EMIT(VR, VI) Pp[(long long)(b * n_f + f) * ps] = make_double2((VR), (VI))\n";
+  for (int pi = pa; pi < pb; ++pi) {
+    const HornerPlan sub = make_sub_plan(hp, parts[pi]);
+    Sections S;
+    gen_sections(ft, sub, ls, kLeafLoad, E, S);
+    o << "__device__ __noinline__ void ami_part_" << pi
+      << "(const double* __restrict__ Lp, const long long ls, double2* __restrict__ Pp, const long long ps, const int n_b, "
+         "const int n_f) {\n  const int CB = "
+      << ls.n_real << " + n_b * " << ls.n_fermi << ";\n" << S.sec[0].str()
+      << "#pragma unroll 1\n  for (int b = 0; b < n_b; ++b) {\n" << S.sec[1].str()
+      << "#pragma unroll 1\n    for (int f = 0; f < n_f; ++f) {\n" << S.sec[2].str() << S.sec[3].str() << "    }\n  }\n";
+    // the macros that name this part's denominators end with it
+    for (size_t u = 0; u < ft.leafD.size(); ++u) o << "#undef Dr" << u << "\n#undef Di" << u << "\n";
+    o << "}\n\n";
+  }
+  // grid.y = part within this module; p.part0 = index of the module's first part.
+  // The parts kernels of a chunk are independent of one another (each reads the leaf array and writes its own
+  // partial results), so they are launched as a chain of programmatic dependents: launch_dependents at the top lets
+  // the next kernel of the chain start as soon as every CTA of this one is running -- the tail of one launch
+  // overlaps the head of the next instead of leaving the SMs half empty between them.  The leaf kernel never
+  // triggers early, so the first parts kernel (and with it every later one) starts after the leaves are complete.
+  // The wait at the END makes this grid complete only after its predecessor has: when the combine kernel's wait
+  // returns, every parts kernel of the chunk is done.
+  o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_split_parts(const __grid_constant__ AmiBatch p) {\n"
+       "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
+       "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n"
+       "  if (s >= p.n) { asm volatile(\"griddepcontrol.wait;\" ::: \"memory\"); return; }\n"
+       "  const double* Lp = p.leaves + s;\n"
+       "  double2* Pp = reinterpret_cast<double2*>(p.partial) + (long long)(p.part0 + blockIdx.y) * p.n_b * p.n_f * p.partial_stride + s;\n"
+       "  switch (blockIdx.y) {\n";
+  for (int pi = pa; pi < pb; ++pi)
+    o << "    case " << pi - pa << ": ami_part_" << pi << "(Lp, p.leaf_stride, Pp, p.partial_stride, p.n_b, p.n_f); break;\n";
+  o << "  }\n  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n}\n";
+  sources.push_back(o.str());
+  }
+  return sources;
 }
 
 int jit_mode(const FlatTable& ft, const HornerPlan& hp) {
@@ -768,17 +948,9 @@ int jit_mode(const FlatTable& ft, const HornerPlan& hp) {
     if (off[0] == '1') return kJitNone;
   long long leaf_doubles = (long long)ft.leafF.size();
   for (size_t u = 0; u < ft.leafD.size(); ++u) leaf_doubles += hp.d_is_real[u] ? 1 : 2;
-  long long max_leaf = 160, max_edges = 24000, max_scratch_edges = 400000;
-  if (const char* env = getenv("AMI_JIT_MAX_LEAF_DOUBLES")) max_leaf = atoll(env);   // tuning knobs
-  if (const char* env = getenv("AMI_JIT_MAX_EDGES")) max_edges = atoll(env);
-  if (const char* env = getenv("AMI_JIT_MAX_SCRATCH_EDGES")) max_scratch_edges = atoll(env);
   const long long edges = hp.n_fnodes + 4 * hp.n_dnodes;
-  if (leaf_doubles <= max_leaf && edges <= max_edges) return kJitRegister;
-  // memory-backed variant: Fermi/Bose leaves in shared memory (64 threads per CTA), the rest in scratch.
-  // Opt-in (AMI_JIT_SCRATCH=1): NVRTC needs minutes for bodies of this size (order 7: 90 s, order 8: 270 s).
-  const char* opt_in = getenv("AMI_JIT_SCRATCH");
-  if (opt_in && opt_in[0] == '1' && (long long)ft.leafF.size() * 64 * 8 <= 200 * 1024 && edges <= max_scratch_edges)
-    return kJitScratch;
+  if (leaf_doubles <= 160 && edges <= 4000) return kJitRegister;
+  if (edges <= 2000000) return kJitSplit;
   return kJitNone;
 }
 
@@ -798,6 +970,7 @@ struct Nvrtc {
   int (*GetCUBINSize)(void*, size_t*) = nullptr;
   int (*GetCUBIN)(void*, char*) = nullptr;
   int (*DestroyProgram)(void**) = nullptr;
+  int (*Version)(int*, int*) = nullptr;
   const char* (*GetErrorString)(int) = nullptr;
   bool ok = false;
 };
@@ -814,7 +987,7 @@ Nvrtc& nvrtc() {
     if (!n.h) return;
 #define AMI_SYM(f) *(void**)(&n.f) = dlsym(n.h, "nvrtc" #f)
     AMI_SYM(CreateProgram); AMI_SYM(CompileProgram); AMI_SYM(GetProgramLogSize); AMI_SYM(GetProgramLog);
-    AMI_SYM(GetCUBINSize); AMI_SYM(GetCUBIN); AMI_SYM(DestroyProgram); AMI_SYM(GetErrorString);
+    AMI_SYM(GetCUBINSize); AMI_SYM(GetCUBIN); AMI_SYM(DestroyProgram); AMI_SYM(GetErrorString); AMI_SYM(Version);
 #undef AMI_SYM
     n.ok = n.CreateProgram && n.CompileProgram && n.GetProgramLogSize && n.GetProgramLog && n.GetCUBINSize &&
            n.GetCUBIN && n.DestroyProgram;
@@ -822,23 +995,95 @@ Nvrtc& nvrtc() {
   return n;
 }
 
+// ---- on-disk cache of compiled kernels -------------------------------------------------------------
+// A diagrammatic Monte-Carlo user evaluates thousands of diagrams; NVRTC needs 0.6-1 s per diagram, the
+// paper's construct "microseconds".  The cubin of a generated source is therefore kept in
+//   $AMI_JIT_CACHE, else $XDG_CACHE_HOME/ami_b200, else $HOME/.cache/ami_b200
+// under the 128-bit FNV-1a hash of (source text, NVRTC version, target architecture); AMI_JIT_CACHE=0 turns
+// the cache off.  Files are written to a temporary name and renamed, so concurrent processes are safe.
+const char* kJitArch = "sm_100a";
+
+std::string cache_dir() {
+  if (const char* e = getenv("AMI_JIT_CACHE")) {
+    if (!strcmp(e, "0") || !*e) return "";
+    return e;
+  }
+  if (const char* x = getenv("XDG_CACHE_HOME"))
+    if (*x) return std::string(x) + "/ami_b200";
+  if (const char* h = getenv("HOME"))
+    if (*h) return std::string(h) + "/.cache/ami_b200";
+  return "";
+}
+
+std::string cache_key(const std::string& src) {
+  int major = 0, minor = 0;
+  if (nvrtc().Version) nvrtc().Version(&major, &minor);
+  const std::string salt = std::string("|nvrtc ") + std::to_string(major) + "." + std::to_string(minor) + "|" + kJitArch;
+  unsigned long long h1 = 0xcbf29ce484222325ull, h2 = 0x84222325cbf29ce4ull;
+  auto feed = [&](const std::string& t) {
+    for (unsigned char c : t) {
+      h1 = (h1 ^ c) * 0x100000001b3ull;
+      h2 = (h2 ^ (unsigned char)(c + 0x5b)) * 0x100000001b3ull;
+      h2 ^= h2 >> 29;
+    }
+  };
+  feed(src);
+  feed(salt);
+  char buf[40];
+  snprintf(buf, sizeof buf, "%016llx%016llx", h1, h2);
+  return buf;
+}
+
+void make_dirs(const std::string& path) {
+  for (size_t i = 1; i <= path.size(); ++i)
+    if (i == path.size() || path[i] == '/') mkdir(path.substr(0, i).c_str(), 0755);
+}
+
+bool cache_read(const std::string& file, std::vector<char>& cubin) {
+  FILE* f = fopen(file.c_str(), "rb");
+  if (!f) return false;
+  fseek(f, 0, SEEK_END);
+  const long n = ftell(f);
+  fseek(f, 0, SEEK_SET);
+  bool ok = n > 4;
+  if (ok) {
+    cubin.resize((size_t)n);
+    ok = fread(cubin.data(), 1, (size_t)n, f) == (size_t)n && !memcmp(cubin.data(), "\x7f" "ELF", 4);
+  }
+  fclose(f);
+  return ok;
+}
+
+void cache_write(const std::string& dir, const std::string& file, const std::vector<char>& cubin) {
+  make_dirs(dir);
+  const std::string tmp = file + ".tmp" + std::to_string((long)getpid());
+  FILE* f = fopen(tmp.c_str(), "wb");
+  if (!f) return;
+  const bool ok = fwrite(cubin.data(), 1, cubin.size(), f) == cubin.size();
+  fclose(f);
+  if (!ok || rename(tmp.c_str(), file.c_str()) != 0) remove(tmp.c_str());
+}
+
 }  // namespace
 
-int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& log) {
+int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& log, bool use_cache, bool* cache_hit) {
   Nvrtc& n = nvrtc();
+  if (cache_hit) *cache_hit = false;
   if (!n.ok) { log = "NVRTC library not found (set AMI_NVRTC_PATH)"; return AMI_EUNSUPPORTED; }
+  const std::string dir = use_cache ? cache_dir() : "";
+  const std::string file = dir.empty() ? "" : dir + "/" + cache_key(src) + ".cubin";
+  if (!file.empty() && cache_read(file, cubin)) {
+    if (cache_hit) *cache_hit = true;
+    log = "cubin from " + file;
+    return AMI_OK;
+  }
   void* prog = nullptr;
   if (n.CreateProgram(&prog, src.c_str(), "ami_jit.cu", 0, nullptr, nullptr) != 0) {
     log = "nvrtcCreateProgram failed";
     return AMI_EINVAL;
   }
-  std::vector<const char*> opts = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "--ptxas-options=-v",
-                                   "-default-device"};
-  std::string popt;
-  if (const char* env = getenv("AMI_JIT_PTXAS_OPT")) {   // tuning knob: e.g. -O1
-    popt = std::string("--ptxas-options=") + env;
-    opts.push_back(popt.c_str());
-  }
+  const std::string arch = std::string("--gpu-architecture=") + kJitArch;
+  std::vector<const char*> opts = {arch.c_str(), "--std=c++17", "-lineinfo", "--ptxas-options=-v", "-default-device"};
   // (no --maxrregcount: it is ignored for kernels with __launch_bounds__; the register cap is AMI_MINB)
   const int rc = n.CompileProgram(prog, (int)opts.size(), opts.data());
   size_t ls = 0;
@@ -857,6 +1102,7 @@ int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& l
   cubin.resize(cs);
   n.GetCUBIN(prog, cubin.data());
   n.DestroyProgram(&prog);
+  if (cs && !file.empty()) cache_write(dir, file, cubin);
   return cs ? AMI_OK : AMI_EINVAL;
 }
 
@@ -864,18 +1110,22 @@ int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& l
 // module loading and launch through driver entry points obtained from the runtime (the library
 // does not link against libcuda, so that it loads on a machine without a driver)
 // ---------------------------------------------------------------------------------------------
-struct JitState {
-  std::mutex mu;
+struct JitModule {
   bool tried = false;
   int status = AMI_EUNSUPPORTED;
   std::string log;
-  CUmodule mod = nullptr;
-  CUfunction fn_eval = nullptr, fn_fused = nullptr, fn_fused_tally = nullptr;
-  int mode = kJitNone;
-  int block = 0;            // threads per CTA the kernels were generated for
-  int tiles = 1;            // tiles of `block` samples one CTA of the fused kernel walks
-  int scratch_slots = 0;    // doubles of global scratch per sample (memory-backed variant)
-  unsigned smem_bytes = 0;  // dynamic shared memory per CTA (memory-backed variant)
+  std::vector<CUmodule> mods;
+  CUfunction fn_eval = nullptr, fn_fused = nullptr, fn_fused_tally = nullptr;                 // register plan
+  CUfunction fn_leaves_eval = nullptr, fn_leaves_fused = nullptr, fn_combine = nullptr;       // split plan, module 0
+  std::vector<CUfunction> fn_parts;                                                           // split plan, modules 1..M
+  JitLayout layout;
+  double compile_ms = 0.0;
+  int cache_hit = 0;
+};
+
+struct JitState {
+  std::mutex mu;
+  std::map<int, JitModule> variants;   // by JitVariant::key()
 };
 
 namespace {
@@ -888,7 +1138,6 @@ struct Driver {
                            void**, void**) = nullptr;
   CUresult (*GetErrorString)(CUresult, const char**) = nullptr;
   CUresult (*LaunchKernelEx)(const CUlaunchConfig*, CUfunction, void**, void**) = nullptr;   // optional
-  CUresult (*FuncSetAttribute)(CUfunction, CUfunction_attribute, int) = nullptr;
   bool ok = false;
 };
 
@@ -906,82 +1155,110 @@ Driver& driver() {
            get("cuModuleUnload", (void**)&d.ModuleUnload) && get("cuLaunchKernel", (void**)&d.LaunchKernel) &&
            get("cuGetErrorString", (void**)&d.GetErrorString);
     get("cuLaunchKernelEx", (void**)&d.LaunchKernelEx);
-    d.ok = d.ok && get("cuFuncSetAttribute", (void**)&d.FuncSetAttribute);
   });
   return d;
 }
 
 std::mutex g_state_mu;   // guards creation of tab->jit
 
+const JitModule* module_of(const ami_table* tab, const JitVariant& var) {
+  JitState* js = tab->jit;
+  if (!js) return nullptr;
+  std::lock_guard<std::mutex> lk(js->mu);
+  auto it = js->variants.find(var.key());
+  return it == js->variants.end() ? nullptr : &it->second;   // map nodes are stable
+}
+
 }  // namespace
 
-int jit_prepare(ami_table* tab, std::string& err) {
+int jit_prepare(ami_table* tab, const JitVariant& var, std::string& err) {
   {
     std::lock_guard<std::mutex> lk(g_state_mu);
     if (!tab->jit) tab->jit = new JitState;
   }
   JitState& js = *tab->jit;
   std::lock_guard<std::mutex> lk(js.mu);
-  if (js.tried) { err = js.log; return js.status; }
-  js.tried = true;
-  if (tab->dev.device < 0) { js.log = "table has no device copy"; js.status = AMI_ECUDA; err = js.log; return js.status; }
-  if (!jit_eligible(tab->flat, tab->horner)) {
-    js.log = "table too large for the register plan";
-    js.status = AMI_EUNSUPPORTED;
-    err = js.log;
-    return js.status;
+  JitModule& m = js.variants[var.key()];
+  if (m.tried) { err = m.log; return m.status; }
+  m.tried = true;
+  auto fail = [&](int code, const std::string& why) {
+    m.log = why;
+    m.status = code;
+    err = why;
+    return code;
+  };
+  if (tab->dev.device < 0) return fail(AMI_ECUDA, "table has no device copy");
+  if (var.dim < 1 || var.dim > 3 || (var.band != AMI_BAND_TIGHT_BINDING && var.band != AMI_BAND_FREE))
+    return fail(AMI_EINVAL, "bad lattice for the specialised kernels");
+  if (var.cplx) return fail(AMI_EUNSUPPORTED, "complex energies run the table-driven kernels");
+  if (!jit_eligible(tab->flat, tab->horner)) return fail(AMI_EUNSUPPORTED, "table outside the limits of the specialised kernels");
+  const auto t0 = std::chrono::steady_clock::now();
+  const std::vector<std::string> srcs = jit_generate_sources(tab->flat, tab->horner, var, &m.layout);
+  // the modules of a split plan are compiled side by side (NVRTC is thread safe across programs)
+  std::vector<std::vector<char>> cubins(srcs.size());
+  std::vector<std::string> logs(srcs.size());
+  std::vector<int> codes(srcs.size(), AMI_OK);
+  std::vector<char> hits(srcs.size(), 0);
+  {
+    const size_t n_thr = std::max<size_t>(1, std::min<size_t>(srcs.size(), std::thread::hardware_concurrency()));
+    std::atomic<size_t> next{0};
+    auto work = [&] {
+      for (size_t i; (i = next.fetch_add(1)) < srcs.size();) {
+        bool hit = false;
+        codes[i] = jit_compile(srcs[i], cubins[i], logs[i], true, &hit);
+        hits[i] = hit;
+      }
+    };
+    std::vector<std::thread> pool;
+    for (size_t t = 1; t < n_thr; ++t) pool.emplace_back(work);
+    work();
+    for (std::thread& t : pool) t.join();
   }
-  std::vector<char> cubin;
-  js.mode = jit_mode(tab->flat, tab->horner);
-  js.block = js.mode == kJitScratch ? 64 : jit_block_threads();
-  js.tiles = js.mode == kJitScratch ? 1 : jit_tiles_per_cta();
-  const std::string src = jit_generate_source(tab->flat, tab->horner, js.block, js.mode == kJitScratch, &js.scratch_slots);
-  js.smem_bytes = (js.mode == kJitScratch || jit_fermi_in_smem())
-                      ? (unsigned)(tab->flat.leafF.size() * js.block * sizeof(double)) : 0u;
-  js.status = jit_compile(src, cubin, js.log);
-  if (js.status != AMI_OK) { err = js.log; return js.status; }
+  m.cache_hit = 1;
+  for (size_t i = 0; i < srcs.size(); ++i) {
+    m.log += logs[i] + "\n";
+    if (!hits[i]) m.cache_hit = 0;
+  }
+  for (size_t i = 0; i < srcs.size(); ++i)
+    if (codes[i] != AMI_OK) { m.status = codes[i]; err = m.log; return m.status; }
   Driver& d = driver();
-  if (!d.ok) { js.log = "CUDA driver entry points unavailable"; js.status = AMI_ECUDA; err = js.log; return js.status; }
+  if (!d.ok) return fail(AMI_ECUDA, "CUDA driver entry points unavailable");
   cudaSetDevice(tab->dev.device);
   cudaFree(nullptr);   // makes the primary context current
-  CUresult rc = d.ModuleLoadData(&js.mod, cubin.data());
-  if (rc == CUDA_SUCCESS) rc = d.ModuleGetFunction(&js.fn_eval, js.mod, "ami_jit_eval");
-  if (rc == CUDA_SUCCESS) rc = d.ModuleGetFunction(&js.fn_fused, js.mod, "ami_jit_fused");
-  if (rc == CUDA_SUCCESS) rc = d.ModuleGetFunction(&js.fn_fused_tally, js.mod, "ami_jit_fused_tally");
-  if (rc == CUDA_SUCCESS && js.fn_fused_tally && js.smem_bytes > 48 * 1024)
-    rc = d.FuncSetAttribute(js.fn_fused_tally, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)js.smem_bytes);
-  if (rc == CUDA_SUCCESS && js.smem_bytes > 48 * 1024) {
-    rc = d.FuncSetAttribute(js.fn_eval, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)js.smem_bytes);
-    if (rc == CUDA_SUCCESS) rc = d.FuncSetAttribute(js.fn_fused, CU_FUNC_ATTRIBUTE_MAX_DYNAMIC_SHARED_SIZE_BYTES, (int)js.smem_bytes);
+  CUresult rc = CUDA_SUCCESS;
+  m.mods.assign(srcs.size(), nullptr);
+  for (size_t i = 0; i < srcs.size() && rc == CUDA_SUCCESS; ++i) rc = d.ModuleLoadData(&m.mods[i], cubins[i].data());
+  auto get = [&](CUfunction* fn, size_t mod, const char* name) {
+    if (rc == CUDA_SUCCESS) rc = d.ModuleGetFunction(fn, m.mods[mod], name);
+  };
+  if (m.layout.mode == kJitRegister) {
+    get(&m.fn_eval, 0, "ami_jit_eval");
+    get(&m.fn_fused, 0, "ami_jit_fused");
+    get(&m.fn_fused_tally, 0, "ami_jit_fused_tally");
+  } else {
+    get(&m.fn_leaves_eval, 0, "ami_split_leaves_eval");
+    get(&m.fn_leaves_fused, 0, "ami_split_leaves_fused");
+    get(&m.fn_combine, 0, "ami_split_combine");
+    m.fn_parts.assign(srcs.size() - 1, nullptr);
+    for (size_t i = 1; i < srcs.size(); ++i) get(&m.fn_parts[i - 1], i, "ami_split_parts");
   }
   if (rc != CUDA_SUCCESS) {
     const char* msg = nullptr;
     d.GetErrorString(rc, &msg);
-    js.log = std::string("loading the specialised kernels failed: ") + (msg ? msg : "?");
-    js.status = AMI_ECUDA;
-    err = js.log;
-    return js.status;
+    return fail(AMI_ECUDA, std::string("loading the specialised kernels failed: ") + (msg ? msg : "?"));
   }
-  js.status = AMI_OK;
+  m.compile_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  m.status = AMI_OK;
   return AMI_OK;
 }
 
 namespace {
 
-CUresult launch_one(const JitState* js, bool fused, AmiBatch& batch, cudaStream_t st) {
+// Programmatic dependent launch: the register-plan kernels begin with griddepcontrol.launch_dependents + .wait,
+// so the NEXT specialised kernel in the stream may be scheduled while this one drains and starts the moment it
+// has completed (stream order is kept: nothing is read or written before the wait).
+CUresult launch(CUfunction fn, unsigned gx, unsigned gy, unsigned block, AmiBatch& batch, cudaStream_t st, bool pdl) {
   void* args[] = {&batch};
-  // One CTA per `block` samples: the hardware CTA scheduler balances the SMs better than a
-  // persistent grid with a static stride does (measured: persistent + L2 prefetch of the next sample
-  // was 12 % slower on cfg3 and 5 % slower on cfg4, profiles/r01_register_plan.md).  The kernels keep
-  // their grid-stride loop, so any grid size is correct.
-  const unsigned block = (unsigned)js->block;
-  const long long per_cta = (long long)block * (fused ? js->tiles : 1);   // the unfused kernel strides over the grid
-  const unsigned grid = (unsigned)((batch.n + per_cta - 1) / per_cta);
-  // Programmatic dependent launch: the kernels begin with griddepcontrol.launch_dependents + .wait, so
-  // the NEXT specialised kernel in the stream may be scheduled while this one drains and starts the
-  // moment it has completed (stream order is kept: nothing is read or written before the wait).
-  static const bool pdl = [] { const char* e = getenv("AMI_JIT_PDL"); return !(e && e[0] == '0'); }();
-  CUfunction fn = fused ? (batch.tally ? js->fn_fused_tally : js->fn_fused) : js->fn_eval;
   if (!fn) return CUDA_ERROR_INVALID_VALUE;
   if (pdl && driver().LaunchKernelEx) {
     CUlaunchAttribute attr;
@@ -990,59 +1267,104 @@ CUresult launch_one(const JitState* js, bool fused, AmiBatch& batch, cudaStream_
     attr.value.programmaticStreamSerializationAllowed = 1;
     CUlaunchConfig cfg;
     memset(&cfg, 0, sizeof cfg);
-    cfg.gridDimX = grid; cfg.gridDimY = 1; cfg.gridDimZ = 1;
+    cfg.gridDimX = gx; cfg.gridDimY = gy; cfg.gridDimZ = 1;
     cfg.blockDimX = block; cfg.blockDimY = 1; cfg.blockDimZ = 1;
-    cfg.sharedMemBytes = js->smem_bytes; cfg.hStream = (CUstream)st; cfg.attrs = &attr; cfg.numAttrs = 1;
+    cfg.sharedMemBytes = 0; cfg.hStream = (CUstream)st; cfg.attrs = &attr; cfg.numAttrs = 1;
     return driver().LaunchKernelEx(&cfg, fn, args, nullptr);
   }
-  return driver().LaunchKernel(fn, grid, 1, 1, block, 1, 1, js->smem_bytes, (CUstream)st, args, nullptr);
+  return driver().LaunchKernel(fn, gx, gy, 1, block, 1, 1, 0, (CUstream)st, args, nullptr);
 }
 
 }  // namespace
 
-cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cudaStream_t st, int* launches) {
-  const JitState* js = tab->jit;
-  if (!js || js->status != AMI_OK) return cudaErrorInvalidDeviceFunction;
+cudaError_t jit_launch(const ami_table* tab, const JitVariant& var, bool fused, const AmiBatch& b, cudaStream_t st,
+                       int* launches, long long* tally_slots) {
+  const JitModule* m = module_of(tab, var);
+  if (tally_slots) *tally_slots = 0;
+  if (!m || m->status != AMI_OK) return cudaErrorInvalidDeviceFunction;
   if (b.n == 0) return cudaSuccess;
-  if (js->mode != kJitScratch) {
+  const unsigned block = kJitBlockThreads;
+  if (m->layout.mode == kJitRegister) {
+    // One CTA per `block` samples: the hardware CTA scheduler balances the SMs better than a persistent grid
+    // with a static stride does (measured: persistent + L2 prefetch of the next sample was 12 % slower on cfg3
+    // and 5 % slower on cfg4, profiles/r01_final_kernels.md).  The unfused kernel keeps a grid-stride loop.
     AmiBatch copy = b;
-    if (launch_one(js, fused, copy, st) != CUDA_SUCCESS) return cudaErrorLaunchFailure;
+    copy.tiles = 1;
+    copy.tally_acc = 0;
+    if (fused && b.tally && (long long)b.n_b * b.n_f == 1 && b.n >= (long long)kJitTallyTiles * block * 148 * 8) {
+      copy.tiles = kJitTallyTiles;     // every thread adds kJitTallyTiles samples itself, then one warp sum
+      copy.tally_acc = 1;
+    }
+    const long long per_cta = (long long)block * copy.tiles;
+    const unsigned grid = (unsigned)((b.n + per_cta - 1) / per_cta);
+    if (tally_slots && b.tally) *tally_slots = copy.tally_acc ? (long long)grid * (block / 32) : (b.n + 31) / 32;
+    CUfunction fn = fused ? (b.tally ? m->fn_fused_tally : m->fn_fused) : m->fn_eval;
+    if (launch(fn, grid, 1, block, copy, st, true) != CUDA_SUCCESS) return cudaErrorLaunchFailure;
     if (launches) ++*launches;
     return cudaSuccess;
   }
-  // memory-backed variant: a stream-ordered scratch of [slots][chunk] doubles, at most ~512 MiB at a
-  // time, so the batch is walked in chunks of samples
-  const long long per_sample = (long long)js->scratch_slots * 8;
-  long long chunk = std::max<long long>(js->block, ((512LL << 20) / std::max<long long>(per_sample, 1)) / js->block * js->block);
-  chunk = std::min(chunk, (b.n + js->block - 1) / js->block * js->block);
-  double* scratch = nullptr;
-  cudaError_t crc = cudaMallocAsync((void**)&scratch, (size_t)(per_sample * chunk), st);
+  // split plan: leaves -> parts -> combine per chunk of samples; the chunk is sized so that the leaf array and the
+  // parts' partial results (stream-ordered allocations) stay in L2 between the kernels
+  if (b.tally || !b.out) return cudaErrorInvalidValue;
+  const JitLayout& lay = m->layout;
+  const long long rows = (long long)b.n_b * b.n_f;
+  const long long slots = lay.n_real_den + (long long)b.n_b * lay.n_fermi + 2LL * b.n_f * lay.n_cplx_den;
+  const long long per_sample = slots * 8 + rows * lay.n_parts * 16;
+  long long chunk = std::max<long long>(block, ((64LL << 20) / std::max<long long>(per_sample, 1)) / 256 * 256);
+  chunk = std::min(chunk, (b.n + 255) / 256 * 256);
+  double *leaves = nullptr, *partial = nullptr;
+  cudaError_t crc = cudaMallocAsync((void**)&leaves, (size_t)(slots * 8 * chunk), st);
   if (crc != cudaSuccess) return crc;
-  for (long long c0 = 0; c0 < b.n; c0 += chunk) {
+  crc = cudaMallocAsync((void**)&partial, (size_t)(rows * lay.n_parts * 16 * chunk), st);
+  if (crc != cudaSuccess) { cudaFreeAsync(leaves, st); return crc; }
+  bool ok = true;
+  for (long long c0 = 0; c0 < b.n && ok; c0 += chunk) {
     AmiBatch part = b;
     part.n = std::min(chunk, b.n - c0);
     if (part.e) part.e += c0;                       // SoA rows keep their stride
     if (part.e_out) part.e_out += c0;
     if (part.k) part.k += c0 * b.k_stride_sample;
     part.first_sample += c0;
-    if (part.out) part.out += 2 * c0;
-    if (part.tally) part.tally += 4 * (c0 >> 5);   // chunks are multiples of the block size
-    part.scratch = scratch;
-    part.scratch_stride = chunk;
-    if (launch_one(js, fused, part, st) != CUDA_SUCCESS) { cudaFreeAsync(scratch, st); return cudaErrorLaunchFailure; }
-    if (launches) ++*launches;
+    part.out += 2 * c0;
+    part.leaves = leaves; part.leaf_stride = chunk;
+    part.partial = partial; part.partial_stride = chunk;
+    part.n_parts = lay.n_parts;
+    const unsigned gx = (unsigned)((part.n + block - 1) / block);
+    ok = launch(fused ? m->fn_leaves_fused : m->fn_leaves_eval, gx, 1, block, part, st, false) == CUDA_SUCCESS;
+    for (size_t j = 0; j < m->fn_parts.size() && ok; ++j) {
+      part.part0 = lay.part0[j];
+      ok = launch(m->fn_parts[j], gx, (unsigned)(lay.part0[j + 1] - lay.part0[j]), block, part, st, true) == CUDA_SUCCESS;
+    }
+    ok = ok && launch(m->fn_combine, (unsigned)((part.n + 255) / 256), (unsigned)rows, 256, part, st, true) == CUDA_SUCCESS;
+    if (ok && launches) *launches += 2 + (int)m->fn_parts.size();
   }
-  return cudaFreeAsync(scratch, st);
+  cudaFreeAsync(partial, st);
+  crc = cudaFreeAsync(leaves, st);
+  return ok ? crc : cudaErrorLaunchFailure;
 }
 
 int jit_status(const ami_table* tab) {
-  if (!tab->jit || !tab->jit->tried) return 1;
-  return tab->jit->status;
+  const JitModule* m = module_of(tab, JitVariant());
+  if (!m || !m->tried) return 1;
+  return m->status;
+}
+
+bool jit_fused_tally_ok(const ami_table* tab) {
+  const JitModule* m = module_of(tab, JitVariant());
+  return m && m->status == AMI_OK && m->layout.mode == kJitRegister;
+}
+
+double jit_last_compile_ms(const ami_table* tab, int* cache_hit) {
+  const JitModule* m = module_of(tab, JitVariant());
+  if (cache_hit) *cache_hit = m ? m->cache_hit : 0;
+  return m ? m->compile_ms : 0.0;
 }
 
 void jit_destroy(ami_table* tab) {
   if (!tab->jit) return;
-  if (tab->jit->mod && driver().ok) driver().ModuleUnload(tab->jit->mod);
+  for (auto& kv : tab->jit->variants)
+    for (CUmodule mod : kv.second.mods)
+      if (mod && driver().ok) driver().ModuleUnload(mod);
   delete tab->jit;
   tab->jit = nullptr;
 }

@@ -10,41 +10,60 @@
 
 namespace ami {
 
-constexpr int kJitBlockThreadsDefault = 64;
-constexpr int kJitTilesPerCtaDefault = 1;
-constexpr int kJitPrefetchCtasDefault = 0;
-int jit_prefetch_ctas();    // L2 prefetch distance of the fused kernel in CTAs, 0 = off (AMI_JIT_PF, tuning knob)
-constexpr int kJitStoreModeDefault = 1;
-int jit_store_mode();       // result stores: 0 plain, 1 streaming (st.global.cs), 2 write-through (AMI_JIT_STORE, tuning knob)
+constexpr int kJitBlockThreads = 64;       // threads per CTA of every specialised kernel
 constexpr int kJitWarpsPerSmTarget = 12;   // occupancy the register cap of the specialised kernels is set for
-int jit_min_blocks(int block_threads);   // second argument of __launch_bounds__ (AMI_JIT_MINB overrides; tuning knob)
-bool jit_fermi_in_smem();   // Fermi/Bose leaves in shared memory instead of registers (AMI_JIT_SMEM_F=1, tuning knob)
-int jit_tiles_per_cta();    // kJitTilesPerCtaDefault unless AMI_JIT_U overrides it (tuning knob)
-int jit_block_threads();   // kJitBlockThreadsDefault unless AMI_JIT_NT overrides it (tuning knob)
+constexpr int kJitTallyTiles = 8;          // samples a thread adds up itself in the single-row fused tally
 
-// Tables whose straight-line form is small enough to live in registers and in the instruction
-// cache; larger ones are evaluated by the table-driven kernels.
-enum { kJitNone = 0, kJitRegister = 1, kJitScratch = 2 };
-// kJitRegister: every value in registers.  kJitScratch (tables beyond that, e.g. order 8): the same
-// generated arithmetic with Fermi/Bose leaves in shared memory and the long-lived sums in a
-// per-sample column of a global scratch array.  kJitNone: table-driven kernels only.
+// How a table is specialised.
+//   kJitRegister  the whole table is ONE straight-line kernel, every value a register (orders <= 6-7)
+//   kJitSplit     larger tables (order 7-8: 1e4-1e5 terms): a leaf kernel writes the Fermi/Bose values and the
+//                 reciprocal denominators of a chunk of samples to an L2-resident array, then the groups of the
+//                 Horner plan, partitioned into parts of register-plan size, are evaluated by ONE launch whose
+//                 grid.y is the part, and a last kernel adds the parts' partial results in a fixed order
+//   kJitNone      table-driven kernels only (AMI_DISABLE_JIT=1, or outside every limit)
+enum { kJitNone = 0, kJitRegister = 1, kJitSplit = 2 };
 int jit_mode(const FlatTable& ft, const HornerPlan& hp);
 bool jit_eligible(const FlatTable& ft, const HornerPlan& hp);
 
-// *scratch_slots receives the doubles of scratch per sample the generated kernels need (0 in register mode).
-std::string jit_generate_source(const FlatTable& ft, const HornerPlan& hp, int block_threads, bool scratch,
-                                int* scratch_slots);
+// What the generated text is specialised for besides the table: the lattice of the inline dispersion (the
+// momenta have `dim` components, Eq. 14) and its band, and whether the energies are complex.
+struct JitVariant {
+  int dim = 2;
+  int band = AMI_BAND_TIGHT_BINDING;
+  bool cplx = false;
+  int key() const { return dim + 4 * band + 16 * (cplx ? 1 : 0); }
+};
+
+// Layout facts of a generated module that the launcher needs.
+struct JitLayout {
+  int mode = kJitNone;
+  int n_parts = 0;          // split plan: parts of the Horner plan
+  int n_real_den = 0;       // split plan: leaf slots per sample = n_real_den + n_b * U_F + 2 * n_f * n_cplx_den
+  int n_cplx_den = 0;
+  int n_fermi = 0;
+  std::vector<int> part0;   // split plan: module j (of the parts) holds parts part0[j] .. part0[j+1]-1
+};
+
+// The translation units of one variant: one for the register plan; for the split plan the leaf kernels and the
+// combine kernel first, then the parts, a few per unit.
+std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerPlan& hp, const JitVariant& var,
+                                              JitLayout* layout);
 
 // NVRTC: CUDA C++ -> sm_100a cubin.  Needs no GPU.  Returns AMI_OK, AMI_EUNSUPPORTED when the
 // NVRTC library cannot be loaded, or AMI_EINVAL when compilation fails (`log` has the reason).
-int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& log);
+// With `use_cache` the cubin is looked up in / added to the on-disk cache (see ami_jit.cpp).
+int jit_compile(const std::string& src, std::vector<char>& cubin, std::string& log, bool use_cache = true,
+                bool* cache_hit = nullptr);
 
-// Loads the cubin on the table's device.  Thread-safe, idempotent.
-int jit_prepare(ami_table* tab, std::string& err);
-// `launches` (may be NULL) is incremented per kernel launched (the memory-backed variant walks a large
-// batch in chunks).
-cudaError_t jit_launch(const ami_table* tab, bool fused, const AmiBatch& b, cudaStream_t st, int* launches);
+// Compiles (or fetches) and loads the kernels of one variant on the table's device.  Thread-safe, idempotent.
+int jit_prepare(ami_table* tab, const JitVariant& var, std::string& err);
+// `launches` (may be NULL) is incremented per kernel launched; *tally_slots (may be NULL) receives the number of
+// per-row partial sums the fused tally wrote.
+cudaError_t jit_launch(const ami_table* tab, const JitVariant& var, bool fused, const AmiBatch& b, cudaStream_t st,
+                       int* launches, long long* tally_slots);
 void jit_destroy(ami_table* tab);
-int jit_status(const ami_table* tab);   // AMI_OK once loaded, 1 = not tried yet, else the error
+int jit_status(const ami_table* tab);   // of the default variant: AMI_OK once loaded, 1 = not tried yet, else the error
+bool jit_fused_tally_ok(const ami_table* tab);   // the loaded plan forms the Monte-Carlo tally inside its kernel
+double jit_last_compile_ms(const ami_table* tab, int* cache_hit);   // default variant: time spent in jit_prepare
 
 }  // namespace ami

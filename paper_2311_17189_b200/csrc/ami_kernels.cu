@@ -626,21 +626,34 @@ cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long 
 
 // ------------------------------------------------------------------------------------------
 // FP64 pipe probe: independent DFMA chains held in registers.
+//   SRC = 2: x = fma(x, x, b) -- two distinct 64-bit register sources.  Reaches 0.995 of 148 SMs x 64 lanes x
+//            clock on B200: the pipe's issue rate, the roofline's peak.
+//   SRC = 3: x = fma(x, a, b) -- three distinct register sources, the shape of almost every DFMA of real code.
+//            Stops at 0.92 of the same figure even though a and b are shared by all chains (and 0.80 when the
+//            chains alternate between two a's and two b's, profiles/r02_dfma_probe.md): a DFMA that reads three
+//            different register pairs does not issue every second cycle.  Reported beside the peak as the
+//            ceiling of register-operand arithmetic.
 // ------------------------------------------------------------------------------------------
+template <int SRC>
 __global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters, double a, double b) {
-  double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6,
-         x7 = x0 + 7;
+  double x0 = threadIdx.x * 1e-3, x1 = x0 + 0.1, x2 = x0 + 0.2, x3 = x0 + 0.3, x4 = x0 + 0.4, x5 = x0 + 0.5, x6 = x0 + 0.6,
+         x7 = x0 + 0.7;
   for (int i = 0; i < iters; ++i) {
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
-      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
-      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+      if (SRC == 3) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+      } else {
+        x0 = fma(x0, x0, b); x1 = fma(x1, x1, b); x2 = fma(x2, x2, b); x3 = fma(x3, x3, b);
+        x4 = fma(x4, x4, b); x5 = fma(x5, x5, b); x6 = fma(x6, x6, b); x7 = fma(x7, x7, b);
+      }
     }
   }
   out[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
 }
 
-cudaError_t run_fp64_probe(double* dfma_per_s, double* ms_out) {
+cudaError_t run_fp64_probe(int distinct_sources, double* dfma_per_s, double* ms_out) {
   cudaDeviceProp prop;
   int dev = 0;
   cudaError_t rc = cudaGetDevice(&dev);
@@ -657,7 +670,8 @@ cudaError_t run_fp64_probe(double* dfma_per_s, double* ms_out) {
   float best = 1e30f;
   for (int rep = 0; rep < 6; ++rep) {
     cudaEventRecord(e0);
-    dfma_probe_kernel<<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
+    if (distinct_sources == 3) dfma_probe_kernel<3><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
+    else dfma_probe_kernel<2><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
     cudaEventRecord(e1);
     rc = cudaEventSynchronize(e1);
     if (rc != cudaSuccess) break;

@@ -20,8 +20,17 @@ struct AmiBatch {
   long long k_stride_sample, k_stride_comp;
   double q[2 * AMI_K_MAX_EXT];
   double t, mu;
-  double* scratch;          // memory-backed plan: [slots][scratch_stride] doubles, column s belongs to sample s
-  long long scratch_stride;
+  // split plan (tables too large for one register-resident kernel): the leaf kernel writes every Fermi/Bose
+  // value and reciprocal denominator of sample s to column s of leaves[slot][leaf_stride]; part kernel p writes
+  // its partial result of launch-local row r to partial[(p * n_b * n_f + r) * partial_stride + s] (complex)
+  double* leaves;
+  long long leaf_stride;
+  double* partial;
+  long long partial_stride;
+  int n_parts;
+  int part0;                // split plan: index of the first part of the module being launched
+  int tiles;                // fused kernels: consecutive tiles of blockDim.x samples one CTA walks
+  int tally_acc;            // fused tally with ONE result row: every thread adds its `tiles` samples before the warp adds up
   double* e_out;            // optional [n_eps][n] copy of the energies formed by the fused path
   // fused tally (or NULL): per-warp partial sums (re, im, re^2, im^2) of row r at tally[(r * tally_stride + (s >> 5)) * 4]
   double* tally;

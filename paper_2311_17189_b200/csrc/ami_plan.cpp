@@ -245,6 +245,7 @@ void build_horner_plan(const FlatTable& ft, HornerPlan& hp) {
   }
   hp.dn.assign(1, HNode());
   for (int g = 0; g < G; ++g) hp.dn[trie_insert(hp.dn, dseq[g])].group = g;
+  hp.dseq = dseq;
   hp.n_dnodes = (long long)hp.dn.size() - 1;
   count_d_ops(hp, 0, &hp.ops_d_beta, &hp.ops_d);
   // leaf costs on the common path of the routines in ami_device.cuh

@@ -75,6 +75,7 @@ struct HornerPlan {
   std::vector<HGroup> groups;
   std::vector<SNode> snodes; // children have smaller ids than their parents
   std::vector<HNode> dn;     // dn[0] = root
+  std::vector<std::vector<int>> dseq;   // per group: its denominators in the order of its path through dn
   std::vector<char> d_is_real;   // [U_D]: no external-frequency part => purely real denominator
   int f_order = 0;           // which factor ordering won (0 = per-group frequency, 1..4 = global)
   long long n_fnodes = 0, n_dnodes = 0;

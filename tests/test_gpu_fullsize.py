@@ -64,8 +64,8 @@ def test_cfg2_sweep_large_batch_streamed(ami, oracle_mod, name):
     tab = ami.AmiTable.from_diagram(cfg.diagram)
     d_out = torch.empty((1, 8, n), dtype=torch.complex128, device="cuda")
     stats, sums = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, seed=cfg.seed,
-                          d_out=d_out, want_sum=True)
-    assert stats["n_chunks"] >= 5 and stats["h2d_bytes"] == 0
+                          d_out=d_out, want_sum=True, chunk=1 << 21)
+    assert stats["n_chunks"] == 5 and stats["h2d_bytes"] == 0
     sel = np.linspace(0, n - 1, 4000).astype(np.int64)
     got = d_out[:, :, torch.from_numpy(sel).cuda()].cpu().numpy()
     (truth, S), = oracle_subset(oracle_mod, cfg, sel)

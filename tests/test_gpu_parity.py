@@ -242,15 +242,12 @@ def test_register_plan_is_what_auto_runs(ami, torch_mod, name):
 
 
 def test_register_plan_limits(ami, torch_mod):
-    """Tables outside the limits (order 8) and complex energies run the table-driven kernels under
-    AUTO and are refused under an explicit AMI_PLAN_REG."""
+    """Complex energies run the table-driven kernels under AUTO and are refused under an explicit AMI_PLAN_REG;
+    tables beyond one register-resident kernel (order 8) are specialised as a split plan."""
     cfg = A.get_config("stress8")
     tab = ami.AmiTable.from_diagram(cfg.diagram)
-    assert tab.info["reg_plan_status"] == -6
-    e = gpu_energies(torch_mod, tab, cfg, cfg.momenta(40))
-    with pytest.raises(ami.AmiError) as ei:
-        tab.evaluate(e, cfg.z_ext, cfg.betas, plan=ami.PLAN_REG)
-    assert ei.value.code == -6
+    assert tab.info["reg_plan_status"] == 1 and tab.info["plan_kind"] == 2
+    assert ami.AmiTable.from_diagram(A.get_config("cfg4").diagram).info["plan_kind"] == 1
     cfg = A.get_config("cfg3")
     tab = ami.AmiTable.from_diagram(cfg.diagram)
     ec = gpu_energies(torch_mod, tab, cfg, cfg.momenta(40)).to(torch_mod.complex128)
@@ -332,45 +329,62 @@ def test_extreme_temperatures(ami, torch_mod, oracle_mod, name, plan):
     assert all(st["n_nonfinite"] == 0 for st in sts)
 
 
-def test_memory_backed_plan_opt_in(ami, torch_mod):
-    """AMI_JIT_SCRATCH=1: tables beyond the register plan's limits get the same generated arithmetic
-    with leaves in shared memory and long-lived sums in a global scratch.  Run in a fresh process with
-    the limits lowered so that the order-6 table takes that path (an order-8 body compiles for minutes)."""
-    import os
-    import subprocess
-    import sys
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    code = """
-import sys; sys.path.insert(0, 'tests')
-import numpy as np, torch
-import ami_inputs as A, paper_2311_17189_b200 as P, oracle
-from parity import check_parity
-cfg = A.get_config('cfg4'); n = 2000 + 37
-tab = P.AmiTable.from_diagram(cfg.diagram)
-k = tab.generate_momenta(cfg.seed, 0, n)
-out = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=P.PLAN_REG)
-assert tab.refresh_info()['reg_plan_status'] == 0
-ot = oracle.OracleTable.from_diagram(cfg.diagram)
-sel = np.arange(0, n, 7)
-e_rows = ot.dispersion(cfg.momenta(n)[sel], [cfg.q], cfg.t, cfg.mu)
-truth, S = ot.evaluate(e_rows, cfg.z_ext, cfg.betas[0], e_reg=cfg.e_reg, quad=True, threads=oracle.hardware_threads(), want_S=True)
-check_parity(out.cpu().numpy()[0][:, sel], truth, S, label='scratch plan')
-two = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, [[1j], [2.0 + 0.5j]], [3.0, 10.0], e_reg=cfg.e_reg)
-ref = tab.evaluate(tab.dispersion(k, [cfg.q], cfg.t, cfg.mu), [[1j], [2.0 + 0.5j]], [3.0, 10.0], e_reg=cfg.e_reg, plan=P.PLAN_FLAT)
-err = (two - ref).abs().max().item(); scale = ref.abs().max().item()
-assert err <= 1e-9 * scale, (err, scale)
-print('SCRATCH-OK', 'W(' in tab.kernel_source())
-"""
-    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, cwd=root, timeout=600,
-                         env=dict(os.environ, AMI_JIT_SCRATCH="1", AMI_JIT_MAX_EDGES="100"))
-    assert out.returncode == 0, out.stderr[-3000:]
-    assert "SCRATCH-OK True" in out.stdout
+def split_case(name):
+    """Tables beyond one register-resident kernel: the order-8 stress table (T = 40244) and an order-7 one (T = 8598)."""
+    if name == "o7":
+        return A.get_config("stress8", diagram=A.random_self_energy(7, 0), name="o7")
+    return A.get_config(name)
 
 
-def test_generator_knobs_do_not_change_the_bits(ami, torch_mod, tmp_path):
-    """The schedule knobs of the specialised kernels (chains side by side, register cap, store policy, tiles per
-    CTA, L2 prefetch, leaves in shared memory) reorder instructions, not arithmetic: every setting returns the
-    bits of the default build, on the single- and the several-temperature body."""
+@pytest.mark.parametrize("name", ["o7", "stress8"])
+def test_split_plan_large_tables(ami, torch_mod, oracle_mod, name):
+    """AMI_PLAN_AUTO / AMI_PLAN_REG for orders 7-8 (PAPER.md:389-393 runs m = 9): the split plan -- leaf kernel,
+    the Horner plan's groups in parts of register-plan size (one launch, grid.y = part), combine kernel.  Values
+    against the oracle (double precision as truth: quad is too slow for 4e4 terms; the bar is still 1e-10 S),
+    fused == unfused bit for bit, a (beta, frequency) grid, and a batch that spans several sample chunks."""
+    cfg = split_case(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    assert tab.info["plan_kind"] == 2 and tab.info["reg_plan_status"] == 1
+    n = 300 + 7
+    k = torch_mod.from_numpy(cfg.momenta(n)).cuda()
+    e = tab.dispersion(k, [cfg.q], cfg.t, cfg.mu)
+    out = tab.evaluate(e, cfg.z_ext, cfg.betas, plan=ami.PLAN_AUTO)
+    info = tab.refresh_info()
+    assert info["reg_plan_status"] == 0 and info["specialize_ms"] > 0
+    fused = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, plan=ami.PLAN_REG)
+    assert torch_mod.equal(out, fused)
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    e_rows = e.cpu().numpy().T.copy()
+    thr = oracle_mod.hardware_threads()
+    truth, S = ot.evaluate(e_rows, cfg.z_ext, cfg.betas[0], quad=False, threads=thr, want_S=True)
+    st = check_parity(out.cpu().numpy()[0], truth, S, label=name)
+    assert st["n_nonfinite"] == 0
+    # the table-driven interpretation of the same Horner plan agrees too
+    tree = tab.evaluate(e, cfg.z_ext, cfg.betas, plan=ami.PLAN_TREE).cpu().numpy()
+    check_parity(tree[0], truth, S, label=name + " tree")
+    # several temperatures and frequencies (one of them continued to the real axis)
+    z = np.array([[1j * math.pi / 5.0], [0.3 + 0.1j], [3j * math.pi / 5.0]])
+    betas = (5.0, 2.0)
+    grid = tab.evaluate(e[:, :96].contiguous(), z, betas).cpu().numpy()
+    for b, beta in enumerate(betas):
+        truth, S = ot.evaluate(e_rows[:96], z, beta, quad=False, threads=thr, want_S=True)
+        check_parity(grid[b], truth, S, label=f"{name} grid beta={beta}")
+    # a batch larger than one chunk of the leaf array: same bits as the small batch on the shared samples,
+    # and the streamed driver's tally (unfused here: the parts' results are added before they are summed)
+    big = 70_000 + 13
+    kb = tab.generate_momenta(cfg.seed, 0, big)
+    ob = tab.evaluate_momenta(kb, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas)
+    assert torch_mod.equal(ob[:, :, :n], out)
+    tail = tab.evaluate_momenta(kb[big - 500:].contiguous(), [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas)
+    assert torch_mod.equal(ob[:, :, big - 500:], tail)
+    stats, sums = tab.run(5000 + 3, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, want_sum=True)
+    ref = ob[:, :, :5003].sum(dim=2).cpu().numpy()
+    assert np.max(np.abs(sums - ref)) <= 1e-12 * np.abs(ob[:, :, :5003]).sum().item()
+
+
+def test_kernel_cache_on_disk(ami, torch_mod, tmp_path):
+    """The compiled kernels are kept on disk (AMI_JIT_CACHE): a second process on the same diagram loads them
+    without compiling -- reported by ami_table_info -- and returns the same bits; AMI_JIT_CACHE=0 compiles."""
     import os
     import subprocess
     import sys
@@ -378,30 +392,62 @@ def test_generator_knobs_do_not_change_the_bits(ami, torch_mod, tmp_path):
     code = """
 import sys, numpy as np, torch
 import ami_inputs as A, paper_2311_17189_b200 as P
-res = []
-for name in ('cfg3', 'cfg4'):
-    cfg = A.get_config(name); n = 1000 + 29
-    tab = P.AmiTable.from_diagram(cfg.diagram)
-    k = tab.generate_momenta(cfg.seed, 0, n)
-    res.append(tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=P.PLAN_REG).cpu().numpy())
-    res.append(tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, [[1j], [2.0 + 0.5j]], [3.0, 10.0], e_reg=cfg.e_reg, plan=P.PLAN_REG).cpu().numpy())
-    assert tab.refresh_info()['reg_plan_status'] == 0
-np.savez(sys.argv[1], *res)
+cfg = A.get_config('cfg4'); n = 1000 + 29
+tab = P.AmiTable.from_diagram(cfg.diagram)
+info = tab.specialize()
+k = tab.generate_momenta(cfg.seed, 0, n)
+out = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=P.PLAN_REG).cpu().numpy()
+np.save(sys.argv[1], out)
+print('CACHED', info['specialize_cached'], 'MS', info['specialize_ms'])
 """
-    settings = [{}, {"AMI_JIT_WAYS": "4", "AMI_JIT_MINB": "1", "AMI_JIT_STORE": "0"},
-                {"AMI_JIT_WAYS": "3", "AMI_JIT_MINB": "8", "AMI_JIT_STORE": "2", "AMI_JIT_U": "2", "AMI_JIT_PF": "7"},
-                {"AMI_JIT_SMEM_F": "1", "AMI_JIT_NT": "128", "AMI_JIT_PDL": "0"}]
-    outs = []
-    for i, extra in enumerate(settings):
-        path = str(tmp_path / f"knobs{i}.npz")
+    cache = str(tmp_path / "jitcache")
+    runs = []
+    for i, env in enumerate(({"AMI_JIT_CACHE": cache}, {"AMI_JIT_CACHE": cache}, {"AMI_JIT_CACHE": "0"})):
+        path = str(tmp_path / f"out{i}.npy")
         r = subprocess.run([sys.executable, "-c", code, path], capture_output=True, text=True, cwd=root, timeout=600,
-                           env=dict(os.environ, **extra))
-        assert r.returncode == 0, (extra, r.stderr[-3000:])
-        with np.load(path) as z:
-            outs.append([z[key] for key in z.files])
-    for i in range(1, len(outs)):
-        for a, b in zip(outs[0], outs[i]):
-            assert np.array_equal(a, b, equal_nan=True), settings[i]
+                           env=dict(os.environ, **env))
+        assert r.returncode == 0, r.stderr[-3000:]
+        words = r.stdout.split()
+        runs.append((int(words[words.index("CACHED") + 1]), float(words[words.index("MS") + 1]), np.load(path)))
+    assert [r[0] for r in runs] == [0, 1, 0]
+    assert os.listdir(cache)
+    assert runs[1][1] < 100.0 and runs[1][1] < 0.5 * runs[0][1]      # milliseconds instead of an NVRTC compile
+    assert np.array_equal(runs[0][2], runs[1][2]) and np.array_equal(runs[0][2], runs[2][2])
+
+
+@pytest.mark.parametrize("dim,band", [(1, 0), (3, 0), (2, 1), (3, 1)])
+def test_fused_lattice_variants(ami, torch_mod, oracle_mod, dim, band):
+    """ami_evaluate_momenta_lattice and ami_run(dim, band): other dimensions and the free-particle band (Eq. 14,
+    PAPER.md:346; :295) in ONE specialised kernel, bit-identical to ami_dispersion_lattice + ami_evaluate, momenta
+    drawn in the kernel included; values against the oracle from the oracle's own quad dispersion."""
+    from ami_inputs.rng import momenta
+    cfg = A.get_config("cfg3")
+    n = 3000 + 5
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    seed = cfg.seed + 11 * dim + band
+    k_host = momenta(seed, n, cfg.diagram.n_int, d=dim)
+    k = torch_mod.from_numpy(k_host).cuda()
+    q = np.array([0.5 * math.pi, -0.25 * math.pi, 1.0][:dim])
+    t, mu = (1.0, -0.2) if band == 0 else (0.5, 1.5)
+    e = tab.dispersion(k, [q], t, mu, dim=dim, band=band)
+    two = tab.evaluate(e, cfg.z_ext, cfg.betas, plan=ami.PLAN_REG)
+    e_out = torch_mod.zeros_like(e)
+    one = tab.evaluate_momenta(k, [q], t, mu, cfg.z_ext, cfg.betas, plan=ami.PLAN_REG, dim=dim, band=band, e_out=e_out)
+    assert tab.refresh_info()["reg_plan_status"] == 0
+    assert torch_mod.equal(one, two) and torch_mod.equal(e_out, e)
+    gen = tab.generate_momenta(seed, 0, n, dim=dim)
+    assert torch_mod.equal(gen, k)
+    d_out = torch_mod.zeros_like(one)
+    stats, sums = tab.run(n, [q], t, mu, cfg.z_ext, cfg.betas, seed=seed, d_out=d_out, want_sum=True, chunk=1024,
+                          dim=dim, band=band)
+    assert torch_mod.equal(d_out, one)
+    assert np.max(np.abs(sums - one.sum(dim=2).cpu().numpy())) <= 1e-12 * one.abs().sum().item()
+    flat = tab.evaluate_momenta(k, [q], t, mu, cfg.z_ext, cfg.betas, plan=ami.PLAN_FLAT, dim=dim, band=band)   # workspace inside
+    assert torch_mod.equal(flat, tab.evaluate(e, cfg.z_ext, cfg.betas, plan=ami.PLAN_FLAT))
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    truth, S = ot.evaluate(np.ascontiguousarray(e.cpu().numpy().T), cfg.z_ext, cfg.betas[0], quad=True,
+                           threads=oracle_mod.hardware_threads(), want_S=True)
+    check_parity(one.cpu().numpy()[0], truth, S, label=f"fused dim={dim} band={band}")
 
 
 # ------------------------------------------------------------------ S4 streamed driver
@@ -498,6 +544,71 @@ def test_run_fused_tally(ami, torch_mod, name, n):
     # the table-driven plan (results re-read by the tally kernels) agrees to rounding
     _, flat = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, plan=ami.PLAN_FLAT, **kw)
     assert np.all(np.abs(flat - only) <= 1e-9 * np.abs(v).sum(axis=-1))
+
+
+@pytest.mark.parametrize("name,n,kw", [("cfg1", 20_000 + 7, {}), ("cfg3", 6000 + 1, {}), ("cfg3", 150_000 + 9, {"truth_every": 25}),
+                                       ("cfg2_bubble", 9000 + 3, {"chunk": 2048}), ("cfg2_se", 5000, {"plan": "flat"})])
+def test_run_tally_against_oracle_mean(ami, torch_mod, oracle_mod, name, n, kw):
+    """The Monte-Carlo tally of S4 (the integrator averages the result rows) beside the ORACLE's mean
+    and sums of squares of the same seeded samples, under rule (3) of the parity norm: the fused tally (per-warp
+    partials, or per-thread sums when there is one row and the batch is large), the chunked one and the
+    table-driven plan's.  With truth_every the oracle sees every k-th sample and the GPU the same subset through
+    d_out, while the tally of the whole batch is checked against the GPU's own results to rounding."""
+    cfg = A.get_config(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    plan = PLANS[kw.get("plan", "auto")]
+    every = kw.get("truth_every", 1)
+    d_out = torch_mod.zeros((len(cfg.betas), len(cfg.z_ext), n), dtype=torch_mod.complex128, device="cuda") if every > 1 else None
+    stats, sums = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, seed=cfg.seed, want_sum=True,
+                          chunk=kw.get("chunk", 0), plan=plan, d_out=d_out)
+    sumsq = tab.last_sumsq.copy()
+    only_stats, only = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, seed=cfg.seed,
+                               want_sum=True, chunk=kw.get("chunk", 0), plan=plan)
+    assert np.array_equal(only, sums) or every > 1       # with and without stored results: the same tally
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    sel = np.arange(0, n, every)
+    e_rows = ot.dispersion(cfg.momenta(n)[sel], [cfg.q], cfg.t, cfg.mu)
+    for b, beta in enumerate(cfg.betas):
+        truth, S = ot.evaluate(e_rows, cfg.z_ext, beta, e_reg=cfg.e_reg, quad=True, threads=oracle_mod.hardware_threads(),
+                               want_S=True)
+        if every > 1:
+            got = d_out[b][:, torch_mod.from_numpy(sel).cuda()].cpu().numpy()
+            check_parity(got, truth, S, label=f"{name} run subset")
+            ref = d_out[b].sum(dim=1).cpu().numpy()
+            assert np.all(np.abs(sums[b] - ref) <= 1e-12 * d_out[b].abs().sum(dim=1).cpu().numpy())
+            continue
+        mean_gpu, mean_truth = sums[b] / n, truth.mean(axis=1)
+        assert np.all(np.abs(mean_gpu - mean_truth) <= 1e-10 * S.mean(axis=1)), (mean_gpu, mean_truth)
+        well = S.mean(axis=1) <= 1e3 * np.abs(mean_truth)
+        assert np.all(np.abs(mean_gpu - mean_truth)[well] <= 1e-10 * np.abs(mean_truth)[well])
+        sq_truth = np.stack([(truth.real ** 2).sum(axis=1), (truth.imag ** 2).sum(axis=1)], axis=-1)
+        assert np.all(np.abs(sumsq[b] - sq_truth) <= 1e-10 * (S ** 2).sum(axis=1)[:, None])
+
+
+def test_run_workspace_across_plans_and_refusals(ami, torch_mod):
+    """One table, the table-driven plan with a small chunk first and the specialised kernels with a larger chunk
+    afterwards: the driver's workspace (energy buffer of the first call) must not be handed to the second, which
+    forms its energies in registers.  A request with no destination at all is refused, not executed."""
+    cfg = A.get_config("cfg3")
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    n = 20_000 + 3
+    a = torch_mod.zeros((1, 1, n), dtype=torch_mod.complex128, device="cuda")
+    b = torch_mod.zeros_like(a)
+    tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, d_out=a, plan=ami.PLAN_FLAT, chunk=512)
+    tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, d_out=b, plan=ami.PLAN_REG, chunk=8192)
+    torch_mod.cuda.synchronize()
+    ref = tab.evaluate_momenta(tab.generate_momenta(cfg.seed, 0, n), [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas)
+    assert torch_mod.equal(b, ref)
+    assert (a - b).abs().max().item() <= 1e-9 * b.abs().max().item()
+    h_k = torch_mod.from_numpy(cfg.momenta(n).reshape(n, -1)).pin_memory()
+    h_out = torch_mod.zeros((1, 1, n), dtype=torch_mod.complex128).pin_memory()
+    st, _ = tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, h_k=h_k, h_out=h_out, chunk=1000)   # pipelined
+    assert st["n_chunks"] == 21 and torch_mod.equal(h_out.cuda(), ref)
+    with pytest.raises(ami.AmiError) as ei:
+        tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed)       # nowhere to put anything
+    assert ei.value.code == -1
+    with pytest.raises(ami.AmiError):
+        tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, d_out=a, dim=4)
 
 
 def test_run_device_output_and_determinism(ami, torch_mod):
