@@ -572,8 +572,9 @@ def run_ours(args, dist, rank, local, world):
                 continue
             # order7 / stress8: tables beyond one register-resident kernel (T = 8598 / 40244; the paper runs m = 9,
             # PAPER.md:389-393), outside the five graded configurations; they run the split plan
-            c2 = A.get_config("stress8", diagram=A.random_self_energy(7, 0), name="order7") if name == "order7" \
-                else A.get_config(name)
+            c2 = A.get_config("stress8" if name == "order7" else name)
+            if name == "order7":
+                c2.diagram, c2.name = A.random_self_energy(7, 0), "order7"
             r2 = time_workload(pkg, torch, c2, c2.n_samples, 20, 3, plan, 0, None, sample_clocks=False,
                                use_graph=not args.no_graph)
             i2 = r2["info"]

@@ -70,7 +70,7 @@ enum {
                          AMI_PLAN_AUTO runs when the register plan is not available for the table */
   AMI_PLAN_REG = 2    /* specialised kernels: the table written out as straight-line code for this diagram
                          (terms grouped by denominator product, Fermi/Bose and denominator products in Horner
-                         form), compiled with NVRTC on first use and cached on disk; real energies.  Tables of
+                         form), compiled with NVRTC on first use and cached on disk; real or complex energies.  Tables of
                          orders up to 6-7 become ONE kernel with every value in a register (register plan);
                          larger ones (order 7-8, 1e4-1e5 flat terms) are split: a leaf kernel, then the groups
                          of the Horner plan in parts of register-plan size evaluated by one launch (grid.y =
@@ -193,6 +193,15 @@ int ami_search_sum_order(int n_int, int n_ext, int n_g, int n_eps, const int32_t
  * Call with buf = NULL to get the size (terminating NUL included) in *bytes. */
 int ami_table_latex(const ami_table* tab, char* buf, size_t* bytes);
 
+/* The same result in the factorised form the paper prints (PAPER.md:100-104, Eq. 6: FT * R; :115-132): terms grouped
+ * by their denominator product R_g, the Fermi/Bose sums FT_g in Horner form with every sum that several groups share
+ * named once (the library's Horner plan, i.e. what the specialised kernels execute):
+ *   S_{n} ={}& [coef] f(..) [S_{child}] ...   one row per shared sum, children before parents
+ *   I ={}& + S_{root(g)} \frac{1}{(D)^{p}} ...   one row per group
+ * Far shorter than the flat table (order 6: 48 + ~230 rows of a few factors against 688 rows of 11).  Same notation
+ * and buffer protocol as ami_table_latex. */
+int ami_table_latex_factorized(const ami_table* tab, char* buf, size_t* bytes);
+
 /* Serialises the flat table for inspection and tests.  Call with host_buf = NULL to get the size
  * in *bytes; then with a buffer of at least that size.  Layout (little endian, all int32 unless
  * noted): magic 'AMI1', n_int, n_ext, n_eps, U_F, U_D, T, m_f (Fermi factors per term = n_int),
@@ -295,6 +304,13 @@ int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char*
  * the other, ami_table_kernel_cubin_unit compiles unit `unit` (ami_table_kernel_cubin is unit 0). */
 int ami_table_kernel_units(const ami_table* tab, int* n_units);
 int ami_table_kernel_cubin_unit(const ami_table* tab, int unit, void* buf, size_t* bytes, char* log, size_t log_cap);
+/* The kernels are generated per variant: lattice of the inline dispersion (dim, band as in ami_dispersion_lattice) and
+ * real or complex energies (complex ones: tables of register-plan size, ami_evaluate only).  The calls
+ * above return the variant of the configurations (2, tight binding, real); these return any. */
+int ami_table_kernel_source_variant(const ami_table* tab, int dim, int band, int complex_energies, char* buf,
+                                    size_t* bytes);
+int ami_table_kernel_cubin_variant(const ami_table* tab, int dim, int band, int complex_energies, int unit, void* buf,
+                                   size_t* bytes, char* log, size_t log_cap);
 
 /* Streamed driver.  Source of the momenta: if h_k / d_k are both NULL they are generated on the
  * device from `seed` with the counter-based generator of P22 (sample index = first_sample + s) --

@@ -22,7 +22,8 @@ EXPORTS = [
     "ami_table_kernel_cubin", "ami_run", "ami_generate_momenta", "ami_fp64_peak_probe", "ami_strerror",
     "ami_last_cuda_error", "ami_version", "ami_kernel_launches", "ami_search_sum_order", "ami_graph_parse",
     "ami_graph_label", "ami_table_latex", "ami_evaluate_momenta_lattice", "ami_generate_momenta_lattice",
-    "ami_table_kernel_units", "ami_table_kernel_cubin_unit",
+    "ami_table_kernel_units", "ami_table_kernel_cubin_unit", "ami_table_kernel_source_variant",
+    "ami_table_kernel_cubin_variant", "ami_table_latex_factorized",
 ]
 
 
@@ -77,6 +78,7 @@ def lib():
         L.ami_table_export_tree.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.ami_table_destroy.argtypes = [C.c_void_p]
         L.ami_table_latex.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
+        L.ami_table_latex_factorized.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_size_t)]
         L.ami_table_destroy.restype = None
         L.ami_dispersion.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_double,
                                      C.c_double, C.c_int64, C.c_void_p, C.c_void_p]
@@ -99,6 +101,9 @@ def lib():
         L.ami_table_kernel_units.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
         L.ami_table_kernel_cubin_unit.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.POINTER(C.c_size_t), C.c_void_p,
                                                   C.c_size_t]
+        L.ami_table_kernel_source_variant.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.POINTER(C.c_size_t)]
+        L.ami_table_kernel_cubin_variant.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p,
+                                                     C.POINTER(C.c_size_t), C.c_void_p, C.c_size_t]
         L.ami_run.argtypes = [C.c_void_p, C.POINTER(ami_run_cfg), C.POINTER(ami_run_stats)]
         L.ami_generate_momenta.argtypes = [C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
         L.ami_fp64_peak_probe.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -165,12 +170,14 @@ class AmiTable:
 
     __del__ = close
 
-    def latex(self) -> str:
-        """ami_table_latex: the flat term table as LaTeX."""
+    def latex(self, factorized=False) -> str:
+        """ami_table_latex: the flat term table as LaTeX, or (factorized) the FT * R form with
+        the Fermi/Bose sums in Horner form, shared sums named once (ami_table_latex_factorized)."""
+        fn = lib().ami_table_latex_factorized if factorized else lib().ami_table_latex
         n = C.c_size_t(0)
-        _check(lib().ami_table_latex(self._h, None, C.byref(n)))
+        _check(fn(self._h, None, C.byref(n)))
         buf = C.create_string_buffer(n.value)
-        _check(lib().ami_table_latex(self._h, buf, C.byref(n)))
+        _check(fn(self._h, buf, C.byref(n)))
         return buf.value.decode()
 
     def _info(self) -> dict:
@@ -188,11 +195,12 @@ class AmiTable:
         _check(lib().ami_table_specialize(self._h))
         return self.refresh_info()
 
-    def kernel_source(self) -> str:
+    def kernel_source(self, dim=2, band=BAND_TIGHT_BINDING, complex_energies=False) -> str:
         n = C.c_size_t(0)
-        _check(lib().ami_table_kernel_source(self._h, None, C.byref(n)))
+        args = (self._h, int(dim), int(band), int(bool(complex_energies)))
+        _check(lib().ami_table_kernel_source_variant(*args, None, C.byref(n)))
         buf = C.create_string_buffer(n.value)
-        _check(lib().ami_table_kernel_source(self._h, buf, C.byref(n)))
+        _check(lib().ami_table_kernel_source_variant(*args, buf, C.byref(n)))
         return buf.value.decode()
 
     def kernel_units(self) -> int:
@@ -201,12 +209,13 @@ class AmiTable:
         _check(lib().ami_table_kernel_units(self._h, C.byref(n)))
         return n.value
 
-    def kernel_cubin(self, cap=64 << 20, unit=0):
-        """(cubin bytes, compiler log) of translation unit ``unit``; needs NVRTC but no GPU."""
+    def kernel_cubin(self, cap=64 << 20, unit=0, dim=2, band=BAND_TIGHT_BINDING, complex_energies=False):
+        """(cubin bytes, compiler log) of translation unit ``unit`` of a variant; needs NVRTC but no GPU."""
         buf = C.create_string_buffer(cap)
         log = C.create_string_buffer(1 << 18)
         n = C.c_size_t(cap)
-        _check(lib().ami_table_kernel_cubin_unit(self._h, int(unit), buf, C.byref(n), log, len(log)))
+        _check(lib().ami_table_kernel_cubin_variant(self._h, int(dim), int(band), int(bool(complex_energies)), int(unit),
+                                                    buf, C.byref(n), log, len(log)))
         return buf.raw[: n.value], log.value.decode()
 
     def export(self) -> dict:

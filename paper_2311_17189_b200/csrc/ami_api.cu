@@ -345,7 +345,8 @@ int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg
     if (use_tree) *use_tree = true;
     return AMI_OK;
   }
-  if (e_is_complex || !ami::jit_eligible(tab->flat, tab->horner)) {
+  if (!ami::jit_eligible(tab->flat, tab->horner) ||
+      (e_is_complex && ami::jit_mode(tab->flat, tab->horner) != ami::kJitRegister)) {
     if (plan == AMI_PLAN_REG) { g_cuda_err = "register plan unavailable for this table / energy type"; return AMI_EUNSUPPORTED; }
     if (use_tree) *use_tree = tree_auto;        // AUTO: the table-driven Horner program for large tables
     return AMI_OK;
@@ -387,6 +388,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
   bool use_reg = false, use_tree = false;
   ami::JitVariant var;
   if (mom) { var.dim = mom->dim; var.band = mom->band; }
+  var.cplx = e_is_complex != 0;
   int rc = choose_plan(tab, plan, e_is_complex != 0, &use_reg, &use_tree, var);
   if (rc != AMI_OK) return rc;
   const int dim = var.dim;
@@ -603,10 +605,22 @@ int ami_table_specialize(ami_table* tab) {
   return rc;
 }
 
-int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes) {
+namespace {
+int variant_of(int dim, int band, int complex_energies, ami::JitVariant* var) {
+  if (dim < 1 || dim > 3 || (band != AMI_BAND_TIGHT_BINDING && band != AMI_BAND_FREE)) return AMI_EINVAL;
+  var->dim = dim; var->band = band; var->cplx = complex_energies != 0;
+  return AMI_OK;
+}
+}  // namespace
+
+int ami_table_kernel_source_variant(const ami_table* tab, int dim, int band, int complex_energies, char* buf,
+                                    size_t* bytes) {
   if (!tab || !bytes) return AMI_EINVAL;
+  ami::JitVariant var;
+  if (variant_of(dim, band, complex_energies, &var)) return AMI_EINVAL;
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
-  const std::vector<std::string> srcs = ami::jit_generate_sources(tab->flat, tab->horner, ami::JitVariant(), nullptr);
+  if (var.cplx && ami::jit_mode(tab->flat, tab->horner) != ami::kJitRegister) return AMI_EUNSUPPORTED;
+  const std::vector<std::string> srcs = ami::jit_generate_sources(tab->flat, tab->horner, var, nullptr);
   std::string src;
   for (size_t i = 0; i < srcs.size(); ++i) {
     if (srcs.size() > 1) src += "// ======== translation unit " + std::to_string(i) + " of " + std::to_string(srcs.size()) + " ========\n";
@@ -619,6 +633,10 @@ int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes) {
   return AMI_OK;
 }
 
+int ami_table_kernel_source(const ami_table* tab, char* buf, size_t* bytes) {
+  return ami_table_kernel_source_variant(tab, 2, AMI_BAND_TIGHT_BINDING, 0, buf, bytes);
+}
+
 int ami_table_kernel_units(const ami_table* tab, int* n_units) {
   if (!tab || !n_units) return AMI_EINVAL;
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
@@ -626,10 +644,14 @@ int ami_table_kernel_units(const ami_table* tab, int* n_units) {
   return AMI_OK;
 }
 
-int ami_table_kernel_cubin_unit(const ami_table* tab, int unit, void* buf, size_t* bytes, char* log, size_t log_cap) {
+int ami_table_kernel_cubin_variant(const ami_table* tab, int dim, int band, int complex_energies, int unit, void* buf,
+                                   size_t* bytes, char* log, size_t log_cap) {
   if (!tab || !bytes) return AMI_EINVAL;
+  ami::JitVariant var;
+  if (variant_of(dim, band, complex_energies, &var)) return AMI_EINVAL;
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
-  const std::vector<std::string> srcs = ami::jit_generate_sources(tab->flat, tab->horner, ami::JitVariant(), nullptr);
+  if (var.cplx && ami::jit_mode(tab->flat, tab->horner) != ami::kJitRegister) return AMI_EUNSUPPORTED;
+  const std::vector<std::string> srcs = ami::jit_generate_sources(tab->flat, tab->horner, var, nullptr);
   if (unit < 0 || unit >= (int)srcs.size()) return AMI_EINVAL;
   std::vector<char> cubin;
   std::string lg;
@@ -646,6 +668,10 @@ int ami_table_kernel_cubin_unit(const ami_table* tab, int unit, void* buf, size_
   }
   *bytes = cubin.size();
   return AMI_OK;
+}
+
+int ami_table_kernel_cubin_unit(const ami_table* tab, int unit, void* buf, size_t* bytes, char* log, size_t log_cap) {
+  return ami_table_kernel_cubin_variant(tab, 2, AMI_BAND_TIGHT_BINDING, 0, unit, buf, bytes, log, log_cap);
 }
 
 int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char* log, size_t log_cap) {

@@ -257,6 +257,98 @@ CV emit_d_sum(const HornerPlan& hp, const std::vector<std::string>& qname, int n
   return acc;
 }
 
+// ---- complex energies (energy_t is complex128 in the paper; reading P19 variant 5b) ----------
+// The same plan with every value a pair of doubles.  acc + a * b for values that may be purely real:
+CV emit_cv_fma(const CV& a, const CV& b, const CV* accp, Emitter& E, Stmts& out) {
+  CV r;
+  {   // real part: a.re*b.re - a.im*b.im (+ acc.re)
+    std::string inner = accp ? accp->re : "";
+    if (!a.real() && !b.real()) {
+      const std::string t = E.fresh("c");
+      if (inner.empty()) out.push_back("const double " + t + " = -" + a.im + " * " + b.im + ";");
+      else out.push_back("const double " + t + " = fma(-" + a.im + ", " + b.im + ", " + inner + ");");
+      inner = t;
+    }
+    r.re = E.fresh("c");
+    if (inner.empty()) out.push_back("const double " + r.re + " = " + a.re + " * " + b.re + ";");
+    else out.push_back("const double " + r.re + " = fma(" + a.re + ", " + b.re + ", " + inner + ");");
+  }
+  {   // imaginary part: a.re*b.im + a.im*b.re (+ acc.im)
+    std::string inner = (accp && !accp->real()) ? accp->im : "";
+    if (!b.real()) {
+      const std::string t = E.fresh("c");
+      if (inner.empty()) out.push_back("const double " + t + " = " + a.re + " * " + b.im + ";");
+      else out.push_back("const double " + t + " = fma(" + a.re + ", " + b.im + ", " + inner + ");");
+      inner = t;
+    }
+    if (!a.real()) {
+      const std::string t = E.fresh("c");
+      if (inner.empty()) out.push_back("const double " + t + " = " + a.im + " * " + b.re + ";");
+      else out.push_back("const double " + t + " = fma(" + a.im + ", " + b.re + ", " + inner + ");");
+      inner = t;
+    }
+    r.im = inner;
+  }
+  return r;
+}
+
+CV cv_leaf_f(int u) { return CV{"Fr" + std::to_string(u), "Fi" + std::to_string(u)}; }
+CV cv_leaf_d(int u) { return CV{"Dr" + std::to_string(u), "Di" + std::to_string(u)}; }
+CV cv_snode(int id) { return CV{"Sr" + std::to_string(id), "Si" + std::to_string(id)}; }
+
+// S-node `id` with complex leaves: defines Sr<id>, Si<id>
+void emit_snode_cplx(const HornerPlan& hp, int id, Emitter& E, Stmts& out) {
+  const SNode& n = hp.snodes[id];
+  CV acc;
+  bool have = false;
+  for (const SItem& it : n.items) {
+    if (it.child >= 0) {
+      acc = emit_cv_fma(cv_leaf_f(it.leaf), cv_snode(it.child), have ? &acc : nullptr, E, out);
+    } else {
+      const CV coef{dlit((double)it.num / (double)it.den), ""};
+      acc = emit_cv_fma(coef, cv_leaf_f(it.leaf), have ? &acc : nullptr, E, out);
+    }
+    have = true;
+  }
+  const CV s = cv_snode(id);
+  out.push_back("const double " + s.re + " = " + acc.re + ", " + s.im + " = " + (acc.real() ? std::string("0.0") : acc.im) + ";");
+}
+
+// Q(n) as in emit_q; with complex energies the frequency-independent denominators are complex too
+CV emit_q_cplx(const HornerPlan& hp, int n, Emitter& E, Stmts& out, bool* have_out) {
+  CV acc;
+  bool have = false;
+  if (hp.dn[n].group >= 0) {
+    const std::string g = std::to_string(hp.dn[n].group);
+    acc = CV{"FTr" + g, "FTi" + g};
+    have = true;
+  }
+  for (int c : hp.dn[n].kids) {
+    if (!hp.d_is_real[hp.dn[c].leaf]) continue;
+    bool sub_have = false;
+    const CV qc = emit_q_cplx(hp, c, E, out, &sub_have);   // never empty: a trie leaf carries a group
+    acc = emit_cv_fma(cv_leaf_d(hp.dn[c].leaf), qc, have ? &acc : nullptr, E, out);
+    have = true;
+  }
+  *have_out = have;
+  return acc;
+}
+
+CV emit_d_sum_cplx(const HornerPlan& hp, const std::vector<CV>& q, const std::vector<char>& q_have, int n, Emitter& E,
+                   Stmts& out) {
+  CV acc;
+  bool have = false;
+  if (q_have[n]) { acc = q[n]; have = true; }
+  for (int c : hp.dn[n].kids) {
+    if (hp.d_is_real[hp.dn[c].leaf]) continue;
+    const CV s = emit_d_sum_cplx(hp, q, q_have, c, E, out);
+    acc = emit_cv_fma(cv_leaf_d(hp.dn[c].leaf), s, have ? &acc : nullptr, E, out);
+    have = true;
+  }
+  if (!have) { acc.re = "0.0"; acc.im = ""; }
+  return acc;
+}
+
 // ---- split plan: partition of the groups and the Horner plan of one part -----------------------
 // FP64 instructions of the FT sums reachable from S-node `root` that are not in `seen` yet
 long long mark_reachable(const HornerPlan& hp, int root, std::vector<char>& seen) {
@@ -649,6 +741,180 @@ void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls
 #undef o
 }
 
+// The four sections of the body for complex energies e<i>r + i e<i>i (register plan only).
+void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, Emitter& E, Sections& S) {
+  int cur = 0;
+#define o S.sec[cur]
+  std::vector<std::vector<int>> combos;
+  auto combo_ref = [&](const std::vector<int>& c, std::string* sign) -> int {
+    std::vector<int> pos = c;
+    int sg = 0;
+    for (int v : c)
+      if (v) { sg = v > 0 ? 1 : -1; break; }
+    *sign = sg < 0 ? "-" : "";
+    if (!sg) return -1;
+    if (sg < 0)
+      for (int& v : pos) v = -v;
+    size_t j = 0;
+    for (; j < combos.size(); ++j)
+      if (combos[j] == pos) break;
+    if (j == combos.size()) combos.push_back(pos);
+    return (int)j;
+  };
+  for (const LeafD& l : ft.leafD) { std::string sg; combo_ref(l.c, &sg); }
+  for (size_t j = 0; j < combos.size(); ++j)
+    o << "  const double E" << j << "r = " << combo(combos[j], "e", "r") << ", E" << j << "i = " << combo(combos[j], "e", "i") << ";\n";
+  auto emit_d_leaves = [&](bool freq_independent, const std::string& ind) {
+    for (size_t u = 0; u < ft.leafD.size(); ++u) {
+      if ((hp.d_is_real[u] != 0) != freq_independent) continue;
+      const LeafD& l = ft.leafD[u];
+      std::string sg;
+      const int j = combo_ref(l.c, &sg);
+      const std::string er = j < 0 ? "0.0" : sg + "E" + std::to_string(j) + "r", ei = j < 0 ? "0.0" : sg + "E" + std::to_string(j) + "i";
+      o << ind << "double Dr" << u << ", Di" << u << ";\n" << ind << "{\n";
+      if (freq_independent) {
+        o << ind << "  const double re = " << er << " + p.e_reg, im = " << ei << ";\n";      // P10(b): always regulated
+      } else {
+        std::string cond;
+        for (int x = 0; x < ft.n_ext; ++x)
+          if (l.a[x]) cond += (cond.empty() ? "" : " && ") + std::string("zz") + std::to_string(x);
+        o << ind << "  const double re = ((" << combo(l.a, "zr") << ") + " << er << ") + ((" << cond << ") ? p.e_reg : 0.0), im = ("
+          << combo(l.a, "zi") << ") + " << ei << ";\n";
+      }
+      o << ind << "  const double r = fast_rcp(fma(re, re, im * im));\n" << ind << "  Dr" << u << " = re * r; Di" << u << " = -im * r;\n"
+        << ind << "}\n";
+    }
+  };
+  emit_d_leaves(true, "  ");
+  cur = 1;
+  // one exponential per energy symbol: e^{beta e_i} = 2^{n_i} (m_i r + i m_i i), |m_i| in [0.70, 1.42]
+  std::vector<char> sym_used(ft.n_eps, 0);
+  for (const LeafF& l : ft.leafF)
+    for (int i = 0; i < ft.n_eps; ++i)
+      if (l.c[i]) sym_used[i] = 1;
+  for (int i = 0; i < ft.n_eps; ++i) {
+    if (!sym_used[i]) continue;
+    o << "    int n" << i << "; double m" << i << "r, m" << i << "i;\n    {\n      const double x[1] = {beta * e" << i
+      << "r};\n      int nn[1]; double mm[1];\n      exp_split_n<1>(x, nn, mm);\n      double sn, cs;\n      sincos(beta * e" << i
+      << "i, &sn, &cs);\n      n" << i << " = nn[0]; m" << i << "r = mm[0] * cs; m" << i << "i = mm[0] * sn;\n    }\n";
+  }
+  // leaves: f_sigma = B / (sigma 2^N A + B) with A, B complex mantissa products (P12); derivatives by Q_k (P11)
+  std::vector<std::vector<size_t>> base;
+  for (size_t u = 0; u < ft.leafF.size(); ++u) {
+    size_t b = 0;
+    for (; b < base.size(); ++b)
+      if (ft.leafF[base[b][0]].c == ft.leafF[u].c && ft.leafF[base[b][0]].sigma == ft.leafF[u].sigma) break;
+    if (b == base.size()) base.emplace_back();
+    base[b].push_back(u);
+  }
+  for (size_t u = 0; u < ft.leafF.size(); ++u) o << "    double Fr" << u << ", Fi" << u << ";\n";
+  for (const auto& members : base) {
+    const LeafF& l = ft.leafF[members[0]];
+    o << "    {\n";
+    Stmts st;
+    std::string ex;
+    auto product = [&](int sign) -> CV {
+      CV acc;
+      bool have = false;
+      for (int i = 0; i < ft.n_eps; ++i)
+        for (int r = 0; r < l.c[i] * sign; ++r) {
+          const CV m{"m" + std::to_string(i) + "r", "m" + std::to_string(i) + "i"};
+          ex += std::string(sign > 0 ? " + n" : " - n") + std::to_string(i);
+          if (!have) { acc = m; have = true; }
+          else acc = emit_cv_fma(acc, m, nullptr, E, st);
+        }
+      if (!have) acc = CV{"1.0", ""};
+      return acc;
+    };
+    CV A = product(+1);
+    const CV B = product(-1);
+    if (l.sigma < 0) A = emit_cv_fma(CV{"p.ceta[b]", ""}, A, nullptr, E, st);      // e^{beta eta} (P10(a))
+    for (const std::string& s : st) o << "      " << s << "\n";
+    const std::string sg = l.sigma > 0 ? "" : "-";
+    o << "      const double sc = pow2_clamped(0" << ex << ");\n";
+    o << "      const double dr = fma(sc, " << sg << A.re << ", " << B.re << "), di = "
+      << (A.real() ? std::string("0.0") : "sc * " + sg + A.im) << (B.real() ? "" : " + " + B.im) << ";\n";
+    o << "      const double rn = fast_rcp(fma(dr, dr, di * di));\n";
+    // f = B conj(d) / |d|^2,  g = sigma sc A conj(d) / |d|^2
+    if (B.real()) o << "      const double fr = dr * rn, fi = -di * rn;\n";
+    else o << "      const double fr = fma(" << B.re << ", dr, " << B.im << " * di) * rn, fi = fma(" << B.im << ", dr, -" << B.re << " * di) * rn;\n";
+    bool need_g = false;
+    for (size_t u : members) need_g |= ft.leafF[u].k > 0;
+    if (need_g) {
+      const std::string ai = A.real() ? "0.0" : A.im;
+      o << "      const double gr = " << sg << "sc * fma(" << A.re << ", dr, " << ai << " * di) * rn, gi = " << sg << "sc * fma(" << ai
+        << ", dr, -" << A.re << " * di) * rn;\n";
+    }
+    for (size_t u : members) {
+      const int k = ft.leafF[u].k;
+      if (k == 0) { o << "      Fr" << u << " = fr; Fi" << u << " = fi;\n"; continue; }
+      const std::vector<double> q = deriv_poly(k);
+      o << "      {\n        double qr = " << dlit(q.back()) << ", qi = 0.0;\n";
+      for (int i = (int)q.size() - 2; i >= 0; --i)
+        o << "        { const double t = fma(qr, fr, -qi * fi) + " << dlit(q[i]) << "; qi = fma(qr, fi, qi * fr); qr = t; }\n";
+      o << "        double bk = beta;\n";
+      for (int i = 1; i < k; ++i) o << "        bk *= beta;\n";
+      o << "        const double hr = fma(fr, gr, -fi * gi), hi = fma(fr, gi, fi * gr);\n"
+           "        Fr" << u << " = bk * fma(hr, qr, -hi * qi); Fi" << u << " = bk * fma(hr, qi, hi * qr);\n      }\n";
+    }
+    o << "    }\n";
+  }
+  // FT sums, level by level
+  {
+    std::vector<int> order(hp.snodes.size());
+    for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return hp.snodes[a].height < hp.snodes[b].height; });
+    for (size_t i = 0; i < order.size();) {
+      size_t j = i;
+      std::vector<Stmts> lists;
+      while (j < order.size() && hp.snodes[order[j]].height == hp.snodes[order[i]].height) {
+        lists.emplace_back();
+        emit_snode_cplx(hp, order[j], E, lists.back());
+        ++j;
+      }
+      interleave(lists, kWays, o, "    ");
+      i = j;
+    }
+    for (size_t g = 0; g < hp.groups.size(); ++g) {
+      const HGroup& hg = hp.groups[g];
+      if (hg.root >= 0) o << "    const double FTr" << g << " = Sr" << hg.root << ", FTi" << g << " = Si" << hg.root << ";\n";
+      else o << "    const double FTr" << g << " = " << dlit((double)hg.num / (double)hg.den) << ", FTi" << g << " = 0.0;\n";
+    }
+  }
+  std::vector<CV> q(hp.dn.size());
+  std::vector<char> q_have(hp.dn.size(), 0);
+  {
+    std::vector<Stmts> lists;
+    for (size_t n = 0; n < hp.dn.size(); ++n) {
+      if (n != 0 && hp.d_is_real[hp.dn[n].leaf]) continue;
+      lists.emplace_back();
+      bool have = false;
+      q[n] = emit_q_cplx(hp, (int)n, E, lists.back(), &have);
+      q_have[n] = have;
+      if (have && q[n].im.empty()) q[n].im = "0.0";
+      if (have)
+        for (const std::string& nm : {q[n].re, q[n].im})
+          if (nm != "0.0" && std::find(S.keep.begin(), S.keep.end(), nm) == S.keep.end()) S.keep.push_back(nm);
+    }
+    interleave(lists, kWays, o, "    ");
+  }
+  cur = 2;
+  for (int x = 0; x < ft.n_ext; ++x) {
+    o << "      const double zr" << x << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ")], zi" << x
+      << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ") + 1];\n";
+    o << "      const bool zz" << x << " = (zr" << x << " == 0.0 && zi" << x << " == 0.0);\n";
+  }
+  emit_d_leaves(false, "      ");
+  cur = 3;
+  {
+    Stmts st;
+    const CV acc = emit_d_sum_cplx(hp, q, q_have, 0, E, st);
+    for (const std::string& s : st) o << "      " << s << "\n";
+    o << "      AMI_EMIT(" << acc.re << ", " << (acc.real() ? std::string("0.0") : acc.im) << ");\n";
+  }
+#undef o
+}
+
 // Momenta of sample `at` into nk0..: from memory, or drawn in place by the counter-based generator (S4 with a
 // seed: the momenta never exist in memory).  Counter of component c = sample * n_comp + c; the generator's
 // state is seed + GOLDEN (counter + 1), so one 64-bit multiply per sample and an addition per component
@@ -765,8 +1031,13 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
   o << head.str();
   std::string esig, eargs;
   for (int i = 0; i < ft.n_eps; ++i) {
-    esig += ", const double e" + std::to_string(i);
-    eargs += ", e" + std::to_string(i);
+    if (var.cplx) {
+      esig += ", const double e" + std::to_string(i) + "r, const double e" + std::to_string(i) + "i";
+      eargs += ", e" + std::to_string(i) + "r, e" + std::to_string(i) + "i";
+    } else {
+      esig += ", const double e" + std::to_string(i);
+      eargs += ", e" + std::to_string(i);
+    }
   }
   // A fused kernel: a CTA walks `tiles` consecutive tiles of AMI_NT samples -- one, known at compile time, in
   // ami_jit_fused (the loop disappears); p.tiles in the tally kernel, where a thread adds up its own samples.
@@ -793,7 +1064,8 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
   };
   if (mode == kJitRegister) {
     Sections S;
-    gen_sections(ft, hp, ls, kLeafInline, E, S);
+    if (var.cplx) gen_sections_cplx(ft, hp, E, S);
+    else gen_sections(ft, hp, ls, kLeafInline, E, S);
     o << kTallySrc;
     // what a finished row does with its value: store it, and/or add it to the tally
     o << "#define AMI_EMIT(VR, VI) { \\\n"
@@ -837,8 +1109,15 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
          "  double4 t4 = make_double4(0.0, 0.0, 0.0, 0.0);\n"
          "#pragma unroll 1\n"
          "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n";
-    for (int i = 0; i < ft.n_eps; ++i) o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
+    for (int i = 0; i < ft.n_eps; ++i) {
+      if (var.cplx)
+        o << "  const double e" << i << "r = p.e[2 * (" << i << " * p.e_stride + s)], e" << i << "i = p.e[2 * (" << i
+          << " * p.e_stride + s) + 1];\n";
+      else
+        o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
+    }
     o << subst(call, "<false>") << "  }\n}\n\n";
+    if (var.cplx) return std::vector<std::string>(1, o.str());   // momenta give real energies: no fused kernels
     // ---- kernels 2, 3: momenta from memory or drawn in place, dispersion inline; without / with the tally ----
     for (int tally = 0; tally < 2; ++tally) {
       fused_open(tally ? "ami_jit_fused_tally" : "ami_jit_fused", tally ? "p.tiles" : "1");
@@ -1190,8 +1469,9 @@ int jit_prepare(ami_table* tab, const JitVariant& var, std::string& err) {
   if (tab->dev.device < 0) return fail(AMI_ECUDA, "table has no device copy");
   if (var.dim < 1 || var.dim > 3 || (var.band != AMI_BAND_TIGHT_BINDING && var.band != AMI_BAND_FREE))
     return fail(AMI_EINVAL, "bad lattice for the specialised kernels");
-  if (var.cplx) return fail(AMI_EUNSUPPORTED, "complex energies run the table-driven kernels");
   if (!jit_eligible(tab->flat, tab->horner)) return fail(AMI_EUNSUPPORTED, "table outside the limits of the specialised kernels");
+  if (var.cplx && jit_mode(tab->flat, tab->horner) != kJitRegister)
+    return fail(AMI_EUNSUPPORTED, "complex energies: only tables of register-plan size are specialised");
   const auto t0 = std::chrono::steady_clock::now();
   const std::vector<std::string> srcs = jit_generate_sources(tab->flat, tab->horner, var, &m.layout);
   // the modules of a split plan are compiled side by side (NVRTC is thread safe across programs)
@@ -1233,8 +1513,10 @@ int jit_prepare(ami_table* tab, const JitVariant& var, std::string& err) {
   };
   if (m.layout.mode == kJitRegister) {
     get(&m.fn_eval, 0, "ami_jit_eval");
-    get(&m.fn_fused, 0, "ami_jit_fused");
-    get(&m.fn_fused_tally, 0, "ami_jit_fused_tally");
+    if (!var.cplx) {
+      get(&m.fn_fused, 0, "ami_jit_fused");
+      get(&m.fn_fused_tally, 0, "ami_jit_fused_tally");
+    }
   } else {
     get(&m.fn_leaves_eval, 0, "ami_split_leaves_eval");
     get(&m.fn_leaves_fused, 0, "ami_split_leaves_fused");

@@ -77,6 +77,30 @@ def test_order8_is_a_split_plan(ami):
         tab.specialize()
 
 
+@pytest.mark.parametrize("kw", [{"complex_energies": True}, {"dim": 1}, {"dim": 3, "band": 1}])
+def test_kernel_variants_compile(ami, kw):
+    """The kernels are generated per variant -- complex energies, momenta of 1-3 components and either
+    band (Eq. 14) -- and each compiles for sm_100a."""
+    tab = ami.AmiTable.from_diagram(A.get_config("cfg3").diagram, device=None)
+    src = tab.kernel_source(**kw)
+    assert src != tab.kernel_source()
+    if kw.get("complex_energies"):
+        assert "sincos(" in src and "ami_jit_fused" not in src and "Fr0" in src      # momenta give real energies
+    else:
+        assert ("kz0" in src) == (kw["dim"] == 3) and ("cos_bounded_n" in src.split("ami_jit_fused")[-1]) == (kw.get("band", 0) == 0)
+    try:
+        cubin, log = tab.kernel_cubin(**kw)
+    except ami.AmiError as e:
+        if e.code == -6:
+            pytest.skip("NVRTC library not available on this machine")
+        raise
+    assert cubin[:4] == b"\x7fELF" and "ami_jit_eval" in log
+    big = ami.AmiTable.from_diagram(A.get_config("stress8").diagram, device=None)
+    if kw.get("complex_energies"):
+        with pytest.raises(ami.AmiError):          # complex energies: tables of register-plan size only
+            big.kernel_source(**kw)
+
+
 def test_register_plan_can_be_switched_off():
     """AMI_DISABLE_JIT=1: every table reports the register plan as unavailable, so AMI_PLAN_AUTO runs
     the table-driven kernels (checked in a fresh process: the switch is read per call)."""

@@ -166,21 +166,33 @@ def test_cfg5_grid(ami, torch_mod, oracle_mod, plan):
     run_eval_case(ami, torch_mod, oracle_mod, A.get_config("cfg5"), 600 + 3, PLANS[plan], n_truth=150)
 
 
-@pytest.mark.parametrize("plan", list(PLANS))
-def test_complex_energies_variant_5b(ami, torch_mod, oracle_mod, plan):
-    """P19: complex energies e_j - i gamma_j make the Fermi/Bose arguments complex."""
-    if plan == "tree":
-        pytest.skip("the tree plan takes real energies (complex ones run the flat plan)")
-    cfg = A.get_config("cfg5")
+@pytest.mark.parametrize("name", ["cfg5", "cfg3", "cfg2_bubble_doubled"])
+@pytest.mark.parametrize("plan", ["flat", "reg", "auto"])
+def test_complex_energies_variant_5b(ami, torch_mod, oracle_mod, name, plan):
+    """P19: complex energies e_j - i gamma_j (energy_t is complex128) make the Fermi/Bose arguments
+    complex.  The specialised kernels have a complex-energy variant (per-symbol exponential 2^n m (cos + i sin),
+    exponents still added as integers): AMI_PLAN_REG, which never falls back, must succeed and agree with the quad
+    oracle, as must the table-driven flat kernel; cfg3 and the doubled bubble carry derivative leaves."""
+    cfg = A.get_config(name)
     tab = ami.AmiTable.from_diagram(cfg.diagram)
-    n = 500
+    n = 500 + 3
     e_real = gpu_energies(torch_mod, tab, cfg, cfg.momenta(n)).cpu().numpy()
     gam = A.uniform01(99, np.arange(e_real.size, dtype=np.uint64)).reshape(e_real.shape) * 0.05
     e_c = e_real - 1j * gam
     z = cfg.z_ext[::8]
-    out = tab.evaluate(torch_mod.from_numpy(e_c).cuda(), z, [5.0], plan=PLANS[plan]).cpu().numpy()
-    truth, S = truth_for(oracle_mod, cfg, e_c.T.copy(), z, 5.0, 0.0)
-    check_parity(out[0], truth, S, label="5b")
+    betas = [5.0, 11.0] if name != "cfg2_bubble_doubled" else [4.0]
+    pid = {"flat": ami.PLAN_FLAT, "reg": ami.PLAN_REG, "auto": ami.PLAN_AUTO}[plan]
+    out = tab.evaluate(torch_mod.from_numpy(e_c).cuda(), z, betas, e_reg=cfg.e_reg, plan=pid).cpu().numpy()
+    for b, beta in enumerate(betas):
+        truth, S = truth_for(oracle_mod, cfg, e_c.T.copy(), z, beta, cfg.e_reg)
+        check_parity(out[b], truth, S, label=f"5b {name} {plan} beta={beta}")
+    if plan == "reg":      # real energies given as complex numbers: the same values as the real-energy kernels
+        e0 = torch_mod.from_numpy(e_real.astype(np.complex128)).cuda()
+        a = tab.evaluate(e0, z, betas, e_reg=cfg.e_reg, plan=pid)
+        r = tab.evaluate(torch_mod.from_numpy(e_real).cuda(), z, betas, e_reg=cfg.e_reg, plan=pid)
+        truth, S = truth_for(oracle_mod, cfg, e_real.T.copy(), z, betas[0], cfg.e_reg)
+        check_parity(a.cpu().numpy()[0], truth, S, label="5b zero imaginary part")
+        assert np.max(np.abs((a - r).cpu().numpy()[0]) / S) <= 1e-13
 
 
 @pytest.mark.parametrize("plan", list(PLANS))
@@ -242,18 +254,17 @@ def test_register_plan_is_what_auto_runs(ami, torch_mod, name):
 
 
 def test_register_plan_limits(ami, torch_mod):
-    """Complex energies run the table-driven kernels under AUTO and are refused under an explicit AMI_PLAN_REG;
-    tables beyond one register-resident kernel (order 8) are specialised as a split plan."""
+    """Tables beyond one register-resident kernel (order 8) are specialised as a split plan; with complex energies
+    they run the table-driven kernels under AUTO and are refused under an explicit AMI_PLAN_REG."""
     cfg = A.get_config("stress8")
     tab = ami.AmiTable.from_diagram(cfg.diagram)
     assert tab.info["reg_plan_status"] == 1 and tab.info["plan_kind"] == 2
     assert ami.AmiTable.from_diagram(A.get_config("cfg4").diagram).info["plan_kind"] == 1
-    cfg = A.get_config("cfg3")
-    tab = ami.AmiTable.from_diagram(cfg.diagram)
     ec = gpu_energies(torch_mod, tab, cfg, cfg.momenta(40)).to(torch_mod.complex128)
-    with pytest.raises(ami.AmiError):
+    with pytest.raises(ami.AmiError) as ei:      # complex energies: only tables of register-plan size are specialised
         tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=ami.PLAN_REG)
-    tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=ami.PLAN_AUTO)
+    assert ei.value.code == -6
+    tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=ami.PLAN_AUTO)      # the table-driven kernel takes them
 
 
 @pytest.mark.parametrize("name,n", [("cfg1", 10_000), ("cfg3", 50_000 + 3), ("cfg4", 3000 + 1), ("cfg5", 401)])
@@ -331,9 +342,10 @@ def test_extreme_temperatures(ami, torch_mod, oracle_mod, name, plan):
 
 def split_case(name):
     """Tables beyond one register-resident kernel: the order-8 stress table (T = 40244) and an order-7 one (T = 8598)."""
+    cfg = A.get_config("stress8")
     if name == "o7":
-        return A.get_config("stress8", diagram=A.random_self_energy(7, 0), name="o7")
-    return A.get_config(name)
+        cfg.diagram, cfg.name = A.random_self_energy(7, 0), "o7"
+    return cfg
 
 
 @pytest.mark.parametrize("name", ["o7", "stress8"])
@@ -379,7 +391,7 @@ def test_split_plan_large_tables(ami, torch_mod, oracle_mod, name):
     assert torch_mod.equal(ob[:, :, big - 500:], tail)
     stats, sums = tab.run(5000 + 3, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, want_sum=True)
     ref = ob[:, :, :5003].sum(dim=2).cpu().numpy()
-    assert np.max(np.abs(sums - ref)) <= 1e-12 * np.abs(ob[:, :, :5003]).sum().item()
+    assert np.max(np.abs(sums - ref)) <= 1e-12 * ob[:, :, :5003].abs().sum().item()
 
 
 def test_kernel_cache_on_disk(ami, torch_mod, tmp_path):
@@ -608,7 +620,7 @@ def test_run_workspace_across_plans_and_refusals(ami, torch_mod):
         tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed)       # nowhere to put anything
     assert ei.value.code == -1
     with pytest.raises(ami.AmiError):
-        tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, d_out=a, dim=4)
+        tab.run(n, [[0.1, 0.2, 0.3, 0.4]], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, d_out=a, dim=4)
 
 
 def test_run_device_output_and_determinism(ami, torch_mod):
