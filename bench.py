@@ -137,18 +137,30 @@ def fp64_work_per_sample(info, n_f, n_b, reg, tree=False):
             "terms": terms}
 
 
-def ncu_traffic(workload, fused):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture
-    (profiles/r01_dram_traffic.csv; commands in profiles/r01_register_plan.md), or None."""
-    p = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+def ncu_capture(workload, fused):
+    """Counters of the dominant kernel from the committed ncu capture of this workload at its configured size
+    (profiles/r02_ncu_<workload>.csv; commands in profiles/r02_ncu_summary.md): DRAM bytes per launch and the warp
+    instructions executed per sample, or None."""
+    import csv
+    p = os.path.join(ROOT, "profiles", f"r02_ncu_{workload}.csv")
     if not fused or not os.path.exists(p):
         return None
     with open(p) as f:
-        for line in f.read().splitlines()[1:]:
-            w, _kernel, rd, wr = line.split(",")
-            if w == workload:
-                return int(rd) + int(wr)
-    return None
+        rows = list(csv.reader(f))
+    hdr, units, first = rows[0], rows[1], rows[2]
+    col = {h: i for i, h in enumerate(hdr)}
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    def nbytes(name):
+        return float(first[col[name]].replace(",", "")) * scale.get(units[col[name]], 1.0)
+    try:
+        n_threads = float(first[col["launch__grid_size"]]) * float(first[col["launch__block_size"]])
+        return {"kernel": first[col["Kernel Name"]],
+                "dram_bytes": int(nbytes("dram__bytes_read.sum") + nbytes("dram__bytes_write.sum")),
+                "warp_instructions": float(first[col["smsp__inst_executed.sum"]]),
+                "threads": n_threads,
+                "fp64_pipe_active_pct": float(first[col["sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active"]])}
+    except (KeyError, ValueError):
+        return None
 
 
 def load_measured_peaks():
@@ -401,9 +413,48 @@ def time_e2e(pkg, torch, tab, cfg, n, steps, warmup, plan, first_sample, dist):
                            h_out=h_out)
     torch.cuda.synchronize()
     dt = sharding.max_over_ranks(time.perf_counter() - t0, dist)
-    return {"seconds": dt, "h2d": int(stats["h2d_bytes"]), "d2h": int(stats["d2h_bytes"]),
+    # the floor of this step on this box: the same pinned momenta copied alone, same clock
+    d_k = torch.empty_like(h_k, device="cuda")
+    d_k.copy_(h_k, non_blocking=True)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    for _ in range(steps):
+        d_k.copy_(h_k, non_blocking=True)
+    torch.cuda.synchronize()
+    floor_s = (time.perf_counter() - t1) / steps
+    return {"seconds": dt, "h2d_copy_alone_ms": floor_s * 1e3, "h2d": int(stats["h2d_bytes"]), "d2h": int(stats["d2h_bytes"]),
             "chunks": int(stats["n_chunks"]), "launches_per_step": int(stats["kernel_launches"]),
             "finite": bool(torch.isfinite(torch.view_as_real(h_out[0, 0, :1024])).all().item())}
+
+
+def time_complex_energies(pkg, torch, cfg, peaks, dfma_per_s, steps=10):
+    """Variant 5b of reading P19 (energy_t is complex128): cfg5's table and grid fed with complex
+    energies e - i gamma, gamma in [0, 0.05).  Energies are supplied, so a step is ami_evaluate alone (S2+S3) on the
+    complex-energy variant of the specialised kernels; the same call with the table-driven flat kernel beside it."""
+    import ami_inputs as A
+    n, n_f, n_b = cfg.n_samples, len(cfg.z_ext), len(cfg.betas)
+    tab = pkg.AmiTable.from_diagram(cfg.diagram, device=torch.cuda.current_device())
+    k = tab.generate_momenta(cfg.seed, 0, n)
+    e = tab.dispersion(k, [cfg.q], cfg.t, cfg.mu)
+    gam = torch.from_numpy(A.uniform01(99, np.arange(e.numel(), dtype=np.uint64)).reshape(tuple(e.shape)) * 0.05).cuda()
+    ec = torch.complex(e, -gam)
+    out = torch.empty((n_b, n_f, n), dtype=torch.complex128, device="cuda")
+    res = {}
+    for label, plan, reps in (("register", 2, steps), ("flat", 1, 2)):
+        tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=plan, out=out)
+        torch.cuda.synchronize()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record()
+        for _ in range(reps):
+            tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=plan, out=out)
+        t1.record()
+        torch.cuda.synchronize()
+        res[label] = t0.elapsed_time(t1) / reps
+    T = int(tab.info["n_terms"])
+    return {"T_flat": T, "samples": n, "n_freq": n_f, "n_beta": n_b, "plan": "register, complex-energy variant (ami_evaluate)",
+            "ms_per_step": res["register"], "term_evals_per_s": T * n * n_f * n_b / (res["register"] * 1e-3),
+            "samples_per_s": n * n_f * n_b / (res["register"] * 1e-3), "flat_plan_ms_per_step": res["flat"],
+            "hbm_frac": (ec.numel() * 16 + out.numel() * 16) / (res["register"] * 1e-3) / 1e9 / peaks["hbm_gbs"]}
 
 
 def time_e2e_seeded(torch, tab, cfg, n, steps, plan, T):
@@ -530,8 +581,13 @@ def run_ours(args, dist, rank, local, world):
     ms_per_step = res["total_ms"] / args.steps
     value = T * units_per_step / (ms_per_step * 1e-3)
     roof, disp = roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s, dfma3_per_s)
-    if n == cfg.n_samples:
-        roof["traffic"] = ncu_traffic(cfg.name, res["fused"])     # per launch, from profiles/ (ncu --set full)
+    cap = ncu_capture(cfg.name, res["fused"]) if n == cfg.n_samples else None
+    if cap:      # per launch, from profiles/ (ncu --set full of the same command, committed)
+        roof["traffic"] = cap["dram_bytes"]
+        roof["ncu"] = {"source": f"profiles/r02_ncu_{cfg.name}.csv", "kernel": cap["kernel"],
+                       "warp_instructions_per_sample": 32.0 * cap["warp_instructions"] / n,
+                       "fp64_pipe_active_pct_of_active_cycles": cap["fp64_pipe_active_pct"],
+                       "fp64_slots_counted_per_sample": roof["fp64_slots_counted"]}
     e2e = time_e2e(pkg, torch, res["tab"], cfg, n, max(2, args.steps // 4), 1, plan, first, dist)
     e2e_steps = max(2, args.steps // 4)
     e2e_value = T * units_per_step * e2e_steps / e2e["seconds"]
@@ -559,7 +615,10 @@ def run_ours(args, dist, rank, local, world):
                     "two_stream_ms_per_step": res["two_stream_ms"]},
         "roofline": roof,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
-                "steps": e2e_steps, "chunks_per_step": e2e["chunks"], "api": "ami_run(h_k -> h_out)"},
+                "steps": e2e_steps, "chunks_per_step": e2e["chunks"], "api": "ami_run(h_k -> h_out)",
+                "ms_per_step": 1e3 * e2e["seconds"] / e2e_steps, "h2d_copy_alone_ms": e2e["h2d_copy_alone_ms"],
+                "note": "H2D copy | kernels | D2H copy of consecutive chunks overlap on three streams; the input copy "
+                        "alone (h2d_copy_alone_ms, same pinned buffer, same clock) is the floor of the step on this box"},
         "gpu_launches": launches,
         "clocks": res["clocks"],
         "fp64_probe_dfma_per_s": dfma_per_s, "fp64_probe_three_source_dfma_per_s": dfma3_per_s,
@@ -598,6 +657,7 @@ def run_ours(args, dist, rank, local, world):
                 others[name]["bound"] = "L2 bandwidth (leaf array reads), see DESIGN.md 6.5"
             del r2
             torch.cuda.empty_cache()
+        others["cfg5b"] = time_complex_energies(pkg, torch, A.get_config("cfg5"), peaks, dfma_per_s)
         line["other_workloads"] = others
         line["monte_carlo"] = time_monte_carlo(torch, res["tab"], cfg, 10 * n, 5, plan)
         w_mc = fp64_work_per_sample(info, n_f, n_b, res["fused"])

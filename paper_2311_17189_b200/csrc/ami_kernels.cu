@@ -629,10 +629,9 @@ cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long 
 //   SRC = 2: x = fma(x, x, b) -- two distinct 64-bit register sources.  Reaches 0.995 of 148 SMs x 64 lanes x
 //            clock on B200: the pipe's issue rate, the roofline's peak.
 //   SRC = 3: x = fma(x, a, b) -- three distinct register sources, the shape of almost every DFMA of real code.
-//            Stops at 0.92 of the same figure even though a and b are shared by all chains (and 0.80 when the
-//            chains alternate between two a's and two b's, profiles/r02_dfma_probe.md): a DFMA that reads three
-//            different register pairs does not issue every second cycle.  Reported beside the peak as the
-//            ceiling of register-operand arithmetic.
+//            Stops at 0.92 of the same figure although a and b are shared by all chains: a DFMA that reads
+//            three different register pairs does not issue every second cycle.  Reported beside the peak as
+//            the ceiling of register-operand arithmetic (bench.py: fp64_probe_three_source_dfma_per_s).
 // ------------------------------------------------------------------------------------------
 template <int SRC>
 __global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters, double a, double b) {
