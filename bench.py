@@ -422,7 +422,19 @@ def time_e2e(pkg, torch, tab, cfg, n, steps, warmup, plan, first_sample, dist):
         d_k.copy_(h_k, non_blocking=True)
     torch.cuda.synchronize()
     floor_s = (time.perf_counter() - t1) / steps
-    return {"seconds": dt, "h2d_copy_alone_ms": floor_s * 1e3, "h2d": int(stats["h2d_bytes"]), "d2h": int(stats["d2h_bytes"]),
+    # ... and both directions at once (what the step must move): the input in, a result-sized buffer out, two streams
+    d_o = torch.empty(h_out.shape, dtype=torch.complex128, device="cuda")
+    s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    t2 = time.perf_counter()
+    for _ in range(steps):
+        with torch.cuda.stream(s_in):
+            d_k.copy_(h_k, non_blocking=True)
+        with torch.cuda.stream(s_out):
+            h_out.copy_(d_o, non_blocking=True)
+        torch.cuda.synchronize()
+    both_s = (time.perf_counter() - t2) / steps
+    return {"seconds": dt, "h2d_copy_alone_ms": floor_s * 1e3, "both_copies_alone_ms": both_s * 1e3, "h2d": int(stats["h2d_bytes"]), "d2h": int(stats["d2h_bytes"]),
             "chunks": int(stats["n_chunks"]), "launches_per_step": int(stats["kernel_launches"]),
             "finite": bool(torch.isfinite(torch.view_as_real(h_out[0, 0, :1024])).all().item())}
 
@@ -491,6 +503,7 @@ def time_monte_carlo(torch, tab, cfg, n, steps, plan):
     mean = sums / n
     err = np.sqrt(np.maximum(tab.last_sumsq[..., 0] / n - mean.real ** 2, 0.0) / n)
     return {"samples_per_step": n, "ms_per_step": dt * 1e3, "samples_per_s": n * n_f * n_b / dt,
+            "gpu_ms_per_step": float(stats["gpu_ms"]),
             "chunks_per_step": int(stats["n_chunks"]), "launches_per_step": int(stats["kernel_launches"]),
             "d2h_bytes_per_step": int(stats["d2h_bytes"]), "timed": "host clock around ami_run (synchronous)",
             "mean_re_first_row": float(mean[0, 0].real), "stderr_re_first_row": float(err[0, 0])}
@@ -617,8 +630,10 @@ def run_ours(args, dist, rank, local, world):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                 "steps": e2e_steps, "chunks_per_step": e2e["chunks"], "api": "ami_run(h_k -> h_out)",
                 "ms_per_step": 1e3 * e2e["seconds"] / e2e_steps, "h2d_copy_alone_ms": e2e["h2d_copy_alone_ms"],
+                "both_copies_alone_ms": e2e["both_copies_alone_ms"],
                 "note": "H2D copy | kernels | D2H copy of consecutive chunks overlap on three streams; the input copy "
-                        "alone (h2d_copy_alone_ms, same pinned buffer, same clock) is the floor of the step on this box"},
+                        "alone (h2d_copy_alone_ms, same pinned buffer, same clock) and both copies of the step issued at once "
+                        "without any kernel (both_copies_alone_ms) are the floors of the step on this box"},
         "gpu_launches": launches,
         "clocks": res["clocks"],
         "fp64_probe_dfma_per_s": dfma_per_s, "fp64_probe_three_source_dfma_per_s": dfma3_per_s,
@@ -663,6 +678,9 @@ def run_ours(args, dist, rank, local, world):
         w_mc = fp64_work_per_sample(info, n_f, n_b, res["fused"])
         line["monte_carlo"]["alu_frac"] = (w_mc["evaluate"] + w_mc["dispersion"]) * line["monte_carlo"]["samples_per_s"] \
             / dfma_per_s
+        # the same against the CUDA-event time of the call's device work (without the host's launch and sync costs)
+        line["monte_carlo"]["alu_frac_device_time"] = (w_mc["evaluate"] + w_mc["dispersion"]) * 10 * n * n_f * n_b \
+            / (line["monte_carlo"]["gpu_ms_per_step"] * 1e-3) / dfma_per_s
         line["e2e_seeded"] = time_e2e_seeded(torch, res["tab"], cfg, n, max(2, args.steps // 4), plan, T)
         import oracle
         threads = oracle.hardware_threads()

@@ -724,6 +724,8 @@ struct RunBuffers {
   double* wp = nullptr;                   // per-warp partial sums of the fused tally
   double* partial = nullptr;
   double* sum = nullptr;
+  double* h_tally = nullptr;              // pinned host copy of `sum` (a pageable destination would stage the copy)
+  size_t cap_h_tally = 0;
   size_t cap_k = 0, cap_out = 0, cap_e = 0, cap_wp = 0, cap_partial = 0, cap_sum = 0;
   int init() {
     if (ev_start) return AMI_OK;
@@ -758,6 +760,13 @@ struct RunBuffers {
     if ((rc = grow(&e, &cap_e, be)) || (rc = grow(&wp, &cap_wp, bw)) ||
         (rc = grow(&partial, &cap_partial, bs * ami::kMaxSumBlocks)) || (rc = grow(&sum, &cap_sum, bs)))
       return rc;
+    if (bs > cap_h_tally) {
+      if (h_tally) cudaFreeHost(h_tally);
+      h_tally = nullptr;
+      cap_h_tally = 0;
+      CU(cudaHostAlloc((void**)&h_tally, bs, cudaHostAllocDefault));
+      cap_h_tally = bs;
+    }
     return AMI_OK;
   }
   ~RunBuffers() {
@@ -771,6 +780,7 @@ struct RunBuffers {
     if (ev_start) cudaEventDestroy(ev_start);
     if (ev_stop) cudaEventDestroy(ev_stop);
     cudaFree(e); cudaFree(wp); cudaFree(partial); cudaFree(sum);
+    if (h_tally) cudaFreeHost(h_tally);
   }
 };
 
@@ -847,7 +857,6 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
                        own_out ? (size_t)chunk * rows * 16 : 0, cfg->want_sum ? (size_t)rows * 32 : 0,
                        fused_tally ? (size_t)rows * wp_stride * 32 : 0)))
     return rc;
-  if (cfg->want_sum) CU(cudaMemsetAsync(rb.sum, 0, (size_t)rows * 32, user));
   const bool pipelined = host_io && cfg->n > chunk;
   cudaStream_t s_in = pipelined ? rb.s_in : user, s_k = pipelined ? rb.s_k : user, s_out = pipelined ? rb.s_out : user;
   CU(cudaEventRecord(rb.ev_start, user));
@@ -889,15 +898,18 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
       if (erc) return erc;
       if (cfg->want_sum) {   // on the kernel stream, in chunk order: the running sum is deterministic
         if (fused_tally)
-          CU(ami::launch_warp_partial_sums(rb.wp, rows, tally_slots, wp_stride, rb.partial, rb.sum, s_k, &launches));
+          CU(ami::launch_warp_partial_sums(rb.wp, rows, tally_slots, wp_stride, rb.partial, rb.sum, ci == 0, s_k, &launches));
         else
-          CU(ami::launch_block_sums(obuf, rows, nc, ostride, rb.partial, rb.sum, s_k, &launches));
+          CU(ami::launch_block_sums(obuf, rows, nc, ostride, rb.partial, rb.sum, ci == 0, s_k, &launches));
       }
       if (pipelined) CU(cudaEventRecord(rb.ev_k[b], s_k));
       if (cfg->h_out) {
         if (pipelined) CU(cudaStreamWaitEvent(s_out, rb.ev_k[b], 0));
-        CU(cudaMemcpy2DAsync((char*)cfg->h_out + (size_t)c0 * 16, (size_t)cfg->n * 16, obuf, (size_t)ostride * 16,
-                             (size_t)nc * 16, (size_t)rows, cudaMemcpyDeviceToHost, s_out));
+        if (rows == 1)
+          CU(cudaMemcpyAsync((char*)cfg->h_out + (size_t)c0 * 16, obuf, (size_t)nc * 16, cudaMemcpyDeviceToHost, s_out));
+        else
+          CU(cudaMemcpy2DAsync((char*)cfg->h_out + (size_t)c0 * 16, (size_t)cfg->n * 16, obuf, (size_t)ostride * 16,
+                               (size_t)nc * 16, (size_t)rows, cudaMemcpyDeviceToHost, s_out));
         if (pipelined) CU(cudaEventRecord(rb.ev_out[b], s_out));
         local.d2h_bytes += nc * rows * 16;
       }
@@ -912,10 +924,9 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
     }
   }
   if (rc) return rc;
-  std::vector<double> tally;
+  const double* tally = rb.h_tally;
   if (cfg->want_sum) {
-    tally.resize((size_t)rows * 4);
-    CU(cudaMemcpyAsync(tally.data(), rb.sum, (size_t)rows * 32, cudaMemcpyDeviceToHost, user));
+    CU(cudaMemcpyAsync(rb.h_tally, rb.sum, (size_t)rows * 32, cudaMemcpyDeviceToHost, user));
     local.d2h_bytes += rows * 32;
   }
   CU(cudaEventRecord(rb.ev_stop, user));

@@ -540,7 +540,7 @@ __global__ void __launch_bounds__(256) row_partial_kernel(const double2* __restr
 // One CTA per row: thread t adds partials t, t+256, ... in that order, then a shared-memory tree with a fixed
 // shape, and thread 0 folds the result into the running tally.  Fixed order -> deterministic.
 __global__ void __launch_bounds__(256) row_final_kernel(const double4* __restrict__ partial, int n_partial,
-                                                        double4* __restrict__ sum) {
+                                                        double4* __restrict__ sum, int first) {
   __shared__ double4 sh[256];
   const long long r = blockIdx.x;
   double4 acc = make_double4(0.0, 0.0, 0.0, 0.0);
@@ -560,8 +560,8 @@ __global__ void __launch_bounds__(256) row_final_kernel(const double4* __restric
     }
     __syncthreads();
   }
-  if (threadIdx.x == 0) {
-    double4 t = sum[r];
+  if (threadIdx.x == 0) {     // the first chunk of a run starts the tally, the others add to it
+    double4 t = first ? make_double4(0.0, 0.0, 0.0, 0.0) : sum[r];
     t.x += sh[0].x; t.y += sh[0].y; t.z += sh[0].z; t.w += sh[0].w;
     sum[r] = t;
   }
@@ -597,7 +597,7 @@ __global__ void __launch_bounds__(256) row_partial4_kernel(const double4* __rest
 }
 
 cudaError_t launch_warp_partial_sums(const double* d_warp_partials, long long n_rows, long long n_warps,
-                                     long long row_stride, double* d_partial, double* d_sum, cudaStream_t st,
+                                     long long row_stride, double* d_partial, double* d_sum, bool first, cudaStream_t st,
                                      int* launches) {
   if (n_rows == 0) return cudaSuccess;
   const int nblk = sum_blocks(n_rows, n_warps);
@@ -605,21 +605,21 @@ cudaError_t launch_warp_partial_sums(const double* d_warp_partials, long long n_
   row_partial4_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double4*>(d_warp_partials), n_warps, row_stride,
                                             reinterpret_cast<double4*>(d_partial));
   row_final_kernel<<<(unsigned)n_rows, 256, 0, st>>>(reinterpret_cast<const double4*>(d_partial), nblk,
-                                                     reinterpret_cast<double4*>(d_sum));
+                                                     reinterpret_cast<double4*>(d_sum), first ? 1 : 0);
   count_launch(launches, 2);
   return cudaGetLastError();
 }
 
 // d_partial: [n_rows][<= kMaxSumBlocks] double4, d_sum: [n_rows] double4 running tallies
 cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long n, long long row_stride,
-                              double* d_partial, double* d_sum, cudaStream_t st, int* launches) {
+                              double* d_partial, double* d_sum, bool first, cudaStream_t st, int* launches) {
   if (n_rows == 0) return cudaSuccess;
   const int nblk = sum_blocks(n_rows, n);
   dim3 grid((unsigned)nblk, (unsigned)n_rows);
   row_partial_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const double2*>(d_vals), n, row_stride,
                                            reinterpret_cast<double4*>(d_partial));
   row_final_kernel<<<(unsigned)n_rows, 256, 0, st>>>(reinterpret_cast<const double4*>(d_partial), nblk,
-                                                    reinterpret_cast<double4*>(d_sum));
+                                                    reinterpret_cast<double4*>(d_sum), first ? 1 : 0);
   count_launch(launches, 2);
   return cudaGetLastError();
 }

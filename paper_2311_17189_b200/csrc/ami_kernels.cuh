@@ -63,10 +63,10 @@ bool tree_values_fit_smem(const EvalParams& p);
 cudaError_t launch_generate_momenta(uint64_t seed, long long first, long long n, int n_comp, double* d_k,
                                     cudaStream_t st);
 cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long n, long long row_stride,
-                              double* d_partial, double* d_sum, cudaStream_t st, int* launches);
+                              double* d_partial, double* d_sum, bool first, cudaStream_t st, int* launches);
 cudaError_t launch_warp_partial_sums(const double* d_warp_partials, long long n_rows, long long n_warps,
-                                     long long row_stride, double* d_partial, double* d_sum, cudaStream_t st,
-                                     int* launches);
+                                     long long row_stride, double* d_partial, double* d_sum, bool first,
+                                     cudaStream_t st, int* launches);
 cudaError_t run_fp64_probe(int distinct_sources, double* dfma_per_s, double* ms);
 long long total_launches();
 void count_external_launch(int* launches);

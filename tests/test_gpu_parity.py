@@ -423,7 +423,7 @@ print('CACHED', info['specialize_cached'], 'MS', info['specialize_ms'])
         runs.append((int(words[words.index("CACHED") + 1]), float(words[words.index("MS") + 1]), np.load(path)))
     assert [r[0] for r in runs] == [0, 1, 0]
     assert os.listdir(cache)
-    assert runs[1][1] < 100.0 and runs[1][1] < 0.5 * runs[0][1]      # milliseconds instead of an NVRTC compile
+    assert runs[1][1] < 250.0 and runs[1][1] < 0.5 * runs[0][1]      # milliseconds instead of an NVRTC compile
     assert np.array_equal(runs[0][2], runs[1][2]) and np.array_equal(runs[0][2], runs[2][2])
 
 
