@@ -134,3 +134,37 @@ def test_large_momenta_take_the_library_cosine(ami, oracle_mod):
     e2 = torch.zeros((cfg.diagram.n_eps, 256), dtype=torch.float64, device="cuda")
     tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_out=e2)
     assert np.array_equal(e2.cpu().numpy(), e)
+
+
+def test_bench_line_contract():
+    """bench.py as the driver runs it (defaults, fewer steps): ONE JSON line with the contract's keys -- metric and
+    config of BASELINE.json, roofline and cpu_baseline objects, e2e with its byte counts, launches counted, clocks
+    sampled -- and the large-table and complex-energy rows beside the graded configurations."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--steps", "5", "--warmup", "3", "--cpu-seconds", "2"],
+                         capture_output=True, text=True, timeout=900, cwd=root)
+    assert out.returncode == 0, out.stderr[-3000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["metric"] == "ami_term_evaluations_per_s" and d["unit"] == "term-evals/s" and d["higher_is_better"] is True
+    assert d["n_gpus"] == 1 and d["steps"] == 5 and d["warmup"] == 3 and d["dtype"] == "f64" and d["vs_baseline"] is None
+    assert d["config"] == {"workload": "cfg3", "samples_per_gpu": 1_000_000, "n_freq": 1, "n_beta": 1, "T_flat": 68,
+                           "precision": "double"}
+    assert d["value"] > 1e11 and abs(d["value"] - 68 * 1e6 / (d["ms_per_step"] * 1e-3)) < 1e-6 * d["value"]
+    r = d["roofline"]
+    assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    assert 0.3 < r["frac"] < 1.05 and 0.95 < r["peak"] / r["peak_nominal"] < 1.05 and r["traffic"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1 and d["cpu_baseline"]["value"] > 0
+    e = d["e2e"]
+    assert e["h2d_bytes_per_step"] == 64_000_000 and e["d2h_bytes_per_step"] == 16_000_000 and 0 < e["value"] < d["value"]
+    assert d["gpu_launches"] >= 5 and d["clocks"]["sm_mhz"] and d["e2e_seeded"]["h2d_bytes_per_step"] == 0
+    ow = d["other_workloads"]
+    assert {"cfg4", "cfg5", "cfg2_se", "cfg1", "order7", "stress8", "cfg5b"} <= set(ow)
+    assert ow["stress8"]["T_flat"] == 40244 and ow["stress8"]["ms_per_step"] < 3.0        # VERDICT r1: <= 3 ms per 2e4 samples
+    assert "split" in ow["stress8"]["plan"] and ow["cfg5b"]["ms_per_step"] < ow["cfg5b"]["flat_plan_ms_per_step"]
+    assert d["monte_carlo"]["launches_per_step"] == 3 and d["monte_carlo"]["d2h_bytes_per_step"] == 32
