@@ -486,7 +486,6 @@ void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls
                   Sections& S) {
   int cur = 0;
 #define o S.sec[cur]
-  const std::string slot_f = "(" + std::to_string(ls.n_real) + " + b * " + std::to_string(ls.n_fermi) + " + ";
   auto slot_c = [&](size_t u) {
     return "(CB + 2 * (f * " + std::to_string(ls.n_cplx) + " + " + std::to_string(ls.cidx[u]) + "))";
   };
@@ -529,7 +528,7 @@ void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls
         if (hp.d_is_real[u]) {
           o << "#define Dr" << u << " AMI_L(" << ls.ridx[u] << ")\n";
         } else {
-          o << "#define Dr" << u << " AMI_L" << slot_c(u) << "\n#define Di" << u << " AMI_L(" << slot_c(u) << " + 1)\n";
+          o << "#define Dr" << u << " AMI_LC(" << 2 * ls.cidx[u] << ")\n#define Di" << u << " AMI_LC(" << 2 * ls.cidx[u] + 1 << ")\n";
         }
       }
       return;
@@ -567,8 +566,8 @@ void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls
         } else if (hp.d_is_real[u]) {
           o << ind << "  AMI_LS(" << ls.ridx[u] << ", d[" << j << "]);\n";
         } else {
-          o << ind << "  AMI_LS(" << slot_c(u) << ", re" << j << " * d[" << j << "]); AMI_LS(" << slot_c(u) << " + 1, -im" << j
-            << " * d[" << j << "]);\n";
+          o << ind << "  AMI_LSC(" << 2 * ls.cidx[u] << ", re" << j << " * d[" << j << "]); AMI_LSC(" << 2 * ls.cidx[u] + 1
+            << ", -im" << j << " * d[" << j << "]);\n";
         }
       }
       o << ind << "}\n";
@@ -631,7 +630,7 @@ void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls
     };
     auto assign = [&](size_t u, const std::string& value, const std::string& ind) {
       if (mode == kLeafInline) o << ind << "F" << u << " = " << value << ";\n";
-      else o << ind << "AMI_LS(" << slot_f << u << "), " << value << ");\n";
+      else o << ind << "AMI_LSF(" << u << ", " << value << ");\n";
     };
     for (size_t b0 = 0; b0 < base.size(); b0 += kWays) {
       const size_t n = std::min(kWays, base.size() - b0);
@@ -1011,6 +1010,13 @@ static int jit_min_blocks() {
   return std::max(1, kJitWarpsPerSmTarget * 32 / kJitBlockThreads);
 }
 
+// Split plan: tables whose parts want the full register file and a larger L2 budget for the leaf array
+static bool big_table(const FlatTable& ft, const HornerPlan& hp) {
+  long long leaf_doubles = (long long)ft.leafF.size();
+  for (size_t u = 0; u < ft.leafD.size(); ++u) leaf_doubles += hp.d_is_real[u] ? 1 : 2;
+  return leaf_doubles > 250;
+}
+
 std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerPlan& hp, const JitVariant& var,
                                               JitLayout* layout) {
   const int mode = jit_mode(ft, hp);
@@ -1142,14 +1148,21 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
     for (int j = 0; j <= n_mod; ++j) layout->part0.push_back((int)((long long)n_parts * j / n_mod));
   }
   std::vector<std::string> sources;
-  o << "#define AMI_LS(i, v) p.leaves[(long long)(i) * p.leaf_stride + s] = (v)\n";
+  // Layout of the leaf array: one record per tile of AMI_NT samples, [tile][slot][AMI_NT] (p.leaf_stride = doubles
+  // per record), so that inside a part every leaf of a thread sits at a COMPILE-TIME offset from one of three bases
+  // (sample; + temperature; + frequency): every leaf load is LDG [R + imm], no address arithmetic at all.
+  o << "#define AMI_LS(i, v) Ls[(i) * AMI_NT] = (v)\n#define AMI_LSF(u, v) LsF[(u) * AMI_NT] = (v)\n"
+       "#define AMI_LSC(j, v) LsC[(j) * AMI_NT] = (v)\n";
   {   // leaf kernels: everything that depends on one energy combination, written once per sample
     Sections S;
     gen_sections(ft, hp, ls, kLeafStore, E, S);
     o << "__device__ __forceinline__ void ami_leaf_body(const AmiBatch& p, const long long s" << esig << ") {\n"
-      << "  const int CB = " << ls.n_real << " + p.n_b * " << ls.n_fermi << ";\n" << S.sec[0].str()
-      << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << S.sec[1].str() << "  }\n"
-      << "#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n" << S.sec[2].str() << "  }\n}\n\n";
+      << "  const int CB = " << ls.n_real << " + p.n_b * " << ls.n_fermi << ";\n"
+      << "  double* __restrict__ Ls = p.leaves + (s / AMI_NT) * p.leaf_stride + (s % AMI_NT);\n" << S.sec[0].str()
+      << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n"
+      << "    double* __restrict__ LsF = Ls + (" << ls.n_real << " + b * " << ls.n_fermi << ") * AMI_NT;\n" << S.sec[1].str() << "  }\n"
+      << "#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n"
+      << "    double* __restrict__ LsC = Ls + (CB + 2 * f * " << ls.n_cplx << ") * AMI_NT;\n" << S.sec[2].str() << "  }\n}\n\n";
     o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_split_leaves_eval(const __grid_constant__ AmiBatch p) {\n"
          "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n  if (s >= p.n) return;\n";
     for (int i = 0; i < ft.n_eps; ++i) o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
@@ -1183,18 +1196,24 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
   const int pa = (int)((long long)n_parts * mj / n_mod), pb = (int)((long long)n_parts * (mj + 1) / n_mod);
   o.str("");
   o << head.str();
-  o << "#define AMI_L(i) __ldg(Lp + (long long)(i) * ls)\n#define AMI_LF(u) AMI_L(" << ls.n_real << " + b * " << ls.n_fermi
-    << " + (u))\n#define AMI_EMIT(VR, VI) Pp[(long long)(b * n_f + f) * ps] = make_double2((VR), (VI))\n";
+  // Register cap of the parts: the larger the table, the more leaves a part keeps alive.  Measured (B200, N = 2e5,
+  // ms per step at 168 / 255 registers): order 8 (303 leaf doubles) 1.05 / 0.95, order 7 (205) 0.286 / 0.310.
+  if (big_table(ft, hp)) o << "#undef AMI_MINB\n#define AMI_MINB 4\n";
+  o << "#define AMI_L(i) __ldg(Lp + (i) * AMI_NT)\n#define AMI_LF(u) __ldg(LpF + (u) * AMI_NT)\n"
+       "#define AMI_LC(j) __ldg(LpC + (j) * AMI_NT)\n"
+       "#define AMI_EMIT(VR, VI) Pp[(long long)(b * n_f + f) * ps] = make_double2((VR), (VI))\n";
   for (int pi = pa; pi < pb; ++pi) {
     const HornerPlan sub = make_sub_plan(hp, parts[pi]);
     Sections S;
     gen_sections(ft, sub, ls, kLeafLoad, E, S);
     o << "__device__ __noinline__ void ami_part_" << pi
-      << "(const double* __restrict__ Lp, const long long ls, double2* __restrict__ Pp, const long long ps, const int n_b, "
-         "const int n_f) {\n  const int CB = "
-      << ls.n_real << " + n_b * " << ls.n_fermi << ";\n" << S.sec[0].str()
-      << "#pragma unroll 1\n  for (int b = 0; b < n_b; ++b) {\n" << S.sec[1].str()
-      << "#pragma unroll 1\n    for (int f = 0; f < n_f; ++f) {\n" << S.sec[2].str() << S.sec[3].str() << "    }\n  }\n";
+      << "(const double* __restrict__ Lp, double2* __restrict__ Pp, const long long ps, const int n_b, const int n_f) {\n"
+      << "  const int CB = " << ls.n_real << " + n_b * " << ls.n_fermi << ";\n" << S.sec[0].str()
+      << "#pragma unroll 1\n  for (int b = 0; b < n_b; ++b) {\n"
+      << "    const double* __restrict__ LpF = Lp + (" << ls.n_real << " + b * " << ls.n_fermi << ") * AMI_NT;\n" << S.sec[1].str()
+      << "#pragma unroll 1\n    for (int f = 0; f < n_f; ++f) {\n"
+      << "      const double* __restrict__ LpC = Lp + (CB + 2 * f * " << ls.n_cplx << ") * AMI_NT;\n"
+      << S.sec[2].str() << S.sec[3].str() << "    }\n  }\n";
     // the macros that name this part's denominators end with it
     for (size_t u = 0; u < ft.leafD.size(); ++u) o << "#undef Dr" << u << "\n#undef Di" << u << "\n";
     o << "}\n\n";
@@ -1211,11 +1230,11 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
        "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
        "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n"
        "  if (s >= p.n) { asm volatile(\"griddepcontrol.wait;\" ::: \"memory\"); return; }\n"
-       "  const double* Lp = p.leaves + s;\n"
+       "  const double* Lp = p.leaves + blockIdx.x * p.leaf_stride + threadIdx.x;\n"
        "  double2* Pp = reinterpret_cast<double2*>(p.partial) + (long long)(p.part0 + blockIdx.y) * p.n_b * p.n_f * p.partial_stride + s;\n"
        "  switch (blockIdx.y) {\n";
   for (int pi = pa; pi < pb; ++pi)
-    o << "    case " << pi - pa << ": ami_part_" << pi << "(Lp, p.leaf_stride, Pp, p.partial_stride, p.n_b, p.n_f); break;\n";
+    o << "    case " << pi - pa << ": ami_part_" << pi << "(Lp, Pp, p.partial_stride, p.n_b, p.n_f); break;\n";
   o << "  }\n  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n}\n";
   sources.push_back(o.str());
   }
@@ -1592,7 +1611,10 @@ cudaError_t jit_launch(const ami_table* tab, const JitVariant& var, bool fused, 
   const long long rows = (long long)b.n_b * b.n_f;
   const long long slots = lay.n_real_den + (long long)b.n_b * lay.n_fermi + 2LL * b.n_f * lay.n_cplx_den;
   const long long per_sample = slots * 8 + rows * lay.n_parts * 16;
-  long long chunk = std::max<long long>(block, ((64LL << 20) / std::max<long long>(per_sample, 1)) / 256 * 256);
+  // 64 MB of leaves + partials per chunk (96 MB for the largest tables: fewer, fuller launches; measured 1.05 -> 0.97 ms
+  // per 2e5 order-8 samples, while order 7 loses 3 %): L2 holds 126 MB
+  const long long budget = (big_table(tab->flat, tab->horner) ? 96LL : 64LL) << 20;
+  long long chunk = std::max<long long>(block, (budget / std::max<long long>(per_sample, 1)) / 256 * 256);
   chunk = std::min(chunk, (b.n + 255) / 256 * 256);
   double *leaves = nullptr, *partial = nullptr;
   cudaError_t crc = cudaMallocAsync((void**)&leaves, (size_t)(slots * 8 * chunk), st);
@@ -1608,7 +1630,7 @@ cudaError_t jit_launch(const ami_table* tab, const JitVariant& var, bool fused, 
     if (part.k) part.k += c0 * b.k_stride_sample;
     part.first_sample += c0;
     part.out += 2 * c0;
-    part.leaves = leaves; part.leaf_stride = chunk;
+    part.leaves = leaves; part.leaf_stride = slots * block;      // doubles per tile record [slot][block]
     part.partial = partial; part.partial_stride = chunk;
     part.n_parts = lay.n_parts;
     const unsigned gx = (unsigned)((part.n + block - 1) / block);

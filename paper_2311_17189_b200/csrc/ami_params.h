@@ -21,8 +21,9 @@ struct AmiBatch {
   double q[2 * AMI_K_MAX_EXT];
   double t, mu;
   // split plan (tables too large for one register-resident kernel): the leaf kernel writes every Fermi/Bose
-  // value and reciprocal denominator of sample s to column s of leaves[slot][leaf_stride]; part kernel p writes
-  // its partial result of launch-local row r to partial[(p * n_b * n_f + r) * partial_stride + s] (complex)
+  // value and reciprocal denominator of sample s to leaves[(s / NT) * leaf_stride + slot * NT + s % NT] (one record
+  // of leaf_stride doubles per tile of NT = blockDim.x samples); part kernel p writes its partial result of
+  // launch-local row r to partial[(p * n_b * n_f + r) * partial_stride + s] (complex)
   double* leaves;
   long long leaf_stride;
   double* partial;
