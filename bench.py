@@ -641,14 +641,14 @@ def run_ours(args, dist, rank, local, world):
     if world == 1 and rank == 0 and not args.no_extra:
         # secondary workloads (north_star names order 4 AND order 6), short runs, same code path
         others = {}
-        for name in ("cfg4", "cfg5", "cfg2_se", "cfg1", "order7", "stress8"):
+        for name in ("cfg4", "cfg5", "cfg2_se", "cfg1", "order7", "stress8", "order9"):
             if name == cfg.name:
                 continue
-            # order7 / stress8: tables beyond one register-resident kernel (T = 8598 / 40244; the paper runs m = 9,
-            # PAPER.md:389-393), outside the five graded configurations; they run the split plan
-            c2 = A.get_config("stress8" if name == "order7" else name)
-            if name == "order7":
-                c2.diagram, c2.name = A.random_self_energy(7, 0), "order7"
+            # order7 / stress8 / order9: tables beyond one register-resident kernel (T = 8598 / 40244 / 137644; the paper
+            # runs m = 9), outside the five graded configurations; they run the split plan
+            c2 = A.get_config("stress8" if name in ("order7", "order9") else name)
+            if name in ("order7", "order9"):      # order 9: the largest order the paper benchmarks (T = 137644)
+                c2.diagram, c2.name = A.random_self_energy(int(name[-1]), 0), name
             r2 = time_workload(pkg, torch, c2, c2.n_samples, 20, 3, plan, 0, None, sample_clocks=False,
                                use_graph=not args.no_graph)
             i2 = r2["info"]

@@ -446,7 +446,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
       return AMI_OK;
     }
     p.v_stride = (n_e + 255) / 256 * 256;
-    const cudaError_t arc = cudaMallocAsync((void**)&v_scratch, (size_t)p.n_slots * p.v_stride * sizeof(double), st);
+    const cudaError_t arc = ami::scratch_alloc((void**)&v_scratch, (size_t)p.n_slots * p.v_stride * sizeof(double), st);
     if (arc != cudaSuccess) return cuda_fail(arc);
     p.v_scratch = v_scratch;
   }
@@ -560,7 +560,7 @@ int ami_evaluate_momenta_lattice(const ami_table* tab, const double* d_k, int64_
     rc = choose_plan(tab, plan, false, &use_reg, nullptr, var);
     if (rc) return rc;
     if (!use_reg) {
-      CU(cudaMallocAsync((void**)&ws, (size_t)tab->flat.n_eps * (size_t)n * sizeof(double), (cudaStream_t)stream));
+      CU(ami::scratch_alloc((void**)&ws, (size_t)tab->flat.n_eps * (size_t)n * sizeof(double), (cudaStream_t)stream));
       d_e = ws;
     }
   }

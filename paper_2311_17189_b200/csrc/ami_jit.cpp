@@ -373,28 +373,89 @@ void groups_in_trie_order(const HornerPlan& hp, int n, std::vector<int>& out) {
   for (int c : hp.dn[n].kids) groups_in_trie_order(hp, c, out);
 }
 
-// Cuts that order into parts of about `budget` FP64 instructions each (sums a part shares with an earlier
-// part are counted, and formed, again).
-std::vector<std::vector<int>> partition_groups(const HornerPlan& hp, long long budget) {
-  std::vector<int> order;
-  groups_in_trie_order(hp, 0, order);
+// Cuts an order of the groups into parts of about `budget` FP64 instructions each: the FT sums a part reaches (sums
+// it shares with an earlier part are counted, and formed, again) plus its slice of the denominator trie.  Returns the
+// total work of all parts in *total.
+std::vector<std::vector<int>> cut_into_parts(const HornerPlan& hp, const std::vector<int>& order,
+                                             const std::vector<std::vector<int>>& path, long long budget, long long* total) {
   std::vector<std::vector<int>> parts(1);
-  std::vector<char> seen(hp.snodes.size(), 0);
+  std::vector<char> seen(hp.snodes.size(), 0), dseen(hp.dn.size(), 0);
   long long cur = 0;
-  for (int g : order) {
+  *total = 0;
+  auto cost_of = [&](int g, bool commit) {
     const HGroup& hg = hp.groups[g];
-    const long long add = (hg.root >= 0 ? mark_reachable(hp, hg.root, seen) : 0) + 4 * (long long)hg.d.size();
+    long long add = 0;
+    if (hg.root >= 0) {
+      if (commit) {
+        add += mark_reachable(hp, hg.root, seen);
+      } else {
+        std::vector<int> stack(1, hg.root), touched;
+        while (!stack.empty()) {
+          const int id = stack.back();
+          stack.pop_back();
+          if (seen[id]) continue;
+          seen[id] = 1;
+          touched.push_back(id);
+          add += (long long)hp.snodes[id].items.size();
+          for (const SItem& it : hp.snodes[id].items)
+            if (it.child >= 0 && !seen[it.child]) stack.push_back(it.child);
+        }
+        for (int id : touched) seen[id] = 0;
+      }
+    }
+    for (int n : path[g])
+      if (!dseen[n]) {
+        add += hp.d_is_real[hp.dn[n].leaf] ? 1 : 4;
+        if (commit) dseen[n] = 1;
+      }
+    return add;
+  };
+  for (int g : order) {
+    long long add = cost_of(g, false);
     if (cur > 0 && cur + add > budget) {
       parts.emplace_back();
       std::fill(seen.begin(), seen.end(), 0);
-      cur = hg.root >= 0 ? mark_reachable(hp, hg.root, seen) : 0;
-      cur += 4 * (long long)hg.d.size();
-    } else {
-      cur += add;
+      std::fill(dseen.begin(), dseen.end(), 0);
+      cur = 0;
     }
+    add = cost_of(g, true);
+    cur += add;
+    *total += add;
     parts.back().push_back(g);
   }
   return parts;
+}
+
+// Two orders of the groups are tried and the cheaper partition is kept: the depth-first order of the denominator
+// trie (neighbours share denominator prefixes) and the order of the groups' top-level Fermi/Bose sums (neighbours share
+// FT sums).  Which one wins depends on the diagram: order 8 (seed 0) 1.5x / 1.4x the work of the undivided plan,
+// order 9 (seed 0) 3.6x / 1.5x.
+std::vector<std::vector<int>> partition_groups(const HornerPlan& hp, long long budget) {
+  const int G = (int)hp.groups.size();
+  std::vector<std::vector<int>> path(G);          // trie nodes on the way to each group
+  for (int g = 0; g < G; ++g) {
+    int cur = 0;
+    for (int leaf : hp.dseq[g])
+      for (int c : hp.dn[cur].kids)
+        if (hp.dn[c].leaf == leaf) { cur = c; path[g].push_back(c); break; }
+  }
+  std::vector<int> by_trie;
+  groups_in_trie_order(hp, 0, by_trie);
+  std::vector<int> pos(G, 0);
+  for (int i = 0; i < G; ++i) pos[by_trie[i]] = i;
+  std::vector<std::vector<int>> sig(G);           // children of the group's top-level sum
+  for (int g = 0; g < G; ++g)
+    if (hp.groups[g].root >= 0) {
+      for (const SItem& it : hp.snodes[hp.groups[g].root].items)
+        if (it.child >= 0) sig[g].push_back(it.child);
+      std::sort(sig[g].begin(), sig[g].end());
+    }
+  std::vector<int> by_sum = by_trie;
+  std::stable_sort(by_sum.begin(), by_sum.end(), [&](int a, int b) { return sig[a] != sig[b] ? sig[a] < sig[b] : pos[a] < pos[b]; });
+  long long cost_trie = 0, cost_sum = 0;
+  std::vector<std::vector<int>> p_trie = cut_into_parts(hp, by_trie, path, budget, &cost_trie);
+  std::vector<std::vector<int>> p_sum = cut_into_parts(hp, by_sum, path, budget, &cost_sum);
+  return cost_sum < cost_trie ? p_sum : p_trie;
 }
 
 // The Horner plan restricted to `groups`: their FT sums (renumbered, children still before parents) and the
@@ -1617,9 +1678,9 @@ cudaError_t jit_launch(const ami_table* tab, const JitVariant& var, bool fused, 
   long long chunk = std::max<long long>(block, (budget / std::max<long long>(per_sample, 1)) / 256 * 256);
   chunk = std::min(chunk, (b.n + 255) / 256 * 256);
   double *leaves = nullptr, *partial = nullptr;
-  cudaError_t crc = cudaMallocAsync((void**)&leaves, (size_t)(slots * 8 * chunk), st);
+  cudaError_t crc = scratch_alloc((void**)&leaves, (size_t)(slots * 8 * chunk), st);
   if (crc != cudaSuccess) return crc;
-  crc = cudaMallocAsync((void**)&partial, (size_t)(rows * lay.n_parts * 16 * chunk), st);
+  crc = scratch_alloc((void**)&partial, (size_t)(rows * lay.n_parts * 16 * chunk), st);
   if (crc != cudaSuccess) { cudaFreeAsync(leaves, st); return crc; }
   bool ok = true;
   for (long long c0 = 0; c0 < b.n && ok; c0 += chunk) {

@@ -49,6 +49,9 @@ struct JitLayout {
 std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerPlan& hp, const JitVariant& var,
                                               JitLayout* layout);
 
+// stream-ordered workspace from the library's own memory pool (ami_kernels.cu; free with cudaFreeAsync)
+cudaError_t scratch_alloc(void** ptr, size_t bytes, cudaStream_t st);
+
 // NVRTC: CUDA C++ -> sm_100a cubin.  Needs no GPU.  Returns AMI_OK, AMI_EUNSUPPORTED when the
 // NVRTC library cannot be loaded, or AMI_EINVAL when compilation fails (`log` has the reason).
 // With `use_cache` the cubin is looked up in / added to the on-disk cache (see ami_jit.cpp).

@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <atomic>
 #include <cstdio>
+#include <mutex>
 
 #include "ami_device.cuh"
 #include "ami_kernels.cuh"
@@ -21,6 +22,39 @@ void count_external_launch(int* launches) {
 static inline void count_launch(int* launches, int n = 1) {
   g_launches += n;
   if (launches) *launches += n;
+}
+
+// ------------------------------------------------------------------------------------------
+// Stream-ordered workspace (leaf arrays, partial results, value slots, energies).  The default pool of
+// cudaMallocAsync gives its memory back to the driver at every synchronisation (release threshold 0), after which
+// the next call pays a millisecond to get it again; the library's own pool keeps what it has been given.
+// ------------------------------------------------------------------------------------------
+cudaError_t scratch_alloc(void** ptr, size_t bytes, cudaStream_t st) {
+  static std::mutex mu;
+  static cudaMemPool_t pools[64] = {};
+  int dev = 0;
+  cudaError_t rc = cudaGetDevice(&dev);
+  if (rc != cudaSuccess) return rc;
+  cudaMemPool_t pool = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(mu);
+    if (dev >= 0 && dev < 64 && !pools[dev]) {
+      cudaMemPoolProps props = {};
+      props.allocType = cudaMemAllocationTypePinned;
+      props.handleTypes = cudaMemHandleTypeNone;
+      props.location.type = cudaMemLocationTypeDevice;
+      props.location.id = dev;
+      if (cudaMemPoolCreate(&pools[dev], &props) == cudaSuccess) {
+        unsigned long long keep = ~0ull;
+        cudaMemPoolSetAttribute(pools[dev], cudaMemPoolAttrReleaseThreshold, &keep);
+      } else {
+        pools[dev] = nullptr;
+        cudaGetLastError();
+      }
+    }
+    if (dev >= 0 && dev < 64) pool = pools[dev];
+  }
+  return pool ? cudaMallocFromPoolAsync(ptr, bytes, pool, st) : cudaMallocAsync(ptr, bytes, st);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -67,6 +67,8 @@ cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long 
 cudaError_t launch_warp_partial_sums(const double* d_warp_partials, long long n_rows, long long n_warps,
                                      long long row_stride, double* d_partial, double* d_sum, bool first,
                                      cudaStream_t st, int* launches);
+// stream-ordered workspace from the library's own memory pool (free with cudaFreeAsync)
+cudaError_t scratch_alloc(void** ptr, size_t bytes, cudaStream_t st);
 cudaError_t run_fp64_probe(int distinct_sources, double* dfma_per_s, double* ms);
 long long total_launches();
 void count_external_launch(int* launches);
