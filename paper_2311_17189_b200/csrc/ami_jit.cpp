@@ -141,7 +141,8 @@ void emit_snode(const HornerPlan& hp, int id, const std::string& fsuffix, Emitte
 // `leaf_load` (split plan) the Fermi/Bose leaves these nodes use are first loaded into names private
 // to this chunk, so that a leaf occupies a register only while a chunk that uses it is being formed.
 void emit_ft_chunk(const HornerPlan& hp, size_t g0, size_t g1, std::vector<char>& done, Emitter& E,
-                   std::ostringstream& o, const char* indent, const std::string* leaf_load) {
+                   std::ostringstream& o, const char* indent, const std::string* leaf_load,
+                   std::ostringstream* loads = nullptr) {
   std::vector<int> need, stack;
   for (size_t g = g0; g < g1; ++g)
     if (hp.groups[g].root >= 0) stack.push_back(hp.groups[g].root);
@@ -164,7 +165,8 @@ void emit_ft_chunk(const HornerPlan& hp, size_t g0, size_t g1, std::vector<char>
     std::set<int> used;
     for (int id : need)
       for (const SItem& it : hp.snodes[id].items) used.insert(it.leaf);
-    for (int u : used) o << indent << "const double F" << u << fsuffix << " = " << *leaf_load << "(" << u << ");\n";
+    for (int u : used)
+      (loads ? *loads : o) << indent << "const double F" << u << fsuffix << " = " << *leaf_load << "(" << u << ");\n";
   }
   for (size_t i = 0; i < need.size();) {
     size_t j = i;
@@ -746,9 +748,25 @@ void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls
     // FT sums of every group (per beta): a DAG shared by all groups, emitted a few groups at a time
     std::vector<char> done(hp.snodes.size(), 0);
     const std::string loader = "AMI_LF";
-    for (size_t g0 = 0; g0 < hp.groups.size(); g0 += kGroupsPerChunk)
-      emit_ft_chunk(hp, g0, std::min(hp.groups.size(), g0 + kGroupsPerChunk), done, E, o, "    ",
-                    mode == kLeafLoad ? &loader : nullptr);
+    if (mode != kLeafLoad) {
+      for (size_t g0 = 0; g0 < hp.groups.size(); g0 += kGroupsPerChunk)
+        emit_ft_chunk(hp, g0, std::min(hp.groups.size(), g0 + kGroupsPerChunk), done, E, o, "    ", nullptr);
+    } else {
+      // split plan: the leaves of chunk c+1 are requested before the sums of chunk c are formed, so that their
+      // way from L2 (ncu: half of the stall samples were waits for these loads) overlaps arithmetic
+      std::vector<std::string> loads, bodies;
+      for (size_t g0 = 0; g0 < hp.groups.size(); g0 += kGroupsPerChunk) {
+        std::ostringstream l, b;
+        emit_ft_chunk(hp, g0, std::min(hp.groups.size(), g0 + kGroupsPerChunk), done, E, b, "    ", &loader, &l);
+        loads.push_back(l.str());
+        bodies.push_back(b.str());
+      }
+      if (!loads.empty()) o << loads[0];
+      for (size_t c = 0; c < bodies.size(); ++c) {
+        if (c + 1 < loads.size()) o << loads[c + 1];
+        o << bodies[c];
+      }
+    }
     // frequency-independent parts of the R sums (products under purely real denominators), per beta
     std::vector<Stmts> lists;
     for (size_t n = 0; n < hp.dn.size(); ++n) {
