@@ -18,7 +18,8 @@
  * Conventions
  *   - Every function returns int: 0 = AMI_OK, negative = error (see enum).  Nothing throws or
  *     aborts across this boundary.  ami_strerror() names a code, ami_last_cuda_error() gives the
- *     CUDA runtime's message for the last AMI_ECUDA on this thread.
+ *     CUDA runtime's message for the last AMI_ECUDA on this thread.  (ami_tally_static also leaves
+ *     the reason of its own refusals there.)
  *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. a torch tensor's
  *     data_ptr()); h_* and unprefixed array arguments are HOST pointers, read during the call
  *     only.  The library owns only ami_table objects.
@@ -371,6 +372,31 @@ int ami_generate_momenta_lattice(const ami_table* tab, uint64_t seed, int64_t fi
  * real code -- sustains (0.92 of that).  Returns in *dfma_per_s the rate of double-precision FMA lane-operations
  * per second. */
 int ami_fp64_peak_probe(int device, int distinct_sources, double* dfma_per_s, double* elapsed_ms);
+
+/* Allocation-free tally (the one entry point of this library that is safe where cudaMalloc is not: under CUDA
+ * graph capture, in serving loops, in harnesses that forbid allocation).  Computes what ami_run's want_sum does
+ * (Monte-Carlo tally of PAPER.md:291, error bar of :295) for results that are already on the device:
+ *   d_tally[r] = (sum_i re v[r][i], sum_i im v[r][i], sum_i re^2, sum_i im^2),  r < n_rows,
+ * v = d_vals, device complex128, row r starting at element r * row_stride (row_stride >= n; e.g. the
+ * [n_b][n_f][n] result of ami_evaluate with n_rows = n_b * n_f, row_stride = n); d_tally: device double
+ * [n_rows][4], every entry overwritten.  Deterministic: for given (n_rows, n) the order of every sum is fixed.
+ * Asynchronous on `stream`; the call is one cudaMemsetAsync and one kernel, and calls no cudaMalloc, cudaFree or
+ * any allocating routine.
+ * Workspace: the per-block partial sums and the per-row arrival counters live in a file-scope device array of
+ * AMI_TALLY_STATIC_BYTES (516 KiB) that every GPU on which the library is used holds until the process exits.
+ * Limit: n_rows <= AMI_TALLY_STATIC_MAX_ROWS (1024), else AMI_EUNSUPPORTED with the reason in
+ * ami_last_cuda_error(); n is not limited.
+ * ALL calls on a device share that array: calls that may overlap on the GPU (different streams, parallel branches
+ * of a graph, several host threads) race on it and give wrong sums -- order them on one stream or with events.
+ * The counters are cleared by every call; nothing else of the previous call's contents is read.
+ * The first call on a device looks the array's address up (cudaGetSymbolAddress, which may load the module):
+ * call once with n_rows = 0 -- set-up only -- before starting a stream capture.
+ * Errors: AMI_EINVAL (device outside 0..63, null pointer, negative size, row_stride < n), AMI_EUNSUPPORTED
+ * (n_rows above the limit), AMI_ECUDA. */
+#define AMI_TALLY_STATIC_MAX_ROWS 1024
+#define AMI_TALLY_STATIC_BYTES (4096 + 16384 * 32)
+int ami_tally_static(int device, const void* d_vals, int64_t n_rows, int64_t n, int64_t row_stride, double* d_tally,
+                     void* stream);
 
 /* Total number of kernels this library has launched in the calling process so far (all tables, all
  * streams); bench.py reports the difference over its timed region as "gpu_launches". */

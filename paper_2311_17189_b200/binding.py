@@ -23,7 +23,7 @@ EXPORTS = [
     "ami_last_cuda_error", "ami_version", "ami_kernel_launches", "ami_search_sum_order", "ami_graph_parse",
     "ami_graph_label", "ami_table_latex", "ami_evaluate_momenta_lattice", "ami_generate_momenta_lattice",
     "ami_table_kernel_units", "ami_table_kernel_cubin_unit", "ami_table_kernel_source_variant",
-    "ami_table_kernel_cubin_variant", "ami_table_latex_factorized",
+    "ami_table_kernel_cubin_variant", "ami_table_latex_factorized", "ami_tally_static",
 ]
 
 
@@ -107,6 +107,7 @@ def lib():
         L.ami_run.argtypes = [C.c_void_p, C.POINTER(ami_run_cfg), C.POINTER(ami_run_stats)]
         L.ami_generate_momenta.argtypes = [C.c_void_p, C.c_uint64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
         L.ami_fp64_peak_probe.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.ami_tally_static.argtypes = [C.c_int, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
         L.ami_strerror.restype = C.c_char_p
         L.ami_strerror.argtypes = [C.c_int]
         L.ami_last_cuda_error.restype = C.c_char_p
@@ -423,3 +424,26 @@ def fp64_peak_probe(device=0, distinct_sources=2):
     r, ms = C.c_double(0), C.c_double(0)
     _check(lib().ami_fp64_peak_probe(int(device), int(distinct_sources), C.byref(r), C.byref(ms)))
     return r.value, ms.value
+
+
+TALLY_STATIC_MAX_ROWS = 1024   # AMI_TALLY_STATIC_MAX_ROWS
+
+
+def tally_static(vals, tally, stream=None):
+    """ami_tally_static, the allocation-free tally: ``vals`` a contiguous complex128 CUDA tensor [..., n] (every
+    leading index a row), ``tally`` a contiguous float64 CUDA tensor [rows][4] that receives (sum re, sum im,
+    sum re^2, sum im^2) of each row.  Nothing is allocated, by the library or here; at most 1024 rows per call; calls
+    that overlap on the GPU race on the library's static workspace."""
+    n = int(vals.shape[-1]) if vals.dim() else 1
+    rows = int(vals.numel() // n) if n else int(tally.shape[0])
+    if not (vals.is_cuda and tally.is_cuda and vals.is_contiguous() and tally.is_contiguous()) or \
+            vals.element_size() != 16 or tally.element_size() != 8 or tally.numel() != 4 * rows:
+        raise AmiError(-1, "tally_static: vals complex128 [..., n] and tally float64 [rows][4], contiguous CUDA tensors")
+    _check(lib().ami_tally_static(int(vals.device.index or 0), C.c_void_p(vals.data_ptr()), rows, n, n,
+                                  C.c_void_p(tally.data_ptr()), _stream_ptr(stream)))
+
+
+def tally_static_setup(device=0):
+    """The set-up half of ami_tally_static alone (n_rows = 0): looks up the static workspace of ``device``; call it
+    before a stream capture."""
+    _check(lib().ami_tally_static(int(device), None, 0, 0, 0, None, None))

@@ -946,3 +946,132 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   if (stats) *stats = local;
   return AMI_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// ami_tally_static: the Monte-Carlo tally of PAPER.md:291 / :295 for callers that must not allocate (code
+// under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  ami_run forms the same tally with
+// per-block partial sums in a cudaMalloc'ed workspace and a second kernel; here the partial sums and the per-row
+// arrival counters live in ONE file-scope device array that every GPU loading the library holds until exit, and
+// one kernel does both stages: the CTA that arrives last for a row adds the row's partials in a fixed order.
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kStaticTallyMaxRows = AMI_TALLY_STATIC_MAX_ROWS;   // result rows (n_b * n_f) per call
+constexpr int kStaticTallyMaxPartials = 16384;                   // double4 partial sums over all rows of a call
+constexpr size_t kStaticCounterBytes = (size_t)kStaticTallyMaxRows * sizeof(unsigned int);            // 4 KiB
+constexpr size_t kStaticTallyBytes = kStaticCounterBytes + (size_t)kStaticTallyMaxPartials * 32;      // 516 KiB
+static_assert(kStaticCounterBytes % 256 == 0, "the partial sums start on a 256-byte boundary");
+static_assert(kStaticTallyBytes == AMI_TALLY_STATIC_BYTES, "ami.h states the size of the array");
+
+// [0, 4 KiB): arrival counter of each row; [4 KiB, 516 KiB): double4 partial sums [row][block].
+// In host code this name is a stand-in, not a device address: static_tally_scratch() asks the runtime for it.
+static __device__ __align__(256) unsigned char g_static_tally[kStaticTallyBytes];
+
+// Device address of g_static_tally on the CURRENT device: looked up once per device, with that device current.
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+void* g_static_ptr[kStaticMaxDevices] = {};
+
+cudaError_t static_tally_scratch(int device, void** ptr) {
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[device]) {
+    void* p = nullptr;
+    const cudaError_t rc = cudaGetSymbolAddress(&p, g_static_tally);
+    if (rc != cudaSuccess) return rc;
+    g_static_ptr[device] = p;
+  }
+  *ptr = g_static_ptr[device];
+  return cudaSuccess;
+}
+
+// grid (blocks per row, rows) x 256 threads.  Stage 1 as row_partial_kernel (ami_kernels.cu): CTA x of row y adds
+// its slice of the row, (re, im, re^2, im^2), and stores the partial.  Stage 2: the CTA whose ticket says that all
+// others of its row have stored theirs adds the row's partials -- thread t takes partials t, t+256, ... in that
+// order, then a tree of fixed shape -- so the result does not depend on WHICH CTA came last.
+__global__ void __launch_bounds__(256) tally_static_kernel(const double2* __restrict__ v, long long n,
+                                                           long long row_stride, unsigned int* done,
+                                                           double4* partial, double4* __restrict__ tally) {
+  __shared__ double4 sh[256];
+  __shared__ bool last;
+  const long long row = blockIdx.y;
+  const double2* r = v + row * row_stride;
+  const long long per = (n + gridDim.x - 1) / gridDim.x;
+  const long long a = blockIdx.x * per, b = a + per < n ? a + per : n;
+  double4 acc = make_double4(0.0, 0.0, 0.0, 0.0);
+#pragma unroll 4
+  for (long long i = a + threadIdx.x; i < b; i += blockDim.x) {
+    const double2 x = r[i];
+    acc.x += x.x;
+    acc.y += x.y;
+    acc.z = fma(x.x, x.x, acc.z);
+    acc.w = fma(x.y, x.y, acc.w);
+  }
+  auto block_sum = [&]() {
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+      if (threadIdx.x < w) {
+        sh[threadIdx.x].x += sh[threadIdx.x + w].x;
+        sh[threadIdx.x].y += sh[threadIdx.x + w].y;
+        sh[threadIdx.x].z += sh[threadIdx.x + w].z;
+        sh[threadIdx.x].w += sh[threadIdx.x + w].w;
+      }
+      __syncthreads();
+    }
+  };
+  block_sum();
+  if (threadIdx.x == 0) {
+    partial[row * gridDim.x + blockIdx.x] = sh[0];
+    __threadfence();                                   // the partial is visible before the ticket is taken
+    last = atomicAdd(&done[row], 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();                                     // the other CTAs' partials are visible to every thread here
+  acc = make_double4(0.0, 0.0, 0.0, 0.0);
+  for (int i = threadIdx.x; i < (int)gridDim.x; i += 256) {
+    const double2* q = reinterpret_cast<const double2*>(&partial[row * gridDim.x + i]);   // L2 loads: not via a stale L1 line
+    const double2 lo = __ldcg(q), hi = __ldcg(q + 1);
+    acc.x += lo.x; acc.y += lo.y; acc.z += hi.x; acc.w += hi.y;
+  }
+  block_sum();
+  if (threadIdx.x == 0) tally[row] = sh[0];
+}
+
+// blocks per row: a function of (rows, n) only, so the order of the sum is fixed
+int static_tally_blocks(long long n_rows, long long n) {
+  long long b = (8 * 148 + n_rows - 1) / n_rows;
+  b = std::min<long long>(b, (n + 1023) / 1024);
+  b = std::min<long long>(b, kStaticTallyMaxPartials / n_rows);
+  return (int)std::max<long long>(1, b);
+}
+
+}  // namespace
+
+extern "C" int ami_tally_static(int device, const void* d_vals, int64_t n_rows, int64_t n, int64_t row_stride,
+                                double* d_tally, void* stream) {
+  if (device < 0 || device >= kStaticMaxDevices || n_rows < 0 || n < 0 || (n_rows > 0 && !d_tally) ||
+      (n_rows > 0 && n > 0 && !d_vals) || (n_rows > 1 && row_stride < n)) {
+    g_cuda_err = "ami_tally_static: bad argument (device, null pointer, negative size, or row_stride < n)";
+    return AMI_EINVAL;
+  }
+  if (n_rows > kStaticTallyMaxRows) {
+    g_cuda_err = "ami_tally_static: " + std::to_string((long long)n_rows) + " rows exceed the static workspace's maximum of " +
+                 std::to_string(kStaticTallyMaxRows) + " rows per call (split the rows over several calls)";
+    return AMI_EUNSUPPORTED;
+  }
+  CU(cudaSetDevice(device));
+  void* scratch = nullptr;
+  CU(static_tally_scratch(device, &scratch));   // n_rows = 0: set-up only (do this once before a graph capture)
+  if (n_rows == 0) return AMI_OK;
+  const cudaStream_t st = (cudaStream_t)stream;
+  unsigned int* done = (unsigned int*)scratch;
+  double4* partial = (double4*)((unsigned char*)scratch + kStaticCounterBytes);
+  // the array keeps what the last call left: the counters of the rows of THIS call start at zero
+  CU(cudaMemsetAsync(done, 0, (size_t)n_rows * sizeof(unsigned int), st));
+  dim3 grid((unsigned)static_tally_blocks(n_rows, n), (unsigned)n_rows);
+  tally_static_kernel<<<grid, 256, 0, st>>>((const double2*)d_vals, n, row_stride, done, partial, (double4*)d_tally);
+  ami::count_external_launch(nullptr);
+  CU(cudaGetLastError());
+  return AMI_OK;
+}
