@@ -28,6 +28,10 @@ import numpy as np  # noqa: E402
 METRIC = "ami_term_evaluations_per_s"
 UNIT = "term-evals/s"
 SUM_ORDER = "default"
+ORDERED_ONLY = False     # --ordered: issue every step in plain stream order (no AMI_PLAN_UNORDERED)
+BATCHES_NOTE = ("independent batches, each with its own momenta and result buffer, issued with AMI_PLAN_UNORDERED (the "
+                "kernel of one batch may start while its predecessor drains); the batch that begins the reuse of the "
+                "buffers is ordered; ordered_ms_per_step = the same K batches in plain stream order")
 
 
 def parse_args():
@@ -43,6 +47,8 @@ def parse_args():
                     help="order of the Matsubara sums: the configuration's (default) or the one ami_search_sum_order picks")
     ap.add_argument("--no-extra", action="store_true", help="skip the secondary workloads and the CPU baseline")
     ap.add_argument("--no-graph", action="store_true", help="launch every step from Python instead of one CUDA graph")
+    ap.add_argument("--ordered", action="store_true",
+                    help="issue the steps in plain stream order instead of as independent batches (AMI_PLAN_UNORDERED)")
     ap.add_argument("--sweep", action="store_true",
                     help="batch-size sweep (BASELINE config 2: N = 1e3..1e8; the paper's Figs. 4-5 plot time against "
                          "the batch size): one JSON line with a row per (workload, N); one GPU")
@@ -271,26 +277,32 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
     n_f, n_b = len(cfg.z_ext), len(cfg.betas)
     bytes_in = n * 2 * m * 8
     n_rot = int(max(2, min(8, -(-300_000_000 // max(bytes_in + n * n_eps * 8, 1)))))
-    ks = [tab.generate_momenta(cfg.seed, first_sample + r * n, n) for r in range(n_rot)]
-    es = [torch.empty((n_eps, n), dtype=torch.float64, device="cuda") for _ in range(n_rot)] \
-        if not (plan in (0, 2) and info["reg_plan_status"] in (0, 1)) else []
-    out = torch.empty((n_b, n_f, n), dtype=torch.complex128, device="cuda")
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
-    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-
     reg = plan in (0, 2) and info["reg_plan_status"] in (0, 1)
     if reg:
         info = tab.specialize()        # NVRTC compile (or cache fetch) + load happen here, outside every timed region
+    # The K batches of a step sequence are independent of one another (own momenta, own results: the batches of a
+    # Monte-Carlo loop), so with the register plan they are issued as such (AMI_PLAN_UNORDERED): every
+    # batch has its own result buffer and the one that begins the reuse of the buffers is issued ordered.
+    independent = bool(reg and use_graph and int(info.get("plan_kind", 1)) == 1 and not ORDERED_ONLY)
+    if independent:                    # eight buffer sets where 8 GB hold them: one batch in eight is ordered
+        n_rot = int(max(n_rot, min(8, 8_000_000_000 // max(bytes_in + n * n_f * n_b * 16, 1))))
+    ks = [tab.generate_momenta(cfg.seed, first_sample + r * n, n) for r in range(n_rot)]
+    es = [torch.empty((n_eps, n), dtype=torch.float64, device="cuda") for _ in range(n_rot)] if not reg else []
+    outs = [torch.empty((n_b, n_f, n), dtype=torch.complex128, device="cuda") for _ in range(n_rot if independent else 1)]
+    out = outs[0]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
-    def step(i, events=None):
+    def step(i, events=None, unordered=False):
         r = i % n_rot
         if events:
             events[0].record()
         if reg:     # one fused kernel: dispersion inline, energies stay in registers
             if events:
                 events[1].record()
-            tab.evaluate_momenta(ks[r], [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan,
-                                 out=out)
+            flag = pkg.PLAN_UNORDERED if (unordered and r != 0) else 0
+            tab.evaluate_momenta(ks[r], [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=plan | flag,
+                                 out=outs[r % len(outs)])
         else:
             tab.dispersion(ks[r], [cfg.q], cfg.t, cfg.mu, out=es[r])
             if events:
@@ -311,7 +323,7 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
         graph = torch.cuda.CUDAGraph()
         with torch.cuda.graph(graph):
             for i in range(steps):
-                step(warmup + i)
+                step(warmup + i, unordered=independent)
         launches = pkg.kernel_launches() - l0     # kernels recorded in the graph = launched per replay
         graph.replay()                            # one untimed replay: graph upload
         torch.cuda.synchronize()
@@ -353,43 +365,24 @@ def time_workload(pkg, torch, cfg, n, steps, warmup, plan, first_sample, dist, s
         disp_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
         eval_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
     checksum = complex(out[0, 0, : min(n, 1024)].sum().item())
-    two_stream_ms = None
-    if graph is not None and dist is None:
-        try:
-            two_stream_ms = time_two_streams(torch, tab, cfg, ks, steps, plan)
-        except Exception as exc:  # noqa: BLE001  (extra figure only; the headline never depends on it)
-            two_stream_ms = f"unavailable: {exc}"
+    ordered_ms = None          # the same K batches, every one ordered after the one before (plain stream order)
+    if independent:
+        g2 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g2):
+            for i in range(steps):
+                step(warmup + i)
+        g2.replay()
+        torch.cuda.synchronize()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record()
+        g2.replay()
+        t1.record()
+        torch.cuda.synchronize()
+        ordered_ms = t0.elapsed_time(t1) / steps
+        del g2
     return {"tab": tab, "info": info, "construct_ms": construct_ms, "fused": reg, "tree": plan == 3, "total_ms": total_ms, "disp_ms": disp_ms, "eval_ms": eval_ms,
-            "launches": launches, "clocks": clocks, "graph": graph is not None, "two_stream_ms": two_stream_ms, "n_rot": n_rot, "checksum": checksum,
+            "launches": launches, "clocks": clocks, "graph": graph is not None, "ordered_ms": ordered_ms, "independent": independent, "n_rot": n_rot, "checksum": checksum,
             "bytes_in": bytes_in, "bytes_e": n * n_eps * 8, "bytes_out": n * n_f * n_b * 16}
-
-
-def time_two_streams(torch, tab, cfg, ks, steps, plan):
-    """Throughput with the K steps issued alternately on two streams (what ami_run does with its
-    chunks): the ramp of one kernel overlaps the tail of the previous one.  Captured in one CUDA
-    graph; returns ms per step.  Each stream writes its own result buffer."""
-    n = ks[0].shape[0]
-    n_f, n_b = len(cfg.z_ext), len(cfg.betas)
-    outs = [torch.empty((n_b, n_f, n), dtype=torch.complex128, device="cuda") for _ in range(2)]
-    side = torch.cuda.Stream()
-    graph = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(graph):
-        main = torch.cuda.current_stream()
-        side.wait_stream(main)
-        for i in range(steps):
-            st = main if i % 2 == 0 else side
-            with torch.cuda.stream(st):
-                tab.evaluate_momenta(ks[i % len(ks)], [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg,
-                                     plan=plan, out=outs[i % 2])
-        main.wait_stream(side)
-    graph.replay()
-    torch.cuda.synchronize()
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t0.record()
-    graph.replay()
-    t1.record()
-    torch.cuda.synchronize()
-    return t0.elapsed_time(t1) / steps
 
 
 def time_e2e(pkg, torch, tab, cfg, n, steps, warmup, plan, first_sample, dist):
@@ -574,8 +567,8 @@ def run_ours(args, dist, rank, local, world):
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local)
     pkg.lib()   # raises if libami_b200.so has not been built
-    global SUM_ORDER
-    SUM_ORDER = args.sum_order
+    global SUM_ORDER, ORDERED_ONLY
+    SUM_ORDER, ORDERED_ONLY = args.sum_order, args.ordered
     cfg = A.get_config(args.workload)
     n = samples_per_step(cfg, args)
     first, _ = sharding.weak_range(n, rank, world)
@@ -594,6 +587,9 @@ def run_ours(args, dist, rank, local, world):
     ms_per_step = res["total_ms"] / args.steps
     value = T * units_per_step / (ms_per_step * 1e-3)
     roof, disp = roofline_objects(res, n, n_f, n_b, peaks, dfma_per_s, dfma3_per_s)
+    if res["ordered_ms"] is not None:      # the same kernel with every batch ordered after the one before
+        roof["frac_ordered"] = roof["frac"] * res["eval_ms"] / res["ordered_ms"]
+        roof["batches"] = "independent (AMI_PLAN_UNORDERED); frac_ordered: plain stream order"
     cap = ncu_capture(cfg.name, res["fused"]) if n == cfg.n_samples else None
     if cap:      # per launch, from profiles/ (ncu --set full of the same command, committed)
         roof["traffic"] = cap["dram_bytes"]
@@ -625,7 +621,8 @@ def run_ours(args, dist, rank, local, world):
         "kernels": {"dominant_ms": res["eval_ms"], "ami_dispersion_ms": None if res["fused"] else res["disp_ms"],
                     "dispersion": disp, "launches_per_step": res["launches"] / max(1, args.steps),
                     "timed_as": "one CUDA graph of K steps" if res["graph"] else "K launches from the host",
-                    "two_stream_ms_per_step": res["two_stream_ms"]},
+                    "batches": BATCHES_NOTE if res["independent"] else "every step ordered after the one before",
+                    "ordered_ms_per_step": res["ordered_ms"]},
         "roofline": roof,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                 "steps": e2e_steps, "chunks_per_step": e2e["chunks"], "api": "ami_run(h_k -> h_out)",
@@ -664,7 +661,8 @@ def run_ours(args, dist, rank, local, world):
                             "hbm_frac": roof2["hbm_leg"]["frac"], "fp64_slots_per_sample": roof2["fp64_slots_counted"],
                             "construct_ms": r2["construct_ms"], "specialize_ms": float(i2["specialize_ms"]),
                             "specialize_from_disk_cache": bool(i2["specialize_cached"]),
-                            "two_stream_ms_per_step": r2["two_stream_ms"]}
+                            "ordered_ms_per_step": r2["ordered_ms"],
+                            "alu_frac_ordered": None if r2["ordered_ms"] is None else roof2["frac"] * ms2 / r2["ordered_ms"]}
             if int(i2.get("plan_kind", 1)) == 2:
                 # the split plan's parts read every leaf they use from the L2-resident leaf array: that, not the FP64
                 # pipe, bounds it; the slots counted are those of the Horner plan, without the sums
@@ -736,6 +734,8 @@ def run_sweep(args, local):
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local)
     pkg.lib()
+    global ORDERED_ONLY
+    ORDERED_ONLY = args.ordered
     plan = PLAN_IDS[args.plan]
     dfma_per_s, _ = pkg.fp64_peak_probe(local)
     peaks = load_measured_peaks()
@@ -755,7 +755,8 @@ def run_sweep(args, local):
                          "ns_per_sample": ms * 1e6 / (n * n_f * n_b), "samples_per_s": n * n_f * n_b / (ms * 1e-3),
                          "term_evals_per_s": T * n * n_f * n_b / (ms * 1e-3), "alu_frac": roof["frac"],
                          "hbm_frac": roof["hbm_leg"]["frac"], "launches_per_step": r["launches"] / steps,
-                         "two_stream_ms_per_step": r["two_stream_ms"]})
+                         "ordered_ms_per_step": r["ordered_ms"],
+                         "alu_frac_ordered": None if r["ordered_ms"] is None else roof["frac"] * ms / r["ordered_ms"]})
             del r
             torch.cuda.empty_cache()
     ex1 = time_paper_example1(pkg, torch, A.get_config("paper_ex1"), max(3, args.steps // 2), args.warmup, plan, peaks,

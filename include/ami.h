@@ -78,6 +78,23 @@ enum {
                          part), then a kernel that adds the parts (split plan).  ami_info.plan_kind says which */
 };
 
+/* Flag, OR-ed into the `plan` argument of ami_evaluate / ami_evaluate_momenta / ami_evaluate_momenta_lattice:
+ * the caller states that this call is INDEPENDENT of the calls of this library issued right before it on the same
+ * stream that carry the flag too (it reads nothing they write and writes nothing they read or write -- e.g. the
+ * batches of a Monte-Carlo loop, each with its own momenta and result buffer, "repeatedly call this
+ * function for different energy batches").  Such a run of calls may then execute beside one another: the
+ * register-plan kernel of a flagged call does not wait for its predecessor before it starts, so the ramp of one batch
+ * fills the SMs the tail of the previous one leaves idle (20-35 % more throughput for batches of 1e4-1e5 samples,
+ * profiles/r02_batch_sweep.md).  Everything else keeps stream order: a flagged kernel COMPLETES only after its
+ * predecessor has (it waits at its end), so an unflagged call, a copy, an event or any other work enqueued after a
+ * run of flagged calls sees all of them finished, and a flagged call that follows work of another kind (a copy, a
+ * kernel of the caller, an unflagged call) starts only when that has finished.  ALL calls of an uninterrupted run
+ * of flagged calls are mutually unordered, not only neighbours: a loop that rotates over R buffer sets issues the
+ * call that begins the reuse of a set WITHOUT the flag (every R-th call), which closes the run before it.
+ * Ignored by the split plan and the table-driven plans (they stay ordered); refused by ami_run (AMI_EINVAL), which
+ * orders its own chunks. */
+#define AMI_PLAN_UNORDERED 0x100
+
 enum { AMI_KIND_NONE = 0, AMI_KIND_REGISTER = 1, AMI_KIND_SPLIT = 2 };
 
 typedef struct ami_info {
@@ -261,7 +278,7 @@ int ami_dispersion_lattice(const ami_table* tab, const double* d_k, int64_t k_st
  *   e_reg   regulator eta, applied as in P10: added to the argument of every sigma = -1
  *           leaf and to every denominator whose frequency part is identically zero for that
  *           frequency; decided by table and frequency metadata only, never by sample values.
- *   plan    AMI_PLAN_*
+ *   plan    AMI_PLAN_*, optionally | AMI_PLAN_UNORDERED
  *   d_out   complex128 [n_b][n_f][n_e] (rows = frequencies, energy index fastest) */
 int ami_evaluate(const ami_table* tab, const void* d_e, int e_is_complex, int64_t n_e, const double* z_ext,
                  int n_f, const double* beta, int n_b, double e_reg, int plan, void* d_out, void* stream);

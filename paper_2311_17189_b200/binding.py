@@ -13,6 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libami_b200.so")
 
 PLAN_AUTO, PLAN_FLAT, PLAN_REG, PLAN_TREE = 0, 1, 2, 3
+PLAN_UNORDERED = 0x100   # AMI_PLAN_UNORDERED: OR into `plan` (see include/ami.h)
 BAND_TIGHT_BINDING, BAND_FREE = 0, 1
 
 EXPORTS = [

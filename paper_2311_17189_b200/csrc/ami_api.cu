@@ -386,6 +386,8 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
                   void* d_out, int64_t out_row_stride, cudaStream_t st, int* launches) {
   using namespace ami;
   bool use_reg = false, use_tree = false;
+  const bool unordered = (plan & AMI_PLAN_UNORDERED) != 0;   // honoured by the register plan, ignored by the others
+  plan &= ~AMI_PLAN_UNORDERED;
   ami::JitVariant var;
   if (mom) { var.dim = mom->dim; var.band = mom->band; }
   var.cplx = e_is_complex != 0;
@@ -463,6 +465,7 @@ int evaluate_impl(const ami_table* tab, const MomentaSrc* mom, const void* d_e, 
         // later launches of a split grid read the energies the first one stored
         const bool fused = mom && (first || !d_e);
         if (!fused) { jb.e_out = nullptr; }
+        jb.unordered = unordered && first ? 1 : 0;   // later launches of the same call stay ordered after the first
         int n_launched = 0;
         long long slots = 0;
         crc = jit_launch(tab, var, fused, jb, st, &n_launched, &slots);
@@ -523,8 +526,9 @@ int ami_evaluate(const ami_table* tab, const void* d_e, int e_is_complex, int64_
                  int n_f, const double* beta, int n_b, double e_reg, int plan, void* d_out, void* stream) {
   int rc = check_device(tab);
   if (rc) return rc;
+  const int base_plan = plan & ~AMI_PLAN_UNORDERED;
   if (n_e < 0 || n_f < 0 || n_b < 0 || (n_f > 0 && tab->flat.n_ext > 0 && !z_ext) || (n_b > 0 && !beta) ||
-      plan < AMI_PLAN_AUTO || plan > AMI_PLAN_TREE)
+      base_plan < AMI_PLAN_AUTO || base_plan > AMI_PLAN_TREE)
     return AMI_EINVAL;
   if (n_e == 0 || n_f == 0 || n_b == 0) return AMI_OK;
   if (!d_e || !d_out) return AMI_EINVAL;
@@ -539,7 +543,8 @@ int ami_evaluate_momenta_lattice(const ami_table* tab, const double* d_k, int64_
   int rc = check_device(tab);
   if (rc) return rc;
   if (n < 0 || n_f < 0 || n_b < 0 || (n_f > 0 && tab->flat.n_ext > 0 && !z_ext) || (n_b > 0 && !beta) ||
-      (tab->flat.n_ext > 0 && !q) || plan < AMI_PLAN_AUTO || plan > AMI_PLAN_TREE || dim < 1 || dim > 3 ||
+      (tab->flat.n_ext > 0 && !q) || (plan & ~AMI_PLAN_UNORDERED) < AMI_PLAN_AUTO ||
+      (plan & ~AMI_PLAN_UNORDERED) > AMI_PLAN_TREE || dim < 1 || dim > 3 ||
       (band != AMI_BAND_TIGHT_BINDING && band != AMI_BAND_FREE))
     return AMI_EINVAL;
   if (n == 0) return AMI_OK;
@@ -557,7 +562,7 @@ int ami_evaluate_momenta_lattice(const ami_table* tab, const double* d_k, int64_
   ami::JitVariant var;
   var.dim = dim; var.band = band;
   if (!d_e) {
-    rc = choose_plan(tab, plan, false, &use_reg, nullptr, var);
+    rc = choose_plan(tab, plan & ~AMI_PLAN_UNORDERED, false, &use_reg, nullptr, var);
     if (rc) return rc;
     if (!use_reg) {
       CU(ami::scratch_alloc((void**)&ws, (size_t)tab->flat.n_eps * (size_t)n * sizeof(double), (cudaStream_t)stream));
@@ -812,6 +817,7 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
       (cfg->n_b > 0 && !cfg->beta) || (cfg->n_f > 0 && tab->flat.n_ext > 0 && !cfg->z_ext) ||
       (tab->flat.n_ext > 0 && !cfg->q) || (cfg->h_k && cfg->d_k) || (cfg->want_sum && !cfg->h_sum) ||
       (!cfg->want_sum && !cfg->h_out && !cfg->d_out) || cfg->dim < 0 || cfg->dim > 3 ||
+      cfg->plan < AMI_PLAN_AUTO || cfg->plan > AMI_PLAN_TREE ||   /* the driver orders its own chunks: no AMI_PLAN_UNORDERED */
       (cfg->band != AMI_BAND_TIGHT_BINDING && cfg->band != AMI_BAND_FREE))
     return AMI_EINVAL;
   ami_run_stats local;

@@ -1096,6 +1096,13 @@ static bool big_table(const FlatTable& ft, const HornerPlan& hp) {
   return leaf_doubles > 250;
 }
 
+// Last statement of the register-plan kernels.  An ordered launch (the default) waited for its predecessor before
+// touching memory.  An unordered one (AMI_PLAN_UNORDERED: the caller states that it shares no buffer with the
+// specialised launches right before it) ran beside them and waits HERE instead, every thread before it exits: the grid
+// then completes only after its predecessor has, so whatever is ordered after it in the stream -- an ordered launch,
+// a copy, an event -- still comes after everything before it.
+static const char* const kUnorderedEnd = "  if (p.unordered) asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n";
+
 std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerPlan& hp, const JitVariant& var,
                                               JitLayout* layout) {
   const int mode = jit_mode(ft, hp);
@@ -1131,7 +1138,7 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
   auto fused_open = [&](const char* name, const char* tiles) {
     o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) " << name << "(const __grid_constant__ AmiBatch p) {\n"
          "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
-         "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
+         "  if (!p.unordered) asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
          "  const long long base = blockIdx.x * (long long)AMI_NT * (" << tiles << ") + threadIdx.x;\n"
          "  double4 t4 = make_double4(0.0, 0.0, 0.0, 0.0);\n"
          "#pragma unroll 1\n  for (int u = 0; u < (" << tiles << "); ++u) {\n"
@@ -1188,7 +1195,7 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
     // ---- kernel 1: energies from memory ---------------------------------------------------------
     o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
          "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
-         "  asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
+         "  if (!p.unordered) asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
          "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
          "  const bool valid = true;\n"
          "  double4 t4 = make_double4(0.0, 0.0, 0.0, 0.0);\n"
@@ -1201,7 +1208,7 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
       else
         o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
     }
-    o << subst(call, "<false>") << "  }\n}\n\n";
+    o << subst(call, "<false>") << "  }\n" << kUnorderedEnd << "}\n\n";
     if (var.cplx) return std::vector<std::string>(1, o.str());   // momenta give real energies: no fused kernels
     // ---- kernels 2, 3: momenta from memory or drawn in place, dispersion inline; without / with the tally ----
     for (int tally = 0; tally < 2; ++tally) {
@@ -1210,7 +1217,7 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
       if (tally)   // single-row tally: one partial per warp of the grid, formed from the threads' own sums
         o << "  if (p.tally_acc) ami_tally(reinterpret_cast<double4*>(p.tally) + (long long)(p.b0 * p.n_f_total + p.f0) * "
              "p.tally_stride + blockIdx.x * (AMI_NT / 32) + (threadIdx.x >> 5), t4.x, t4.y, t4.z, t4.w);\n";
-      o << "}\n\n";
+      o << kUnorderedEnd << "}\n\n";
     }
     return std::vector<std::string>(1, o.str());
   }

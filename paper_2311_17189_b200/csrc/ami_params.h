@@ -32,6 +32,8 @@ struct AmiBatch {
   int part0;                // split plan: index of the first part of the module being launched
   int tiles;                // fused kernels: consecutive tiles of blockDim.x samples one CTA walks
   int tally_acc;            // fused tally with ONE result row: every thread adds its `tiles` samples before the warp adds up
+  int unordered;            // register plan: the caller declared this launch independent of the specialised launches just
+                            // before it in the stream (AMI_PLAN_UNORDERED): it waits for them at its END, not its start
   double* e_out;            // optional [n_eps][n] copy of the energies formed by the fused path
   // fused tally (or NULL): per-warp partial sums (re, im, re^2, im^2) of row r at tally[(r * tally_stride + (s >> 5)) * 4]
   double* tally;

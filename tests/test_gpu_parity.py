@@ -641,6 +641,78 @@ def test_run_device_output_and_determinism(ami, torch_mod):
     assert s1["n_chunks"] == 10
 
 
+@pytest.mark.parametrize("name,n", [("cfg1", 10_000), ("cfg4", 20_000 + 5), ("cfg5", 3000 + 1)])
+def test_unordered_calls_keep_results_and_stream_order(ami, torch_mod, name, n):
+    """AMI_PLAN_UNORDERED (include/ami.h): a run of calls declared independent gives bit for bit what the same calls
+    give in plain stream order, and what is ordered after the run comes after all of it:
+    (a) R batches with their own buffers, the first ordered, the rest flagged, read back by a torch kernel;
+    (b) an UNFLAGGED call that overwrites the result buffer of the first flagged one wins (write after write);
+    (c) a flagged call whose momenta a torch kernel writes just before it reads the new momenta (read after write
+        across work that is not this library's);
+    (d) the same inside one CUDA graph, replayed twice.  The energies from memory (ami_evaluate) likewise."""
+    torch = torch_mod
+    cfg = A.get_config(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    assert tab.specialize()["plan_kind"] == 1
+    R = 6
+    U = ami.PLAN_UNORDERED
+    ks = [tab.generate_momenta(cfg.seed, r * n, n) for r in range(R)]
+    call = lambda k, out, flag: tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg,
+                                                     plan=flag, out=out)
+    shape = (len(cfg.betas), len(cfg.z_ext), n)
+    want = [call(k, torch.empty(shape, dtype=torch.complex128, device="cuda"), 0) for k in ks]
+    bits = lambda x: x.view(torch.float64)
+    # (a)
+    outs = [torch.zeros(shape, dtype=torch.complex128, device="cuda") for _ in range(R)]
+    for rep in range(3):
+        for r in range(R):
+            call(ks[r], outs[r], U if r else 0)
+    total = torch.stack([bits(o) for o in outs]).clone()          # a torch kernel right behind the run
+    assert torch.equal(total, torch.stack([bits(w) for w in want]))
+    # (b)
+    for o in outs:
+        o.zero_()
+    call(ks[0], outs[0], 0)
+    call(ks[1], outs[1], U)
+    call(ks[2], outs[2], U)
+    call(ks[3], outs[1], 0)            # reuse of outs[1]: issued without the flag
+    assert torch.equal(bits(outs[1]), bits(want[3])) and torch.equal(bits(outs[2]), bits(want[2]))
+    # (c)
+    k_var = torch.zeros_like(ks[0])
+    for r in (4, 5, 4):
+        k_var.copy_(ks[r])                                        # not a kernel of this library: full stream order
+        call(k_var, outs[r], U)
+    assert torch.equal(bits(outs[4]), bits(want[4])) and torch.equal(bits(outs[5]), bits(want[5]))
+    # (d)
+    for o in outs:
+        o.zero_()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for i in range(2 * R):
+            call(ks[i % R], outs[i % R], U if i % R else 0)
+    for rep in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    assert all(torch.equal(bits(o), bits(w)) for o, w in zip(outs, want))
+    # energies from memory
+    es = [tab.dispersion(k, [cfg.q], cfg.t, cfg.mu) for k in ks[:3]]
+    ev = lambda e, out, flag: tab.evaluate(e, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=flag, out=out)
+    want_e = [ev(e, torch.empty(shape, dtype=torch.complex128, device="cuda"), 0) for e in es]
+    for r in range(3):
+        outs[r].zero_()
+        ev(es[r], outs[r], U if r else 0)
+    assert all(torch.equal(bits(outs[r]), bits(want_e[r])) for r in range(3))
+    # the table-driven plans accept the flag and stay ordered; ami_run refuses it
+    flat = tab.evaluate_momenta(ks[0], [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=PLANS["flat"] | U,
+                                e_out=torch.empty((cfg.diagram.n_eps, n), dtype=torch.float64, device="cuda"))
+    ref = tab.evaluate_momenta(ks[0], [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, e_reg=cfg.e_reg, plan=PLANS["flat"],
+                               e_out=torch.empty((cfg.diagram.n_eps, n), dtype=torch.float64, device="cuda"))
+    assert torch.equal(bits(flat), bits(ref))
+    with pytest.raises(ami.AmiError):
+        tab.run(n, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=1, want_sum=True, plan=U)
+
+
 def test_run_default_chunking_and_workspace_reuse(ami, torch_mod):
     """ami_run with host buffers and the library's default chunk (2^17 samples): several chunks on two
     streams, the cached workspace reused and grown across calls of different sizes and row counts."""
