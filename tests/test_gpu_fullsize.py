@@ -54,6 +54,41 @@ def test_full_size_fused_call(ami, oracle_mod, name, n_truth):
     assert np.array_equal(again.cpu().numpy(), got)
 
 
+@pytest.mark.parametrize("name,n_truth", [("cfg3", 1500), ("cfg4", 300)])
+def test_full_size_independent_batches_in_a_graph(ami, oracle_mod, name, n_truth):
+    """The launch configuration bench.py times since AMI_PLAN_UNORDERED exists: K full-size batches with their own
+    momenta and result buffers captured in ONE CUDA graph, the first of every round over the buffer sets ordered, the
+    others flagged.  Sampled outputs of the LAST and of a middle batch against the oracle; every batch bit-equal to
+    the same batch evaluated alone."""
+    import torch
+    cfg = A.get_config(name)
+    n, R, K = cfg.n_samples, 4, 9
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    tab.specialize()
+    ks = [tab.generate_momenta(cfg.seed, r * n, n) for r in range(R)]
+    outs = [torch.zeros((len(cfg.betas), len(cfg.z_ext), n), dtype=torch.complex128, device="cuda") for _ in range(R)]
+    call = lambda r, out, flag: tab.evaluate_momenta(ks[r], [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas,
+                                                     e_reg=cfg.e_reg, plan=flag, out=out)
+    call(0, outs[0], 0)          # warm-up outside the capture
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for i in range(K):
+            call(i % R, outs[i % R], ami.PLAN_UNORDERED if i % R else 0)
+    for o in outs:
+        o.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    for r in (K - 1) % R, 2:
+        sel = np.unique(np.concatenate([np.linspace(0, n - 1, n_truth).astype(np.int64), [0, 63, 64, n - 65, n - 1]]))
+        got = outs[r][:, :, torch.from_numpy(sel).cuda()].cpu().numpy()
+        for b, (truth, S) in enumerate(oracle_subset(oracle_mod, cfg, sel + r * n)):
+            check_parity(got[b], truth, S, label=f"{name} batch {r} of the graph")
+    for r in range(R):
+        alone = call(r, torch.empty_like(outs[r]), 0)
+        assert torch.equal(alone.view(torch.float64), outs[r].view(torch.float64)), f"batch {r}"
+
+
 @pytest.mark.parametrize("name", ["cfg2_se", "cfg2_bubble", "cfg2_bubble_doubled"])
 def test_cfg2_sweep_large_batch_streamed(ami, oracle_mod, name):
     """N = 1e7 samples x 8 frequencies through the streamed driver with device-generated momenta
