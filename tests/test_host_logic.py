@@ -31,6 +31,56 @@ def test_library_exports_every_declared_symbol(ami):
     assert L.ami_version() >= 1
 
 
+C_CALLER = r"""
+/* A caller written in C99: the header must be valid C and the library usable without C++ or Python. */
+#include <stdio.h>
+#include <string.h>
+#include "ami.h"
+
+int main(void) {
+  /* order-2 self-energy (PAPER.md:207-231): R0 = three lines, alpha = (1,0,0), (0,1,0), (1,-1,1), external last */
+  const int32_t alpha[9] = {1, 0, 0, 0, 1, 0, 1, -1, 1};
+  const int32_t eps[9] = {1, 0, 0, 0, 1, 0, 0, 0, 1};
+  const uint8_t fermionic[3] = {1, 1, 1};
+  ami_table* tab = NULL;
+  ami_info info;
+  size_t bytes = 0;
+  int rc = ami_construct(2, 1, 3, 3, alpha, eps, fermionic, NULL, 1.0, -1, &tab);
+  if (rc != AMI_OK) { printf("construct: %s\n", ami_strerror(rc)); return 1; }
+  memset(&info, 0, sizeof info);
+  rc = ami_table_info(tab, &info);
+  if (rc != AMI_OK) return 2;
+  if (ami_table_latex(tab, NULL, &bytes) != AMI_OK || bytes == 0) return 3;
+  /* a table without a device copy refuses the kernels: no CPU fallback */
+  rc = ami_evaluate(tab, NULL, 0, 1, NULL, 0, NULL, 0, 0.0, AMI_PLAN_AUTO | AMI_PLAN_UNORDERED, NULL, NULL);
+  printf("version %d terms %lld U_F %d U_D %d has_device_copy %d evaluate_without_device %d max_rows %d\n", ami_version(),
+         (long long)info.n_terms, (int)info.n_fermi_leaves, (int)info.n_den_leaves, (int)info.has_device_copy, rc,
+         AMI_TALLY_STATIC_MAX_ROWS);
+  ami_table_destroy(tab);
+  return 0;
+}
+"""
+
+
+def test_header_is_c99_and_a_c_program_links(ami, tmp_path):
+    """include/ami.h through a C compiler in pedantic C99 mode, and a caller written in C linked against the
+    library (host-only table: runs without a GPU)."""
+    import subprocess
+    src = tmp_path / "caller.c"
+    src.write_text(C_CALLER)
+    exe = tmp_path / "caller"
+    lib_dir = os.path.dirname(ami.LIB_PATH)
+    subprocess.run(["gcc", "-std=c99", "-pedantic", "-Wall", "-Wextra", "-Werror", "-I", os.path.join(ROOT, "include"),
+                    str(src), "-o", str(exe), "-L", lib_dir, "-l:libami_b200.so", f"-Wl,-rpath,{lib_dir}"],
+                   check=True, capture_output=True, text=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout
+    m = re.match(r"version (\d+) terms (\d+) U_F (\d+) U_D (\d+) has_device_copy 0 evaluate_without_device (-?\d+) max_rows 1024", out)
+    assert m, out
+    tab = ami.AmiTable.from_diagram(A.self_energy_order2(), device=None)
+    assert int(m.group(2)) == tab.info["n_terms"] and int(m.group(3)) == tab.info["n_fermi_leaves"]
+    assert int(m.group(5)) == -4        # AMI_ECUDA: the table has no device copy
+
+
 def numpy_eval_export(tab, e, z, beta, prefactor=1.0):
     """Evaluates an exported flat table with numpy (test-side restatement of the layout documented
     in include/ami.h; real energies, derivative order <= 1)."""
