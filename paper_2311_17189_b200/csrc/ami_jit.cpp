@@ -1142,9 +1142,14 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
          "  const long long base = blockIdx.x * (long long)AMI_NT * (" << tiles << ") + threadIdx.x;\n"
          "  double4 t4 = make_double4(0.0, 0.0, 0.0, 0.0);\n"
          "#pragma unroll 1\n  for (int u = 0; u < (" << tiles << "); ++u) {\n"
-         "  const long long s = base + (long long)u * AMI_NT;\n"
-         "  if (s - (threadIdx.x & 31) >= p.n) break;\n"
-         "  const bool valid = s < p.n;\n";
+         "  const long long s = base + (long long)u * AMI_NT;\n";
+    // a warp past the end of the batch leaves; where the loop has one trip it EXITS there, so that the compiler keeps
+    // treating what follows as converged code (uniform datapath, no reconvergence stack: 40 instructions less).  It may
+    // skip the end-of-kernel wait of an unordered launch: the grid completes when its LAST thread has left, and the
+    // threads that hold a sample (there is at least one) wait
+    if (std::string(tiles) == "1") o << "  if (s - (threadIdx.x & 31) >= p.n) return;\n";
+    else o << "  if (s - (threadIdx.x & 31) >= p.n) break;\n";
+    o << "  const bool valid = s < p.n;\n";
     for (int c = 0; c < n_comp; ++c) o << "  double nk" << c << " = 0.0;\n";
     o << "  if (valid) {\n";
     emit_momenta(o, n_comp, "s", "    ");
@@ -1196,11 +1201,11 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
     o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_jit_eval(const __grid_constant__ AmiBatch p) {\n"
          "  asm volatile(\"griddepcontrol.launch_dependents;\");\n"
          "  if (!p.unordered) asm volatile(\"griddepcontrol.wait;\" ::: \"memory\");\n"
-         "  const long long stride = (long long)gridDim.x * AMI_NT;\n"
+         "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;   // the grid covers the batch\n"
+         "  if (s >= p.n) return;       // (an unordered launch: the threads that hold a sample wait at the end)\n"
          "  const bool valid = true;\n"
          "  double4 t4 = make_double4(0.0, 0.0, 0.0, 0.0);\n"
-         "#pragma unroll 1\n"
-         "  for (long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x; s < p.n; s += stride) {\n";
+         "  {\n";
     for (int i = 0; i < ft.n_eps; ++i) {
       if (var.cplx)
         o << "  const double e" << i << "r = p.e[2 * (" << i << " * p.e_stride + s)], e" << i << "i = p.e[2 * (" << i
@@ -1674,7 +1679,7 @@ cudaError_t jit_launch(const ami_table* tab, const JitVariant& var, bool fused, 
   if (m->layout.mode == kJitRegister) {
     // One CTA per `block` samples: the hardware CTA scheduler balances the SMs better than a persistent grid
     // with a static stride does (measured: persistent + L2 prefetch of the next sample was 12 % slower on cfg3
-    // and 5 % slower on cfg4, profiles/r01_final_kernels.md).  The unfused kernel keeps a grid-stride loop.
+    // and 5 % slower on cfg4, profiles/r01_final_kernels.md).
     AmiBatch copy = b;
     copy.tiles = 1;
     copy.tally_acc = 0;
