@@ -576,6 +576,8 @@ def run_ours(args, dist, rank, local, world):
     plan = PLAN_IDS[args.plan]
     dfma_per_s, _ = pkg.fp64_peak_probe(local, 2)       # the pipe's issue rate: the roofline's peak
     dfma3_per_s, _ = pkg.fp64_peak_probe(local, 3)      # DFMAs with three distinct register sources (context)
+    dfma4_per_s, _ = pkg.fp64_peak_probe(local, 4)      # three register sources that change from one DFMA to the next
+    dfma5_per_s, _ = pkg.fp64_peak_probe(local, 5)      # the same with one integer instruction per two DFMAs
     peaks = load_measured_peaks()
 
     res = time_workload(pkg, torch, cfg, n, args.steps, args.warmup, plan, first, dist, sample_clocks=True,
@@ -590,6 +592,12 @@ def run_ours(args, dist, rank, local, world):
     if res["ordered_ms"] is not None:      # the same kernel with every batch ordered after the one before
         roof["frac_ordered"] = roof["frac"] * res["eval_ms"] / res["ordered_ms"]
         roof["batches"] = "independent (AMI_PLAN_UNORDERED); frac_ordered: plain stream order"
+    # context for `frac`: what DFMA chains reach when every DFMA reads three register pairs that differ
+    # from its predecessor's (register-file bandwidth: one 64-bit operand per lane and cycle), without and with integer
+    # instructions beside them in the proportion of the specialised kernels
+    roof["register_file_context"] = {
+        "three_changing_sources_dfma_per_s": dfma4_per_s, "frac_of_peak": dfma4_per_s / dfma_per_s,
+        "with_integer_work_dfma_per_s": dfma5_per_s, "with_integer_work_frac_of_peak": dfma5_per_s / dfma_per_s}
     cap = ncu_capture(cfg.name, res["fused"]) if n == cfg.n_samples else None
     if cap:      # per launch, from profiles/ (ncu --set full of the same command, committed)
         roof["traffic"] = cap["dram_bytes"]

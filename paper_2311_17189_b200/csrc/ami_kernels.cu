@@ -666,15 +666,29 @@ cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long 
 //            Stops at 0.92 of the same figure although a and b are shared by all chains: a DFMA that reads
 //            three different register pairs does not issue every second cycle.  Reported beside the peak as
 //            the ceiling of register-operand arithmetic (bench.py: fp64_probe_three_source_dfma_per_s).
+//   SRC = 4: x_i = fma(x_i, y_j, z_k), y_j and z_k different from one DFMA to the next: three distinct register pairs
+//            and no operand the reuse cache could keep.  0.68: the register file hands out one 64-bit operand per lane
+//            and cycle, so this DFMA holds it for three cycles where the pipe needs two.
+//   SRC = 5: SRC = 4 plus one 32-bit integer instruction per two DFMAs (multiply-add, shift-xor), the proportion of
+//            the specialised kernels.  0.54: integer instructions read the same register file.
 // ------------------------------------------------------------------------------------------
 template <int SRC>
 __global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters, double a, double b) {
   double x0 = threadIdx.x * 1e-3, x1 = x0 + 0.1, x2 = x0 + 0.2, x3 = x0 + 0.3, x4 = x0 + 0.4, x5 = x0 + 0.5, x6 = x0 + 0.6,
          x7 = x0 + 0.7;
+  double y0 = a, y1 = a - 1e-7 * threadIdx.x, y2 = a - 2e-7 * threadIdx.x, y3 = a - 3e-7 * threadIdx.x;
+  double z0 = b, z1 = b * (1 + threadIdx.x), z2 = b * (2 + threadIdx.x), z3 = b * (3 + threadIdx.x);
+  unsigned k0 = threadIdx.x, k1 = blockIdx.x, k2 = 17, k3 = 29;
   for (int i = 0; i < iters; ++i) {
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
-      if (SRC == 3) {
+      if (SRC == 4 || SRC == 5) {
+        x0 = fma(x0, y0, z0); x1 = fma(x1, y1, z1); x2 = fma(x2, y2, z2); x3 = fma(x3, y3, z3);
+        x4 = fma(x4, y1, z2); x5 = fma(x5, y2, z3); x6 = fma(x6, y3, z0); x7 = fma(x7, y0, z1);
+        if (SRC == 5) {     // integer work beside the DFMAs in the proportion of the specialised kernels (1 : 2)
+          k0 = k0 * 0x9E3779B9u + (unsigned)j; k1 ^= k0 >> 7; k2 = k2 * 0x85EBCA6Bu + k1; k3 ^= k2 >> 11;
+        }
+      } else if (SRC == 3) {
         x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
         x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
       } else {
@@ -683,7 +697,8 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters,
       }
     }
   }
-  out[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  out[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7)) +
+                                                        (SRC == 5 ? (double)(k0 ^ k1 ^ k2 ^ k3) : 0.0);
 }
 
 cudaError_t run_fp64_probe(int distinct_sources, double* dfma_per_s, double* ms_out) {
@@ -703,7 +718,9 @@ cudaError_t run_fp64_probe(int distinct_sources, double* dfma_per_s, double* ms_
   float best = 1e30f;
   for (int rep = 0; rep < 6; ++rep) {
     cudaEventRecord(e0);
-    if (distinct_sources == 3) dfma_probe_kernel<3><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
+    if (distinct_sources == 5) dfma_probe_kernel<5><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
+    else if (distinct_sources == 4) dfma_probe_kernel<4><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
+    else if (distinct_sources == 3) dfma_probe_kernel<3><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
     else dfma_probe_kernel<2><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
     cudaEventRecord(e1);
     rc = cudaEventSynchronize(e1);

@@ -115,3 +115,21 @@ def test_register_plan_can_be_switched_off():
                          env=dict(os.environ, AMI_DISABLE_JIT="1"), timeout=120)
     assert out.returncode == 0, out.stderr
     assert out.stdout.strip() == "-6"
+
+
+def test_inspect_kernels_reports_register_operands():
+    """The inspection tool's operand classes (register-file ceiling) on the smallest table: every FP64
+    instruction is classified with 0-3 distinct register operands, most polynomial steps read two."""
+    import ami_inputs as A
+    import paper_2311_17189_b200 as pkg
+    from paper_2311_17189_b200 import inspect_kernels as ik
+    tab = pkg.AmiTable.from_diagram(A.get_config("cfg1").diagram, device=None)
+    cubin, _ = tab.kernel_cubin()
+    hist, classes = ik.histogram(cubin), ik.operand_classes(cubin)
+    assert set(hist) == set(classes) and "ami_jit_fused" in classes
+    c = classes["ami_jit_fused"]
+    n_fp = sum(c["fp64"].values())
+    assert n_fp == sum(hist["ami_jit_fused"][o] for o in ("DFMA", "DMUL", "DADD", "DSETP")) > 100
+    assert all(0 <= k[2] <= k[1] <= 3 for k in c["fp64"])
+    two = sum(v for k, v in c["fp64"].items() if k[1] <= 2)
+    assert two > 0.6 * n_fp and c["other"] > 0
