@@ -134,6 +134,10 @@ def fp64_work_per_sample(info, n_f, n_b, reg, tree=False):
         dens = n_f * int(info["fp64_ops_leaf_den"])     # complex reciprocals once per frequency, shared by all beta
         ft = int(info["fp64_ops_tree_fermi"])
         terms = n_b * ft + n_b * n_f * (int(info["fp64_ops_tree"]) - ft)
+        if n_b > 1 and int(info.get("plan_kind", 1)) == 1:
+            # several temperatures per launch (register plan): prefix products of the complex reciprocals once per
+            # frequency, then 2 instructions per (term of the sum, temperature) -- DESIGN.md 6.2
+            terms = n_b * ft + n_f * int(info["fp64_ops_mb_prefix"]) + n_b * n_f * int(info["fp64_ops_mb_sum"])
     elif tree:   # same Horner sums, interpreted; leaves per leaf and reciprocals per (beta, frequency) as in the flat plan
         ft = int(info["fp64_ops_tree_fermi"])
         terms = n_b * ft + n_b * n_f * (int(info["fp64_ops_tree"]) - ft)

@@ -126,6 +126,12 @@ typedef struct ami_info {
   int32_t specialize_cached; /* 1 if the loaded kernels came from the on-disk cache */
   double specialize_ms;     /* host time ami_table_specialize (or the first evaluation) spent generating, compiling
                                (or fetching) and loading the kernels; 0 until then */
+  /* register plan with several temperatures per launch: where it takes fewer instructions from two temperatures on,
+     the R part is evaluated as Q(root) + sum_n Q(n) P_n, P_n the product of the complex reciprocals on the way to trie
+     node n (once per frequency), Q(n) the per-temperature sums; otherwise in the Horner form of one temperature
+     (then fp64_ops_mb_prefix = 0 and fp64_ops_mb_sum = the R part of fp64_ops_tree) */
+  int64_t fp64_ops_mb_prefix; /* FP64 instructions per (sample,frequency) of the prefix products */
+  int64_t fp64_ops_mb_sum;    /* FP64 instructions per (sample,beta,frequency) of the sum */
 } ami_info;
 
 /* ---- Diagram files (Fig. 2; "Feature: Feynman Graph Representation") ----------

@@ -42,7 +42,8 @@ class ami_info(C.Structure):
                                          "fp64_ops_tree_fermi", "fp64_ops_leaf_fermi", "fp64_ops_leaf_den",
                                          "fp64_ops_dispersion", "fp64_ops_combos", "tree_plan_words", "tree_plan_slots")] + \
                [("has_device_copy", C.c_int32), ("reg_plan_status", C.c_int32), ("plan_kind", C.c_int32),
-                ("specialize_cached", C.c_int32), ("specialize_ms", C.c_double)]
+                ("specialize_cached", C.c_int32), ("specialize_ms", C.c_double), ("fp64_ops_mb_prefix", C.c_int64),
+                ("fp64_ops_mb_sum", C.c_int64)]
 
 
 class ami_run_cfg(C.Structure):

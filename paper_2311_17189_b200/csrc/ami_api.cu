@@ -258,6 +258,8 @@ int ami_table_info(const ami_table* tab, ami_info* info) {
   info->fp64_ops_leaf_den = tab->horner.ops_leaf_d;
   info->fp64_ops_dispersion = tab->horner.ops_disp;
   info->fp64_ops_combos = tab->horner.ops_combo;
+  info->fp64_ops_mb_prefix = tab->horner.mb_prefix ? tab->horner.ops_prefix : 0;
+  info->fp64_ops_mb_sum = tab->horner.mb_prefix ? tab->horner.ops_qsum : tab->horner.ops_d;
   info->tree_plan_words = tab->tree.ok ? (int64_t)(tab->tree.code_beta.size() + tab->tree.code_freq.size()) : -1;
   info->tree_plan_slots = tab->tree.n_slots;
   info->has_device_copy = tab->dev.device >= 0;

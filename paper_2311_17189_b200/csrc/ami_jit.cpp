@@ -35,6 +35,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <functional>
 #include <map>
 #include <mutex>
 #include <set>
@@ -525,6 +526,14 @@ enum LeafMode { kLeafInline, kLeafStore, kLeafLoad };
 struct Sections {
   std::ostringstream sec[4];
   std::vector<std::string> keep;   // per-beta values the R part reads (for the several-temperature body)
+  // several-temperature body, R part as a sum over prefix products: S_D(root) = Q(root) + sum_n Q(n) P_n with
+  // P_n = the product of the complex reciprocals on the way from the root to trie node n.  The P_n depend on the
+  // frequency only (secP: once per frequency, 4 instructions per node below the first level), the Q(n) on the
+  // temperature only (keep), so a (frequency, temperature) pair costs 2 instructions per node that carries a Q
+  // instead of the 2-4 per trie edge of the Horner form in sec[3].
+  std::ostringstream secP;
+  struct QRef { int keep; std::string pr, pi; };   // pr empty: the root's own Q (no product)
+  std::vector<QRef> qrefs;
 };
 
 struct LeafSlots {                 // layout of the split plan's leaf array
@@ -817,6 +826,38 @@ void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls
     o << "      AMI_EMIT(" << acc.re << ", " << (acc.real() ? std::string("0.0") : acc.im) << ");\n";
   }
 #undef o
+  // prefix products for the several-temperature body (register plan only)
+  if (mode == kLeafInline) {
+    auto keep_index = [&](const std::string& q) {
+      return (int)(std::find(S.keep.begin(), S.keep.end(), q) - S.keep.begin());
+    };
+    if (!qname[0].empty()) S.qrefs.push_back({keep_index(qname[0]), "", ""});
+    std::vector<Stmts> lists;
+    // P of a node on the first level is its reciprocal itself; below, (P.re + i P.im)(Dr + i Di): 4 instructions
+    std::function<void(int, const CV&)> below = [&](int n, const CV& P) {
+      if (!qname[n].empty()) S.qrefs.push_back({keep_index(qname[n]), P.re, P.im});
+      for (int c : hp.dn[n].kids) {
+        const int u = hp.dn[c].leaf;
+        if (hp.d_is_real[u]) continue;
+        const std::string dr = "Dr" + std::to_string(u), di = "Di" + std::to_string(u);
+        const CV Pc{E.fresh("P"), E.fresh("P")};
+        const std::string t0 = E.fresh("P"), t1 = E.fresh("P");
+        Stmts& out = lists.back();
+        out.push_back("const double " + t0 + " = -" + P.im + " * " + di + ";");
+        out.push_back("const double " + t1 + " = " + P.re + " * " + di + ";");
+        out.push_back("const double " + Pc.re + " = fma(" + P.re + ", " + dr + ", " + t0 + ");");
+        out.push_back("const double " + Pc.im + " = fma(" + P.im + ", " + dr + ", " + t1 + ");");
+        below(c, Pc);
+      }
+    };
+    for (int c : hp.dn[0].kids) {
+      const int u = hp.dn[c].leaf;
+      if (hp.d_is_real[u]) continue;
+      lists.emplace_back();
+      below(c, CV{"Dr" + std::to_string(u), "Di" + std::to_string(u)});
+    }
+    interleave(lists, kWays, S.secP, "      ");
+  }
 }
 
 // The four sections of the body for complex energies e<i>r + i e<i>i (register plan only).
@@ -1181,14 +1222,77 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
       << "#pragma unroll 1\n    for (int f = 0; f < p.n_f; ++f) {\n" << S.sec[2].str() << S.sec[3].str() << "    }\n  }\n}\n\n";
     // ---- body for several temperatures: the per-beta values the R part needs are kept in a small
     // per-thread array, then frequency { reciprocals once; beta { R part } } --------------------------
+    // R part: per frequency the prefix products P_n of the complex reciprocals (secP), then per temperature
+    // Q(root) + sum_n Q(n) P_n: two instructions per term, W temperatures side by side so that consecutive DFMAs share
+    // the P_n operand (a DFMA with three changing register operands runs at 2/3 of the rate) and each
+    // temperature's sum is a chain of its own.
+    if (var.cplx || !hp.mb_prefix) {   // the Horner form of the single-temperature body (complex energies: the Q(n) are
+                                       // complex too; small R parts: the prefix products would cost more than they save)
+      o << "template <bool AMI_TALLY> __device__ __forceinline__ void ami_body_mb" << sig << S.sec[0].str();
+      o << "  double kept[AMI_K_MAX_BETA][" << std::max<size_t>(S.keep.size(), 1) << "];\n";
+      o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << S.sec[1].str();
+      for (size_t i = 0; i < S.keep.size(); ++i) o << "    kept[b][" << i << "] = " << S.keep[i] << ";\n";
+      o << "  }\n#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n" << S.sec[2].str()
+        << "#pragma unroll 1\n    for (int b = 0; b < p.n_b; ++b) {\n";
+      for (size_t i = 0; i < S.keep.size(); ++i) o << "      const double " << S.keep[i] << " = kept[b][" << i << "];\n";
+      o << S.sec[3].str() << "    }\n  }\n}\n\n";
+    } else {
     o << "template <bool AMI_TALLY> __device__ __forceinline__ void ami_body_mb" << sig << S.sec[0].str();
-    o << "  double kept[AMI_K_MAX_BETA][" << std::max<size_t>(S.keep.size(), 1) << "];\n";
+    o << "  double kept[" << std::max<size_t>(S.keep.size(), 1) << "][AMI_K_MAX_BETA];\n";
     o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << S.sec[1].str();
-    for (size_t i = 0; i < S.keep.size(); ++i) o << "    kept[b][" << i << "] = " << S.keep[i] << ";\n";
-    o << "  }\n#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n" << S.sec[2].str()
-      << "#pragma unroll 1\n    for (int b = 0; b < p.n_b; ++b) {\n";
-    for (size_t i = 0; i < S.keep.size(); ++i) o << "      const double " << S.keep[i] << " = kept[b][" << i << "];\n";
-    o << S.sec[3].str() << "    }\n  }\n}\n\n";
+    for (size_t i = 0; i < S.keep.size(); ++i) o << "    kept[" << i << "][b] = " << S.keep[i] << ";\n";
+    o << "  }\n#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n" << S.sec[2].str() << S.secP.str();
+    auto block = [&](int W) {
+      const int A = std::max(1, 4 / W);       // partial sums per temperature: at least 8 chains in flight
+      std::ostringstream q;
+      q << "      {\n";
+      for (int w = 0; w < W; ++w)
+        for (const Sections::QRef& r : S.qrefs)
+          q << "        const double k" << w << "_" << r.keep << " = kept[" << r.keep << "][b0 + " << w << "];\n";
+      std::vector<std::vector<char>> init(W, std::vector<char>(A, 0));
+      for (int w = 0; w < W; ++w)
+        for (int a = 0; a < A; ++a) q << "        double vr" << w << "_" << a << ", vi" << w << "_" << a << ";\n";
+      int j = 0;
+      for (const Sections::QRef& r : S.qrefs) {
+        if (r.pr.empty()) continue;
+        const int a = j++ % A;
+        for (int w = 0; w < W; ++w) {
+          const std::string k = "k" + std::to_string(w) + "_" + std::to_string(r.keep);
+          const std::string vr = "vr" + std::to_string(w) + "_" + std::to_string(a), vi = "vi" + std::to_string(w) + "_" + std::to_string(a);
+          if (!init[w][a]) {
+            q << "        " << vr << " = " << k << " * " << r.pr << "; " << vi << " = " << k << " * " << r.pi << ";\n";
+            init[w][a] = 1;
+          } else {
+            q << "        " << vr << " = fma(" << k << ", " << r.pr << ", " << vr << "); " << vi << " = fma(" << k << ", " << r.pi
+              << ", " << vi << ");\n";
+          }
+        }
+      }
+      for (int w = 0; w < W; ++w) {
+        std::string re, im;
+        for (int a = 0; a < A; ++a) {
+          if (!init[w][a]) continue;
+          re += (re.empty() ? "" : " + ") + std::string("vr") + std::to_string(w) + "_" + std::to_string(a);
+          im += (im.empty() ? "" : " + ") + std::string("vi") + std::to_string(w) + "_" + std::to_string(a);
+        }
+        if (A == 4 && init[0][3]) {   // pairwise
+          re = "(vr" + std::to_string(w) + "_0 + vr" + std::to_string(w) + "_1) + (vr" + std::to_string(w) + "_2 + vr" + std::to_string(w) + "_3)";
+          im = "(vi" + std::to_string(w) + "_0 + vi" + std::to_string(w) + "_1) + (vi" + std::to_string(w) + "_2 + vi" + std::to_string(w) + "_3)";
+        }
+        for (const Sections::QRef& r : S.qrefs)
+          if (r.pr.empty()) re = re.empty() ? "k" + std::to_string(w) + "_" + std::to_string(r.keep)
+                                            : "(" + re + ") + k" + std::to_string(w) + "_" + std::to_string(r.keep);
+        if (re.empty()) re = "0.0";
+        if (im.empty()) im = "0.0";
+        q << "        { const int b = b0 + " << w << "; AMI_EMIT(" << re << ", " << im << "); }\n";
+      }
+      q << "      }\n";
+      return q.str();
+    };
+    o << "    int b0 = 0;\n#pragma unroll 1\n    for (; b0 + 4 <= p.n_b; b0 += 4)\n" << block(4)
+      << "    if (b0 + 2 <= p.n_b) {\n" << block(2) << "      b0 += 2;\n    }\n"
+      << "    if (b0 < p.n_b)\n" << block(1) << "  }\n}\n\n";
+    }
     const std::string call_args = "(p, s, valid, t4" + eargs + ");\n";
     // @T@ = <false> / <true>: without / with the fused tally (a compile-time switch: the reductions cost the kernels
     // that do not tally nothing)

@@ -248,6 +248,27 @@ void build_horner_plan(const FlatTable& ft, HornerPlan& hp) {
   hp.dseq = dseq;
   hp.n_dnodes = (long long)hp.dn.size() - 1;
   count_d_ops(hp, 0, &hp.ops_d_beta, &hp.ops_d);
+  {   // the same R part as a sum over prefix products (several temperatures per launch)
+    auto has_q = [&](int n) {
+      if (hp.dn[n].group >= 0) return true;
+      for (int c : hp.dn[n].kids)
+        if (hp.d_is_real[hp.dn[c].leaf]) return true;
+      return false;
+    };
+    if (has_q(0)) hp.ops_qsum += 1;
+    std::vector<std::pair<int, int>> stack;   // (node, depth among the complex denominators)
+    for (int c : hp.dn[0].kids)
+      if (!hp.d_is_real[hp.dn[c].leaf]) stack.emplace_back(c, 1);
+    while (!stack.empty()) {
+      const auto [n, depth] = stack.back();
+      stack.pop_back();
+      if (depth >= 2) hp.ops_prefix += 4;
+      if (has_q(n)) hp.ops_qsum += 2;
+      for (int c : hp.dn[n].kids)
+        if (!hp.d_is_real[hp.dn[c].leaf]) stack.emplace_back(c, depth + 1);
+    }
+    hp.mb_prefix = hp.ops_prefix + 2 * hp.ops_qsum <= 2 * hp.ops_d;   // fewer instructions at n_b = 2 already
+  }
   // leaf costs on the common path of the routines in ami_device.cuh
   const int kExpCore = 15;   // magic fma, subtract, 2 reduction fma, 10 polynomial fma, final fma
   const int kNewton = 3, kCos = 15;   // one third-order reciprocal step = 3 fma

@@ -82,6 +82,10 @@ struct HornerPlan {
   long long ops_f = 0;       // FP64 instructions per (sample, beta) of all FT sums
   long long ops_d = 0;       // FP64 instructions per (sample, beta, frequency) of the R part
   long long ops_d_beta = 0;  // R-part products under purely real denominators: per (sample, beta) only
+  // several-temperature body of the register plan (ami_jit.cpp): R part as Q(root) + sum_n Q(n) P_n
+  long long ops_prefix = 0;  // per (sample, frequency): the prefix products P_n, 4 per complex trie node below the first level
+  long long ops_qsum = 0;    // per (sample, beta, frequency): 2 per complex trie node that carries a Q, 1 for the root's
+  bool mb_prefix = false;    // that form is what the several-temperature body uses: it is the cheaper one from two temperatures on
   long long ops_leaf_f = 0;  // FP64 instructions per (sample, beta) of the Fermi/Bose leaves
   long long ops_leaf_d = 0;  // FP64 instructions per (sample, beta, frequency) of the reciprocals
   long long ops_disp = 0;    // FP64 instructions per sample of the dispersion
