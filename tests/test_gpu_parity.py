@@ -324,8 +324,35 @@ def test_grid_larger_than_one_launch(ami, torch_mod, oracle_mod, plan, fused):
         check_parity(out[b][:, sel], truth, S, label=f"split grid beta#{b}")
     # rows computed alone equal the rows of the split call, bit for bit
     one = tab.evaluate(e, z[64:], [betas[8]], plan=PLANS[plan]).cpu().numpy()
-    # (the register plan's several-temperature body keeps per-beta values in memory: same arithmetic, same bits)
+    # (both are launches of ONE temperature, hence the same body of the register plan: same arithmetic, same bits;
+    # a row computed among several temperatures may differ from them in rounding)
     assert np.array_equal(one[0], out[8, 64:])
+
+
+@pytest.mark.parametrize("n_b", [2, 3, 5, 6, 7, 8])
+@pytest.mark.parametrize("name", ["cfg5", "cfg1", "cfg4"])
+def test_several_temperatures_per_launch(ami, torch_mod, oracle_mod, name, n_b):
+    """The several-temperature body of the register plan for every way n_b splits into blocks of four, two and one
+    temperatures (cfg5 and cfg1 take the prefix-product form of the R part, cfg4 keeps the Horner
+    form): every (temperature, frequency) row against the oracle, and against the same temperature evaluated alone
+    (another summation order: equal to rounding on the scale S of the sample, not bit for bit)."""
+    cfg = A.get_config(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    assert tab.specialize()["plan_kind"] == 1
+    n = 257
+    betas = [1.5, 2.0, 3.0, 5.0, 7.0, 10.0, 14.0, 20.0][:n_b]
+    z = (np.array([-2.5, -0.3, 0.9, 3.1, 0.0]) + np.array([0.1, 0.1, 0.2, 0.05, math.pi / 5.0]) * 1j).reshape(5, 1)
+    k_host = cfg.momenta(n)
+    k = torch_mod.from_numpy(k_host).cuda()
+    e = tab.dispersion(k, [cfg.q], cfg.t, cfg.mu)
+    out = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, z, betas, e_reg=cfg.e_reg).cpu().numpy()
+    assert out.shape == (n_b, 5, n)
+    e_rows = e.cpu().numpy().T.copy()
+    for b, beta in enumerate(betas):
+        truth, S = truth_for(oracle_mod, cfg, e_rows, z, beta, cfg.e_reg)
+        check_parity(out[b], truth, S, label=f"{name} n_b={n_b} beta#{b}")
+        alone = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, z, [beta], e_reg=cfg.e_reg).cpu().numpy()[0]
+        assert np.all(np.abs(alone - out[b]) <= 1e-12 * S + 1e-280), f"{name} n_b={n_b} beta#{b} against the row computed alone"
 
 
 @pytest.mark.parametrize("plan", list(PLANS))
