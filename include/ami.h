@@ -247,6 +247,8 @@ int ami_table_export(const ami_table* tab, void* host_buf, size_t* bytes);
  * flag << 28 | a << 16 | b; DESIGN.md (6.3) says what a node computes. */
 int ami_table_export_tree(const ami_table* tab, void* host_buf, size_t* bytes);
 
+/* Frees the table, its device copy, its specialised kernels and the workspace of ami_run.  Waits for the work
+ * outstanding on the table's device first (kernel entry points are asynchronous); NULL is accepted. */
 void ami_table_destroy(ami_table* tab);
 
 /* ami_dispersion -- Eqs. 8-18 for the 2D square lattice:

@@ -229,6 +229,8 @@ int ami_search_sum_order(int n_int, int n_ext, int n_g, int n_eps, const int32_t
 
 void ami_table_destroy(ami_table* tab) {
   if (!tab) return;
+  if (tab->dev.device >= 0 && cudaSetDevice(tab->dev.device) == cudaSuccess)
+    cudaDeviceSynchronize();   // kernels of this table may still run (launches are asynchronous): wait before unloading them
   ami::jit_destroy(tab);
   free_run_workspace(tab);
   free_device_copy(tab->dev);
