@@ -733,7 +733,8 @@ def time_paper_example1(pkg, torch, cfg, steps, warmup, plan, peaks, dfma_per_s)
             "hbm_frac": bytes_alg / (ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "algorithmic_bytes": bytes_alg}
 
 
-SWEEP = (("cfg2_se", 8), ("cfg2_bubble", 8), ("cfg3", 7), ("cfg4", 7))   # workload, largest power of ten
+SWEEP = (("cfg2_se", 8), ("cfg2_bubble", 8), ("cfg3", 7), ("cfg4", 7), ("stress8", 6))   # workload, largest power of ten
+# (orders 2, 4, 6: register plan; stress8 = order 8, T = 40244: split plan)
 
 
 def run_sweep(args, local):
