@@ -582,6 +582,8 @@ def run_ours(args, dist, rank, local, world):
     dfma3_per_s, _ = pkg.fp64_peak_probe(local, 3)      # DFMAs with three distinct register sources (context)
     dfma4_per_s, _ = pkg.fp64_peak_probe(local, 4)      # three register sources that change from one DFMA to the next
     dfma5_per_s, _ = pkg.fp64_peak_probe(local, 5)      # the same with one integer instruction per two DFMAs
+    dfma6_per_s, _ = pkg.fp64_peak_probe(local, 6)      # two changing register sources and an immediate
+    dfma7_per_s, _ = pkg.fp64_peak_probe(local, 7)      # the same with that integer work
     peaks = load_measured_peaks()
 
     res = time_workload(pkg, torch, cfg, n, args.steps, args.warmup, plan, first, dist, sample_clocks=True,
@@ -601,7 +603,9 @@ def run_ours(args, dist, rank, local, world):
     # instructions beside them in the proportion of the specialised kernels
     roof["register_file_context"] = {
         "three_changing_sources_dfma_per_s": dfma4_per_s, "frac_of_peak": dfma4_per_s / dfma_per_s,
-        "with_integer_work_dfma_per_s": dfma5_per_s, "with_integer_work_frac_of_peak": dfma5_per_s / dfma_per_s}
+        "with_integer_work_dfma_per_s": dfma5_per_s, "with_integer_work_frac_of_peak": dfma5_per_s / dfma_per_s,
+        "two_changing_sources_frac_of_peak": dfma6_per_s / dfma_per_s,
+        "two_changing_sources_with_integer_work_frac_of_peak": dfma7_per_s / dfma_per_s}
     cap = ncu_capture(cfg.name, res["fused"]) if n == cfg.n_samples else None
     if cap:      # per launch, from profiles/ (ncu --set full of the same command, committed)
         roof["traffic"] = cap["dram_bytes"]

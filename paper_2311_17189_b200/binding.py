@@ -423,7 +423,8 @@ def kernel_launches() -> int:
 def fp64_peak_probe(device=0, distinct_sources=2):
     """Measured DFMA lane-operations per second of ``device`` (register-only chains): 2 = two distinct register
     sources per DFMA (the pipe's issue rate), 3 = three of which two repeat (operand reuse), 4 = three that change
-    from one DFMA to the next (register-file bandwidth), 5 = 4 with integer instructions in between (include/ami.h)."""
+    from one DFMA to the next (register-file bandwidth), 5 = 4 with integer instructions in between, 6 / 7 = two changing
+    register operands and an immediate addend without / with that integer work (include/ami.h)."""
     r, ms = C.c_double(0), C.c_double(0)
     _check(lib().ami_fp64_peak_probe(int(device), int(distinct_sources), C.byref(r), C.byref(ms)))
     return r.value, ms.value

@@ -702,7 +702,7 @@ int ami_generate_momenta(const ami_table* tab, uint64_t seed, int64_t first_samp
 }
 
 int ami_fp64_peak_probe(int device, int distinct_sources, double* dfma_per_s, double* elapsed_ms) {
-  if (!dfma_per_s || !elapsed_ms || device < 0 || distinct_sources < 2 || distinct_sources > 5) return AMI_EINVAL;
+  if (!dfma_per_s || !elapsed_ms || device < 0 || distinct_sources < 2 || distinct_sources > 7) return AMI_EINVAL;
   CU(cudaSetDevice(device));
   CU(ami::run_fp64_probe(distinct_sources, dfma_per_s, elapsed_ms));
   return AMI_OK;

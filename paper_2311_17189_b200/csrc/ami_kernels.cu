@@ -670,7 +670,9 @@ cudaError_t launch_block_sums(const double* d_vals, long long n_rows, long long 
 //            and no operand the reuse cache could keep.  0.68: the register file hands out one 64-bit operand per lane
 //            and cycle, so this DFMA holds it for three cycles where the pipe needs two.
 //   SRC = 5: SRC = 4 plus one 32-bit integer instruction per two DFMAs (multiply-add, shift-xor), the proportion of
-//            the specialised kernels.  0.54: integer instructions read the same register file.
+//            the specialised kernels.  0.54-0.60: integer instructions read the same register file.
+//   SRC = 6, 7: x_i = fma(x_i, y_j, immediate): two changing register operands; without / with that integer work:
+//            0.94 / 0.66.
 // ------------------------------------------------------------------------------------------
 template <int SRC>
 __global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters, double a, double b) {
@@ -682,7 +684,13 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters,
   for (int i = 0; i < iters; ++i) {
 #pragma unroll
     for (int j = 0; j < 8; ++j) {
-      if (SRC == 4 || SRC == 5) {
+      if (SRC == 6 || SRC == 7) {   // two changing register operands and an immediate addend
+        x0 = fma(x0, y0, 1e-9); x1 = fma(x1, y1, 1e-9); x2 = fma(x2, y2, 1e-9); x3 = fma(x3, y3, 1e-9);
+        x4 = fma(x4, y1, 1e-9); x5 = fma(x5, y2, 1e-9); x6 = fma(x6, y3, 1e-9); x7 = fma(x7, y0, 1e-9);
+        if (SRC == 7) {
+          k0 = k0 * 0x9E3779B9u + (unsigned)j; k1 ^= k0 >> 7; k2 = k2 * 0x85EBCA6Bu + k1; k3 ^= k2 >> 11;
+        }
+      } else if (SRC == 4 || SRC == 5) {
         x0 = fma(x0, y0, z0); x1 = fma(x1, y1, z1); x2 = fma(x2, y2, z2); x3 = fma(x3, y3, z3);
         x4 = fma(x4, y1, z2); x5 = fma(x5, y2, z3); x6 = fma(x6, y3, z0); x7 = fma(x7, y0, z1);
         if (SRC == 5) {     // integer work beside the DFMAs in the proportion of the specialised kernels (1 : 2)
@@ -698,7 +706,8 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double* out, int iters,
     }
   }
   out[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7)) +
-                                                        (SRC == 5 ? (double)(k0 ^ k1 ^ k2 ^ k3) : 0.0);
+                                                        ((SRC == 5 || SRC == 7) ? (double)(k0 ^ k1 ^ k2 ^ k3) : 0.0) +
+                                                        (SRC >= 4 ? (z0 + z1) + (z2 + z3) : 0.0);
 }
 
 cudaError_t run_fp64_probe(int distinct_sources, double* dfma_per_s, double* ms_out) {
@@ -718,7 +727,9 @@ cudaError_t run_fp64_probe(int distinct_sources, double* dfma_per_s, double* ms_
   float best = 1e30f;
   for (int rep = 0; rep < 6; ++rep) {
     cudaEventRecord(e0);
-    if (distinct_sources == 5) dfma_probe_kernel<5><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
+    if (distinct_sources == 7) dfma_probe_kernel<7><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
+    else if (distinct_sources == 6) dfma_probe_kernel<6><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
+    else if (distinct_sources == 5) dfma_probe_kernel<5><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
     else if (distinct_sources == 4) dfma_probe_kernel<4><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
     else if (distinct_sources == 3) dfma_probe_kernel<3><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
     else dfma_probe_kernel<2><<<blocks, nt>>>(d, iters, 0.999999, 1e-9);
