@@ -532,7 +532,7 @@ struct Sections {
   // temperature only (keep), so a (frequency, temperature) pair costs 2 instructions per node that carries a Q
   // instead of the 2-4 per trie edge of the Horner form in sec[3].
   std::ostringstream secP;
-  struct QRef { int keep; std::string pr, pi; };   // pr empty: the root's own Q (no product)
+  struct QRef { int keep, keep_im; std::string pr, pi; };   // keep_im < 0: Q is real; pr empty: the root's own Q (no product)
   std::vector<QRef> qrefs;
 };
 
@@ -551,6 +551,42 @@ LeafSlots leaf_slots(const FlatTable& ft, const HornerPlan& hp) {
   }
   ls.n_fermi = (int)ft.leafF.size();
   return ls;
+}
+
+// The R part as Q(root) + sum_n Q(n) P_n (several-temperature body of the register plan; see Sections): the
+// statements that form the prefix products P_n (S.secP) and, in depth-first order, which kept value meets which P_n
+// (S.qrefs).  q[n] names Q(n) (re empty: there is none; im empty: it is real).
+void build_prefix_form(const HornerPlan& hp, const std::vector<CV>& q, Emitter& E, Sections& S) {
+  auto keep_index = [&](const std::string& name) {
+    if (name.empty() || name == "0.0") return -1;
+    return (int)(std::find(S.keep.begin(), S.keep.end(), name) - S.keep.begin());
+  };
+  if (!q[0].re.empty()) S.qrefs.push_back({keep_index(q[0].re), keep_index(q[0].im), "", ""});
+  std::vector<Stmts> lists;
+  // P of a node on the first level is its reciprocal itself; below, (P.re + i P.im)(Dr + i Di): 4 instructions
+  std::function<void(int, const CV&)> below = [&](int n, const CV& P) {
+    if (!q[n].re.empty()) S.qrefs.push_back({keep_index(q[n].re), keep_index(q[n].im), P.re, P.im});
+    for (int c : hp.dn[n].kids) {
+      const int u = hp.dn[c].leaf;
+      if (hp.d_is_real[u]) continue;
+      const std::string dr = "Dr" + std::to_string(u), di = "Di" + std::to_string(u);
+      const CV Pc{E.fresh("P"), E.fresh("P")};
+      const std::string t0 = E.fresh("P"), t1 = E.fresh("P");
+      Stmts& out = lists.back();
+      out.push_back("const double " + t0 + " = -" + P.im + " * " + di + ";");
+      out.push_back("const double " + t1 + " = " + P.re + " * " + di + ";");
+      out.push_back("const double " + Pc.re + " = fma(" + P.re + ", " + dr + ", " + t0 + ");");
+      out.push_back("const double " + Pc.im + " = fma(" + P.im + ", " + dr + ", " + t1 + ");");
+      below(c, Pc);
+    }
+  };
+  for (int c : hp.dn[0].kids) {
+    const int u = hp.dn[c].leaf;
+    if (hp.d_is_real[u]) continue;
+    lists.emplace_back();
+    below(c, CV{"Dr" + std::to_string(u), "Di" + std::to_string(u)});
+  }
+  interleave(lists, kWays, S.secP, "      ");
 }
 
 // `hp` may be the plan of one part; leaf ids and `ls` are those of the whole table
@@ -826,37 +862,10 @@ void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls
     o << "      AMI_EMIT(" << acc.re << ", " << (acc.real() ? std::string("0.0") : acc.im) << ");\n";
   }
 #undef o
-  // prefix products for the several-temperature body (register plan only)
   if (mode == kLeafInline) {
-    auto keep_index = [&](const std::string& q) {
-      return (int)(std::find(S.keep.begin(), S.keep.end(), q) - S.keep.begin());
-    };
-    if (!qname[0].empty()) S.qrefs.push_back({keep_index(qname[0]), "", ""});
-    std::vector<Stmts> lists;
-    // P of a node on the first level is its reciprocal itself; below, (P.re + i P.im)(Dr + i Di): 4 instructions
-    std::function<void(int, const CV&)> below = [&](int n, const CV& P) {
-      if (!qname[n].empty()) S.qrefs.push_back({keep_index(qname[n]), P.re, P.im});
-      for (int c : hp.dn[n].kids) {
-        const int u = hp.dn[c].leaf;
-        if (hp.d_is_real[u]) continue;
-        const std::string dr = "Dr" + std::to_string(u), di = "Di" + std::to_string(u);
-        const CV Pc{E.fresh("P"), E.fresh("P")};
-        const std::string t0 = E.fresh("P"), t1 = E.fresh("P");
-        Stmts& out = lists.back();
-        out.push_back("const double " + t0 + " = -" + P.im + " * " + di + ";");
-        out.push_back("const double " + t1 + " = " + P.re + " * " + di + ";");
-        out.push_back("const double " + Pc.re + " = fma(" + P.re + ", " + dr + ", " + t0 + ");");
-        out.push_back("const double " + Pc.im + " = fma(" + P.im + ", " + dr + ", " + t1 + ");");
-        below(c, Pc);
-      }
-    };
-    for (int c : hp.dn[0].kids) {
-      const int u = hp.dn[c].leaf;
-      if (hp.d_is_real[u]) continue;
-      lists.emplace_back();
-      below(c, CV{"Dr" + std::to_string(u), "Di" + std::to_string(u)});
-    }
-    interleave(lists, kWays, S.secP, "      ");
+    std::vector<CV> q(hp.dn.size());
+    for (size_t n = 0; n < hp.dn.size(); ++n) q[n].re = qname[n];
+    build_prefix_form(hp, q, E, S);
   }
 }
 
@@ -949,21 +958,20 @@ void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, Emitter& E, Se
     const CV B = product(-1);
     if (l.sigma < 0) A = emit_cv_fma(CV{"p.ceta[b]", ""}, A, nullptr, E, st);      // e^{beta eta} (P10(a))
     for (const std::string& s : st) o << "      " << s << "\n";
+    // d = sigma 2^N A + B is formed as d' = A' + B' with A' = sigma 2^min(N,0) A and B' = 2^-max(N,0) B, i.e. divided by
+    // 2^N when that is large: |d'| stays of order one, so |d'|^2 cannot overflow for any beta (P12), and
+    // f = B' conj(d') / |d'|^2,  g = 1 - f = A' conj(d') / |d'|^2  hold in both cases.
     const std::string sg = l.sigma > 0 ? "" : "-";
-    o << "      const double sc = pow2_clamped(0" << ex << ");\n";
-    o << "      const double dr = fma(sc, " << sg << A.re << ", " << B.re << "), di = "
-      << (A.real() ? std::string("0.0") : "sc * " + sg + A.im) << (B.real() ? "" : " + " + B.im) << ";\n";
-    o << "      const double rn = fast_rcp(fma(dr, dr, di * di));\n";
-    // f = B conj(d) / |d|^2,  g = sigma sc A conj(d) / |d|^2
-    if (B.real()) o << "      const double fr = dr * rn, fi = -di * rn;\n";
-    else o << "      const double fr = fma(" << B.re << ", dr, " << B.im << " * di) * rn, fi = fma(" << B.im << ", dr, -" << B.re << " * di) * rn;\n";
+    o << "      const int N = 0" << ex << ";\n"
+      << "      const double s1 = pow2_clamped(min(N, 0)), s2 = pow2_clamped(-max(N, 0));\n"
+      << "      const double ar = s1 * " << sg << A.re << ", ai = " << (A.real() ? std::string("0.0") : "s1 * " + sg + A.im) << ";\n"
+      << "      const double br = s2 * " << B.re << ", bi = " << (B.real() ? std::string("0.0") : "s2 * " + B.im) << ";\n"
+      << "      const double dr = ar + br, di = ai + bi;\n"
+      << "      const double rn = fast_rcp(fma(dr, dr, di * di));\n"
+      << "      const double fr = fma(br, dr, bi * di) * rn, fi = fma(bi, dr, -br * di) * rn;\n";
     bool need_g = false;
     for (size_t u : members) need_g |= ft.leafF[u].k > 0;
-    if (need_g) {
-      const std::string ai = A.real() ? "0.0" : A.im;
-      o << "      const double gr = " << sg << "sc * fma(" << A.re << ", dr, " << ai << " * di) * rn, gi = " << sg << "sc * fma(" << ai
-        << ", dr, -" << A.re << " * di) * rn;\n";
-    }
+    if (need_g) o << "      const double gr = fma(ar, dr, ai * di) * rn, gi = fma(ai, dr, -ar * di) * rn;\n";
     for (size_t u : members) {
       const int k = ft.leafF[u].k;
       if (k == 0) { o << "      Fr" << u << " = fr; Fi" << u << " = fi;\n"; continue; }
@@ -1032,6 +1040,12 @@ void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, Emitter& E, Se
     o << "      AMI_EMIT(" << acc.re << ", " << (acc.real() ? std::string("0.0") : acc.im) << ");\n";
   }
 #undef o
+  {
+    std::vector<CV> qq(hp.dn.size());
+    for (size_t n = 0; n < hp.dn.size(); ++n)
+      if (q_have[n]) qq[n] = q[n];
+    build_prefix_form(hp, qq, E, S);
+  }
 }
 
 // Momenta of sample `at` into nk0..: from memory, or drawn in place by the counter-based generator (S4 with a
@@ -1226,8 +1240,8 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
     // Q(root) + sum_n Q(n) P_n: two instructions per term, W temperatures side by side so that consecutive DFMAs share
     // the P_n operand (a DFMA with three changing register operands runs at 2/3 of the rate) and each
     // temperature's sum is a chain of its own.
-    if (var.cplx || !hp.mb_prefix) {   // the Horner form of the single-temperature body (complex energies: the Q(n) are
-                                       // complex too; small R parts: the prefix products would cost more than they save)
+    if (!hp.mb_prefix) {   // the Horner form of the single-temperature body (small R parts: the prefix products would
+                           // cost more than they save)
       o << "template <bool AMI_TALLY> __device__ __forceinline__ void ami_body_mb" << sig << S.sec[0].str();
       o << "  double kept[AMI_K_MAX_BETA][" << std::max<size_t>(S.keep.size(), 1) << "];\n";
       o << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n" << S.sec[1].str();
@@ -1246,9 +1260,14 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
       const int A = std::max(1, 4 / W);       // partial sums per temperature: at least 8 chains in flight
       std::ostringstream q;
       q << "      {\n";
-      for (int w = 0; w < W; ++w)
+      auto kname = [](int w, int keep) { return "k" + std::to_string(w) + "_" + std::to_string(keep); };
+      for (int w = 0; w < W; ++w) {
+        std::set<int> loaded;
         for (const Sections::QRef& r : S.qrefs)
-          q << "        const double k" << w << "_" << r.keep << " = kept[" << r.keep << "][b0 + " << w << "];\n";
+          for (int keep : {r.keep, r.keep_im})
+            if (keep >= 0 && loaded.insert(keep).second)
+              q << "        const double " << kname(w, keep) << " = kept[" << keep << "][b0 + " << w << "];\n";
+      }
       std::vector<std::vector<char>> init(W, std::vector<char>(A, 0));
       for (int w = 0; w < W; ++w)
         for (int a = 0; a < A; ++a) q << "        double vr" << w << "_" << a << ", vi" << w << "_" << a << ";\n";
@@ -1257,15 +1276,18 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
         if (r.pr.empty()) continue;
         const int a = j++ % A;
         for (int w = 0; w < W; ++w) {
-          const std::string k = "k" + std::to_string(w) + "_" + std::to_string(r.keep);
+          const std::string kr = kname(w, r.keep), ki = r.keep_im >= 0 ? kname(w, r.keep_im) : "";
           const std::string vr = "vr" + std::to_string(w) + "_" + std::to_string(a), vi = "vi" + std::to_string(w) + "_" + std::to_string(a);
           if (!init[w][a]) {
-            q << "        " << vr << " = " << k << " * " << r.pr << "; " << vi << " = " << k << " * " << r.pi << ";\n";
+            q << "        " << vr << " = " << kr << " * " << r.pr << "; " << vi << " = " << kr << " * " << r.pi << ";\n";
             init[w][a] = 1;
           } else {
-            q << "        " << vr << " = fma(" << k << ", " << r.pr << ", " << vr << "); " << vi << " = fma(" << k << ", " << r.pi
+            q << "        " << vr << " = fma(" << kr << ", " << r.pr << ", " << vr << "); " << vi << " = fma(" << kr << ", " << r.pi
               << ", " << vi << ");\n";
           }
+          if (!ki.empty())   // complex Q: (kr + i ki)(Pr + i Pi)
+            q << "        " << vr << " = fma(-" << ki << ", " << r.pi << ", " << vr << "); " << vi << " = fma(" << ki << ", " << r.pr
+              << ", " << vi << ");\n";
         }
       }
       for (int w = 0; w < W; ++w) {
@@ -1279,9 +1301,11 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
           re = "(vr" + std::to_string(w) + "_0 + vr" + std::to_string(w) + "_1) + (vr" + std::to_string(w) + "_2 + vr" + std::to_string(w) + "_3)";
           im = "(vi" + std::to_string(w) + "_0 + vi" + std::to_string(w) + "_1) + (vi" + std::to_string(w) + "_2 + vi" + std::to_string(w) + "_3)";
         }
-        for (const Sections::QRef& r : S.qrefs)
-          if (r.pr.empty()) re = re.empty() ? "k" + std::to_string(w) + "_" + std::to_string(r.keep)
-                                            : "(" + re + ") + k" + std::to_string(w) + "_" + std::to_string(r.keep);
+        for (const Sections::QRef& r : S.qrefs) {
+          if (!r.pr.empty()) continue;      // the root's own Q
+          re = re.empty() ? kname(w, r.keep) : "(" + re + ") + " + kname(w, r.keep);
+          if (r.keep_im >= 0) im = im.empty() ? kname(w, r.keep_im) : "(" + im + ") + " + kname(w, r.keep_im);
+        }
         if (re.empty()) re = "0.0";
         if (im.empty()) im = "0.0";
         q << "        { const int b = b0 + " << w << "; AMI_EMIT(" << re << ", " << im << "); }\n";

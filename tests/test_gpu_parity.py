@@ -186,6 +186,12 @@ def test_complex_energies_variant_5b(ami, torch_mod, oracle_mod, name, plan):
     for b, beta in enumerate(betas):
         truth, S = truth_for(oracle_mod, cfg, e_c.T.copy(), z, beta, cfg.e_reg)
         check_parity(out[b], truth, S, label=f"5b {name} {plan} beta={beta}")
+    # one very cold and one very hot temperature alone in a launch (single-temperature body; P12: |d|^2 of the complex
+    # leaves must not overflow -- it did in the specialised kernels until the leaf was rescaled by 2^-N)
+    for beta in (5000.0, 200.0, 1e-3):
+        cold = tab.evaluate(torch_mod.from_numpy(e_c).cuda(), z, [beta], e_reg=cfg.e_reg, plan=pid).cpu().numpy()
+        truth, S = truth_for(oracle_mod, cfg, e_c.T.copy(), z, beta, cfg.e_reg)
+        check_parity(cold[0], truth, S, label=f"5b {name} {plan} beta={beta}")
     if plan == "reg":      # real energies given as complex numbers: the same values as the real-energy kernels
         e0 = torch_mod.from_numpy(e_real.astype(np.complex128)).cuda()
         a = tab.evaluate(e0, z, betas, e_reg=cfg.e_reg, plan=pid)
@@ -355,6 +361,15 @@ def test_several_temperatures_per_launch(ami, torch_mod, oracle_mod, name, n_b):
         check_parity(out[b], truth, S, label=f"{name} n_b={n_b} beta#{b}")
         alone = tab.evaluate_momenta(k, [cfg.q], cfg.t, cfg.mu, z, [beta], e_reg=cfg.e_reg).cpu().numpy()[0]
         assert np.all(np.abs(alone - out[b]) <= 1e-12 * S + 1e-280), f"{name} n_b={n_b} beta#{b} against the row computed alone"
+    if name != "cfg5":
+        return
+    # the same with complex energies: complex Q(n) in the prefix-product form
+    gam = A.uniform01(7, np.arange(e_rows.size, dtype=np.uint64)).reshape(e_rows.shape) * 0.05
+    e_c = e_rows - 1j * gam
+    out_c = tab.evaluate(torch_mod.from_numpy(np.ascontiguousarray(e_c.T)).cuda(), z, betas, e_reg=cfg.e_reg).cpu().numpy()
+    for b, beta in enumerate(betas):
+        truth, S = truth_for(oracle_mod, cfg, e_c, z, beta, cfg.e_reg)
+        check_parity(out_c[b], truth, S, label=f"{name} complex energies n_b={n_b} beta#{b}")
 
 
 @pytest.mark.parametrize("plan", list(PLANS))
