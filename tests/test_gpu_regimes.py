@@ -1,0 +1,63 @@
+"""GPU parity across parameter regimes the fixed configurations do not visit: seeded random draws of the energy
+scale (1e-2 .. 30 times the band width), one to five temperatures per launch with beta log-uniform in 1e-3 .. 5e3,
+external frequencies on the Matsubara axis, near the real axis, far out and anywhere in the plane, degenerate energy
+symbols, real and complex energies (imaginary parts 1e-6 .. 1) -- every (plan, temperature) block against the quad
+oracle under the norm of tests/parity.py.  (This is the sweep that found the overflow of the complex-energy leaf at
+beta |Re E| of a few hundred; it stays as a regression net for the specialised kernels' leaf arithmetic.)"""
+import math
+
+import numpy as np
+import pytest
+
+import ami_inputs as A
+from parity import check_parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ami():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2311_17189_b200 import build
+    build.build()
+    import paper_2311_17189_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2_se", "cfg2_bubble", "cfg2_bubble_doubled", "cfg3", "cfg4", "cfg5"])
+def test_random_regimes_against_the_oracle(ami, oracle_mod, name):
+    import torch
+    cfg = A.get_config(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    rng = np.random.default_rng(20231117 + sum(map(ord, name)))
+    n, n_checks = 96, 0
+    fermionic_ext = "bubble" not in name
+    for trial in range(12):
+        scale = 10.0 ** rng.uniform(-2, 1.5)
+        betas = list(10.0 ** rng.uniform(-3, 3.7, size=int(rng.integers(1, 6))))
+        e = rng.uniform(-4, 4, size=(n, cfg.diagram.n_eps)) * scale
+        if trial % 4 == 1:
+            e[:, 1] = e[:, 0]                       # two symbols with the same energy
+        kind = trial % 4
+        if kind == 0:       # Matsubara points of the first temperature
+            z = np.array([[1j * (2 * m + (1 if fermionic_ext else 0)) * math.pi / betas[0]] for m in (0, 1, -3)])
+        elif kind == 1:     # continued to just above the real axis
+            z = np.array([[w + 1j * g] for w, g in ((0.3, 0.1), (-2.0, 1e-3), (0.0, 1e-6))])
+        elif kind == 2:     # far out
+            z = np.array([[complex(rng.uniform(-50, 50), rng.uniform(1e-3, 2))] for _ in range(2)])
+        else:               # anywhere
+            z = np.array([[complex(rng.uniform(-5, 5), rng.uniform(-2, 2))] for _ in range(3)])
+        ee = e - 1j * rng.uniform(0, 1, size=e.shape) * 10.0 ** rng.uniform(-6, 0) if trial % 2 else e
+        et = torch.from_numpy(np.ascontiguousarray(ee.T)).cuda()
+        for plan, pn in ((ami.PLAN_REG, "reg"), (ami.PLAN_FLAT, "flat")):
+            out = tab.evaluate(et, z, betas, e_reg=cfg.e_reg, plan=plan).cpu().numpy()
+            for b, beta in enumerate(betas):
+                truth, S = ot.evaluate(ee, z, beta, e_reg=cfg.e_reg, quad=True, threads=oracle_mod.hardware_threads(),
+                                       want_S=True)
+                check_parity(out[b], truth, S, label=f"{name} trial {trial} {pn} scale={scale:.2e} beta={beta:.3e} "
+                                                     f"n_b={len(betas)} complex={trial % 2}")
+                n_checks += 1
+    assert n_checks >= 48
