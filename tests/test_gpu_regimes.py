@@ -61,3 +61,33 @@ def test_random_regimes_against_the_oracle(ami, oracle_mod, name):
                                                      f"n_b={len(betas)} complex={trial % 2}")
                 n_checks += 1
     assert n_checks >= 48
+
+
+@pytest.mark.parametrize("order,seeds", [(2, range(4)), (3, range(6)), (4, range(6)), (5, range(5)), (6, (1, 2))])
+def test_random_diagrams_against_the_oracle(ami, oracle_mod, order, seeds):
+    """Topologies the fixed configurations do not contain: seeded random 1PI self-energy diagrams (SURVEY 8(d) generator)
+    of orders 2-6 -- some with double poles, the largest order-6 tables on the split plan -- constructed by the library
+    and by the oracle independently, evaluated by every plan the table supports, against the quad oracle."""
+    import torch
+    thr = oracle_mod.hardware_threads()
+    for seed in seeds:
+        d = A.random_self_energy(order, seed)
+        tab = ami.AmiTable.from_diagram(d)
+        ot = oracle_mod.OracleTable.from_diagram(d)
+        n = 128 if order < 6 else 48
+        rng = np.random.default_rng(1000 * order + seed)
+        k = torch.from_numpy(rng.uniform(-math.pi, math.pi, size=(n, d.n_int, 2))).cuda()
+        betas = [float(10 ** rng.uniform(-1, 1.5)), 8.0]
+        z = np.array([[1j * math.pi / betas[0]], [0.4 + 0.05j]])
+        e = tab.dispersion(k, [[0.5 * math.pi, 0.5 * math.pi]], 1.0, -0.1)
+        e_rows = e.cpu().numpy().T.copy()
+        truths = [ot.evaluate(e_rows, z, beta, e_reg=1e-8, quad=True, threads=thr, want_S=True) for beta in betas]
+        for plan, pn in ((ami.PLAN_AUTO, "auto"), (ami.PLAN_FLAT, "flat"), (ami.PLAN_TREE, "tree")):
+            try:
+                out = tab.evaluate(e, z, betas, e_reg=1e-8, plan=plan).cpu().numpy()
+            except ami.AmiError:
+                assert plan == ami.PLAN_TREE        # the only plan a table may be outside of
+                continue
+            for b, (truth, S) in enumerate(truths):
+                check_parity(out[b], truth, S, label=f"order {order} seed {seed} {pn} beta={betas[b]:.3g} "
+                                                     f"T={tab.info['n_terms']}")
