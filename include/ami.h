@@ -342,7 +342,7 @@ int ami_table_kernel_cubin_variant(const ami_table* tab, int dim, int band, int 
  * device from `seed` with the counter-based generator of P22 (sample index = first_sample + s) --
  * with the register plan INSIDE the evaluation kernel, so the momenta never exist in memory; with
  * the table-driven plans by a generation kernel into a chunk buffer.  With the register plan and at
- * most 16 result rows the tally is formed inside the evaluation kernel too (per-warp partial sums,
+ * most 1024 result rows the tally is formed inside the evaluation kernel too (per-warp partial sums,
  * added in a fixed order), and per-sample results are written only if h_out / d_out is given;
  * else read from the given buffer, layout [n][2*n_int] (Eq. 8).  Results: per-sample values to
  * h_out / d_out (complex128 [n_b][n_f][n]) when given, and/or the running sum over samples to

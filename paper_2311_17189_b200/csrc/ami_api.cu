@@ -364,7 +364,10 @@ int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg
   return AMI_OK;
 }
 
-constexpr int64_t kFusedTallyMaxRows = 16;   // beyond this the warp reductions cost more than re-reading the results
+// The tally is formed inside the evaluation kernel up to this many result rows: a warp reduction per (row, 32 samples)
+// costs a sixth of the kernel's instructions at 256 rows, storing the results and reading them back a third of its time
+// (cfg5, 64 frequencies x 4 temperatures, 1e6 samples: 4.1 -> 3.2 ms).  The limit only bounds the partial-sum workspace.
+constexpr int64_t kFusedTallyMaxRows = 1024;
 
 struct MomentaSrc {
   const double* d_k = nullptr;
@@ -854,6 +857,7 @@ extern "C" int ami_run(const ami_table* tab, const ami_run_cfg* cfg, ami_run_sta
   // (measured: 2^17 samples); otherwise as large as the workspace allows (one chunk = no per-chunk overhead)
   int64_t chunk = cfg->chunk ? cfg->chunk : (host_io ? (int64_t)1 << 17 : (int64_t)1 << 26);
   while (chunk > 1024 && ((own_out && chunk * rows * 16 > ((int64_t)256 << 20)) ||
+                          (fused_tally && chunk * rows > ((int64_t)1 << 30)) ||     // per-warp partials: rows x chunk bytes
                           (own_k && chunk * n_comp * 8 > ((int64_t)256 << 20)) ||
                           (!use_reg && chunk * n_eps * 8 > ((int64_t)256 << 20))))
     chunk /= 2;

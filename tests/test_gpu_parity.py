@@ -585,9 +585,9 @@ def test_run_streamed_matches_stagewise(ami, torch_mod, oracle_mod, mode):
     check_parity(h_out.numpy()[0][:, sel], truth, S, label="run")
 
 
-@pytest.mark.parametrize("name,n", [("cfg1", 1), ("cfg1", 33), ("cfg3", 5000 + 19), ("cfg2_se", 4096 + 31)])
+@pytest.mark.parametrize("name,n", [("cfg1", 1), ("cfg1", 33), ("cfg3", 5000 + 19), ("cfg2_se", 4096 + 31), ("cfg5", 2500 + 3)])
 def test_run_fused_tally(ami, torch_mod, name, n):
-    """Register plan with a few rows: the evaluation kernel leaves per-warp partial sums and nothing else has to be
+    """Register plan (cfg5: a grid of 256 rows): the evaluation kernel leaves per-warp partial sums and nothing else has to be
     stored.  Tally-only call == tally beside stored results == numpy sums of those results (ragged last warp,
     several chunks, several rows); the squares give the error bar.  Deterministic."""
     cfg = A.get_config(name)
