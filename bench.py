@@ -679,6 +679,14 @@ def run_ours(args, dist, rank, local, world):
                             "specialize_from_disk_cache": bool(i2["specialize_cached"]),
                             "ordered_ms_per_step": r2["ordered_ms"],
                             "alu_frac_ordered": None if r2["ordered_ms"] is None else roof2["frac"] * ms2 / r2["ordered_ms"]}
+            if name == "cfg5":
+                # the paper's use of the path: the momentum integral on a (frequency, temperature)
+                # grid -- 256 result rows tallied inside the evaluation kernel, nothing but the sums leaves the device
+                mc5 = time_monte_carlo(torch, r2["tab"], c2, 5 * c2.n_samples, 3, plan)
+                w5 = fp64_work_per_sample(i2, f2, b2, r2["fused"])
+                mc5["alu_frac_device_time"] = (w5["evaluate"] + w5["dispersion"]) * 5 * c2.n_samples \
+                    / (mc5["gpu_ms_per_step"] * 1e-3) / dfma_per_s
+                others[name]["monte_carlo_grid"] = mc5
             if int(i2.get("plan_kind", 1)) == 2:
                 # the split plan's parts read every leaf they use from the L2-resident leaf array: that, not the FP64
                 # pipe, bounds it; the slots counted are those of the Horner plan, without the sums
