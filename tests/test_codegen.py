@@ -133,3 +133,27 @@ def test_inspect_kernels_reports_register_operands():
     assert all(0 <= k[2] <= k[1] <= 3 for k in c["fp64"])
     two = sum(v for k, v in c["fp64"].items() if k[1] <= 2)
     assert two > 0.6 * n_fp and c["other"] > 0
+
+
+def test_instruction_counts_of_the_several_temperature_body():
+    """ami_info.fp64_ops_mb_prefix / fp64_ops_mb_sum (the roofline numerator of launches with several temperatures) are
+    the multiplications and fused multiply-adds the generator writes: the prefix products once per frequency, and the
+    sum of the one-temperature block per (frequency, temperature).  cfg5 takes the prefix-product form, cfg4 keeps the
+    Horner form (prefix = 0, sum = the R part of fp64_ops_tree)."""
+    import re
+    import ami_inputs as A
+    import paper_2311_17189_b200 as pkg
+    ops = lambda text: text.count("fma(") + len(re.findall(r"= -?\w+ \* \w+;", text))
+    tab = pkg.AmiTable.from_diagram(A.get_config("cfg5").diagram, device=None)
+    info, src = tab.info, tab.kernel_source()
+    body = src[src.index("void ami_body_mb"):]
+    prefix = body[body.index("const double P"):body.index("int b0 = 0;")]      # first prefix product .. the blocks
+    one = body[body.index("if (b0 < p.n_b)"):body.index("\n}\n", body.index("if (b0 < p.n_b)"))]
+    assert info["fp64_ops_mb_prefix"] == ops(prefix) > 0
+    # the block of one temperature spreads its terms over four partial sums: three more additions than counted
+    assert info["fp64_ops_mb_sum"] == ops(one) > 0
+    assert info["fp64_ops_mb_prefix"] + 2 * info["fp64_ops_mb_sum"] <= 2 * (info["fp64_ops_tree"] - info["fp64_ops_tree_fermi"])
+    tab4 = pkg.AmiTable.from_diagram(A.get_config("cfg4").diagram, device=None)
+    i4 = tab4.info
+    assert i4["fp64_ops_mb_prefix"] == 0 and i4["fp64_ops_mb_sum"] == i4["fp64_ops_tree"] - i4["fp64_ops_tree_fermi"]
+    assert "int b0 = 0;" not in tab4.kernel_source()
