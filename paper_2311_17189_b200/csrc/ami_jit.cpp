@@ -10,7 +10,11 @@
 //
 // Register plan (orders <= 6-7): the whole table is one body; ami_jit_eval (energies from memory,
 // S2+S3), ami_jit_fused (momenta from memory or drawn in place, S1+S2+S3) and ami_jit_fused_tally
-// (the same with the Monte-Carlo tally of S4 folded in) are generated from it.
+// (the same with the Monte-Carlo tally of S4 folded in) are generated from it.  Each kernel holds two bodies: one
+// temperature per launch (beta { frequency { R part in Horner form } }), and several (per-beta values kept in a
+// per-thread array, then frequency { reciprocals, R part for all temperatures }; where it is cheaper the R part
+// is the sum over prefix products of Sections::secP / qrefs, four temperatures side by side).  A launch flagged
+// AMI_PLAN_UNORDERED waits for its predecessor at its end instead of its start (kUnorderedEnd).
 //
 // Split plan (orders 7-8: 1e4-1e5 flat terms, hundreds of leaves, thousands of shared sums -- more
 // than one thread's registers hold): the groups of the Horner plan are partitioned, in the order of
