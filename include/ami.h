@@ -331,7 +331,7 @@ int ami_table_kernel_cubin(const ami_table* tab, void* buf, size_t* bytes, char*
 int ami_table_kernel_units(const ami_table* tab, int* n_units);
 int ami_table_kernel_cubin_unit(const ami_table* tab, int unit, void* buf, size_t* bytes, char* log, size_t log_cap);
 /* The kernels are generated per variant: lattice of the inline dispersion (dim, band as in ami_dispersion_lattice) and
- * real or complex energies (complex ones: tables of register-plan size, ami_evaluate only).  The calls
+ * real or complex energies (complex ones through ami_evaluate only: momenta give real energies).  The calls
  * above return the variant of the configurations (2, tight binding, real); these return any. */
 int ami_table_kernel_source_variant(const ami_table* tab, int dim, int band, int complex_energies, char* buf,
                                     size_t* bytes);

@@ -349,8 +349,7 @@ int choose_plan(const ami_table* tab, int plan, bool e_is_complex, bool* use_reg
     if (use_tree) *use_tree = true;
     return AMI_OK;
   }
-  if (!ami::jit_eligible(tab->flat, tab->horner) ||
-      (e_is_complex && ami::jit_mode(tab->flat, tab->horner) != ami::kJitRegister)) {
+  if (!ami::jit_eligible(tab->flat, tab->horner)) {
     if (plan == AMI_PLAN_REG) { g_cuda_err = "register plan unavailable for this table / energy type"; return AMI_EUNSUPPORTED; }
     if (use_tree) *use_tree = tree_auto;        // AUTO: the table-driven Horner program for large tables
     return AMI_OK;
@@ -631,7 +630,6 @@ int ami_table_kernel_source_variant(const ami_table* tab, int dim, int band, int
   ami::JitVariant var;
   if (variant_of(dim, band, complex_energies, &var)) return AMI_EINVAL;
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
-  if (var.cplx && ami::jit_mode(tab->flat, tab->horner) != ami::kJitRegister) return AMI_EUNSUPPORTED;
   const std::vector<std::string> srcs = ami::jit_generate_sources(tab->flat, tab->horner, var, nullptr);
   std::string src;
   for (size_t i = 0; i < srcs.size(); ++i) {
@@ -662,7 +660,6 @@ int ami_table_kernel_cubin_variant(const ami_table* tab, int dim, int band, int 
   ami::JitVariant var;
   if (variant_of(dim, band, complex_energies, &var)) return AMI_EINVAL;
   if (!ami::jit_eligible(tab->flat, tab->horner)) return AMI_EUNSUPPORTED;
-  if (var.cplx && ami::jit_mode(tab->flat, tab->horner) != ami::kJitRegister) return AMI_EUNSUPPORTED;
   const std::vector<std::string> srcs = ami::jit_generate_sources(tab->flat, tab->horner, var, nullptr);
   if (unit < 0 || unit >= (int)srcs.size()) return AMI_EINVAL;
   std::vector<char> cubin;

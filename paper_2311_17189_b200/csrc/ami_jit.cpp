@@ -874,9 +874,20 @@ void gen_sections(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls
 }
 
 // The four sections of the body for complex energies e<i>r + i e<i>i (register plan only).
-void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, Emitter& E, Sections& S) {
+// `ls` (split plan only): the leaf slots of the whole table, every value two doubles (re at the slot, im at the next).
+void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, const LeafSlots& ls, LeafMode mode, Emitter& E,
+                       Sections& S) {
   int cur = 0;
 #define o S.sec[cur]
+  // which leaves this plan uses (a part of the split plan: those its sums and its slice of the trie reach)
+  std::vector<char> useF(ft.leafF.size(), 1), useD(ft.leafD.size(), 1);
+  if (mode == kLeafLoad) {
+    std::fill(useF.begin(), useF.end(), 0);
+    std::fill(useD.begin(), useD.end(), 0);
+    for (const SNode& n : hp.snodes)
+      for (const SItem& it : n.items) useF[it.leaf] = 1;
+    for (size_t n = 1; n < hp.dn.size(); ++n) useD[hp.dn[n].leaf] = 1;
+  }
   std::vector<std::vector<int>> combos;
   auto combo_ref = [&](const std::vector<int>& c, std::string* sign) -> int {
     std::vector<int> pos = c;
@@ -893,12 +904,20 @@ void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, Emitter& E, Se
     if (j == combos.size()) combos.push_back(pos);
     return (int)j;
   };
-  for (const LeafD& l : ft.leafD) { std::string sg; combo_ref(l.c, &sg); }
-  for (size_t j = 0; j < combos.size(); ++j)
-    o << "  const double E" << j << "r = " << combo(combos[j], "e", "r") << ", E" << j << "i = " << combo(combos[j], "e", "i") << ";\n";
+  if (mode != kLeafLoad) {
+    for (const LeafD& l : ft.leafD) { std::string sg; combo_ref(l.c, &sg); }
+    for (size_t j = 0; j < combos.size(); ++j)
+      o << "  const double E" << j << "r = " << combo(combos[j], "e", "r") << ", E" << j << "i = " << combo(combos[j], "e", "i") << ";\n";
+  }
   auto emit_d_leaves = [&](bool freq_independent, const std::string& ind) {
     for (size_t u = 0; u < ft.leafD.size(); ++u) {
       if ((hp.d_is_real[u] != 0) != freq_independent) continue;
+      if (mode == kLeafLoad) {     // read where it is used
+        if (!useD[u]) continue;
+        if (freq_independent) o << "#define Dr" << u << " AMI_L(" << ls.ridx[u] << ")\n#define Di" << u << " AMI_L(" << ls.ridx[u] + 1 << ")\n";
+        else o << "#define Dr" << u << " AMI_LC(" << 2 * ls.cidx[u] << ")\n#define Di" << u << " AMI_LC(" << 2 * ls.cidx[u] + 1 << ")\n";
+        continue;
+      }
       const LeafD& l = ft.leafD[u];
       std::string sg;
       const int j = combo_ref(l.c, &sg);
@@ -915,10 +934,18 @@ void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, Emitter& E, Se
       }
       o << ind << "  const double r = fast_rcp(fma(re, re, im * im));\n" << ind << "  Dr" << u << " = re * r; Di" << u << " = -im * r;\n"
         << ind << "}\n";
+      if (mode == kLeafStore) {
+        if (freq_independent) o << ind << "AMI_LS(" << ls.ridx[u] << ", Dr" << u << "); AMI_LS(" << ls.ridx[u] + 1 << ", Di" << u << ");\n";
+        else o << ind << "AMI_LSC(" << 2 * ls.cidx[u] << ", Dr" << u << "); AMI_LSC(" << 2 * ls.cidx[u] + 1 << ", Di" << u << ");\n";
+      }
     }
   };
   emit_d_leaves(true, "  ");
   cur = 1;
+  if (mode == kLeafLoad) {
+    for (size_t u = 0; u < ft.leafF.size(); ++u)
+      if (useF[u]) o << "#define Fr" << u << " AMI_LF(" << 2 * u << ")\n#define Fi" << u << " AMI_LF(" << 2 * u + 1 << ")\n";
+  } else {
   // one exponential per energy symbol: e^{beta e_i} = 2^{n_i} (m_i r + i m_i i), |m_i| in [0.70, 1.42]
   std::vector<char> sym_used(ft.n_eps, 0);
   for (const LeafF& l : ft.leafF)
@@ -990,8 +1017,13 @@ void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, Emitter& E, Se
     }
     o << "    }\n";
   }
+  if (mode == kLeafStore)
+    for (size_t u = 0; u < ft.leafF.size(); ++u) o << "    AMI_LSF(" << 2 * u << ", Fr" << u << "); AMI_LSF(" << 2 * u + 1 << ", Fi" << u << ");\n";
+  }   // leaves computed here
+  std::vector<CV> q(hp.dn.size());
+  std::vector<char> q_have(hp.dn.size(), 0);
   // FT sums, level by level
-  {
+  if (mode != kLeafStore) {
     std::vector<int> order(hp.snodes.size());
     for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return hp.snodes[a].height < hp.snodes[b].height; });
@@ -1012,9 +1044,7 @@ void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, Emitter& E, Se
       else o << "    const double FTr" << g << " = " << dlit((double)hg.num / (double)hg.den) << ", FTi" << g << " = 0.0;\n";
     }
   }
-  std::vector<CV> q(hp.dn.size());
-  std::vector<char> q_have(hp.dn.size(), 0);
-  {
+  if (mode != kLeafStore) {
     std::vector<Stmts> lists;
     for (size_t n = 0; n < hp.dn.size(); ++n) {
       if (n != 0 && hp.d_is_real[hp.dn[n].leaf]) continue;
@@ -1030,21 +1060,22 @@ void gen_sections_cplx(const FlatTable& ft, const HornerPlan& hp, Emitter& E, Se
     interleave(lists, kWays, o, "    ");
   }
   cur = 2;
-  for (int x = 0; x < ft.n_ext; ++x) {
-    o << "      const double zr" << x << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ")], zi" << x
-      << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ") + 1];\n";
-    o << "      const bool zz" << x << " = (zr" << x << " == 0.0 && zi" << x << " == 0.0);\n";
-  }
+  if (mode != kLeafLoad)
+    for (int x = 0; x < ft.n_ext; ++x) {
+      o << "      const double zr" << x << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ")], zi" << x
+        << " = p.z[2 * (f * " << ft.n_ext << " + " << x << ") + 1];\n";
+      o << "      const bool zz" << x << " = (zr" << x << " == 0.0 && zi" << x << " == 0.0);\n";
+    }
   emit_d_leaves(false, "      ");
   cur = 3;
-  {
+  if (mode != kLeafStore) {
     Stmts st;
     const CV acc = emit_d_sum_cplx(hp, q, q_have, 0, E, st);
     for (const std::string& s : st) o << "      " << s << "\n";
     o << "      AMI_EMIT(" << acc.re << ", " << (acc.real() ? std::string("0.0") : acc.im) << ");\n";
   }
 #undef o
-  {
+  if (mode == kLeafInline) {
     std::vector<CV> qq(hp.dn.size());
     for (size_t n = 0; n < hp.dn.size(); ++n)
       if (q_have[n]) qq[n] = q[n];
@@ -1220,7 +1251,7 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
   };
   if (mode == kJitRegister) {
     Sections S;
-    if (var.cplx) gen_sections_cplx(ft, hp, E, S);
+    if (var.cplx) gen_sections_cplx(ft, hp, ls, kLeafInline, E, S);
     else gen_sections(ft, hp, ls, kLeafInline, E, S);
     o << kTallySrc;
     // what a finished row does with its value: store it, and/or add it to the tally
@@ -1362,7 +1393,17 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
   // Module 0: the leaf kernels and the kernel that adds the parts.  Modules 1..M: the parts, a few per module, so
   // that NVRTC compiles them side by side on the host's cores (a part is 1-2 k statements; one translation unit
   // with all of an order-8 table's parts takes 20 s, eight of them 3-5 s).
-  const std::vector<std::vector<int>> parts = partition_groups(hp, split_budget());
+  // complex energies: every leaf is two doubles (re at its slot, im at the next), and a complex sum costs three to
+  // four times the instructions of a real one, so the parts are cut smaller
+  LeafSlots lsc = ls;
+  if (var.cplx) {
+    for (int& r : lsc.ridx)
+      if (r >= 0) r *= 2;
+    lsc.n_real = 2 * ls.n_real;
+    lsc.n_fermi = 2 * ls.n_fermi;
+    if (layout) { layout->n_real_den = lsc.n_real; layout->n_fermi = lsc.n_fermi; }
+  }
+  const std::vector<std::vector<int>> parts = partition_groups(hp, var.cplx ? std::max(100LL, split_budget() / 3) : split_budget());
   const int n_parts = (int)parts.size();
   const int n_mod = std::min(n_parts, 8);
   if (layout) {
@@ -1378,18 +1419,26 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
        "#define AMI_LSC(j, v) LsC[(j) * AMI_NT] = (v)\n";
   {   // leaf kernels: everything that depends on one energy combination, written once per sample
     Sections S;
-    gen_sections(ft, hp, ls, kLeafStore, E, S);
+    if (var.cplx) gen_sections_cplx(ft, hp, lsc, kLeafStore, E, S);
+    else gen_sections(ft, hp, ls, kLeafStore, E, S);
     o << "__device__ __forceinline__ void ami_leaf_body(const AmiBatch& p, const long long s" << esig << ") {\n"
-      << "  const int CB = " << ls.n_real << " + p.n_b * " << ls.n_fermi << ";\n"
+      << "  const int CB = " << lsc.n_real << " + p.n_b * " << lsc.n_fermi << ";\n"
       << "  double* __restrict__ Ls = p.leaves + (s / AMI_NT) * p.leaf_stride + (s % AMI_NT);\n" << S.sec[0].str()
       << "#pragma unroll 1\n  for (int b = 0; b < p.n_b; ++b) {\n    const double beta = p.beta[b];\n"
-      << "    double* __restrict__ LsF = Ls + (" << ls.n_real << " + b * " << ls.n_fermi << ") * AMI_NT;\n" << S.sec[1].str() << "  }\n"
+      << "    double* __restrict__ LsF = Ls + (" << lsc.n_real << " + b * " << lsc.n_fermi << ") * AMI_NT;\n" << S.sec[1].str() << "  }\n"
       << "#pragma unroll 1\n  for (int f = 0; f < p.n_f; ++f) {\n"
       << "    double* __restrict__ LsC = Ls + (CB + 2 * f * " << ls.n_cplx << ") * AMI_NT;\n" << S.sec[2].str() << "  }\n}\n\n";
     o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_split_leaves_eval(const __grid_constant__ AmiBatch p) {\n"
          "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n  if (s >= p.n) return;\n";
-    for (int i = 0; i < ft.n_eps; ++i) o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
+    for (int i = 0; i < ft.n_eps; ++i) {
+      if (var.cplx)
+        o << "  const double e" << i << "r = p.e[2 * (" << i << " * p.e_stride + s)], e" << i << "i = p.e[2 * (" << i
+          << " * p.e_stride + s) + 1];\n";
+      else
+        o << "  const double e" << i << " = p.e[" << i << " * p.e_stride + s];\n";
+    }
     o << "  ami_leaf_body(p, s" << eargs << ");\n}\n\n";
+    if (!var.cplx) {   // momenta give real energies: no fused leaf kernel for complex ones
     o << "extern \"C\" __global__ void __launch_bounds__(AMI_NT, AMI_MINB) ami_split_leaves_fused(const __grid_constant__ AmiBatch p) {\n"
          "  const long long s = blockIdx.x * (long long)AMI_NT + threadIdx.x;\n  if (s >= p.n) return;\n";
     for (int c = 0; c < n_comp; ++c) o << "  double nk" << c << ";\n";
@@ -1398,6 +1447,7 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
     o << "  if (p.e_out) {\n";
     for (int i = 0; i < ft.n_eps; ++i) o << "    p.e_out[" << i << " * p.e_stride + s] = e" << i << ";\n";
     o << "  }\n  ami_leaf_body(p, s" << eargs << ");\n}\n\n";
+    }
   }
   // the parts' partial results, added in the order of the parts (fixed: deterministic), times the prefactor
   // (launched as a programmatic dependent of the last parts kernel: see ami_split_parts)
@@ -1428,17 +1478,20 @@ std::vector<std::string> jit_generate_sources(const FlatTable& ft, const HornerP
   for (int pi = pa; pi < pb; ++pi) {
     const HornerPlan sub = make_sub_plan(hp, parts[pi]);
     Sections S;
-    gen_sections(ft, sub, ls, kLeafLoad, E, S);
+    if (var.cplx) gen_sections_cplx(ft, sub, lsc, kLeafLoad, E, S);
+    else gen_sections(ft, sub, ls, kLeafLoad, E, S);
     o << "__device__ __noinline__ void ami_part_" << pi
       << "(const double* __restrict__ Lp, double2* __restrict__ Pp, const long long ps, const int n_b, const int n_f) {\n"
-      << "  const int CB = " << ls.n_real << " + n_b * " << ls.n_fermi << ";\n" << S.sec[0].str()
+      << "  const int CB = " << lsc.n_real << " + n_b * " << lsc.n_fermi << ";\n" << S.sec[0].str()
       << "#pragma unroll 1\n  for (int b = 0; b < n_b; ++b) {\n"
-      << "    const double* __restrict__ LpF = Lp + (" << ls.n_real << " + b * " << ls.n_fermi << ") * AMI_NT;\n" << S.sec[1].str()
+      << "    const double* __restrict__ LpF = Lp + (" << lsc.n_real << " + b * " << lsc.n_fermi << ") * AMI_NT;\n" << S.sec[1].str()
       << "#pragma unroll 1\n    for (int f = 0; f < n_f; ++f) {\n"
       << "      const double* __restrict__ LpC = Lp + (CB + 2 * f * " << ls.n_cplx << ") * AMI_NT;\n"
       << S.sec[2].str() << S.sec[3].str() << "    }\n  }\n";
     // the macros that name this part's denominators end with it
     for (size_t u = 0; u < ft.leafD.size(); ++u) o << "#undef Dr" << u << "\n#undef Di" << u << "\n";
+    if (var.cplx)
+      for (size_t u = 0; u < ft.leafF.size(); ++u) o << "#undef Fr" << u << "\n#undef Fi" << u << "\n";
     o << "}\n\n";
   }
   // grid.y = part within this module; p.part0 = index of the module's first part.
@@ -1712,8 +1765,6 @@ int jit_prepare(ami_table* tab, const JitVariant& var, std::string& err) {
   if (var.dim < 1 || var.dim > 3 || (var.band != AMI_BAND_TIGHT_BINDING && var.band != AMI_BAND_FREE))
     return fail(AMI_EINVAL, "bad lattice for the specialised kernels");
   if (!jit_eligible(tab->flat, tab->horner)) return fail(AMI_EUNSUPPORTED, "table outside the limits of the specialised kernels");
-  if (var.cplx && jit_mode(tab->flat, tab->horner) != kJitRegister)
-    return fail(AMI_EUNSUPPORTED, "complex energies: only tables of register-plan size are specialised");
   const auto t0 = std::chrono::steady_clock::now();
   const std::vector<std::string> srcs = jit_generate_sources(tab->flat, tab->horner, var, &m.layout);
   // the modules of a split plan are compiled side by side (NVRTC is thread safe across programs)
@@ -1761,7 +1812,7 @@ int jit_prepare(ami_table* tab, const JitVariant& var, std::string& err) {
     }
   } else {
     get(&m.fn_leaves_eval, 0, "ami_split_leaves_eval");
-    get(&m.fn_leaves_fused, 0, "ami_split_leaves_fused");
+    if (!var.cplx) get(&m.fn_leaves_fused, 0, "ami_split_leaves_fused");
     get(&m.fn_combine, 0, "ami_split_combine");
     m.fn_parts.assign(srcs.size() - 1, nullptr);
     for (size_t i = 1; i < srcs.size(); ++i) get(&m.fn_parts[i - 1], i, "ami_split_parts");
@@ -1829,7 +1880,7 @@ cudaError_t jit_launch(const ami_table* tab, const JitVariant& var, bool fused, 
   }
   // split plan: leaves -> parts -> combine per chunk of samples; the chunk is sized so that the leaf array and the
   // parts' partial results (stream-ordered allocations) stay in L2 between the kernels
-  if (b.tally || !b.out) return cudaErrorInvalidValue;
+  if (b.tally || !b.out || (var.cplx && fused)) return cudaErrorInvalidValue;
   const JitLayout& lay = m->layout;
   const long long rows = (long long)b.n_b * b.n_f;
   const long long slots = lay.n_real_den + (long long)b.n_b * lay.n_fermi + 2LL * b.n_f * lay.n_cplx_den;
@@ -1848,7 +1899,7 @@ cudaError_t jit_launch(const ami_table* tab, const JitVariant& var, bool fused, 
   for (long long c0 = 0; c0 < b.n && ok; c0 += chunk) {
     AmiBatch part = b;
     part.n = std::min(chunk, b.n - c0);
-    if (part.e) part.e += c0;                       // SoA rows keep their stride
+    if (part.e) part.e += var.cplx ? 2 * c0 : c0;   // SoA rows keep their stride (complex: two doubles per sample)
     if (part.e_out) part.e_out += c0;
     if (part.k) part.k += c0 * b.k_stride_sample;
     part.first_sample += c0;

@@ -95,10 +95,12 @@ def test_kernel_variants_compile(ami, kw):
             pytest.skip("NVRTC library not available on this machine")
         raise
     assert cubin[:4] == b"\x7fELF" and "ami_jit_eval" in log
-    big = ami.AmiTable.from_diagram(A.get_config("stress8").diagram, device=None)
-    if kw.get("complex_energies"):
-        with pytest.raises(ami.AmiError):          # complex energies: tables of register-plan size only
-            big.kernel_source(**kw)
+    if kw.get("complex_energies"):     # tables of split-plan size: leaf kernel for energies from memory only, leaves in pairs
+        big = ami.AmiTable.from_diagram(A.random_self_energy(7, 0), device=None)
+        src = big.kernel_source(**kw)
+        assert "ami_split_leaves_eval" in src and "ami_split_leaves_fused" not in src and "#define Fi" in src
+        cubin, log = big.kernel_cubin(unit=big.kernel_units() - 1, **kw)
+        assert cubin[:4] == b"\x7fELF" and "ami_split_parts" in log
 
 
 def test_register_plan_can_be_switched_off():

@@ -260,17 +260,18 @@ def test_register_plan_is_what_auto_runs(ami, torch_mod, name):
 
 
 def test_register_plan_limits(ami, torch_mod):
-    """Tables beyond one register-resident kernel (order 8) are specialised as a split plan; with complex energies
-    they run the table-driven kernels under AUTO and are refused under an explicit AMI_PLAN_REG."""
+    """Tables beyond one register-resident kernel (order 8) are specialised as a split plan, for real and for complex
+    energies; what no specialised kernel covers (a tally or momenta with the split plan's complex variant) is refused
+    by the launcher, not run."""
     cfg = A.get_config("stress8")
     tab = ami.AmiTable.from_diagram(cfg.diagram)
     assert tab.info["reg_plan_status"] == 1 and tab.info["plan_kind"] == 2
     assert ami.AmiTable.from_diagram(A.get_config("cfg4").diagram).info["plan_kind"] == 1
     ec = gpu_energies(torch_mod, tab, cfg, cfg.momenta(40)).to(torch_mod.complex128)
-    with pytest.raises(ami.AmiError) as ei:      # complex energies: only tables of register-plan size are specialised
-        tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=ami.PLAN_REG)
-    assert ei.value.code == -6
-    tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=ami.PLAN_AUTO)      # the table-driven kernel takes them
+    a = tab.evaluate(ec, cfg.z_ext, cfg.betas, plan=ami.PLAN_REG)       # complex energies, zero imaginary parts ...
+    r = tab.evaluate(ec.real.contiguous(), cfg.z_ext, cfg.betas, plan=ami.PLAN_REG)   # ... against the real-energy kernels
+    scale = r.abs().max().item()
+    assert (a - r).abs().max().item() <= 1e-9 * scale
 
 
 @pytest.mark.parametrize("name,n", [("cfg1", 10_000), ("cfg3", 50_000 + 3), ("cfg4", 3000 + 1), ("cfg5", 401)])
@@ -445,6 +446,43 @@ def test_split_plan_large_tables(ami, torch_mod, oracle_mod, name):
     stats, sums = tab.run(5000 + 3, [cfg.q], cfg.t, cfg.mu, cfg.z_ext, cfg.betas, seed=cfg.seed, want_sum=True)
     ref = ob[:, :, :5003].sum(dim=2).cpu().numpy()
     assert np.max(np.abs(sums - ref)) <= 1e-12 * ob[:, :, :5003].abs().sum().item()
+
+
+@pytest.mark.parametrize("name", ["o7", "stress8"])
+def test_split_plan_complex_energies(ami, torch_mod, oracle_mod, name):
+    """Complex energies on tables of split-plan size: leaf kernel, parts and combine kernel with every
+    leaf a pair of doubles; a (temperature, frequency) grid with a cold temperature in it, two chunks of the leaf array,
+    against the oracle (double precision as truth, as in test_split_plan_large_tables) and the table-driven kernel."""
+    cfg = split_case(name)
+    tab = ami.AmiTable.from_diagram(cfg.diagram)
+    assert tab.info["plan_kind"] == 2
+    n = 96 + 5
+    k = torch_mod.from_numpy(cfg.momenta(n)).cuda()
+    e_real = tab.dispersion(k, [cfg.q], cfg.t, cfg.mu).cpu().numpy()
+    gam = A.uniform01(5, np.arange(e_real.size, dtype=np.uint64)).reshape(e_real.shape) * 0.05
+    e_c = torch_mod.from_numpy(e_real - 1j * gam).cuda()
+    z = np.array([[1j * math.pi / 5.0], [0.3 + 0.1j]])
+    betas = (5.0, 300.0, 0.5)
+    out = tab.evaluate(e_c, z, betas, e_reg=cfg.e_reg, plan=ami.PLAN_REG).cpu().numpy()
+    assert out.shape == (3, 2, n) and np.isfinite(out).all()
+    ot = oracle_mod.OracleTable.from_diagram(cfg.diagram)
+    e_rows = np.ascontiguousarray(e_c.cpu().numpy().T)
+    thr = oracle_mod.hardware_threads()
+    for b, beta in enumerate(betas):       # double truth on all samples at the moderate temperatures, quad on a few at all
+        if beta < 100.0:
+            truth, S = ot.evaluate(e_rows, z, beta, e_reg=cfg.e_reg, quad=False, threads=thr, want_S=True)
+            check_parity(out[b], truth, S, label=f"{name} complex beta={beta}")
+        nq = 20 if name == "o7" else 5          # quad truth costs 40 ms per sample and row at order 8
+        truth, S = ot.evaluate(e_rows[:nq], z, beta, e_reg=cfg.e_reg, quad=True, threads=thr, want_S=True)
+        check_parity(out[b][:, :nq], truth, S, label=f"{name} complex beta={beta} (quad)")
+    flat = tab.evaluate(e_c[:, :16].contiguous(), z, betas[:1], e_reg=cfg.e_reg, plan=ami.PLAN_FLAT).cpu().numpy()
+    truth, S = ot.evaluate(e_rows[:16], z, betas[0], e_reg=cfg.e_reg, quad=False, threads=thr, want_S=True)
+    check_parity(flat[0], truth, S, label=f"{name} complex flat")
+    # AUTO takes the same kernels; a batch of several leaf-array chunks gives the same bits on the shared samples
+    big = 30_000 + 11
+    eb = e_c.repeat(1, big // n + 1)[:, :big].contiguous()
+    ob = tab.evaluate(eb, z, betas, e_reg=cfg.e_reg).cpu().numpy()
+    assert np.array_equal(ob[:, :, :n], out) and np.array_equal(ob[:, :, n:2 * n], out)
 
 
 def test_kernel_cache_on_disk(ami, torch_mod, tmp_path):
