@@ -91,3 +91,10 @@ def test_random_diagrams_against_the_oracle(ami, oracle_mod, order, seeds):
             for b, (truth, S) in enumerate(truths):
                 check_parity(out[b], truth, S, label=f"order {order} seed {seed} {pn} beta={betas[b]:.3g} "
                                                      f"T={tab.info['n_terms']}")
+        # the same table with complex energies (specialised kernels of either kind, and the table-driven one)
+        ee = e_rows[:32] - 1j * rng.uniform(0, 0.1, size=e_rows[:32].shape)
+        et = torch.from_numpy(np.ascontiguousarray(ee.T)).cuda()
+        truth, S = ot.evaluate(ee, z, betas[1], e_reg=1e-8, quad=True, threads=thr, want_S=True)
+        for plan, pn in ((ami.PLAN_AUTO, "auto"), (ami.PLAN_FLAT, "flat")):
+            out = tab.evaluate(et, z, betas[1:], e_reg=1e-8, plan=plan).cpu().numpy()
+            check_parity(out[0], truth, S, label=f"order {order} seed {seed} {pn} complex energies")
