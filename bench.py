@@ -610,6 +610,12 @@ def run_ours(args, dist, rank, local, world):
         "with_integer_work_dfma_per_s": dfma5_per_s, "with_integer_work_frac_of_peak": dfma5_per_s / dfma_per_s,
         "two_changing_sources_frac_of_peak": dfma6_per_s / dfma_per_s,
         "two_changing_sources_with_integer_work_frac_of_peak": dfma7_per_s / dfma_per_s}
+    # per cycle ("report the fraction per cycle so clock drift drops out"): the probe is a 4 ms burst at the
+    # maximum SM clock, the timed steps follow 0.2 s of the same load with the board at its power cap
+    ck = res.get("clocks") or {}
+    if ck.get("sm_mhz") and ck.get("sm_max_mhz"):
+        roof["frac_per_cycle"] = roof["frac"] * float(ck["sm_max_mhz"]) / float(ck["sm_mhz"])
+        roof["frac_per_cycle_note"] = "frac x sm_max_mhz / sm_mhz (median SM clock sampled during the timed steps)"
     cap = ncu_capture(cfg.name, res["fused"]) if n == cfg.n_samples else None
     if cap:      # per launch, from profiles/ (ncu --set full of the same command, committed)
         roof["traffic"] = cap["dram_bytes"]
