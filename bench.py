@@ -672,7 +672,7 @@ def run_ours(args, dist, rank, local, world):
             c2 = A.get_config("stress8" if name in ("order7", "order9") else name)
             if name in ("order7", "order9"):      # order 9: the largest order the paper benchmarks (T = 137644)
                 c2.diagram, c2.name = A.random_self_energy(int(name[-1]), 0), name
-            r2 = time_workload(pkg, torch, c2, c2.n_samples, 20, 3, plan, 0, None, sample_clocks=False,
+            r2 = time_workload(pkg, torch, c2, c2.n_samples, 20, 3, plan, 0, None, sample_clocks=True,
                                use_graph=not args.no_graph)
             i2 = r2["info"]
             pn2 = plan_name_of(i2, args.plan)
@@ -684,6 +684,9 @@ def run_ours(args, dist, rank, local, world):
                             "term_evals_per_s": int(i2["n_terms"]) * c2.n_samples * f2 * b2 / (ms2 * 1e-3),
                             "samples_per_s": c2.n_samples * f2 * b2 / (ms2 * 1e-3),
                             "alu_frac": roof2["frac"], "alu_frac_of_nominal": roof2["frac_of_nominal"],
+                            "sm_mhz": (r2["clocks"] or {}).get("sm_mhz"),
+                            "alu_frac_per_cycle": roof2["frac"] * float(r2["clocks"]["sm_max_mhz"]) / float(r2["clocks"]["sm_mhz"])
+                            if r2["clocks"] and r2["clocks"].get("sm_mhz") else None,
                             "hbm_frac": roof2["hbm_leg"]["frac"], "fp64_slots_per_sample": roof2["fp64_slots_counted"],
                             "construct_ms": r2["construct_ms"], "specialize_ms": float(i2["specialize_ms"]),
                             "specialize_from_disk_cache": bool(i2["specialize_cached"]),
